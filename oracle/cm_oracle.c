@@ -1,0 +1,930 @@
+/*
+ * cm_oracle.c -- CPU ORACLE for the GSPM hot path of CuPyMag (arXiv 2510.09812).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference leg may load this library.  It shares no code, header,
+ * table or helper with the CUDA library (paper_2510_09812_b200/csrc); neither includes
+ * the other.  It is written from the paper, plainly: loops over elements and rows in
+ * index order, no blocking, no fusion, no reordering, so it can be checked against the
+ * paper by eye.  "P:n" = /root/reference/PAPER.md line n.  "R#" = reading # listed in
+ * DESIGN.md (the points where the paper is silent or ambiguous).
+ *
+ * Compiled twice: -DORC_F32 gives the single-precision twin (R20: matrices, geometry and
+ * vectors stored in fp32; set-up quantities computed in fp64 then rounded; every
+ * reduction accumulated in fp64).  OpenMP pragmas sit on independent row loops only.
+ *
+ * Pins (tests/test_oracle_pins.py): element volumes sum to the box volume; grad(phi)
+ * duality; K symmetric, zero row sums, patch test, u^T K u = |a|^2 vol for linear u;
+ * M row sums = lumped mass, u^T M u = int (a.x+b)^2; K^mech rigid-body null space and
+ * u^T K u = vol * symG:C:symG; volume average of a linear field = value at centroid;
+ * uniform m => b^ms = 0 and h_d = -N_d mbar (sphere: -mbar/3); gradient/stress recovery
+ * exact on linear fields; fields h_an, h_d, h_me = -(1/mass) dEnergy/dm by central finite
+ * differences; closed-form energies of uniform states; CG against dense solves; the GSPM
+ * step against the analytic macrospin solution (first order in dtau), fixed points,
+ * |m| = 1 and energy decay.  Unpinned: the choice between gspm_variant 0 and 1 (R1) and
+ * between the adjoint and literal magnetostatic RHS (R9) -- "parity unpinned" between
+ * readings; each reading is pinned by the invariants above.
+ */
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef ORC_F32
+typedef float real;
+#else
+typedef double real;
+#endif
+
+typedef unsigned char uchar;
+
+#define ORC_OK 0
+#define ORC_E_BADARG (-1)
+#define ORC_E_DEGENERATE (-2)
+#define ORC_E_RANGE (-3)
+#define ORC_E_ALLOC (-4)
+#define ORC_E_BREAKDOWN (-6)
+#define ORC_W_MAXITER (-7)
+
+#define T_ANIS 1u
+#define T_ZEEMAN 2u
+#define T_DEMAG 4u
+#define T_FARFIELD 8u
+#define T_MAGEL 16u
+
+enum { MAT_K_MS = 0, MAT_K_GS1 = 1, MAT_K_GS2 = 2, MAT_MASS = 3, MAT_K_MECH = 4,
+       MAT_K_FREE = 5, MAT_K_M = 6, MAT_K_MECH_FREE = 7 };
+
+typedef struct {
+    double Ms, Aex, K1, lambda100, lambda111, alpha, gamma, length_scale;
+    double Nd[9];
+    int n_elastic;
+    const double *C_voigt; /* n_elastic x 36, Pa */
+} orc_material;
+
+typedef struct {
+    double dt;
+    double Hext[3];
+    unsigned terms;
+    int gspm_variant;
+    double cg_tol;
+    int cg_maxiter;
+    int cg_fixed_iters;
+} orc_step_params;
+
+typedef struct {
+    int it_ms, it_mech, it_gs[8];
+    double res_ms, res_mech, res_gs[8];
+    double mbar[3];
+    double mean_dm;
+    double energy;
+} orc_step_info;
+
+typedef struct {
+    long N, Ne, nnz;
+    double *x;      /* N x 3, nondimensional x/l_d (O-0) */
+    int *tet;       /* Ne x 4 */
+    uchar *mag;     /* Ne */
+    int *eid;       /* Ne */
+    real *V;        /* Ne          element volumes (|J|/6) */
+    real *G;        /* Ne x 4 x 3  grad phi_k of each element */
+    real *mL, *mLm; /* N lumped masses (all tets / magnetic tets) */
+    uchar *live;    /* N: touched by a magnetic tet */
+    int *n2e_ptr, *n2e; /* node -> (element*4 + local) */
+    int *rowptr, *col;
+    /* scalar matrices on the shared pattern */
+    real *K, *Kms, *Km, *Mm, *Kgs1, *Kgs2;
+    /* 3x3 block matrices [nnz][3][3] */
+    real *Kmech, *Kmech_free;
+    uchar *clamp; long pin;
+    double dt, Astar, Kstar, dtau, eps1, eps2, alpha, lam100, lam111, Ms, Nd[9];
+    int n_elastic; double *Cstar; /* n_elastic x 36, C/(mu0 Ms^2) */
+    double Vtot, Vmag;
+} oracle;
+
+static const double MU0 = 4.0e-7 * 3.14159265358979323846;
+
+/* ------------------------------------------------------------------------------------ */
+/* S0: reordering, relabelling, node->element lists, sparsity pattern (R21)              */
+/* ------------------------------------------------------------------------------------ */
+
+static int build_n2e(long N, long Ne, const int *tet, int **ptr_out, int **lst_out)
+{
+    int *ptr = (int *)calloc((size_t)N + 1, sizeof(int));
+    int *lst = (int *)malloc((size_t)Ne * 4 * sizeof(int));
+    if (!ptr || !lst) return ORC_E_ALLOC;
+    for (long e = 0; e < Ne; e++)
+        for (int k = 0; k < 4; k++) ptr[tet[4 * e + k] + 1]++;
+    for (long i = 0; i < N; i++) ptr[i + 1] += ptr[i];
+    int *fill = (int *)malloc((size_t)N * sizeof(int));
+    memcpy(fill, ptr, (size_t)N * sizeof(int));
+    for (long e = 0; e < Ne; e++) /* ascending e => each list is ascending in e */
+        for (int k = 0; k < 4; k++) lst[fill[tet[4 * e + k]]++] = (int)(4 * e + k);
+    free(fill);
+    *ptr_out = ptr; *lst_out = lst;
+    return ORC_OK;
+}
+
+static int cmp_int(const void *a, const void *b)
+{
+    int x = *(const int *)a, y = *(const int *)b;
+    return (x > y) - (x < y);
+}
+
+/* Row pattern of node i = { j : i and j share a tet } U { i }, columns ascending. */
+static int build_pattern(long N, const int *tet, const int *ptr, const int *lst,
+                         int **rowptr_out, int **col_out, long *nnz_out)
+{
+    int *rowptr = (int *)calloc((size_t)N + 1, sizeof(int));
+    int cap = 4096; int *tmp = (int *)malloc(cap * sizeof(int));
+    if (!rowptr || !tmp) return ORC_E_ALLOC;
+    for (int pass = 0; pass < 2; pass++) {
+        int *col = pass ? *col_out : NULL;
+        for (long i = 0; i < N; i++) {
+            int m = 0, cnt = ptr[i + 1] - ptr[i];
+            if (4 * cnt + 1 > cap) { cap = 8 * cnt + 1; tmp = (int *)realloc(tmp, cap * sizeof(int)); }
+            tmp[m++] = (int)i;
+            for (int s = ptr[i]; s < ptr[i + 1]; s++) {
+                int e = lst[s] >> 2;
+                for (int k = 0; k < 4; k++) tmp[m++] = tet[4 * e + k];
+            }
+            qsort(tmp, m, sizeof(int), cmp_int);
+            int u = 0;
+            for (int q = 0; q < m; q++) if (q == 0 || tmp[q] != tmp[q - 1]) tmp[u++] = tmp[q];
+            if (!pass) rowptr[i + 1] = u;
+            else memcpy(col + rowptr[i], tmp, u * sizeof(int));
+        }
+        if (!pass) {
+            for (long i = 0; i < N; i++) rowptr[i + 1] += rowptr[i];
+            *col_out = (int *)malloc((size_t)rowptr[N] * sizeof(int));
+            if (!*col_out) return ORC_E_ALLOC;
+        }
+    }
+    free(tmp);
+    *rowptr_out = rowptr; *nnz_out = rowptr[N];
+    return ORC_OK;
+}
+
+typedef struct { unsigned long long key; int idx; } keyidx;
+static int cmp_keyidx(const void *a, const void *b)
+{
+    const keyidx *x = (const keyidx *)a, *y = (const keyidx *)b;
+    if (x->key != y->key) return x->key < y->key ? -1 : 1;
+    return (x->idx > y->idx) - (x->idx < y->idx);
+}
+
+/* Morton order (R21): q_d = floor((x_d-min_d)/(max_d-min_d)*(2^21-1)) in fp64; 63-bit
+ * interleave with x in the least significant lane; stable sort by (code, user index). */
+static void order_morton(long N, const double *xyz, int *order)
+{
+    double lo[3], hi[3];
+    for (int d = 0; d < 3; d++) { lo[d] = xyz[d]; hi[d] = xyz[d]; }
+    for (long i = 0; i < N; i++)
+        for (int d = 0; d < 3; d++) {
+            if (xyz[3 * i + d] < lo[d]) lo[d] = xyz[3 * i + d];
+            if (xyz[3 * i + d] > hi[d]) hi[d] = xyz[3 * i + d];
+        }
+    keyidx *k = (keyidx *)malloc((size_t)N * sizeof(keyidx));
+    for (long i = 0; i < N; i++) {
+        unsigned long long code = 0, q[3];
+        for (int d = 0; d < 3; d++) {
+            double span = hi[d] - lo[d];
+            double t = span > 0 ? (xyz[3 * i + d] - lo[d]) / span * 2097151.0 : 0.0;
+            q[d] = (unsigned long long)floor(t);
+        }
+        for (int b = 0; b < 21; b++)
+            for (int d = 0; d < 3; d++) code |= ((q[d] >> b) & 1ull) << (3 * b + d);
+        k[i].key = code; k[i].idx = (int)i;
+    }
+    qsort(k, N, sizeof(keyidx), cmp_keyidx);
+    for (long i = 0; i < N; i++) order[i] = k[i].idx;
+    free(k);
+}
+
+/* Reverse Cuthill-McKee (R21): per component start at the unvisited node of minimum
+ * degree (lowest index on ties); BFS, appending the unvisited neighbours of each node by
+ * (degree, index) ascending; reverse the final order. */
+static void order_rcm(long N, const int *rowptr, const int *col, int *order)
+{
+    keyidx *bydeg = (keyidx *)malloc((size_t)N * sizeof(keyidx));
+    uchar *seen = (uchar *)calloc((size_t)N, 1);
+    int *cm = (int *)malloc((size_t)N * sizeof(int));
+    for (long i = 0; i < N; i++) { bydeg[i].key = (unsigned long long)(rowptr[i + 1] - rowptr[i] - 1); bydeg[i].idx = (int)i; }
+    qsort(bydeg, N, sizeof(keyidx), cmp_keyidx);
+    long head = 0, tail = 0, scan = 0;
+    int cap = 64; keyidx *nb = (keyidx *)malloc(cap * sizeof(keyidx));
+    while (tail < N) {
+        while (seen[bydeg[scan].idx]) scan++;
+        int s = bydeg[scan].idx;
+        seen[s] = 1; cm[tail++] = s;
+        while (head < tail) {
+            int v = cm[head++], m = 0;
+            if (rowptr[v + 1] - rowptr[v] > cap) { cap = 2 * (rowptr[v + 1] - rowptr[v]); nb = (keyidx *)realloc(nb, cap * sizeof(keyidx)); }
+            for (int q = rowptr[v]; q < rowptr[v + 1]; q++) {
+                int j = col[q];
+                if (j != v && !seen[j]) { nb[m].key = (unsigned long long)(rowptr[j + 1] - rowptr[j] - 1); nb[m].idx = j; m++; seen[j] = 1; }
+            }
+            qsort(nb, m, sizeof(keyidx), cmp_keyidx);
+            for (int q = 0; q < m; q++) cm[tail++] = nb[q].idx;
+        }
+    }
+    for (long i = 0; i < N; i++) order[i] = cm[N - 1 - i];
+    free(bydeg); free(seen); free(cm); free(nb);
+}
+
+/* Public: compute the locality permutation and the relabelled, sorted connectivity.
+ * method: 0 none, 1 Morton, 2 RCM.  order[new] = old node; iperm[old] = new node.
+ * Tets keep their local node order and are sorted by (min new node id, user tet index);
+ * tet_order[new_tet] = old tet. */
+int orc_reorder(const double *xyz, long N, const int *tets, long Ne, int method,
+                int *order, int *iperm, int *tets_new, int *tet_order)
+{
+    if (method == 0) for (long i = 0; i < N; i++) order[i] = (int)i;
+    else if (method == 1) order_morton(N, xyz, order);
+    else if (method == 2) {
+        int *ptr, *lst, *rowptr, *col; long nnz;
+        int rc = build_n2e(N, Ne, tets, &ptr, &lst); if (rc) return rc;
+        rc = build_pattern(N, tets, ptr, lst, &rowptr, &col, &nnz); if (rc) return rc;
+        order_rcm(N, rowptr, col, order);
+        free(ptr); free(lst); free(rowptr); free(col);
+    } else return ORC_E_BADARG;
+    for (long i = 0; i < N; i++) iperm[order[i]] = (int)i;
+    keyidx *k = (keyidx *)malloc((size_t)Ne * sizeof(keyidx));
+    for (long e = 0; e < Ne; e++) {
+        int mn = iperm[tets[4 * e]];
+        for (int q = 1; q < 4; q++) if (iperm[tets[4 * e + q]] < mn) mn = iperm[tets[4 * e + q]];
+        k[e].key = (unsigned long long)mn; k[e].idx = (int)e;
+    }
+    qsort(k, Ne, sizeof(keyidx), cmp_keyidx);
+    for (long e = 0; e < Ne; e++) {
+        tet_order[e] = k[e].idx;
+        for (int q = 0; q < 4; q++) tets_new[4 * e + q] = iperm[tets[4 * k[e].idx + q]];
+    }
+    free(k);
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* O-1 geometry, O-2 matrices                                                            */
+/* ------------------------------------------------------------------------------------ */
+
+/* B_i^T C B_j for Voigt order xx,yy,zz,yz,xz,xy with engineering shears (P:476 order). */
+static void strain_disp(const double g[3], double B[6][3])
+{
+    memset(B, 0, 18 * sizeof(double));
+    B[0][0] = g[0]; B[1][1] = g[1]; B[2][2] = g[2];
+    B[3][1] = g[2]; B[3][2] = g[1];
+    B[4][0] = g[2]; B[4][2] = g[0];
+    B[5][0] = g[1]; B[5][1] = g[0];
+}
+
+static long find_col(const oracle *o, long i, int j)
+{
+    for (long q = o->rowptr[i]; q < o->rowptr[i + 1]; q++) if (o->col[q] == j) return q;
+    return -1;
+}
+
+void orc_destroy(oracle *o);
+
+int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const uchar *magnetic,
+               const int *elastic_id, const orc_material *mat, double dt, const uchar *clamp_dof,
+               long pin_node, oracle **out)
+{
+    if (!xyz_m || !tets || !mat || !out || N <= 0 || Ne <= 0) return ORC_E_BADARG;
+    oracle *o = (oracle *)calloc(1, sizeof(oracle));
+    if (!o) return ORC_E_ALLOC;
+    o->N = N; o->Ne = Ne;
+    /* O-0 nondimensionalisation */
+    double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
+    o->Ms = mat->Ms; o->dt = dt;
+    o->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
+    o->Kstar = mat->K1 / mu0Ms2;
+    o->dtau = mat->gamma * mat->Ms * dt;
+    o->alpha = mat->alpha;
+    o->eps1 = o->Astar * o->dtau;              /* Step 1 */
+    o->eps2 = o->alpha * o->Astar * o->dtau;   /* Step 3 */
+    o->lam100 = mat->lambda100; o->lam111 = mat->lambda111;
+    memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
+    o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
+    o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
+    for (int q = 0; q < o->n_elastic * 36; q++) o->Cstar[q] = mat->C_voigt[q] / mu0Ms2;
+
+    o->x = (double *)malloc((size_t)N * 3 * sizeof(double));
+    o->tet = (int *)malloc((size_t)Ne * 4 * sizeof(int));
+    o->mag = (uchar *)malloc((size_t)Ne);
+    o->eid = (int *)calloc((size_t)Ne, sizeof(int));
+    o->V = (real *)malloc((size_t)Ne * sizeof(real));
+    o->G = (real *)malloc((size_t)Ne * 12 * sizeof(real));
+    o->mL = (real *)malloc((size_t)N * sizeof(real));
+    o->mLm = (real *)malloc((size_t)N * sizeof(real));
+    o->live = (uchar *)calloc((size_t)N, 1);
+    o->clamp = (uchar *)calloc((size_t)N * 3, 1);
+    if (!o->x || !o->tet || !o->mag || !o->eid || !o->V || !o->G || !o->mL || !o->mLm || !o->live || !o->clamp) { orc_destroy(o); return ORC_E_ALLOC; }
+    for (long i = 0; i < 3 * N; i++) o->x[i] = xyz_m[i] / ld;
+    memcpy(o->tet, tets, (size_t)Ne * 4 * sizeof(int));
+    for (long e = 0; e < Ne; e++) o->mag[e] = magnetic ? (magnetic[e] != 0) : 1;
+    if (elastic_id) memcpy(o->eid, elastic_id, (size_t)Ne * sizeof(int));
+    if (clamp_dof) for (long i = 0; i < 3 * N; i++) o->clamp[i] = clamp_dof[i] != 0;
+    o->pin = pin_node;
+    for (long e = 0; e < Ne; e++) {
+        for (int k = 0; k < 4; k++) if (tets[4 * e + k] < 0 || tets[4 * e + k] >= N) { orc_destroy(o); return ORC_E_RANGE; }
+        if (o->n_elastic && (o->eid[e] < 0 || o->eid[e] >= o->n_elastic)) { orc_destroy(o); return ORC_E_RANGE; }
+    }
+    if (pin_node < 0 || pin_node >= N) { orc_destroy(o); return ORC_E_BADARG; }
+
+    /* O-1: V_e = |det J|/6, grad phi_k = k-th row of J^-1 (k=1..3), grad phi_0 = -sum */
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++) {
+        if (o->x[3 * i + d] < lo[d]) lo[d] = o->x[3 * i + d];
+        if (o->x[3 * i + d] > hi[d]) hi[d] = o->x[3 * i + d];
+    }
+    double diag = sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
+    double Vmin = 1e-14 * diag * diag * diag;
+    double *mL = (double *)calloc((size_t)N, sizeof(double)), *mLm = (double *)calloc((size_t)N, sizeof(double));
+    o->Vtot = 0; o->Vmag = 0;
+    for (long e = 0; e < Ne; e++) {
+        const double *x0 = o->x + 3 * tets[4 * e], *x1 = o->x + 3 * tets[4 * e + 1],
+                     *x2 = o->x + 3 * tets[4 * e + 2], *x3 = o->x + 3 * tets[4 * e + 3];
+        double a[3], b[3], c[3];
+        for (int d = 0; d < 3; d++) { a[d] = x1[d] - x0[d]; b[d] = x2[d] - x0[d]; c[d] = x3[d] - x0[d]; }
+        double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+        double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+        double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+        double det = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+        double V = fabs(det) / 6.0;
+        if (!(V > Vmin)) { free(mL); free(mLm); orc_destroy(o); return ORC_E_DEGENERATE; }
+        double g[4][3];
+        for (int d = 0; d < 3; d++) {
+            g[1][d] = bc[d] / det; g[2][d] = ca[d] / det; g[3][d] = ab[d] / det;
+            g[0][d] = -(g[1][d] + g[2][d] + g[3][d]);
+        }
+        o->V[e] = (real)V;
+        for (int k = 0; k < 4; k++) for (int d = 0; d < 3; d++) o->G[12 * e + 3 * k + d] = (real)g[k][d];
+        o->Vtot += V;
+        if (o->mag[e]) o->Vmag += V;
+        for (int k = 0; k < 4; k++) {
+            mL[tets[4 * e + k]] += V / 4.0;            /* int_e phi_i = V_e/4 */
+            if (o->mag[e]) { mLm[tets[4 * e + k]] += V / 4.0; o->live[tets[4 * e + k]] = 1; }
+        }
+    }
+    for (long i = 0; i < N; i++) { o->mL[i] = (real)mL[i]; o->mLm[i] = (real)mLm[i]; }
+    free(mL); free(mLm);
+
+    int rc = build_n2e(N, Ne, o->tet, &o->n2e_ptr, &o->n2e); if (rc) { orc_destroy(o); return rc; }
+    rc = build_pattern(N, o->tet, o->n2e_ptr, o->n2e, &o->rowptr, &o->col, &o->nnz); if (rc) { orc_destroy(o); return rc; }
+
+    /* O-2 (Eq. 12): accumulate in fp64 in element order, round once (R20). */
+    long nnz = o->nnz;
+    double *K = (double *)calloc((size_t)nnz, sizeof(double)), *Km = (double *)calloc((size_t)nnz, sizeof(double)),
+           *Mm = (double *)calloc((size_t)nnz, sizeof(double));
+    double *Kme = o->n_elastic ? (double *)calloc((size_t)nnz * 9, sizeof(double)) : NULL;
+    if (!K || !Km || !Mm || (o->n_elastic && !Kme)) { orc_destroy(o); return ORC_E_ALLOC; }
+    for (long e = 0; e < Ne; e++) {
+        /* recompute the fp64 geometry of this element (not the rounded copy) */
+        const int *t = tets + 4 * e;
+        const double *x0 = o->x + 3 * t[0], *x1 = o->x + 3 * t[1], *x2 = o->x + 3 * t[2], *x3 = o->x + 3 * t[3];
+        double a[3], b[3], c[3];
+        for (int d = 0; d < 3; d++) { a[d] = x1[d] - x0[d]; b[d] = x2[d] - x0[d]; c[d] = x3[d] - x0[d]; }
+        double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+        double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+        double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+        double det = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+        double V = fabs(det) / 6.0, g[4][3];
+        for (int d = 0; d < 3; d++) {
+            g[1][d] = bc[d] / det; g[2][d] = ca[d] / det; g[3][d] = ab[d] / det;
+            g[0][d] = -(g[1][d] + g[2][d] + g[3][d]);
+        }
+        const double *C = o->n_elastic ? o->Cstar + 36 * o->eid[e] : NULL;
+        for (int i = 0; i < 4; i++) for (int j = 0; j < 4; j++) {
+            long q = find_col(o, t[i], t[j]);
+            double kij = V * (g[i][0] * g[j][0] + g[i][1] * g[j][1] + g[i][2] * g[j][2]); /* int grad.grad */
+            double mij = V * (i == j ? 2.0 : 1.0) / 20.0;                                 /* int phi phi  */
+            K[q] += kij;
+            if (o->mag[e]) { Km[q] += kij; Mm[q] += mij; }
+            if (C) {
+                double Bi[6][3], Bj[6][3], CB[6][3];
+                strain_disp(g[i], Bi); strain_disp(g[j], Bj);
+                for (int r = 0; r < 6; r++) for (int s = 0; s < 3; s++) {
+                    double acc = 0; for (int w = 0; w < 6; w++) acc += C[6 * r + w] * Bj[w][s];
+                    CB[r][s] = acc;
+                }
+                for (int r = 0; r < 3; r++) for (int s = 0; s < 3; s++) {
+                    double acc = 0; for (int w = 0; w < 6; w++) acc += Bi[w][r] * CB[w][s];
+                    Kme[9 * q + 3 * r + s] += V * acc;
+                }
+            }
+        }
+    }
+    o->K = (real *)malloc((size_t)nnz * sizeof(real)); o->Kms = (real *)malloc((size_t)nnz * sizeof(real));
+    o->Km = (real *)malloc((size_t)nnz * sizeof(real)); o->Mm = (real *)malloc((size_t)nnz * sizeof(real));
+    o->Kgs1 = (real *)malloc((size_t)nnz * sizeof(real)); o->Kgs2 = (real *)malloc((size_t)nnz * sizeof(real));
+    if (Kme) { o->Kmech = (real *)malloc((size_t)nnz * 9 * sizeof(real)); o->Kmech_free = (real *)malloc((size_t)nnz * 9 * sizeof(real)); }
+    for (long i = 0; i < N; i++)
+        for (long q = o->rowptr[i]; q < o->rowptr[i + 1]; q++) {
+            long j = o->col[q];
+            o->K[q] = (real)K[q]; o->Km[q] = (real)Km[q]; o->Mm[q] = (real)Mm[q];
+            /* constraints as the symmetric projection P A P + (I-P)  (R11) */
+            double kms = K[q];
+            if (i == o->pin || j == o->pin) kms = (i == j) ? 1.0 : 0.0;
+            o->Kms[q] = (real)kms;
+            /* K^GS(eps) = M_m + eps K_m, identity rows on dead nodes (R12) */
+            double dead = (i == j && !o->live[i]) ? 1.0 : 0.0;
+            o->Kgs1[q] = (real)(Mm[q] + o->eps1 * Km[q] + dead);
+            o->Kgs2[q] = (real)(Mm[q] + o->eps2 * Km[q] + dead);
+            if (Kme) for (int r = 0; r < 3; r++) for (int s = 0; s < 3; s++) {
+                double v = Kme[9 * q + 3 * r + s];
+                o->Kmech_free[9 * q + 3 * r + s] = (real)v;
+                if (o->clamp[3 * i + r] || o->clamp[3 * j + s]) v = (i == j && r == s) ? 1.0 : 0.0;
+                o->Kmech[9 * q + 3 * r + s] = (real)v;
+            }
+        }
+    free(K); free(Km); free(Mm); free(Kme);
+    *out = o;
+    return ORC_OK;
+}
+
+void orc_destroy(oracle *o)
+{
+    if (!o) return;
+    free(o->x); free(o->tet); free(o->mag); free(o->eid); free(o->V); free(o->G); free(o->mL); free(o->mLm);
+    free(o->live); free(o->n2e_ptr); free(o->n2e); free(o->rowptr); free(o->col); free(o->K); free(o->Kms);
+    free(o->Km); free(o->Mm); free(o->Kgs1); free(o->Kgs2); free(o->Kmech); free(o->Kmech_free); free(o->clamp);
+    free(o->Cstar); free(o);
+}
+
+/* accessors: sizes, then copies */
+long orc_nnz(const oracle *o) { return o->nnz; }
+double orc_scalar(const oracle *o, int what)
+{
+    switch (what) {
+    case 0: return o->Vtot; case 1: return o->Vmag; case 2: return o->Astar; case 3: return o->Kstar;
+    case 4: return o->dtau; case 5: return o->eps1; case 6: return o->eps2;
+    } return NAN;
+}
+/* what: 0 rowptr(int N+1) 1 col(int nnz) 2 n2e_ptr(int N+1) 3 n2e(int 4Ne) 4 V(real Ne) 5 G(real 12Ne)
+ *       6 mL(real N) 7 mLm(real N) 8 live(uchar N) */
+int orc_get(const oracle *o, int what, void *dst)
+{
+    switch (what) {
+    case 0: memcpy(dst, o->rowptr, (size_t)(o->N + 1) * sizeof(int)); break;
+    case 1: memcpy(dst, o->col, (size_t)o->nnz * sizeof(int)); break;
+    case 2: memcpy(dst, o->n2e_ptr, (size_t)(o->N + 1) * sizeof(int)); break;
+    case 3: memcpy(dst, o->n2e, (size_t)o->Ne * 4 * sizeof(int)); break;
+    case 4: memcpy(dst, o->V, (size_t)o->Ne * sizeof(real)); break;
+    case 5: memcpy(dst, o->G, (size_t)o->Ne * 12 * sizeof(real)); break;
+    case 6: memcpy(dst, o->mL, (size_t)o->N * sizeof(real)); break;
+    case 7: memcpy(dst, o->mLm, (size_t)o->N * sizeof(real)); break;
+    case 8: memcpy(dst, o->live, (size_t)o->N); break;
+    default: return ORC_E_BADARG;
+    }
+    return ORC_OK;
+}
+
+static const real *mat_values(const oracle *o, int id, int *bs)
+{
+    *bs = 1;
+    switch (id) {
+    case MAT_K_MS: return o->Kms; case MAT_K_GS1: return o->Kgs1; case MAT_K_GS2: return o->Kgs2;
+    case MAT_MASS: return o->Mm; case MAT_K_FREE: return o->K; case MAT_K_M: return o->Km;
+    case MAT_K_MECH: *bs = 3; return o->Kmech; case MAT_K_MECH_FREE: *bs = 3; return o->Kmech_free;
+    } return NULL;
+}
+
+int orc_get_values(const oracle *o, int id, void *dst)
+{
+    int bs; const real *v = mat_values(o, id, &bs);
+    if (!v) return ORC_E_BADARG;
+    memcpy(dst, v, (size_t)o->nnz * bs * bs * sizeof(real));
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* SpMV and O-4 CG                                                                       */
+/* ------------------------------------------------------------------------------------ */
+
+/* y = A x.  Scalar matrices: x, y have `stride` interleaved components and component
+ * `comp` is used (stride 1 for plain vectors).  Block matrices: x, y are N x 3. */
+static void spmv(const oracle *o, int id, const real *x, real *y, int stride, int comp)
+{
+    int bs; const real *v = mat_values(o, id, &bs);
+    long N = o->N;
+    if (bs == 1) {
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < N; i++) {
+            real acc = 0;
+            for (long q = o->rowptr[i]; q < o->rowptr[i + 1]; q++) acc += v[q] * x[(long)o->col[q] * stride + comp];
+            y[i * stride + comp] = acc;
+        }
+    } else {
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < N; i++) {
+            real acc[3] = {0, 0, 0};
+            for (long q = o->rowptr[i]; q < o->rowptr[i + 1]; q++) {
+                const real *xb = x + 3 * (long)o->col[q], *a = v + 9 * q;
+                for (int r = 0; r < 3; r++) acc[r] += a[3 * r] * xb[0] + a[3 * r + 1] * xb[1] + a[3 * r + 2] * xb[2];
+            }
+            y[3 * i] = acc[0]; y[3 * i + 1] = acc[1]; y[3 * i + 2] = acc[2];
+        }
+    }
+}
+
+int orc_spmv(const oracle *o, int id, const void *x, void *y)
+{
+    int bs; if (!mat_values(o, id, &bs)) return ORC_E_BADARG;
+    spmv(o, id, (const real *)x, (real *)y, 1, 0);
+    return ORC_OK;
+}
+
+static double dot(long n, const real *a, const real *b, int stride, int comp)
+{
+    double s = 0;
+#pragma omp parallel for reduction(+ : s) schedule(static)
+    for (long i = 0; i < n; i++) s += (double)a[i * stride + comp] * (double)b[i * stride + comp];
+    return s;
+}
+
+/* Textbook unpreconditioned CG (O-4).  Stop when ||r|| < tol ||b||
+ * (recurrence residual), tested before each iteration; fixed >= 0 runs exactly `fixed`
+ * iterations.  Dots in fp64; alpha, beta formed in fp64 and cast to the vector type. */
+static int cg(const oracle *o, int id, const real *b, real *x, int stride, int comp, double tol, int maxiter,
+              int fixed, int *iters, double *relres)
+{
+    int bs; mat_values(o, id, &bs);
+    long N = o->N, n = (bs == 3) ? 3 * N : N;   /* entries visited through (stride, comp) */
+    if (bs == 3) { stride = 1; comp = 0; }
+    long len = (bs == 3) ? 3 * N : N * stride;
+    real *r = (real *)calloc((size_t)len, sizeof(real)), *p = (real *)calloc((size_t)len, sizeof(real)),
+         *Ap = (real *)calloc((size_t)len, sizeof(real));
+    int status = ORC_OK, k = 0;
+    double bb = dot(n, b, b, stride, comp);
+    if (bb == 0.0 && fixed < 0) {       /* ||b|| = 0 -> x = 0, 0 iterations */
+        for (long i = 0; i < n; i++) x[i * stride + comp] = 0;
+        *iters = 0; *relres = 0; free(r); free(p); free(Ap); return ORC_OK;
+    }
+    spmv(o, id, x, Ap, stride, comp);
+    for (long i = 0; i < n; i++) { r[i * stride + comp] = b[i * stride + comp] - Ap[i * stride + comp]; p[i * stride + comp] = r[i * stride + comp]; }
+    double rr = dot(n, r, r, stride, comp);
+    for (;;) {
+        if (rr == 0.0) break;
+        if (fixed >= 0) { if (k == fixed) break; }
+        else { if (rr < tol * tol * bb) break; if (k >= maxiter) { status = ORC_W_MAXITER; break; } }
+        spmv(o, id, p, Ap, stride, comp);
+        double pAp = dot(n, p, Ap, stride, comp);
+        if (!(pAp > 0.0)) { status = ORC_E_BREAKDOWN; break; }
+        real alpha = (real)(rr / pAp);
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; i++) {
+            x[i * stride + comp] += alpha * p[i * stride + comp];
+            r[i * stride + comp] -= alpha * Ap[i * stride + comp];
+        }
+        double rr_new = dot(n, r, r, stride, comp);
+        real beta = (real)(rr_new / rr);
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; i++) p[i * stride + comp] = r[i * stride + comp] + beta * p[i * stride + comp];
+        rr = rr_new; k++;
+    }
+    *iters = k; *relres = bb > 0 ? sqrt(rr / bb) : 0.0;
+    free(r); free(p); free(Ap);
+    return status;
+}
+
+int orc_cg(const oracle *o, int id, const void *b, void *x, double tol, int maxiter, int fixed, int *iters, double *relres)
+{
+    int bs; if (!mat_values(o, id, &bs)) return ORC_E_BADARG;
+    return cg(o, id, (const real *)b, (real *)x, 1, 0, tol, maxiter, fixed, iters, relres);
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* S2 volume average (Eq. 16-17).  For P1 tets the Gauss sum is exact:        */
+/* int_e g = V_e * mean of the 4 nodal values.                                           */
+/* ------------------------------------------------------------------------------------ */
+int orc_volume_average(const oracle *o, const void *g_, int ncomp, double *out)
+{
+    const real *g = (const real *)g_;
+    double den = 0; double num[16];
+    if (ncomp < 1 || ncomp > 16) return ORC_E_BADARG;
+    for (int c = 0; c < ncomp; c++) num[c] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        const int *t = o->tet + 4 * e;
+        for (int c = 0; c < ncomp; c++) {
+            double ge = ((double)g[(long)t[0] * ncomp + c] + (double)g[(long)t[1] * ncomp + c] +
+                         (double)g[(long)t[2] * ncomp + c] + (double)g[(long)t[3] * ncomp + c]) / 4.0;
+            num[c] += ge * (double)o->V[e];
+        }
+        den += (double)o->V[e];
+    }
+    for (int c = 0; c < ncomp; c++) out[c] = num[c] / den;
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* S3 magnetostatic RHS (Eq. 9, 13, 14; R9 adjoint form):                                */
+/* b_i = sum_{e contains i} V_e grad phi_i . (mean_e(m) - mbar); b[pin] = 0.             */
+/* ------------------------------------------------------------------------------------ */
+int orc_rhs_ms(const oracle *o, const void *m_, const double *mbar, void *b_)
+{
+    const real *m = (const real *)m_; real *b = (real *)b_;
+    for (long i = 0; i < o->N; i++) b[i] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        const int *t = o->tet + 4 * e; const real *G = o->G + 12 * e;
+        real mt[3];
+        for (int d = 0; d < 3; d++)
+            mt[d] = (m[3 * (long)t[0] + d] + m[3 * (long)t[1] + d] + m[3 * (long)t[2] + d] + m[3 * (long)t[3] + d]) / (real)4 - (real)mbar[d];
+        for (int k = 0; k < 4; k++)
+            b[t[k]] += o->V[e] * (G[3 * k] * mt[0] + G[3 * k + 1] * mt[1] + G[3 * k + 2] * mt[2]);
+    }
+    b[o->pin] = 0;
+    return ORC_OK;
+}
+
+/* S5 gradient recovery and demagnetising field (Eq. 4, 15; R8, R10):
+ * grad U_e = sum_k U_k grad phi_k;  <grad U> = sum_e V_e grad U_e / V;
+ * h_d,i = -sum_{e contains i} V_e grad U_e/(4 mL_i) [+ <grad U>] (DEMAG)  - N_d mbar (FARFIELD). */
+int orc_demag_field(const oracle *o, const void *U_, const double *mbar, unsigned terms, void *hd_, double *gradU_mean)
+{
+    const real *U = (const real *)U_; real *hd = (real *)hd_;
+    long N = o->N;
+    for (long i = 0; i < 3 * N; i++) hd[i] = 0;
+    double gm[3] = {0, 0, 0};
+    if (terms & T_DEMAG) {
+        double acc[3] = {0, 0, 0};
+        for (long e = 0; e < o->Ne; e++) {
+            const int *t = o->tet + 4 * e; const real *G = o->G + 12 * e;
+            real gU[3];
+            for (int d = 0; d < 3; d++) gU[d] = U[t[0]] * G[d] + U[t[1]] * G[3 + d] + U[t[2]] * G[6 + d] + U[t[3]] * G[9 + d];
+            for (int d = 0; d < 3; d++) acc[d] += (double)o->V[e] * (double)gU[d];
+            for (int k = 0; k < 4; k++) for (int d = 0; d < 3; d++) hd[3 * (long)t[k] + d] += o->V[e] * gU[d];
+        }
+        for (int d = 0; d < 3; d++) gm[d] = acc[d] / o->Vtot;
+        for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++)
+            hd[3 * i + d] = -hd[3 * i + d] / ((real)4 * o->mL[i]) + (real)gm[d];
+    }
+    if (terms & T_FARFIELD)
+        for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++)
+            hd[3 * i + d] -= (real)(o->Nd[3 * d] * mbar[0] + o->Nd[3 * d + 1] * mbar[1] + o->Nd[3 * d + 2] * mbar[2]);
+    if (gradU_mean) for (int d = 0; d < 3; d++) gradU_mean[d] = gm[d];
+    return ORC_OK;
+}
+
+/* E0(m), Table A.1, Voigt engineering vector (E11,E22,E33,2E23,2E13,2E12). */
+static void E0_voigt(const oracle *o, const real *m, real e0[6])
+{
+    real l1 = (real)o->lam100, l2 = (real)o->lam111, th = (real)1.5;
+    e0[0] = th * l1 * (m[0] * m[0] - (real)(1.0 / 3.0));
+    e0[1] = th * l1 * (m[1] * m[1] - (real)(1.0 / 3.0));
+    e0[2] = th * l1 * (m[2] * m[2] - (real)(1.0 / 3.0));
+    e0[3] = (real)2 * th * l2 * m[1] * m[2];
+    e0[4] = (real)2 * th * l2 * m[0] * m[2];
+    e0[5] = (real)2 * th * l2 * m[0] * m[1];
+}
+
+/* mean over the 4 nodes of a magnetic tet of E0(m_k) (R13) */
+static void mean_E0(const oracle *o, const real *m, const int *t, real e0[6])
+{
+    for (int q = 0; q < 6; q++) e0[q] = 0;
+    for (int k = 0; k < 4; k++) {
+        real ek[6]; E0_voigt(o, m + 3 * (long)t[k], ek);
+        for (int q = 0; q < 6; q++) e0[q] += ek[q];
+    }
+    for (int q = 0; q < 6; q++) e0[q] /= (real)4;
+}
+
+static void C_times(const oracle *o, long e, const real eps[6], real sig[6])
+{
+    const double *C = o->Cstar + 36 * o->eid[e];
+    for (int r = 0; r < 6; r++) {
+        real acc = 0;
+        for (int s = 0; s < 6; s++) acc += (real)C[6 * r + s] * eps[s];
+        sig[r] = acc;
+    }
+}
+
+/* S6 mechanical RHS (Eq. 10, 13, 14):
+ * b_(i,a) = sum_{e contains i, magnetic} V_e [C*_e : mean_e E0(m)]_ab d_b phi_i; clamped DOFs zeroed. */
+int orc_rhs_mech(const oracle *o, const void *m_, void *b_)
+{
+    const real *m = (const real *)m_; real *b = (real *)b_;
+    if (!o->n_elastic) return ORC_E_BADARG;
+    for (long i = 0; i < 3 * o->N; i++) b[i] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        if (!o->mag[e]) continue;
+        const int *t = o->tet + 4 * e; const real *G = o->G + 12 * e;
+        real e0[6], s[6];
+        mean_E0(o, m, t, e0);
+        C_times(o, e, e0, s);   /* Voigt stress xx,yy,zz,yz,xz,xy */
+        for (int k = 0; k < 4; k++) {
+            const real *g = G + 3 * k;
+            b[3 * (long)t[k] + 0] += o->V[e] * (s[0] * g[0] + s[5] * g[1] + s[4] * g[2]);
+            b[3 * (long)t[k] + 1] += o->V[e] * (s[5] * g[0] + s[1] * g[1] + s[3] * g[2]);
+            b[3 * (long)t[k] + 2] += o->V[e] * (s[4] * g[0] + s[3] * g[1] + s[2] * g[2]);
+        }
+    }
+    for (long i = 0; i < 3 * o->N; i++) if (o->clamp[i]) b[i] = 0;
+    return ORC_OK;
+}
+
+/* element strain E_e = sym(sum_k u_k (x) grad phi_k), Voigt engineering vector */
+static void elem_strain(const oracle *o, long e, const real *u, real eps[6])
+{
+    const int *t = o->tet + 4 * e; const real *G = o->G + 12 * e;
+    real H[3][3];  /* H[a][b] = d_b u_a */
+    for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) {
+        real acc = 0;
+        for (int k = 0; k < 4; k++) acc += u[3 * (long)t[k] + a] * G[3 * k + b];
+        H[a][b] = acc;
+    }
+    eps[0] = H[0][0]; eps[1] = H[1][1]; eps[2] = H[2][2];
+    eps[3] = H[1][2] + H[2][1]; eps[4] = H[0][2] + H[2][0]; eps[5] = H[0][1] + H[1][0];
+}
+
+/* S8 stress recovery (O-3 item 5): sigma_e = C*_e:(E_e(u) - mean_e E0(w)) on magnetic tets;
+ * sigma_hat_i = sum_{e contains i, magnetic} V_e sigma_e/(4 mLm_i).  Output N x 6 Voigt. */
+int orc_stress_recover(const oracle *o, const void *u_, const void *w_, void *sig_)
+{
+    const real *u = (const real *)u_, *w = (const real *)w_; real *sg = (real *)sig_;
+    if (!o->n_elastic) return ORC_E_BADARG;
+    for (long i = 0; i < 6 * o->N; i++) sg[i] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        if (!o->mag[e]) continue;
+        const int *t = o->tet + 4 * e;
+        real eps[6], e0[6], s[6];
+        elem_strain(o, e, u, eps);
+        mean_E0(o, w, t, e0);
+        for (int q = 0; q < 6; q++) eps[q] -= e0[q];
+        C_times(o, e, eps, s);
+        for (int k = 0; k < 4; k++) for (int q = 0; q < 6; q++) sg[6 * (long)t[k] + q] += o->V[e] * s[q];
+    }
+    for (long i = 0; i < o->N; i++)
+        for (int q = 0; q < 6; q++) sg[6 * i + q] = o->live[i] ? sg[6 * i + q] / ((real)4 * o->mLm[i]) : (real)0;
+    return ORC_OK;
+}
+
+/* O-3 item 5: h(w)_i = h_an + h_ext + h_d,i + h_me on live nodes, 0 on dead nodes.
+ * h_an,1 = -2K* w1 (w2^2 + w3^2) and cyclic (kappa_1 term of Eq. 1);
+ * h_me,1 = 3 [lam100 w1 s11 + lam111 (w2 s12 + w3 s13)] and cyclic (R14). */
+int orc_field(const oracle *o, const void *w_, const void *hd_, const void *sig_, const double *hext, unsigned terms, void *h_)
+{
+    const real *w = (const real *)w_, *hd = (const real *)hd_, *sg = (const real *)sig_; real *h = (real *)h_;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < o->N; i++) {
+        real hi[3] = {0, 0, 0};
+        if (o->live[i]) {
+            const real *m = w + 3 * i;
+            if (terms & T_ANIS) {
+                real k2 = (real)(2.0 * o->Kstar);
+                hi[0] -= k2 * m[0] * (m[1] * m[1] + m[2] * m[2]);
+                hi[1] -= k2 * m[1] * (m[2] * m[2] + m[0] * m[0]);
+                hi[2] -= k2 * m[2] * (m[0] * m[0] + m[1] * m[1]);
+            }
+            if (terms & T_ZEEMAN) for (int d = 0; d < 3; d++) hi[d] += (real)hext[d];
+            if (terms & (T_DEMAG | T_FARFIELD)) for (int d = 0; d < 3; d++) hi[d] += hd[3 * i + d];
+            if (terms & T_MAGEL) {
+                const real *s = sg + 6 * i; /* xx,yy,zz,yz,xz,xy */
+                real l1 = (real)o->lam100, l2 = (real)o->lam111;
+                hi[0] += (real)3 * (l1 * m[0] * s[0] + l2 * (m[1] * s[5] + m[2] * s[4]));
+                hi[1] += (real)3 * (l1 * m[1] * s[1] + l2 * (m[0] * s[5] + m[2] * s[3]));
+                hi[2] += (real)3 * (l1 * m[2] * s[2] + l2 * (m[0] * s[4] + m[1] * s[3]));
+            }
+        }
+        h[3 * i] = hi[0]; h[3 * i + 1] = hi[1]; h[3 * i + 2] = hi[2];
+    }
+    return ORC_OK;
+}
+
+/* discrete energy / (mu0 Ms^2 l_d^3)  (O-3 item 10); used by tests only */
+double orc_energy(const oracle *o, const void *m_, const void *U_, const void *u_, const double *hext, unsigned terms)
+{
+    const real *m = (const real *)m_, *U = (const real *)U_, *u = (const real *)u_;
+    long N = o->N;
+    double E = 0;
+    real *y = (real *)malloc((size_t)3 * N * sizeof(real));
+    for (int c = 0; c < 3; c++) { /* exchange 1/2 A* m_a^T K_m m_a */
+        spmv(o, MAT_K_M, m, y, 3, c);
+        E += 0.5 * o->Astar * dot(N, m, y, 3, c);
+    }
+    for (long i = 0; i < N; i++) {
+        double a = m[3 * i], b = m[3 * i + 1], c = m[3 * i + 2];
+        if (terms & T_ANIS) E += o->Kstar * (double)o->mLm[i] * (a * a * b * b + b * b * c * c + c * c * a * a);
+        if (terms & T_ZEEMAN) E -= (double)o->mLm[i] * (hext[0] * a + hext[1] * b + hext[2] * c);
+    }
+    double mbar[3]; orc_volume_average(o, m, 3, mbar);
+    if (terms & T_DEMAG) { spmv(o, MAT_K_FREE, U, y, 1, 0); E += 0.5 * dot(N, U, y, 1, 0); }
+    if (terms & T_FARFIELD)
+        for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) E += 0.5 * o->Vtot * mbar[a] * o->Nd[3 * a + b] * mbar[b];
+    if ((terms & T_MAGEL) && o->n_elastic)
+        for (long e = 0; e < o->Ne; e++) {
+            real eps[6], e0[6], s[6];
+            elem_strain(o, e, u, eps);
+            if (o->mag[e]) { mean_E0(o, m, o->tet + 4 * e, e0); for (int q = 0; q < 6; q++) eps[q] -= e0[q]; }
+            C_times(o, e, eps, s);
+            double w = 0; for (int q = 0; q < 6; q++) w += (double)eps[q] * (double)s[q];
+            E += 0.5 * (double)o->V[e] * w;
+        }
+    free(y);
+    return E;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* O-3: one GSPM step (Alg. B.1)                                              */
+/* ------------------------------------------------------------------------------------ */
+
+/* Helmholtz solve (M_m + eps K_m) g_a = M_m f_a, x0 = f_a (R15), for component a */
+static int helmholtz(const oracle *o, int id, const real *f, real *g, int a, const orc_step_params *p, int *it, double *res, real *b)
+{
+    spmv(o, MAT_MASS, f, b, 3, a);                                  /* b = M_m f (Eq. 14) */
+    for (long i = 0; i < o->N; i++) g[3 * i + a] = f[3 * i + a];
+    return cg(o, id, b, g, 3, a, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, it, res);
+}
+
+int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_, void *u_, orc_step_info *info)
+{
+    real *m = (real *)m_, *U = (real *)U_, *u = (real *)u_;
+    long N = o->N; unsigned terms = p->terms;
+    int worst = ORC_OK, rc;
+    if (p->dt != o->dt) return ORC_E_BADARG; /* K^GS was assembled for the dt given at create */
+    real *b = (real *)calloc((size_t)3 * N, sizeof(real)), *hd = (real *)calloc((size_t)3 * N, sizeof(real)),
+         *sg = (real *)calloc((size_t)6 * N, sizeof(real)), *hn = (real *)calloc((size_t)3 * N, sizeof(real)),
+         *f = (real *)calloc((size_t)3 * N, sizeof(real)), *gn = (real *)calloc((size_t)3 * N, sizeof(real)),
+         *gs = (real *)calloc((size_t)3 * N, sizeof(real)), *ms = (real *)calloc((size_t)3 * N, sizeof(real)),
+         *mss = (real *)calloc((size_t)3 * N, sizeof(real));
+    double hext[3] = {p->Hext[0] / o->Ms, p->Hext[1] / o->Ms, p->Hext[2] / o->Ms};
+    real dtau = (real)o->dtau, adtau = (real)(o->alpha * o->dtau);
+    memset(info, 0, sizeof(*info)); info->energy = NAN;
+
+    /* 1. mbar over all of Omega_c (Eq. 17) */
+    double mbar[3]; orc_volume_average(o, m, 3, mbar);
+    for (int d = 0; d < 3; d++) info->mbar[d] = mbar[d];
+    /* 2. magnetostatic solve, warm start (Eq. 5, 9) */
+    if (terms & T_DEMAG) {
+        orc_rhs_ms(o, m, mbar, b);
+        rc = cg(o, MAT_K_MS, b, U, 1, 0, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, &info->it_ms, &info->res_ms);
+        if (rc < worst) worst = rc;
+    }
+    /* 3. demagnetising field (Eq. 4) */
+    orc_demag_field(o, U, mbar, terms, hd, NULL);
+    /* 4. mechanical equilibrium (Eq. 6, 10), warm start */
+    if (terms & T_MAGEL) {
+        orc_rhs_mech(o, m, b);
+        rc = cg(o, MAT_K_MECH, b, u, 1, 0, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, &info->it_mech, &info->res_mech);
+        if (rc < worst) worst = rc;
+        orc_stress_recover(o, u, m, sg);
+    }
+    /* 5. h[m^n] */
+    orc_field(o, m, hd, sg, hext, terms, hn);
+    /* 6. Step 1: g^n */
+    for (long i = 0; i < 3 * N; i++) f[i] = m[i] + dtau * hn[i];
+    for (int a = 0; a < 3; a++) {
+        if (p->gspm_variant == 1 && a == 0) continue;  /* g_1^n unused in the Gauss-Seidel variant (R1) */
+        rc = helmholtz(o, MAT_K_GS1, f, gn, a, p, &info->it_gs[a], &info->res_gs[a], b);
+        if (rc < worst) worst = rc;
+    }
+    /* 7. Step 2 interleaved with the g* solves (g* uses m* and h[m^n]) */
+    for (long i = 0; i < N; i++) ms[3 * i] = m[3 * i] + (gn[3 * i + 1] * m[3 * i + 2] - gn[3 * i + 2] * m[3 * i + 1]);
+    if (p->gspm_variant == 0) {
+        for (long i = 0; i < N; i++) ms[3 * i + 1] = m[3 * i + 1] + (gn[3 * i + 2] * m[3 * i] - gn[3 * i] * m[3 * i + 2]);
+        for (long i = 0; i < N; i++) for (int a = 0; a < 2; a++) f[3 * i + a] = ms[3 * i + a] + dtau * hn[3 * i + a];
+        for (int a = 0; a < 2; a++) {
+            rc = helmholtz(o, MAT_K_GS1, f, gs, a, p, &info->it_gs[3 + a], &info->res_gs[3 + a], b);
+            if (rc < worst) worst = rc;
+        }
+    } else {
+        for (long i = 0; i < N; i++) f[3 * i] = ms[3 * i] + dtau * hn[3 * i];
+        rc = helmholtz(o, MAT_K_GS1, f, gs, 0, p, &info->it_gs[3], &info->res_gs[3], b); if (rc < worst) worst = rc;
+        for (long i = 0; i < N; i++) ms[3 * i + 1] = m[3 * i + 1] + (gn[3 * i + 2] * ms[3 * i] - gs[3 * i] * m[3 * i + 2]);
+        for (long i = 0; i < N; i++) f[3 * i + 1] = ms[3 * i + 1] + dtau * hn[3 * i + 1];
+        rc = helmholtz(o, MAT_K_GS1, f, gs, 1, p, &info->it_gs[4], &info->res_gs[4], b); if (rc < worst) worst = rc;
+    }
+    for (long i = 0; i < N; i++) ms[3 * i + 2] = m[3 * i + 2] + (gs[3 * i] * ms[3 * i + 1] - gs[3 * i + 1] * ms[3 * i]);
+    /* 8. Step 3: h* = h[m*] with U, u frozen (R3) */
+    if (terms & T_MAGEL) orc_stress_recover(o, u, ms, sg);
+    orc_field(o, ms, hd, sg, hext, terms, hn);
+    for (long i = 0; i < 3 * N; i++) f[i] = ms[i] + adtau * hn[i];
+    for (int a = 0; a < 3; a++) {
+        rc = helmholtz(o, MAT_K_GS2, f, mss, a, p, &info->it_gs[5 + a], &info->res_gs[5 + a], b);
+        if (rc < worst) worst = rc;
+    }
+    /* 9. Step 4 projection on live nodes; 10. mean |dm| over live nodes */
+    double sdm = 0; long nlive = 0;
+    for (long i = 0; i < N; i++) {
+        if (!o->live[i]) { m[3 * i] = m[3 * i + 1] = m[3 * i + 2] = 0; continue; }
+        real *v = mss + 3 * i;
+        real nrm = (real)sqrt((double)(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+        real nw[3] = {m[3 * i], m[3 * i + 1], m[3 * i + 2]};
+        if (nrm > 0) for (int d = 0; d < 3; d++) nw[d] = v[d] / nrm;
+        double d0 = (double)nw[0] - (double)m[3 * i], d1 = (double)nw[1] - (double)m[3 * i + 1], d2 = (double)nw[2] - (double)m[3 * i + 2];
+        sdm += sqrt(d0 * d0 + d1 * d1 + d2 * d2); nlive++;
+        m[3 * i] = nw[0]; m[3 * i + 1] = nw[1]; m[3 * i + 2] = nw[2];
+    }
+    info->mean_dm = nlive ? sdm / (double)nlive : 0.0;
+    free(b); free(hd); free(sg); free(hn); free(f); free(gn); free(gs); free(ms); free(mss);
+    return worst;
+}
+
+/* Helmholtz right-hand side b = M_m f for all three components (Eq. 14) */
+int orc_rhs_gs(const oracle *o, const void *f_, void *b_)
+{
+    for (int a = 0; a < 3; a++) spmv(o, MAT_MASS, (const real *)f_, (real *)b_, 3, a);
+    return ORC_OK;
+}
+
+int orc_sizeof_real(void) { return (int)sizeof(real); }
