@@ -1,0 +1,191 @@
+/*
+ * cupymag_b200.h -- C ABI of the B200-native GSPM hot path of CuPyMag (arXiv 2510.09812).
+ *
+ * One GPU, one process.  Plain pointers and sizes only; no torch / C++ types cross this
+ * boundary.  "P:n" cites /root/reference/PAPER.md line n; "R#" the readings in DESIGN.md.
+ *
+ * Conventions
+ *  - Every function returns CM_OK (0) or a negative cm_status; it never throws or exits.
+ *    cm_last_error() gives a thread-local message for the last failure.
+ *  - "host" pointers are read (or written) only during the call.  "dev" pointers are CUDA
+ *    device pointers owned by the CALLER (e.g. torch tensors' data_ptr()); `stream` is a
+ *    cudaStream_t passed as void* (NULL = default stream).
+ *  - The library owns cm_mesh / cm_system and every internal device buffer; nothing is
+ *    allocated inside cm_spmv / cm_cg_solve / cm_field_rhs / cm_gspm_step.
+ *  - All field vectors are in USER node order, interleaved [node][component], of the
+ *    system's dtype (double for CM_F64, float for CM_F32).  The locality reordering is
+ *    internal; cm_mesh_get exposes it for bit-exact structure parity.
+ *  - Quantities are nondimensional as in P:131: lengths x/l_d, fields H/m_s,
+ *    potential U/(m_s l_d), displacement u/l_d, stiffness C/(mu0 m_s^2), time gamma m_s t.
+ *  - Calls are asynchronous on `stream` except those that return host scalars
+ *    (cm_cg_solve, cm_volume_average, cm_gspm_step with info != NULL, the *_host calls,
+ *    the getters), which synchronise that stream before returning.
+ *  - There is no CPU fallback: without a CUDA device every compute call fails with CM_E_CUDA.
+ */
+#ifndef CUPYMAG_B200_H
+#define CUPYMAG_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cm_mesh cm_mesh;     /* opaque: reordered connectivity, node->element lists, CSR pattern */
+typedef struct cm_system cm_system; /* opaque: geometry, assembled matrices, masks, work vectors (one dtype) */
+
+typedef enum { CM_F64 = 0, CM_F32 = 1 } cm_dtype;
+typedef enum { CM_REORDER_NONE = 0, CM_REORDER_MORTON = 1, CM_REORDER_RCM = 2 } cm_reorder;
+
+/* Matrices of Eq. 12 on the shared sparsity pattern; constraints applied as the symmetric
+ * projection P A P + (I - P).  K_MS: all tets, one pinned node.  K_GS1/2 = M_m + eps K_m over
+ * magnetic tets with eps1 = A* dtau (Alg. B.1 Step 1), eps2 = alpha A* dtau (Step 3),
+ * identity rows on non-magnetic ("dead") nodes.  MASS = M_m = F^GS of Eq. 13.
+ * K_MECH: 3x3 blocks, clamped DOFs. */
+typedef enum { CM_MAT_K_MS = 0, CM_MAT_K_GS1 = 1, CM_MAT_K_GS2 = 2, CM_MAT_MASS = 3, CM_MAT_K_MECH = 4 } cm_matrix_id;
+
+/* Outputs of cm_field_rhs (Eq. 14; Eq. 15). */
+typedef enum {
+    CM_RHS_MS = 0,    /* b (N):    sum_e V_e grad phi_i . (mean_e m - mbar), 0 at the pin (R9)              */
+    CM_RHS_MECH = 1,  /* b (N x 3): sum_{e magnetic} V_e [C*_e : mean_e E0(m)] grad phi_i, 0 at clamped DOFs  */
+    CM_RHS_GS = 2,    /* b (N x 3): M_m (m + coeff * h(m; U, u))                                              */
+    CM_OUT_HD = 3,    /* h_d (N x 3): -recovered grad U + <grad U> - N_d mbar (Eq. 4; R8, R10)         */
+    CM_OUT_SIGMA = 4, /* sigma_hat (N x 6, Voigt xx,yy,zz,yz,xz,xy): recovered C*:(E(u) - E0(m))             */
+    CM_OUT_FIELD = 5  /* h(m) (N x 3): anisotropy + Zeeman + demag + magnetoelastic (no exchange)     */
+} cm_rhs_id;
+
+enum { CM_TERM_ANIS = 1, CM_TERM_ZEEMAN = 2, CM_TERM_DEMAG = 4, CM_TERM_FARFIELD = 8, CM_TERM_MAGEL = 16 };
+
+typedef enum {
+    CM_OK = 0,
+    CM_E_BADARG = -1,
+    CM_E_DEGENERATE_TET = -2, /* V_e <= 1e-14 * (bounding-box diagonal)^3 */
+    CM_E_INDEX_RANGE = -3,
+    CM_E_ALLOC = -4,
+    CM_E_CUDA = -5,
+    CM_E_CG_BREAKDOWN = -6,   /* p^T A p <= 0 */
+    CM_E_CG_MAXITER = -7      /* warning: the iterate is still written */
+} cm_status;
+
+/* what-codes of cm_mesh_get (all int32 arrays except COUNTS) */
+enum {
+    CM_GET_COUNTS = 0,    /* long[3]: n_nodes, n_tets, nnz                                   */
+    CM_GET_ORDER = 1,     /* order[new] = user node                                          */
+    CM_GET_IPERM = 2,     /* iperm[user] = new node                                          */
+    CM_GET_TETS = 3,      /* n_tets x 4, relabelled, sorted by (min new node id, user tet)   */
+    CM_GET_TET_ORDER = 4, /* tet_order[new] = user tet                                       */
+    CM_GET_ROWPTR = 5,    /* n_nodes + 1                                                     */
+    CM_GET_COLIDX = 6,    /* nnz, ascending in each row, diagonal present                    */
+    CM_GET_N2E_PTR = 7,   /* n_nodes + 1                                                     */
+    CM_GET_N2E = 8        /* 4 n_tets entries element*4 + local index, ascending per node    */
+};
+
+/* Material constants of Eq. 1 and Appendix A; SI units. */
+typedef struct {
+    double Ms;           /* saturation magnetisation m_s, A/m */
+    double Aex;          /* exchange coefficient A, J/m */
+    double K1;           /* cubic anisotropy kappa_1, J/m^3 */
+    double lambda100, lambda111; /* magnetostriction constants (E0(m)) */
+    double alpha;        /* damping constant (Eq. 7) */
+    double gamma;        /* gyromagnetic ratio in m/(A s): tau = gamma m_s t (R4) */
+    double length_scale; /* l_d, metres */
+    double Nd[9];        /* demagnetisation tensor of the ellipsoid, row-major (Eq. 4) */
+    int n_elastic;       /* number of elastic materials; 0 = no mechanics */
+    const double *C_voigt; /* host, n_elastic x 36 row-major, Pa; Voigt order xx,yy,zz,yz,xz,xy, engineering shears */
+} cm_material;
+
+typedef struct {
+    double dt;            /* s; must equal the dt given to cm_assemble_csr */
+    double Hext[3];       /* A/m */
+    unsigned terms;       /* CM_TERM_* bitmask; exchange is always on */
+    int gspm_variant;     /* 0: Alg. B.1 as printed; 1: fully Gauss-Seidel second component (R1) */
+    double cg_tol;        /* stop when ||r||_2 < cg_tol ||b||_2 */
+    int cg_maxiter;
+    int cg_fixed_iters;   /* >= 0: run exactly this many iterations in every solve; < 0: off */
+} cm_step_params;
+
+/* it_gs / res_gs slots: 0-2 g^n components, 3-4 g*_1, g*_2, 5-7 m** components. */
+typedef struct {
+    int it_ms, it_mech, it_gs[8];
+    double res_ms, res_mech, res_gs[8];
+    double mbar[3];       /* volume average of m^n (Eq. 17) */
+    double mean_dm;       /* mean over magnetic nodes of ||m^{n+1}_i - m^n_i||_2 */
+    double energy;        /* NaN (not computed on the device) */
+} cm_step_info;
+
+/* Kernel-class timers (CUDA events on the caller's stream) and launch counters. */
+enum { CM_PROF_CG_MS = 0, CM_PROF_CG_MECH = 1, CM_PROF_CG_GS = 2, CM_PROF_SPMV = 3, CM_PROF_ELEMENT = 4,
+       CM_PROF_POINTWISE = 5, CM_PROF_NCLASS = 6 };
+typedef struct {
+    double ms[CM_PROF_NCLASS];        /* accumulated device time per class, milliseconds */
+    long launches[CM_PROF_NCLASS];    /* kernel launches per class */
+    long cg_iters[CM_PROF_NCLASS];    /* CG iterations summed over right-hand sides (CG classes only) */
+    long cg_matrix_passes[CM_PROF_NCLASS]; /* SpMV passes over the matrix inside CG (a 3-RHS solve reads it once per iteration) */
+} cm_profile;
+
+/* S0: validate, reorder (R21), relabel, node->element lists, CSR pattern.
+ * xyz: host, n_nodes x 3, metres.  tets: host, n_tets x 4, 0-based user node ids.
+ * magnetic: host, n_tets, 1 = ferromagnet (NULL = all magnetic).  elastic_id: host, n_tets, index
+ * into cm_material.C_voigt (NULL = all 0).  Errors: BADARG, INDEX_RANGE, DEGENERATE_TET, ALLOC, CUDA. */
+int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
+                   const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out);
+int cm_mesh_destroy(cm_mesh *mesh);
+/* Copies structure arrays to host_out (capacity in elements); returns BADARG if capacity is too small. */
+int cm_mesh_get(const cm_mesh *mesh, int what, void *host_out, long capacity);
+
+/* S1: geometry (V_e, grad phi SoA, lumped masses) and matrix values on the device (Eq. 12), for one
+ * dtype and one dt (which fixes eps1, eps2).  clamp_dof: host, 3 n_nodes flags in user order or NULL.
+ * pin_node: user index of the pinned node of K^ms.  The mesh must outlive the system. */
+int cm_assemble_csr(cm_mesh *mesh, const cm_material *material, cm_dtype dtype, double dt,
+                    const unsigned char *clamp_dof, long pin_node, void *stream, cm_system **out);
+int cm_system_destroy(cm_system *sys);
+/* Matrix values in LIBRARY node order, plain CSR (nnz) or block-CSR (nnz x 3 x 3 row-major), system dtype. */
+int cm_system_get_values(const cm_system *sys, cm_matrix_id id, void *host_out, long capacity);
+/* Geometry in library order: what = 0 V_e (n_tets), 1 grad phi (n_tets x 4 x 3), 2 mL (n_nodes), 3 mLm (n_nodes);
+ * system dtype. */
+int cm_system_get_geometry(const cm_system *sys, int what, void *host_out, long capacity);
+
+/* y = A x.  x_dev, y_dev: N (scalar matrices) or N x 3 (K_MECH), user order. */
+int cm_spmv(cm_system *sys, cm_matrix_id id, const void *x_dev, void *y_dev, void *stream);
+/* Mass product for three interleaved components: y (N x 3) = M_m x (N x 3)  (b^GS of Eq. 14). */
+int cm_spmv3(cm_system *sys, cm_matrix_id id, const void *x_dev, void *y_dev, void *stream);
+
+/* Unpreconditioned CG (O-4): x_dev holds x0 on entry and x on exit.  Stops when the recurrence
+ * residual satisfies ||r|| < tol ||b|| (tested before each iteration), after maxiter iterations
+ * (CM_E_CG_MAXITER), or after exactly fixed_iters iterations when fixed_iters >= 0.  ||b|| = 0 gives x = 0
+ * and 0 iterations.  One persistent cooperative kernel; the stopping test runs on the device. */
+int cm_cg_solve(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter,
+                int fixed_iters, int *iters_out, double *relres_out, void *stream);
+/* Three independent CG solves with one scalar matrix (b, x: N x 3 interleaved), the matrix read once per
+ * iteration; iters_out / relres_out have 3 entries. */
+int cm_cg_solve3(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter,
+                 int fixed_iters, int *iters_out, double *relres_out, void *stream);
+
+/* Element-wise gather / compute / deterministic gather-scatter assembly (see cm_rhs_id).  m_dev: N x 3;
+ * U_dev: N (may be NULL when DEMAG is off); u_dev: N x 3 (may be NULL when MAGEL is off); coeff: dtau or
+ * alpha dtau for CM_RHS_GS.  b_dev: output of the size listed at cm_rhs_id. */
+int cm_field_rhs(cm_system *sys, cm_rhs_id id, const void *m_dev, const void *U_dev, const void *u_dev,
+                 const cm_step_params *params, double coeff, void *b_dev, void *stream);
+
+/* Volume average (Eq. 16-17) of an ncomp-component nodal field (user order): out_host[c]. */
+int cm_volume_average(const cm_mesh *mesh, cm_dtype dtype, const void *g_dev, int ncomp, double *out_host,
+                      void *stream);
+
+/* One Gauss-Seidel projection step (Alg. B.1; SURVEY O-3).  m_dev (N x 3), U_dev (N), u_dev
+ * (N x 3) are updated in place (U, u are the warm starts of the magnetostatic / mechanical CG).
+ * info may be NULL (then the call does not synchronise).  Returns the worst CG status. */
+int cm_gspm_step(cm_system *sys, const cm_step_params *params, void *m_dev, void *U_dev, void *u_dev,
+                 cm_step_info *info, void *stream);
+/* Same with HOST buffers: copies m, U, u to the device, steps, copies them back (end-to-end path). */
+int cm_gspm_step_host(cm_system *sys, const cm_step_params *params, void *m_host, void *U_host, void *u_host,
+                      cm_step_info *info, void *stream);
+
+int cm_profile_enable(cm_system *sys, int on);
+int cm_profile_get(cm_system *sys, cm_profile *out); /* synchronises outstanding timers */
+int cm_profile_reset(cm_system *sys);
+
+const char *cm_last_error(void);
+const char *cm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUPYMAG_B200_H */

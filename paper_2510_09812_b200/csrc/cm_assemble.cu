@@ -1,0 +1,339 @@
+// S1: geometry (O-1) and matrix values (O-2; Eq. 12) on the device.
+// All set-up arithmetic is fp64 and rounded once to the system dtype (R20).  Matrix entries
+// are accumulated by one thread per row over the row's incident elements in ascending element order
+// (deterministic; no atomics), each element's 4x4 local matrix being recomputed from the coordinates.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "cm_internal.h"
+
+int build_tiling(const std::vector<int> &rowptr, long N, int tile, Tiling *out, cudaStream_t st);
+
+static const double MU0 = 4.0e-7 * 3.14159265358979323846;
+
+struct TetGeom {
+    double V;
+    double g[4][3];
+};
+
+__device__ __forceinline__ void tet_geometry(const double *__restrict__ xyz, const int *t, double ld, TetGeom &G)
+{
+    double x[4][3];
+#pragma unroll
+    for (int k = 0; k < 4; k++)
+#pragma unroll
+        for (int d = 0; d < 3; d++) x[k][d] = xyz[3 * (long)t[k] + d] / ld;
+    double a[3], b[3], c[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) { a[d] = x[1][d] - x[0][d]; b[d] = x[2][d] - x[0][d]; c[d] = x[3][d] - x[0][d]; }
+    double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+    double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+    double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+    double det = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+    G.V = fabs(det) / 6.0;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        G.g[1][d] = bc[d] / det; G.g[2][d] = ca[d] / det; G.g[3][d] = ab[d] / det;
+        G.g[0][d] = -(G.g[1][d] + G.g[2][d] + G.g[3][d]);
+    }
+}
+
+// one thread per element: V_e, grad phi SoA (rounded to T), fp64 volume copy for the lumped masses
+template <typename T>
+__global__ void geom_kernel(long Ne, const int *__restrict__ tets, const double *__restrict__ xyz, double ld, T *V, T *G,
+                            double *Vd)
+{
+    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= Ne) return;
+    int t[4];
+    *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(tets)[e];
+    TetGeom g;
+    tet_geometry(xyz, t, ld, g);
+    V[e] = (T)g.V;
+    Vd[e] = g.V;
+#pragma unroll
+    for (int k = 0; k < 4; k++)
+#pragma unroll
+        for (int d = 0; d < 3; d++) G[(long)(3 * k + d) * Ne + e] = (T)g.g[k][d];
+}
+
+// one thread per node: lumped masses over all / magnetic incident tets, live flag
+template <typename T>
+__global__ void lump_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const double *__restrict__ Vd,
+                            const uchar *__restrict__ mag, T *mL, T *mLm, uchar *live)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double a = 0, am = 0;
+    bool lv = false;
+    for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
+        int e = n2e[s] >> 2;
+        double v = Vd[e] / 4.0;
+        a += v;
+        if (mag[e]) { am += v; lv = true; }
+    }
+    mL[i] = (T)a; mLm[i] = (T)am; live[i] = lv;
+}
+
+// deterministic sum of Vd (all, magnetic): one block
+__global__ void volume_sum_kernel(long Ne, const double *__restrict__ Vd, const uchar *__restrict__ mag, double *out)
+{
+    __shared__ double sa[1024], sm[1024];
+    double a = 0, m = 0;
+    for (long e = threadIdx.x; e < Ne; e += blockDim.x) { a += Vd[e]; if (mag[e]) m += Vd[e]; }
+    sa[threadIdx.x] = a; sm[threadIdx.x] = m;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) { sa[threadIdx.x] += sa[threadIdx.x + o]; sm[threadIdx.x] += sm[threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[0] = sa[0]; out[1] = sm[0]; }
+}
+
+__device__ __forceinline__ void strain_disp(const double g[3], double B[6][3])
+{
+#pragma unroll
+    for (int r = 0; r < 6; r++)
+#pragma unroll
+        for (int s = 0; s < 3; s++) B[r][s] = 0;
+    B[0][0] = g[0]; B[1][1] = g[1]; B[2][2] = g[2];
+    B[3][1] = g[2]; B[3][2] = g[1];
+    B[4][0] = g[2]; B[4][2] = g[0];
+    B[5][0] = g[1]; B[5][1] = g[0];
+}
+
+// one thread per row i: accumulate scalar entries K (all tets), K_m, M_m (magnetic tets) and, if
+// Cstar != NULL, the 3x3 blocks of K^mech into fp64 scratch arrays laid out on the CSR pattern.
+__global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const double *__restrict__ xyz, double ld,
+                                     const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const uchar *__restrict__ mag,
+                                     const int *__restrict__ eid, const double *__restrict__ Cstar, const int *__restrict__ rowptr,
+                                     const int *__restrict__ col, double *K, double *Km, double *Mm, double *Kme)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int q0 = rowptr[i], q1 = rowptr[i + 1];
+    for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
+        const int e = n2e[s] >> 2, k = n2e[s] & 3;
+        int t[4];
+        *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(tets)[e];
+        TetGeom g;
+        tet_geometry(xyz, t, ld, g);
+        const bool m = mag[e];
+        double CBt[3][6]; // (B_k^T C): row r, Voigt column w
+        if (Cstar) {
+            const double *C = Cstar + 36 * eid[e];
+            double Bk[6][3];
+            strain_disp(g.g[k], Bk);
+            for (int r = 0; r < 3; r++)
+                for (int w = 0; w < 6; w++) {
+                    double acc = 0;
+                    for (int v = 0; v < 6; v++) acc += Bk[v][r] * C[6 * v + w];
+                    CBt[r][w] = acc;
+                }
+        }
+        for (int l = 0; l < 4; l++) {
+            const int j = t[l];
+            int lo = q0, hi = q1 - 1; // binary search of j in the sorted row
+            while (lo < hi) {
+                int mid = (lo + hi) >> 1;
+                if (col[mid] < j) lo = mid + 1; else hi = mid;
+            }
+            const double kij = g.V * (g.g[k][0] * g.g[l][0] + g.g[k][1] * g.g[l][1] + g.g[k][2] * g.g[l][2]);
+            const double mij = g.V * (k == l ? 2.0 : 1.0) / 20.0;
+            K[lo] += kij;
+            if (m) { Km[lo] += kij; Mm[lo] += mij; }
+            if (Cstar) {
+                double Bl[6][3];
+                strain_disp(g.g[l], Bl);
+                for (int r = 0; r < 3; r++)
+                    for (int c = 0; c < 3; c++) {
+                        double acc = 0;
+                        for (int w = 0; w < 6; w++) acc += CBt[r][w] * Bl[w][c];
+                        Kme[9 * (long)lo + 3 * r + c] += g.V * acc;
+                    }
+            }
+        }
+    }
+}
+
+// one thread per nonzero: apply constraints (P A P + (I - P)), form K^GS(eps), round to T, lay out K^mech tile-SoA
+template <typename T>
+__global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr, const int *__restrict__ col, const double *K,
+                                const double *Km, const double *Mm, const double *Kme, const uchar *__restrict__ live,
+                                const uchar *__restrict__ clamp, int pin, double eps1, double eps2, T *Kms, T *Kgs1, T *Kgs2, T *MmT,
+                                T *Kmech)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    for (int q = rowptr[i]; q < rowptr[i + 1]; q++) {
+        const int j = col[q];
+        double kms = K[q];
+        if (i == pin || j == pin) kms = (i == j) ? 1.0 : 0.0;
+        Kms[q] = (T)kms;
+        const double dead = (i == j && !live[i]) ? 1.0 : 0.0;
+        Kgs1[q] = (T)(Mm[q] + eps1 * Km[q] + dead);
+        Kgs2[q] = (T)(Mm[q] + eps2 * Km[q] + dead);
+        MmT[q] = (T)Mm[q];
+        if (Kme) {
+            T *dst = Kmech + (long)(q >> 5) * 288 + (q & 31);
+            for (int r = 0; r < 3; r++)
+                for (int c = 0; c < 3; c++) {
+                    double v = Kme[9 * (long)q + 3 * r + c];
+                    if (clamp[3 * i + r] || clamp[3 * (long)j + c]) v = (i == j && r == c) ? 1.0 : 0.0;
+                    dst[32 * (3 * r + c)] = (T)v;
+                }
+        }
+    }
+}
+
+template <typename T>
+System<T>::~System()
+{
+    T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, escr, sig, stg_m, stg_U, stg_u};
+    for (T *q : ptrs) cudaFree(q);
+    cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
+    cudaFree(til1.d_tile_row); cudaFree(til3.d_tile_row);
+    if (h_res) cudaFreeHost(h_res);
+    if (h_scal) cudaFreeHost(h_scal);
+}
+template struct System<double>;
+template struct System<float>;
+
+template <typename T>
+int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, long pin_user, cudaStream_t st)
+{
+    cm_mesh *M = S->mesh;
+    const long N = S->N, Ne = S->Ne, nnz = S->nnz;
+    const double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
+    // O-0 nondimensionalisation
+    S->Ms = mat->Ms;
+    S->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
+    S->Kstar = mat->K1 / mu0Ms2;
+    S->dtau = mat->gamma * mat->Ms * S->dt;
+    S->alpha = mat->alpha;
+    S->eps1 = S->Astar * S->dtau;
+    S->eps2 = S->alpha * S->Astar * S->dtau;
+    S->lam100 = mat->lambda100; S->lam111 = mat->lambda111;
+    std::memcpy(S->Nd, mat->Nd, sizeof(S->Nd));
+    S->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
+    S->pin = M->iperm[pin_user];
+    int dev = 0;
+    CM_CUDA(cudaGetDevice(&dev));
+    CM_CUDA(cudaDeviceGetAttribute(&S->num_sms, cudaDevAttrMultiProcessorCount, dev));
+
+    auto alloc = [&](auto **p, size_t n) -> int {
+        CM_CUDA(cudaMalloc((void **)p, std::max<size_t>(n, 1) * sizeof(**p) + 256));
+        CM_CUDA(cudaMemsetAsync(*p, 0, std::max<size_t>(n, 1) * sizeof(**p) + 256, st));
+        return CM_OK;
+    };
+    CM_TRY(alloc(&S->V, Ne)); CM_TRY(alloc(&S->G, 12 * Ne)); CM_TRY(alloc(&S->mL, N)); CM_TRY(alloc(&S->mLm, N));
+    CM_TRY(alloc(&S->live, N)); CM_TRY(alloc(&S->clamp, 3 * N));
+    CM_TRY(alloc(&S->Kms, nnz)); CM_TRY(alloc(&S->Kgs1, nnz)); CM_TRY(alloc(&S->Kgs2, nnz)); CM_TRY(alloc(&S->Mm, nnz));
+    const long nnz_pad = (nnz + 31) / 32 * 32;
+    if (S->n_elastic) CM_TRY(alloc(&S->Kmech, 9 * nnz_pad));
+
+    // elastic constants C* = C / (mu0 Ms^2): fp64 for assembly, T for the element kernels
+    double *Cd = nullptr;
+    if (S->n_elastic) {
+        std::vector<double> Cs(36 * S->n_elastic);
+        std::vector<T> Ct(36 * S->n_elastic);
+        for (size_t q = 0; q < Cs.size(); q++) { Cs[q] = mat->C_voigt[q] / mu0Ms2; Ct[q] = (T)Cs[q]; }
+        CM_CUDA(cudaMalloc((void **)&Cd, Cs.size() * sizeof(double)));
+        CM_CUDA(cudaMemcpyAsync(Cd, Cs.data(), Cs.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+        CM_TRY(alloc(&S->Cstar, Ct.size()));
+        CM_CUDA(cudaMemcpyAsync(S->Cstar, Ct.data(), Ct.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+        CM_CUDA(cudaStreamSynchronize(st));
+    }
+    // clamp flags to library order
+    {
+        std::vector<uchar> cl(3 * N, 0);
+        if (clamp_user)
+            for (long i = 0; i < N; i++)
+                for (int d = 0; d < 3; d++) cl[3 * i + d] = clamp_user[3 * (long)M->order[i] + d] != 0;
+        CM_CUDA(cudaMemcpyAsync(S->clamp, cl.data(), cl.size(), cudaMemcpyHostToDevice, st));
+        CM_CUDA(cudaStreamSynchronize(st));
+    }
+    // geometry
+    double *Vd = nullptr, *vsum = nullptr;
+    CM_CUDA(cudaMalloc((void **)&Vd, Ne * sizeof(double)));
+    CM_CUDA(cudaMalloc((void **)&vsum, 2 * sizeof(double)));
+    const int B = 256;
+    geom_kernel<T><<<(unsigned)((Ne + B - 1) / B), B, 0, st>>>(Ne, M->d_tets, M->d_xyz, ld, S->V, S->G, Vd);
+    lump_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, M->d_n2e_ptr, M->d_n2e, Vd, M->d_mag, S->mL, S->mLm, S->live);
+    volume_sum_kernel<<<1, 1024, 0, st>>>(Ne, Vd, M->d_mag, vsum);
+    CM_CUDA(cudaGetLastError());
+    double hv[2];
+    CM_CUDA(cudaMemcpyAsync(hv, vsum, sizeof(hv), cudaMemcpyDeviceToHost, st));
+    CM_CUDA(cudaStreamSynchronize(st));
+    S->Vtot = hv[0]; S->Vmag = hv[1];
+    {
+        std::vector<uchar> lv(N);
+        CM_CUDA(cudaMemcpy(lv.data(), S->live, N, cudaMemcpyDeviceToHost));
+        S->nlive = 0;
+        for (long i = 0; i < N; i++) S->nlive += lv[i];
+    }
+    // matrices: fp64 scratch on the pattern
+    double *K = nullptr, *Km = nullptr, *Mm = nullptr, *Kme = nullptr;
+    CM_TRY(alloc(&K, nnz)); CM_TRY(alloc(&Km, nnz)); CM_TRY(alloc(&Mm, nnz));
+    if (S->n_elastic) CM_TRY(alloc(&Kme, 9 * nnz));
+    const int BA = 128;
+    assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_xyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag,
+                                                                      M->d_eid, Cd, M->d_rowptr, M->d_col, K, Km, Mm, Kme);
+    finalize_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, nnz, M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->live, S->clamp, S->pin,
+                                                                 S->eps1, S->eps2, S->Kms, S->Kgs1, S->Kgs2, S->Mm, S->Kmech);
+    CM_CUDA(cudaGetLastError());
+    CM_CUDA(cudaStreamSynchronize(st));
+    cudaFree(K); cudaFree(Km); cudaFree(Mm); cudaFree(Kme); cudaFree(Vd); cudaFree(vsum); cudaFree(Cd);
+
+    // tilings and work vectors
+    CM_TRY(build_tiling(M->rowptr, N, CM_TILE_S1, &S->til1, st));
+    CM_TRY(build_tiling(M->rowptr, N, CM_TILE_3, &S->til3, st));
+    T **vecs3[] = {&S->r, &S->p, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->f, &S->gn, &S->gs, &S->ms, &S->mss, &S->xin, &S->xout, &S->stg_m, &S->stg_u};
+    for (T **v : vecs3) CM_TRY(alloc(v, 3 * N));
+    CM_TRY(alloc(&S->U, N)); CM_TRY(alloc(&S->stg_U, N)); CM_TRY(alloc(&S->sig, 6 * N));
+    CM_TRY(alloc(&S->escr, 12 * Ne));
+    S->grid_cap = S->num_sms * 8;
+    CM_TRY(alloc(&S->partial, (size_t)2 * S->grid_cap * 3));
+    CM_TRY(alloc(&S->d_res, 8));
+    CM_TRY(alloc(&S->red, (size_t)4096 * 16));
+    CM_TRY(alloc(&S->dscal, 32));
+    CM_CUDA(cudaMallocHost((void **)&S->h_res, 8 * sizeof(CgResult)));
+    CM_CUDA(cudaMallocHost((void **)&S->h_scal, 32 * sizeof(double)));
+    CM_CUDA(cudaStreamSynchronize(st));
+    return CM_OK;
+}
+
+// values back to the host in standard CSR / BSR order (for parity tests)
+template <typename T>
+int sys_get_values(const System<T> *S, cm_matrix_id id, void *host_out, long capacity)
+{
+    const long nnz = S->nnz;
+    const T *src = nullptr;
+    switch (id) {
+    case CM_MAT_K_MS: src = S->Kms; break;
+    case CM_MAT_K_GS1: src = S->Kgs1; break;
+    case CM_MAT_K_GS2: src = S->Kgs2; break;
+    case CM_MAT_MASS: src = S->Mm; break;
+    case CM_MAT_K_MECH: src = S->Kmech; break;
+    }
+    if (!src) { cm_set_error("cm_system_get_values: matrix %d not assembled", (int)id); return CM_E_BADARG; }
+    if (id != CM_MAT_K_MECH) {
+        if (capacity < nnz) { cm_set_error("cm_system_get_values: capacity"); return CM_E_BADARG; }
+        CM_CUDA(cudaMemcpy(host_out, src, nnz * sizeof(T), cudaMemcpyDeviceToHost));
+        return CM_OK;
+    }
+    if (capacity < 9 * nnz) { cm_set_error("cm_system_get_values: capacity"); return CM_E_BADARG; }
+    const long nnz_pad = (nnz + 31) / 32 * 32;
+    std::vector<T> tmp(9 * nnz_pad);
+    CM_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * sizeof(T), cudaMemcpyDeviceToHost));
+    T *out = (T *)host_out;
+    for (long q = 0; q < nnz; q++)
+        for (int k = 0; k < 9; k++) out[9 * q + k] = tmp[(q >> 5) * 288 + 32 * k + (q & 31)];
+    return CM_OK;
+}
+
+template int sys_assemble<double>(System<double> *, const cm_material *, const uchar *, long, cudaStream_t);
+template int sys_assemble<float>(System<float> *, const cm_material *, const uchar *, long, cudaStream_t);
+template int sys_get_values<double>(const System<double> *, cm_matrix_id, void *, long);
+template int sys_get_values<float>(const System<float> *, cm_matrix_id, void *, long);

@@ -1,0 +1,712 @@
+// S2, S3, S5, S6, S8, S9, S11, S12: volume averages, element-wise gather / compute /
+// deterministic gather-scatter right-hand sides, field recovery, the pointwise Gauss-Seidel algebra and the
+// projection; and the orchestration of one GSPM step (Alg. B.1).
+//
+// Scatter is deterministic: an element pass (one thread per tetrahedron, 128-bit connectivity load, SoA
+// gradients, 4 nodal gathers) writes per-element or per-(element, local node) contributions to a scratch
+// array; a node pass (one thread per node) sums its incident entries through the node->element CSR in
+// ascending element order.  No float atomics.
+#include <cmath>
+#include <cstring>
+#include <limits>
+
+#include "cm_internal.h"
+
+namespace {
+
+constexpr int BS = 256;
+inline unsigned nblk(long n, int b = BS) { return (unsigned)((n + b - 1) / b); }
+
+// ---------------------------------------------------------------- reductions (deterministic, two-stage)
+template <int NV>
+__device__ __forceinline__ void block_reduce_write(double (&v)[NV], double *out /* [gridDim][NV] */)
+{
+    __shared__ double sh[NV * 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; k++)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+    if (lane == 0)
+#pragma unroll
+        for (int k = 0; k < NV; k++) sh[k * 32 + warp] = v[k];
+    __syncthreads();
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < NV; k++) {
+            double s = 0;
+            for (int w = 0; w < nwarp; w++) s += sh[k * 32 + w];
+            out[(long)blockIdx.x * NV + k] = s;
+        }
+}
+
+// single block: out[k] = scale * sum_j partial[j][k]
+__global__ void reduce_final_kernel(int nparts, int nv, const double *__restrict__ partial, double scale, double *out)
+{
+    __shared__ double sh[1024];
+    for (int k = 0; k < nv; k++) {
+        double s = 0;
+        for (int j = threadIdx.x; j < nparts; j += blockDim.x) s += partial[(long)j * nv + k];
+        sh[threadIdx.x] = s;
+        __syncthreads();
+        for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+            if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) out[k] = scale * sh[0];
+        __syncthreads();
+    }
+}
+
+constexpr int RED_BLOCKS = 2048; // partial blocks of the node-parallel reductions
+
+// S2: sum_i w_i g[i][c]  (w = lumped volume fraction; algebraically Eq. 17 for P1 elements)
+template <typename T, int NC>
+__global__ void wsum_kernel(long N, const double *__restrict__ w, const T *__restrict__ g, double *partial)
+{
+    double acc[NC];
+#pragma unroll
+    for (int c = 0; c < NC; c++) acc[c] = 0;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < N; i += (long)gridDim.x * blockDim.x) {
+        const double wi = w[i];
+#pragma unroll
+        for (int c = 0; c < NC; c++) acc[c] += wi * (double)g[i * NC + c];
+    }
+    block_reduce_write<NC>(acc, partial);
+}
+
+// ---------------------------------------------------------------- permutation
+template <typename T>
+__global__ void permute_in_kernel(long N, int nc, const int *__restrict__ order, const T *__restrict__ user, T *lib)
+{
+    long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (k >= N * nc) return;
+    long i = k / nc;
+    int c = (int)(k - i * nc);
+    lib[k] = user[(long)order[i] * nc + c];
+}
+template <typename T>
+__global__ void permute_out_kernel(long N, int nc, const int *__restrict__ order, const T *__restrict__ lib, T *user)
+{
+    long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (k >= N * nc) return;
+    long i = k / nc;
+    int c = (int)(k - i * nc);
+    user[(long)order[i] * nc + c] = lib[k];
+}
+
+// ---------------------------------------------------------------- element helpers
+template <typename T>
+struct Elem {
+    int t[4];
+    T V;
+    T g[4][3];
+};
+
+template <typename T>
+__device__ __forceinline__ void load_elem(long e, long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
+                                          Elem<T> &E)
+{
+    *reinterpret_cast<int4 *>(E.t) = __ldg(reinterpret_cast<const int4 *>(tets) + e);
+    E.V = __ldg(V + e);
+#pragma unroll
+    for (int k = 0; k < 4; k++)
+#pragma unroll
+        for (int d = 0; d < 3; d++) E.g[k][d] = __ldg(G + (long)(3 * k + d) * Ne + e);
+}
+
+// E0(m), Table A.1, Voigt engineering vector (E11, E22, E33, 2 E23, 2 E13, 2 E12)
+template <typename T>
+__device__ __forceinline__ void E0_voigt(const T *m, T l1, T l2, T e0[6])
+{
+    const T th = (T)1.5, third = (T)(1.0 / 3.0);
+    e0[0] = th * l1 * (m[0] * m[0] - third);
+    e0[1] = th * l1 * (m[1] * m[1] - third);
+    e0[2] = th * l1 * (m[2] * m[2] - third);
+    e0[3] = (T)2 * th * l2 * m[1] * m[2];
+    e0[4] = (T)2 * th * l2 * m[0] * m[2];
+    e0[5] = (T)2 * th * l2 * m[0] * m[1];
+}
+
+template <typename T>
+__device__ __forceinline__ void mean_E0(const T *__restrict__ w, const int *t, T l1, T l2, T e0[6])
+{
+#pragma unroll
+    for (int q = 0; q < 6; q++) e0[q] = 0;
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        T mk[3] = {w[3 * (long)t[k]], w[3 * (long)t[k] + 1], w[3 * (long)t[k] + 2]}, ek[6];
+        E0_voigt(mk, l1, l2, ek);
+#pragma unroll
+        for (int q = 0; q < 6; q++) e0[q] += ek[q];
+    }
+#pragma unroll
+    for (int q = 0; q < 6; q++) e0[q] /= (T)4;
+}
+
+template <typename T>
+__device__ __forceinline__ void C_times(const T *__restrict__ C, const T eps[6], T sig[6])
+{
+#pragma unroll
+    for (int r = 0; r < 6; r++) {
+        T acc = 0;
+#pragma unroll
+        for (int s = 0; s < 6; s++) acc += __ldg(C + 6 * r + s) * eps[s];
+        sig[r] = acc;
+    }
+}
+
+// ---------------------------------------------------------------- S3 magnetostatic RHS
+// element pass: contribution of tet e to its 4 nodes, c_k = V_e grad phi_k . (mean_e m - mbar)
+template <typename T>
+__global__ void elem_ms_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
+                               const T *__restrict__ m, const double *__restrict__ mbar, T *scr)
+{
+    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= Ne) return;
+    Elem<T> E;
+    load_elem(e, Ne, tets, V, G, E);
+    T mt[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++)
+        mt[d] = (m[3 * (long)E.t[0] + d] + m[3 * (long)E.t[1] + d] + m[3 * (long)E.t[2] + d] + m[3 * (long)E.t[3] + d]) / (T)4 - (T)mbar[d];
+#pragma unroll
+    for (int k = 0; k < 4; k++) scr[4 * e + k] = E.V * (E.g[k][0] * mt[0] + E.g[k][1] * mt[1] + E.g[k][2] * mt[2]);
+}
+
+// node pass: b_i = sum over incident (e,k) of scr[(4e+k) * NC + c]; zero where mask says so
+template <typename T, int NC>
+__global__ void node_gather_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const T *__restrict__ scr,
+                                   const uchar *__restrict__ zero_mask /* N*NC or NULL */, int zero_node, T *b)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    T acc[NC];
+#pragma unroll
+    for (int c = 0; c < NC; c++) acc[c] = 0;
+    for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
+        const long q = __ldg(n2e + s);
+#pragma unroll
+        for (int c = 0; c < NC; c++) acc[c] += scr[q * NC + c];
+    }
+#pragma unroll
+    for (int c = 0; c < NC; c++) {
+        if (zero_mask && zero_mask[i * NC + c]) acc[c] = 0;
+        if (i == zero_node) acc[c] = 0;
+        b[i * NC + c] = acc[c];
+    }
+}
+
+// ---------------------------------------------------------------- S5 gradient recovery
+// element pass: scr[e][0..2] = V_e grad U_e ; block partial sums of the same (fp64) for <grad U>
+template <typename T>
+__global__ void elem_gradU_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
+                                  const T *__restrict__ U, T *scr, double *partial)
+{
+    double acc[3] = {0, 0, 0};
+    for (long e = blockIdx.x * (long)blockDim.x + threadIdx.x; e < Ne; e += (long)gridDim.x * blockDim.x) {
+        Elem<T> E;
+        load_elem(e, Ne, tets, V, G, E);
+        const T u0 = U[E.t[0]], u1 = U[E.t[1]], u2 = U[E.t[2]], u3 = U[E.t[3]];
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            const T gU = u0 * E.g[0][d] + u1 * E.g[1][d] + u2 * E.g[2][d] + u3 * E.g[3][d];
+            scr[3 * e + d] = E.V * gU;
+            acc[d] += (double)E.V * (double)gU;
+        }
+    }
+    block_reduce_write<3>(acc, partial);
+}
+
+// node pass: h_d,i = -sum_{e} V_e grad U_e / (4 mL_i) + <grad U>   (DEMAG)   - N_d mbar   (FARFIELD)
+template <typename T>
+__global__ void node_hd_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const T *__restrict__ scr,
+                               const T *__restrict__ mL, const double *__restrict__ scal /* mbar[0..2], gradU mean[3..5] */,
+                               double Vtot_inv_unused, unsigned terms, double n00, double n01, double n02, double n10, double n11,
+                               double n12, double n20, double n21, double n22, T *hd)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    T h[3] = {0, 0, 0};
+    if (terms & CM_TERM_DEMAG) {
+        T acc[3] = {0, 0, 0};
+        for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
+            const long e = __ldg(n2e + s) >> 2;
+#pragma unroll
+            for (int d = 0; d < 3; d++) acc[d] += scr[3 * e + d];
+        }
+        const T den = (T)4 * mL[i];
+#pragma unroll
+        for (int d = 0; d < 3; d++) h[d] = -acc[d] / den + (T)scal[3 + d];
+    }
+    if (terms & CM_TERM_FARFIELD) {
+        const double m0 = scal[0], m1 = scal[1], m2 = scal[2];
+        h[0] -= (T)(n00 * m0 + n01 * m1 + n02 * m2);
+        h[1] -= (T)(n10 * m0 + n11 * m1 + n12 * m2);
+        h[2] -= (T)(n20 * m0 + n21 * m1 + n22 * m2);
+    }
+    hd[3 * i] = h[0]; hd[3 * i + 1] = h[1]; hd[3 * i + 2] = h[2];
+}
+
+// ---------------------------------------------------------------- S6 mechanical RHS
+// element pass (magnetic tets): S = C*_e : mean_e E0(m);  scr[(4e+k)*3 + a] = V_e (S grad phi_k)_a
+template <typename T>
+__global__ void elem_mech_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
+                                 const uchar *__restrict__ mag, const int *__restrict__ eid, const T *__restrict__ Cstar,
+                                 const T *__restrict__ m, T l1, T l2, T *scr)
+{
+    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= Ne) return;
+    if (!mag[e]) {
+#pragma unroll
+        for (int q = 0; q < 12; q++) scr[12 * e + q] = 0;
+        return;
+    }
+    Elem<T> E;
+    load_elem(e, Ne, tets, V, G, E);
+    T e0[6], s[6];
+    mean_E0(m, E.t, l1, l2, e0);
+    C_times(Cstar + 36 * eid[e], e0, s);
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const T *g = E.g[k];
+        scr[12 * e + 3 * k + 0] = E.V * (s[0] * g[0] + s[5] * g[1] + s[4] * g[2]);
+        scr[12 * e + 3 * k + 1] = E.V * (s[5] * g[0] + s[1] * g[1] + s[3] * g[2]);
+        scr[12 * e + 3 * k + 2] = E.V * (s[4] * g[0] + s[3] * g[1] + s[2] * g[2]);
+    }
+}
+
+// ---------------------------------------------------------------- S8 stress recovery
+// element pass (magnetic tets): scr[e][0..5] = V_e C*_e : (E_e(u) - mean_e E0(w))
+template <typename T>
+__global__ void elem_stress_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
+                                   const uchar *__restrict__ mag, const int *__restrict__ eid, const T *__restrict__ Cstar,
+                                   const T *__restrict__ u, const T *__restrict__ w, T l1, T l2, T *scr)
+{
+    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= Ne) return;
+    if (!mag[e]) {
+#pragma unroll
+        for (int q = 0; q < 6; q++) scr[6 * e + q] = 0;
+        return;
+    }
+    Elem<T> E;
+    load_elem(e, Ne, tets, V, G, E);
+    T H[3][3]; // H[a][b] = d_b u_a
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+#pragma unroll
+        for (int b = 0; b < 3; b++) {
+            T acc = 0;
+#pragma unroll
+            for (int k = 0; k < 4; k++) acc += u[3 * (long)E.t[k] + a] * E.g[k][b];
+            H[a][b] = acc;
+        }
+    T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]}, e0[6], s[6];
+    mean_E0(w, E.t, l1, l2, e0);
+#pragma unroll
+    for (int q = 0; q < 6; q++) eps[q] -= e0[q];
+    C_times(Cstar + 36 * eid[e], eps, s);
+#pragma unroll
+    for (int q = 0; q < 6; q++) scr[6 * e + q] = E.V * s[q];
+}
+
+// ---------------------------------------------------------------- S9 nodal field
+// node pass: sigma_hat_i (gathered from scr when MAGEL), h = h_an + h_ext + h_d + h_me on live nodes;
+// optionally also writes sigma_hat (parity output).
+template <typename T>
+__global__ void node_field_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const T *__restrict__ scr,
+                                  const T *__restrict__ mLm, const uchar *__restrict__ live, const T *__restrict__ w,
+                                  const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, T l1, T l2, T *h, T *sig_out)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    T hi[3] = {0, 0, 0}, s[6] = {0, 0, 0, 0, 0, 0};
+    if (live[i]) {
+        const T m[3] = {w[3 * i], w[3 * i + 1], w[3 * i + 2]};
+        if (terms & CM_TERM_ANIS) {
+            hi[0] -= Kstar2 * m[0] * (m[1] * m[1] + m[2] * m[2]);
+            hi[1] -= Kstar2 * m[1] * (m[2] * m[2] + m[0] * m[0]);
+            hi[2] -= Kstar2 * m[2] * (m[0] * m[0] + m[1] * m[1]);
+        }
+        if (terms & CM_TERM_ZEEMAN) { hi[0] += hx; hi[1] += hy; hi[2] += hz; }
+        if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) { hi[0] += hd[3 * i]; hi[1] += hd[3 * i + 1]; hi[2] += hd[3 * i + 2]; }
+        if (terms & CM_TERM_MAGEL) {
+            for (int q = n2e_ptr[i]; q < n2e_ptr[i + 1]; q++) {
+                const long e = __ldg(n2e + q) >> 2;
+#pragma unroll
+                for (int c = 0; c < 6; c++) s[c] += scr[6 * e + c];
+            }
+            const T den = (T)4 * mLm[i];
+#pragma unroll
+            for (int c = 0; c < 6; c++) s[c] /= den;
+            hi[0] += (T)3 * (l1 * m[0] * s[0] + l2 * (m[1] * s[5] + m[2] * s[4]));
+            hi[1] += (T)3 * (l1 * m[1] * s[1] + l2 * (m[0] * s[5] + m[2] * s[3]));
+            hi[2] += (T)3 * (l1 * m[2] * s[2] + l2 * (m[0] * s[4] + m[1] * s[3]));
+        }
+    }
+    if (h) { h[3 * i] = hi[0]; h[3 * i + 1] = hi[1]; h[3 * i + 2] = hi[2]; }
+    if (sig_out)
+#pragma unroll
+        for (int c = 0; c < 6; c++) sig_out[6 * i + c] = s[c];
+}
+
+// ---------------------------------------------------------------- pointwise GSPM algebra (S9, S11, S12)
+// f = base + c h   (3N entries)
+template <typename T>
+__global__ void axpby_kernel(long n, const T *__restrict__ base, const T *__restrict__ h, T c, T *f)
+{
+    long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (k < n) f[k] = base[k] + c * h[k];
+}
+
+// Step 2, first part.  variant 0: m*_1, m*_2 from level-n values; f_a = m*_a + dtau h_a[m^n], a = 1, 2.
+// variant 1, stage 0: m*_1 and f_1 only; stage 1: m*_2 = m_2 + (g^n_3 m*_1 - g*_1 m_3) and f_2.
+template <typename T>
+__global__ void gs_step2_kernel(long N, int variant, int stage, const T *__restrict__ m, const T *__restrict__ gn,
+                                const T *__restrict__ gs, const T *__restrict__ hn, T dtau, T *ms, T *f)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const T m0 = m[3 * i], m1 = m[3 * i + 1], m2 = m[3 * i + 2];
+    if (variant == 0 || stage == 0) {
+        const T s0 = m0 + (gn[3 * i + 1] * m2 - gn[3 * i + 2] * m1);
+        ms[3 * i] = s0;
+        f[3 * i] = s0 + dtau * hn[3 * i];
+    }
+    if (variant == 0) {
+        const T s1 = m1 + (gn[3 * i + 2] * m0 - gn[3 * i] * m2);
+        ms[3 * i + 1] = s1;
+        f[3 * i + 1] = s1 + dtau * hn[3 * i + 1];
+    } else if (stage == 1) {
+        const T s1 = m1 + (gn[3 * i + 2] * ms[3 * i] - gs[3 * i] * m2);
+        ms[3 * i + 1] = s1;
+        f[3 * i + 1] = s1 + dtau * hn[3 * i + 1];
+    }
+}
+
+// m*_3 = m_3 + (g*_1 m*_2 - g*_2 m*_1)
+template <typename T>
+__global__ void gs_step2c_kernel(long N, const T *__restrict__ m, const T *__restrict__ gs, T *ms)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    ms[3 * i + 2] = m[3 * i + 2] + (gs[3 * i] * ms[3 * i + 1] - gs[3 * i + 1] * ms[3 * i]);
+}
+
+// Step 4: projection on live nodes, dead nodes zero; partial sums of ||m_new - m_old||_2
+template <typename T>
+__global__ void project_kernel(long N, const uchar *__restrict__ live, const T *__restrict__ mss, T *m, double *partial)
+{
+    double acc[1] = {0};
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < N; i += (long)gridDim.x * blockDim.x) {
+        if (!live[i]) { m[3 * i] = 0; m[3 * i + 1] = 0; m[3 * i + 2] = 0; continue; }
+        const T v0 = mss[3 * i], v1 = mss[3 * i + 1], v2 = mss[3 * i + 2];
+        const T nrm = (T)sqrt((double)(v0 * v0 + v1 * v1 + v2 * v2));
+        const T o0 = m[3 * i], o1 = m[3 * i + 1], o2 = m[3 * i + 2];
+        T n0 = o0, n1 = o1, n2 = o2;
+        if (nrm > 0) { n0 = v0 / nrm; n1 = v1 / nrm; n2 = v2 / nrm; }
+        const double d0 = (double)n0 - (double)o0, d1 = (double)n1 - (double)o1, d2 = (double)n2 - (double)o2;
+        acc[0] += sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+        m[3 * i] = n0; m[3 * i + 1] = n1; m[3 * i + 2] = n2;
+    }
+    block_reduce_write<1>(acc, partial);
+}
+
+} // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host launchers
+// ------------------------------------------------------------------------------------------------
+#define LAUNCH_CHECK() CM_CUDA(cudaGetLastError())
+
+template <typename T>
+int sys_permute_in(System<T> *S, const T *user, T *lib, int nc, cudaStream_t st)
+{
+    const long n = S->N * nc;
+    if (S->mesh->identity) { CM_CUDA(cudaMemcpyAsync(lib, user, n * sizeof(T), cudaMemcpyDeviceToDevice, st)); return CM_OK; }
+    S->prof.begin(CM_PROF_POINTWISE, st);
+    permute_in_kernel<T><<<nblk(n), BS, 0, st>>>(S->N, nc, S->mesh->d_order, user, lib);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+template <typename T>
+int sys_permute_out(System<T> *S, const T *lib, T *user, int nc, cudaStream_t st)
+{
+    const long n = S->N * nc;
+    if (S->mesh->identity) { CM_CUDA(cudaMemcpyAsync(user, lib, n * sizeof(T), cudaMemcpyDeviceToDevice, st)); return CM_OK; }
+    S->prof.begin(CM_PROF_POINTWISE, st);
+    permute_out_kernel<T><<<nblk(n), BS, 0, st>>>(S->N, nc, S->mesh->d_order, lib, user);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+// volume average of an NC-component library-order field into dst[0..NC) (device)
+template <typename T>
+static int wavg(const cm_mesh *M, const T *g_lib, int nc, double *red, double *dst, cudaStream_t st)
+{
+    const int nb = (int)std::min<long>(RED_BLOCKS, nblk(M->N));
+    switch (nc) {
+    case 1: wsum_kernel<T, 1><<<nb, BS, 0, st>>>(M->N, M->d_wvol, g_lib, red); break;
+    case 3: wsum_kernel<T, 3><<<nb, BS, 0, st>>>(M->N, M->d_wvol, g_lib, red); break;
+    case 6: wsum_kernel<T, 6><<<nb, BS, 0, st>>>(M->N, M->d_wvol, g_lib, red); break;
+    default: cm_set_error("volume average: ncomp must be 1, 3 or 6"); return CM_E_BADARG;
+    }
+    reduce_final_kernel<<<1, 1024, 0, st>>>(nb, nc, red, 1.0, dst);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_mbar(System<T> *S, const T *m_lib, cudaStream_t st)
+{
+    S->prof.begin(CM_PROF_POINTWISE, st, 2);
+    int rc = wavg<T>(S->mesh, m_lib, 3, S->red, S->dscal, st);
+    S->prof.end(st);
+    return rc;
+}
+
+template <typename T>
+int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
+{
+    cm_mesh *M = S->mesh;
+    S->prof.begin(CM_PROF_ELEMENT, st, 2);
+    elem_ms_kernel<T><<<nblk(S->Ne), BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, m_lib, S->dscal, S->escr);
+    node_gather_kernel<T, 1><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, nullptr, S->pin, b);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStream_t st)
+{
+    cm_mesh *M = S->mesh;
+    S->prof.begin(CM_PROF_ELEMENT, st, (terms & CM_TERM_DEMAG) ? 3 : 1);
+    if (terms & CM_TERM_DEMAG) {
+        const int nb = (int)std::min<long>(RED_BLOCKS, nblk(S->Ne));
+        elem_gradU_kernel<T><<<nb, BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, U_lib, S->escr, S->red);
+        reduce_final_kernel<<<1, 1024, 0, st>>>(nb, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
+    }
+    const double *n = S->Nd;
+    node_hd_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, S->mL, S->dscal, 0.0, terms, n[0], n[1], n[2], n[3],
+                                                 n[4], n[5], n[6], n[7], n[8], hd);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
+{
+    cm_mesh *M = S->mesh;
+    if (!S->n_elastic) { cm_set_error("mechanics requested but the material has no elastic constants"); return CM_E_BADARG; }
+    S->prof.begin(CM_PROF_ELEMENT, st, 2);
+    elem_mech_kernel<T><<<nblk(S->Ne), BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, M->d_mag, M->d_eid, S->Cstar, m_lib, (T)S->lam100,
+                                                   (T)S->lam111, S->escr);
+    node_gather_kernel<T, 3><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, S->clamp, -1, b);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st)
+{
+    cm_mesh *M = S->mesh;
+    if (!S->n_elastic) { cm_set_error("mechanics requested but the material has no elastic constants"); return CM_E_BADARG; }
+    S->prof.begin(CM_PROF_ELEMENT, st);
+    elem_stress_kernel<T><<<nblk(S->Ne), BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, M->d_mag, M->d_eid, S->Cstar, u_lib, w_lib,
+                                                     (T)S->lam100, (T)S->lam111, S->escr);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h, T *sig_out, cudaStream_t st)
+{
+    cm_mesh *M = S->mesh;
+    S->prof.begin(CM_PROF_ELEMENT, st);
+    node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, S->mLm, S->live, w_lib, hd, terms,
+                                                   (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], (T)S->lam100, (T)S->lam111, h,
+                                                   sig_out);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t st)
+{
+    S->prof.begin(CM_PROF_POINTWISE, st);
+    axpby_kernel<T><<<nblk(3 * S->N), BS, 0, st>>>(3 * S->N, base, h, c, f);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// one GSPM step (O-3)
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_user, cm_step_info *info, cudaStream_t st)
+{
+    const long N = S->N;
+    const unsigned terms = p->terms;
+    if (p->dt != S->dt) { cm_set_error("cm_gspm_step: params->dt differs from the dt given to cm_assemble_csr"); return CM_E_BADARG; }
+    if ((terms & CM_TERM_MAGEL) && !S->n_elastic) { cm_set_error("cm_gspm_step: MAGEL needs elastic constants"); return CM_E_BADARG; }
+    if (((terms & CM_TERM_DEMAG) && !U_user) || ((terms & CM_TERM_MAGEL) && !u_user) || !m_user) {
+        cm_set_error("cm_gspm_step: null field pointer");
+        return CM_E_BADARG;
+    }
+    const double hext[3] = {p->Hext[0] / S->Ms, p->Hext[1] / S->Ms, p->Hext[2] / S->Ms};
+    const T dtau = (T)S->dtau, adtau = (T)(S->alpha * S->dtau);
+    const double tol = p->cg_tol;
+    const int mx = p->cg_maxiter, fx = p->cg_fixed_iters;
+    CM_CUDA(cudaMemsetAsync(S->d_res, 0, 8 * sizeof(CgResult), st));
+
+    CM_TRY(sys_permute_in(S, m_user, S->m, 3, st));
+    // 1. mbar (Eq. 17)
+    CM_TRY(sys_mbar(S, S->m, st));
+    // 2. magnetostatic solve, warm start (Eq. 5, 9)
+    if (terms & CM_TERM_DEMAG) {
+        CM_TRY(sys_permute_in(S, U_user, S->U, 1, st));
+        CM_TRY(sys_rhs_ms(S, S->m, S->bvec, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_MS, MODE_CSR1, S->bvec, S->U, tol, mx, fx, 1u, 0, CM_PROF_CG_MS, st));
+    }
+    // 3. demagnetising field (Eq. 4)
+    if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) CM_TRY(sys_demag_field(S, S->U, terms, S->hd, st));
+    // 4. mechanical equilibrium (Eq. 6, 10), warm start; stress at m^n
+    if (terms & CM_TERM_MAGEL) {
+        CM_TRY(sys_permute_in(S, u_user, S->u, 3, st));
+        CM_TRY(sys_rhs_mech(S, S->m, S->bvec, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, st));
+        CM_TRY(sys_stress(S, S->u, S->m, st));
+    }
+    // 5. h[m^n];  6. Step 1: g^n
+    CM_TRY(sys_field(S, S->m, S->hd, hext, terms, S->hn, (T *)nullptr, st));
+    CM_TRY(sys_axpby3(S, S->m, S->hn, dtau, S->f, st));
+    CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
+    CM_CUDA(cudaMemcpyAsync(S->gn, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gn, tol, mx, fx, p->gspm_variant == 1 ? 6u : 7u, 2, CM_PROF_CG_GS, st));
+    // 7. Step 2 interleaved with the g* solves
+    S->prof.begin(CM_PROF_POINTWISE, st);
+    gs_step2_kernel<T><<<nblk(N), BS, 0, st>>>(N, p->gspm_variant, 0, S->m, S->gn, S->gs, S->hn, dtau, S->ms, S->f);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    if (p->gspm_variant == 0) {
+        CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
+        CM_CUDA(cudaMemcpyAsync(S->gs, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gs, tol, mx, fx, 3u, 3, CM_PROF_CG_GS, st));
+    } else {
+        CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
+        CM_CUDA(cudaMemcpyAsync(S->gs, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gs, tol, mx, fx, 1u, 3, CM_PROF_CG_GS, st));
+        S->prof.begin(CM_PROF_POINTWISE, st);
+        gs_step2_kernel<T><<<nblk(N), BS, 0, st>>>(N, 1, 1, S->m, S->gn, S->gs, S->hn, dtau, S->ms, S->f);
+        S->prof.end(st);
+        LAUNCH_CHECK();
+        CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
+        // x0 = f for component 2 only (component 1 already holds g*_1)
+        CM_CUDA(cudaMemcpy2DAsync(S->gs + 1, 3 * sizeof(T), S->f + 1, 3 * sizeof(T), sizeof(T), N, cudaMemcpyDeviceToDevice, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gs, tol, mx, fx, 2u, 4, CM_PROF_CG_GS, st));
+    }
+    S->prof.begin(CM_PROF_POINTWISE, st);
+    gs_step2c_kernel<T><<<nblk(N), BS, 0, st>>>(N, S->m, S->gs, S->ms);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    // 8. Step 3: h* = h[m*] with U, u frozen (R3)
+    if (terms & CM_TERM_MAGEL) CM_TRY(sys_stress(S, S->u, S->ms, st));
+    CM_TRY(sys_field(S, S->ms, S->hd, hext, terms, S->hn, (T *)nullptr, st));
+    CM_TRY(sys_axpby3(S, S->ms, S->hn, adtau, S->f, st));
+    CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
+    CM_CUDA(cudaMemcpyAsync(S->mss, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    CM_TRY(sys_cg(S, CM_MAT_K_GS2, MODE_CSR3, S->bvec, S->mss, tol, mx, fx, 7u, 5, CM_PROF_CG_GS, st));
+    // 9. Step 4 projection; 10. diagnostics
+    {
+        const int nb = (int)std::min<long>(RED_BLOCKS, nblk(N));
+        S->prof.begin(CM_PROF_POINTWISE, st, 2);
+        project_kernel<T><<<nb, BS, 0, st>>>(N, S->live, S->mss, S->m, S->red);
+        reduce_final_kernel<<<1, 1024, 0, st>>>(nb, 1, S->red, S->nlive ? 1.0 / (double)S->nlive : 0.0, S->dscal + 6);
+        S->prof.end(st);
+        LAUNCH_CHECK();
+    }
+    CM_TRY(sys_permute_out(S, S->m, m_user, 3, st));
+    if (terms & CM_TERM_DEMAG) CM_TRY(sys_permute_out(S, S->U, U_user, 1, st));
+    if (terms & CM_TERM_MAGEL) CM_TRY(sys_permute_out(S, S->u, u_user, 3, st));
+
+    int worst = CM_OK;
+    if (info) {
+        CM_CUDA(cudaMemcpyAsync(S->h_res, S->d_res, 8 * sizeof(CgResult), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaMemcpyAsync(S->h_scal, S->dscal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaStreamSynchronize(st));
+        std::memset(info, 0, sizeof(*info));
+        const CgResult *R = S->h_res;
+        info->it_ms = R[0].iters[0]; info->res_ms = R[0].relres[0];
+        info->it_mech = R[1].iters[0]; info->res_mech = R[1].relres[0];
+        for (int a = 0; a < 3; a++) { info->it_gs[a] = R[2].iters[a]; info->res_gs[a] = R[2].relres[a]; }
+        if (p->gspm_variant == 0) {
+            for (int a = 0; a < 2; a++) { info->it_gs[3 + a] = R[3].iters[a]; info->res_gs[3 + a] = R[3].relres[a]; }
+        } else {
+            info->it_gs[3] = R[3].iters[0]; info->res_gs[3] = R[3].relres[0];
+            info->it_gs[4] = R[4].iters[1]; info->res_gs[4] = R[4].relres[1];
+        }
+        for (int a = 0; a < 3; a++) { info->it_gs[5 + a] = R[5].iters[a]; info->res_gs[5 + a] = R[5].relres[a]; }
+        for (int d = 0; d < 3; d++) info->mbar[d] = S->h_scal[d];
+        info->mean_dm = S->h_scal[6];
+        info->energy = std::numeric_limits<double>::quiet_NaN();
+        for (int s = 0; s < 6; s++) worst = std::min(worst, R[s].status);
+        // profiler bookkeeping of CG work
+        S->prof.cg_iters[CM_PROF_CG_MS] += R[0].iters[0]; S->prof.cg_passes[CM_PROF_CG_MS] += R[0].iters[0];
+        S->prof.cg_iters[CM_PROF_CG_MECH] += R[1].iters[0]; S->prof.cg_passes[CM_PROF_CG_MECH] += R[1].iters[0];
+        for (int s = 2; s < 6; s++) {
+            int mxit = 0;
+            for (int a = 0; a < 3; a++) { S->prof.cg_iters[CM_PROF_CG_GS] += R[s].iters[a]; mxit = std::max(mxit, R[s].iters[a]); }
+            S->prof.cg_passes[CM_PROF_CG_GS] += mxit;
+        }
+    }
+    return worst;
+}
+
+#define INST(T)                                                                                                       \
+    template int sys_permute_in<T>(System<T> *, const T *, T *, int, cudaStream_t);                                   \
+    template int sys_permute_out<T>(System<T> *, const T *, T *, int, cudaStream_t);                                  \
+    template int sys_mbar<T>(System<T> *, const T *, cudaStream_t);                                                   \
+    template int sys_rhs_ms<T>(System<T> *, const T *, T *, cudaStream_t);                                            \
+    template int sys_demag_field<T>(System<T> *, const T *, unsigned, T *, cudaStream_t);                             \
+    template int sys_rhs_mech<T>(System<T> *, const T *, T *, cudaStream_t);                                          \
+    template int sys_stress<T>(System<T> *, const T *, const T *, cudaStream_t);                                      \
+    template int sys_field<T>(System<T> *, const T *, const T *, const double *, unsigned, T *, T *, cudaStream_t);   \
+    template int sys_axpby3<T>(System<T> *, const T *, const T *, T, T *, cudaStream_t);                              \
+    template int sys_step<T>(System<T> *, const cm_step_params *, T *, T *, T *, cm_step_info *, cudaStream_t);
+INST(double)
+INST(float)
+
+// volume average entry used by cm_volume_average (user-order input)
+template <typename T>
+int mesh_volume_average(cm_mesh *M, const T *g_user, int nc, double *out_host, cudaStream_t st)
+{
+    const long n = M->N * nc;
+    const T *g_lib = g_user;
+    if (!M->identity) {
+        if (M->tmp_bytes < (long)(n * sizeof(T))) {
+            cudaFree(M->d_tmp);
+            M->d_tmp = nullptr;
+            M->tmp_bytes = 0;
+            CM_CUDA(cudaMalloc(&M->d_tmp, n * sizeof(T)));
+            M->tmp_bytes = n * sizeof(T);
+        }
+        permute_in_kernel<T><<<nblk(n), BS, 0, st>>>(M->N, nc, M->d_order, g_user, (T *)M->d_tmp);
+        g_lib = (const T *)M->d_tmp;
+    }
+    CM_TRY(wavg<T>(M, g_lib, nc, M->d_red, M->d_red + RED_BLOCKS * 8, st));
+    CM_CUDA(cudaMemcpyAsync(M->h_red, M->d_red + RED_BLOCKS * 8, nc * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CM_CUDA(cudaStreamSynchronize(st));
+    for (int c = 0; c < nc; c++) out_host[c] = M->h_red[c];
+    return CM_OK;
+}
+template int mesh_volume_average<double>(cm_mesh *, const double *, int, double *, cudaStream_t);
+template int mesh_volume_average<float>(cm_mesh *, const float *, int, double *, cudaStream_t);

@@ -1,0 +1,152 @@
+// Internal declarations of the CuPyMag-B200 library (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/cupymag_b200.h"
+
+typedef unsigned char uchar;
+
+void cm_set_error(const char *fmt, ...);
+
+#define CM_CUDA(call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            cm_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return CM_E_CUDA;                                                                  \
+        }                                                                                      \
+    } while (0)
+
+#define CM_TRY(call)             \
+    do {                         \
+        int rc_ = (call);        \
+        if (rc_ < 0) return rc_; \
+    } while (0)
+
+// Persistent-kernel launch shape: NT threads per CTA everywhere in the SpMV / CG path.
+// NT is a multiple of 3 so that thread t always serves component t % 3.
+constexpr int CM_NT = 384;
+constexpr int CM_TILE_S1 = 4 * CM_NT; // nnz per tile, scalar CSR with one right-hand side
+constexpr int CM_TILE_3 = 2 * CM_NT;  // nnz (blocks) per tile, 3-component modes (CSR3, BSR3)
+
+enum SpmvMode { MODE_CSR1 = 0, MODE_CSR3 = 1, MODE_BSR3 = 2 };
+
+struct cm_mesh {
+    long N = 0, Ne = 0, nnz = 0;
+    bool identity = true;
+    // host copies, library order
+    std::vector<int> order, iperm, tets, tet_order, rowptr, col, n2e_ptr, n2e, eid;
+    std::vector<uchar> mag;
+    std::vector<double> xyz;   // N x 3 metres, library order
+    std::vector<double> wvol;  // N: lumped volume fraction mL_i / V (sums to 1)
+    // device
+    int *d_order = nullptr, *d_tets = nullptr, *d_rowptr = nullptr, *d_col = nullptr, *d_n2e_ptr = nullptr, *d_n2e = nullptr,
+        *d_eid = nullptr;
+    uchar *d_mag = nullptr;
+    double *d_xyz = nullptr, *d_wvol = nullptr;
+    // scratch for cm_volume_average
+    double *d_red = nullptr;   // partials
+    void *d_tmp = nullptr;     // N x 16 x 8 bytes? (allocated lazily, see cm_volume_average)
+    long tmp_bytes = 0;
+    double *h_red = nullptr;   // pinned, 16 doubles
+};
+
+struct CgResult {
+    int iters[3];
+    double relres[3];
+    int status;
+    int pad;
+};
+
+struct Profiler {
+    bool on = false;
+    struct Rec { cudaEvent_t a, b; int cls; };
+    std::vector<Rec> pending;
+    std::vector<cudaEvent_t> pool;
+    double ms[CM_PROF_NCLASS] = {0};
+    long launches[CM_PROF_NCLASS] = {0};
+    long cg_iters[CM_PROF_NCLASS] = {0};
+    long cg_passes[CM_PROF_NCLASS] = {0};
+    cudaEvent_t get();
+    void begin(int cls, cudaStream_t s, int nlaunch = 1); // counts launches always, times them when `on`
+    void end(cudaStream_t s);
+    int flush();
+    ~Profiler();
+};
+
+// One scalar tiling = row ranges with at most TILE nonzeros each.
+struct Tiling {
+    int tile = 0;
+    int ntiles = 0;
+    int *d_tile_row = nullptr; // ntiles + 1
+};
+
+struct SystemBase {
+    cm_mesh *mesh = nullptr;
+    cm_dtype dtype = CM_F64;
+    long N = 0, Ne = 0, nnz = 0;
+    double dt = 0, Astar = 0, Kstar = 0, dtau = 0, eps1 = 0, eps2 = 0, alpha = 0, lam100 = 0, lam111 = 0, Ms = 0;
+    double Nd[9] = {0};
+    int n_elastic = 0;
+    double Vtot = 0, Vmag = 0;
+    long nlive = 0;
+    int pin = 0; // library index
+    int num_sms = 0;
+    Profiler prof;
+    virtual ~SystemBase() {}
+};
+
+template <typename T>
+struct System : SystemBase {
+    // geometry
+    T *V = nullptr, *G = nullptr; // G: 12 planes [3k + a][Ne]
+    T *mL = nullptr, *mLm = nullptr;
+    T *Cstar = nullptr; // n_elastic x 36
+    uchar *live = nullptr, *clamp = nullptr;
+    // matrices
+    T *Kms = nullptr, *Kgs1 = nullptr, *Kgs2 = nullptr, *Mm = nullptr;
+    T *Kmech = nullptr; // tile-SoA: [ceil(nnz/32)][9][32]
+    Tiling til1, til3;
+    // CG work
+    T *r = nullptr, *p = nullptr, *Ap = nullptr, *bvec = nullptr;
+    double *partial = nullptr;
+    int grid_cap = 0;
+    CgResult *d_res = nullptr, *h_res = nullptr; // 8 slots
+    // step state (library order)
+    T *m = nullptr, *U = nullptr, *u = nullptr, *hd = nullptr, *hn = nullptr, *f = nullptr, *gn = nullptr, *gs = nullptr,
+      *ms = nullptr, *mss = nullptr, *xin = nullptr, *xout = nullptr;
+    T *sig = nullptr;                                        // N x 6 parity output of CM_OUT_SIGMA
+    T *stg_m = nullptr, *stg_U = nullptr, *stg_u = nullptr;  // device staging of the host-buffer step
+    T *escr = nullptr;     // element scratch, 12 Ne
+    double *red = nullptr; // reduction partials
+    double *dscal = nullptr, *h_scal = nullptr; // device / pinned scalars: mbar[3], gradU mean[3], dm sum, ...
+    ~System();
+};
+
+// ---- cm_mesh.cu ----
+int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long Ne, const uchar *mag, const int *eid,
+                    cm_reorder reorder);
+
+// ---- kernels (templated launchers; defined in the .cu files, instantiated for float and double) ----
+template <typename T> int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, long pin_user, cudaStream_t st);
+template <typename T> int sys_spmv(System<T> *S, cm_matrix_id id, int mode, const T *x, T *y, cudaStream_t st);
+template <typename T> int sys_cg(System<T> *S, cm_matrix_id id, int mode, const T *b, T *x, double tol, int maxiter, int fixed,
+                                 unsigned mask, int slot, int prof_cls, cudaStream_t st);
+template <typename T> int sys_get_values(const System<T> *S, cm_matrix_id id, void *host_out, long capacity);
+template <typename T> int sys_permute_in(System<T> *S, const T *user, T *lib, int ncomp, cudaStream_t st);
+template <typename T> int sys_permute_out(System<T> *S, const T *lib, T *user, int ncomp, cudaStream_t st);
+template <typename T> int sys_mbar(System<T> *S, const T *m_lib, cudaStream_t st);                         // -> dscal[0..2]
+template <typename T> int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st);                 // uses dscal[0..2]
+template <typename T> int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStream_t st);
+template <typename T> int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st);
+template <typename T> int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st);       // -> escr (V sigma per element)
+template <typename T> int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h,
+                                    T *sig_out, cudaStream_t st);                                          // gathers escr when MAGEL
+template <typename T> int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_user, cm_step_info *info,
+                                   cudaStream_t st);
+template <typename T> int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t st);

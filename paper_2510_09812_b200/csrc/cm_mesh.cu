@@ -1,0 +1,327 @@
+// S0: mesh preprocessing -- validation, locality reordering (Morton / RCM, R21),
+// relabelled + sorted connectivity, node->element CSR, sparsity pattern, lumped volume fractions.
+// Host C++ (set-up, once per mesh; not in the timed step), results uploaded to the device.
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <numeric>
+
+#include "cm_internal.h"
+
+static thread_local char g_err[512] = "";
+void cm_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+extern "C" const char *cm_last_error(void) { return g_err; }
+extern "C" const char *cm_version(void) { return "cupymag-b200 0.1 (sm_100a)"; }
+
+namespace {
+
+// Spread the low 21 bits of v so that bit b lands at position 3b.
+inline uint64_t spread3(uint64_t v)
+{
+    v &= 0x1fffffull;
+    v = (v | v << 32) & 0x1f00000000ffffull;
+    v = (v | v << 16) & 0x1f0000ff0000ffull;
+    v = (v | v << 8) & 0x100f00f00f00f00full;
+    v = (v | v << 4) & 0x10c30c30c30c30c3ull;
+    v = (v | v << 2) & 0x1249249249249249ull;
+    return v;
+}
+
+void morton_order(long N, const double *xyz, std::vector<int> &order)
+{
+    double lo[3], hi[3];
+    for (int d = 0; d < 3; d++) lo[d] = hi[d] = xyz[d];
+    for (long i = 0; i < N; i++)
+        for (int d = 0; d < 3; d++) {
+            lo[d] = std::min(lo[d], xyz[3 * i + d]);
+            hi[d] = std::max(hi[d], xyz[3 * i + d]);
+        }
+    std::vector<std::pair<uint64_t, int>> key(N);
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < N; i++) {
+        uint64_t q[3];
+        for (int d = 0; d < 3; d++) {
+            double span = hi[d] - lo[d];
+            double t = span > 0 ? (xyz[3 * i + d] - lo[d]) / span * 2097151.0 : 0.0;
+            q[d] = (uint64_t)std::floor(t);
+        }
+        key[i] = {spread3(q[0]) | spread3(q[1]) << 1 | spread3(q[2]) << 2, (int)i};
+    }
+    std::sort(key.begin(), key.end()); // (code, user index): unique keys, so equal to a stable sort by code
+    order.resize(N);
+    for (long i = 0; i < N; i++) order[i] = key[i].second;
+}
+
+void build_n2e(long N, long Ne, const int *tets, std::vector<int> &ptr, std::vector<int> &lst)
+{
+    ptr.assign(N + 1, 0);
+    lst.resize(4 * Ne);
+    for (long q = 0; q < 4 * Ne; q++) ptr[tets[q] + 1]++;
+    for (long i = 0; i < N; i++) ptr[i + 1] += ptr[i];
+    std::vector<int> fill(ptr.begin(), ptr.end() - 1);
+    for (long q = 0; q < 4 * Ne; q++) lst[fill[tets[q]]++] = (int)q; // q = 4 e + k, ascending
+}
+
+void build_pattern(long N, const int *tets, const std::vector<int> &ptr, const std::vector<int> &lst, std::vector<int> &rowptr,
+                   std::vector<int> &col)
+{
+    rowptr.assign(N + 1, 0);
+    std::vector<int> cnt(N);
+#pragma omp parallel
+    {
+        std::vector<int> tmp;
+#pragma omp for schedule(dynamic, 4096)
+        for (long i = 0; i < N; i++) {
+            tmp.clear();
+            tmp.push_back((int)i);
+            for (int s = ptr[i]; s < ptr[i + 1]; s++) {
+                const int *t = tets + 4 * (lst[s] >> 2);
+                tmp.insert(tmp.end(), t, t + 4);
+            }
+            std::sort(tmp.begin(), tmp.end());
+            cnt[i] = (int)(std::unique(tmp.begin(), tmp.end()) - tmp.begin());
+        }
+    }
+    for (long i = 0; i < N; i++) rowptr[i + 1] = rowptr[i] + cnt[i];
+    col.resize(rowptr[N]);
+#pragma omp parallel
+    {
+        std::vector<int> tmp;
+#pragma omp for schedule(dynamic, 4096)
+        for (long i = 0; i < N; i++) {
+            tmp.clear();
+            tmp.push_back((int)i);
+            for (int s = ptr[i]; s < ptr[i + 1]; s++) {
+                const int *t = tets + 4 * (lst[s] >> 2);
+                tmp.insert(tmp.end(), t, t + 4);
+            }
+            std::sort(tmp.begin(), tmp.end());
+            auto e = std::unique(tmp.begin(), tmp.end());
+            std::copy(tmp.begin(), e, col.begin() + rowptr[i]);
+        }
+    }
+}
+
+// Reverse Cuthill-McKee as specified in DESIGN.md R21.
+void rcm_order(long N, const std::vector<int> &rowptr, const std::vector<int> &col, std::vector<int> &order)
+{
+    auto deg = [&](int i) { return rowptr[i + 1] - rowptr[i] - 1; };
+    std::vector<int> bydeg(N);
+    std::iota(bydeg.begin(), bydeg.end(), 0);
+    std::sort(bydeg.begin(), bydeg.end(), [&](int a, int b) { return deg(a) != deg(b) ? deg(a) < deg(b) : a < b; });
+    std::vector<uchar> seen(N, 0);
+    std::vector<int> cm;
+    cm.reserve(N);
+    std::vector<int> nb;
+    size_t head = 0;
+    long scan = 0;
+    while ((long)cm.size() < N) {
+        while (seen[bydeg[scan]]) scan++;
+        int s = bydeg[scan];
+        seen[s] = 1;
+        cm.push_back(s);
+        while (head < cm.size()) {
+            int v = cm[head++];
+            nb.clear();
+            for (int q = rowptr[v]; q < rowptr[v + 1]; q++) {
+                int j = col[q];
+                if (j != v && !seen[j]) { seen[j] = 1; nb.push_back(j); }
+            }
+            std::sort(nb.begin(), nb.end(), [&](int a, int b) { return deg(a) != deg(b) ? deg(a) < deg(b) : a < b; });
+            cm.insert(cm.end(), nb.begin(), nb.end());
+        }
+    }
+    order.assign(cm.rbegin(), cm.rend());
+}
+
+} // namespace
+
+int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long Ne, const uchar *mag, const int *eid,
+                    cm_reorder reorder)
+{
+    M->N = N;
+    M->Ne = Ne;
+    for (long q = 0; q < 4 * Ne; q++)
+        if (tets[q] < 0 || tets[q] >= N) {
+            cm_set_error("cm_mesh_create: tet %ld references node %d outside [0, %ld)", q / 4, tets[q], N);
+            return CM_E_INDEX_RANGE;
+        }
+    // geometry validation + lumped volume fractions (fp64, metres), user order
+    double lo[3], hi[3];
+    for (int d = 0; d < 3; d++) lo[d] = hi[d] = xyz[d];
+    for (long i = 0; i < N; i++)
+        for (int d = 0; d < 3; d++) {
+            lo[d] = std::min(lo[d], xyz[3 * i + d]);
+            hi[d] = std::max(hi[d], xyz[3 * i + d]);
+        }
+    double diag = std::sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
+    double vmin = 1e-14 * diag * diag * diag, vtot = 0;
+    std::vector<double> w_user(N, 0.0);
+    for (long e = 0; e < Ne; e++) {
+        const double *x0 = xyz + 3 * (long)tets[4 * e], *x1 = xyz + 3 * (long)tets[4 * e + 1], *x2 = xyz + 3 * (long)tets[4 * e + 2],
+                     *x3 = xyz + 3 * (long)tets[4 * e + 3];
+        double a[3], b[3], c[3];
+        for (int d = 0; d < 3; d++) { a[d] = x1[d] - x0[d]; b[d] = x2[d] - x0[d]; c[d] = x3[d] - x0[d]; }
+        double det = a[0] * (b[1] * c[2] - b[2] * c[1]) + a[1] * (b[2] * c[0] - b[0] * c[2]) + a[2] * (b[0] * c[1] - b[1] * c[0]);
+        double V = std::fabs(det) / 6.0;
+        if (!(V > vmin)) {
+            cm_set_error("cm_mesh_create: tet %ld is degenerate (V = %.3e <= %.3e)", e, V, vmin);
+            return CM_E_DEGENERATE_TET;
+        }
+        vtot += V;
+        for (int k = 0; k < 4; k++) w_user[tets[4 * e + k]] += V * 0.25;
+    }
+
+    // ordering
+    std::vector<int> ptr_u, lst_u;
+    if (reorder == CM_REORDER_NONE) {
+        M->order.resize(N);
+        std::iota(M->order.begin(), M->order.end(), 0);
+    } else if (reorder == CM_REORDER_MORTON) {
+        morton_order(N, xyz, M->order);
+    } else if (reorder == CM_REORDER_RCM) {
+        std::vector<int> rp, cl;
+        build_n2e(N, Ne, tets, ptr_u, lst_u);
+        build_pattern(N, tets, ptr_u, lst_u, rp, cl);
+        rcm_order(N, rp, cl, M->order);
+    } else {
+        cm_set_error("cm_mesh_create: unknown reorder %d", (int)reorder);
+        return CM_E_BADARG;
+    }
+    M->identity = true;
+    M->iperm.resize(N);
+    for (long i = 0; i < N; i++) {
+        M->iperm[M->order[i]] = (int)i;
+        if (M->order[i] != i) M->identity = false;
+    }
+    // tets: relabel, keep local order, sort by (min new id, user tet index)
+    std::vector<std::pair<int, int>> key(Ne);
+#pragma omp parallel for schedule(static)
+    for (long e = 0; e < Ne; e++) {
+        int mn = M->iperm[tets[4 * e]];
+        for (int k = 1; k < 4; k++) mn = std::min(mn, M->iperm[tets[4 * e + k]]);
+        key[e] = {mn, (int)e};
+    }
+    std::sort(key.begin(), key.end());
+    M->tets.resize(4 * Ne);
+    M->tet_order.resize(Ne);
+    M->mag.resize(Ne);
+    M->eid.resize(Ne);
+#pragma omp parallel for schedule(static)
+    for (long e = 0; e < Ne; e++) {
+        int old = key[e].second;
+        M->tet_order[e] = old;
+        for (int k = 0; k < 4; k++) M->tets[4 * e + k] = M->iperm[tets[4 * old + k]];
+        M->mag[e] = mag ? (mag[old] != 0) : 1;
+        M->eid[e] = eid ? eid[old] : 0;
+    }
+    M->xyz.resize(3 * N);
+    M->wvol.resize(N);
+    for (long i = 0; i < N; i++) {
+        for (int d = 0; d < 3; d++) M->xyz[3 * i + d] = xyz[3 * (long)M->order[i] + d];
+        M->wvol[i] = w_user[M->order[i]] / vtot;
+    }
+    build_n2e(N, Ne, M->tets.data(), M->n2e_ptr, M->n2e);
+    build_pattern(N, M->tets.data(), M->n2e_ptr, M->n2e, M->rowptr, M->col);
+    M->nnz = M->rowptr[N];
+    return CM_OK;
+}
+
+template <typename U>
+static int upload(U **dst, const std::vector<U> &src, cudaStream_t st)
+{
+    CM_CUDA(cudaMalloc((void **)dst, std::max<size_t>(src.size(), 1) * sizeof(U) + 64));
+    CM_CUDA(cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(U), cudaMemcpyHostToDevice, st));
+    return CM_OK;
+}
+
+extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
+                              const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out)
+{
+    if (!xyz || !tets || !out || n_nodes <= 0 || n_tets <= 0 || n_nodes > 0x7fffffffL / 4 || n_tets > 0x7fffffffL / 16) {
+        cm_set_error("cm_mesh_create: bad argument");
+        return CM_E_BADARG;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cm_set_error("cm_mesh_create: no CUDA device (this library has no CPU fallback)");
+        return CM_E_CUDA;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cm_mesh *M = new (std::nothrow) cm_mesh();
+    if (!M) return CM_E_ALLOC;
+    int rc;
+    try {
+        rc = mesh_build_host(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, reorder);
+    } catch (const std::bad_alloc &) {
+        cm_set_error("cm_mesh_create: out of host memory");
+        rc = CM_E_ALLOC;
+    }
+    if (rc == CM_OK) {
+        auto up = [&]() -> int {
+            CM_TRY(upload(&M->d_order, M->order, st));
+            CM_TRY(upload(&M->d_tets, M->tets, st));
+            CM_TRY(upload(&M->d_rowptr, M->rowptr, st));
+            CM_TRY(upload(&M->d_col, M->col, st));
+            CM_TRY(upload(&M->d_n2e_ptr, M->n2e_ptr, st));
+            CM_TRY(upload(&M->d_n2e, M->n2e, st));
+            CM_TRY(upload(&M->d_eid, M->eid, st));
+            CM_TRY(upload(&M->d_mag, M->mag, st));
+            CM_TRY(upload(&M->d_xyz, M->xyz, st));
+            CM_TRY(upload(&M->d_wvol, M->wvol, st));
+            CM_CUDA(cudaMalloc((void **)&M->d_red, 4096 * 16 * sizeof(double)));
+            CM_CUDA(cudaMallocHost((void **)&M->h_red, 16 * sizeof(double)));
+            CM_CUDA(cudaStreamSynchronize(st));
+            return CM_OK;
+        };
+        rc = up();
+    }
+    if (rc != CM_OK) {
+        cm_mesh_destroy(M);
+        return rc;
+    }
+    *out = M;
+    return CM_OK;
+}
+
+extern "C" int cm_mesh_destroy(cm_mesh *M)
+{
+    if (!M) return CM_OK;
+    cudaFree(M->d_order); cudaFree(M->d_tets); cudaFree(M->d_rowptr); cudaFree(M->d_col); cudaFree(M->d_n2e_ptr);
+    cudaFree(M->d_n2e); cudaFree(M->d_eid); cudaFree(M->d_mag); cudaFree(M->d_xyz); cudaFree(M->d_wvol);
+    cudaFree(M->d_red); cudaFree(M->d_tmp);
+    if (M->h_red) cudaFreeHost(M->h_red);
+    delete M;
+    return CM_OK;
+}
+
+extern "C" int cm_mesh_get(const cm_mesh *M, int what, void *host_out, long capacity)
+{
+    if (!M || !host_out) { cm_set_error("cm_mesh_get: null argument"); return CM_E_BADARG; }
+    const std::vector<int> *v = nullptr;
+    switch (what) {
+    case CM_GET_COUNTS:
+        if (capacity < 3) { cm_set_error("cm_mesh_get: capacity"); return CM_E_BADARG; }
+        ((long *)host_out)[0] = M->N; ((long *)host_out)[1] = M->Ne; ((long *)host_out)[2] = M->nnz;
+        return CM_OK;
+    case CM_GET_ORDER: v = &M->order; break;
+    case CM_GET_IPERM: v = &M->iperm; break;
+    case CM_GET_TETS: v = &M->tets; break;
+    case CM_GET_TET_ORDER: v = &M->tet_order; break;
+    case CM_GET_ROWPTR: v = &M->rowptr; break;
+    case CM_GET_COLIDX: v = &M->col; break;
+    case CM_GET_N2E_PTR: v = &M->n2e_ptr; break;
+    case CM_GET_N2E: v = &M->n2e; break;
+    default: cm_set_error("cm_mesh_get: unknown what=%d", what); return CM_E_BADARG;
+    }
+    if (capacity < (long)v->size()) { cm_set_error("cm_mesh_get: capacity %ld < %zu", capacity, v->size()); return CM_E_BADARG; }
+    std::memcpy(host_out, v->data(), v->size() * sizeof(int));
+    return CM_OK;
+}

@@ -1,0 +1,423 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: bit-exact structure; <= 1e-12 (fp64) / 1e-5 (fp32) relative on
+matrix values, SpMV and right-hand sides; CG iteration counts within +-1; max |dm| <= 1e-9 (fp64) / 1e-4 (fp32)
+after 10 GSPM steps.  Relative = max-norm of the difference over max-norm of the oracle's result."""
+import numpy as np
+import pytest
+
+from paper_2510_09812_b200 import inputs
+from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD, TERM_MAGEL, TERM_ZEEMAN
+
+pytestmark = pytest.mark.gpu
+
+NM = 1e-9
+TOL = {"f64": 1e-12, "f32": 1e-5}
+ALL = TERM_ANIS | TERM_ZEEMAN | TERM_DEMAG | TERM_FARFIELD | TERM_MAGEL
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def cm():
+    from paper_2510_09812_b200 import binding
+    binding.lib()
+    return binding
+
+
+def rel(a, b):
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
+
+
+def mat2():
+    C = inputs.isotropic_voigt(200e9, 0.3)
+    return inputs.Material(C_voigt=np.stack([C, 2 * C]))
+
+
+def medium_mesh():
+    """7429 nodes / 38k tets / ~105k nnz: ~70 scalar tiles, ~140 block tiles, ragged tail; spherical inclusion."""
+    mesh = inputs.kuhn_box((23, 19, 17), (66 * NM, 54 * NM, 48 * NM), seed_mesh=51, seed_perm=52)
+    return inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (14 * NM, 12 * NM, 10 * NM))
+
+
+class Case:
+    def __init__(self, cm, orc, torch, mesh, mat, dt, dtype, reorder, clamp=None, pin=0):
+        self.mesh, self.mat, self.dt, self.dtype = mesh, mat, dt, dtype
+        self.gm = cm.Mesh(mesh.xyz, mesh.tets, mesh.magnetic, mesh.elastic_id, reorder)
+        self.gs = cm.System(self.gm, mat, dt, dtype, clamp, pin)
+        self.o = orc.Oracle(mesh, mat, dt, clamp_dof=clamp, pin_node=pin, dtype="f64")
+        self.torch = torch
+        self.td = torch.float64 if dtype == "f64" else torch.float32
+
+    def dev(self, a):
+        return self.torch.as_tensor(np.ascontiguousarray(a), dtype=self.td, device="cuda")
+
+
+@pytest.fixture(scope="module", params=["f64", "f32"])
+def case(request, cm, oracle_mod, torch):
+    mesh = medium_mesh()
+    return Case(cm, oracle_mod, torch, mesh, mat2(), 2e-12, request.param, cm.CM_REORDER_MORTON, clamp=inputs.clamp_bottom(mesh), pin=5)
+
+
+# ---------------------------------------------------------------------------------------------- structure
+@pytest.mark.parametrize("reorder", [0, 1, 2])
+def test_structure_bit_exact(cm, oracle_mod, torch, reorder):
+    mesh = inputs.kuhn_box((9, 8, 7), (20 * NM, 18 * NM, 15 * NM), seed_mesh=61, seed_perm=62)
+    gm = cm.Mesh(mesh.xyz, mesh.tets, reorder=reorder)
+    order, iperm, tnew, torder = oracle_mod.reorder(mesh.xyz, mesh.tets, reorder)
+    assert np.array_equal(gm.get(cm.CM_GET_ORDER), order)
+    assert np.array_equal(gm.get(cm.CM_GET_IPERM), iperm)
+    assert np.array_equal(gm.get(cm.CM_GET_TETS), tnew)
+    assert np.array_equal(gm.get(cm.CM_GET_TET_ORDER), torder)
+    # pattern and node->element lists of the relabelled mesh
+    relab = inputs.replace(mesh, xyz=mesh.xyz[order], tets=tnew)
+    o = oracle_mod.Oracle(relab, inputs.Material(), 1e-12)
+    assert gm.nnz == o.nnz
+    assert np.array_equal(gm.get(cm.CM_GET_ROWPTR), o.rowptr())
+    assert np.array_equal(gm.get(cm.CM_GET_COLIDX), o.colidx())
+    assert np.array_equal(gm.get(cm.CM_GET_N2E_PTR), o.n2e_ptr())
+    assert np.array_equal(gm.get(cm.CM_GET_N2E), o.n2e())
+
+
+def test_errors(cm, torch):
+    mesh = inputs.kuhn_box((4, 4, 4), (9 * NM,) * 3)
+    bad = mesh.tets.copy(); bad[0, 1] = bad[0, 0]
+    with pytest.raises(cm.CmError) as e:
+        cm.Mesh(mesh.xyz, bad)
+    assert e.value.code == cm.CM_E_DEGENERATE_TET
+    bad = mesh.tets.copy(); bad[3, 2] = mesh.n_nodes
+    with pytest.raises(cm.CmError) as e:
+        cm.Mesh(mesh.xyz, bad)
+    assert e.value.code == cm.CM_E_INDEX_RANGE
+    gm = cm.Mesh(mesh.xyz, mesh.tets)
+    with pytest.raises(cm.CmError) as e:
+        cm.System(gm, inputs.Material(), 1e-12, pin_node=mesh.n_nodes)
+    assert e.value.code == cm.CM_E_BADARG
+    gs = cm.System(gm, inputs.Material(), 1e-12)
+    m = torch.zeros((mesh.n_nodes, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(cm.CmError) as e:          # dt mismatch
+        gs.gspm_step(cm.make_params(2e-12, terms=TERM_ANIS), m, None, None)
+    assert e.value.code == cm.CM_E_BADARG
+    with pytest.raises(cm.CmError):               # DEMAG without U
+        gs.gspm_step(cm.make_params(1e-12, terms=TERM_DEMAG), m, None, None)
+
+
+# ---------------------------------------------------------------------------------------------- geometry, matrices
+def _to_user(case, vals_lib, block):
+    """library-order CSR/BSR values -> scipy matrix in user order"""
+    import scipy.sparse as sp
+    gm = case.gm
+    rp, ci = gm.get(5), gm.get(6)
+    iperm = gm.get(2)
+    N = gm.n_nodes
+    if not block:
+        A = sp.csr_matrix((vals_lib.astype(np.float64), ci, rp), shape=(N, N))
+        return A[iperm][:, iperm].tocsr()
+    A = sp.bsr_matrix((vals_lib.astype(np.float64), ci, rp), shape=(3 * N, 3 * N)).tocsr()
+    idx = (3 * iperm[:, None] + np.arange(3)[None, :]).ravel()
+    return A[idx][:, idx].tocsr()
+
+
+def test_geometry_and_matrices(case, cm, oracle_mod):
+    o, gs, gm = case.o, case.gs, case.gm
+    tol = TOL[case.dtype] if case.dtype == "f64" else 2e-7      # fp32: one rounding of an fp64 set-up value
+    torder, order = gm.get(cm.CM_GET_TET_ORDER), gm.get(cm.CM_GET_ORDER)
+    assert rel(gs.geometry(0), o.V()[torder]) < tol
+    assert rel(gs.geometry(1), o.G()[torder]) < tol
+    assert rel(gs.geometry(2), o.mL()[order]) < tol
+    assert rel(gs.geometry(3), o.mLm()[order]) < tol
+    for mat_g, mat_o in ((cm.CM_MAT_K_MS, oracle_mod.MAT_K_MS), (cm.CM_MAT_K_GS1, oracle_mod.MAT_K_GS1),
+                         (cm.CM_MAT_K_GS2, oracle_mod.MAT_K_GS2), (cm.CM_MAT_MASS, oracle_mod.MAT_MASS),
+                         (cm.CM_MAT_K_MECH, oracle_mod.MAT_K_MECH)):
+        A = _to_user(case, gs.values(mat_g), mat_g == cm.CM_MAT_K_MECH)
+        B = o.csr(mat_o)
+        assert abs(A - B).max() < tol * abs(B).max(), mat_g
+
+
+# ---------------------------------------------------------------------------------------------- SpMV
+def test_spmv(case, cm, oracle_mod):
+    rng = np.random.default_rng(7)
+    N = case.o.N
+    for mat_g, mat_o in ((cm.CM_MAT_K_MS, oracle_mod.MAT_K_MS), (cm.CM_MAT_K_GS1, oracle_mod.MAT_K_GS1),
+                         (cm.CM_MAT_MASS, oracle_mod.MAT_MASS)):
+        x = rng.normal(size=N).astype(case.gs.np_dtype)
+        y = case.gs.spmv(mat_g, case.dev(x)).cpu().numpy()
+        assert rel(y, case.o.spmv(mat_o, x.astype(np.float64))) < TOL[case.dtype]
+    x = rng.normal(size=(N, 3)).astype(case.gs.np_dtype)
+    y = case.gs.spmv(cm.CM_MAT_K_MECH, case.dev(x)).cpu().numpy()
+    assert rel(y.ravel(), case.o.spmv(oracle_mod.MAT_K_MECH, x.astype(np.float64).ravel())) < TOL[case.dtype]
+    y3 = case.gs.spmv3(cm.CM_MAT_MASS, case.dev(x)).cpu().numpy()
+    assert rel(y3, case.o.rhs_gs(x.astype(np.float64))) < TOL[case.dtype]
+
+
+# ---------------------------------------------------------------------------------------------- RHS, fields
+def test_rhs_and_fields(case, cm, oracle_mod):
+    o, gs = case.o, case.gs
+    tol = TOL[case.dtype]
+    rng = np.random.default_rng(8)
+    m = inputs.init_m_random(case.mesh, 9).astype(gs.np_dtype)
+    U = rng.normal(size=o.N).astype(gs.np_dtype)
+    u = (1e-3 * rng.normal(size=(o.N, 3))).astype(gs.np_dtype)
+    m64, U64, u64 = m.astype(np.float64), U.astype(np.float64), u.astype(np.float64)
+    md, Ud, ud = case.dev(m), case.dev(U), case.dev(u)
+    Hext = np.array([3e4, -1e4, 2e4])
+    p = cm.make_params(case.dt, Hext, ALL)
+    # volume average (S2)
+    mbar = case.gm.volume_average(md)
+    assert np.abs(mbar - o.volume_average(m64)).max() < (1e-13 if case.dtype == "f64" else 1e-7)
+    # S3
+    assert rel(gs.field_rhs(cm.CM_RHS_MS, md).cpu().numpy(), o.rhs_ms(m64)) < tol
+    # S6
+    assert rel(gs.field_rhs(cm.CM_RHS_MECH, md).cpu().numpy(), o.rhs_mech(m64)) < tol
+    # S5
+    hd_o, _ = o.demag_field(U64, o.volume_average(m64), TERM_DEMAG | TERM_FARFIELD)
+    hd = gs.field_rhs(cm.CM_OUT_HD, md, Ud, None, p).cpu().numpy()
+    assert rel(hd, hd_o) < tol
+    # S8
+    sig_o = o.stress_recover(u64, m64)
+    sig = gs.field_rhs(cm.CM_OUT_SIGMA, md, None, ud, p).cpu().numpy()
+    assert rel(sig, sig_o) < tol
+    # S9 field and Helmholtz RHS
+    h_o = o.field(m64, hd_o, sig_o, Hext / case.mat.Ms, ALL)
+    h = gs.field_rhs(cm.CM_OUT_FIELD, md, Ud, ud, p).cpu().numpy()
+    assert rel(h, h_o) < tol
+    b_o = o.rhs_gs(m64 + 0.37 * h_o)
+    b = gs.field_rhs(cm.CM_RHS_GS, md, Ud, ud, p, coeff=0.37).cpu().numpy()
+    assert rel(b, b_o) < tol
+    # term subsets: anisotropy + Zeeman only (config 1), demag without far field
+    for terms in (TERM_ANIS | TERM_ZEEMAN, TERM_DEMAG, TERM_FARFIELD | TERM_MAGEL):
+        pp = cm.make_params(case.dt, Hext, terms)
+        hd_t, _ = o.demag_field(U64, o.volume_average(m64), terms)
+        h_t = o.field(m64, hd_t, sig_o, Hext / case.mat.Ms, terms)
+        assert rel(gs.field_rhs(cm.CM_OUT_FIELD, md, Ud, ud, pp).cpu().numpy(), h_t) < tol
+
+
+# ---------------------------------------------------------------------------------------------- CG
+def test_cg(case, cm, oracle_mod):
+    o, gs = case.o, case.gs
+    rng = np.random.default_rng(10)
+    f64 = case.dtype == "f64"
+    tol_cg = 1e-10 if f64 else 1e-5
+    xtol = 1e-7 if f64 else 2e-3
+    for mat_g, mat_o, n in ((cm.CM_MAT_K_MS, oracle_mod.MAT_K_MS, o.N), (cm.CM_MAT_K_GS1, oracle_mod.MAT_K_GS1, o.N),
+                            (cm.CM_MAT_K_MECH, oracle_mod.MAT_K_MECH, 3 * o.N)):
+        b = rng.normal(size=n).astype(gs.np_dtype)
+        if mat_g == cm.CM_MAT_K_MS:
+            b[5] = 0
+        if mat_g == cm.CM_MAT_K_MECH:
+            b[inputs.clamp_bottom(case.mesh).astype(bool)] = 0
+        shape = (o.N, 3) if mat_g == cm.CM_MAT_K_MECH else (o.N,)
+        x = case.torch.zeros(shape, dtype=case.td, device="cuda")
+        it, res, rc = gs.cg_solve(mat_g, case.dev(b.reshape(shape)), x, tol=tol_cg)
+        oo = o if f64 else oracle_mod.Oracle(case.mesh, case.mat, case.dt, clamp_dof=inputs.clamp_bottom(case.mesh), pin_node=5, dtype="f32")
+        xo, ito, reso, rco = oo.cg(mat_o, b, tol=tol_cg)
+        assert rc == 0 and rco == 0
+        assert abs(it - ito) <= (1 if f64 else max(2, ito // 50)), (mat_g, it, ito)
+        assert res < tol_cg
+        x64, _, _, _ = o.cg(mat_o, b.astype(np.float64), tol=1e-13)
+        assert rel(x.cpu().numpy().ravel(), x64) < xtol, mat_g
+        # fixed iteration count: identical algorithm step by step
+        x = case.torch.zeros(shape, dtype=case.td, device="cuda")
+        it, res, rc = gs.cg_solve(mat_g, case.dev(b.reshape(shape)), x, fixed_iters=3)
+        x3, it3, res3, _ = o.cg(mat_o, b.astype(np.float64), fixed=3)
+        assert it == 3 and it3 == 3
+        assert rel(x.cpu().numpy().ravel(), x3) < (1e-11 if f64 else 1e-4)
+        assert res == pytest.approx(res3, rel=1e-9 if f64 else 1e-3)
+    # zero RHS -> x = 0, 0 iterations; warm start at the solution -> 0 iterations
+    x = case.dev(rng.normal(size=o.N))
+    it, res, rc = gs.cg_solve(cm.CM_MAT_K_GS1, case.torch.zeros(o.N, dtype=case.td, device="cuda"), x)
+    assert it == 0 and float(x.abs().max()) == 0.0
+    # maxiter -> warning code, iterate still written
+    b = rng.normal(size=o.N).astype(gs.np_dtype); b[5] = 0
+    x = case.torch.zeros(o.N, dtype=case.td, device="cuda")
+    it, res, rc = gs.cg_solve(cm.CM_MAT_K_MS, case.dev(b), x, tol=1e-12, maxiter=4)
+    assert it == 4 and rc == cm.CM_E_CG_MAXITER and float(x.abs().max()) > 0
+
+
+def test_cg3_independent_systems(case, cm, oracle_mod):
+    o, gs = case.o, case.gs
+    rng = np.random.default_rng(11)
+    f64 = case.dtype == "f64"
+    b = rng.normal(size=(o.N, 3)).astype(gs.np_dtype)
+    b[:, 1] *= 1e-3
+    b[:, 2] = 0                                  # third system: zero rhs -> 0 iterations, x = 0
+    x0 = rng.normal(size=(o.N, 3)).astype(gs.np_dtype)
+    x = case.dev(x0)
+    tol_cg = 1e-11 if f64 else 1e-5
+    its, ress, rc = gs.cg_solve3(cm.CM_MAT_K_GS2, case.dev(b), x, tol=tol_cg)
+    xh = x.cpu().numpy()
+    for c in range(3):
+        xo, ito, reso, rco = o.cg(oracle_mod.MAT_K_GS2, b[:, c].astype(np.float64), x0=x0[:, c].astype(np.float64), tol=tol_cg)
+        assert abs(its[c] - ito) <= 1, (c, its, ito)
+        if c < 2:
+            assert rel(xh[:, c], xo) < (1e-9 if f64 else 1e-3)
+    assert its[2] == 0 and np.abs(xh[:, 2]).max() == 0
+
+
+# ---------------------------------------------------------------------------------------------- GSPM steps
+def _run_steps(cm, orc, torch, mesh, mat, dt, terms, nsteps, dtype, Hext, clamp=None, variant=0, reorder=1, cg_tol=1e-12,
+               fixed=-1, m0=None, host=False):
+    gm = cm.Mesh(mesh.xyz, mesh.tets, mesh.magnetic, mesh.elastic_id, reorder)
+    gs = cm.System(gm, mat, dt, dtype, clamp)
+    o = orc.Oracle(mesh, mat, dt, clamp_dof=clamp, dtype="f64")
+    td = torch.float64 if dtype == "f64" else torch.float32
+    N = mesh.n_nodes
+    m = m0.copy()
+    U = np.zeros(N); u = np.zeros((N, 3))
+    if host:
+        mg = m0.astype(gs.np_dtype).copy(); Ug = np.zeros(N, gs.np_dtype); ug = np.zeros((N, 3), gs.np_dtype)
+    else:
+        mg = torch.as_tensor(m0, dtype=td, device="cuda").contiguous()
+        Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+    infos = []
+    for k in range(nsteps):
+        p = cm.make_params(dt, Hext[k], terms, variant, cg_tol, 100000, fixed)
+        io, rco = o.gspm_step(m, U, u, dt, Hext[k], terms, variant=variant, cg_tol=cg_tol, cg_fixed_iters=fixed)
+        ig, rcg = (gs.gspm_step_host(p, mg, Ug, ug) if host else gs.gspm_step(p, mg, Ug, ug))
+        assert rco == 0 and rcg == 0
+        infos.append((io, ig))
+    mgh = mg if host else mg.cpu().numpy()
+    Ugh = Ug if host else Ug.cpu().numpy()
+    ugh = ug if host else ug.cpu().numpy()
+    return m, U, u, mgh, Ugh, ugh, infos, o
+
+
+def _check_iters(infos, slack=1):
+    for io, ig in infos:
+        assert abs(io.it_ms - ig.it_ms) <= slack
+        assert abs(io.it_mech - ig.it_mech) <= slack
+        for a in range(8):
+            assert abs(io.it_gs[a] - ig.it_gs[a]) <= slack, (a, list(io.it_gs), list(ig.it_gs))
+
+
+@pytest.mark.parametrize("reorder", [0, 1, 2])
+def test_gspm_config0_10_steps_f64(cm, oracle_mod, torch, reorder):
+    cfg = inputs.make_config(0)
+    m, U, u, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, cfg.mesh, cfg.material, cfg.dt, cfg.terms, 10, "f64",
+                                               cfg.Hext, reorder=reorder)
+    assert np.abs(mg - m).max() <= 1e-9
+    assert np.abs(Ug - U).max() <= 1e-9 * max(1.0, np.abs(U).max())
+    assert np.abs(np.linalg.norm(mg, axis=1) - 1).max() <= 4 * np.finfo(float).eps
+    _check_iters(infos)
+    for io, ig in infos:
+        assert np.allclose(ig.mbar[:], io.mbar[:], atol=1e-11)
+        assert ig.mean_dm == pytest.approx(io.mean_dm, abs=1e-10)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_gspm_magnetoelastic_inclusion_f64(cm, oracle_mod, torch, variant):
+    """Reduced instance of config 2: all terms, spherical non-magnetic inclusion with x2 stiffness, clamped bottom."""
+    mesh = inputs.kuhn_box((13, 13, 7), (40 * NM, 40 * NM, 20 * NM), seed_mesh=21, seed_perm=22)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * NM,) * 3)
+    m0 = inputs.init_m_noisy_x(mesh, 23)
+    H = np.tile([2e4, 0, 0], (10, 1))
+    m, U, u, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 10, "f64", H,
+                                               clamp=inputs.clamp_bottom(mesh), variant=variant)
+    assert np.abs(mg - m).max() <= 1e-9
+    assert np.abs(ug - u).max() <= 1e-9 * max(1.0, np.abs(u).max())
+    live = o.live().astype(bool)
+    assert np.abs(mg[~live]).max() == 0
+    _check_iters(infos)
+    assert infos[0][1].it_mech > 10 and infos[0][1].it_ms > 10
+
+
+def test_gspm_host_buffers_and_config1_terms(cm, oracle_mod, torch):
+    """Reduced instance of config 1 (anisotropy + Zeeman, -50 mT) through the HOST-buffer entry point."""
+    cfg = inputs.make_config(1, grid=(21, 21, 7))
+    m, U, u, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, cfg.mesh, cfg.material, cfg.dt, cfg.terms, 10, "f64",
+                                               cfg.Hext, host=True)
+    assert np.abs(mg - m).max() <= 1e-9
+    _check_iters(infos)
+
+
+def test_gspm_f32_10_steps(cm, oracle_mod, torch):
+    """fp32 build against the fp64 oracle: max |dm| <= 1e-4 after 10 steps (fixed CG counts taken from
+    an fp64-oracle run at tol 1e-5 would differ per solve; here both sides iterate to tol 1e-6)."""
+    cfg = inputs.make_config(0)
+    m, U, u, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, cfg.mesh, cfg.material, cfg.dt, cfg.terms, 10, "f32",
+                                               cfg.Hext, cg_tol=1e-6)
+    assert np.abs(mg - m).max() <= 1e-4
+    assert np.abs(np.linalg.norm(mg, axis=1) - 1).max() <= 4 * np.finfo(np.float32).eps
+    _check_iters(infos, slack=3)
+
+
+def test_gspm_fixed_iterations(cm, oracle_mod, torch):
+    """cg_fixed_iters = 3 (the throughput variant of SURVEY 8d): identical arithmetic, no stopping test."""
+    cfg = inputs.make_config(0)
+    m, U, u, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, cfg.mesh, cfg.material, cfg.dt, cfg.terms, 5, "f64",
+                                               cfg.Hext, fixed=3)
+    assert np.abs(mg - m).max() <= 1e-11
+    for io, ig in infos:
+        assert ig.it_ms == 3 and list(ig.it_gs) == [3] * 8
+
+
+# ---------------------------------------------------------------------------------------------- edge cases
+def test_single_tet_and_tiny_meshes(cm, oracle_mod, torch):
+    xyz = np.array([[0, 0, 0], [2, 0, 0], [0, 3, 0], [0, 0, 1.5]]) * NM
+    tets = np.array([[0, 1, 2, 3]], np.int32)
+    mesh = inputs.Mesh(xyz, tets, np.ones(1, np.uint8), np.zeros(1, np.int32), (2, 2, 2), (2 * NM, 3 * NM, 1.5 * NM), np.arange(4))
+    m0 = inputs.init_m_random(mesh, 1)
+    H = np.zeros((3, 3))
+    m, U, u, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, mesh, inputs.Material(), 1e-12,
+                                               TERM_ANIS | TERM_DEMAG | TERM_FARFIELD, 3, "f64", H)
+    assert np.abs(mg - m).max() <= 1e-12
+
+
+def hub_mesh(nlat=42, nlon=48):
+    """One hub node at the centre of a triangulated sphere: its row has ~2000 nonzeros (> one tile)."""
+    th = np.linspace(0.05, np.pi - 0.05, nlat)
+    ph = np.linspace(0, 2 * np.pi, nlon, endpoint=False)
+    T, P = np.meshgrid(th, ph, indexing="ij")
+    r = 10 * NM
+    pts = np.stack([r * np.sin(T) * np.cos(P), r * np.sin(T) * np.sin(P), r * np.cos(T)], axis=-1).reshape(-1, 3)
+    xyz = np.vstack([np.zeros((1, 3)), pts])
+    tets = []
+    idx = lambda i, j: 1 + i * nlon + (j % nlon)
+    for i in range(nlat - 1):
+        for j in range(nlon):
+            tets.append([0, idx(i, j), idx(i + 1, j), idx(i, j + 1)])
+            tets.append([0, idx(i + 1, j), idx(i + 1, j + 1), idx(i, j + 1)])
+    tets = np.array(tets, np.int32)
+    n = xyz.shape[0]
+    return inputs.Mesh(xyz, tets, np.ones(len(tets), np.uint8), np.zeros(len(tets), np.int32), (0, 0, 0), (0, 0, 0), np.arange(n))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_row_longer_than_a_tile(cm, oracle_mod, torch, dtype):
+    mesh = hub_mesh()
+    assert mesh.n_nodes - 1 > 1536                     # the hub row exceeds both tile sizes
+    c = Case(cm, oracle_mod, torch, mesh, inputs.Material(), 1e-12, dtype, cm.CM_REORDER_MORTON, pin=3)
+    rng = np.random.default_rng(12)
+    x = rng.normal(size=mesh.n_nodes).astype(c.gs.np_dtype)
+    y = c.gs.spmv(cm.CM_MAT_K_GS1, c.dev(x)).cpu().numpy()
+    assert rel(y, c.o.spmv(oracle_mod.MAT_K_GS1, x.astype(np.float64))) < TOL[dtype] * 10
+    x3 = rng.normal(size=(mesh.n_nodes, 3)).astype(c.gs.np_dtype)
+    assert rel(c.gs.spmv3(cm.CM_MAT_MASS, c.dev(x3)).cpu().numpy(), c.o.rhs_gs(x3.astype(np.float64))) < TOL[dtype] * 10
+    y = c.gs.spmv(cm.CM_MAT_K_MECH, c.dev(x3)).cpu().numpy()
+    assert rel(y.ravel(), c.o.spmv(oracle_mod.MAT_K_MECH, x3.astype(np.float64).ravel())) < TOL[dtype] * 10
+    b = rng.normal(size=mesh.n_nodes).astype(c.gs.np_dtype)
+    xg = torch.zeros(mesh.n_nodes, dtype=c.td, device="cuda")
+    it, res, rc = c.gs.cg_solve(cm.CM_MAT_K_GS1, c.dev(b), xg, tol=1e-10 if dtype == "f64" else 1e-5)
+    xo, ito, _, _ = c.o.cg(oracle_mod.MAT_K_GS1, b.astype(np.float64), tol=1e-10 if dtype == "f64" else 1e-5)
+    assert rc == 0 and abs(it - ito) <= 2
+    assert rel(xg.cpu().numpy(), xo) < (1e-8 if dtype == "f64" else 1e-3)
+
+
+def test_profile_counters(case, cm):
+    gs = case.gs
+    gs.profile_enable(True)
+    gs.profile_reset()
+    x = case.torch.ones(case.o.N, dtype=case.td, device="cuda")
+    b = gs.spmv(cm.CM_MAT_K_GS1, x)
+    xs = case.torch.zeros_like(x)
+    it, _, _ = gs.cg_solve(cm.CM_MAT_K_GS1, b, xs, tol=1e-6)
+    prof = gs.profile()
+    assert prof["spmv"]["launches"] == 1 and prof["spmv"]["ms"] > 0
+    assert prof["cg_gs"]["launches"] == 1 and prof["cg_gs"]["cg_iters"] == it and prof["cg_gs"]["ms"] > 0
+    gs.profile_enable(False)
