@@ -1,0 +1,289 @@
+#!/usr/bin/env python
+"""bench.py -- GSPM time steps/s at the 3M-node mesh (BASELINE.json config 3), one replica per GPU.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--impl ours|reference]
+
+A "step" is one cm_gspm_step: the whole hot path (volume average, magnetostatic RHS + CG, gradient recovery,
+mechanical RHS + CG, stress recovery, field, 8 Helmholtz CG solves, Gauss-Seidel update, projection) on the
+synthetic 245x245x50-node magnetoelastic mesh with an ellipsoidal inclusion, fp64, CG tolerance 1e-7,
+field sweep of config 3.  The path does not shard ("replicas only"): with N > 1 every rank steps its own
+replica, no collective on the data path; value = replicas * steps / max-over-ranks time.
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2510_09812_b200 import inputs  # noqa: E402
+
+NM = 1e-9
+METRIC = "gspm_time_steps_per_s_3M_nodes"
+UNIT = "steps/s"
+CG_TOL = 1e-7           # the paper's CG tolerance
+FULL_GRID = (245, 245, 50)
+SAMPLE_GRID, SAMPLE_BOX = (62, 62, 50), (250 * NM, 250 * NM, 200 * NM)   # same spacing, 1/16 of the area
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.stop = index, [], threading.Event()
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 2 + k and r[2 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def sample_config():
+    return inputs.make_config(3, grid=SAMPLE_GRID, box=SAMPLE_BOX)
+
+
+def time_oracle(steps: int, warmup: int):
+    """The oracle as it stands, on the box's host cores, on the bounded sample.  Returns (steps/s scaled to the
+    3M-node mesh by node count, description, threads)."""
+    import oracle
+    cfg = sample_config()
+    o = oracle.Oracle(cfg.mesh, cfg.material, cfg.dt, clamp_dof=cfg.clamp_dof)
+    m = cfg.m0.copy(); U = np.zeros(o.N); u = np.zeros((o.N, 3))
+    its = []
+    t0 = None
+    for k in range(warmup + steps):
+        if k == warmup:
+            t0 = time.perf_counter()
+        info, rc = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, cg_tol=CG_TOL)
+        its.append((info.it_ms, info.it_mech, sum(info.it_gs)))
+    dt = time.perf_counter() - t0
+    n_full = FULL_GRID[0] * FULL_GRID[1] * FULL_GRID[2]
+    scale = o.N / n_full
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    desc = (f"{steps} GSPM step(s) of config 3 on a {SAMPLE_GRID[0]}x{SAMPLE_GRID[1]}x{SAMPLE_GRID[2]}-node sub-box "
+            f"({o.N} nodes, same spacing/physics/tol {CG_TOL:g}); steps/s multiplied by {o.N}/{n_full} (node count); "
+            f"CG its (ms, mech, sum gs) last step {its[-1]}")
+    return steps / dt * scale, dt / steps, desc, cores
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    value, sec_per_step, desc, cores = time_oracle(args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config3_paper_scale (bounded CPU sample)", "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def algorithmic_bytes(N, nnz, s):
+    """SURVEY 8(d) per-unit figures (x-vector gathers counted once), s = bytes per value."""
+    spmv_csr = nnz * (s + 4) + N * (4 + s + s)
+    spmv_bsr = nnz * (9 * s + 4) + N * (4 + 3 * s + 3 * s)
+    return {
+        "cg_iter_csr1": spmv_csr + 10 * N * s,                  # SpMV + ~10 vector words (SURVEY: 277 B/row fp64)
+        "cg_iter_bsr3": spmv_bsr + 10 * 3 * N * s,              # SURVEY: 1415 B/node fp64
+        "cg_iter_csr3": nnz * (s + 4) + N * 4 + 2 * 3 * N * s + 10 * 3 * N * s,   # 3-RHS: matrix read once per iteration
+        "spmv_csr3": nnz * (s + 4) + N * 4 + 2 * 3 * N * s,
+    }
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2510_09812_b200 import binding as cm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    dtype = args.dtype
+    td = torch.float64 if dtype == "f64" else torch.float32
+    s = 8 if dtype == "f64" else 4
+
+    grid = tuple(int(g) for g in args.grid.split("x")) if args.grid else None
+    cfg = inputs.make_config(3, grid=grid)
+    t_setup = time.perf_counter()
+    mesh = cm.Mesh(cfg.mesh.xyz, cfg.mesh.tets, cfg.mesh.magnetic, cfg.mesh.elastic_id, cm.CM_REORDER_MORTON)
+    sysm = cm.System(mesh, cfg.material, cfg.dt, dtype, cfg.clamp_dof, cfg.pin_node)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t_setup
+    N, nnz = mesh.n_nodes, mesh.nnz
+
+    m = torch.as_tensor(cfg.m0, dtype=td, device=dev).contiguous()
+    U = torch.zeros(N, dtype=td, device=dev)
+    u = torch.zeros((N, 3), dtype=td, device=dev)
+
+    def params(k):
+        return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, 0, CG_TOL, 100000, args.fixed_iters)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    k = 0
+    for _ in range(args.warmup):
+        sysm.gspm_step(params(k), m, U, u); k += 1
+    sysm.profile_enable(True)
+    sysm.profile_reset()
+    infos = []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            info, rc = sysm.gspm_step(params(k), m, U, u); k += 1
+            infos.append(info)
+        ev1.record()
+        barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    prof = sysm.profile()
+    sysm.profile_enable(False)
+    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total = float(tmax.item())
+    value = world * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    mh = m.cpu().pin_memory(); Uh = U.cpu().pin_memory(); uh = u.cpu().pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sysm.gspm_step_host(params(k), mh, Uh, uh); k += 1
+    torch.cuda.synchronize()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = world * e2e_steps / float(e2e_s.item())
+    io_bytes = 7 * N * s
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (by accumulated device time)
+    ab = algorithmic_bytes(N, nnz, s)
+    peak, peak_src = measured_peaks()
+    per_class = {}
+    for name, key in (("cg_mech", "cg_iter_bsr3"), ("cg_ms", "cg_iter_csr1"), ("cg_gs", "cg_iter_csr3")):
+        p = prof[name]
+        if p["ms"] > 0 and p["cg_matrix_passes"] > 0:
+            gbs = ab[key] * p["cg_matrix_passes"] / (p["ms"] * 1e-3) / 1e9
+            per_class[name] = {"ms": p["ms"], "launches": p["launches"], "matrix_passes": p["cg_matrix_passes"],
+                               "algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak}
+    for name in ("spmv", "element", "pointwise"):
+        per_class[name] = {"ms": prof[name]["ms"], "launches": prof[name]["launches"]}
+    dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
+    traffic = None
+    tf = ROOT / "profiles" / "traffic.json"
+    if tf.exists():
+        try:
+            traffic = json.loads(tf.read_text()).get(f"{dom}_{dtype}", {}).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roof = {"bound": "hbm", "kernel": f"cg_kernel<{dtype},{dom}> (persistent cooperative CG solve)",
+            "achieved": per_class.get(dom, {}).get("algorithmic_GBps"), "peak": peak, "unit": "GB/s",
+            "frac": per_class.get(dom, {}).get("frac_of_measured_peak"), "traffic": traffic, "peak_source": peak_src,
+            "share_of_step": prof[dom]["ms"] / ms_total,
+            "algorithmic_bytes_per_matrix_pass": ab[{"cg_mech": "cg_iter_bsr3", "cg_ms": "cg_iter_csr1", "cg_gs": "cg_iter_csr3"}[dom]]}
+
+    launches = sum(p["launches"] for p in prof.values())
+    last = infos[-1]
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": dtype, "data": "synthetic",
+            "config": {"workload": "config3_paper_scale", "grid": "x".join(map(str, cfg.mesh.grid)), "n_nodes": N,
+                       "n_tets": mesh.n_tets, "nnz": nnz, "dt_ps": cfg.dt * 1e12, "cg_tol": CG_TOL, "cg_fixed_iters": args.fixed_iters,
+                       "terms": "exchange+anis+zeeman+demag+farfield+magel", "parallelism": f"replicas x{world}",
+                       "l2": "inputs larger than L2 (matrices 3.2 GB fp64 per solve)", "setup_s": t_setup,
+                       "cg_iters_last_step": {"ms": last.it_ms, "mech": last.it_mech, "gs": list(last.it_gs)}},
+            "clocks": clocks.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
+                    "steps": e2e_steps},
+            "gpu_launches": launches, "roofline": roof, "kernels": per_class}
+    if world == 1 and not args.no_cpu_baseline:
+        v, sps, desc, cores = time_oracle(1, 0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--fixed-iters", type=int, default=-1, help="run every CG solve for exactly this many iterations")
+    ap.add_argument("--grid", default="", help="override the node grid, e.g. 81x81x21 (not the headline workload)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

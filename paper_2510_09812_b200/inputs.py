@@ -196,9 +196,10 @@ def _mT_to_Am(mT: float) -> float:
     return mT * 1e-3 / MU0
 
 
-def make_config(idx: int, scale: float = 1.0, grid=None) -> Config:
-    """BASELINE.json configs 0..3.  `grid` overrides the node grid (same box, same recipe) so
-    the parity tests can run the oracle on a reduced instance of the big configs."""
+def make_config(idx: int, grid=None, box=None) -> Config:
+    """BASELINE.json configs 0..3.  `grid` / `box` override the node grid / box lengths (same recipe,
+    same seeds) so that parity tests and the timed CPU baseline can run a reduced instance of the big
+    configs (e.g. a sub-box of config 3 at the same mesh spacing)."""
     nm = 1e-9
     if idx == 0:
         g = grid or (8, 8, 8)
@@ -219,7 +220,7 @@ def make_config(idx: int, scale: float = 1.0, grid=None) -> Config:
                       TERM_ANIS | TERM_ZEEMAN, 5e-12, steps, H, dtypes=("f64", "f32"))
     if idx == 2:
         g = grid or (129, 129, 31)
-        box = (400 * nm, 400 * nm, 100 * nm)
+        box = box or (400 * nm, 400 * nm, 100 * nm)
         mesh = kuhn_box(g, box, seed_mesh=21, seed_perm=22)
         mesh = flag_inclusion(mesh, np.array(box) / 2, (40 * nm,) * 3)
         C = isotropic_voigt(200e9, 0.3)
@@ -230,7 +231,7 @@ def make_config(idx: int, scale: float = 1.0, grid=None) -> Config:
                       10e-12, steps, np.zeros((steps, 3)), clamp_dof=clamp_bottom(mesh))
     if idx == 3:
         g = grid or (245, 245, 50)
-        box = (1000 * nm, 1000 * nm, 200 * nm)
+        box = box or (1000 * nm, 1000 * nm, 200 * nm)
         mesh = kuhn_box(g, box, seed_mesh=31, seed_perm=32)
         mesh = flag_inclusion(mesh, np.array(box) / 2, (120 * nm, 60 * nm, 40 * nm),
                               rotation=random_rotation(34))
