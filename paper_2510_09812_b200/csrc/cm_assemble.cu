@@ -193,7 +193,7 @@ System<T>::~System()
     T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, escr, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
-    cudaFree(til1.d_tile_row); cudaFree(til3.d_tile_row);
+    for (Tiling &t : til) cudaFree(t.d_tile);
     if (h_res) cudaFreeHost(h_res);
     if (h_scal) cudaFreeHost(h_scal);
 }
@@ -287,8 +287,9 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     cudaFree(K); cudaFree(Km); cudaFree(Mm); cudaFree(Kme); cudaFree(Vd); cudaFree(vsum); cudaFree(Cd);
 
     // tilings and work vectors
-    CM_TRY(build_tiling(M->rowptr, N, CM_TILE_S1, &S->til1, st));
-    CM_TRY(build_tiling(M->rowptr, N, CM_TILE_3, &S->til3, st));
+    CM_TRY(build_tiling(M->rowptr, N, CM_WT_CSR1, &S->til[MODE_CSR1], st));
+    CM_TRY(build_tiling(M->rowptr, N, CM_WT_CSR3, &S->til[MODE_CSR3], st));
+    CM_TRY(build_tiling(M->rowptr, N, CM_WT_BSR3, &S->til[MODE_BSR3], st));
     T **vecs3[] = {&S->r, &S->p, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->f, &S->gn, &S->gs, &S->ms, &S->mss, &S->xin, &S->xout, &S->stg_m, &S->stg_u};
     for (T **v : vecs3) CM_TRY(alloc(v, 3 * N));
     CM_TRY(alloc(&S->U, N)); CM_TRY(alloc(&S->stg_U, N)); CM_TRY(alloc(&S->sig, 6 * N));

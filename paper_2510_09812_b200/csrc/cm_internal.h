@@ -31,8 +31,10 @@ void cm_set_error(const char *fmt, ...);
 // Persistent-kernel launch shape: NT threads per CTA everywhere in the SpMV / CG path.
 // NT is a multiple of 3 so that thread t always serves component t % 3.
 constexpr int CM_NT = 384;
-constexpr int CM_TILE_S1 = 4 * CM_NT; // nnz per tile, scalar CSR with one right-hand side
-constexpr int CM_TILE_3 = 2 * CM_NT;  // nnz (blocks) per tile, 3-component modes (CSR3, BSR3)
+// nonzeros (blocks) per warp tile = 32 x (loads in flight per lane)
+constexpr int CM_WT_CSR1 = 256; // scalar CSR, one right-hand side:    8 x 12 B per lane in flight
+constexpr int CM_WT_CSR3 = 128; // scalar CSR, three right-hand sides: 4 x 12 B + 4 x 24 B gathers
+constexpr int CM_WT_BSR3 = 64;  // 3x3 blocks:                         2 x 76 B per lane in flight
 
 enum SpmvMode { MODE_CSR1 = 0, MODE_CSR3 = 1, MODE_BSR3 = 2 };
 
@@ -79,11 +81,11 @@ struct Profiler {
     ~Profiler();
 };
 
-// One scalar tiling = row ranges with at most TILE nonzeros each.
+// One tiling = consecutive row ranges with at most `tile` nonzeros each; descriptor = {first row, first nonzero}.
 struct Tiling {
     int tile = 0;
     int ntiles = 0;
-    int *d_tile_row = nullptr; // ntiles + 1
+    int2 *d_tile = nullptr; // ntiles + 1
 };
 
 struct SystemBase {
@@ -111,7 +113,7 @@ struct System : SystemBase {
     // matrices
     T *Kms = nullptr, *Kgs1 = nullptr, *Kgs2 = nullptr, *Mm = nullptr;
     T *Kmech = nullptr; // tile-SoA: [ceil(nnz/32)][9][32]
-    Tiling til1, til3;
+    Tiling til[3]; // indexed by SpmvMode
     // CG work
     T *r = nullptr, *p = nullptr, *Ap = nullptr, *bvec = nullptr;
     double *partial = nullptr;

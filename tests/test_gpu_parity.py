@@ -332,7 +332,9 @@ def test_gspm_magnetoelastic_inclusion_f64(cm, oracle_mod, torch, variant):
     # steps the two states differ by O(tol), so the warm starts and right-hand sides are no longer the same problem
     _, _, _, _, _, _, infos7, _ = _run_steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 3, "f64", H,
                                              clamp=inputs.clamp_bottom(mesh), variant=variant, m0=m0, cg_tol=1e-7)
-    _check_iters(infos7[:1])
+    # (the mechanical count moves by +-2 of ~235 even between two runs of the ORACLE, whose OpenMP reductions are
+    # not order-deterministic: the unpreconditioned residual curve is flat where it crosses the threshold)
+    _check_iters(infos7[:1], mech_frac=0.015)
     _check_iters(infos7[1:], slack=2, mech_frac=0.03)
 
 
