@@ -140,7 +140,7 @@ def algorithmic_bytes(N, nnz, s):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2510_09812_b200 import binding as cm
+    from paper_2510_09812_b200 import binding as cm, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -195,11 +195,7 @@ def run_ours(args):
     ms_total = ev0.elapsed_time(ev1)
     prof = sysm.profile()
     sysm.profile_enable(False)
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total = float(tmax.item())
-    value = world * args.steps / (ms_total * 1e-3)
+    _, ms_total, value = replicas.aggregate(args.steps, ms_total, dist if world > 1 else None, dev)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     mh = m.cpu().pin_memory(); Uh = U.cpu().pin_memory(); uh = u.cpu().pin_memory()
@@ -209,10 +205,7 @@ def run_ours(args):
     for _ in range(e2e_steps):
         sysm.gspm_step_host(params(k), mh, Uh, uh); k += 1
     torch.cuda.synchronize()
-    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
-    e2e_value = world * e2e_steps / float(e2e_s.item())
+    _, _, e2e_value = replicas.aggregate(e2e_steps, (time.perf_counter() - t0) * 1e3, dist if world > 1 else None, dev)
     io_bytes = 7 * N * s
 
     if rank != 0:
