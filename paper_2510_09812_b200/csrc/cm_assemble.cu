@@ -8,8 +8,6 @@
 
 #include "cm_internal.h"
 
-int build_tiling(const std::vector<int> &rowptr, long N, int tile, Tiling *out, cudaStream_t st);
-
 static const double MU0 = 4.0e-7 * 3.14159265358979323846;
 
 struct TetGeom {
@@ -157,31 +155,38 @@ __global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const
     }
 }
 
-// one thread per nonzero: apply constraints (P A P + (I - P)), form K^GS(eps), round to T, lay out K^mech tile-SoA
+// one thread per row: apply constraints (P A P + (I - P)), form K^GS(eps), round to T and store in the sliced
+// layouts (cm_internal.h): scalar matrices at spS[i / CS] + j * CS + i % CS, the 9 entries of a K^mech block in
+// the 9 planes of its slice, plane k at 9 * spB[s] + k * L_s + (j * CB + i % CB).
 template <typename T>
 __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr, const int *__restrict__ col, const double *K,
                                 const double *Km, const double *Mm, const double *Kme, const uchar *__restrict__ live,
-                                const uchar *__restrict__ clamp, int pin, double eps1, double eps2, T *Kms, T *Kgs1, T *Kgs2, T *MmT,
-                                T *Kmech)
+                                const uchar *__restrict__ clamp, int pin, double eps1, double eps2, const int *__restrict__ spS,
+                                const int *__restrict__ spB, T *Kms, T *Kgs1, T *Kgs2, T *MmT, T *Kmech)
 {
+    constexpr int CS = CM_C_SCALAR, CB = CM_C_BLOCK;
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
-    for (int q = rowptr[i]; q < rowptr[i + 1]; q++) {
+    const long baseS = spS[i / CS] + i % CS;
+    const long bB = spB[i / CB], LB = spB[i / CB + 1] - bB;
+    const int q0 = rowptr[i];
+    for (int q = q0; q < rowptr[i + 1]; q++) {
         const int j = col[q];
+        const long dS = baseS + (long)(q - q0) * CS;
         double kms = K[q];
         if (i == pin || j == pin) kms = (i == j) ? 1.0 : 0.0;
-        Kms[q] = (T)kms;
+        Kms[dS] = (T)kms;
         const double dead = (i == j && !live[i]) ? 1.0 : 0.0;
-        Kgs1[q] = (T)(Mm[q] + eps1 * Km[q] + dead);
-        Kgs2[q] = (T)(Mm[q] + eps2 * Km[q] + dead);
-        MmT[q] = (T)Mm[q];
+        Kgs1[dS] = (T)(Mm[q] + eps1 * Km[q] + dead);
+        Kgs2[dS] = (T)(Mm[q] + eps2 * Km[q] + dead);
+        MmT[dS] = (T)Mm[q];
         if (Kme) {
-            T *dst = Kmech + (long)(q >> 5) * 288 + (q & 31);
+            T *dst = Kmech + 9 * bB + (long)(q - q0) * CB + i % CB;
             for (int r = 0; r < 3; r++)
                 for (int c = 0; c < 3; c++) {
                     double v = Kme[9 * (long)q + 3 * r + c];
                     if (clamp[3 * i + r] || clamp[3 * (long)j + c]) v = (i == j && r == c) ? 1.0 : 0.0;
-                    dst[32 * (3 * r + c)] = (T)v;
+                    dst[LB * (3 * r + c)] = (T)v;
                 }
         }
     }
@@ -190,10 +195,9 @@ __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr
 template <typename T>
 System<T>::~System()
 {
-    T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, escr, sig, stg_m, stg_U, stg_u};
+    T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, escr, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
-    for (Tiling &t : til) cudaFree(t.d_tile);
     if (h_res) cudaFreeHost(h_res);
     if (h_scal) cudaFreeHost(h_scal);
 }
@@ -229,9 +233,9 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     };
     CM_TRY(alloc(&S->V, Ne)); CM_TRY(alloc(&S->G, 12 * Ne)); CM_TRY(alloc(&S->mL, N)); CM_TRY(alloc(&S->mLm, N));
     CM_TRY(alloc(&S->live, N)); CM_TRY(alloc(&S->clamp, 3 * N));
-    CM_TRY(alloc(&S->Kms, nnz)); CM_TRY(alloc(&S->Kgs1, nnz)); CM_TRY(alloc(&S->Kgs2, nnz)); CM_TRY(alloc(&S->Mm, nnz));
-    const long nnz_pad = (nnz + 31) / 32 * 32;
-    if (S->n_elastic) CM_TRY(alloc(&S->Kmech, 9 * nnz_pad));
+    const long ES = M->sell[0].E, EB = M->sell[1].E; // stored elements of the sliced layouts (padding is zero)
+    CM_TRY(alloc(&S->Kms, ES)); CM_TRY(alloc(&S->Kgs1, ES)); CM_TRY(alloc(&S->Kgs2, ES)); CM_TRY(alloc(&S->Mm, ES));
+    if (S->n_elastic) CM_TRY(alloc(&S->Kmech, 9 * EB));
 
     // elastic constants C* = C / (mu0 Ms^2): fp64 for assembly, T for the element kernels
     double *Cd = nullptr;
@@ -281,21 +285,19 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_xyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag,
                                                                       M->d_eid, Cd, M->d_rowptr, M->d_col, K, Km, Mm, Kme);
     finalize_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, nnz, M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->live, S->clamp, S->pin,
-                                                                 S->eps1, S->eps2, S->Kms, S->Kgs1, S->Kgs2, S->Mm, S->Kmech);
+                                                                 S->eps1, S->eps2, M->sell[0].d_sp, M->sell[1].d_sp, S->Kms, S->Kgs1, S->Kgs2,
+                                                                 S->Mm, S->Kmech);
     CM_CUDA(cudaGetLastError());
     CM_CUDA(cudaStreamSynchronize(st));
     cudaFree(K); cudaFree(Km); cudaFree(Mm); cudaFree(Kme); cudaFree(Vd); cudaFree(vsum); cudaFree(Cd);
 
-    // tilings and work vectors
-    CM_TRY(build_tiling(M->rowptr, N, CM_WT_CSR1, &S->til[MODE_CSR1], st));
-    CM_TRY(build_tiling(M->rowptr, N, CM_WT_CSR3, &S->til[MODE_CSR3], st));
-    CM_TRY(build_tiling(M->rowptr, N, CM_WT_BSR3, &S->til[MODE_BSR3], st));
-    T **vecs3[] = {&S->r, &S->p, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->f, &S->gn, &S->gs, &S->ms, &S->mss, &S->xin, &S->xout, &S->stg_m, &S->stg_u};
+    // work vectors
+    T **vecs3[] = {&S->r, &S->p, &S->p2, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->f, &S->gn, &S->gs, &S->ms, &S->mss, &S->xin, &S->xout, &S->stg_m, &S->stg_u};
     for (T **v : vecs3) CM_TRY(alloc(v, 3 * N));
     CM_TRY(alloc(&S->U, N)); CM_TRY(alloc(&S->stg_U, N)); CM_TRY(alloc(&S->sig, 6 * N));
     CM_TRY(alloc(&S->escr, 12 * Ne));
     S->grid_cap = S->num_sms * 8;
-    CM_TRY(alloc(&S->partial, (size_t)2 * S->grid_cap * 3));
+    CM_TRY(alloc(&S->partial, (size_t)4 * S->grid_cap * 3));
     CM_TRY(alloc(&S->d_res, 8));
     CM_TRY(alloc(&S->red, (size_t)4096 * 16));
     CM_TRY(alloc(&S->dscal, 32));
@@ -319,18 +321,27 @@ int sys_get_values(const System<T> *S, cm_matrix_id id, void *host_out, long cap
     case CM_MAT_K_MECH: src = S->Kmech; break;
     }
     if (!src) { cm_set_error("cm_system_get_values: matrix %d not assembled", (int)id); return CM_E_BADARG; }
+    const cm_mesh *M = S->mesh;
+    const std::vector<int> &rp = M->rowptr;
+    T *out = (T *)host_out;
     if (id != CM_MAT_K_MECH) {
         if (capacity < nnz) { cm_set_error("cm_system_get_values: capacity"); return CM_E_BADARG; }
-        CM_CUDA(cudaMemcpy(host_out, src, nnz * sizeof(T), cudaMemcpyDeviceToHost));
+        const Sell &L = M->sell[0];
+        std::vector<T> tmp(L.E);
+        CM_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * sizeof(T), cudaMemcpyDeviceToHost));
+        for (long i = 0; i < S->N; i++)
+            for (int q = rp[i]; q < rp[i + 1]; q++) out[q] = tmp[L.sp[i / L.C] + (long)(q - rp[i]) * L.C + i % L.C];
         return CM_OK;
     }
     if (capacity < 9 * nnz) { cm_set_error("cm_system_get_values: capacity"); return CM_E_BADARG; }
-    const long nnz_pad = (nnz + 31) / 32 * 32;
-    std::vector<T> tmp(9 * nnz_pad);
+    const Sell &L = M->sell[1];
+    std::vector<T> tmp(9 * L.E);
     CM_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * sizeof(T), cudaMemcpyDeviceToHost));
-    T *out = (T *)host_out;
-    for (long q = 0; q < nnz; q++)
-        for (int k = 0; k < 9; k++) out[9 * q + k] = tmp[(q >> 5) * 288 + 32 * k + (q & 31)];
+    for (long i = 0; i < S->N; i++) {
+        const long b = L.sp[i / L.C], len = L.sp[i / L.C + 1] - b;
+        for (int q = rp[i]; q < rp[i + 1]; q++)
+            for (int k = 0; k < 9; k++) out[9 * (long)q + k] = tmp[9 * b + k * len + (long)(q - rp[i]) * L.C + i % L.C];
+    }
     return CM_OK;
 }
 

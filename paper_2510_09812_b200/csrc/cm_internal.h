@@ -29,14 +29,25 @@ void cm_set_error(const char *fmt, ...);
     } while (0)
 
 // Persistent-kernel launch shape: NT threads per CTA everywhere in the SpMV / CG path.
-// NT is a multiple of 3 so that thread t always serves component t % 3.
+// NT is a multiple of 3 so that thread t always serves the same vector component in the streaming phases.
 constexpr int CM_NT = 384;
-// nonzeros (blocks) per warp tile = 32 x (loads in flight per lane)
-constexpr int CM_WT_CSR1 = 256; // scalar CSR, one right-hand side:    8 x 12 B per lane in flight
-constexpr int CM_WT_CSR3 = 128; // scalar CSR, three right-hand sides: 4 x 12 B + 4 x 24 B gathers
-constexpr int CM_WT_BSR3 = 64;  // 3x3 blocks:                         2 x 76 B per lane in flight
+// Sliced storage (SELL-C): rows are grouped into slices of C consecutive rows, every row of a slice is padded to the
+// slice's longest row and the slice is stored column-major, so element (row i, j-th nonzero) sits at
+// sp[i / C] + j * C + i % C.  One warp works on one slice with all 32 lanes: lane -> (row i % C, column phase
+// lane / C).  Scalar matrices use C = 16, the 3x3-block matrix C = 8.
+constexpr int CM_C_SCALAR = 16;
+constexpr int CM_C_BLOCK = 8;
 
 enum SpmvMode { MODE_CSR1 = 0, MODE_CSR3 = 1, MODE_BSR3 = 2 };
+
+// One sliced pattern (shared by every matrix with that slice height).
+struct Sell {
+    int C = 0;
+    int nslices = 0;
+    long E = 0;                 // stored elements including padding = sp[nslices]
+    std::vector<int> sp, col;   // host copies: nslices + 1 offsets, E column indices (padding: the row itself)
+    int *d_sp = nullptr, *d_col = nullptr;
+};
 
 struct cm_mesh {
     long N = 0, Ne = 0, nnz = 0;
@@ -51,6 +62,7 @@ struct cm_mesh {
         *d_eid = nullptr;
     uchar *d_mag = nullptr;
     double *d_xyz = nullptr, *d_wvol = nullptr;
+    Sell sell[2];              // [0]: C = CM_C_SCALAR, [1]: C = CM_C_BLOCK
     // scratch for cm_volume_average
     double *d_red = nullptr;   // partials
     void *d_tmp = nullptr;     // N x 16 x 8 bytes? (allocated lazily, see cm_volume_average)
@@ -81,13 +93,6 @@ struct Profiler {
     ~Profiler();
 };
 
-// One tiling = consecutive row ranges with at most `tile` nonzeros each; descriptor = {first row, first nonzero}.
-struct Tiling {
-    int tile = 0;
-    int ntiles = 0;
-    int2 *d_tile = nullptr; // ntiles + 1
-};
-
 struct SystemBase {
     cm_mesh *mesh = nullptr;
     cm_dtype dtype = CM_F64;
@@ -112,10 +117,9 @@ struct System : SystemBase {
     uchar *live = nullptr, *clamp = nullptr;
     // matrices
     T *Kms = nullptr, *Kgs1 = nullptr, *Kgs2 = nullptr, *Mm = nullptr;
-    T *Kmech = nullptr; // tile-SoA: [ceil(nnz/32)][9][32]
-    Tiling til[3]; // indexed by SpmvMode
+    T *Kmech = nullptr; // sliced, 9 planes per slice: [slice][3 r + c][L_slice]
     // CG work
-    T *r = nullptr, *p = nullptr, *Ap = nullptr, *bvec = nullptr;
+    T *r = nullptr, *p = nullptr, *p2 = nullptr, *Ap = nullptr, *bvec = nullptr;
     double *partial = nullptr;
     int grid_cap = 0;
     CgResult *d_res = nullptr, *h_res = nullptr; // 8 slots
@@ -133,6 +137,7 @@ struct System : SystemBase {
 // ---- cm_mesh.cu ----
 int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long Ne, const uchar *mag, const int *eid,
                     cm_reorder reorder);
+int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out);
 
 // ---- kernels (templated launchers; defined in the .cu files, instantiated for float and double) ----
 template <typename T> int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, long pin_user, cudaStream_t st);

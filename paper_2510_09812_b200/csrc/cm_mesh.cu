@@ -231,6 +231,40 @@ int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long
     build_n2e(N, Ne, M->tets.data(), M->n2e_ptr, M->n2e);
     build_pattern(N, M->tets.data(), M->n2e_ptr, M->n2e, M->rowptr, M->col);
     M->nnz = M->rowptr[N];
+    if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
+    if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
+    return CM_OK;
+}
+
+// Sliced (SELL-C) copy of the CSR pattern: element (i, j) -> sp[i / C] + j * C + i % C; padding entries point at the
+// row itself (clamped to N - 1 in the ragged last slice) and carry zero values.
+int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out)
+{
+    const long ns = (N + C - 1) / C;
+    out->C = C;
+    out->nslices = (int)ns;
+    out->sp.assign(ns + 1, 0);
+    long E = 0;
+    for (long s = 0; s < ns; s++) {
+        int w = 0;
+        for (long i = s * C; i < std::min(N, (s + 1) * C); i++) w = std::max(w, rowptr[i + 1] - rowptr[i]);
+        out->sp[s] = (int)E;
+        E += (long)w * C;
+        if (E > 0x7fffffffL / 9) { cm_set_error("cm_mesh_create: sliced matrix too large for 32-bit offsets"); return CM_E_BADARG; }
+    }
+    out->sp[ns] = (int)E;
+    out->E = E;
+    out->col.resize(E);
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < ns; s++) {
+        const int b = out->sp[s], w = (out->sp[s + 1] - b) / C;
+        for (int rl = 0; rl < C; rl++) {
+            const long i = s * C + rl;
+            const long ic = std::min(i, N - 1);
+            const int len = i < N ? rowptr[i + 1] - rowptr[i] : 0;
+            for (int j = 0; j < w; j++) out->col[b + (long)j * C + rl] = j < len ? col[rowptr[i] + j] : (int)ic;
+        }
+    }
     return CM_OK;
 }
 
@@ -276,6 +310,10 @@ extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, 
             CM_TRY(upload(&M->d_mag, M->mag, st));
             CM_TRY(upload(&M->d_xyz, M->xyz, st));
             CM_TRY(upload(&M->d_wvol, M->wvol, st));
+            for (Sell &L : M->sell) {
+                CM_TRY(upload(&L.d_sp, L.sp, st));
+                CM_TRY(upload(&L.d_col, L.col, st));
+            }
             CM_CUDA(cudaMalloc((void **)&M->d_red, 4096 * 16 * sizeof(double)));
             CM_CUDA(cudaMallocHost((void **)&M->h_red, 16 * sizeof(double)));
             CM_CUDA(cudaStreamSynchronize(st));
@@ -297,6 +335,7 @@ extern "C" int cm_mesh_destroy(cm_mesh *M)
     cudaFree(M->d_order); cudaFree(M->d_tets); cudaFree(M->d_rowptr); cudaFree(M->d_col); cudaFree(M->d_n2e_ptr);
     cudaFree(M->d_n2e); cudaFree(M->d_eid); cudaFree(M->d_mag); cudaFree(M->d_xyz); cudaFree(M->d_wvol);
     cudaFree(M->d_red); cudaFree(M->d_tmp);
+    for (Sell &L : M->sell) { cudaFree(L.d_sp); cudaFree(L.d_col); }
     if (M->h_red) cudaFreeHost(M->h_red);
     delete M;
     return CM_OK;

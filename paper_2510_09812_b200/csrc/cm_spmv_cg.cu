@@ -1,23 +1,26 @@
 // S4 / S7 / S10: sparse matrix-vector products and the fused, persistent, unpreconditioned
 // conjugate-gradient solver (O-4).
 //
-// Layout.  All scalar matrices share rowptr / colidx; values are plain CSR arrays.  The 3x3-block
-// elasticity matrix is stored "tile-SoA": blocks are grouped by 32 and inside a group the 9 block
-// entries are 9 contiguous planes of 32 values, [nnz/32][9][32], so that a warp reading 32 consecutive
-// blocks issues 9 fully coalesced 256-byte (fp64) loads and the whole matrix is one sequential stream.
+// Layout.  Matrices are stored sliced (SELL-C, cm_internal.h): C consecutive rows form a slice, padded to the
+// slice's longest row and stored column-major, so that the 32 lanes of a warp read 32 consecutive elements of
+// every array.  The 3x3-block elasticity matrix keeps its 9 block entries in 9 planes per slice
+// ([slice][3r + c][L_slice]): each plane is one coalesced stream.  On the paper's tetrahedral meshes almost every
+// row has 15 entries, so the padding is about 1.5 % (config 3).
 //
-// Work decomposition.  Rows are cut once, on the host, into "warp tiles" of consecutive rows holding at most
-// WT = 32 U nonzeros (blocks).  A CTA owns a contiguous range of tiles for the whole solve and its warps take
-// them round-robin, each warp on its own -- there is no block-wide barrier inside the SpMV.  Per tile:
-//   phase 1  one lane per nonzero, U in flight per lane: stream value(s) + column index, gather x[col] (1 or 3
-//            components, L1/L2 hits thanks to the locality ordering), write the product(s) to the warp's
-//            private shared-memory slots;
-//   phase 2  one lane per (row, component): sum the row's segment of products in column order
-//            (deterministic, same order as the definition), write y, accumulate the dot p.Ap.
-// The CG kernel is ONE cooperative launch per solve: SpMV, both dot products, the three vector updates
-// and the convergence test run on the device with grid-wide barriers in between; every CTA reduces the
-// per-CTA partial sums in the same fixed order, so all CTAs take the same decision and the result is
-// bit-reproducible run to run.  No float atomics anywhere.
+// SpMV.  One warp per slice, all 32 lanes busy: lane -> (row i % C of the slice, column phase lane / C).  A lane
+// streams its elements (value(s) + column index, U iterations in flight, L1 bypassed, L2 evict-first), gathers
+// x[col] (L1 / L2 hits thanks to the locality ordering) and accumulates in registers in column order; the
+// 32 / C column phases of a row are combined with a fixed shuffle butterfly.  No shared memory, no atomics.
+//
+// CG.  ONE cooperative launch per solve with TWO grid-wide barriers per iteration (after each dot product).
+// A CTA owns a contiguous range of slices, hence of rows.  Per iteration k:
+//   C'  p_k = r_k + beta p_{k-1} on the CTA's own rows (into the other p buffer), CTA-local barrier;
+//   A   Ap = A p_k: columns inside the own range read p_k, columns outside (the halo) recompute
+//       fma(beta, p_{k-1}, r_k) from the two globally visible vectors -- bit-identical to what the owner wrote,
+//       which removes the third grid barrier of the textbook loop; dot p.Ap;               -> barrier, alpha
+//   B   x += alpha p, r -= alpha Ap, dot r.r;                                              -> barrier, beta
+// Every CTA reduces the per-CTA partial sums in the same fixed order, so all CTAs take the same decisions and the
+// result is bit-reproducible run to run.  Dot products accumulate in fp64 in both precisions (R20).
 #include <cooperative_groups.h>
 
 #include <algorithm>
@@ -28,26 +31,55 @@ namespace cg = cooperative_groups;
 
 template <typename T>
 struct MatView {
-    const int *rowptr;
-    const int *col;
-    const T *val;
-    const int2 *tile; // ntiles + 1 descriptors {first row, first nonzero}
-    int ntiles;
+    const int *sp;  // nslices + 1 element offsets
+    const int *col; // E column indices, sliced order
+    const T *val;   // E values (scalar) or 9 E (block: 9 planes per slice)
+    int nslices;
     long N;
 };
 
-// WT = nonzeros (blocks) per warp tile = 32 * U, U loads in flight per lane.
+// NC vector components per node, NR independent right-hand sides, NV stored values per element, C rows per slice,
+// U 32-element iterations in flight per warp.
 template <int MODE> struct ModeTraits;
-template <> struct ModeTraits<MODE_CSR1> { static constexpr int NC = 1, NR = 1, NV = 1, WT = CM_WT_CSR1; };
-template <> struct ModeTraits<MODE_CSR3> { static constexpr int NC = 3, NR = 3, NV = 1, WT = CM_WT_CSR3; };
-template <> struct ModeTraits<MODE_BSR3> { static constexpr int NC = 3, NR = 1, NV = 9, WT = CM_WT_BSR3; };
+template <> struct ModeTraits<MODE_CSR1> { static constexpr int NC = 1, NR = 1, NV = 1, C = CM_C_SCALAR, U = 8; };
+template <> struct ModeTraits<MODE_CSR3> { static constexpr int NC = 3, NR = 3, NV = 1, C = CM_C_SCALAR, U = 4; };
+template <> struct ModeTraits<MODE_BSR3> { static constexpr int NC = 3, NR = 1, NV = 9, C = CM_C_BLOCK, U = 2; };
 
-// Contiguous tile range of CTA `b` out of `nb`.
-__device__ __forceinline__ void cta_tiles(int ntiles, int b, int nb, int &t0, int &t1)
+// ---- streaming loads of the matrix: read once per pass, so keep them out of L1 and first in line for L2 eviction
+__device__ __forceinline__ unsigned long long policy_evict_first()
 {
-    int q = ntiles / nb, r = ntiles % nb;
-    t0 = b * q + min(b, r);
-    t1 = t0 + q + (b < r ? 1 : 0);
+    unsigned long long p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double ld_stream(const double *p, unsigned long long pol)
+{
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float ld_stream(const float *p, unsigned long long pol)
+{
+    float v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ int ld_stream(const int *p, unsigned long long pol)
+{
+    int v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
+    return v;
+}
+
+__device__ __forceinline__ double fma_t(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float fma_t(float a, float b, float c) { return fmaf(a, b, c); }
+
+// Contiguous slice range of CTA `b` out of `nb`.
+__device__ __forceinline__ void cta_units(int n, int b, int nb, int &u0, int &u1)
+{
+    int q = n / nb, r = n % nb;
+    u0 = b * q + min(b, r);
+    u1 = u0 + q + (b < r ? 1 : 0);
 }
 
 // Deterministic block-wide sum of NV doubles per thread; result broadcast to all threads.
@@ -73,129 +105,238 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double *sh /* >= NV *
     }
 }
 
-// y = A x on the warp tiles [t0, t1) of this CTA (warp w takes t0 + w, t0 + w + nwarps, ...); optionally
-// accumulates dot[c] += y.x over the rows written.  `prod` = this warp's private NC * WT shared-memory slots.
-// No block-wide barrier: warps stream independently, so DRAM latency is hidden by the other warps of the SM.
-template <typename T, int MODE, bool DOT>
-__device__ __forceinline__ void spmv_warp_tiles(const MatView<T> &A, const T *x, T *y, int t0, int t1, T *prod, double (&dot)[3])
+template <int NR, typename V>
+__device__ __forceinline__ V pick(const V (&a)[NR], int c)
 {
-    constexpr int NC = ModeTraits<MODE>::NC, NV = ModeTraits<MODE>::NV, WT = ModeTraits<MODE>::WT, U = WT / 32;
+    V r = a[0];
+    if (NR == 3) { if (c == 1) r = a[1]; else if (c == 2) r = a[2]; }
+    return r;
+}
+
+// Where the multiplied vector comes from.  Plain: x.  Fused (CG): p_k = x on the rows [own0, own1) the CTA has
+// already updated, fma(beta, pold, r) elsewhere.
+template <typename T, int MODE, bool FUSED>
+struct XSource {
+    const T *x;
+    const T *pold, *r;
+    T beta[ModeTraits<MODE>::NR];
+    int own0, own1;
+};
+
+template <typename T, int MODE, bool FUSED>
+__device__ __forceinline__ void fetch(const XSource<T, MODE, FUSED> &X, int col, T (&out)[ModeTraits<MODE>::NC])
+{
+    constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR;
+    const long o = (long)col * NC;
+    if (!FUSED) {
+#pragma unroll
+        for (int c = 0; c < NC; c++) out[c] = X.x[o + c];
+    } else {
+        // branch-free: one unconditional load (own: p_k, halo: r_k) and one predicated load (halo: p_{k-1})
+        const bool own = col >= X.own0 && col < X.own1;
+        const T *a = own ? X.x : X.r;
+#pragma unroll
+        for (int c = 0; c < NC; c++) {
+            const T av = a[o + c];
+            const T pv = own ? (T)0 : X.pold[o + c];
+            out[c] = own ? av : fma_t(X.beta[NR == 3 ? c : 0], pv, av);
+        }
+    }
+}
+
+// y = A x on the slices [u0, u1) of this CTA (warp w takes u0 + w, u0 + w + nwarps, ...); optionally accumulates
+// dot[c] += y.x over the rows written (x must then be valid on those rows: the own range when FUSED).
+template <typename T, int MODE, bool FUSED, bool DOT>
+__device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T, MODE, FUSED> &X, T *y, int u0, int u1, double (&dot)[3])
+{
+    constexpr int NC = ModeTraits<MODE>::NC, NV = ModeTraits<MODE>::NV, C = ModeTraits<MODE>::C, U = ModeTraits<MODE>::U;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    int t = t0 + warp;
-    if (t >= t1) return;
-    int2 d0 = __ldg(A.tile + t), d1 = __ldg(A.tile + t + 1);
+    const int rl = lane % C, jl = lane / C;
+    const unsigned long long pol = policy_evict_first();
+    int s = u0 + warp;
+    if (s >= u1) return;
+    int b0 = __ldg(A.sp + s), b1 = __ldg(A.sp + s + 1);
     for (;;) {
-        const int r0 = d0.x, q0 = d0.y, r1 = d1.x, q1 = d1.y;
-        const int tn = t + nw;
-        if (tn < t1) { d0 = __ldg(A.tile + tn); d1 = __ldg(A.tile + tn + 1); } // prefetch the next descriptors
-        if (q1 - q0 <= WT) {
-            // ---- phase 1: all streaming loads first (U per lane in flight), then the dependent gathers
+        const int sn = s + nw;
+        int n0 = 0, n1 = 0;
+        if (sn < u1) { n0 = __ldg(A.sp + sn); n1 = __ldg(A.sp + sn + 1); } // prefetch the next slice's extent
+        const int L = b1 - b0;
+        const int *colp = A.col + b0;
+        const T *valp = A.val + (long)NV * b0; // plane k at valp + k * L
+        T acc[NC];
+#pragma unroll
+        for (int c = 0; c < NC; c++) acc[c] = 0;
+        for (int it = 0; it < L; it += 32 * U) {
             int col[U];
             T v[U][NV];
+            // all streaming loads of the batch first (U per array per lane in flight), then the dependent gathers
 #pragma unroll
-            for (int j = 0; j < U; j++) {
-                const int q = q0 + lane + 32 * j;
-                col[j] = 0;
+            for (int u = 0; u < U; u++) {
+                const int e = it + 32 * u + lane;
+                col[u] = 0;
 #pragma unroll
-                for (int k = 0; k < NV; k++) v[j][k] = 0;
-                if (q < q1) {
-                    col[j] = __ldg(A.col + q);
+                for (int k = 0; k < NV; k++) v[u][k] = 0;
+                if (e < L) {
+                    col[u] = ld_stream(colp + e, pol);
+#pragma unroll
+                    for (int k = 0; k < NV; k++) v[u][k] = ld_stream(valp + (long)k * L + e, pol);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int e = it + 32 * u + lane;
+                if (e < L) {
+                    T xv[NC];
+                    fetch<T, MODE, FUSED>(X, col[u], xv);
                     if (MODE == MODE_BSR3) {
-                        const T *vp = A.val + (long)(q >> 5) * 288 + (q & 31);
-#pragma unroll
-                        for (int k = 0; k < NV; k++) v[j][k] = __ldg(vp + 32 * k);
+                        acc[0] += v[u][0] * xv[0] + v[u][1] * xv[1] + v[u][2] * xv[2];
+                        acc[1] += v[u][3] * xv[0] + v[u][4] * xv[1] + v[u][5] * xv[2];
+                        acc[2] += v[u][6] * xv[0] + v[u][7] * xv[1] + v[u][8] * xv[2];
                     } else {
-                        v[j][0] = __ldg(A.val + q);
+#pragma unroll
+                        for (int c = 0; c < NC; c++) acc[c] += v[u][0] * xv[c];
                     }
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < U; j++) {
-                const int q = q0 + lane + 32 * j;
-                if (q < q1) {
-                    const int o = q - q0;
-                    if (MODE == MODE_CSR1) {
-                        prod[o] = v[j][0] * x[col[j]];
-                    } else {
-                        const T *xc = x + 3 * (long)col[j];
-                        const T x0 = xc[0], x1 = xc[1], x2 = xc[2];
-                        if (MODE == MODE_CSR3) {
-                            prod[o] = v[j][0] * x0; prod[WT + o] = v[j][0] * x1; prod[2 * WT + o] = v[j][0] * x2;
-                        } else {
-                            prod[o] = v[j][0] * x0 + v[j][1] * x1 + v[j][2] * x2;
-                            prod[WT + o] = v[j][3] * x0 + v[j][4] * x1 + v[j][5] * x2;
-                            prod[2 * WT + o] = v[j][6] * x0 + v[j][7] * x1 + v[j][8] * x2;
-                        }
-                    }
-                }
-            }
-            __syncwarp();
-            // ---- phase 2: lane -> (row, component); sum the row's products in column order
-            const int ntask = (r1 - r0) * NC;
-            for (int k = lane; k < ntask; k += 32) {
-                const int row = r0 + k / NC, c = k % NC;
-                const int a = __ldg(A.rowptr + row) - q0, b = __ldg(A.rowptr + row + 1) - q0;
-                T acc = 0;
-                for (int j = a; j < b; j++) acc += prod[c * WT + j];
-                const long o = (long)row * NC + c;
-                y[o] = acc;
-                if (DOT) {
-                    const double d = (double)acc * (double)x[o];
-                    if (MODE != MODE_CSR3 || c == 0) dot[0] += d;
-                    else if (c == 1) dot[1] += d;
-                    else dot[2] += d;
-                }
-            }
-            __syncwarp();
-        } else {
-            // a single row longer than a warp tile (r1 == r0 + 1): lane-strided accumulation, shuffle reduction
-            double acc[3] = {0, 0, 0};
-            for (int q = q0 + lane; q < q1; q += 32) {
-                const int c = __ldg(A.col + q);
-                if (MODE == MODE_CSR1) {
-                    acc[0] += (double)(__ldg(A.val + q) * x[c]);
-                } else if (MODE == MODE_CSR3) {
-                    const T a = __ldg(A.val + q);
-                    const T *xc = x + 3 * (long)c;
-                    acc[0] += (double)(a * xc[0]); acc[1] += (double)(a * xc[1]); acc[2] += (double)(a * xc[2]);
-                } else {
-                    const T *vp = A.val + (long)(q >> 5) * 288 + (q & 31);
-                    const T *xc = x + 3 * (long)c;
-                    const T x0 = xc[0], x1 = xc[1], x2 = xc[2];
-                    acc[0] += (double)(__ldg(vp) * x0 + __ldg(vp + 32) * x1 + __ldg(vp + 64) * x2);
-                    acc[1] += (double)(__ldg(vp + 96) * x0 + __ldg(vp + 128) * x1 + __ldg(vp + 160) * x2);
-                    acc[2] += (double)(__ldg(vp + 192) * x0 + __ldg(vp + 224) * x1 + __ldg(vp + 256) * x2);
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < 3; k++)
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
-            if (lane == 0) {
-#pragma unroll
-                for (int c = 0; c < NC; c++) {
-                    const long o = (long)r0 * NC + c;
-                    const T yv = (T)acc[c];
-                    y[o] = yv;
-                    if (DOT) dot[MODE == MODE_CSR3 ? c : 0] += (double)yv * (double)x[o];
                 }
             }
         }
-        if (tn >= t1) break;
-        t = tn;
+        // combine the 32 / C column phases of each row (fixed butterfly: every lane ends with the same sum)
+#pragma unroll
+        for (int o = C; o < 32; o <<= 1)
+#pragma unroll
+            for (int c = 0; c < NC; c++) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
+        const long row = (long)s * C + rl;
+        if (row < A.N) {
+            if (MODE == MODE_BSR3) {
+                // 32 / C = 4 >= 3 phases: phase jl writes component jl
+                if (jl < 3) {
+                    const T a = jl == 0 ? acc[0] : (jl == 1 ? acc[1] : acc[2]);
+                    y[3 * row + jl] = a;
+                    if (DOT) dot[0] += (double)a * (double)X.x[3 * row + jl];
+                }
+            } else if (jl == 0) {
+#pragma unroll
+                for (int c = 0; c < NC; c++) {
+                    y[NC * row + c] = acc[c];
+                    if (DOT) dot[c] += (double)acc[c] * (double)X.x[NC * row + c];
+                }
+            }
+        }
+        if (sn >= u1) break;
+        s = sn; b0 = n0; b1 = n1;
     }
 }
 
 template <typename T, int MODE>
-__global__ void __launch_bounds__(CM_NT) spmv_kernel(MatView<T> A, const T *x, T *y)
+__global__ void __launch_bounds__(CM_NT, 2) spmv_kernel(MatView<T> A, const T *x, T *y)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int PW = ModeTraits<MODE>::NC * ModeTraits<MODE>::WT;
-    T *prod = reinterpret_cast<T *>(smem_raw) + (threadIdx.x >> 5) * PW;
-    int t0, t1;
-    cta_tiles(A.ntiles, blockIdx.x, gridDim.x, t0, t1);
+    int u0, u1;
+    cta_units(A.nslices, blockIdx.x, gridDim.x, u0, u1);
+    XSource<T, MODE, false> X;
+    X.x = x;
     double dot[3] = {0, 0, 0};
-    spmv_warp_tiles<T, MODE, false>(A, x, y, t0, t1, prod, dot);
+    spmv_units<T, MODE, false, false>(A, X, y, u0, u1, dot);
+}
+
+// --------------------------------------------------------------------------------------------------
+// streaming vector phases of CG: 128-bit accesses, UN vectors per array per thread in flight
+// --------------------------------------------------------------------------------------------------
+template <typename T> struct VecOf;
+template <> struct VecOf<double> { typedef double2 V; static constexpr int W = 2; };
+template <> struct VecOf<float> { typedef float4 V; static constexpr int W = 4; };
+
+// lane-wise c[j] * a[j] + b[j]
+__device__ __forceinline__ double2 vfma(const double (&c)[2], double2 a, double2 b) { return make_double2(fma(c[0], a.x, b.x), fma(c[1], a.y, b.y)); }
+__device__ __forceinline__ float4 vfma(const float (&c)[4], float4 a, float4 b)
+{
+    return make_float4(fmaf(c[0], a.x, b.x), fmaf(c[1], a.y, b.y), fmaf(c[2], a.z, b.z), fmaf(c[3], a.w, b.w));
+}
+// lane-wise acc[j] += v[j]^2 in fp64
+__device__ __forceinline__ void vsq(double (&acc)[2], double2 v) { acc[0] += v.x * v.x; acc[1] += v.y * v.y; }
+__device__ __forceinline__ void vsq(double (&acc)[4], float4 v)
+{
+    acc[0] += (double)v.x * (double)v.x; acc[1] += (double)v.y * (double)v.y;
+    acc[2] += (double)v.z * (double)v.z; acc[3] += (double)v.w * (double)v.w;
+}
+
+// The streaming phases run over the CTA's own entries [e0, e1): a 16-byte aligned vector body (e0 is a multiple
+// of 8 entries because slices hold 8 or 16 rows) plus a scalar tail.  e0 % 3 == 0 and blockDim.x * W % 3 == 0, so
+// the component served by lane j of a thread's vectors is the same in every trip: (tid * W + j) % 3.
+
+// C': pnew = r + beta pold
+template <typename T, int NR>
+__device__ __forceinline__ void phase_p(T *pnew, const T *pold, const T *r, long e0, long e1, const T (&beta)[NR])
+{
+    constexpr int W = VecOf<T>::W, UN = 4;
+    typedef typename VecOf<T>::V V;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const long a1 = e0 + (e1 - e0) / W * W, nv = (a1 - e0) / W;
+    T be[W];
+#pragma unroll
+    for (int j = 0; j < W; j++) be[j] = pick<NR>(beta, NR == 3 ? (tid * W + j) % 3 : 0);
+    V *pn = reinterpret_cast<V *>(pnew + e0);
+    const V *po = reinterpret_cast<const V *>(pold + e0), *rv = reinterpret_cast<const V *>(r + e0);
+    long v = tid;
+    for (; v + (long)(UN - 1) * nt < nv; v += (long)nt * UN) {
+        V a[UN], b[UN];
+#pragma unroll
+        for (int q = 0; q < UN; q++) { a[q] = po[v + (long)q * nt]; b[q] = rv[v + (long)q * nt]; }
+#pragma unroll
+        for (int q = 0; q < UN; q++) pn[v + (long)q * nt] = vfma(be, a[q], b[q]);
+    }
+    for (; v < nv; v += nt) pn[v] = vfma(be, po[v], rv[v]);
+    for (long i = a1 + tid; i < e1; i += nt) pnew[i] = fma_t(pick<NR>(beta, NR == 3 ? (int)(i % 3) : 0), pold[i], r[i]);
+}
+
+// B: x += alpha p, r -= alpha Ap; s[c] += sum of r_new^2 per component
+template <typename T, int NR>
+__device__ __forceinline__ void phase_xr(T *x, T *r, const T *p, const T *Ap, long e0, long e1, const T (&alpha)[NR], double (&s)[3])
+{
+    constexpr int W = VecOf<T>::W, UN = 2;
+    typedef typename VecOf<T>::V V;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const long a1 = e0 + (e1 - e0) / W * W, nv = (a1 - e0) / W;
+    T al[W], nal[W];
+    int cj[W];
+    double acc[W];
+#pragma unroll
+    for (int j = 0; j < W; j++) { cj[j] = NR == 3 ? (tid * W + j) % 3 : 0; al[j] = pick<NR>(alpha, cj[j]); nal[j] = -al[j]; acc[j] = 0; }
+    V *xv = reinterpret_cast<V *>(x + e0), *rv = reinterpret_cast<V *>(r + e0);
+    const V *pv = reinterpret_cast<const V *>(p + e0), *av = reinterpret_cast<const V *>(Ap + e0);
+    long v = tid;
+    for (; v + (long)(UN - 1) * nt < nv; v += (long)nt * UN) {
+        V a[UN], b[UN], c[UN], d[UN];
+#pragma unroll
+        for (int q = 0; q < UN; q++) {
+            const long vv = v + (long)q * nt;
+            a[q] = pv[vv]; b[q] = av[vv]; c[q] = xv[vv]; d[q] = rv[vv];
+        }
+#pragma unroll
+        for (int q = 0; q < UN; q++) {
+            const long vv = v + (long)q * nt;
+            xv[vv] = vfma(al, a[q], c[q]);
+            const V rn = vfma(nal, b[q], d[q]);
+            rv[vv] = rn;
+            vsq(acc, rn);
+        }
+    }
+    for (; v < nv; v += nt) {
+        xv[v] = vfma(al, pv[v], xv[v]);
+        const V rn = vfma(nal, av[v], rv[v]);
+        rv[v] = rn;
+        vsq(acc, rn);
+    }
+#pragma unroll
+    for (int j = 0; j < W; j++)
+#pragma unroll
+        for (int q = 0; q < 3; q++) s[q] += (cj[j] == q) ? acc[j] : 0.0;
+    for (long i = a1 + tid; i < e1; i += nt) {
+        const int c = NR == 3 ? (int)(i % 3) : 0;
+        const T a = pick<NR>(alpha, c);
+        x[i] = fma_t(a, p[i], x[i]);
+        const T ri = fma_t(-a, Ap[i], r[i]);
+        r[i] = ri;
+        s[c] += (double)ri * (double)ri;
+    }
 }
 
 // --------------------------------------------------------------------------------------------------
@@ -205,8 +346,8 @@ template <typename T>
 struct CgArgs {
     MatView<T> A;
     const T *b;
-    T *x, *r, *p, *Ap;
-    double *partial; // [2][grid][3]
+    T *x, *r, *p, *p2, *Ap;
+    double *partial; // [4][grid][3]
     double tol;
     int maxiter, fixed;
     unsigned mask;
@@ -229,42 +370,35 @@ __device__ __forceinline__ void grid_sum(const double *partial, int slot, double
     for (int c = 0; c < NR; c++) out[c] = v[c];
 }
 
-template <int NR, typename V>
-__device__ __forceinline__ V pick(const V (&a)[NR], int c)
-{
-    V r = a[0];
-    if (NR == 3) { if (c == 1) r = a[1]; else if (c == 2) r = a[2]; }
-    return r;
-}
-
 template <typename T, int MODE>
 __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
 {
-    constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR, VU = 2;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int PW = NC * ModeTraits<MODE>::WT;
-    T *prod = reinterpret_cast<T *>(smem_raw) + (threadIdx.x >> 5) * PW;
+    constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR, C = ModeTraits<MODE>::C;
     __shared__ double red[6 * 32];
     cg::grid_group grid = cg::this_grid();
     const int tid = threadIdx.x, nt = blockDim.x, nb = gridDim.x, bid = blockIdx.x;
-    int t0, t1;
-    cta_tiles(a.A.ntiles, bid, nb, t0, t1);
-    // own entries: [e0, e1) of the interleaved vectors
-    const long e0 = (long)a.A.tile[t0].x * NC, e1 = (long)a.A.tile[t1].x * NC;
-    double *part0 = a.partial + ((long)0 * nb + bid) * 3, *part1 = a.partial + ((long)1 * nb + bid) * 3;
-    // component served by this thread in the vector phases: e0 % 3 == 0 and nt % 3 == 0, so it is fixed
+    int u0, u1;
+    cta_units(a.A.nslices, bid, nb, u0, u1);
+    // own rows [own0, own1) and own entries [e0, e1) of the interleaved vectors
+    const int own0 = (int)min((long)u0 * C, a.A.N), own1 = (int)min((long)u1 * C, a.A.N);
+    const long e0 = (long)own0 * NC, e1 = (long)own1 * NC;
+    auto part = [&](int slot) { return a.partial + ((long)slot * nb + bid) * 3; };
+    // component served by this thread in the scalar loops below: e0 % 3 == 0 and nt % 3 == 0, so it is fixed
     const int c = (NR == 3) ? tid % 3 : 0;
     double nodot[3] = {0, 0, 0};
 
-    // ---- r = b - A x0, p = r, rr, bb
-    spmv_warp_tiles<T, MODE, false>(a.A, a.x, a.Ap, t0, t1, prod, nodot);
+    // ---- r = b - A x0, rr, bb
+    {
+        XSource<T, MODE, false> X0;
+        X0.x = a.x;
+        spmv_units<T, MODE, false, false>(a.A, X0, a.Ap, u0, u1, nodot);
+    }
     __syncthreads(); // Ap of the CTA's rows was written by other warps
     {
         double srr = 0, sbb = 0;
         for (long i = e0 + tid; i < e1; i += nt) {
             const T bi = a.b[i], ri = bi - a.Ap[i];
             a.r[i] = ri;
-            a.p[i] = ri;
             srr += (double)ri * (double)ri;
             sbb += (double)bi * (double)bi;
         }
@@ -273,13 +407,12 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         for (int k = 0; k < 3; k++) { v[k] = (k == c) ? srr : 0.0; v[3 + k] = (k == c) ? sbb : 0.0; }
         block_sum<6>(v, red);
         if (tid == 0)
-            for (int k = 0; k < 3; k++) { part0[k] = v[k]; part1[k] = v[3 + k]; }
+            for (int k = 0; k < 3; k++) { part(2)[k] = v[k]; part(3)[k] = v[3 + k]; }
     }
     grid.sync();
     double rr[NR], bb[NR];
-    grid_sum<NR>(a.partial, 0, rr, red);
-    grid_sum<NR>(a.partial, 1, bb, red);
-    grid.sync(); // partial slots are reused below
+    grid_sum<NR>(a.partial, 2, rr, red);
+    grid_sum<NR>(a.partial, 3, bb, red);
 
     bool active[NR];
     int iters[NR], status = CM_OK;
@@ -294,6 +427,13 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
     if (pick<NR>(zero_rhs, c))
         for (long i = e0 + tid; i < e1; i += nt) a.x[i] = 0;
 
+    // p_0 = r_0: beta = 0 and "p_{-1}" = r (any finite vector)
+    T beta[NR];
+#pragma unroll
+    for (int q = 0; q < NR; q++) beta[q] = 0;
+    const T *pold = a.r;
+    T *pnew = a.p, *pother = a.p2;
+
     for (int k = 0;; k++) {
         bool any = false;
 #pragma unroll
@@ -306,12 +446,21 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
             any |= active[q];
         }
         if (!any) break;
-        // ---- A: Ap = A p, pAp
+        // ---- C': p_k on the own rows
+        phase_p<T, NR>(pnew, pold, a.r, e0, e1, beta);
+        __syncthreads();
+        // ---- A: Ap = A p_k (halo columns recomputed from r_k, p_{k-1}), pAp
         double s_pap[3] = {0, 0, 0};
-        spmv_warp_tiles<T, MODE, true>(a.A, a.p, a.Ap, t0, t1, prod, s_pap);
+        {
+            XSource<T, MODE, true> X;
+            X.x = pnew; X.pold = pold; X.r = a.r; X.own0 = own0; X.own1 = own1;
+#pragma unroll
+            for (int q = 0; q < NR; q++) X.beta[q] = beta[q];
+            spmv_units<T, MODE, true, true>(a.A, X, a.Ap, u0, u1, s_pap);
+        }
         block_sum<3>(s_pap, red);
         if (tid == 0)
-            for (int q = 0; q < 3; q++) part0[q] = s_pap[q];
+            for (int q = 0; q < 3; q++) part(0)[q] = s_pap[q];
         grid.sync();
         double pap[NR];
         grid_sum<NR>(a.partial, 0, pap, red);
@@ -323,65 +472,24 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
             if (!(pap[q] > 0.0)) { active[q] = false; status = CM_E_CG_BREAKDOWN; continue; }
             alpha[q] = (T)(rr[q] / pap[q]);
         }
-        // ---- B: x += alpha p, r -= alpha Ap, rr_new   (VU independent elements per thread in flight)
-        const bool my_active = pick<NR>(active, c);
-        double snew = 0;
-        if (my_active) {
-            const T al = pick<NR>(alpha, c);
-            for (long i = e0 + tid; i < e1; i += (long)nt * VU) {
-                T pv[VU], av[VU], xv[VU], rv[VU];
-#pragma unroll
-                for (int q = 0; q < VU; q++) {
-                    const long ii = i + (long)q * nt;
-                    if (ii < e1) { pv[q] = a.p[ii]; av[q] = a.Ap[ii]; xv[q] = a.x[ii]; rv[q] = a.r[ii]; }
-                }
-#pragma unroll
-                for (int q = 0; q < VU; q++) {
-                    const long ii = i + (long)q * nt;
-                    if (ii < e1) {
-                        a.x[ii] = xv[q] + al * pv[q];
-                        const T ri = rv[q] - al * av[q];
-                        a.r[ii] = ri;
-                        snew += (double)ri * (double)ri;
-                    }
-                }
-            }
-        }
-        {
-            double v[3];
-#pragma unroll
-            for (int q = 0; q < 3; q++) v[q] = (q == c) ? snew : 0.0;
-            block_sum<3>(v, red);
-            if (tid == 0)
-                for (int q = 0; q < 3; q++) part1[q] = v[q];
-        }
+        // ---- B: x += alpha p, r -= alpha Ap, rr_new (alpha = 0 freezes a finished component)
+        double snew[3] = {0, 0, 0};
+        phase_xr<T, NR>(a.x, a.r, pnew, a.Ap, e0, e1, alpha, snew);
+        block_sum<3>(snew, red);
+        if (tid == 0)
+            for (int q = 0; q < 3; q++) part(1)[q] = snew[q];
         grid.sync();
         double rr_new[NR];
         grid_sum<NR>(a.partial, 1, rr_new, red);
-        // ---- C: p = r + beta p
-        T beta[NR];
 #pragma unroll
-        for (int q = 0; q < NR; q++) beta[q] = active[q] ? (T)(rr_new[q] / rr[q]) : (T)0;
-        if (my_active) {
-            const T be = pick<NR>(beta, c);
-            for (long i = e0 + tid; i < e1; i += (long)nt * VU) {
-                T pv[VU], rv[VU];
-#pragma unroll
-                for (int q = 0; q < VU; q++) {
-                    const long ii = i + (long)q * nt;
-                    if (ii < e1) { pv[q] = a.p[ii]; rv[q] = a.r[ii]; }
-                }
-#pragma unroll
-                for (int q = 0; q < VU; q++) {
-                    const long ii = i + (long)q * nt;
-                    if (ii < e1) a.p[ii] = rv[q] + be * pv[q];
-                }
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < NR; q++)
+        for (int q = 0; q < NR; q++) {
+            beta[q] = active[q] ? (T)(rr_new[q] / rr[q]) : (T)0;
             if (active[q]) { rr[q] = rr_new[q]; iters[q]++; }
-        grid.sync();
+        }
+        // rotate the p buffers: p_k becomes p_{k-1}
+        T *t = (pold == a.r) ? pother : const_cast<T *>(pold);
+        pold = pnew;
+        pnew = t;
     }
     if (bid == 0 && tid == 0) {
         for (int q = 0; q < 3; q++) { a.out->iters[q] = 0; a.out->relres[q] = 0; }
@@ -396,25 +504,6 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
 // --------------------------------------------------------------------------------------------------
 // host side
 // --------------------------------------------------------------------------------------------------
-int build_tiling(const std::vector<int> &rowptr, long N, int tile, Tiling *out, cudaStream_t st)
-{
-    std::vector<int2> td;
-    long r = 0;
-    while (r < N) {
-        td.push_back(make_int2((int)r, rowptr[r]));
-        long r1 = r + 1; // always at least one row (a single over-long row forms its own tile)
-        while (r1 < N && rowptr[r1 + 1] - rowptr[r] <= tile) r1++;
-        r = r1;
-    }
-    td.push_back(make_int2((int)N, rowptr[N]));
-    out->tile = tile;
-    out->ntiles = (int)td.size() - 1;
-    CM_CUDA(cudaMalloc((void **)&out->d_tile, td.size() * sizeof(int2)));
-    CM_CUDA(cudaMemcpyAsync(out->d_tile, td.data(), td.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
-    CM_CUDA(cudaStreamSynchronize(st));
-    return CM_OK;
-}
-
 template <typename T>
 static const T *mat_values(const System<T> *S, cm_matrix_id id)
 {
@@ -434,23 +523,20 @@ static int make_view(const System<T> *S, cm_matrix_id id, int mode, MatView<T> *
     const T *v = mat_values(S, id);
     if (!v) { cm_set_error("matrix %d is not assembled (no elastic material?)", (int)id); return CM_E_BADARG; }
     if ((id == CM_MAT_K_MECH) != (mode == MODE_BSR3)) { cm_set_error("matrix %d does not match mode %d", (int)id, mode); return CM_E_BADARG; }
-    const Tiling &tl = S->til[mode];
-    A->rowptr = S->mesh->d_rowptr; A->col = S->mesh->d_col; A->val = v;
-    A->tile = tl.d_tile; A->ntiles = tl.ntiles; A->N = S->N;
+    const Sell &L = S->mesh->sell[mode == MODE_BSR3 ? 1 : 0];
+    A->sp = L.d_sp; A->col = L.d_col; A->val = v;
+    A->nslices = L.nslices; A->N = S->N;
     return CM_OK;
 }
-
-template <typename T, int MODE>
-static size_t smem_bytes() { return (size_t)(CM_NT / 32) * ModeTraits<MODE>::NC * ModeTraits<MODE>::WT * sizeof(T); }
 
 template <typename T, int MODE>
 static int launch_spmv(System<T> *S, const MatView<T> &A, const T *x, T *y, cudaStream_t st)
 {
     int occ = 0;
-    CM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_kernel<T, MODE>, CM_NT, smem_bytes<T, MODE>()));
-    int grid = std::max(1, std::min(A.ntiles, occ * S->num_sms));
+    CM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_kernel<T, MODE>, CM_NT, 0));
+    int grid = std::max(1, std::min(A.nslices, occ * S->num_sms));
     S->prof.begin(CM_PROF_SPMV, st);
-    spmv_kernel<T, MODE><<<grid, CM_NT, smem_bytes<T, MODE>(), st>>>(A, x, y);
+    spmv_kernel<T, MODE><<<grid, CM_NT, 0, st>>>(A, x, y);
     S->prof.end(st);
     CM_CUDA(cudaGetLastError());
     return CM_OK;
@@ -473,12 +559,12 @@ template <typename T, int MODE>
 static int launch_cg(System<T> *S, CgArgs<T> &a, int prof_cls, cudaStream_t st)
 {
     int occ = 0;
-    CM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cg_kernel<T, MODE>, CM_NT, smem_bytes<T, MODE>()));
+    CM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cg_kernel<T, MODE>, CM_NT, 0));
     if (occ < 1) { cm_set_error("cg kernel does not fit on an SM"); return CM_E_CUDA; }
-    int grid = std::max(1, std::min({a.A.ntiles, occ * S->num_sms, S->grid_cap}));
+    int grid = std::max(1, std::min({a.A.nslices, occ * S->num_sms, S->grid_cap}));
     void *args[] = {&a};
     S->prof.begin(prof_cls, st);
-    cudaError_t e = cudaLaunchCooperativeKernel((void *)cg_kernel<T, MODE>, dim3(grid), dim3(CM_NT), args, smem_bytes<T, MODE>(), st);
+    cudaError_t e = cudaLaunchCooperativeKernel((void *)cg_kernel<T, MODE>, dim3(grid), dim3(CM_NT), args, 0, st);
     S->prof.end(st);
     if (e != cudaSuccess) { cm_set_error("cudaLaunchCooperativeKernel: %s", cudaGetErrorString(e)); return CM_E_CUDA; }
     return CM_OK;
@@ -491,7 +577,7 @@ int sys_cg(System<T> *S, cm_matrix_id id, int mode, const T *b, T *x, double tol
 {
     CgArgs<T> a;
     CM_TRY(make_view(S, id, mode, &a.A));
-    a.b = b; a.x = x; a.r = S->r; a.p = S->p; a.Ap = S->Ap; a.partial = S->partial;
+    a.b = b; a.x = x; a.r = S->r; a.p = S->p; a.p2 = S->p2; a.Ap = S->Ap; a.partial = S->partial;
     a.tol = tol; a.maxiter = maxiter; a.fixed = fixed; a.mask = mask; a.out = S->d_res + slot;
     switch (mode) {
     case MODE_CSR1: return launch_cg<T, MODE_CSR1>(S, a, prof_cls, st);
