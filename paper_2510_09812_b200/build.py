@@ -27,15 +27,19 @@ def needs_build() -> bool:
     return any(d.stat().st_mtime > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, defines: tuple = (), out: Path | None = None) -> Path:
+    """Compiles csrc/*.cu and links the shared library.  `defines` (e.g. ("CM_U_CSR1=4",)) and `out` build a tuning
+    variant beside the default library; load it with CUPYMAG_B200_LIB=<out>."""
+    if out is None and not defines and not force and not needs_build():
         return LIB
-    objdir = HERE / "build"
-    objdir.mkdir(exist_ok=True)
+    lib = Path(out) if out is not None else LIB
+    objdir = HERE / "build" / (lib.stem if out is not None else "default")
+    objdir.mkdir(parents=True, exist_ok=True)
+    dflags = [f"-D{d}" for d in defines]
 
     def compile_one(src: str) -> Path:
         obj = objdir / (src + ".o")
-        cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", str(CSRC / src), "-o", str(obj)]
+        cmd = [_nvcc(), *NVCC_FLAGS, *dflags, *(["-Xptxas", "-v"] if verbose else []), "-c", str(CSRC / src), "-o", str(obj)]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode:
             sys.stderr.write(r.stdout + r.stderr)
@@ -45,10 +49,12 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
-    cmd = [_nvcc(), "-shared", "-o", str(LIB), *map(str, objs), "-Xcompiler", "-fopenmp", "-lgomp"]
+    cmd = [_nvcc(), "-shared", "-o", str(lib), *map(str, objs), "-Xcompiler", "-fopenmp", "-lgomp"]
     subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    defs = tuple(a[2:] for a in sys.argv[1:] if a.startswith("-D"))
+    outs = [a.split("=", 1)[1] for a in sys.argv[1:] if a.startswith("--out=")]
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=defs, out=Path(outs[0]) if outs else None))

@@ -12,13 +12,12 @@
 // x[col] (L1 / L2 hits thanks to the locality ordering) and accumulates in registers in column order; the
 // 32 / C column phases of a row are combined with a fixed shuffle butterfly.  No shared memory, no atomics.
 //
-// CG.  ONE cooperative launch per solve with TWO grid-wide barriers per iteration (after each dot product).
-// A CTA owns a contiguous range of slices, hence of rows.  Per iteration k:
-//   C'  p_k = r_k + beta p_{k-1} on the CTA's own rows (into the other p buffer), CTA-local barrier;
-//   A   Ap = A p_k: columns inside the own range read p_k, columns outside (the halo) recompute
-//       fma(beta, p_{k-1}, r_k) from the two globally visible vectors -- bit-identical to what the owner wrote,
-//       which removes the third grid barrier of the textbook loop; dot p.Ap;               -> barrier, alpha
+// CG.  ONE cooperative launch per solve; a CTA owns a contiguous range of slices, hence of rows, for the whole
+// solve.  Per iteration k (three grid-wide barriers, the two dot products ride on two of them):
+//   C   p_k = r_k + beta p_{k-1} on the own rows (128-bit accesses);                       -> barrier
+//   A   Ap = A p_k, dot p.Ap;                                                              -> barrier, alpha
 //   B   x += alpha p, r -= alpha Ap, dot r.r;                                              -> barrier, beta
+// (CM_HALO selects a two-barrier variant that recomputes p on halo columns; measured slower, see below.)
 // Every CTA reduces the per-CTA partial sums in the same fixed order, so all CTAs take the same decisions and the
 // result is bit-reproducible run to run.  Dot products accumulate in fp64 in both precisions (R20).
 #include <cooperative_groups.h>
@@ -41,9 +40,31 @@ struct MatView {
 // NC vector components per node, NR independent right-hand sides, NV stored values per element, C rows per slice,
 // U 32-element iterations in flight per warp.
 template <int MODE> struct ModeTraits;
-template <> struct ModeTraits<MODE_CSR1> { static constexpr int NC = 1, NR = 1, NV = 1, C = CM_C_SCALAR, U = 8; };
-template <> struct ModeTraits<MODE_CSR3> { static constexpr int NC = 3, NR = 3, NV = 1, C = CM_C_SCALAR, U = 4; };
-template <> struct ModeTraits<MODE_BSR3> { static constexpr int NC = 3, NR = 1, NV = 9, C = CM_C_BLOCK, U = 2; };
+#ifndef CM_U_CSR1
+#define CM_U_CSR1 8
+#endif
+#ifndef CM_U_CSR3
+#define CM_U_CSR3 4
+#endif
+#ifndef CM_U_BSR3
+#define CM_U_BSR3 2
+#endif
+#ifndef CM_HALO
+// bit m set: the CG of mode m recomputes p = r + beta p_old on the columns outside the CTA's own rows instead of
+// waiting for their owners (two grid barriers per iteration instead of three).  Measured on B200 at 3M nodes, fp64,
+// algorithmic GB/s with / without: K^mech 5966 / 6185, K^ms 5020 / 6509, K^GS (3 rhs) 3868 / 4816 -- the extra
+// gather and the range test in the inner loop cost more than the ~3 us barrier, so it is off.
+#define CM_HALO 0
+#endif
+#ifndef CM_PIPELINE
+// bit m set: mode m issues the next batch's streaming loads before the current batch's gathers (two register
+// buffers).  Measured on B200 at 3M nodes: no gain for any mode (fp64 SpMV 91 % vs 95 % of the copy peak for CSR1,
+// register spills for BSR3), so it is off; the 24 resident warps per SM hide the gather latency by themselves.
+#define CM_PIPELINE 0
+#endif
+template <> struct ModeTraits<MODE_CSR1> { static constexpr int NC = 1, NR = 1, NV = 1, C = CM_C_SCALAR, U = CM_U_CSR1; };
+template <> struct ModeTraits<MODE_CSR3> { static constexpr int NC = 3, NR = 3, NV = 1, C = CM_C_SCALAR, U = CM_U_CSR3; };
+template <> struct ModeTraits<MODE_BSR3> { static constexpr int NC = 3, NR = 1, NV = 9, C = CM_C_BLOCK, U = CM_U_BSR3; };
 
 // ---- streaming loads of the matrix: read once per pass, so keep them out of L1 and first in line for L2 eviction
 __device__ __forceinline__ unsigned long long policy_evict_first()
@@ -144,85 +165,120 @@ __device__ __forceinline__ void fetch(const XSource<T, MODE, FUSED> &X, int col,
     }
 }
 
+// One batch = U consecutive 32-element groups of one slice: the unit of the load pipeline.
+template <typename T, int MODE>
+struct Batch {
+    int col[ModeTraits<MODE>::U];
+    T v[ModeTraits<MODE>::U][ModeTraits<MODE>::NV];
+};
+
+// position in the stream of batches of a warp: slice s with extent [b0, b0 + L), batch offset it
+struct Cursor {
+    int s, b0, L, it;
+};
+
+template <typename T, int MODE>
+__device__ __forceinline__ void load_batch(const MatView<T> &A, const Cursor &c, int lane, unsigned long long pol, Batch<T, MODE> &B)
+{
+    constexpr int NV = ModeTraits<MODE>::NV, U = ModeTraits<MODE>::U;
+    const int *colp = A.col + c.b0;
+    const T *valp = A.val + (long)NV * c.b0; // plane k at valp + k * L
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const int e = c.it + 32 * u + lane;
+        B.col[u] = 0;
+#pragma unroll
+        for (int k = 0; k < NV; k++) B.v[u][k] = 0;
+        if (e < c.L) {
+            B.col[u] = ld_stream(colp + e, pol);
+#pragma unroll
+            for (int k = 0; k < NV; k++) B.v[u][k] = ld_stream(valp + (long)k * c.L + e, pol);
+        }
+    }
+}
+
 // y = A x on the slices [u0, u1) of this CTA (warp w takes u0 + w, u0 + w + nwarps, ...); optionally accumulates
 // dot[c] += y.x over the rows written (x must then be valid on those rows: the own range when FUSED).
 template <typename T, int MODE, bool FUSED, bool DOT>
 __device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T, MODE, FUSED> &X, T *y, int u0, int u1, double (&dot)[3])
 {
-    constexpr int NC = ModeTraits<MODE>::NC, NV = ModeTraits<MODE>::NV, C = ModeTraits<MODE>::C, U = ModeTraits<MODE>::U;
+    constexpr int NC = ModeTraits<MODE>::NC, C = ModeTraits<MODE>::C, U = ModeTraits<MODE>::U;
+    constexpr bool PIPE = (CM_PIPELINE >> MODE) & 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int rl = lane % C, jl = lane / C;
     const unsigned long long pol = policy_evict_first();
-    int s = u0 + warp;
-    if (s >= u1) return;
-    int b0 = __ldg(A.sp + s), b1 = __ldg(A.sp + s + 1);
+    Cursor cur;
+    cur.s = u0 + warp;
+    if (cur.s >= u1) return;
+    cur.b0 = __ldg(A.sp + cur.s);
+    cur.L = __ldg(A.sp + cur.s + 1) - cur.b0;
+    cur.it = 0;
+    // extent of the slice after the current one, fetched one slice ahead
+    int n0 = 0, n1 = 0;
+    if (cur.s + nw < u1) { n0 = __ldg(A.sp + cur.s + nw); n1 = __ldg(A.sp + cur.s + nw + 1); }
+    Batch<T, MODE> Bc, Bn;
+    load_batch<T, MODE>(A, cur, lane, pol, Bc);
+    T acc[NC];
+#pragma unroll
+    for (int c = 0; c < NC; c++) acc[c] = 0;
     for (;;) {
-        const int sn = s + nw;
-        int n0 = 0, n1 = 0;
-        if (sn < u1) { n0 = __ldg(A.sp + sn); n1 = __ldg(A.sp + sn + 1); } // prefetch the next slice's extent
-        const int L = b1 - b0;
-        const int *colp = A.col + b0;
-        const T *valp = A.val + (long)NV * b0; // plane k at valp + k * L
-        T acc[NC];
+        // ---- advance the cursor and issue the next batch's streaming loads
+        Cursor nxt = cur;
+        nxt.it += 32 * U;
+        const bool last_of_slice = nxt.it >= cur.L;
+        if (last_of_slice) {
+            nxt.s = cur.s + nw; nxt.b0 = n0; nxt.L = n1 - n0; nxt.it = 0;
+            if (nxt.s + nw < u1) { n0 = __ldg(A.sp + nxt.s + nw); n1 = __ldg(A.sp + nxt.s + nw + 1); }
+        }
+        const bool more = nxt.s < u1;
+        if (PIPE && more) load_batch<T, MODE>(A, nxt, lane, pol, Bn);
+        // ---- current batch: dependent gathers, multiply-accumulate in column order
 #pragma unroll
-        for (int c = 0; c < NC; c++) acc[c] = 0;
-        for (int it = 0; it < L; it += 32 * U) {
-            int col[U];
-            T v[U][NV];
-            // all streaming loads of the batch first (U per array per lane in flight), then the dependent gathers
+        for (int u = 0; u < U; u++) {
+            const int e = cur.it + 32 * u + lane;
+            if (e < cur.L) {
+                T xv[NC];
+                fetch<T, MODE, FUSED>(X, Bc.col[u], xv);
+                if (MODE == MODE_BSR3) {
+                    acc[0] += Bc.v[u][0] * xv[0] + Bc.v[u][1] * xv[1] + Bc.v[u][2] * xv[2];
+                    acc[1] += Bc.v[u][3] * xv[0] + Bc.v[u][4] * xv[1] + Bc.v[u][5] * xv[2];
+                    acc[2] += Bc.v[u][6] * xv[0] + Bc.v[u][7] * xv[1] + Bc.v[u][8] * xv[2];
+                } else {
 #pragma unroll
-            for (int u = 0; u < U; u++) {
-                const int e = it + 32 * u + lane;
-                col[u] = 0;
-#pragma unroll
-                for (int k = 0; k < NV; k++) v[u][k] = 0;
-                if (e < L) {
-                    col[u] = ld_stream(colp + e, pol);
-#pragma unroll
-                    for (int k = 0; k < NV; k++) v[u][k] = ld_stream(valp + (long)k * L + e, pol);
+                    for (int c = 0; c < NC; c++) acc[c] += Bc.v[u][0] * xv[c];
                 }
             }
+        }
+        if (last_of_slice) {
+            // combine the 32 / C column phases of each row (fixed butterfly: every lane ends with the same sum)
 #pragma unroll
-            for (int u = 0; u < U; u++) {
-                const int e = it + 32 * u + lane;
-                if (e < L) {
-                    T xv[NC];
-                    fetch<T, MODE, FUSED>(X, col[u], xv);
-                    if (MODE == MODE_BSR3) {
-                        acc[0] += v[u][0] * xv[0] + v[u][1] * xv[1] + v[u][2] * xv[2];
-                        acc[1] += v[u][3] * xv[0] + v[u][4] * xv[1] + v[u][5] * xv[2];
-                        acc[2] += v[u][6] * xv[0] + v[u][7] * xv[1] + v[u][8] * xv[2];
-                    } else {
+            for (int o = C; o < 32; o <<= 1)
 #pragma unroll
-                        for (int c = 0; c < NC; c++) acc[c] += v[u][0] * xv[c];
+                for (int c = 0; c < NC; c++) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
+            const long row = (long)cur.s * C + rl;
+            if (row < A.N) {
+                if (MODE == MODE_BSR3) {
+                    // 32 / C = 4 >= 3 phases: phase jl writes component jl
+                    if (jl < 3) {
+                        const T a = jl == 0 ? acc[0] : (jl == 1 ? acc[1] : acc[2]);
+                        y[3 * row + jl] = a;
+                        if (DOT) dot[0] += (double)a * (double)X.x[3 * row + jl];
+                    }
+                } else if (jl == 0) {
+#pragma unroll
+                    for (int c = 0; c < NC; c++) {
+                        y[NC * row + c] = acc[c];
+                        if (DOT) dot[c] += (double)acc[c] * (double)X.x[NC * row + c];
                     }
                 }
             }
+#pragma unroll
+            for (int c = 0; c < NC; c++) acc[c] = 0;
         }
-        // combine the 32 / C column phases of each row (fixed butterfly: every lane ends with the same sum)
-#pragma unroll
-        for (int o = C; o < 32; o <<= 1)
-#pragma unroll
-            for (int c = 0; c < NC; c++) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
-        const long row = (long)s * C + rl;
-        if (row < A.N) {
-            if (MODE == MODE_BSR3) {
-                // 32 / C = 4 >= 3 phases: phase jl writes component jl
-                if (jl < 3) {
-                    const T a = jl == 0 ? acc[0] : (jl == 1 ? acc[1] : acc[2]);
-                    y[3 * row + jl] = a;
-                    if (DOT) dot[0] += (double)a * (double)X.x[3 * row + jl];
-                }
-            } else if (jl == 0) {
-#pragma unroll
-                for (int c = 0; c < NC; c++) {
-                    y[NC * row + c] = acc[c];
-                    if (DOT) dot[c] += (double)acc[c] * (double)X.x[NC * row + c];
-                }
-            }
-        }
-        if (sn >= u1) break;
-        s = sn; b0 = n0; b1 = n1;
+        if (!more) break;
+        cur = nxt;
+        if (PIPE) Bc = Bn;
+        else load_batch<T, MODE>(A, cur, lane, pol, Bc);
     }
 }
 
@@ -342,6 +398,30 @@ __device__ __forceinline__ void phase_xr(T *x, T *r, const T *p, const T *Ap, lo
 // --------------------------------------------------------------------------------------------------
 // persistent CG
 // --------------------------------------------------------------------------------------------------
+#ifdef CM_TRACE
+// tuning aid (not built by default): per-CTA phase time stamps of the first CM_TRACE_IT iterations
+constexpr int CM_TRACE_IT = 8;
+__device__ unsigned long long cm_trace_buf[2048 * CM_TRACE_IT * 4];
+__device__ __forceinline__ unsigned long long gtime()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ unsigned smid()
+{
+    unsigned s;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(s));
+    return s;
+}
+#define TRACE(k, slot) if (threadIdx.x == 0 && (k) < CM_TRACE_IT) cm_trace_buf[((long)blockIdx.x * CM_TRACE_IT + (k)) * 4 + (slot)] = (slot) == 3 ? (unsigned long long)smid() : gtime()
+extern "C" int cm_debug_trace(unsigned long long *host_out, long n)
+{
+    return cudaMemcpyFromSymbol(host_out, cm_trace_buf, n * sizeof(unsigned long long)) == cudaSuccess ? 0 : -1;
+}
+#else
+#define TRACE(k, slot)
+#endif
 template <typename T>
 struct CgArgs {
     MatView<T> A;
@@ -374,6 +454,7 @@ template <typename T, int MODE>
 __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
 {
     constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR, C = ModeTraits<MODE>::C;
+    constexpr bool HALO = (CM_HALO >> MODE) & 1;
     __shared__ double red[6 * 32];
     cg::grid_group grid = cg::this_grid();
     const int tid = threadIdx.x, nt = blockDim.x, nb = gridDim.x, bid = blockIdx.x;
@@ -447,21 +528,29 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         }
         if (!any) break;
         // ---- C': p_k on the own rows
+        TRACE(k, 0);
         phase_p<T, NR>(pnew, pold, a.r, e0, e1, beta);
-        __syncthreads();
-        // ---- A: Ap = A p_k (halo columns recomputed from r_k, p_{k-1}), pAp
         double s_pap[3] = {0, 0, 0};
-        {
+        if (HALO) {
+            __syncthreads();
+            // ---- A: Ap = A p_k (halo columns recomputed from r_k, p_{k-1}), pAp
             XSource<T, MODE, true> X;
             X.x = pnew; X.pold = pold; X.r = a.r; X.own0 = own0; X.own1 = own1;
 #pragma unroll
             for (int q = 0; q < NR; q++) X.beta[q] = beta[q];
             spmv_units<T, MODE, true, true>(a.A, X, a.Ap, u0, u1, s_pap);
+        } else {
+            grid.sync(); // textbook loop: p_k visible everywhere before the product
+            XSource<T, MODE, false> X;
+            X.x = pnew;
+            spmv_units<T, MODE, false, true>(a.A, X, a.Ap, u0, u1, s_pap);
         }
         block_sum<3>(s_pap, red);
         if (tid == 0)
             for (int q = 0; q < 3; q++) part(0)[q] = s_pap[q];
+        TRACE(k, 1);
         grid.sync();
+        TRACE(k, 3);
         double pap[NR];
         grid_sum<NR>(a.partial, 0, pap, red);
         T alpha[NR];
@@ -478,6 +567,7 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         block_sum<3>(snew, red);
         if (tid == 0)
             for (int q = 0; q < 3; q++) part(1)[q] = snew[q];
+        TRACE(k, 2);
         grid.sync();
         double rr_new[NR];
         grid_sum<NR>(a.partial, 1, rr_new, red);
