@@ -195,7 +195,7 @@ __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr
 template <typename T>
 System<T>::~System()
 {
-    T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, escr, sig, stg_m, stg_U, stg_u};
+    T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
     if (h_res) cudaFreeHost(h_res);
@@ -295,11 +295,11 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     T **vecs3[] = {&S->r, &S->p, &S->p2, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->f, &S->gn, &S->gs, &S->ms, &S->mss, &S->xin, &S->xout, &S->stg_m, &S->stg_u};
     for (T **v : vecs3) CM_TRY(alloc(v, 3 * N));
     CM_TRY(alloc(&S->U, N)); CM_TRY(alloc(&S->stg_U, N)); CM_TRY(alloc(&S->sig, 6 * N));
-    CM_TRY(alloc(&S->escr, 12 * Ne));
+    CM_TRY(alloc(&S->hpart, (size_t)6 * M->ck.nslots));
     S->grid_cap = S->num_sms * 8;
     CM_TRY(alloc(&S->partial, (size_t)4 * S->grid_cap * 3));
     CM_TRY(alloc(&S->d_res, 8));
-    CM_TRY(alloc(&S->red, (size_t)4096 * 16));
+    CM_TRY(alloc(&S->red, std::max<size_t>((size_t)4096 * 16, (size_t)8 * M->ck.nchunks)));
     CM_TRY(alloc(&S->dscal, 32));
     CM_CUDA(cudaMallocHost((void **)&S->h_res, 8 * sizeof(CgResult)));
     CM_CUDA(cudaMallocHost((void **)&S->h_scal, 32 * sizeof(double)));

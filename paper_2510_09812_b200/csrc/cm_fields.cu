@@ -2,10 +2,9 @@
 // deterministic gather-scatter right-hand sides, field recovery, the pointwise Gauss-Seidel algebra and the
 // projection; and the orchestration of one GSPM step (Alg. B.1).
 //
-// Scatter is deterministic: an element pass (one thread per tetrahedron, 128-bit connectivity load, SoA
-// gradients, 4 nodal gathers) writes per-element or per-(element, local node) contributions to a scratch
-// array; a node pass (one thread per node) sums its incident entries through the node->element CSR in
-// ascending element order.  No float atomics.
+// Scatter is deterministic: a chunk pass (one CTA per element chunk; nodal inputs and per-element contributions
+// staged in shared memory) reduces every chunk to one partial per local node ("slot"); a node pass sums a node's
+// slots in ascending chunk order.  No float atomics, no per-element scratch in HBM.
 #include <cmath>
 #include <cstring>
 #include <limits>
@@ -95,24 +94,43 @@ __global__ void permute_out_kernel(long N, int nc, const int *__restrict__ order
     user[(long)order[i] * nc + c] = lib[k];
 }
 
-// ---------------------------------------------------------------- element helpers
-template <typename T>
-struct Elem {
-    int t[4];
-    T V;
-    T g[4][3];
-};
+// ---------------------------------------------------------------- element passes (S3, S5, S6, S8)
+// One CTA per element chunk (cm_internal.h).  Phase 0 stages the chunk's nodal inputs in shared memory (one
+// global gather per local node instead of one per element corner).  Phase 1, one thread per tetrahedron: coalesced
+// loads of the local ids, V_e and the nine stored gradient words (grad phi_0 = -sum of the others, O-1), compute,
+// contributions to shared memory.  Phase 2, one thread per local node: sums the node's incidences inside the chunk
+// in ascending element order and writes ONE partial per slot.  A node pass then adds a node's slots in ascending
+// chunk order -- a deterministic gather end to end, no float atomics, and no per-element scratch in HBM.
+enum ElemKind { EK_MS = 0, EK_GRADU = 1, EK_MECH = 2, EK_STRESS = 3 };
+// NIN staged words per node, NOUT shared-memory words per element, NC words per slot, PERK: contribution depends on
+// the local node index k (NOUT = 4 NC) or is the same for the 4 nodes (NOUT = NC).
+template <int KIND> struct KindTraits;
+template <> struct KindTraits<EK_MS> { static constexpr int NIN = 3, NOUT = 4, NC = 1; static constexpr bool PERK = true; };
+template <> struct KindTraits<EK_GRADU> { static constexpr int NIN = 1, NOUT = 3, NC = 3; static constexpr bool PERK = false; };
+template <> struct KindTraits<EK_MECH> { static constexpr int NIN = 3, NOUT = 12, NC = 3; static constexpr bool PERK = true; };
+template <> struct KindTraits<EK_STRESS> { static constexpr int NIN = 6, NOUT = 6, NC = 6; static constexpr bool PERK = false; };
+
+constexpr int EK_NT = 256;
 
 template <typename T>
-__device__ __forceinline__ void load_elem(long e, long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
-                                          Elem<T> &E)
+struct ChunkArgs {
+    const int *eptr, *nptr, *nodes;
+    const unsigned short *lid, *lptr, *lent, *emat;
+    const T *V, *G; // G: 12 planes [3k + d][Ne]; planes 3..11 are read
+    long Ne;
+    const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w
+    const double *mbar;   // MS
+    const T *Cstar;       // MECH, STRESS
+    T l1, l2;
+    T *hpart;             // [slot][NC]
+    double *partial;      // GRADU: per-chunk sums of V_e grad U_e (fp64)
+};
+
+template <int KIND, typename T>
+constexpr size_t chunk_smem_bytes()
 {
-    *reinterpret_cast<int4 *>(E.t) = __ldg(reinterpret_cast<const int4 *>(tets) + e);
-    E.V = __ldg(V + e);
-#pragma unroll
-    for (int k = 0; k < 4; k++)
-#pragma unroll
-        for (int d = 0; d < 3; d++) E.g[k][d] = __ldg(G + (long)(3 * k + d) * Ne + e);
+    return (size_t)(CM_NL_MAX * KindTraits<KIND>::NIN + CM_EC_MAX * KindTraits<KIND>::NOUT) * sizeof(T) +
+           (size_t)(CM_NL_MAX + 2 + 4 * CM_EC_MAX) * sizeof(unsigned short);
 }
 
 // E0(m), Table A.1, Voigt engineering vector (E11, E22, E33, 2 E23, 2 E13, 2 E12)
@@ -128,14 +146,16 @@ __device__ __forceinline__ void E0_voigt(const T *m, T l1, T l2, T e0[6])
     e0[5] = (T)2 * th * l2 * m[0] * m[1];
 }
 
-template <typename T>
-__device__ __forceinline__ void mean_E0(const T *__restrict__ w, const int *t, T l1, T l2, T e0[6])
+// mean over the 4 corners of E0(w); w_k = sw[ST * l[k] + OFF ..]
+template <typename T, int ST, int OFF>
+__device__ __forceinline__ void mean_E0(const T *sw, const int *l, T l1, T l2, T e0[6])
 {
 #pragma unroll
     for (int q = 0; q < 6; q++) e0[q] = 0;
 #pragma unroll
     for (int k = 0; k < 4; k++) {
-        T mk[3] = {w[3 * (long)t[k]], w[3 * (long)t[k] + 1], w[3 * (long)t[k] + 2]}, ek[6];
+        const T *w = sw + ST * l[k] + OFF;
+        T mk[3] = {w[0], w[1], w[2]}, ek[6];
         E0_voigt(mk, l1, l2, ek);
 #pragma unroll
         for (int q = 0; q < 6; q++) e0[q] += ek[q];
@@ -156,27 +176,132 @@ __device__ __forceinline__ void C_times(const T *__restrict__ C, const T eps[6],
     }
 }
 
-// ---------------------------------------------------------------- S3 magnetostatic RHS
-// element pass: contribution of tet e to its 4 nodes, c_k = V_e grad phi_k . (mean_e m - mbar)
-template <typename T>
-__global__ void elem_ms_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
-                               const T *__restrict__ m, const double *__restrict__ mbar, T *scr)
+template <typename T, int KIND>
+__global__ void __launch_bounds__(EK_NT) elem_chunk_kernel(ChunkArgs<T> a)
 {
-    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (e >= Ne) return;
-    Elem<T> E;
-    load_elem(e, Ne, tets, V, G, E);
-    T mt[3];
+    typedef KindTraits<KIND> K;
+    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *sin = reinterpret_cast<T *>(smem_raw);               // [nl][NIN]
+    T *scr = sin + CM_NL_MAX * NIN;                         // [NOUT][EC]
+    unsigned short *slp = reinterpret_cast<unsigned short *>(scr + EC * NOUT); // [nl + 1]
+    unsigned short *sle = slp + CM_NL_MAX + 2;              // [4 ne], 4-byte aligned
+    const int c = blockIdx.x, tid = threadIdx.x;
+    const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
+
+    // ---- phase 0: nodal inputs, incidence runs
+    for (int l = tid; l < nl; l += EK_NT) {
+        const long g = a.nodes[s0 + l];
+        if (KIND == EK_GRADU) {
+            sin[l] = a.in0[g];
+        } else {
 #pragma unroll
-    for (int d = 0; d < 3; d++)
-        mt[d] = (m[3 * (long)E.t[0] + d] + m[3 * (long)E.t[1] + d] + m[3 * (long)E.t[2] + d] + m[3 * (long)E.t[3] + d]) / (T)4 - (T)mbar[d];
+            for (int d = 0; d < 3; d++) sin[NIN * l + d] = a.in0[3 * g + d];
+            if (KIND == EK_STRESS)
 #pragma unroll
-    for (int k = 0; k < 4; k++) scr[4 * e + k] = E.V * (E.g[k][0] * mt[0] + E.g[k][1] * mt[1] + E.g[k][2] * mt[2]);
+                for (int d = 0; d < 3; d++) sin[NIN * l + 3 + d] = a.in1[3 * g + d];
+        }
+    }
+    for (int l = tid; l <= nl; l += EK_NT) slp[l] = a.lptr[s0 + c + l];
+    {
+        // 4 ne incidences; e0 * 4 entries of 2 bytes: 8-byte aligned rows, copied as 32-bit pairs
+        const unsigned *src = reinterpret_cast<const unsigned *>(a.lent + 4L * e0);
+        unsigned *dst = reinterpret_cast<unsigned *>(sle);
+        for (int q = tid; q < 2 * ne; q += EK_NT) dst[q] = __ldg(src + q);
+    }
+    __syncthreads();
+
+    // ---- phase 1: one thread per tetrahedron
+    double gsum[3] = {0, 0, 0};
+    for (int el = tid; el < ne; el += EK_NT) {
+        const long e = e0 + el;
+        const ushort4 lq = __ldg(reinterpret_cast<const ushort4 *>(a.lid) + e);
+        const int l[4] = {lq.x, lq.y, lq.z, lq.w};
+        const T V = __ldg(a.V + e);
+        T g[4][3];
+#pragma unroll
+        for (int k = 1; k < 4; k++)
+#pragma unroll
+            for (int d = 0; d < 3; d++) g[k][d] = __ldg(a.G + (long)(3 * k + d) * a.Ne + e);
+#pragma unroll
+        for (int d = 0; d < 3; d++) g[0][d] = -(g[1][d] + g[2][d] + g[3][d]);
+
+        if (KIND == EK_MS) {
+            // c_k = V_e grad phi_k . (mean_e m - mbar)
+            T mt[3];
+#pragma unroll
+            for (int d = 0; d < 3; d++)
+                mt[d] = (sin[3 * l[0] + d] + sin[3 * l[1] + d] + sin[3 * l[2] + d] + sin[3 * l[3] + d]) / (T)4 - (T)a.mbar[d];
+#pragma unroll
+            for (int k = 0; k < 4; k++) scr[k * EC + el] = V * (g[k][0] * mt[0] + g[k][1] * mt[1] + g[k][2] * mt[2]);
+        } else if (KIND == EK_GRADU) {
+            // V_e grad U_e, and its fp64 sum for <grad U>
+            const T u0 = sin[l[0]], u1 = sin[l[1]], u2 = sin[l[2]], u3 = sin[l[3]];
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                const T gU = u0 * g[0][d] + u1 * g[1][d] + u2 * g[2][d] + u3 * g[3][d];
+                scr[d * EC + el] = V * gU;
+                gsum[d] += (double)V * (double)gU;
+            }
+        } else {
+            const unsigned em = __ldg(a.emat + e);
+            if (!(em & 1u)) {
+#pragma unroll
+                for (int q = 0; q < NOUT; q++) scr[q * EC + el] = 0;
+            } else if (KIND == EK_MECH) {
+                // S = C*_e : mean_e E0(m);  c_(k,a) = V_e (S grad phi_k)_a
+                T e0v[6], sg[6];
+                mean_E0<T, 3, 0>(sin, l, a.l1, a.l2, e0v);
+                C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
+#pragma unroll
+                for (int k = 0; k < 4; k++) {
+                    scr[(3 * k + 0) * EC + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
+                    scr[(3 * k + 1) * EC + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
+                    scr[(3 * k + 2) * EC + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
+                }
+            } else {
+                // V_e C*_e : (E_e(u) - mean_e E0(w)),  H[a][b] = d_b u_a
+                T H[3][3];
+#pragma unroll
+                for (int x = 0; x < 3; x++)
+#pragma unroll
+                    for (int y = 0; y < 3; y++) {
+                        T acc = 0;
+#pragma unroll
+                        for (int k = 0; k < 4; k++) acc += sin[6 * l[k] + x] * g[k][y];
+                        H[x][y] = acc;
+                    }
+                T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]}, e0v[6], sg[6];
+                mean_E0<T, 6, 3>(sin, l, a.l1, a.l2, e0v);
+#pragma unroll
+                for (int q = 0; q < 6; q++) eps[q] -= e0v[q];
+                C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+#pragma unroll
+                for (int q = 0; q < 6; q++) scr[q * EC + el] = V * sg[q];
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 2: one thread per local node, incidences in ascending element order
+    for (int l = tid; l < nl; l += EK_NT) {
+        T acc[NC];
+#pragma unroll
+        for (int q = 0; q < NC; q++) acc[q] = 0;
+        for (int q = slp[l]; q < slp[l + 1]; q++) {
+            const int ent = sle[q], el = ent >> 2, k = ent & 3;
+#pragma unroll
+            for (int x = 0; x < NC; x++) acc[x] += scr[(K::PERK ? NC * k + x : x) * EC + el];
+        }
+#pragma unroll
+        for (int x = 0; x < NC; x++) a.hpart[(long)(s0 + l) * NC + x] = acc[x];
+    }
+    if (KIND == EK_GRADU) block_reduce_write<3>(gsum, a.partial);
 }
 
-// node pass: b_i = sum over incident (e,k) of scr[(4e+k) * NC + c]; zero where mask says so
+// node pass: b_i = sum of the node's slot partials (ascending chunk order); zero where the mask says so
 template <typename T, int NC>
-__global__ void node_gather_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const T *__restrict__ scr,
+__global__ void node_gather_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                    const uchar *__restrict__ zero_mask /* N*NC or NULL */, int zero_node, T *b)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -184,10 +309,10 @@ __global__ void node_gather_kernel(long N, const int *__restrict__ n2e_ptr, cons
     T acc[NC];
 #pragma unroll
     for (int c = 0; c < NC; c++) acc[c] = 0;
-    for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
-        const long q = __ldg(n2e + s);
+    for (int s = ns_ptr[i]; s < ns_ptr[i + 1]; s++) {
+        const long q = __ldg(ns_slot + s);
 #pragma unroll
-        for (int c = 0; c < NC; c++) acc[c] += scr[q * NC + c];
+        for (int c = 0; c < NC; c++) acc[c] += hpart[q * NC + c];
     }
 #pragma unroll
     for (int c = 0; c < NC; c++) {
@@ -197,32 +322,11 @@ __global__ void node_gather_kernel(long N, const int *__restrict__ n2e_ptr, cons
     }
 }
 
-// ---------------------------------------------------------------- S5 gradient recovery
-// element pass: scr[e][0..2] = V_e grad U_e ; block partial sums of the same (fp64) for <grad U>
+// node pass of S5: h_d,i = -sum_{e} V_e grad U_e / (4 mL_i) + <grad U>   (DEMAG)   - N_d mbar   (FARFIELD)
 template <typename T>
-__global__ void elem_gradU_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
-                                  const T *__restrict__ U, T *scr, double *partial)
-{
-    double acc[3] = {0, 0, 0};
-    for (long e = blockIdx.x * (long)blockDim.x + threadIdx.x; e < Ne; e += (long)gridDim.x * blockDim.x) {
-        Elem<T> E;
-        load_elem(e, Ne, tets, V, G, E);
-        const T u0 = U[E.t[0]], u1 = U[E.t[1]], u2 = U[E.t[2]], u3 = U[E.t[3]];
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            const T gU = u0 * E.g[0][d] + u1 * E.g[1][d] + u2 * E.g[2][d] + u3 * E.g[3][d];
-            scr[3 * e + d] = E.V * gU;
-            acc[d] += (double)E.V * (double)gU;
-        }
-    }
-    block_reduce_write<3>(acc, partial);
-}
-
-// node pass: h_d,i = -sum_{e} V_e grad U_e / (4 mL_i) + <grad U>   (DEMAG)   - N_d mbar   (FARFIELD)
-template <typename T>
-__global__ void node_hd_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const T *__restrict__ scr,
+__global__ void node_hd_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                const T *__restrict__ mL, const double *__restrict__ scal /* mbar[0..2], gradU mean[3..5] */,
-                               double Vtot_inv_unused, unsigned terms, double n00, double n01, double n02, double n10, double n11,
+                               unsigned terms, double n00, double n01, double n02, double n10, double n11,
                                double n12, double n20, double n21, double n22, T *hd)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -230,10 +334,10 @@ __global__ void node_hd_kernel(long N, const int *__restrict__ n2e_ptr, const in
     T h[3] = {0, 0, 0};
     if (terms & CM_TERM_DEMAG) {
         T acc[3] = {0, 0, 0};
-        for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
-            const long e = __ldg(n2e + s) >> 2;
+        for (int s = ns_ptr[i]; s < ns_ptr[i + 1]; s++) {
+            const long q = __ldg(ns_slot + s);
 #pragma unroll
-            for (int d = 0; d < 3; d++) acc[d] += scr[3 * e + d];
+            for (int d = 0; d < 3; d++) acc[d] += hpart[3 * q + d];
         }
         const T den = (T)4 * mL[i];
 #pragma unroll
@@ -248,74 +352,11 @@ __global__ void node_hd_kernel(long N, const int *__restrict__ n2e_ptr, const in
     hd[3 * i] = h[0]; hd[3 * i + 1] = h[1]; hd[3 * i + 2] = h[2];
 }
 
-// ---------------------------------------------------------------- S6 mechanical RHS
-// element pass (magnetic tets): S = C*_e : mean_e E0(m);  scr[(4e+k)*3 + a] = V_e (S grad phi_k)_a
-template <typename T>
-__global__ void elem_mech_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
-                                 const uchar *__restrict__ mag, const int *__restrict__ eid, const T *__restrict__ Cstar,
-                                 const T *__restrict__ m, T l1, T l2, T *scr)
-{
-    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (e >= Ne) return;
-    if (!mag[e]) {
-#pragma unroll
-        for (int q = 0; q < 12; q++) scr[12 * e + q] = 0;
-        return;
-    }
-    Elem<T> E;
-    load_elem(e, Ne, tets, V, G, E);
-    T e0[6], s[6];
-    mean_E0(m, E.t, l1, l2, e0);
-    C_times(Cstar + 36 * eid[e], e0, s);
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        const T *g = E.g[k];
-        scr[12 * e + 3 * k + 0] = E.V * (s[0] * g[0] + s[5] * g[1] + s[4] * g[2]);
-        scr[12 * e + 3 * k + 1] = E.V * (s[5] * g[0] + s[1] * g[1] + s[3] * g[2]);
-        scr[12 * e + 3 * k + 2] = E.V * (s[4] * g[0] + s[3] * g[1] + s[2] * g[2]);
-    }
-}
-
-// ---------------------------------------------------------------- S8 stress recovery
-// element pass (magnetic tets): scr[e][0..5] = V_e C*_e : (E_e(u) - mean_e E0(w))
-template <typename T>
-__global__ void elem_stress_kernel(long Ne, const int *__restrict__ tets, const T *__restrict__ V, const T *__restrict__ G,
-                                   const uchar *__restrict__ mag, const int *__restrict__ eid, const T *__restrict__ Cstar,
-                                   const T *__restrict__ u, const T *__restrict__ w, T l1, T l2, T *scr)
-{
-    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (e >= Ne) return;
-    if (!mag[e]) {
-#pragma unroll
-        for (int q = 0; q < 6; q++) scr[6 * e + q] = 0;
-        return;
-    }
-    Elem<T> E;
-    load_elem(e, Ne, tets, V, G, E);
-    T H[3][3]; // H[a][b] = d_b u_a
-#pragma unroll
-    for (int a = 0; a < 3; a++)
-#pragma unroll
-        for (int b = 0; b < 3; b++) {
-            T acc = 0;
-#pragma unroll
-            for (int k = 0; k < 4; k++) acc += u[3 * (long)E.t[k] + a] * E.g[k][b];
-            H[a][b] = acc;
-        }
-    T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]}, e0[6], s[6];
-    mean_E0(w, E.t, l1, l2, e0);
-#pragma unroll
-    for (int q = 0; q < 6; q++) eps[q] -= e0[q];
-    C_times(Cstar + 36 * eid[e], eps, s);
-#pragma unroll
-    for (int q = 0; q < 6; q++) scr[6 * e + q] = E.V * s[q];
-}
-
 // ---------------------------------------------------------------- S9 nodal field
-// node pass: sigma_hat_i (gathered from scr when MAGEL), h = h_an + h_ext + h_d + h_me on live nodes;
-// optionally also writes sigma_hat (parity output).
+// node pass: sigma_hat_i (from the slot partials of the stress pass when MAGEL), h = h_an + h_ext + h_d + h_me on
+// live nodes; optionally also writes sigma_hat (parity output).
 template <typename T>
-__global__ void node_field_kernel(long N, const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const T *__restrict__ scr,
+__global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                   const T *__restrict__ mLm, const uchar *__restrict__ live, const T *__restrict__ w,
                                   const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, T l1, T l2, T *h, T *sig_out)
 {
@@ -332,10 +373,10 @@ __global__ void node_field_kernel(long N, const int *__restrict__ n2e_ptr, const
         if (terms & CM_TERM_ZEEMAN) { hi[0] += hx; hi[1] += hy; hi[2] += hz; }
         if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) { hi[0] += hd[3 * i]; hi[1] += hd[3 * i + 1]; hi[2] += hd[3 * i + 2]; }
         if (terms & CM_TERM_MAGEL) {
-            for (int q = n2e_ptr[i]; q < n2e_ptr[i + 1]; q++) {
-                const long e = __ldg(n2e + q) >> 2;
+            for (int q = ns_ptr[i]; q < ns_ptr[i + 1]; q++) {
+                const long sl = __ldg(ns_slot + q);
 #pragma unroll
-                for (int c = 0; c < 6; c++) s[c] += scr[6 * e + c];
+                for (int c = 0; c < 6; c++) s[c] += hpart[6 * sl + c];
             }
             const T den = (T)4 * mLm[i];
 #pragma unroll
@@ -469,12 +510,40 @@ int sys_mbar(System<T> *S, const T *m_lib, cudaStream_t st)
 }
 
 template <typename T>
+static ChunkArgs<T> chunk_args(System<T> *S)
+{
+    const cm_mesh *M = S->mesh;
+    const Chunks &K = M->ck;
+    ChunkArgs<T> a;
+    a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
+    a.emat = M->d_emat; a.V = S->V; a.G = S->G; a.Ne = S->Ne;
+    a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
+    a.hpart = S->hpart; a.partial = S->red;
+    return a;
+}
+
+template <typename T, int KIND>
+static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
+{
+    constexpr size_t smem = chunk_smem_bytes<KIND, T>();
+    static bool configured = false; // per instantiation; the attribute is per function, so once is enough
+    if (!configured) {
+        CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = true;
+    }
+    elem_chunk_kernel<T, KIND><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(a);
+    return CM_OK;
+}
+
+template <typename T>
 int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
 {
-    cm_mesh *M = S->mesh;
+    const Chunks &K = S->mesh->ck;
+    ChunkArgs<T> a = chunk_args(S);
+    a.in0 = m_lib;
     S->prof.begin(CM_PROF_ELEMENT, st, 2);
-    elem_ms_kernel<T><<<nblk(S->Ne), BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, m_lib, S->dscal, S->escr);
-    node_gather_kernel<T, 1><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, nullptr, S->pin, b);
+    CM_TRY((launch_chunks<T, EK_MS>(S, a, st)));
+    node_gather_kernel<T, 1><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, nullptr, S->pin, b);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -483,15 +552,16 @@ int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
 template <typename T>
 int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStream_t st)
 {
-    cm_mesh *M = S->mesh;
+    const Chunks &K = S->mesh->ck;
     S->prof.begin(CM_PROF_ELEMENT, st, (terms & CM_TERM_DEMAG) ? 3 : 1);
     if (terms & CM_TERM_DEMAG) {
-        const int nb = (int)std::min<long>(RED_BLOCKS, nblk(S->Ne));
-        elem_gradU_kernel<T><<<nb, BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, U_lib, S->escr, S->red);
-        reduce_final_kernel<<<1, 1024, 0, st>>>(nb, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
+        ChunkArgs<T> a = chunk_args(S);
+        a.in0 = U_lib;
+        CM_TRY((launch_chunks<T, EK_GRADU>(S, a, st)));
+        reduce_final_kernel<<<1, 1024, 0, st>>>(K.nchunks, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
     }
     const double *n = S->Nd;
-    node_hd_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, S->mL, S->dscal, 0.0, terms, n[0], n[1], n[2], n[3],
+    node_hd_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mL, S->dscal, terms, n[0], n[1], n[2], n[3],
                                                  n[4], n[5], n[6], n[7], n[8], hd);
     S->prof.end(st);
     LAUNCH_CHECK();
@@ -501,12 +571,13 @@ int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStr
 template <typename T>
 int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
 {
-    cm_mesh *M = S->mesh;
+    const Chunks &K = S->mesh->ck;
     if (!S->n_elastic) { cm_set_error("mechanics requested but the material has no elastic constants"); return CM_E_BADARG; }
+    ChunkArgs<T> a = chunk_args(S);
+    a.in0 = m_lib;
     S->prof.begin(CM_PROF_ELEMENT, st, 2);
-    elem_mech_kernel<T><<<nblk(S->Ne), BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, M->d_mag, M->d_eid, S->Cstar, m_lib, (T)S->lam100,
-                                                   (T)S->lam111, S->escr);
-    node_gather_kernel<T, 3><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, S->clamp, -1, b);
+    CM_TRY((launch_chunks<T, EK_MECH>(S, a, st)));
+    node_gather_kernel<T, 3><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->clamp, -1, b);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -515,11 +586,11 @@ int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
 template <typename T>
 int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st)
 {
-    cm_mesh *M = S->mesh;
     if (!S->n_elastic) { cm_set_error("mechanics requested but the material has no elastic constants"); return CM_E_BADARG; }
+    ChunkArgs<T> a = chunk_args(S);
+    a.in0 = u_lib; a.in1 = w_lib;
     S->prof.begin(CM_PROF_ELEMENT, st);
-    elem_stress_kernel<T><<<nblk(S->Ne), BS, 0, st>>>(S->Ne, M->d_tets, S->V, S->G, M->d_mag, M->d_eid, S->Cstar, u_lib, w_lib,
-                                                     (T)S->lam100, (T)S->lam111, S->escr);
+    CM_TRY((launch_chunks<T, EK_STRESS>(S, a, st)));
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -528,9 +599,9 @@ int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st)
 template <typename T>
 int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h, T *sig_out, cudaStream_t st)
 {
-    cm_mesh *M = S->mesh;
+    const Chunks &K = S->mesh->ck;
     S->prof.begin(CM_PROF_ELEMENT, st);
-    node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, M->d_n2e_ptr, M->d_n2e, S->escr, S->mLm, S->live, w_lib, hd, terms,
+    node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mLm, S->live, w_lib, hd, terms,
                                                    (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], (T)S->lam100, (T)S->lam111, h,
                                                    sig_out);
     S->prof.end(st);

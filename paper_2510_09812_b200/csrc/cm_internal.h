@@ -49,6 +49,26 @@ struct Sell {
     int *d_sp = nullptr, *d_col = nullptr;
 };
 
+// Element chunks for the assembly passes (S3, S5, S6, S8): consecutive elements are cut into chunks of at most
+// CM_EC_MAX elements that reference at most CM_NL_MAX distinct nodes.  A chunk numbers its nodes locally (sorted by
+// global id); "slot" nptr[c] + l is local node l of chunk c, and every slot owns one partial sum per pass.
+//   eptr[c]            first element of chunk c
+//   nptr[c]            first slot of chunk c;  nodes[slot] = global node id
+//   lid[4 e + k]       local id of node k of element e within its chunk
+//   lptr[slot + c]     start of the slot's run in the chunk's incidence list (runs of chunk c end at lptr[nptr[c+1] + c])
+//   lent[4 eptr[c] + q] incidence q of chunk c: 4 * (e - eptr[c]) + k, ascending inside every run
+//   ns_ptr / ns_slot   node -> its slots, ascending (so ascending chunk = ascending element order)
+constexpr int CM_EC_MAX = 768;
+constexpr int CM_NL_MAX = 768;
+struct Chunks {
+    int nchunks = 0;
+    long nslots = 0;
+    std::vector<int> eptr, nptr, nodes, ns_ptr, ns_slot;
+    std::vector<unsigned short> lid, lptr, lent;
+    int *d_eptr = nullptr, *d_nptr = nullptr, *d_nodes = nullptr, *d_ns_ptr = nullptr, *d_ns_slot = nullptr;
+    unsigned short *d_lid = nullptr, *d_lptr = nullptr, *d_lent = nullptr;
+};
+
 struct cm_mesh {
     long N = 0, Ne = 0, nnz = 0;
     bool identity = true;
@@ -63,6 +83,9 @@ struct cm_mesh {
     uchar *d_mag = nullptr;
     double *d_xyz = nullptr, *d_wvol = nullptr;
     Sell sell[2];              // [0]: C = CM_C_SCALAR, [1]: C = CM_C_BLOCK
+    Chunks ck;
+    std::vector<unsigned short> emat; // per element: elastic id << 1 | magnetic flag
+    unsigned short *d_emat = nullptr;
     // scratch for cm_volume_average
     double *d_red = nullptr;   // partials
     void *d_tmp = nullptr;     // N x 16 x 8 bytes? (allocated lazily, see cm_volume_average)
@@ -128,7 +151,7 @@ struct System : SystemBase {
       *ms = nullptr, *mss = nullptr, *xin = nullptr, *xout = nullptr;
     T *sig = nullptr;                                        // N x 6 parity output of CM_OUT_SIGMA
     T *stg_m = nullptr, *stg_U = nullptr, *stg_u = nullptr;  // device staging of the host-buffer step
-    T *escr = nullptr;     // element scratch, 12 Ne
+    T *hpart = nullptr;    // per-slot partial sums of the element passes, 6 per slot
     double *red = nullptr; // reduction partials
     double *dscal = nullptr, *h_scal = nullptr; // device / pinned scalars: mbar[3], gradU mean[3], dm sum, ...
     ~System();
@@ -138,6 +161,7 @@ struct System : SystemBase {
 int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long Ne, const uchar *mag, const int *eid,
                     cm_reorder reorder);
 int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out);
+int build_chunks(long N, long Ne, const int *tets, Chunks *out);
 
 // ---- kernels (templated launchers; defined in the .cu files, instantiated for float and double) ----
 template <typename T> int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, long pin_user, cudaStream_t st);
@@ -151,9 +175,9 @@ template <typename T> int sys_mbar(System<T> *S, const T *m_lib, cudaStream_t st
 template <typename T> int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st);                 // uses dscal[0..2]
 template <typename T> int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStream_t st);
 template <typename T> int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st);
-template <typename T> int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st);       // -> escr (V sigma per element)
+template <typename T> int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st);       // -> hpart (V sigma per slot)
 template <typename T> int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h,
-                                    T *sig_out, cudaStream_t st);                                          // gathers escr when MAGEL
+                                    T *sig_out, cudaStream_t st);                                          // gathers hpart when MAGEL
 template <typename T> int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_user, cm_step_info *info,
                                    cudaStream_t st);
 template <typename T> int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t st);

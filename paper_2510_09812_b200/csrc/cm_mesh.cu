@@ -233,6 +233,12 @@ int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long
     M->nnz = M->rowptr[N];
     if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
     if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
+    CM_TRY(build_chunks(N, Ne, M->tets.data(), &M->ck));
+    M->emat.resize(Ne);
+    for (long e = 0; e < Ne; e++) {
+        if (M->eid[e] < 0 || M->eid[e] > 0x7ffe) { cm_set_error("cm_mesh_create: elastic_id %d outside [0, 32766]", M->eid[e]); return CM_E_INDEX_RANGE; }
+        M->emat[e] = (unsigned short)(M->eid[e] << 1 | (M->mag[e] ? 1 : 0));
+    }
     return CM_OK;
 }
 
@@ -265,6 +271,78 @@ int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &c
             for (int j = 0; j < w; j++) out->col[b + (long)j * C + rl] = j < len ? col[rowptr[i] + j] : (int)ic;
         }
     }
+    return CM_OK;
+}
+
+// Element chunks (cm_internal.h): greedy cut of the element sequence, local numbering, per-chunk incidence lists and
+// the node -> slot transpose.  Elements are sorted by their smallest node id, so with a locality ordering a chunk
+// touches a compact node set (about 230 nodes per 768 elements on the paper's meshes).
+int build_chunks(long N, long Ne, const int *tets, Chunks *out)
+{
+    Chunks &K = *out;
+    K.eptr.assign(1, 0);
+    K.nptr.assign(1, 0);
+    K.nodes.clear();
+    K.nodes.reserve(Ne / 2 + 16);
+    // pass 1 (sequential): chunk boundaries and the nodes of every chunk in first-seen order
+    std::vector<int> stamp(N, -1);
+    int cur = 0, ne = 0, nl = 0;
+    for (long e = 0; e < Ne; e++) {
+        int fresh = 0;
+        for (int k = 0; k < 4; k++) {
+            const int v = tets[4 * e + k];
+            bool dup = stamp[v] == cur;
+            for (int j = 0; j < k && !dup; j++) dup = tets[4 * e + j] == v;
+            fresh += !dup;
+        }
+        if (ne + 1 > CM_EC_MAX || nl + fresh > CM_NL_MAX) {
+            K.eptr.push_back((int)e);
+            K.nptr.push_back((int)K.nodes.size());
+            cur++; ne = 0; nl = 0;
+        }
+        for (int k = 0; k < 4; k++) {
+            const int v = tets[4 * e + k];
+            if (stamp[v] != cur) { stamp[v] = cur; K.nodes.push_back(v); nl++; }
+        }
+        ne++;
+    }
+    K.eptr.push_back((int)Ne);
+    K.nptr.push_back((int)K.nodes.size());
+    K.nchunks = (int)K.eptr.size() - 1;
+    K.nslots = (long)K.nodes.size();
+    if (K.nslots > 0x7fffffffL / 8) { cm_set_error("cm_mesh_create: too many chunk slots for 32-bit offsets"); return CM_E_BADARG; }
+    // pass 2 (parallel over chunks): sort the local nodes, local ids, incidence runs
+    K.lid.resize(4 * Ne);
+    K.lent.resize(4 * Ne);
+    K.lptr.assign(K.nslots + K.nchunks, 0);
+#pragma omp parallel
+    {
+        std::vector<int> cnt;
+#pragma omp for schedule(dynamic, 64)
+        for (int c = 0; c < K.nchunks; c++) {
+            const int s0 = K.nptr[c], n = K.nptr[c + 1] - s0, e0 = K.eptr[c], m = K.eptr[c + 1] - e0;
+            int *nd = K.nodes.data() + s0;
+            std::sort(nd, nd + n);
+            cnt.assign(n + 1, 0);
+            for (long q = 4L * e0; q < 4L * (e0 + m); q++) {
+                const int l = (int)(std::lower_bound(nd, nd + n, tets[q]) - nd);
+                K.lid[q] = (unsigned short)l;
+                cnt[l + 1]++;
+            }
+            for (int l = 0; l < n; l++) cnt[l + 1] += cnt[l];
+            unsigned short *lp = K.lptr.data() + s0 + c;
+            for (int l = 0; l <= n; l++) lp[l] = (unsigned short)cnt[l];
+            unsigned short *le = K.lent.data() + 4L * e0;
+            for (int q = 0; q < 4 * m; q++) le[cnt[K.lid[4L * e0 + q]]++] = (unsigned short)q; // q = 4 (e - e0) + k ascending
+        }
+    }
+    // pass 3: node -> slots, ascending
+    K.ns_ptr.assign(N + 1, 0);
+    for (long s = 0; s < K.nslots; s++) K.ns_ptr[K.nodes[s] + 1]++;
+    for (long i = 0; i < N; i++) K.ns_ptr[i + 1] += K.ns_ptr[i];
+    K.ns_slot.resize(K.nslots);
+    std::vector<int> fill(K.ns_ptr.begin(), K.ns_ptr.end() - 1);
+    for (long s = 0; s < K.nslots; s++) K.ns_slot[fill[K.nodes[s]]++] = (int)s;
     return CM_OK;
 }
 
@@ -314,6 +392,11 @@ extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, 
                 CM_TRY(upload(&L.d_sp, L.sp, st));
                 CM_TRY(upload(&L.d_col, L.col, st));
             }
+            Chunks &K = M->ck;
+            CM_TRY(upload(&K.d_eptr, K.eptr, st)); CM_TRY(upload(&K.d_nptr, K.nptr, st)); CM_TRY(upload(&K.d_nodes, K.nodes, st));
+            CM_TRY(upload(&K.d_ns_ptr, K.ns_ptr, st)); CM_TRY(upload(&K.d_ns_slot, K.ns_slot, st));
+            CM_TRY(upload(&K.d_lid, K.lid, st)); CM_TRY(upload(&K.d_lptr, K.lptr, st)); CM_TRY(upload(&K.d_lent, K.lent, st));
+            CM_TRY(upload(&M->d_emat, M->emat, st));
             CM_CUDA(cudaMalloc((void **)&M->d_red, 4096 * 16 * sizeof(double)));
             CM_CUDA(cudaMallocHost((void **)&M->h_red, 16 * sizeof(double)));
             CM_CUDA(cudaStreamSynchronize(st));
@@ -336,6 +419,9 @@ extern "C" int cm_mesh_destroy(cm_mesh *M)
     cudaFree(M->d_n2e); cudaFree(M->d_eid); cudaFree(M->d_mag); cudaFree(M->d_xyz); cudaFree(M->d_wvol);
     cudaFree(M->d_red); cudaFree(M->d_tmp);
     for (Sell &L : M->sell) { cudaFree(L.d_sp); cudaFree(L.d_col); }
+    Chunks &K = M->ck;
+    cudaFree(K.d_eptr); cudaFree(K.d_nptr); cudaFree(K.d_nodes); cudaFree(K.d_ns_ptr); cudaFree(K.d_ns_slot);
+    cudaFree(K.d_lid); cudaFree(K.d_lptr); cudaFree(K.d_lent); cudaFree(M->d_emat);
     if (M->h_red) cudaFreeHost(M->h_red);
     delete M;
     return CM_OK;
