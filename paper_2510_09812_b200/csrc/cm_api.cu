@@ -127,15 +127,21 @@ static int get_geometry(const System<T> *S, int what, void *host_out, long capac
     T *out = (T *)host_out;
     switch (what) {
     case 0:
-        if (capacity < Ne) break;
-        CM_CUDA(cudaMemcpy(out, S->V, Ne * sizeof(T), cudaMemcpyDeviceToHost));
-        return CM_OK;
     case 1: {
-        if (capacity < 12 * Ne) break;
-        std::vector<T> tmp(12 * Ne);
-        CM_CUDA(cudaMemcpy(tmp.data(), S->G, 12 * Ne * sizeof(T), cudaMemcpyDeviceToHost));
-        for (long e = 0; e < Ne; e++)
-            for (int q = 0; q < 12; q++) out[12 * e + q] = tmp[(long)q * Ne + e];
+        if (capacity < (what == 0 ? Ne : 12 * Ne)) break;
+        std::vector<T> tmp(10 * (Ne + 8));
+        CM_CUDA(cudaMemcpy(tmp.data(), S->EG, tmp.size() * sizeof(T), cudaMemcpyDeviceToHost));
+        const Chunks &K = S->mesh->ck;
+        for (int c = 0; c < K.nchunks; c++) {
+            const long e0 = K.eptr[c], ne = K.eptr[c + 1] - e0, ne8 = (ne + 7) & ~7L;
+            const T *blk = tmp.data() + 10 * e0;
+            for (long el = 0; el < ne; el++) {
+                if (what == 0) { out[e0 + el] = blk[el]; continue; }
+                T *g = out + 12 * (e0 + el);
+                for (int q = 0; q < 9; q++) g[3 + q] = blk[(q + 1) * ne8 + el];
+                for (int d = 0; d < 3; d++) g[d] = -(g[3 + d] + g[6 + d] + g[9 + d]); // grad phi_0 (O-1)
+            }
+        }
         return CM_OK;
     }
     case 2:

@@ -37,23 +37,27 @@ __device__ __forceinline__ void tet_geometry(const double *__restrict__ xyz, con
     }
 }
 
-// one thread per element: V_e, grad phi SoA (rounded to T), fp64 volume copy for the lumped masses
+// one CTA per element chunk: V_e and grad phi_1..3 (rounded to T) into the chunk-blocked geometry array
+// (cm_internal.h), fp64 volume copy for the lumped masses
 template <typename T>
-__global__ void geom_kernel(long Ne, const int *__restrict__ tets, const double *__restrict__ xyz, double ld, T *V, T *G,
+__global__ void geom_kernel(const int *__restrict__ eptr, const int *__restrict__ tets, const double *__restrict__ xyz, double ld, T *EG,
                             double *Vd)
 {
-    long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (e >= Ne) return;
-    int t[4];
-    *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(tets)[e];
-    TetGeom g;
-    tet_geometry(xyz, t, ld, g);
-    V[e] = (T)g.V;
-    Vd[e] = g.V;
+    const int c = blockIdx.x, e0 = eptr[c], ne = eptr[c + 1] - e0, ne8 = (ne + 7) & ~7;
+    T *blk = EG + 10L * e0;
+    for (int el = threadIdx.x; el < ne; el += blockDim.x) {
+        const long e = e0 + el;
+        int t[4];
+        *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(tets)[e];
+        TetGeom g;
+        tet_geometry(xyz, t, ld, g);
+        Vd[e] = g.V;
+        blk[el] = (T)g.V;
 #pragma unroll
-    for (int k = 0; k < 4; k++)
+        for (int k = 1; k < 4; k++)
 #pragma unroll
-        for (int d = 0; d < 3; d++) G[(long)(3 * k + d) * Ne + e] = (T)g.g[k][d];
+            for (int d = 0; d < 3; d++) blk[(long)(3 * (k - 1) + d + 1) * ne8 + el] = (T)g.g[k][d];
+    }
 }
 
 // one thread per node: lumped masses over all / magnetic incident tets, live flag
@@ -195,7 +199,7 @@ __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr
 template <typename T>
 System<T>::~System()
 {
-    T *ptrs[] = {V, G, mL, mLm, Cstar, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
+    T *ptrs[] = {EG, mL, mLm, Cstar, Ccub, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
     if (h_res) cudaFreeHost(h_res);
@@ -231,7 +235,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         CM_CUDA(cudaMemsetAsync(*p, 0, std::max<size_t>(n, 1) * sizeof(**p) + 256, st));
         return CM_OK;
     };
-    CM_TRY(alloc(&S->V, Ne)); CM_TRY(alloc(&S->G, 12 * Ne)); CM_TRY(alloc(&S->mL, N)); CM_TRY(alloc(&S->mLm, N));
+    CM_TRY(alloc(&S->EG, 10 * (Ne + 8))); CM_TRY(alloc(&S->mL, N)); CM_TRY(alloc(&S->mLm, N));
     CM_TRY(alloc(&S->live, N)); CM_TRY(alloc(&S->clamp, 3 * N));
     const long ES = M->sell[0].E, EB = M->sell[1].E; // stored elements of the sliced layouts (padding is zero)
     CM_TRY(alloc(&S->Kms, ES)); CM_TRY(alloc(&S->Kgs1, ES)); CM_TRY(alloc(&S->Kgs2, ES)); CM_TRY(alloc(&S->Mm, ES));
@@ -247,6 +251,21 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         CM_CUDA(cudaMemcpyAsync(Cd, Cs.data(), Cs.size() * sizeof(double), cudaMemcpyHostToDevice, st));
         CM_TRY(alloc(&S->Cstar, Ct.size()));
         CM_CUDA(cudaMemcpyAsync(S->Cstar, Ct.data(), Ct.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+        // cubic / isotropic / orthotropic stiffness in the crystal frame: only the normal 3x3 block and the three shear
+        // diagonals are non-zero.  Skipping exact zeros leaves every product C : eps unchanged, so the element
+        // kernels then read 12 words per material instead of 36.
+        S->cubic_pattern = true;
+        std::vector<T> Cc(12 * S->n_elastic);
+        for (int q = 0; q < S->n_elastic; q++)
+            for (int r = 0; r < 6; r++)
+                for (int c = 0; c < 6; c++) {
+                    const bool in = (r < 3 && c < 3) || r == c;
+                    if (!in && Cs[36 * q + 6 * r + c] != 0.0) S->cubic_pattern = false;
+                    if (r < 3 && c < 3) Cc[12 * q + 3 * r + c] = Ct[36 * q + 6 * r + c];
+                    if (r >= 3 && r == c) Cc[12 * q + 9 + (r - 3)] = Ct[36 * q + 6 * r + c];
+                }
+        CM_TRY(alloc(&S->Ccub, Cc.size()));
+        CM_CUDA(cudaMemcpyAsync(S->Ccub, Cc.data(), Cc.size() * sizeof(T), cudaMemcpyHostToDevice, st));
         CM_CUDA(cudaStreamSynchronize(st));
     }
     // clamp flags to library order
@@ -263,7 +282,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     CM_CUDA(cudaMalloc((void **)&Vd, Ne * sizeof(double)));
     CM_CUDA(cudaMalloc((void **)&vsum, 2 * sizeof(double)));
     const int B = 256;
-    geom_kernel<T><<<(unsigned)((Ne + B - 1) / B), B, 0, st>>>(Ne, M->d_tets, M->d_xyz, ld, S->V, S->G, Vd);
+    geom_kernel<T><<<M->ck.nchunks, B, 0, st>>>(M->ck.d_eptr, M->d_tets, M->d_xyz, ld, S->EG, Vd);
     lump_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, M->d_n2e_ptr, M->d_n2e, Vd, M->d_mag, S->mL, S->mLm, S->live);
     volume_sum_kernel<<<1, 1024, 0, st>>>(Ne, Vd, M->d_mag, vsum);
     CM_CUDA(cudaGetLastError());

@@ -95,12 +95,15 @@ __global__ void permute_out_kernel(long N, int nc, const int *__restrict__ order
 }
 
 // ---------------------------------------------------------------- element passes (S3, S5, S6, S8)
-// One CTA per element chunk (cm_internal.h).  Phase 0 stages the chunk's nodal inputs in shared memory (one
-// global gather per local node instead of one per element corner).  Phase 1, one thread per tetrahedron: coalesced
-// loads of the local ids, V_e and the nine stored gradient words (grad phi_0 = -sum of the others, O-1), compute,
-// contributions to shared memory.  Phase 2, one thread per local node: sums the node's incidences inside the chunk
-// in ascending element order and writes ONE partial per slot.  A node pass then adds a node's slots in ascending
-// chunk order -- a deterministic gather end to end, no float atomics, and no per-element scratch in HBM.
+// One CTA per element chunk (cm_internal.h).  At entry one thread issues four TMA bulk copies (cp.async.bulk) that
+// stream the chunk's element data -- the chunk-blocked geometry (V_e and nine gradient words per tetrahedron;
+// grad phi_0 = -sum of the others, O-1), local node ids, incidence list, material flags -- into shared memory, all
+// bytes in flight at once and landing on an mbarrier.  Meanwhile phase 0 stages the chunk's nodal inputs (one global
+// gather per local node instead of one per element corner).  Phase 1, one thread per tetrahedron: compute from shared
+// memory; the contributions overwrite the element's own column of the staged planes.  Phase 2, one thread per local
+// node: sums the node's incidences inside the chunk in ascending element order and writes ONE partial per slot.  A
+// node pass then adds a node's slots in ascending chunk order -- a deterministic gather end to end, no float
+// atomics, and no per-element scratch in HBM.
 enum ElemKind { EK_MS = 0, EK_GRADU = 1, EK_MECH = 2, EK_STRESS = 3 };
 // NIN staged words per node, NOUT shared-memory words per element, NC words per slot, PERK: contribution depends on
 // the local node index k (NOUT = 4 NC) or is the same for the 4 nodes (NOUT = NC).
@@ -110,27 +113,67 @@ template <> struct KindTraits<EK_GRADU> { static constexpr int NIN = 1, NOUT = 3
 template <> struct KindTraits<EK_MECH> { static constexpr int NIN = 3, NOUT = 12, NC = 3; static constexpr bool PERK = true; };
 template <> struct KindTraits<EK_STRESS> { static constexpr int NIN = 6, NOUT = 6, NC = 6; static constexpr bool PERK = false; };
 
-constexpr int EK_NT = 256;
+#ifndef CM_EK_NT
+#define CM_EK_NT 384
+#endif
+#ifndef CM_EK_MINB
+#define CM_EK_MINB 2
+#endif
+constexpr int EK_NT = CM_EK_NT;
 
 template <typename T>
 struct ChunkArgs {
     const int *eptr, *nptr, *nodes;
     const unsigned short *lid, *lptr, *lent, *emat;
-    const T *V, *G; // G: 12 planes [3k + d][Ne]; planes 3..11 are read
-    long Ne;
+    const T *EG;          // chunk-blocked geometry, 10 planes per chunk (cm_internal.h)
     const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w
     const double *mbar;   // MS
-    const T *Cstar;       // MECH, STRESS
+    const T *Cstar;       // MECH, STRESS: 36 words per material, or the 12 of the cubic pattern
     T l1, l2;
     T *hpart;             // [slot][NC]
     double *partial;      // GRADU: per-chunk sums of V_e grad U_e (fp64)
 };
 
+// shared-memory layout (every region a multiple of 16 bytes):
+//   planes [max(10, NOUT)][ne8] T   staged geometry, overwritten in place by the contributions
+//   sin    [CM_NL_MAX][NIN] T       nodal inputs
+//   slid   [EC] ushort4, sle [4 EC] ushort, sem [EC] ushort, slp [CM_NL_MAX + 8] ushort, mbarrier
+template <int KIND> constexpr int chunk_planes() { return KindTraits<KIND>::NOUT > 10 ? KindTraits<KIND>::NOUT : 10; }
 template <int KIND, typename T>
 constexpr size_t chunk_smem_bytes()
 {
-    return (size_t)(CM_NL_MAX * KindTraits<KIND>::NIN + CM_EC_MAX * KindTraits<KIND>::NOUT) * sizeof(T) +
-           (size_t)(CM_NL_MAX + 2 + 4 * CM_EC_MAX) * sizeof(unsigned short);
+    return (size_t)(chunk_planes<KIND>() * CM_EC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
+           (size_t)(4 * CM_EC_MAX + 4 * CM_EC_MAX + CM_EC_MAX + CM_NL_MAX + 8) * sizeof(unsigned short) + 16;
+}
+
+// ---- TMA bulk copy global -> shared, completion on an mbarrier
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "WAIT_%=:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra DONE_%=;\n"
+                 "bra WAIT_%=;\n"
+                 "DONE_%=:\n"
+                 "}" ::"r"(smem_u32(bar)), "r"(parity)
+                 : "memory");
 }
 
 // E0(m), Table A.1, Voigt engineering vector (E11, E22, E33, 2 E23, 2 E13, 2 E12)
@@ -176,19 +219,55 @@ __device__ __forceinline__ void C_times(const T *__restrict__ C, const T eps[6],
     }
 }
 
-template <typename T, int KIND>
-__global__ void __launch_bounds__(EK_NT) elem_chunk_kernel(ChunkArgs<T> a)
+// same product when C* has the cubic pattern; Cc = (C11 C12 C13 C21 C22 C23 C31 C32 C33 C44 C55 C66)
+template <typename T>
+__device__ __forceinline__ void C_times_cubic(const T *__restrict__ Cc, const T eps[6], T sig[6])
+{
+    T c[12];
+    if (sizeof(T) == 8) {
+#pragma unroll
+        for (int q = 0; q < 6; q++) *reinterpret_cast<double2 *>(c + 2 * q) = __ldg(reinterpret_cast<const double2 *>(Cc) + q);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 3; q++) *reinterpret_cast<float4 *>(c + 4 * q) = __ldg(reinterpret_cast<const float4 *>(Cc) + q);
+    }
+#pragma unroll
+    for (int r = 0; r < 3; r++) {
+        T acc = 0;
+#pragma unroll
+        for (int s = 0; s < 3; s++) acc += c[3 * r + s] * eps[s];
+        sig[r] = acc;
+    }
+#pragma unroll
+    for (int r = 3; r < 6; r++) sig[r] = c[6 + r] * eps[r];
+}
+
+template <typename T, int KIND, bool CUBIC>
+__global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs<T> a)
 {
     typedef KindTraits<KIND> K;
-    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *sin = reinterpret_cast<T *>(smem_raw);               // [nl][NIN]
-    T *scr = sin + CM_NL_MAX * NIN;                         // [NOUT][EC]
-    unsigned short *slp = reinterpret_cast<unsigned short *>(scr + EC * NOUT); // [nl + 1]
-    unsigned short *sle = slp + CM_NL_MAX + 2;              // [4 ne], 4-byte aligned
+    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX, NP = chunk_planes<KIND>();
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    T *scr = reinterpret_cast<T *>(smem_raw);                                   // [NP][ne8]
+    T *sin = scr + NP * EC;                                                     // [nl][NIN]
+    ushort4 *slid = reinterpret_cast<ushort4 *>(sin + CM_NL_MAX * NIN);         // [ne]
+    unsigned short *sle = reinterpret_cast<unsigned short *>(slid + EC);        // [4 ne]
+    unsigned short *sem = sle + 4 * EC;                                         // [ne]
+    unsigned short *slp = sem + EC;                                             // [nl + 1]
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(slp + CM_NL_MAX + 8);
     const int c = blockIdx.x, tid = threadIdx.x;
-    const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
+    const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, ne8 = (ne + 7) & ~7, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
 
+    // ---- element data: four bulk copies, all of the chunk's streaming bytes in flight at once
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        const unsigned bg = 10u * ne8 * sizeof(T), bl = 8u * ne8, be = 2u * ne8;
+        mbar_expect_tx(bar, bg + 2 * bl + be);
+        bulk_g2s(scr, a.EG + 10L * e0, bg, bar);
+        bulk_g2s(slid, a.lid + 4L * e0, bl, bar);
+        bulk_g2s(sle, a.lent + 4L * e0, bl, bar);
+        bulk_g2s(sem, a.emat + e0, be, bar);
+    }
     // ---- phase 0: nodal inputs, incidence runs
     for (int l = tid; l < nl; l += EK_NT) {
         const long g = a.nodes[s0 + l];
@@ -203,26 +282,20 @@ __global__ void __launch_bounds__(EK_NT) elem_chunk_kernel(ChunkArgs<T> a)
         }
     }
     for (int l = tid; l <= nl; l += EK_NT) slp[l] = a.lptr[s0 + c + l];
-    {
-        // 4 ne incidences; e0 * 4 entries of 2 bytes: 8-byte aligned rows, copied as 32-bit pairs
-        const unsigned *src = reinterpret_cast<const unsigned *>(a.lent + 4L * e0);
-        unsigned *dst = reinterpret_cast<unsigned *>(sle);
-        for (int q = tid; q < 2 * ne; q += EK_NT) dst[q] = __ldg(src + q);
-    }
-    __syncthreads();
+    __syncthreads(); // also orders the mbarrier initialisation before the waits
+    mbar_wait(bar, 0);
 
-    // ---- phase 1: one thread per tetrahedron
+    // ---- phase 1: one thread per tetrahedron; its contributions replace its own column of the staged planes
     double gsum[3] = {0, 0, 0};
     for (int el = tid; el < ne; el += EK_NT) {
-        const long e = e0 + el;
-        const ushort4 lq = __ldg(reinterpret_cast<const ushort4 *>(a.lid) + e);
+        const ushort4 lq = slid[el];
         const int l[4] = {lq.x, lq.y, lq.z, lq.w};
-        const T V = __ldg(a.V + e);
+        const T V = scr[el];
         T g[4][3];
 #pragma unroll
         for (int k = 1; k < 4; k++)
 #pragma unroll
-            for (int d = 0; d < 3; d++) g[k][d] = __ldg(a.G + (long)(3 * k + d) * a.Ne + e);
+            for (int d = 0; d < 3; d++) g[k][d] = scr[(3 * (k - 1) + d + 1) * ne8 + el];
 #pragma unroll
         for (int d = 0; d < 3; d++) g[0][d] = -(g[1][d] + g[2][d] + g[3][d]);
 
@@ -233,31 +306,32 @@ __global__ void __launch_bounds__(EK_NT) elem_chunk_kernel(ChunkArgs<T> a)
             for (int d = 0; d < 3; d++)
                 mt[d] = (sin[3 * l[0] + d] + sin[3 * l[1] + d] + sin[3 * l[2] + d] + sin[3 * l[3] + d]) / (T)4 - (T)a.mbar[d];
 #pragma unroll
-            for (int k = 0; k < 4; k++) scr[k * EC + el] = V * (g[k][0] * mt[0] + g[k][1] * mt[1] + g[k][2] * mt[2]);
+            for (int k = 0; k < 4; k++) scr[k * ne8 + el] = V * (g[k][0] * mt[0] + g[k][1] * mt[1] + g[k][2] * mt[2]);
         } else if (KIND == EK_GRADU) {
             // V_e grad U_e, and its fp64 sum for <grad U>
             const T u0 = sin[l[0]], u1 = sin[l[1]], u2 = sin[l[2]], u3 = sin[l[3]];
 #pragma unroll
             for (int d = 0; d < 3; d++) {
                 const T gU = u0 * g[0][d] + u1 * g[1][d] + u2 * g[2][d] + u3 * g[3][d];
-                scr[d * EC + el] = V * gU;
+                scr[d * ne8 + el] = V * gU;
                 gsum[d] += (double)V * (double)gU;
             }
         } else {
-            const unsigned em = __ldg(a.emat + e);
+            const unsigned em = sem[el];
             if (!(em & 1u)) {
 #pragma unroll
-                for (int q = 0; q < NOUT; q++) scr[q * EC + el] = 0;
+                for (int q = 0; q < NOUT; q++) scr[q * ne8 + el] = 0;
             } else if (KIND == EK_MECH) {
                 // S = C*_e : mean_e E0(m);  c_(k,a) = V_e (S grad phi_k)_a
                 T e0v[6], sg[6];
                 mean_E0<T, 3, 0>(sin, l, a.l1, a.l2, e0v);
-                C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
+                if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), e0v, sg);
+                else C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
-                    scr[(3 * k + 0) * EC + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
-                    scr[(3 * k + 1) * EC + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
-                    scr[(3 * k + 2) * EC + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
+                    scr[(3 * k + 0) * ne8 + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
+                    scr[(3 * k + 1) * ne8 + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
+                    scr[(3 * k + 2) * ne8 + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
                 }
             } else {
                 // V_e C*_e : (E_e(u) - mean_e E0(w)),  H[a][b] = d_b u_a
@@ -275,9 +349,10 @@ __global__ void __launch_bounds__(EK_NT) elem_chunk_kernel(ChunkArgs<T> a)
                 mean_E0<T, 6, 3>(sin, l, a.l1, a.l2, e0v);
 #pragma unroll
                 for (int q = 0; q < 6; q++) eps[q] -= e0v[q];
-                C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+                if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), eps, sg);
+                else C_times(a.Cstar + 36 * (em >> 1), eps, sg);
 #pragma unroll
-                for (int q = 0; q < 6; q++) scr[q * EC + el] = V * sg[q];
+                for (int q = 0; q < 6; q++) scr[q * ne8 + el] = V * sg[q];
             }
         }
     }
@@ -291,7 +366,7 @@ __global__ void __launch_bounds__(EK_NT) elem_chunk_kernel(ChunkArgs<T> a)
         for (int q = slp[l]; q < slp[l + 1]; q++) {
             const int ent = sle[q], el = ent >> 2, k = ent & 3;
 #pragma unroll
-            for (int x = 0; x < NC; x++) acc[x] += scr[(K::PERK ? NC * k + x : x) * EC + el];
+            for (int x = 0; x < NC; x++) acc[x] += scr[(K::PERK ? NC * k + x : x) * ne8 + el];
         }
 #pragma unroll
         for (int x = 0; x < NC; x++) a.hpart[(long)(s0 + l) * NC + x] = acc[x];
@@ -516,7 +591,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     const Chunks &K = M->ck;
     ChunkArgs<T> a;
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
-    a.emat = M->d_emat; a.V = S->V; a.G = S->G; a.Ne = S->Ne;
+    a.emat = M->d_emat; a.EG = S->EG;
     a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.hpart = S->hpart; a.partial = S->red;
     return a;
@@ -526,12 +601,17 @@ template <typename T, int KIND>
 static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
 {
     constexpr size_t smem = chunk_smem_bytes<KIND, T>();
-    static bool configured = false; // per instantiation; the attribute is per function, so once is enough
-    if (!configured) {
-        CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
+    constexpr bool USES_C = KIND == EK_MECH || KIND == EK_STRESS;
+    // per device and per function; a host-side table lookup, set on every launch so that any device / context works
+    CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (USES_C) CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (USES_C && S->cubic_pattern) {
+        ChunkArgs<T> b = a;
+        b.Cstar = S->Ccub;
+        elem_chunk_kernel<T, KIND, true><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(b);
+    } else {
+        elem_chunk_kernel<T, KIND, false><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(a);
     }
-    elem_chunk_kernel<T, KIND><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(a);
     return CM_OK;
 }
 

@@ -50,7 +50,8 @@ struct Sell {
 };
 
 // Element chunks for the assembly passes (S3, S5, S6, S8): consecutive elements are cut into chunks of at most
-// CM_EC_MAX elements that reference at most CM_NL_MAX distinct nodes.  A chunk numbers its nodes locally (sorted by
+// CM_EC_MAX elements that reference at most CM_NL_MAX distinct nodes; every chunk starts at a multiple of 8 elements
+// (16-byte aligned rows for the bulk copies), so only the last chunk has a ragged size.  A chunk numbers its nodes locally (sorted by
 // global id); "slot" nptr[c] + l is local node l of chunk c, and every slot owns one partial sum per pass.
 //   eptr[c]            first element of chunk c
 //   nptr[c]            first slot of chunk c;  nodes[slot] = global node id
@@ -59,7 +60,7 @@ struct Sell {
 //   lent[4 eptr[c] + q] incidence q of chunk c: 4 * (e - eptr[c]) + k, ascending inside every run
 //   ns_ptr / ns_slot   node -> its slots, ascending (so ascending chunk = ascending element order)
 constexpr int CM_EC_MAX = 768;
-constexpr int CM_NL_MAX = 768;
+constexpr int CM_NL_MAX = 512;
 struct Chunks {
     int nchunks = 0;
     long nslots = 0;
@@ -134,9 +135,13 @@ struct SystemBase {
 template <typename T>
 struct System : SystemBase {
     // geometry
-    T *V = nullptr, *G = nullptr; // G: 12 planes [3k + a][Ne]
+    // element geometry, chunk-blocked: chunk c owns 10 planes of ne8 = round_up(ne_c, 8) values at EG + 10 eptr[c]:
+    // plane 0 = V_e, plane 3 (k - 1) + d + 1 = d-th component of grad phi_k, k = 1..3 (grad phi_0 = -sum, O-1)
+    T *EG = nullptr;
     T *mL = nullptr, *mLm = nullptr;
     T *Cstar = nullptr; // n_elastic x 36
+    T *Ccub = nullptr;  // n_elastic x 12 (C11 C12 C13 C21 .. C33, C44 C55 C66) when every C* is zero outside that pattern
+    bool cubic_pattern = false;
     uchar *live = nullptr, *clamp = nullptr;
     // matrices
     T *Kms = nullptr, *Kgs1 = nullptr, *Kgs2 = nullptr, *Mm = nullptr;

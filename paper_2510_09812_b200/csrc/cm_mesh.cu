@@ -284,27 +284,28 @@ int build_chunks(long N, long Ne, const int *tets, Chunks *out)
     K.nptr.assign(1, 0);
     K.nodes.clear();
     K.nodes.reserve(Ne / 2 + 16);
-    // pass 1 (sequential): chunk boundaries and the nodes of every chunk in first-seen order
+    // pass 1 (sequential): chunk boundaries and the nodes of every chunk in first-seen order; elements are taken in
+    // groups of 8 so that chunks start at multiples of 8
     std::vector<int> stamp(N, -1);
     int cur = 0, ne = 0, nl = 0;
-    for (long e = 0; e < Ne; e++) {
-        int fresh = 0;
-        for (int k = 0; k < 4; k++) {
-            const int v = tets[4 * e + k];
-            bool dup = stamp[v] == cur;
-            for (int j = 0; j < k && !dup; j++) dup = tets[4 * e + j] == v;
-            fresh += !dup;
-        }
-        if (ne + 1 > CM_EC_MAX || nl + fresh > CM_NL_MAX) {
-            K.eptr.push_back((int)e);
+    std::vector<int> grp;
+    for (long g0 = 0; g0 < Ne; g0 += 8) {
+        const long g1 = std::min(Ne, g0 + 8);
+        grp.clear();
+        for (long q = 4 * g0; q < 4 * g1; q++)
+            if (stamp[tets[q]] != cur) grp.push_back(tets[q]);
+        std::sort(grp.begin(), grp.end());
+        const int fresh = (int)(std::unique(grp.begin(), grp.end()) - grp.begin());
+        if (ne > 0 && (ne + 8 > CM_EC_MAX || nl + fresh > CM_NL_MAX)) {
+            K.eptr.push_back((int)g0);
             K.nptr.push_back((int)K.nodes.size());
             cur++; ne = 0; nl = 0;
         }
-        for (int k = 0; k < 4; k++) {
-            const int v = tets[4 * e + k];
+        for (long q = 4 * g0; q < 4 * g1; q++) {
+            const int v = tets[q];
             if (stamp[v] != cur) { stamp[v] = cur; K.nodes.push_back(v); nl++; }
         }
-        ne++;
+        ne += (int)(g1 - g0);
     }
     K.eptr.push_back((int)Ne);
     K.nptr.push_back((int)K.nodes.size());

@@ -35,6 +35,13 @@ def model_bytes(N, nnz, s):
             "cg_bsr3": nnz * (9 * s + 4) + N * 4 + 36 * N * s}
 
 
+def elem_bytes(N, Ne, s):
+    """Element passes, stored gradients: 16 B connectivity + 13 words per tet, nodal input and output once."""
+    tet = Ne * (16 + 13 * s)
+    return {"elem_rhs_ms": tet + N * 4 * s, "elem_hd": tet + N * 4 * s, "elem_rhs_mech": tet + N * 6 * s,
+            "elem_sigma": tet + N * 12 * s}
+
+
 def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False):
     import torch
     from . import binding as cm
@@ -109,6 +116,15 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False):
                         x.zero_(); its.append(gs.cg_solve(matid, b, x, tol=tol, maxiter=200000)[0])
                     t, p = kernel_ms(ft, cls, 2)
                     cases.append((name + "_tol1e-8", t, its[-1] * mb[key], its[-1]))
+                eb = elem_bytes(N, gm.n_tets, s)
+                m3 = torch.as_tensor(inputs.init_m_noisy_x(mesh, 44), dtype=td, device="cuda").contiguous()
+                for name, rid, kw in (("elem_rhs_ms", cm.CM_RHS_MS, {}), ("elem_hd", cm.CM_OUT_HD, {"U": b1}),
+                                      ("elem_rhs_mech", cm.CM_RHS_MECH, {}), ("elem_sigma", cm.CM_OUT_SIGMA, {"u": b3})):
+                    if only and name not in only and "elem" not in only:
+                        continue
+                    t, p = kernel_ms(lambda: gs.field_rhs(rid, m3, **kw), "element", reps)
+                    # kernel_ms divides by launches; a pass is 2-3 launches, so take the class total per call
+                    cases.append((name, p["ms"] / reps, eb[name], None))
                 if not only or "cg_csr3" in only:
                     def f33():
                         x3.zero_(); gs.cg_solve3(cm.CM_MAT_K_GS1, b3, x3, fixed_iters=3)
@@ -116,7 +132,7 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False):
                     cases.append(("cg_csr3_fixed3", t, 3 * mb["cg_csr3"], 3))
                 for name, t, byts, its in cases:
                     gbs = byts / (t * 1e-3) / 1e9
-                    resident = (mb["spmv_bsr3" if "bsr" in name else "spmv_csr1"] < L2)
+                    resident = (mb["spmv_bsr3" if "bsr" in name else "spmv_csr1"] < L2) and not name.startswith("elem")
                     rows.append({"side": side, "n_nodes": N, "nnz": nnz, "reorder": ro, "dtype": dtype, "kernel": name, "ms": t,
                                  "iters": its, "algorithmic_GBps": gbs, "frac_of_measured_hbm": gbs / peak,
                                  "l2_resident": bool(resident)})

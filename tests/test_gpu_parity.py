@@ -198,6 +198,29 @@ def test_rhs_and_fields(case, cm, oracle_mod):
         assert rel(gs.field_rhs(cm.CM_OUT_FIELD, md, Ud, ud, pp).cpu().numpy(), h_t) < tol
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_full_anisotropic_stiffness(cm, oracle_mod, torch, dtype):
+    """A stiffness that is dense in Voigt form (symmetric positive definite, no zero entries) takes the general
+    36-word path of the element kernels; the isotropic materials of the other tests take the 12-word cubic-pattern path."""
+    mesh = inputs.kuhn_box((9, 8, 7), (27 * NM, 24 * NM, 21 * NM), seed_mesh=61, seed_perm=62)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (6 * NM, 5 * NM, 5 * NM))
+    rng = np.random.default_rng(63)
+    A = rng.normal(size=(2, 6, 6))
+    C = np.stack([inputs.isotropic_voigt(200e9, 0.3) + 2e10 * (a @ a.T) for a in A])
+    assert np.all(C != 0)
+    mat = inputs.Material(C_voigt=C)
+    c = Case(cm, oracle_mod, torch, mesh, mat, 2e-12, dtype, cm.CM_REORDER_MORTON, clamp=inputs.clamp_bottom(mesh))
+    tol = TOL[dtype]
+    m = inputs.init_m_random(mesh, 64).astype(c.gs.np_dtype)
+    u = (1e-3 * rng.normal(size=(c.o.N, 3))).astype(c.gs.np_dtype)
+    p = cm.make_params(c.dt, np.zeros(3), ALL)
+    assert rel(c.gs.field_rhs(cm.CM_RHS_MECH, c.dev(m)).cpu().numpy(), c.o.rhs_mech(m.astype(np.float64))) < tol
+    sig = c.gs.field_rhs(cm.CM_OUT_SIGMA, c.dev(m), None, c.dev(u), p).cpu().numpy()
+    assert rel(sig, c.o.stress_recover(u.astype(np.float64), m.astype(np.float64))) < tol
+    x = rng.normal(size=(c.o.N, 3)).astype(c.gs.np_dtype)
+    assert rel(c.gs.spmv(cm.CM_MAT_K_MECH, c.dev(x)).cpu().numpy(), c.o.spmv(oracle_mod.MAT_K_MECH, x.astype(np.float64))) < tol
+
+
 # ---------------------------------------------------------------------------------------------- CG
 def test_cg(case, cm, oracle_mod):
     o, gs = case.o, case.gs
