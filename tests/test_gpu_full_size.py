@@ -140,3 +140,33 @@ def test_full_size_gspm_step_fixed_iterations(full, oracle_mod):
     live = o.live().astype(bool)
     assert np.abs(np.linalg.norm(mgh[live], axis=1) - 1).max() <= 4 * np.finfo(float).eps
     assert np.abs(mgh[~live]).max() == 0.0
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config1_full_size_10_steps(oracle_mod, dtype):
+    """BASELINE config 1 at its own size (81x81x21 = 137,781 nodes, anisotropy + Zeeman at -50 mT, dt = 5 ps): ten steps,
+    every solve iterated to convergence on both sides.  fp64: tol 1e-12, max |dm| <= 1e-9, counts +-1;  fp32 against the
+    fp64 oracle: tol 1e-6, max |dm| <= 1e-4."""
+    import torch
+    from paper_2510_09812_b200 import binding as cm
+    cfg = inputs.make_config(1)
+    assert cfg.mesh.n_nodes == 137781
+    f64 = dtype == "f64"
+    tol = 1e-12 if f64 else 1e-6
+    td = torch.float64 if f64 else torch.float32
+    gm = cm.Mesh(cfg.mesh.xyz, cfg.mesh.tets, cfg.mesh.magnetic, cfg.mesh.elastic_id, cm.CM_REORDER_MORTON)
+    gs = cm.System(gm, cfg.material, cfg.dt, dtype, cfg.clamp_dof, cfg.pin_node)
+    o = oracle_mod.Oracle(cfg.mesh, cfg.material, cfg.dt, clamp_dof=cfg.clamp_dof, pin_node=cfg.pin_node)
+    N = o.N
+    m = cfg.m0.copy(); U = np.zeros(N); u = np.zeros((N, 3))
+    mg = torch.as_tensor(cfg.m0, dtype=td, device="cuda").contiguous()
+    Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+    for k in range(10):
+        p = cm.make_params(cfg.dt, cfg.Hext[k], cfg.terms, 0, tol)
+        io, rco = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k], cfg.terms, cg_tol=tol)
+        ig, rcg = gs.gspm_step(p, mg, Ug, ug)
+        assert rco == 0 and rcg == 0
+        for a in range(8):
+            assert abs(io.it_gs[a] - ig.it_gs[a]) <= (1 if f64 else 3), (k, a, list(io.it_gs), list(ig.it_gs))
+    err = np.abs(mg.cpu().numpy().astype(np.float64) - m).max()
+    assert err <= (1e-9 if f64 else 1e-4), err
