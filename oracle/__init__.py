@@ -68,7 +68,7 @@ def _lib(dtype: str):
         L.orc_nnz.restype = C.c_long
         for name in ("orc_scalar", "orc_nnz", "orc_get", "orc_get_values", "orc_spmv", "orc_cg", "orc_volume_average",
                      "orc_rhs_ms", "orc_demag_field", "orc_rhs_mech", "orc_stress_recover", "orc_field", "orc_energy",
-                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy"):
+                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap"):
             getattr(L, name).argtypes = None
         _libs[dtype] = L
     return _libs[dtype]
@@ -92,15 +92,30 @@ def reorder(xyz, tets, method: int):
     return order, iperm, tnew, torder
 
 
+def periodic_wrap(xyz, axes: int, rel_tol: float = 1e-9):
+    """dof_of_node (int32, n_nodes) and n_dof for the periodic directions in the bit mask `axes`."""
+    L = _lib("f64")
+    xyz = np.ascontiguousarray(xyz, np.float64)
+    n = xyz.shape[0]
+    dof = np.empty(n, np.int32)
+    nd = C.c_long()
+    rc = L.orc_periodic_wrap(_p(xyz), C.c_long(n), C.c_uint(axes), C.c_double(rel_tol), _p(dof), C.byref(nd))
+    if rc:
+        raise RuntimeError(f"orc_periodic_wrap rc={rc}")
+    return dof, int(nd.value)
+
+
 class Oracle:
     """One mesh + material + dt, in the node order it is given (no reordering)."""
 
-    def __init__(self, mesh, material, dt, clamp_dof=None, pin_node=0, dtype="f64"):
+    def __init__(self, mesh, material, dt, clamp_dof=None, pin_node=0, dtype="f64", dof_of_node=None, n_dof=None):
         self.dtype = dtype
         self.real = np.float64 if dtype == "f64" else np.float32
         self.L = _lib(dtype)
         assert self.L.orc_sizeof_real() == np.dtype(self.real).itemsize
-        self.N, self.Ne = mesh.n_nodes, mesh.n_tets
+        self.Ng, self.Ne = mesh.n_nodes, mesh.n_tets
+        self.N = self.Ng if dof_of_node is None else int(n_dof)       # degrees of freedom (P:233-235)
+        dof = None if dof_of_node is None else np.ascontiguousarray(dof_of_node, np.int32)
         xyz = np.ascontiguousarray(mesh.xyz, np.float64)
         tets = np.ascontiguousarray(mesh.tets, np.int32)
         mag = np.ascontiguousarray(mesh.magnetic, np.uint8)
@@ -112,8 +127,8 @@ class Oracle:
                       None if self._Cv is None else self._Cv.ctypes.data_as(C.POINTER(C.c_double)))
         clamp = None if clamp_dof is None else np.ascontiguousarray(clamp_dof, np.uint8)
         h = C.c_void_p()
-        rc = self.L.orc_create(_p(xyz), C.c_long(self.N), _p(tets), C.c_long(self.Ne), _p(mag), _p(eid), C.byref(m),
-                               C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
+        rc = self.L.orc_create_wrapped(_p(xyz), C.c_long(self.Ng), _p(tets), C.c_long(self.Ne), _p(mag), _p(eid), _p(dof),
+                                       C.c_long(self.N), C.byref(m), C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
         if rc:
             raise RuntimeError(f"orc_create rc={rc}")
         self.h = h

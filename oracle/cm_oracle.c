@@ -265,6 +265,88 @@ int orc_reorder(const double *xyz, long N, const int *tets, long Ne, int method,
 }
 
 /* ------------------------------------------------------------------------------------ */
+/* Periodic boundary conditions by node wrapping (R23)               */
+/* ------------------------------------------------------------------------------------ */
+/* "wrapping any node whose coordinate in a given direction lies at the domain's maximum extent to the corresponding
+ * node at the domain's minimum extent in that direction.  Then [...] inserts each wrapped node pair into a hash map
+ * and assigns a unique global index."
+ * axes: bit d set = direction d periodic.  A node is wrapped along d when x_d >= hi_d - tol_d (tol_d = rel_tol * span_d);
+ * its image is x - span_d e_d for every such d.  Nodes wrapped along no direction are the representatives and are
+ * numbered 0.. in ascending node index; a wrapped node takes the number of the one representative within tol of its
+ * image (none or several: ORC_E_BADARG, "only works for [...] perfectly matched node distributions"). */
+static unsigned long long cell_hash(long long cx, long long cy, long long cz)
+{
+    unsigned long long h = (unsigned long long)cx * 0x9E3779B97F4A7C15ull;
+    h ^= (unsigned long long)cy * 0xC2B2AE3D27D4EB4Full + (h << 6) + (h >> 2);
+    h ^= (unsigned long long)cz * 0x165667B19E3779F9ull + (h << 6) + (h >> 2);
+    return h;
+}
+
+int orc_periodic_wrap(const double *xyz, long N, unsigned axes, double rel_tol, int *dof, long *ndof_out)
+{
+    if (!xyz || !dof || !ndof_out || N <= 0 || !(rel_tol > 0) || rel_tol > 1e-3) return ORC_E_BADARG;
+    double lo[3], hi[3], span[3], tol[3], h[3];
+    for (int d = 0; d < 3; d++) { lo[d] = 1e300; hi[d] = -1e300; }
+    for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++) {
+        if (xyz[3 * i + d] < lo[d]) lo[d] = xyz[3 * i + d];
+        if (xyz[3 * i + d] > hi[d]) hi[d] = xyz[3 * i + d];
+    }
+    for (int d = 0; d < 3; d++) {
+        span[d] = hi[d] - lo[d];
+        if (((axes >> d) & 1u) && !(span[d] > 0)) return ORC_E_BADARG;
+        tol[d] = rel_tol * span[d];
+        h[d] = span[d] > 0 ? 4.0 * tol[d] : 1.0;
+    }
+    /* pass 1: representatives, numbered in ascending node index */
+    long nrep = 0;
+    for (long i = 0; i < N; i++) {
+        int wrapped = 0;
+        for (int d = 0; d < 3; d++) if (((axes >> d) & 1u) && xyz[3 * i + d] >= hi[d] - tol[d]) wrapped = 1;
+        dof[i] = wrapped ? -1 : (int)nrep++;
+    }
+    *ndof_out = nrep;
+    if (nrep == N) return ORC_OK;
+    /* hash map: cell of side 4 tol -> chain of representatives */
+    long nb = 1; while (nb < 2 * nrep) nb <<= 1;
+    int *head = (int *)malloc((size_t)nb * sizeof(int)), *next = (int *)malloc((size_t)N * sizeof(int));
+    if (!head || !next) { free(head); free(next); return ORC_E_ALLOC; }
+    for (long b = 0; b < nb; b++) head[b] = -1;
+    for (long i = 0; i < N; i++) {
+        if (dof[i] < 0) continue;
+        long long c[3];
+        for (int d = 0; d < 3; d++) c[d] = (long long)floor((xyz[3 * i + d] - lo[d]) / h[d]);
+        unsigned long long b = cell_hash(c[0], c[1], c[2]) & (unsigned long long)(nb - 1);
+        next[i] = head[b]; head[b] = (int)i;
+    }
+    int rc = ORC_OK;
+    for (long i = 0; i < N && rc == ORC_OK; i++) {
+        if (dof[i] >= 0) continue;
+        double w[3]; long long c[3];
+        for (int d = 0; d < 3; d++) {
+            w[d] = xyz[3 * i + d];
+            if (((axes >> d) & 1u) && w[d] >= hi[d] - tol[d]) w[d] -= span[d];
+            c[d] = (long long)floor((w[d] - lo[d]) / h[d]);
+        }
+        int found = -1, count = 0;
+        for (int a = -1; a <= 1; a++) for (int bq = -1; bq <= 1; bq++) for (int cq = -1; cq <= 1; cq++) {
+            long long cx = c[0] + a, cy = c[1] + bq, cz = c[2] + cq;
+            unsigned long long b = cell_hash(cx, cy, cz) & (unsigned long long)(nb - 1);
+            for (int j = head[b]; j >= 0; j = next[j]) {
+                /* the chain of a bucket may hold other cells (hash collisions): test the cell, then the distance */
+                if ((long long)floor((xyz[3 * j] - lo[0]) / h[0]) != cx || (long long)floor((xyz[3 * j + 1] - lo[1]) / h[1]) != cy ||
+                    (long long)floor((xyz[3 * j + 2] - lo[2]) / h[2]) != cz) continue;
+                if (fabs(xyz[3 * j] - w[0]) <= tol[0] && fabs(xyz[3 * j + 1] - w[1]) <= tol[1] && fabs(xyz[3 * j + 2] - w[2]) <= tol[2]) {
+                    found = j; count++;
+                }
+            }
+        }
+        if (count != 1) rc = ORC_E_BADARG; else dof[i] = dof[found];
+    }
+    free(head); free(next);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------ */
 /* O-1 geometry, O-2 matrices                                                            */
 /* ------------------------------------------------------------------------------------ */
 
@@ -286,14 +368,29 @@ static long find_col(const oracle *o, long i, int j)
 
 void orc_destroy(oracle *o);
 
-int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const uchar *magnetic,
-               const int *elastic_id, const orc_material *mat, double dt, const uchar *clamp_dof,
-               long pin_node, oracle **out)
+/* Periodic boundary conditions: `dof` (NULL = identity) maps each of the Ng geometric nodes to one of N
+ * unified degrees of freedom ("the two nodes in the pair are treated as one unified node").  Element geometry is
+ * computed from the element's own corner coordinates; every nodal quantity (matrix rows, lumped masses, fields)
+ * is indexed by DOF. */
+int orc_create_wrapped(const double *xyz_m, long Ng, const int *gtets, long Ne, const uchar *magnetic,
+                       const int *elastic_id, const int *dof, long N, const orc_material *mat, double dt,
+                       const uchar *clamp_dof, long pin_node, oracle **out)
 {
-    if (!xyz_m || !tets || !mat || !out || N <= 0 || Ne <= 0) return ORC_E_BADARG;
+    if (!xyz_m || !gtets || !mat || !out || N <= 0 || Ng <= 0 || Ne <= 0) return ORC_E_BADARG;
+    if (!dof && N != Ng) return ORC_E_BADARG;
     oracle *o = (oracle *)calloc(1, sizeof(oracle));
     if (!o) return ORC_E_ALLOC;
     o->N = N; o->Ne = Ne;
+    int *tets = (int *)malloc((size_t)Ne * 4 * sizeof(int));   /* DOF connectivity */
+    if (!tets) { free(o); return ORC_E_ALLOC; }
+    for (long q = 0; q < 4 * Ne; q++) {
+        if (gtets[q] < 0 || gtets[q] >= Ng) { free(tets); free(o); return ORC_E_RANGE; }
+        tets[q] = dof ? dof[gtets[q]] : gtets[q];
+        if (tets[q] < 0 || tets[q] >= N) { free(tets); free(o); return ORC_E_RANGE; }
+    }
+    if (dof) for (long e = 0; e < Ne; e++) /* two corners on one DOF: the domain is a single cell wide in a periodic direction */
+        for (int i = 0; i < 4; i++) for (int j = i + 1; j < 4; j++)
+            if (tets[4 * e + i] == tets[4 * e + j]) { free(tets); free(o); return ORC_E_BADARG; }
     /* O-0 nondimensionalisation */
     double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
     o->Ms = mat->Ms; o->dt = dt;
@@ -309,8 +406,8 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
     for (int q = 0; q < o->n_elastic * 36; q++) o->Cstar[q] = mat->C_voigt[q] / mu0Ms2;
 
-    o->x = (double *)malloc((size_t)N * 3 * sizeof(double));
-    o->tet = (int *)malloc((size_t)Ne * 4 * sizeof(int));
+    o->x = (double *)malloc((size_t)Ng * 3 * sizeof(double));
+    o->tet = tets;
     o->mag = (uchar *)malloc((size_t)Ne);
     o->eid = (int *)calloc((size_t)Ne, sizeof(int));
     o->V = (real *)malloc((size_t)Ne * sizeof(real));
@@ -320,21 +417,19 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     o->live = (uchar *)calloc((size_t)N, 1);
     o->clamp = (uchar *)calloc((size_t)N * 3, 1);
     if (!o->x || !o->tet || !o->mag || !o->eid || !o->V || !o->G || !o->mL || !o->mLm || !o->live || !o->clamp) { orc_destroy(o); return ORC_E_ALLOC; }
-    for (long i = 0; i < 3 * N; i++) o->x[i] = xyz_m[i] / ld;
-    memcpy(o->tet, tets, (size_t)Ne * 4 * sizeof(int));
+    for (long i = 0; i < 3 * Ng; i++) o->x[i] = xyz_m[i] / ld;
     for (long e = 0; e < Ne; e++) o->mag[e] = magnetic ? (magnetic[e] != 0) : 1;
     if (elastic_id) memcpy(o->eid, elastic_id, (size_t)Ne * sizeof(int));
     if (clamp_dof) for (long i = 0; i < 3 * N; i++) o->clamp[i] = clamp_dof[i] != 0;
     o->pin = pin_node;
     for (long e = 0; e < Ne; e++) {
-        for (int k = 0; k < 4; k++) if (tets[4 * e + k] < 0 || tets[4 * e + k] >= N) { orc_destroy(o); return ORC_E_RANGE; }
         if (o->n_elastic && (o->eid[e] < 0 || o->eid[e] >= o->n_elastic)) { orc_destroy(o); return ORC_E_RANGE; }
     }
     if (pin_node < 0 || pin_node >= N) { orc_destroy(o); return ORC_E_BADARG; }
 
     /* O-1: V_e = |det J|/6, grad phi_k = k-th row of J^-1 (k=1..3), grad phi_0 = -sum */
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-    for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++) {
+    for (long i = 0; i < Ng; i++) for (int d = 0; d < 3; d++) {
         if (o->x[3 * i + d] < lo[d]) lo[d] = o->x[3 * i + d];
         if (o->x[3 * i + d] > hi[d]) hi[d] = o->x[3 * i + d];
     }
@@ -343,8 +438,8 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     double *mL = (double *)calloc((size_t)N, sizeof(double)), *mLm = (double *)calloc((size_t)N, sizeof(double));
     o->Vtot = 0; o->Vmag = 0;
     for (long e = 0; e < Ne; e++) {
-        const double *x0 = o->x + 3 * tets[4 * e], *x1 = o->x + 3 * tets[4 * e + 1],
-                     *x2 = o->x + 3 * tets[4 * e + 2], *x3 = o->x + 3 * tets[4 * e + 3];
+        const double *x0 = o->x + 3 * gtets[4 * e], *x1 = o->x + 3 * gtets[4 * e + 1],
+                     *x2 = o->x + 3 * gtets[4 * e + 2], *x3 = o->x + 3 * gtets[4 * e + 3];
         double a[3], b[3], c[3];
         for (int d = 0; d < 3; d++) { a[d] = x1[d] - x0[d]; b[d] = x2[d] - x0[d]; c[d] = x3[d] - x0[d]; }
         double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
@@ -381,8 +476,8 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     if (!K || !Km || !Mm || (o->n_elastic && !Kme)) { orc_destroy(o); return ORC_E_ALLOC; }
     for (long e = 0; e < Ne; e++) {
         /* recompute the fp64 geometry of this element (not the rounded copy) */
-        const int *t = tets + 4 * e;
-        const double *x0 = o->x + 3 * t[0], *x1 = o->x + 3 * t[1], *x2 = o->x + 3 * t[2], *x3 = o->x + 3 * t[3];
+        const int *t = tets + 4 * e, *tg = gtets + 4 * e;
+        const double *x0 = o->x + 3 * tg[0], *x1 = o->x + 3 * tg[1], *x2 = o->x + 3 * tg[2], *x3 = o->x + 3 * tg[3];
         double a[3], b[3], c[3];
         for (int d = 0; d < 3; d++) { a[d] = x1[d] - x0[d]; b[d] = x2[d] - x0[d]; c[d] = x3[d] - x0[d]; }
         double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
@@ -441,6 +536,13 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     free(K); free(Km); free(Mm); free(Kme);
     *out = o;
     return ORC_OK;
+}
+
+int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const uchar *magnetic,
+               const int *elastic_id, const orc_material *mat, double dt, const uchar *clamp_dof,
+               long pin_node, oracle **out)
+{
+    return orc_create_wrapped(xyz_m, N, tets, Ne, magnetic, elastic_id, NULL, N, mat, dt, clamp_dof, pin_node, out);
 }
 
 void orc_destroy(oracle *o)
