@@ -127,6 +127,21 @@ typedef struct {
  * into cm_material.C_voigt (NULL = all 0).  Errors: BADARG, INDEX_RANGE, DEGENERATE_TET, ALLOC, CUDA. */
 int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
                    const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out);
+/* Periodic boundary conditions by node wrapping (R23).
+ * cm_periodic_wrap: "wrapping any node whose coordinate in a given direction lies at the domain's maximum extent to the
+ * corresponding node at the domain's minimum extent in that direction", each wrapped pair getting one unified index.
+ * axes: bit d set = direction d periodic.  A node is wrapped along d when x_d >= max_d - rel_tol * span_d; nodes wrapped
+ * along no direction are the representatives, numbered 0.. in ascending node index; a wrapped node takes the number of the
+ * one representative within rel_tol * span of its image x - span_d e_d.  dof_of_node: host out, n_nodes; *n_dof: host out.
+ * Host-only (no device needed).  Errors: BADARG (no or several partners: faces do not match).
+ * cm_mesh_create_wrapped: as cm_mesh_create, with dof_of_node (host, n_nodes, values in [0, n_dof); NULL = identity).
+ * Element geometry comes from the element's own corner coordinates; every nodal quantity is indexed by DOF: the mesh then
+ * has n_dof "nodes" (cm_mesh_get counts, field vectors, clamp_dof, pin_node are all in DOF numbering).  A tet with two
+ * corners on one DOF (domain one cell wide in a periodic direction) is rejected with BADARG. */
+int cm_periodic_wrap(const double *xyz, long n_nodes, unsigned axes, double rel_tol, int *dof_of_node, long *n_dof);
+int cm_mesh_create_wrapped(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
+                           const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream,
+                           cm_mesh **out);
 int cm_mesh_destroy(cm_mesh *mesh);
 /* Copies structure arrays to host_out (capacity in elements); returns BADARG if capacity is too small. */
 int cm_mesh_get(const cm_mesh *mesh, int what, void *host_out, long capacity);

@@ -29,7 +29,7 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
-EXPORTS = ("cm_mesh_create", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
+EXPORTS = ("cm_mesh_create", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
            "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_field_rhs", "cm_volume_average",
            "cm_gspm_step", "cm_gspm_step_host", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
@@ -76,6 +76,8 @@ def lib():
         L = C.CDLL(str(LIB_PATH))
         vp, lg, it, db = C.c_void_p, C.c_long, C.c_int, C.c_double
         L.cm_mesh_create.argtypes = [vp, lg, vp, lg, vp, vp, it, vp, C.POINTER(vp)]
+        L.cm_mesh_create_wrapped.argtypes = [vp, lg, vp, lg, vp, vp, vp, lg, it, vp, C.POINTER(vp)]
+        L.cm_periodic_wrap.argtypes = [vp, lg, C.c_uint, db, vp, C.POINTER(lg)]
         L.cm_mesh_destroy.argtypes = [vp]
         L.cm_mesh_get.argtypes = [vp, it, vp, lg]
         L.cm_assemble_csr.argtypes = [vp, C.POINTER(cm_material), it, db, vp, lg, vp, C.POINTER(vp)]
@@ -130,16 +132,32 @@ def make_params(dt, Hext=(0, 0, 0), terms=0, variant=0, cg_tol=1e-7, cg_maxiter=
                           int(cg_fixed_iters))
 
 
+def periodic_wrap(xyz, axes: int, rel_tol: float = 1e-9):
+    """cm_periodic_wrap: (dof_of_node int32[n_nodes], n_dof) for the periodic directions in the bit mask `axes`."""
+    xyz = _np(xyz, np.float64)
+    dof = np.empty(xyz.shape[0], np.int32)
+    nd = C.c_long()
+    _check(lib().cm_periodic_wrap(_hp(xyz), xyz.shape[0], int(axes), float(rel_tol), _hp(dof), C.byref(nd)))
+    return dof, int(nd.value)
+
+
 class Mesh:
     """cm_mesh_create: S0 preprocessing (reordering, node->element lists, CSR pattern)."""
 
-    def __init__(self, xyz, tets, magnetic=None, elastic_id=None, reorder=CM_REORDER_MORTON):
+    def __init__(self, xyz, tets, magnetic=None, elastic_id=None, reorder=CM_REORDER_MORTON, dof_of_node=None, n_dof=None):
+        """dof_of_node / n_dof (from periodic_wrap): cm_mesh_create_wrapped, the mesh then has n_dof "nodes"."""
         L = lib()
         xyz = _np(xyz, np.float64); tets = _np(tets, np.int32)
         mag = _np(magnetic, np.uint8); eid = _np(elastic_id, np.int32)
         self.h = C.c_void_p()
-        _check(L.cm_mesh_create(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), reorder, _stream(),
-                                C.byref(self.h)))
+        if dof_of_node is None:
+            _check(L.cm_mesh_create(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), reorder, _stream(),
+                                    C.byref(self.h)))
+        else:
+            dof = _np(dof_of_node, np.int32)
+            assert dof.shape[0] == xyz.shape[0]
+            _check(L.cm_mesh_create_wrapped(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), _hp(dof), int(n_dof),
+                                            reorder, _stream(), C.byref(self.h)))
         cnt = np.zeros(3, np.int64)
         _check(L.cm_mesh_get(self.h, CM_GET_COUNTS, _hp(cnt), 3))
         self.n_nodes, self.n_tets, self.nnz = (int(c) for c in cnt)

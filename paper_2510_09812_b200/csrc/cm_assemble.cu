@@ -40,7 +40,7 @@ __device__ __forceinline__ void tet_geometry(const double *__restrict__ xyz, con
 // one CTA per element chunk: V_e and grad phi_1..3 (rounded to T) into the chunk-blocked geometry array
 // (cm_internal.h), fp64 volume copy for the lumped masses
 template <typename T>
-__global__ void geom_kernel(const int *__restrict__ eptr, const int *__restrict__ tets, const double *__restrict__ xyz, double ld, T *EG,
+__global__ void geom_kernel(const int *__restrict__ eptr, const int *__restrict__ gtets, const double *__restrict__ xyz, double ld, T *EG,
                             double *Vd)
 {
     const int c = blockIdx.x, e0 = eptr[c], ne = eptr[c + 1] - e0, ne8 = (ne + 7) & ~7;
@@ -48,7 +48,7 @@ __global__ void geom_kernel(const int *__restrict__ eptr, const int *__restrict_
     for (int el = threadIdx.x; el < ne; el += blockDim.x) {
         const long e = e0 + el;
         int t[4];
-        *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(tets)[e];
+        *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(gtets)[e];
         TetGeom g;
         tet_geometry(xyz, t, ld, g);
         Vd[e] = g.V;
@@ -107,7 +107,8 @@ __device__ __forceinline__ void strain_disp(const double g[3], double B[6][3])
 
 // one thread per row i: accumulate scalar entries K (all tets), K_m, M_m (magnetic tets) and, if
 // Cstar != NULL, the 3x3 blocks of K^mech into fp64 scratch arrays laid out on the CSR pattern.
-__global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const double *__restrict__ xyz, double ld,
+__global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const int *__restrict__ gtets, const double *__restrict__ xyz,
+                                     double ld,
                                      const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const uchar *__restrict__ mag,
                                      const int *__restrict__ eid, const double *__restrict__ Cstar, const int *__restrict__ rowptr,
                                      const int *__restrict__ col, double *K, double *Km, double *Mm, double *Kme)
@@ -117,10 +118,11 @@ __global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const
     const int q0 = rowptr[i], q1 = rowptr[i + 1];
     for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
         const int e = n2e[s] >> 2, k = n2e[s] & 3;
-        int t[4];
+        int t[4], tg[4]; // DOF ids (matrix columns) and geometric node ids (coordinates; the same unless the mesh is wrapped)
         *reinterpret_cast<int4 *>(t) = reinterpret_cast<const int4 *>(tets)[e];
+        *reinterpret_cast<int4 *>(tg) = reinterpret_cast<const int4 *>(gtets)[e];
         TetGeom g;
-        tet_geometry(xyz, t, ld, g);
+        tet_geometry(xyz, tg, ld, g);
         const bool m = mag[e];
         double CBt[3][6]; // (B_k^T C): row r, Voigt column w
         if (Cstar) {
@@ -282,7 +284,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     CM_CUDA(cudaMalloc((void **)&Vd, Ne * sizeof(double)));
     CM_CUDA(cudaMalloc((void **)&vsum, 2 * sizeof(double)));
     const int B = 256;
-    geom_kernel<T><<<M->ck.nchunks, B, 0, st>>>(M->ck.d_eptr, M->d_tets, M->d_xyz, ld, S->EG, Vd);
+    geom_kernel<T><<<M->ck.nchunks, B, 0, st>>>(M->ck.d_eptr, M->d_gtets, M->d_gxyz, ld, S->EG, Vd);
     lump_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, M->d_n2e_ptr, M->d_n2e, Vd, M->d_mag, S->mL, S->mLm, S->live);
     volume_sum_kernel<<<1, 1024, 0, st>>>(Ne, Vd, M->d_mag, vsum);
     CM_CUDA(cudaGetLastError());
@@ -301,7 +303,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     CM_TRY(alloc(&K, nnz)); CM_TRY(alloc(&Km, nnz)); CM_TRY(alloc(&Mm, nnz));
     if (S->n_elastic) CM_TRY(alloc(&Kme, 9 * nnz));
     const int BA = 128;
-    assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_xyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag,
+    assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_gtets, M->d_gxyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag,
                                                                       M->d_eid, Cd, M->d_rowptr, M->d_col, K, Km, Mm, Kme);
     finalize_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, nnz, M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->live, S->clamp, S->pin,
                                                                  S->eps1, S->eps2, M->sell[0].d_sp, M->sell[1].d_sp, S->Kms, S->Kgs1, S->Kgs2,

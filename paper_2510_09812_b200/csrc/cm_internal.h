@@ -76,7 +76,15 @@ struct cm_mesh {
     // host copies, library order
     std::vector<int> order, iperm, tets, tet_order, rowptr, col, n2e_ptr, n2e, eid;
     std::vector<uchar> mag;
-    std::vector<double> xyz;   // N x 3 metres, library order
+    std::vector<double> xyz;   // N x 3 metres, library order (wrapped mesh: coordinates of the DOF's representative node)
+    // geometric connectivity: corner k of tet e has coordinates gxyz[gtets[4 e + k]].  Plain mesh: the same arrays as
+    // tets / xyz.  Wrapped (periodic): gtets holds the caller's node ids (library tet order), gxyz its xyz.
+    bool wrapped = false;
+    long Ng = 0;
+    std::vector<int> gtets;
+    std::vector<double> gxyz;
+    int *d_gtets = nullptr;    // == d_tets when !wrapped
+    double *d_gxyz = nullptr;  // == d_xyz when !wrapped
     std::vector<double> wvol;  // N: lumped volume fraction mL_i / V (sums to 1)
     // device
     int *d_order = nullptr, *d_tets = nullptr, *d_rowptr = nullptr, *d_col = nullptr, *d_n2e_ptr = nullptr, *d_n2e = nullptr,
@@ -163,8 +171,8 @@ struct System : SystemBase {
 };
 
 // ---- cm_mesh.cu ----
-int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long Ne, const uchar *mag, const int *eid,
-                    cm_reorder reorder);
+int mesh_build_host(cm_mesh *M, const double *xyz, long Ng, const int *gtets, long Ne, const uchar *mag, const int *eid,
+                    const int *dof, long N, cm_reorder reorder);
 int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out);
 int build_chunks(long N, long Ne, const int *tets, Chunks *out);
 

@@ -2,6 +2,7 @@
 // relabelled + sorted connectivity, node->element CSR, sparsity pattern, lumped volume fractions.
 // Host C++ (set-up, once per mesh; not in the timed step), results uploaded to the device.
 #include <algorithm>
+#include <limits>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -143,30 +144,62 @@ void rcm_order(long N, const std::vector<int> &rowptr, const std::vector<int> &c
 
 } // namespace
 
-int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long Ne, const uchar *mag, const int *eid,
-                    cm_reorder reorder)
+int mesh_build_host(cm_mesh *M, const double *gx, long Ng, const int *gtets, long Ne, const uchar *mag, const int *eid,
+                    const int *dof, long N, cm_reorder reorder)
 {
     M->N = N;
     M->Ne = Ne;
+    M->Ng = Ng;
+    M->wrapped = dof != nullptr;
     for (long q = 0; q < 4 * Ne; q++)
-        if (tets[q] < 0 || tets[q] >= N) {
-            cm_set_error("cm_mesh_create: tet %ld references node %d outside [0, %ld)", q / 4, tets[q], N);
+        if (gtets[q] < 0 || gtets[q] >= Ng) {
+            cm_set_error("cm_mesh_create: tet %ld references node %d outside [0, %ld)", q / 4, gtets[q], Ng);
             return CM_E_INDEX_RANGE;
         }
+    // DOF connectivity and DOF coordinates (wrapped mesh: componentwise minimum over the nodes of a DOF = its
+    // representative on the minimum faces)
+    std::vector<int> tets_v;
+    std::vector<double> xyz_v;
+    const int *tets = gtets;
+    const double *xyz = gx;
+    if (dof) {
+        for (long i = 0; i < Ng; i++)
+            if (dof[i] < 0 || dof[i] >= N) {
+                cm_set_error("cm_mesh_create_wrapped: dof_of_node[%ld] = %d outside [0, %ld)", i, dof[i], N);
+                return CM_E_INDEX_RANGE;
+            }
+        tets_v.resize(4 * Ne);
+        for (long q = 0; q < 4 * Ne; q++) tets_v[q] = dof[gtets[q]];
+        for (long e = 0; e < Ne; e++)
+            for (int a = 0; a < 4; a++)
+                for (int b2 = a + 1; b2 < 4; b2++)
+                    if (tets_v[4 * e + a] == tets_v[4 * e + b2]) {
+                        cm_set_error("cm_mesh_create_wrapped: tet %ld has two corners on DOF %d (domain one cell wide in a periodic direction)",
+                                     e, tets_v[4 * e + a]);
+                        return CM_E_BADARG;
+                    }
+        xyz_v.assign(3 * N, std::numeric_limits<double>::infinity());
+        for (long i = 0; i < Ng; i++)
+            for (int d = 0; d < 3; d++) xyz_v[3 * (long)dof[i] + d] = std::min(xyz_v[3 * (long)dof[i] + d], gx[3 * i + d]);
+        for (long i = 0; i < 3 * N; i++)
+            if (!std::isfinite(xyz_v[i])) { cm_set_error("cm_mesh_create_wrapped: DOF %ld has no node", i / 3); return CM_E_BADARG; }
+        tets = tets_v.data();
+        xyz = xyz_v.data();
+    }
     // geometry validation + lumped volume fractions (fp64, metres), user order
     double lo[3], hi[3];
-    for (int d = 0; d < 3; d++) lo[d] = hi[d] = xyz[d];
-    for (long i = 0; i < N; i++)
+    for (int d = 0; d < 3; d++) lo[d] = hi[d] = gx[d];
+    for (long i = 0; i < Ng; i++)
         for (int d = 0; d < 3; d++) {
-            lo[d] = std::min(lo[d], xyz[3 * i + d]);
-            hi[d] = std::max(hi[d], xyz[3 * i + d]);
+            lo[d] = std::min(lo[d], gx[3 * i + d]);
+            hi[d] = std::max(hi[d], gx[3 * i + d]);
         }
     double diag = std::sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
     double vmin = 1e-14 * diag * diag * diag, vtot = 0;
     std::vector<double> w_user(N, 0.0);
     for (long e = 0; e < Ne; e++) {
-        const double *x0 = xyz + 3 * (long)tets[4 * e], *x1 = xyz + 3 * (long)tets[4 * e + 1], *x2 = xyz + 3 * (long)tets[4 * e + 2],
-                     *x3 = xyz + 3 * (long)tets[4 * e + 3];
+        const double *x0 = gx + 3 * (long)gtets[4 * e], *x1 = gx + 3 * (long)gtets[4 * e + 1], *x2 = gx + 3 * (long)gtets[4 * e + 2],
+                     *x3 = gx + 3 * (long)gtets[4 * e + 3];
         double a[3], b[3], c[3];
         for (int d = 0; d < 3; d++) { a[d] = x1[d] - x0[d]; b[d] = x2[d] - x0[d]; c[d] = x3[d] - x0[d]; }
         double det = a[0] * (b[1] * c[2] - b[2] * c[1]) + a[1] * (b[2] * c[0] - b[0] * c[2]) + a[2] * (b[0] * c[1] - b[1] * c[0]);
@@ -221,6 +254,13 @@ int mesh_build_host(cm_mesh *M, const double *xyz, long N, const int *tets, long
         for (int k = 0; k < 4; k++) M->tets[4 * e + k] = M->iperm[tets[4 * old + k]];
         M->mag[e] = mag ? (mag[old] != 0) : 1;
         M->eid[e] = eid ? eid[old] : 0;
+    }
+    if (M->wrapped) {
+        M->gtets.resize(4 * Ne);
+#pragma omp parallel for schedule(static)
+        for (long e = 0; e < Ne; e++)
+            for (int k = 0; k < 4; k++) M->gtets[4 * e + k] = gtets[4 * (long)M->tet_order[e] + k];
+        M->gxyz.assign(gx, gx + 3 * Ng);
     }
     M->xyz.resize(3 * N);
     M->wvol.resize(N);
@@ -355,10 +395,104 @@ static int upload(U **dst, const std::vector<U> &src, cudaStream_t st)
     return CM_OK;
 }
 
+// P:233-235 (R23): sort-based pairing.  Representatives are sorted by their cell (side 4 tol) in lexicographic
+// order; the image of a wrapped node is looked up in its cell and the 26 neighbours by binary search.
+extern "C" int cm_periodic_wrap(const double *xyz, long n_nodes, unsigned axes, double rel_tol, int *dof_of_node, long *n_dof)
+{
+    if (!xyz || !dof_of_node || !n_dof || n_nodes <= 0 || n_nodes > 0x7fffffffL / 4 || !(rel_tol > 0) || rel_tol > 1e-3 || axes > 7u) {
+        cm_set_error("cm_periodic_wrap: bad argument");
+        return CM_E_BADARG;
+    }
+    const long N = n_nodes;
+    double lo[3], hi[3], span[3], tol[3], cell[3];
+    for (int d = 0; d < 3; d++) lo[d] = hi[d] = xyz[d];
+    for (long i = 0; i < N; i++)
+        for (int d = 0; d < 3; d++) {
+            lo[d] = std::min(lo[d], xyz[3 * i + d]);
+            hi[d] = std::max(hi[d], xyz[3 * i + d]);
+        }
+    for (int d = 0; d < 3; d++) {
+        span[d] = hi[d] - lo[d];
+        if (((axes >> d) & 1u) && !(span[d] > 0)) { cm_set_error("cm_periodic_wrap: zero extent along periodic direction %d", d); return CM_E_BADARG; }
+        tol[d] = rel_tol * span[d];
+        cell[d] = span[d] > 0 ? 4.0 * tol[d] : 1.0;
+    }
+    struct Rep { long long c[3]; int node; };
+    auto less = [](const Rep &a, const Rep &b) {
+        if (a.c[0] != b.c[0]) return a.c[0] < b.c[0];
+        if (a.c[1] != b.c[1]) return a.c[1] < b.c[1];
+        return a.c[2] < b.c[2];
+    };
+    try {
+        std::vector<Rep> reps;
+        std::vector<int> wrapped;
+        long nrep = 0;
+        for (long i = 0; i < N; i++) {
+            bool w = false;
+            for (int d = 0; d < 3; d++) w |= ((axes >> d) & 1u) && xyz[3 * i + d] >= hi[d] - tol[d];
+            if (w) { dof_of_node[i] = -1; wrapped.push_back((int)i); continue; }
+            dof_of_node[i] = (int)nrep++;
+            Rep r;
+            for (int d = 0; d < 3; d++) r.c[d] = (long long)std::floor((xyz[3 * i + d] - lo[d]) / cell[d]);
+            r.node = (int)i;
+            reps.push_back(r);
+        }
+        *n_dof = nrep;
+        std::sort(reps.begin(), reps.end(), less);
+        int bad = -1;
+#pragma omp parallel for schedule(static)
+        for (long q = 0; q < (long)wrapped.size(); q++) {
+            const int i = wrapped[q];
+            double w[3];
+            long long c[3];
+            for (int d = 0; d < 3; d++) {
+                w[d] = xyz[3 * (long)i + d];
+                if (((axes >> d) & 1u) && w[d] >= hi[d] - tol[d]) w[d] -= span[d];
+                c[d] = (long long)std::floor((w[d] - lo[d]) / cell[d]);
+            }
+            int found = -1, count = 0;
+            for (int a = -1; a <= 1; a++)
+                for (int b = -1; b <= 1; b++)
+                    for (int g = -1; g <= 1; g++) {
+                        Rep key;
+                        key.c[0] = c[0] + a; key.c[1] = c[1] + b; key.c[2] = c[2] + g; key.node = 0;
+                        for (auto it = std::lower_bound(reps.begin(), reps.end(), key, less); it != reps.end() && !less(key, *it); ++it) {
+                            const double *x = xyz + 3 * (long)it->node;
+                            if (std::fabs(x[0] - w[0]) <= tol[0] && std::fabs(x[1] - w[1]) <= tol[1] && std::fabs(x[2] - w[2]) <= tol[2]) {
+                                found = it->node;
+                                count++;
+                            }
+                        }
+                    }
+            if (count == 1) dof_of_node[i] = dof_of_node[found];
+            else {
+#pragma omp critical
+                bad = i;
+            }
+        }
+        if (bad >= 0) {
+            cm_set_error("cm_periodic_wrap: node %d on a periodic maximum face has no unique partner on the minimum face (P:235: matched faces required)", bad);
+            return CM_E_BADARG;
+        }
+    } catch (const std::bad_alloc &) {
+        cm_set_error("cm_periodic_wrap: out of host memory");
+        return CM_E_ALLOC;
+    }
+    return CM_OK;
+}
+
 extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
                               const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out)
 {
-    if (!xyz || !tets || !out || n_nodes <= 0 || n_tets <= 0 || n_nodes > 0x7fffffffL / 4 || n_tets > 0x7fffffffL / 16) {
+    return cm_mesh_create_wrapped(xyz, n_nodes, tets, n_tets, magnetic, elastic_id, nullptr, n_nodes, reorder, stream, out);
+}
+
+extern "C" int cm_mesh_create_wrapped(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
+                                      const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream,
+                                      cm_mesh **out)
+{
+    if (!xyz || !tets || !out || n_nodes <= 0 || n_tets <= 0 || n_nodes > 0x7fffffffL / 4 || n_tets > 0x7fffffffL / 16 || n_dof <= 0 ||
+        n_dof > n_nodes || (!dof_of_node && n_dof != n_nodes)) {
         cm_set_error("cm_mesh_create: bad argument");
         return CM_E_BADARG;
     }
@@ -372,7 +506,7 @@ extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, 
     if (!M) return CM_E_ALLOC;
     int rc;
     try {
-        rc = mesh_build_host(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, reorder);
+        rc = mesh_build_host(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, dof_of_node, n_dof, reorder);
     } catch (const std::bad_alloc &) {
         cm_set_error("cm_mesh_create: out of host memory");
         rc = CM_E_ALLOC;
@@ -389,6 +523,13 @@ extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, 
             CM_TRY(upload(&M->d_mag, M->mag, st));
             CM_TRY(upload(&M->d_xyz, M->xyz, st));
             CM_TRY(upload(&M->d_wvol, M->wvol, st));
+            if (M->wrapped) {
+                CM_TRY(upload(&M->d_gtets, M->gtets, st));
+                CM_TRY(upload(&M->d_gxyz, M->gxyz, st));
+            } else {
+                M->d_gtets = M->d_tets;
+                M->d_gxyz = M->d_xyz;
+            }
             for (Sell &L : M->sell) {
                 CM_TRY(upload(&L.d_sp, L.sp, st));
                 CM_TRY(upload(&L.d_col, L.col, st));
@@ -419,6 +560,7 @@ extern "C" int cm_mesh_destroy(cm_mesh *M)
     cudaFree(M->d_order); cudaFree(M->d_tets); cudaFree(M->d_rowptr); cudaFree(M->d_col); cudaFree(M->d_n2e_ptr);
     cudaFree(M->d_n2e); cudaFree(M->d_eid); cudaFree(M->d_mag); cudaFree(M->d_xyz); cudaFree(M->d_wvol);
     cudaFree(M->d_red); cudaFree(M->d_tmp);
+    if (M->wrapped) { cudaFree(M->d_gtets); cudaFree(M->d_gxyz); }
     for (Sell &L : M->sell) { cudaFree(L.d_sp); cudaFree(L.d_col); }
     Chunks &K = M->ck;
     cudaFree(K.d_eptr); cudaFree(K.d_nptr); cudaFree(K.d_nodes); cudaFree(K.d_ns_ptr); cudaFree(K.d_ns_slot);

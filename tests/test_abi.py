@@ -61,3 +61,21 @@ def test_product_does_not_import_oracle():
     assert "cupymag_b200.h" not in src and "#include \"../" not in src
     py = (ROOT / "oracle" / "__init__.py").read_text()
     assert "import paper_2510_09812_b200" not in py and "from paper_2510_09812_b200" not in py
+
+
+@pytest.mark.parametrize("axes", [1, 2, 5, 7])
+def test_periodic_wrap_host_logic_matches_oracle(binding, oracle_mod, axes):
+    """cm_periodic_wrap is host code (no device needed): bit-exact against the oracle's hash-map wrap."""
+    import numpy as np
+    from paper_2510_09812_b200 import inputs
+    for grid, box in (((5, 4, 6), (20e-9, 12e-9, 25e-9)), ((33, 21, 17), (200e-9, 120e-9, 50e-9))):
+        mesh = inputs.kuhn_box(grid, box, seed_mesh=3, seed_perm=4)
+        dof, nd = binding.periodic_wrap(mesh.xyz, axes)
+        dof_o, nd_o = oracle_mod.periodic_wrap(mesh.xyz, axes)
+        assert nd == nd_o and np.array_equal(dof, dof_o)
+    xyz = mesh.xyz.copy()
+    i = np.flatnonzero((xyz[:, 0] == xyz[:, 0].max()) & (xyz[:, 1] > 0) & (xyz[:, 1] < xyz[:, 1].max()))[0]
+    xyz[i, 1] += 1e-10
+    with pytest.raises(binding.CmError) as ei:
+        binding.periodic_wrap(xyz, 1)
+    assert ei.value.code == binding.CM_E_BADARG
