@@ -56,6 +56,15 @@ class StepInfo(C.Structure):
                 ("mean_dm", C.c_double), ("energy", C.c_double)]
 
 
+class _HystParams(C.Structure):
+    _fields_ = [("H0", C.c_double * 3), ("dH", C.c_double * 3), ("conv_tol", C.c_double), ("max_fields", C.c_int),
+                ("max_steps", C.c_int)]
+
+
+class HystResult(C.Structure):
+    _fields_ = [("n_fields", C.c_int), ("reversed", C.c_int), ("total_steps", C.c_long)]
+
+
 _libs = {}
 
 
@@ -68,7 +77,7 @@ def _lib(dtype: str):
         L.orc_nnz.restype = C.c_long
         for name in ("orc_scalar", "orc_nnz", "orc_get", "orc_get_values", "orc_spmv", "orc_cg", "orc_volume_average",
                      "orc_rhs_ms", "orc_demag_field", "orc_rhs_mech", "orc_stress_recover", "orc_field", "orc_energy",
-                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap"):
+                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run"):
             getattr(L, name).argtypes = None
         _libs[dtype] = L
     return _libs[dtype]
@@ -262,3 +271,16 @@ class Oracle:
         info = StepInfo()
         rc = self.L.orc_gspm_step(self.h, C.byref(p), _p(m), _p(U), _p(u), C.byref(info))
         return info, rc
+
+    def hysteresis_run(self, m, U, u, dt, H0, dH, terms, conv_tol=5e-10, max_fields=100, max_steps=100000, variant=0,
+                       cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1):
+        """in place on m, U, u.  Returns (H_log, mbar_log, steps_log, HystResult, rc), logs cut to n_fields."""
+        for a in (m, U, u):
+            assert a.dtype == self.real and a.flags.c_contiguous
+        p = _StepParams(dt, (C.c_double * 3)(0, 0, 0), terms, variant, cg_tol, cg_maxiter, cg_fixed_iters)
+        hp = _HystParams((C.c_double * 3)(*H0), (C.c_double * 3)(*dH), conv_tol, max_fields, max_steps)
+        Hl = np.zeros((max_fields, 3)); ml = np.zeros((max_fields, 3)); sl = np.zeros(max_fields, np.int32)
+        res = HystResult()
+        rc = self.L.orc_hysteresis_run(self.h, C.byref(p), C.byref(hp), _p(m), _p(U), _p(u), _p(Hl), _p(ml), _p(sl), C.byref(res))
+        n = res.n_fields
+        return Hl[:n], ml[:n], sl[:n], res, rc

@@ -1023,6 +1023,59 @@ int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_,
 }
 
 /* Helmholtz right-hand side b = M_m f for all three components (Eq. 14) */
+/* ------------------------------------------------------------------------------------ */
+/* Hysteresis driver (R24)               */
+/* ------------------------------------------------------------------------------------ */
+/* "The external field H_ext is decreased in increments up to a critical coercive field H_c, at which the magnetization
+ * field in the domain reverses"; at each field "the LLG equation is solved iteratively by GSPM until
+ * <||m^n - m^{n-1}||_2>_DOF < 5e-10"; "the external field is reduced in intervals of dH = -20 A/m";
+ * the average magnetisation and H_ext are written at convergence (Fig. 1).
+ * Field k is H0 + k dH.  At each field: GSPM steps until mean_dm < conv_tol (or max_steps at that field); then the
+ * volume average of the converged m (Eq. 17) is logged with H and the step count.  The run ends when that average has
+ * a negative component along e0 = H0/|H0| (reversal), or after max_fields fields. */
+typedef struct {
+    double H0[3], dH[3];   /* A/m */
+    double conv_tol;       /* on <||dm||_2> */
+    int max_fields, max_steps;
+} orc_hyst_params;
+
+typedef struct {
+    int n_fields, reversed;
+    long total_steps;
+} orc_hyst_result;
+
+int orc_hysteresis_run(const oracle *o, const orc_step_params *base, const orc_hyst_params *hp, void *m, void *U, void *u,
+                       double *H_log, double *mbar_log, int *steps_log, orc_hyst_result *res)
+{
+    if (!o || !base || !hp || !m || !H_log || !mbar_log || !steps_log || !res || hp->max_fields < 1 || hp->max_steps < 1)
+        return ORC_E_BADARG;
+    double n0 = sqrt(hp->H0[0] * hp->H0[0] + hp->H0[1] * hp->H0[1] + hp->H0[2] * hp->H0[2]);
+    if (!(n0 > 0)) return ORC_E_BADARG;
+    double e0[3] = {hp->H0[0] / n0, hp->H0[1] / n0, hp->H0[2] / n0};
+    res->n_fields = 0; res->reversed = 0; res->total_steps = 0;
+    int worst = ORC_OK;
+    for (int k = 0; k < hp->max_fields; k++) {
+        orc_step_params p = *base;
+        for (int d = 0; d < 3; d++) p.Hext[d] = hp->H0[d] + (double)k * hp->dH[d];
+        int steps = 0;
+        for (;;) {
+            orc_step_info info;
+            int rc = orc_gspm_step(o, &p, m, U, u, &info);
+            if (rc == ORC_E_BADARG || rc == ORC_E_ALLOC) return rc;
+            if (rc < worst) worst = rc;
+            steps++; res->total_steps++;
+            if (info.mean_dm < hp->conv_tol || steps >= hp->max_steps) break;
+        }
+        double mbar[3];
+        orc_volume_average(o, m, 3, mbar);
+        for (int d = 0; d < 3; d++) { H_log[3 * k + d] = p.Hext[d]; mbar_log[3 * k + d] = mbar[d]; }
+        steps_log[k] = steps;
+        res->n_fields = k + 1;
+        if (mbar[0] * e0[0] + mbar[1] * e0[1] + mbar[2] * e0[2] < 0) { res->reversed = 1; break; }
+    }
+    return worst;
+}
+
 int orc_rhs_gs(const oracle *o, const void *f_, void *b_)
 {
     for (int a = 0; a < 3; a++) spmv(o, MAT_MASS, (const real *)f_, (real *)b_, 3, a);
