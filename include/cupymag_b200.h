@@ -193,6 +193,32 @@ int cm_gspm_step(cm_system *sys, const cm_step_params *params, void *m_dev, void
 int cm_gspm_step_host(cm_system *sys, const cm_step_params *params, void *m_host, void *U_host, void *u_host,
                       cm_step_info *info, void *stream);
 
+/* Hysteresis driver (Fig. 1; R24).  Field k is H0 + k dH.  At each field GSPM
+ * steps run until <||m^{n+1} - m^n||_2> over magnetic nodes < conv_tol (5e-10) or max_steps steps; then the volume
+ * average of the converged m (Eq. 17), H and the step count are logged ("written at convergence").  The run ends
+ * when that average has a negative component along H0/|H0| ("the magnetization field in the domain reverses") or
+ * after max_fields fields. */
+typedef struct {
+    double H0[3], dH[3]; /* A/m; 200 A/m e1, -20 A/m e1 */
+    double conv_tol;
+    int max_fields, max_steps;
+} cm_hyst_params;
+typedef struct {
+    int n_fields, reversed;
+    long total_steps;
+    long cg_iters_ms, cg_iters_mech, cg_passes_gs; /* summed over all steps */
+    int worst_cg_status;                           /* CM_OK, CM_E_CG_MAXITER or CM_E_CG_BREAKDOWN */
+    double device_ms;                              /* CUDA-event time of the whole loop */
+} cm_hyst_result;
+/* The WHOLE loop runs on the device: one CUDA graph whose body (one GSPM step with the applied field read from device
+ * memory, the average of the new m, a one-thread controller that tests convergence, logs, decrements the field and
+ * detects reversal) sits in a conditional WHILE node; the host launches it once and synchronises once.
+ * base: step parameters (Hext ignored).  m_dev, U_dev, u_dev: in/out as in cm_gspm_step.  H_log, mbar_log (host,
+ * max_fields x 3) and steps_log (host, max_fields): filled for the first result->n_fields fields.
+ * Returns CM_OK, or the worst CG status.  Errors: BADARG (H0 = 0, non-positive caps, null pointers), CUDA. */
+int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, const cm_hyst_params *hp, void *m_dev, void *U_dev, void *u_dev,
+                      double *H_log, double *mbar_log, int *steps_log, cm_hyst_result *result, void *stream);
+
 int cm_profile_enable(cm_system *sys, int on);
 int cm_profile_get(cm_system *sys, cm_profile *out); /* synchronises outstanding timers */
 int cm_profile_reset(cm_system *sys);

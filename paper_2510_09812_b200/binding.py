@@ -31,7 +31,7 @@ PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
 EXPORTS = ("cm_mesh_create", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
            "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_field_rhs", "cm_volume_average",
-           "cm_gspm_step", "cm_gspm_step_host", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
+           "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
 
 
@@ -56,6 +56,16 @@ class cm_step_info(C.Structure):
     _fields_ = [("it_ms", C.c_int), ("it_mech", C.c_int), ("it_gs", C.c_int * 8), ("res_ms", C.c_double),
                 ("res_mech", C.c_double), ("res_gs", C.c_double * 8), ("mbar", C.c_double * 3), ("mean_dm", C.c_double),
                 ("energy", C.c_double)]
+
+
+class cm_hyst_params(C.Structure):
+    _fields_ = [("H0", C.c_double * 3), ("dH", C.c_double * 3), ("conv_tol", C.c_double), ("max_fields", C.c_int),
+                ("max_steps", C.c_int)]
+
+
+class cm_hyst_result(C.Structure):
+    _fields_ = [("n_fields", C.c_int), ("reversed", C.c_int), ("total_steps", C.c_long), ("cg_iters_ms", C.c_long),
+                ("cg_iters_mech", C.c_long), ("cg_passes_gs", C.c_long), ("worst_cg_status", C.c_int), ("device_ms", C.c_double)]
 
 
 class cm_profile(C.Structure):
@@ -92,6 +102,8 @@ def lib():
         L.cm_volume_average.argtypes = [vp, it, vp, it, C.POINTER(db), vp]
         L.cm_gspm_step.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
         L.cm_gspm_step_host.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
+        L.cm_hysteresis_run.argtypes = [vp, C.POINTER(cm_step_params), C.POINTER(cm_hyst_params), vp, vp, vp, vp, vp, vp,
+                                        C.POINTER(cm_hyst_result), vp]
         L.cm_profile_enable.argtypes = [vp, it]
         L.cm_profile_get.argtypes = [vp, C.POINTER(cm_profile)]
         L.cm_profile_reset.argtypes = [vp]
@@ -285,6 +297,21 @@ class System:
         rc = _check(lib().cm_gspm_step_host(self.h, C.byref(params), hp(m), hp(U), hp(u), C.byref(info), _stream()),
                     allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
         return info, rc
+
+    def hysteresis_run(self, params: cm_step_params, m, U, u, H0, dH, conv_tol=5e-10, max_fields=100, max_steps=100000):
+        """cm_hysteresis_run: the whole field loop on the device (one CUDA graph launch).
+        Returns (H_log, mbar_log, steps_log, cm_hyst_result, rc) with the logs cut to n_fields."""
+        for t in (m, U, u):
+            if t is not None:
+                self._chk(t)
+        hp = cm_hyst_params((C.c_double * 3)(*[float(x) for x in H0]), (C.c_double * 3)(*[float(x) for x in dH]), conv_tol,
+                            int(max_fields), int(max_steps))
+        Hl = np.zeros((max_fields, 3)); ml = np.zeros((max_fields, 3)); sl = np.zeros(max_fields, np.int32)
+        res = cm_hyst_result()
+        rc = _check(lib().cm_hysteresis_run(self.h, C.byref(params), C.byref(hp), _dp(m), _dp(U), _dp(u), _hp(Hl), _hp(ml), _hp(sl),
+                                            C.byref(res), _stream()), allow=(CM_E_CG_MAXITER, CM_E_CG_BREAKDOWN))
+        n = res.n_fields
+        return Hl[:n], ml[:n], sl[:n], res, rc
 
     def profile_enable(self, on=True):
         _check(lib().cm_profile_enable(self.h, int(on)))

@@ -352,6 +352,17 @@ extern "C" int cm_gspm_step_host(cm_system *sys, const cm_step_params *params, v
                         api_step_host<float>(S, params, m_host, U_host, u_host, info, st));
 }
 
+// ---------------------------------------------------------------- hysteresis driver
+extern "C" int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, const cm_hyst_params *hp, void *m_dev, void *U_dev,
+                                 void *u_dev, double *H_log, double *mbar_log, int *steps_log, cm_hyst_result *result, void *stream)
+{
+    CM_TRY(check_sys(sys, "cm_hysteresis_run"));
+    if (!base || !hp) { cm_set_error("cm_hysteresis_run: null params"); return CM_E_BADARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return SYS_DISPATCH(sys, sys_hysteresis<double>(S, base, hp, (double *)m_dev, (double *)U_dev, (double *)u_dev, H_log, mbar_log, steps_log, result, st),
+                        sys_hysteresis<float>(S, base, hp, (float *)m_dev, (float *)U_dev, (float *)u_dev, H_log, mbar_log, steps_log, result, st));
+}
+
 // ---------------------------------------------------------------- profile
 extern "C" int cm_profile_enable(cm_system *sys, int on)
 {

@@ -204,6 +204,7 @@ System<T>::~System()
     T *ptrs[] = {EG, mL, mLm, Cstar, Ccub, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
+    cudaFree(hyst_ctl); cudaFree(hyst_log); cudaFree(hyst_steps);
     if (h_res) cudaFreeHost(h_res);
     if (h_scal) cudaFreeHost(h_scal);
 }

@@ -433,10 +433,12 @@ __global__ void node_hd_kernel(long N, const int *__restrict__ ns_ptr, const int
 template <typename T>
 __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                   const T *__restrict__ mLm, const uchar *__restrict__ live, const T *__restrict__ w,
-                                  const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, T l1, T l2, T *h, T *sig_out)
+                                  const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, const double *__restrict__ hext_dev,
+                                  T l1, T l2, T *h, T *sig_out)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
+    if (hext_dev) { hx = (T)hext_dev[0]; hy = (T)hext_dev[1]; hz = (T)hext_dev[2]; } // device-resident field (hysteresis driver)
     T hi[3] = {0, 0, 0}, s[6] = {0, 0, 0, 0, 0, 0};
     if (live[i]) {
         const T m[3] = {w[3 * i], w[3 * i + 1], w[3 * i + 2]};
@@ -677,13 +679,14 @@ int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st)
 }
 
 template <typename T>
-int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h, T *sig_out, cudaStream_t st)
+int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h, T *sig_out, cudaStream_t st,
+              const double *hext_dev)
 {
     const Chunks &K = S->mesh->ck;
     S->prof.begin(CM_PROF_ELEMENT, st);
     node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mLm, S->live, w_lib, hd, terms,
-                                                   (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], (T)S->lam100, (T)S->lam111, h,
-                                                   sig_out);
+                                                   (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], hext_dev, (T)S->lam100,
+                                                   (T)S->lam111, h, sig_out);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -703,28 +706,35 @@ int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t 
 // one GSPM step (O-3)
 // ------------------------------------------------------------------------------------------------
 template <typename T>
-int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_user, cm_step_info *info, cudaStream_t st)
+static int step_check(System<T> *S, const cm_step_params *p, const T *m_user, const T *U_user, const T *u_user, const char *fn)
+{
+    const unsigned terms = p->terms;
+    if (p->dt != S->dt) { cm_set_error("%s: params->dt differs from the dt given to cm_assemble_csr", fn); return CM_E_BADARG; }
+    if ((terms & CM_TERM_MAGEL) && !S->n_elastic) { cm_set_error("%s: MAGEL needs elastic constants", fn); return CM_E_BADARG; }
+    if (((terms & CM_TERM_DEMAG) && !U_user) || ((terms & CM_TERM_MAGEL) && !u_user) || !m_user) {
+        cm_set_error("%s: null field pointer", fn);
+        return CM_E_BADARG;
+    }
+    return CM_OK;
+}
+
+// Items 1-10 of O-3 on the library-order state S->m, S->U, S->u.  hext_dev != NULL: the nondimensional applied field is
+// read from device memory (3 doubles) by the field kernels instead of params->Hext, so that the same enqueued work --
+// or a captured graph of it -- follows a field that changes on the device.  Ends with <||dm||> in S->dscal[6].
+template <typename T>
+static int step_core(System<T> *S, const cm_step_params *p, const double *hext_dev, cudaStream_t st)
 {
     const long N = S->N;
     const unsigned terms = p->terms;
-    if (p->dt != S->dt) { cm_set_error("cm_gspm_step: params->dt differs from the dt given to cm_assemble_csr"); return CM_E_BADARG; }
-    if ((terms & CM_TERM_MAGEL) && !S->n_elastic) { cm_set_error("cm_gspm_step: MAGEL needs elastic constants"); return CM_E_BADARG; }
-    if (((terms & CM_TERM_DEMAG) && !U_user) || ((terms & CM_TERM_MAGEL) && !u_user) || !m_user) {
-        cm_set_error("cm_gspm_step: null field pointer");
-        return CM_E_BADARG;
-    }
     const double hext[3] = {p->Hext[0] / S->Ms, p->Hext[1] / S->Ms, p->Hext[2] / S->Ms};
     const T dtau = (T)S->dtau, adtau = (T)(S->alpha * S->dtau);
     const double tol = p->cg_tol;
     const int mx = p->cg_maxiter, fx = p->cg_fixed_iters;
     CM_CUDA(cudaMemsetAsync(S->d_res, 0, 8 * sizeof(CgResult), st));
-
-    CM_TRY(sys_permute_in(S, m_user, S->m, 3, st));
     // 1. mbar (Eq. 17)
     CM_TRY(sys_mbar(S, S->m, st));
     // 2. magnetostatic solve, warm start (Eq. 5, 9)
     if (terms & CM_TERM_DEMAG) {
-        CM_TRY(sys_permute_in(S, U_user, S->U, 1, st));
         CM_TRY(sys_rhs_ms(S, S->m, S->bvec, st));
         CM_TRY(sys_cg(S, CM_MAT_K_MS, MODE_CSR1, S->bvec, S->U, tol, mx, fx, 1u, 0, CM_PROF_CG_MS, st));
     }
@@ -732,13 +742,12 @@ int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_u
     if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) CM_TRY(sys_demag_field(S, S->U, terms, S->hd, st));
     // 4. mechanical equilibrium (Eq. 6, 10), warm start; stress at m^n
     if (terms & CM_TERM_MAGEL) {
-        CM_TRY(sys_permute_in(S, u_user, S->u, 3, st));
         CM_TRY(sys_rhs_mech(S, S->m, S->bvec, st));
         CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, st));
         CM_TRY(sys_stress(S, S->u, S->m, st));
     }
     // 5. h[m^n];  6. Step 1: g^n
-    CM_TRY(sys_field(S, S->m, S->hd, hext, terms, S->hn, (T *)nullptr, st));
+    CM_TRY(sys_field(S, S->m, S->hd, hext, terms, S->hn, (T *)nullptr, st, hext_dev));
     CM_TRY(sys_axpby3(S, S->m, S->hn, dtau, S->f, st));
     CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
     CM_CUDA(cudaMemcpyAsync(S->gn, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
@@ -771,7 +780,7 @@ int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_u
     LAUNCH_CHECK();
     // 8. Step 3: h* = h[m*] with U, u frozen (R3)
     if (terms & CM_TERM_MAGEL) CM_TRY(sys_stress(S, S->u, S->ms, st));
-    CM_TRY(sys_field(S, S->ms, S->hd, hext, terms, S->hn, (T *)nullptr, st));
+    CM_TRY(sys_field(S, S->ms, S->hd, hext, terms, S->hn, (T *)nullptr, st, hext_dev));
     CM_TRY(sys_axpby3(S, S->ms, S->hn, adtau, S->f, st));
     CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
     CM_CUDA(cudaMemcpyAsync(S->mss, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
@@ -785,6 +794,18 @@ int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_u
         S->prof.end(st);
         LAUNCH_CHECK();
     }
+    return CM_OK;
+}
+
+template <typename T>
+int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_user, cm_step_info *info, cudaStream_t st)
+{
+    const unsigned terms = p->terms;
+    CM_TRY(step_check(S, p, m_user, U_user, u_user, "cm_gspm_step"));
+    CM_TRY(sys_permute_in(S, m_user, S->m, 3, st));
+    if (terms & CM_TERM_DEMAG) CM_TRY(sys_permute_in(S, U_user, S->U, 1, st));
+    if (terms & CM_TERM_MAGEL) CM_TRY(sys_permute_in(S, u_user, S->u, 3, st));
+    CM_TRY(step_core(S, p, (const double *)nullptr, st));
     CM_TRY(sys_permute_out(S, S->m, m_user, 3, st));
     if (terms & CM_TERM_DEMAG) CM_TRY(sys_permute_out(S, S->U, U_user, 1, st));
     if (terms & CM_TERM_MAGEL) CM_TRY(sys_permute_out(S, S->u, u_user, 3, st));
@@ -822,6 +843,150 @@ int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_u
     return worst;
 }
 
+// ------------------------------------------------------------------------------------------------
+// hysteresis driver (R24): the whole loop on the device
+// ------------------------------------------------------------------------------------------------
+struct HystCtl {
+    double H[3], hnd[3];      // current field (A/m) and H / Ms, read by the field kernels
+    double H0[3], dH[3], e0[3], Ms, conv_tol;
+    int k, steps, done, reversed, max_fields, max_steps, worst, variant;
+    long total, it_ms, it_mech, gs_passes;
+};
+
+// One thread, after every step: dscal[0..2] = volume average of the NEW m, dscal[6] = <||dm||>.
+__global__ void hyst_control_kernel(HystCtl *c, const double *__restrict__ dscal, const CgResult *__restrict__ R, double *log, int *slog,
+                                    int cap, cudaGraphConditionalHandle handle)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    c->steps++;
+    c->total++;
+    c->it_ms += R[0].iters[0];
+    c->it_mech += R[1].iters[0];
+    for (int s = 2; s < 6; s++) c->gs_passes += max(R[s].iters[0], max(R[s].iters[1], R[s].iters[2]));
+    for (int s = 0; s < 6; s++) c->worst = min(c->worst, R[s].status);
+    if (dscal[6] < c->conv_tol || c->steps >= c->max_steps) {
+        const int k = c->k;
+        for (int d = 0; d < 3; d++) { log[3 * k + d] = c->H[d]; log[3 * (cap + k) + d] = dscal[d]; }
+        slog[k] = c->steps;
+        const double proj = dscal[0] * c->e0[0] + dscal[1] * c->e0[1] + dscal[2] * c->e0[2];
+        if (proj < 0) { c->reversed = 1; c->done = 1; }
+        else if (k + 1 >= c->max_fields) c->done = 1;
+        c->k = k + 1;
+        if (!c->done) {
+            c->steps = 0;
+            for (int d = 0; d < 3; d++) {
+                c->H[d] = __dadd_rn(c->H0[d], __dmul_rn((double)(k + 1), c->dH[d])); // H0 + k dH, product rounded first (no FMA)
+                c->hnd[d] = c->H[d] / c->Ms;
+            }
+        }
+    }
+    cudaGraphSetConditional(handle, c->done ? 0u : 1u);
+}
+
+template <typename T>
+int sys_hysteresis(System<T> *S, const cm_step_params *base, const cm_hyst_params *hp, T *m_user, T *U_user, T *u_user, double *H_log,
+                   double *mbar_log, int *steps_log, cm_hyst_result *res, cudaStream_t st)
+{
+    const unsigned terms = base->terms;
+    CM_TRY(step_check(S, base, m_user, U_user, u_user, "cm_hysteresis_run"));
+    const double n0 = std::sqrt(hp->H0[0] * hp->H0[0] + hp->H0[1] * hp->H0[1] + hp->H0[2] * hp->H0[2]);
+    if (!(n0 > 0) || hp->max_fields < 1 || hp->max_steps < 1 || !H_log || !mbar_log || !steps_log || !res) {
+        cm_set_error("cm_hysteresis_run: H0 must be non-zero, max_fields and max_steps positive, outputs non-null");
+        return CM_E_BADARG;
+    }
+    const int cap = hp->max_fields;
+    if (!S->hyst_ctl) CM_CUDA(cudaMalloc(&S->hyst_ctl, sizeof(HystCtl)));
+    if (S->hyst_cap < cap) {
+        cudaFree(S->hyst_log); cudaFree(S->hyst_steps);
+        S->hyst_log = nullptr; S->hyst_steps = nullptr; S->hyst_cap = 0;
+        CM_CUDA(cudaMalloc((void **)&S->hyst_log, (size_t)cap * 6 * sizeof(double)));
+        CM_CUDA(cudaMalloc((void **)&S->hyst_steps, (size_t)cap * sizeof(int)));
+        S->hyst_cap = cap;
+    }
+    HystCtl h0;
+    std::memset(&h0, 0, sizeof(h0));
+    for (int d = 0; d < 3; d++) {
+        h0.H[d] = h0.H0[d] = hp->H0[d]; h0.dH[d] = hp->dH[d]; h0.e0[d] = hp->H0[d] / n0; h0.hnd[d] = hp->H0[d] / S->Ms;
+    }
+    h0.Ms = S->Ms; h0.conv_tol = hp->conv_tol; h0.max_fields = hp->max_fields; h0.max_steps = hp->max_steps; h0.worst = CM_OK;
+    HystCtl *ctl = (HystCtl *)S->hyst_ctl;
+    CM_CUDA(cudaMemcpyAsync(ctl, &h0, sizeof(h0), cudaMemcpyHostToDevice, st));
+    CM_CUDA(cudaMemsetAsync(S->hyst_log, 0, (size_t)cap * 6 * sizeof(double), st));
+    CM_CUDA(cudaMemsetAsync(S->hyst_steps, 0, (size_t)cap * sizeof(int), st));
+    CM_TRY(sys_permute_in(S, m_user, S->m, 3, st));
+    if (terms & CM_TERM_DEMAG) CM_TRY(sys_permute_in(S, U_user, S->U, 1, st));
+    if (terms & CM_TERM_MAGEL) CM_TRY(sys_permute_in(S, u_user, S->u, 3, st));
+    CM_CUDA(cudaStreamSynchronize(st)); // h0 is on this stack frame
+
+    // ---- graph: WHILE (not done) { one GSPM step; average of the new m; controller }
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    const bool prof_on = S->prof.on;
+    S->prof.on = false; // no event records inside a conditional body
+    cudaStream_t cs = nullptr; // capture stream: the caller's may be the legacy default stream, which cannot capture
+    auto build = [&]() -> int {
+        CM_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+        CM_CUDA(cudaGraphCreate(&graph, 0));
+        cudaGraphConditionalHandle handle;
+        CM_CUDA(cudaGraphConditionalHandleCreate(&handle, graph, 1, cudaGraphCondAssignDefault));
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t node;
+        CM_CUDA(cudaGraphAddNode(&node, graph, nullptr, 0, &np));
+        cudaGraph_t body = np.conditional.phGraph_out[0];
+        CM_CUDA(cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+        int rc = step_core(S, base, ctl->hnd, cs);
+        if (rc == CM_OK) rc = sys_mbar(S, S->m, cs);
+        if (rc == CM_OK) {
+            hyst_control_kernel<<<1, 32, 0, cs>>>(ctl, S->dscal, S->d_res, S->hyst_log, S->hyst_steps, cap, handle);
+            if (cudaGetLastError() != cudaSuccess) rc = CM_E_CUDA;
+        }
+        cudaGraph_t captured = nullptr;
+        cudaError_t e = cudaStreamEndCapture(cs, &captured);
+        if (rc != CM_OK) return rc;
+        if (e != cudaSuccess) { cm_set_error("cm_hysteresis_run: stream capture failed: %s", cudaGetErrorString(e)); return CM_E_CUDA; }
+        CM_CUDA(cudaGraphInstantiate(&exec, graph, 0));
+        return CM_OK;
+    };
+    int rc = build();
+    S->prof.on = prof_on;
+    cudaEvent_t ea = nullptr, eb = nullptr;
+    auto run = [&]() -> int {
+        CM_CUDA(cudaEventCreate(&ea));
+        CM_CUDA(cudaEventCreate(&eb));
+        CM_CUDA(cudaEventRecord(ea, st));
+        CM_CUDA(cudaGraphLaunch(exec, st));
+        CM_CUDA(cudaEventRecord(eb, st));
+        CM_TRY(sys_permute_out(S, S->m, m_user, 3, st));
+        if (terms & CM_TERM_DEMAG) CM_TRY(sys_permute_out(S, S->U, U_user, 1, st));
+        if (terms & CM_TERM_MAGEL) CM_TRY(sys_permute_out(S, S->u, u_user, 3, st));
+        HystCtl hr;
+        std::vector<double> lg((size_t)cap * 6);
+        CM_CUDA(cudaMemcpyAsync(&hr, ctl, sizeof(hr), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaMemcpyAsync(lg.data(), S->hyst_log, lg.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaMemcpyAsync(steps_log, S->hyst_steps, (size_t)cap * sizeof(int), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaStreamSynchronize(st));
+        float ms = 0;
+        CM_CUDA(cudaEventElapsedTime(&ms, ea, eb));
+        std::memcpy(H_log, lg.data(), (size_t)cap * 3 * sizeof(double));
+        std::memcpy(mbar_log, lg.data() + (size_t)cap * 3, (size_t)cap * 3 * sizeof(double));
+        res->n_fields = hr.k; res->reversed = hr.reversed; res->total_steps = hr.total;
+        res->cg_iters_ms = hr.it_ms; res->cg_iters_mech = hr.it_mech; res->cg_passes_gs = hr.gs_passes;
+        res->worst_cg_status = hr.worst; res->device_ms = ms;
+        return hr.worst;
+    };
+    if (rc == CM_OK) rc = run();
+    if (ea) cudaEventDestroy(ea);
+    if (eb) cudaEventDestroy(eb);
+    if (exec) cudaGraphExecDestroy(exec);
+    if (cs) cudaStreamDestroy(cs);
+    if (graph) cudaGraphDestroy(graph);
+    return rc;
+}
+
 #define INST(T)                                                                                                       \
     template int sys_permute_in<T>(System<T> *, const T *, T *, int, cudaStream_t);                                   \
     template int sys_permute_out<T>(System<T> *, const T *, T *, int, cudaStream_t);                                  \
@@ -830,9 +995,11 @@ int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_u
     template int sys_demag_field<T>(System<T> *, const T *, unsigned, T *, cudaStream_t);                             \
     template int sys_rhs_mech<T>(System<T> *, const T *, T *, cudaStream_t);                                          \
     template int sys_stress<T>(System<T> *, const T *, const T *, cudaStream_t);                                      \
-    template int sys_field<T>(System<T> *, const T *, const T *, const double *, unsigned, T *, T *, cudaStream_t);   \
+    template int sys_field<T>(System<T> *, const T *, const T *, const double *, unsigned, T *, T *, cudaStream_t, const double *); \
     template int sys_axpby3<T>(System<T> *, const T *, const T *, T, T *, cudaStream_t);                              \
-    template int sys_step<T>(System<T> *, const cm_step_params *, T *, T *, T *, cm_step_info *, cudaStream_t);
+    template int sys_step<T>(System<T> *, const cm_step_params *, T *, T *, T *, cm_step_info *, cudaStream_t);        \
+    template int sys_hysteresis<T>(System<T> *, const cm_step_params *, const cm_hyst_params *, T *, T *, T *, double *, double *, int *, \
+                                   cm_hyst_result *, cudaStream_t);
 INST(double)
 INST(float)
 

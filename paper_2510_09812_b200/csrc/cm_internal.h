@@ -167,6 +167,11 @@ struct System : SystemBase {
     T *hpart = nullptr;    // per-slot partial sums of the element passes, 6 per slot
     double *red = nullptr; // reduction partials
     double *dscal = nullptr, *h_scal = nullptr; // device / pinned scalars: mbar[3], gradU mean[3], dm sum, ...
+    // hysteresis driver (cm_hysteresis_run): device-resident controller state and logs, grown on demand
+    void *hyst_ctl = nullptr;
+    double *hyst_log = nullptr; // [cap][3] H, [cap][3] mbar
+    int *hyst_steps = nullptr;  // [cap]
+    int hyst_cap = 0;
     ~System();
 };
 
@@ -190,7 +195,9 @@ template <typename T> int sys_demag_field(System<T> *S, const T *U_lib, unsigned
 template <typename T> int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st);
 template <typename T> int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st);       // -> hpart (V sigma per slot)
 template <typename T> int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], unsigned terms, T *h,
-                                    T *sig_out, cudaStream_t st);                                          // gathers hpart when MAGEL
+                                    T *sig_out, cudaStream_t st, const double *hext_dev = nullptr);                                          // gathers hpart when MAGEL
 template <typename T> int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_user, cm_step_info *info,
                                    cudaStream_t st);
+template <typename T> int sys_hysteresis(System<T> *S, const cm_step_params *base, const cm_hyst_params *hp, T *m_user, T *U_user,
+                                         T *u_user, double *H_log, double *mbar_log, int *steps_log, cm_hyst_result *res, cudaStream_t st);
 template <typename T> int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t st);
