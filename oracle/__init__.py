@@ -42,7 +42,7 @@ class _Material(C.Structure):
     _fields_ = [("Ms", C.c_double), ("Aex", C.c_double), ("K1", C.c_double), ("lambda100", C.c_double),
                 ("lambda111", C.c_double), ("alpha", C.c_double), ("gamma", C.c_double),
                 ("length_scale", C.c_double), ("Nd", C.c_double * 9), ("n_elastic", C.c_int),
-                ("C_voigt", C.POINTER(C.c_double))]
+                ("C_voigt", C.POINTER(C.c_double)), ("R", C.c_double * 9)]
 
 
 class _StepParams(C.Structure):
@@ -77,7 +77,7 @@ def _lib(dtype: str):
         L.orc_nnz.restype = C.c_long
         for name in ("orc_scalar", "orc_nnz", "orc_get", "orc_get_values", "orc_spmv", "orc_cg", "orc_volume_average",
                      "orc_rhs_ms", "orc_demag_field", "orc_rhs_mech", "orc_stress_recover", "orc_field", "orc_energy",
-                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run"):
+                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run", "orc_voigt_rotation"):
             getattr(L, name).argtypes = None
         _libs[dtype] = L
     return _libs[dtype]
@@ -114,6 +114,15 @@ def periodic_wrap(xyz, axes: int, rel_tol: float = 1e-9):
     return dof, int(nd.value)
 
 
+def voigt_rotation(R):
+    """Eq. D.3: 6x6 M with sigma_sim = M sigma_crystal."""
+    L = _lib("f64")
+    R = np.ascontiguousarray(R, np.float64).reshape(9)
+    M = np.zeros(36)
+    L.orc_voigt_rotation(_p(R), _p(M))
+    return M.reshape(6, 6)
+
+
 class Oracle:
     """One mesh + material + dt, in the node order it is given (no reordering)."""
 
@@ -133,7 +142,8 @@ class Oracle:
         m = _Material(material.Ms, material.Aex, material.K1, material.lambda100, material.lambda111, material.alpha,
                       material.gamma, material.length_scale, (C.c_double * 9)(*material.Nd),
                       0 if self._Cv is None else self._Cv.shape[0],
-                      None if self._Cv is None else self._Cv.ctypes.data_as(C.POINTER(C.c_double)))
+                      None if self._Cv is None else self._Cv.ctypes.data_as(C.POINTER(C.c_double)),
+                      (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())))
         clamp = None if clamp_dof is None else np.ascontiguousarray(clamp_dof, np.uint8)
         h = C.c_void_p()
         rc = self.L.orc_create_wrapped(_p(xyz), C.c_long(self.Ng), _p(tets), C.c_long(self.Ne), _p(mag), _p(eid), _p(dof),

@@ -59,7 +59,8 @@ typedef struct {
     double Ms, Aex, K1, lambda100, lambda111, alpha, gamma, length_scale;
     double Nd[9];
     int n_elastic;
-    const double *C_voigt; /* n_elastic x 36, Pa */
+    const double *C_voigt; /* n_elastic x 36, Pa; in CRYSTAL axes */
+    double R[9];           /* App. D: crystal -> simulation frame, v_sim = R v_crystal (Eq. D.2), row-major; all zeros = identity */
 } orc_material;
 
 typedef struct {
@@ -100,6 +101,7 @@ typedef struct {
     double dt, Astar, Kstar, dtau, eps1, eps2, alpha, lam100, lam111, Ms, Nd[9];
     int n_elastic; double *Cstar; /* n_elastic x 36, C/(mu0 Ms^2) */
     double Vtot, Vmag;
+    double R[9]; int rot; /* App. D rotation (identity: rot = 0) */
 } oracle;
 
 static const double MU0 = 4.0e-7 * 3.14159265358979323846;
@@ -367,6 +369,7 @@ static long find_col(const oracle *o, long i, int j)
 }
 
 void orc_destroy(oracle *o);
+void orc_voigt_rotation(const double *R, double *M);
 
 /* Periodic boundary conditions: `dof` (NULL = identity) maps each of the Ng geometric nodes to one of N
  * unified degrees of freedom ("the two nodes in the pair are treated as one unified node").  Element geometry is
@@ -404,7 +407,28 @@ int orc_create_wrapped(const double *xyz_m, long Ng, const int *gtets, long Ne, 
     memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
     o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
     o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
-    for (int q = 0; q < o->n_elastic * 36; q++) o->Cstar[q] = mat->C_voigt[q] / mu0Ms2;
+    {   /* App. D: R (all zeros = identity) must be a proper rotation; C_sim = M C_crystal M^T (Eq. D.4, Alg. D.1 line 1) */
+        double nrm = 0; for (int q = 0; q < 9; q++) nrm += mat->R[q] * mat->R[q];
+        for (int q = 0; q < 9; q++) o->R[q] = nrm == 0 ? (q % 4 == 0 ? 1.0 : 0.0) : mat->R[q];
+        double dev = 0;
+        for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
+            double acc = 0; for (int k = 0; k < 3; k++) acc += o->R[3 * i + k] * o->R[3 * j + k];
+            dev = fmax(dev, fabs(acc - (i == j)));
+        }
+        const double *r = o->R;
+        double det = r[0] * (r[4] * r[8] - r[5] * r[7]) - r[1] * (r[3] * r[8] - r[5] * r[6]) + r[2] * (r[3] * r[7] - r[4] * r[6]);
+        if (dev > 1e-10 || det < 0) { free(tets); free(o->Cstar); free(o); return ORC_E_BADARG; }
+        o->rot = 0;
+        for (int q = 0; q < 9; q++) if (o->R[q] != (q % 4 == 0 ? 1.0 : 0.0)) o->rot = 1;
+    }
+    for (int k = 0; k < o->n_elastic; k++) {
+        const double *C = mat->C_voigt + 36 * k;
+        double M[36], MC[36];
+        if (!o->rot) { for (int q = 0; q < 36; q++) o->Cstar[36 * k + q] = C[q] / mu0Ms2; continue; }
+        orc_voigt_rotation(o->R, M);
+        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double acc = 0; for (int c = 0; c < 6; c++) acc += M[6 * a + c] * C[6 * c + b]; MC[6 * a + b] = acc; }
+        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double acc = 0; for (int c = 0; c < 6; c++) acc += MC[6 * a + c] * M[6 * b + c]; o->Cstar[36 * k + 6 * a + b] = acc / mu0Ms2; }
+    }
 
     o->x = (double *)malloc((size_t)Ng * 3 * sizeof(double));
     o->tet = tets;
@@ -769,7 +793,42 @@ int orc_demag_field(const oracle *o, const void *U_, const double *mbar, unsigne
 }
 
 /* E0(m), Table A.1, Voigt engineering vector (E11,E22,E33,2E23,2E13,2E12). */
-static void E0_voigt(const oracle *o, const real *m, real e0[6])
+/* ------------------------------------------------------------------------------------ */
+/* Appendix D: rotated coordinate system (R25)                       */
+/* ------------------------------------------------------------------------------------ */
+/* Eq. D.3: the 6x6 matrix M with sigma_sim = M sigma_crystal for Voigt vectors (xx,yy,zz,yz,xz,xy) of tensor
+ * components, so that C_sim = M C_crystal M^T (Eq. D.4) for a stiffness acting on engineering shears. */
+void orc_voigt_rotation(const double *R, double *M)
+{
+    static const int I[6] = {0, 1, 2, 1, 0, 0}, J[6] = {0, 1, 2, 2, 2, 1};
+    for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) {
+        int i = I[a], j = J[a], k = I[b], l = J[b];
+        /* (R S R^T)_ij = sum_kl R_ik R_jl S_kl; S symmetric: off-diagonal (k,l) appears twice */
+        M[6 * a + b] = (b < 3) ? R[3 * i + k] * R[3 * j + k] : R[3 * i + k] * R[3 * j + l] + R[3 * i + l] * R[3 * j + k];
+    }
+}
+
+/* v_c = R^T v (m_100 = R^-1 m_111, Alg. D.1 Step 1) and v = R v_c (h_111 = R h_100, Step 4) */
+static void to_crystal(const oracle *o, const real *v, real *vc)
+{
+    for (int a = 0; a < 3; a++) vc[a] = (real)o->R[a] * v[0] + (real)o->R[3 + a] * v[1] + (real)o->R[6 + a] * v[2];
+}
+static void to_sim(const oracle *o, const real *vc, real *v)
+{
+    for (int a = 0; a < 3; a++) v[a] = (real)o->R[3 * a] * vc[0] + (real)o->R[3 * a + 1] * vc[1] + (real)o->R[3 * a + 2] * vc[2];
+}
+/* symmetric tensor given as (xx,yy,zz,yz,xz,xy) tensor components: t_out = Q t Q^T with Q = R (inv = 0) or R^T (inv = 1) */
+static void rotate_sym(const oracle *o, const real t[6], int inv, real out[6])
+{
+    real A[3][3] = {{t[0], t[5], t[4]}, {t[5], t[1], t[3]}, {t[4], t[3], t[2]}}, B[3][3], Q[3][3];
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) Q[i][j] = (real)(inv ? o->R[3 * j + i] : o->R[3 * i + j]);
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) { real acc = 0; for (int k = 0; k < 3; k++) acc += Q[i][k] * A[k][j]; B[i][j] = acc; }
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) { real acc = 0; for (int k = 0; k < 3; k++) acc += B[i][k] * Q[j][k]; A[i][j] = acc; }
+    out[0] = A[0][0]; out[1] = A[1][1]; out[2] = A[2][2]; out[3] = A[1][2]; out[4] = A[0][2]; out[5] = A[0][1];
+}
+
+/* Table A.1 in crystal axes; engineering-shear Voigt vector */
+static void E0_crystal(const oracle *o, const real *m, real e0[6])
 {
     real l1 = (real)o->lam100, l2 = (real)o->lam111, th = (real)1.5;
     e0[0] = th * l1 * (m[0] * m[0] - (real)(1.0 / 3.0));
@@ -778,6 +837,18 @@ static void E0_voigt(const oracle *o, const real *m, real e0[6])
     e0[3] = (real)2 * th * l2 * m[1] * m[2];
     e0[4] = (real)2 * th * l2 * m[0] * m[2];
     e0[5] = (real)2 * th * l2 * m[0] * m[1];
+}
+
+/* E0 in the simulation frame: Alg. D.1 Step 1, E0_sim(m) = R E0_crystal(R^T m) R^T as a tensor (Eq. D.2) */
+static void E0_voigt(const oracle *o, const real *m, real e0[6])
+{
+    if (!o->rot) { E0_crystal(o, m, e0); return; }
+    real mc[3], ec[6], t[6];
+    to_crystal(o, m, mc);
+    E0_crystal(o, mc, ec);
+    for (int q = 3; q < 6; q++) ec[q] /= (real)2;   /* engineering -> tensor shears */
+    rotate_sym(o, ec, 0, t);
+    for (int q = 0; q < 3; q++) { e0[q] = t[q]; e0[3 + q] = (real)2 * t[3 + q]; }
 }
 
 /* mean over the 4 nodes of a magnetic tet of E0(m_k) (R13) */
@@ -871,22 +942,28 @@ int orc_field(const oracle *o, const void *w_, const void *hd_, const void *sig_
     for (long i = 0; i < o->N; i++) {
         real hi[3] = {0, 0, 0};
         if (o->live[i]) {
+            /* Alg. D.1 Step 4: the m-dependent terms are evaluated in crystal axes (m_c = R^T m, sigma_c = R^T sigma R) and
+             * rotated back, h = R h_c; the applied and demagnetising fields are already in the simulation frame */
+            real mcv[3], scv[6], hc[3] = {0, 0, 0};
             const real *m = w + 3 * i;
+            if (o->rot) { to_crystal(o, w + 3 * i, mcv); m = mcv; }
             if (terms & T_ANIS) {
                 real k2 = (real)(2.0 * o->Kstar);
-                hi[0] -= k2 * m[0] * (m[1] * m[1] + m[2] * m[2]);
-                hi[1] -= k2 * m[1] * (m[2] * m[2] + m[0] * m[0]);
-                hi[2] -= k2 * m[2] * (m[0] * m[0] + m[1] * m[1]);
+                hc[0] -= k2 * m[0] * (m[1] * m[1] + m[2] * m[2]);
+                hc[1] -= k2 * m[1] * (m[2] * m[2] + m[0] * m[0]);
+                hc[2] -= k2 * m[2] * (m[0] * m[0] + m[1] * m[1]);
             }
-            if (terms & T_ZEEMAN) for (int d = 0; d < 3; d++) hi[d] += (real)hext[d];
-            if (terms & (T_DEMAG | T_FARFIELD)) for (int d = 0; d < 3; d++) hi[d] += hd[3 * i + d];
             if (terms & T_MAGEL) {
                 const real *s = sg + 6 * i; /* xx,yy,zz,yz,xz,xy */
+                if (o->rot) { rotate_sym(o, s, 1, scv); s = scv; }
                 real l1 = (real)o->lam100, l2 = (real)o->lam111;
-                hi[0] += (real)3 * (l1 * m[0] * s[0] + l2 * (m[1] * s[5] + m[2] * s[4]));
-                hi[1] += (real)3 * (l1 * m[1] * s[1] + l2 * (m[0] * s[5] + m[2] * s[3]));
-                hi[2] += (real)3 * (l1 * m[2] * s[2] + l2 * (m[0] * s[4] + m[1] * s[3]));
+                hc[0] += (real)3 * (l1 * m[0] * s[0] + l2 * (m[1] * s[5] + m[2] * s[4]));
+                hc[1] += (real)3 * (l1 * m[1] * s[1] + l2 * (m[0] * s[5] + m[2] * s[3]));
+                hc[2] += (real)3 * (l1 * m[2] * s[2] + l2 * (m[0] * s[4] + m[1] * s[3]));
             }
+            if (o->rot) to_sim(o, hc, hi); else for (int d = 0; d < 3; d++) hi[d] = hc[d];
+            if (terms & T_ZEEMAN) for (int d = 0; d < 3; d++) hi[d] += (real)hext[d];
+            if (terms & (T_DEMAG | T_FARFIELD)) for (int d = 0; d < 3; d++) hi[d] += hd[3 * i + d];
         }
         h[3 * i] = hi[0]; h[3 * i + 1] = hi[1]; h[3 * i + 2] = hi[2];
     }
@@ -906,7 +983,10 @@ double orc_energy(const oracle *o, const void *m_, const void *U_, const void *u
     }
     for (long i = 0; i < N; i++) {
         double a = m[3 * i], b = m[3 * i + 1], c = m[3 * i + 2];
-        if (terms & T_ANIS) E += o->Kstar * (double)o->mLm[i] * (a * a * b * b + b * b * c * c + c * c * a * a);
+        real mcv[3] = {m[3 * i], m[3 * i + 1], m[3 * i + 2]};
+        if (o->rot) to_crystal(o, m + 3 * i, mcv);
+        double ac = mcv[0], bc = mcv[1], cc = mcv[2];
+        if (terms & T_ANIS) E += o->Kstar * (double)o->mLm[i] * (ac * ac * bc * bc + bc * bc * cc * cc + cc * cc * ac * ac);
         if (terms & T_ZEEMAN) E -= (double)o->mLm[i] * (hext[0] * a + hext[1] * b + hext[2] * c);
     }
     double mbar[3]; orc_volume_average(o, m, 3, mbar);

@@ -47,7 +47,8 @@ class Material:
     gamma: float = 2.211e5       # m/(A s)
     length_scale: float = 1.0e-9  # l_d, m
     Nd: Tuple[float, ...] = (1 / 3, 0, 0, 0, 1 / 3, 0, 0, 0, 1 / 3)   # sphere
-    C_voigt: np.ndarray = field(default_factory=lambda: isotropic_voigt(200e9, 0.3)[None])
+    C_voigt: np.ndarray = field(default_factory=lambda: isotropic_voigt(200e9, 0.3)[None])   # crystal axes
+    R: Optional[np.ndarray] = None   # App. D: crystal -> simulation frame (3x3, v_sim = R v_crystal); None = identity
 
 
 def isotropic_voigt(E: float, nu: float) -> np.ndarray:
@@ -59,6 +60,20 @@ def isotropic_voigt(E: float, nu: float) -> np.ndarray:
     C[np.arange(3), np.arange(3)] = lam + 2 * mu
     C[np.arange(3, 6), np.arange(3, 6)] = mu
     return C
+
+
+def cubic_voigt(C11: float, C12: float, C44: float) -> np.ndarray:
+    """6x6 stiffness of a cubic crystal in its own axes (Voigt xx,yy,zz,yz,xz,xy; engineering shears), Pa."""
+    C = np.zeros((6, 6))
+    C[:3, :3] = C12
+    C[np.arange(3), np.arange(3)] = C11
+    C[np.arange(3, 6), np.arange(3, 6)] = C44
+    return C
+
+
+R_111 = np.array([[1 / np.sqrt(3), 1 / np.sqrt(3), 1 / np.sqrt(3)],
+                  [-1 / np.sqrt(2), 1 / np.sqrt(2), 0.0],
+                  [-1 / np.sqrt(6), -1 / np.sqrt(6), 2 / np.sqrt(6)]])   # Eq. D.1 (P:466): axes <111>, <-110>, <-1-12>
 
 
 @dataclass
