@@ -89,7 +89,11 @@ typedef struct {
     double length_scale; /* l_d, metres */
     double Nd[9];        /* demagnetisation tensor of the ellipsoid, row-major (Eq. 4) */
     int n_elastic;       /* number of elastic materials; 0 = no mechanics */
-    const double *C_voigt; /* host, n_elastic x 36 row-major, Pa; Voigt order xx,yy,zz,yz,xz,xy, engineering shears */
+    const double *C_voigt; /* host, n_elastic x 36 row-major, Pa; Voigt order xx,yy,zz,yz,xz,xy, engineering shears; CRYSTAL axes */
+    double R[9];         /* Appendix D (R25): rotation crystal -> simulation frame, v_sim = R v_crystal
+                            (Eq. D.2), row-major; all zeros = identity.  The library forms C_sim = M C M^T (Eq. D.3-D.4) and
+                            evaluates E0(m), the anisotropy and the magnetoelastic field in crystal axes (Alg. D.1).
+                            Not a proper rotation: CM_E_BADARG. */
 } cm_material;
 
 typedef struct {

@@ -44,7 +44,7 @@ class CmError(RuntimeError):
 class cm_material(C.Structure):
     _fields_ = [("Ms", C.c_double), ("Aex", C.c_double), ("K1", C.c_double), ("lambda100", C.c_double),
                 ("lambda111", C.c_double), ("alpha", C.c_double), ("gamma", C.c_double), ("length_scale", C.c_double),
-                ("Nd", C.c_double * 9), ("n_elastic", C.c_int), ("C_voigt", C.POINTER(C.c_double))]
+                ("Nd", C.c_double * 9), ("n_elastic", C.c_int), ("C_voigt", C.POINTER(C.c_double)), ("R", C.c_double * 9)]
 
 
 class cm_step_params(C.Structure):
@@ -219,7 +219,8 @@ class System:
         self._Cv = Cv
         m = cm_material(material.Ms, material.Aex, material.K1, material.lambda100, material.lambda111, material.alpha,
                         material.gamma, material.length_scale, (C.c_double * 9)(*material.Nd),
-                        0 if Cv is None else Cv.shape[0], None if Cv is None else Cv.ctypes.data_as(C.POINTER(C.c_double)))
+                        0 if Cv is None else Cv.shape[0], None if Cv is None else Cv.ctypes.data_as(C.POINTER(C.c_double)),
+                        (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())))
         clamp = _np(clamp_dof, np.uint8)
         self.h = C.c_void_p()
         _check(L.cm_assemble_csr(mesh.h, C.byref(m), self.cm_dtype, dt, _hp(clamp), pin_node, _stream(), C.byref(self.h)))

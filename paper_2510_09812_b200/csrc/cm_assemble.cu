@@ -227,6 +227,20 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     S->eps2 = S->alpha * S->Astar * S->dtau;
     S->lam100 = mat->lambda100; S->lam111 = mat->lambda111;
     std::memcpy(S->Nd, mat->Nd, sizeof(S->Nd));
+    {   // App. D: all zeros = identity; otherwise R R^T = I and det R = +1 are required
+        bool zero = true, ident = true;
+        for (int q = 0; q < 9; q++) zero = zero && mat->R[q] == 0.0;
+        for (int q = 0; q < 9; q++) S->R[q] = zero ? (q % 4 == 0 ? 1.0 : 0.0) : mat->R[q];
+        const double *r = S->R;
+        double worst = 0;
+        for (int a = 0; a < 3; a++)
+            for (int b = 0; b < 3; b++)
+                worst = std::max(worst, std::fabs(r[3 * a] * r[3 * b] + r[3 * a + 1] * r[3 * b + 1] + r[3 * a + 2] * r[3 * b + 2] - (a == b ? 1.0 : 0.0)));
+        const double det = r[0] * (r[4] * r[8] - r[5] * r[7]) - r[1] * (r[3] * r[8] - r[5] * r[6]) + r[2] * (r[3] * r[7] - r[4] * r[6]);
+        if (!(worst <= 1e-10) || !(det > 0)) { cm_set_error("cm_assemble_csr: material R is not a proper rotation (|R R^T - I| = %.2e, det = %.3f)", worst, det); return CM_E_BADARG; }
+        for (int q = 0; q < 9; q++) ident = ident && S->R[q] == (q % 4 == 0 ? 1.0 : 0.0);
+        S->rot = !ident;
+    }
     S->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
     S->pin = M->iperm[pin_user];
     int dev = 0;
@@ -249,7 +263,40 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     if (S->n_elastic) {
         std::vector<double> Cs(36 * S->n_elastic);
         std::vector<T> Ct(36 * S->n_elastic);
-        for (size_t q = 0; q < Cs.size(); q++) { Cs[q] = mat->C_voigt[q] / mu0Ms2; Ct[q] = (T)Cs[q]; }
+        // Eq. D.3-D.4: stiffness in the simulation frame, C_sim = M C_crystal M^T, where row (ij), column (kl)
+        // of M holds the coefficient of sigma_kl in (R sigma R^T)_ij
+        double Mv[6][6];
+        {
+            const int vi[6] = {0, 1, 2, 1, 0, 0}, vj[6] = {0, 1, 2, 2, 2, 1};
+            auto Rm = [&](int a, int b) { return S->R[3 * a + b]; };
+            for (int p = 0; p < 6; p++)
+                for (int q = 0; q < 6; q++) {
+                    const int i = vi[p], j = vj[p], k = vi[q], l = vj[q];
+                    Mv[p][q] = k == l ? Rm(i, k) * Rm(j, k) : Rm(i, k) * Rm(j, l) + Rm(i, l) * Rm(j, k);
+                }
+        }
+        for (int e = 0; e < S->n_elastic; e++) {
+            const double *C = mat->C_voigt + 36 * e;
+            double *out = Cs.data() + 36 * e;
+            if (!S->rot) {
+                for (int q = 0; q < 36; q++) out[q] = C[q] / mu0Ms2;
+                continue;
+            }
+            double MC[6][6];
+            for (int p = 0; p < 6; p++)
+                for (int q = 0; q < 6; q++) {
+                    double acc = 0;
+                    for (int w = 0; w < 6; w++) acc += Mv[p][w] * C[6 * w + q];
+                    MC[p][q] = acc;
+                }
+            for (int p = 0; p < 6; p++)
+                for (int q = 0; q < 6; q++) {
+                    double acc = 0;
+                    for (int w = 0; w < 6; w++) acc += MC[p][w] * Mv[q][w];
+                    out[6 * p + q] = acc / mu0Ms2;
+                }
+        }
+        for (size_t q = 0; q < Cs.size(); q++) Ct[q] = (T)Cs[q];
         CM_CUDA(cudaMalloc((void **)&Cd, Cs.size() * sizeof(double)));
         CM_CUDA(cudaMemcpyAsync(Cd, Cs.data(), Cs.size() * sizeof(double), cudaMemcpyHostToDevice, st));
         CM_TRY(alloc(&S->Cstar, Ct.size()));

@@ -130,6 +130,7 @@ struct ChunkArgs {
     const double *mbar;   // MS
     const T *Cstar;       // MECH, STRESS: 36 words per material, or the 12 of the cubic pattern
     T l1, l2;
+    Rot<T> rot;           // App. D: crystal -> simulation frame
     T *hpart;             // [slot][NC]
     double *partial;      // GRADU: per-chunk sums of V_e grad U_e (fp64)
 };
@@ -189,9 +190,63 @@ __device__ __forceinline__ void E0_voigt(const T *m, T l1, T l2, T e0[6])
     e0[5] = (T)2 * th * l2 * m[0] * m[1];
 }
 
+// ---- App. D helpers: v_c = R^T v, v = R v_c, and Q t Q^T for a symmetric tensor given by its 6 tensor components
+template <typename T>
+__device__ __forceinline__ void rot_to_crystal(const Rot<T> &R, const T v[3], T vc[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; a++) vc[a] = R.r[a] * v[0] + R.r[3 + a] * v[1] + R.r[6 + a] * v[2];
+}
+template <typename T>
+__device__ __forceinline__ void rot_to_sim(const Rot<T> &R, const T vc[3], T v[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; a++) v[a] = R.r[3 * a] * vc[0] + R.r[3 * a + 1] * vc[1] + R.r[3 * a + 2] * vc[2];
+}
+template <typename T, bool INV>
+__device__ __forceinline__ void rot_sym(const Rot<T> &R, const T t[6], T out[6])
+{
+    const T A[3][3] = {{t[0], t[5], t[4]}, {t[5], t[1], t[3]}, {t[4], t[3], t[2]}};
+    T B[3][3], Cm[3][3];
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            T acc = 0;
+#pragma unroll
+            for (int k = 0; k < 3; k++) acc += (INV ? R.r[3 * k + i] : R.r[3 * i + k]) * A[k][j];
+            B[i][j] = acc;
+        }
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            T acc = 0;
+#pragma unroll
+            for (int k = 0; k < 3; k++) acc += B[i][k] * (INV ? R.r[3 * k + j] : R.r[3 * j + k]);
+            Cm[i][j] = acc;
+        }
+    out[0] = Cm[0][0]; out[1] = Cm[1][1]; out[2] = Cm[2][2]; out[3] = Cm[1][2]; out[4] = Cm[0][2]; out[5] = Cm[0][1];
+}
+
+// E0 in the simulation frame (Alg. D.1 Step 1): R E0_crystal(R^T m) R^T, engineering-shear Voigt vector
+template <typename T>
+__device__ __forceinline__ void E0_sim(const Rot<T> &R, const T *m, T l1, T l2, T e0[6])
+{
+    if (!R.on) { E0_voigt(m, l1, l2, e0); return; }
+    T mc[3], ec[6], t[6];
+    rot_to_crystal(R, m, mc);
+    E0_voigt(mc, l1, l2, ec);
+#pragma unroll
+    for (int q = 3; q < 6; q++) ec[q] /= (T)2;
+    rot_sym<T, false>(R, ec, t);
+#pragma unroll
+    for (int q = 0; q < 3; q++) { e0[q] = t[q]; e0[3 + q] = (T)2 * t[3 + q]; }
+}
+
 // mean over the 4 corners of E0(w); w_k = sw[ST * l[k] + OFF ..]
 template <typename T, int ST, int OFF>
-__device__ __forceinline__ void mean_E0(const T *sw, const int *l, T l1, T l2, T e0[6])
+__device__ __forceinline__ void mean_E0(const Rot<T> &R, const T *sw, const int *l, T l1, T l2, T e0[6])
 {
 #pragma unroll
     for (int q = 0; q < 6; q++) e0[q] = 0;
@@ -199,7 +254,7 @@ __device__ __forceinline__ void mean_E0(const T *sw, const int *l, T l1, T l2, T
     for (int k = 0; k < 4; k++) {
         const T *w = sw + ST * l[k] + OFF;
         T mk[3] = {w[0], w[1], w[2]}, ek[6];
-        E0_voigt(mk, l1, l2, ek);
+        E0_sim(R, mk, l1, l2, ek);
 #pragma unroll
         for (int q = 0; q < 6; q++) e0[q] += ek[q];
     }
@@ -324,7 +379,7 @@ __global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs
             } else if (KIND == EK_MECH) {
                 // S = C*_e : mean_e E0(m);  c_(k,a) = V_e (S grad phi_k)_a
                 T e0v[6], sg[6];
-                mean_E0<T, 3, 0>(sin, l, a.l1, a.l2, e0v);
+                mean_E0<T, 3, 0>(a.rot, sin, l, a.l1, a.l2, e0v);
                 if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), e0v, sg);
                 else C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
 #pragma unroll
@@ -346,7 +401,7 @@ __global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs
                         H[x][y] = acc;
                     }
                 T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]}, e0v[6], sg[6];
-                mean_E0<T, 6, 3>(sin, l, a.l1, a.l2, e0v);
+                mean_E0<T, 6, 3>(a.rot, sin, l, a.l1, a.l2, e0v);
 #pragma unroll
                 for (int q = 0; q < 6; q++) eps[q] -= e0v[q];
                 if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), eps, sg);
@@ -434,21 +489,22 @@ template <typename T>
 __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                   const T *__restrict__ mLm, const uchar *__restrict__ live, const T *__restrict__ w,
                                   const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, const double *__restrict__ hext_dev,
-                                  T l1, T l2, T *h, T *sig_out)
+                                  T l1, T l2, Rot<T> rot, T *h, T *sig_out)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
     if (hext_dev) { hx = (T)hext_dev[0]; hy = (T)hext_dev[1]; hz = (T)hext_dev[2]; } // device-resident field (hysteresis driver)
     T hi[3] = {0, 0, 0}, s[6] = {0, 0, 0, 0, 0, 0};
     if (live[i]) {
-        const T m[3] = {w[3 * i], w[3 * i + 1], w[3 * i + 2]};
+        // Alg. D.1 Step 4: m-dependent terms in crystal axes (m_c = R^T m, sigma_c = R^T sigma R), then h = R h_c
+        const T ms_[3] = {w[3 * i], w[3 * i + 1], w[3 * i + 2]};
+        T m[3] = {ms_[0], ms_[1], ms_[2]}, hc[3] = {0, 0, 0};
+        if (rot.on) rot_to_crystal(rot, ms_, m);
         if (terms & CM_TERM_ANIS) {
-            hi[0] -= Kstar2 * m[0] * (m[1] * m[1] + m[2] * m[2]);
-            hi[1] -= Kstar2 * m[1] * (m[2] * m[2] + m[0] * m[0]);
-            hi[2] -= Kstar2 * m[2] * (m[0] * m[0] + m[1] * m[1]);
+            hc[0] -= Kstar2 * m[0] * (m[1] * m[1] + m[2] * m[2]);
+            hc[1] -= Kstar2 * m[1] * (m[2] * m[2] + m[0] * m[0]);
+            hc[2] -= Kstar2 * m[2] * (m[0] * m[0] + m[1] * m[1]);
         }
-        if (terms & CM_TERM_ZEEMAN) { hi[0] += hx; hi[1] += hy; hi[2] += hz; }
-        if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) { hi[0] += hd[3 * i]; hi[1] += hd[3 * i + 1]; hi[2] += hd[3 * i + 2]; }
         if (terms & CM_TERM_MAGEL) {
             for (int q = ns_ptr[i]; q < ns_ptr[i + 1]; q++) {
                 const long sl = __ldg(ns_slot + q);
@@ -458,10 +514,16 @@ __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const 
             const T den = (T)4 * mLm[i];
 #pragma unroll
             for (int c = 0; c < 6; c++) s[c] /= den;
-            hi[0] += (T)3 * (l1 * m[0] * s[0] + l2 * (m[1] * s[5] + m[2] * s[4]));
-            hi[1] += (T)3 * (l1 * m[1] * s[1] + l2 * (m[0] * s[5] + m[2] * s[3]));
-            hi[2] += (T)3 * (l1 * m[2] * s[2] + l2 * (m[0] * s[4] + m[1] * s[3]));
+            T sc[6] = {s[0], s[1], s[2], s[3], s[4], s[5]};
+            if (rot.on) rot_sym<T, true>(rot, s, sc);
+            hc[0] += (T)3 * (l1 * m[0] * sc[0] + l2 * (m[1] * sc[5] + m[2] * sc[4]));
+            hc[1] += (T)3 * (l1 * m[1] * sc[1] + l2 * (m[0] * sc[5] + m[2] * sc[3]));
+            hc[2] += (T)3 * (l1 * m[2] * sc[2] + l2 * (m[0] * sc[4] + m[1] * sc[3]));
         }
+        if (rot.on) rot_to_sim(rot, hc, hi);
+        else { hi[0] = hc[0]; hi[1] = hc[1]; hi[2] = hc[2]; }
+        if (terms & CM_TERM_ZEEMAN) { hi[0] += hx; hi[1] += hy; hi[2] += hz; }
+        if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) { hi[0] += hd[3 * i]; hi[1] += hd[3 * i + 1]; hi[2] += hd[3 * i + 2]; }
     }
     if (h) { h[3 * i] = hi[0]; h[3 * i + 1] = hi[1]; h[3 * i + 2] = hi[2]; }
     if (sig_out)
@@ -595,6 +657,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
     a.emat = M->d_emat; a.EG = S->EG;
     a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
+    a.rot = make_rot<T>(S);
     a.hpart = S->hpart; a.partial = S->red;
     return a;
 }
@@ -686,7 +749,7 @@ int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], u
     S->prof.begin(CM_PROF_ELEMENT, st);
     node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mLm, S->live, w_lib, hd, terms,
                                                    (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], hext_dev, (T)S->lam100,
-                                                   (T)S->lam111, h, sig_out);
+                                                   (T)S->lam111, make_rot<T>(S), h, sig_out);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;

@@ -102,6 +102,16 @@ struct cm_mesh {
     double *h_red = nullptr;   // pinned, 16 doubles
 };
 
+// App. D rotation as a kernel argument (by value); on == 0: identity, nothing is rotated
+template <typename T>
+struct Rot {
+    T r[9];
+    int on;
+};
+struct SystemBase;
+template <typename T>
+inline Rot<T> make_rot(const SystemBase *S);
+
 struct CgResult {
     int iters[3];
     double relres[3];
@@ -131,6 +141,8 @@ struct SystemBase {
     long N = 0, Ne = 0, nnz = 0;
     double dt = 0, Astar = 0, Kstar = 0, dtau = 0, eps1 = 0, eps2 = 0, alpha = 0, lam100 = 0, lam111 = 0, Ms = 0;
     double Nd[9] = {0};
+    double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}; // App. D: crystal -> simulation frame
+    bool rot = false;
     int n_elastic = 0;
     double Vtot = 0, Vmag = 0;
     long nlive = 0;
@@ -139,6 +151,15 @@ struct SystemBase {
     Profiler prof;
     virtual ~SystemBase() {}
 };
+
+template <typename T>
+inline Rot<T> make_rot(const SystemBase *S)
+{
+    Rot<T> q;
+    for (int k = 0; k < 9; k++) q.r[k] = (T)S->R[k];
+    q.on = S->rot ? 1 : 0;
+    return q;
+}
 
 template <typename T>
 struct System : SystemBase {
