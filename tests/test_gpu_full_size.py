@@ -170,3 +170,33 @@ def test_config1_full_size_10_steps(oracle_mod, dtype):
             assert abs(io.it_gs[a] - ig.it_gs[a]) <= (1 if f64 else 3), (k, a, list(io.it_gs), list(ig.it_gs))
     err = np.abs(mg.cpu().numpy().astype(np.float64) - m).max()
     assert err <= (1e-9 if f64 else 1e-4), err
+
+
+def test_full_size_fp32_build_against_fp64_oracle(full, oracle_mod):
+    """The fp32 library build at config 3's size (what `bench.py --dtype f32` times) against the fp64 oracle already set up:
+    SpMV, right-hand sides and fields <= 1e-5 over all 3 M outputs; three CG iterations <= 1e-4."""
+    cfg, cm, gm, gs64, o, torch = full
+    gs = cm.System(gm, cfg.material, cfg.dt, "f32", cfg.clamp_dof, cfg.pin_node)
+    dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float32, device="cuda")
+    rng = np.random.default_rng(43)
+    N = o.N
+    x = rng.normal(size=N).astype(np.float32)
+    assert rel(gs.spmv(cm.CM_MAT_K_MS, dev(x)).cpu().numpy(), o.spmv(oracle_mod.MAT_K_MS, x.astype(np.float64))) < 1e-5
+    x3 = rng.normal(size=(N, 3)).astype(np.float32)
+    y3 = gs.spmv(cm.CM_MAT_K_MECH, dev(x3)).cpu().numpy()
+    assert rel(y3.ravel(), o.spmv(oracle_mod.MAT_K_MECH, x3.astype(np.float64).ravel())) < 1e-5
+    m = cfg.m0.astype(np.float32); m64 = m.astype(np.float64)
+    md = dev(m)
+    assert rel(gs.field_rhs(cm.CM_RHS_MS, md).cpu().numpy(), o.rhs_ms(m64)) < 1e-5
+    assert rel(gs.field_rhs(cm.CM_RHS_MECH, md).cpu().numpy(), o.rhs_mech(m64)) < 1e-5
+    U = rng.normal(size=N).astype(np.float32); u = (1e-3 * rng.normal(size=(N, 3))).astype(np.float32)
+    p = cm.make_params(cfg.dt, cfg.Hext[3], cfg.terms)
+    hd_o, _ = o.demag_field(U.astype(np.float64), o.volume_average(m64), cfg.terms)
+    sig_o = o.stress_recover(u.astype(np.float64), m64)
+    h_o = o.field(m64, hd_o, sig_o, np.asarray(cfg.Hext[3]) / cfg.material.Ms, cfg.terms)
+    assert rel(gs.field_rhs(cm.CM_OUT_FIELD, md, dev(U), dev(u), p).cpu().numpy(), h_o) < 1e-5
+    b3 = rng.normal(size=(N, 3)).astype(np.float32); b3[cfg.clamp_dof.reshape(N, 3).astype(bool)] = 0
+    xg = torch.zeros((N, 3), dtype=torch.float32, device="cuda")
+    it, res, rc = gs.cg_solve(cm.CM_MAT_K_MECH, dev(b3), xg, fixed_iters=3)
+    xo, ito, reso, _ = o.cg(oracle_mod.MAT_K_MECH, b3.astype(np.float64).ravel(), fixed=3)
+    assert it == 3 and rel(xg.cpu().numpy().ravel(), xo) < 1e-4 and res == pytest.approx(reso, rel=1e-3)
