@@ -44,7 +44,7 @@ template <int MODE> struct ModeTraits;
 #define CM_U_CSR1 8
 #endif
 #ifndef CM_U_CSR3
-#define CM_U_CSR3 4
+#define CM_U_CSR3 8
 #endif
 #ifndef CM_U_BSR3
 #define CM_U_BSR3 2
