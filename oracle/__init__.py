@@ -77,7 +77,7 @@ def _lib(dtype: str):
         L.orc_nnz.restype = C.c_long
         for name in ("orc_scalar", "orc_nnz", "orc_get", "orc_get_values", "orc_spmv", "orc_cg", "orc_volume_average",
                      "orc_rhs_ms", "orc_demag_field", "orc_rhs_mech", "orc_stress_recover", "orc_field", "orc_energy",
-                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run", "orc_voigt_rotation"):
+                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run", "orc_voigt_rotation", "orc_create_hex"):
             getattr(L, name).argtypes = None
         _libs[dtype] = L
     return _libs[dtype]
@@ -127,6 +127,7 @@ class Oracle:
     """One mesh + material + dt, in the node order it is given (no reordering)."""
 
     def __init__(self, mesh, material, dt, clamp_dof=None, pin_node=0, dtype="f64", dof_of_node=None, n_dof=None):
+        """mesh: inputs.Mesh (tetrahedra) or inputs.HexMesh (linear hexahedra: matrices, lumped masses and volume averages only)."""
         self.dtype = dtype
         self.real = np.float64 if dtype == "f64" else np.float32
         self.L = _lib(dtype)
@@ -135,7 +136,7 @@ class Oracle:
         self.N = self.Ng if dof_of_node is None else int(n_dof)       # degrees of freedom
         dof = None if dof_of_node is None else np.ascontiguousarray(dof_of_node, np.int32)
         xyz = np.ascontiguousarray(mesh.xyz, np.float64)
-        tets = np.ascontiguousarray(mesh.tets, np.int32)
+        tets = None if hasattr(mesh, "hexes") else np.ascontiguousarray(mesh.tets, np.int32)
         mag = np.ascontiguousarray(mesh.magnetic, np.uint8)
         eid = np.ascontiguousarray(mesh.elastic_id, np.int32)
         self._Cv = np.ascontiguousarray(material.C_voigt, np.float64).reshape(-1, 36) if material.C_voigt is not None else None
@@ -146,8 +147,15 @@ class Oracle:
                       (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())))
         clamp = None if clamp_dof is None else np.ascontiguousarray(clamp_dof, np.uint8)
         h = C.c_void_p()
-        rc = self.L.orc_create_wrapped(_p(xyz), C.c_long(self.Ng), _p(tets), C.c_long(self.Ne), _p(mag), _p(eid), _p(dof),
-                                       C.c_long(self.N), C.byref(m), C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
+        self.is_hex = hasattr(mesh, "hexes")
+        if self.is_hex:
+            assert dof is None
+            hexes = np.ascontiguousarray(mesh.hexes, np.int32)
+            rc = self.L.orc_create_hex(_p(xyz), C.c_long(self.Ng), _p(hexes), C.c_long(self.Ne), _p(mag), _p(eid), C.byref(m),
+                                       C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
+        else:
+            rc = self.L.orc_create_wrapped(_p(xyz), C.c_long(self.Ng), _p(tets), C.c_long(self.Ne), _p(mag), _p(eid), _p(dof),
+                                           C.c_long(self.N), C.byref(m), C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
         if rc:
             raise RuntimeError(f"orc_create rc={rc}")
         self.h = h
@@ -183,7 +191,7 @@ class Oracle:
     def rowptr(self): return self._get(0, self.N + 1, np.int32)
     def colidx(self): return self._get(1, self.nnz, np.int32)
     def n2e_ptr(self): return self._get(2, self.N + 1, np.int32)
-    def n2e(self): return self._get(3, self.Ne * 4, np.int32)
+    def n2e(self): return self._get(3, self.Ne * (8 if self.is_hex else 4), np.int32)
     def V(self): return self._get(4, self.Ne, self.real)
     def G(self): return self._get(5, (self.Ne, 4, 3), self.real)
     def mL(self): return self._get(6, self.N, self.real)

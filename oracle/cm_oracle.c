@@ -102,6 +102,7 @@ typedef struct {
     int n_elastic; double *Cstar; /* n_elastic x 36, C/(mu0 Ms^2) */
     double Vtot, Vmag;
     double R[9]; int rot; /* App. D rotation (identity: rot = 0) */
+    int nen; int *hex;    /* nen = 8: linear hexahedra (matrices and averages only); hex = Ne x 8 connectivity; 0 / 4: tetrahedra */
 } oracle;
 
 static const double MU0 = 4.0e-7 * 3.14159265358979323846;
@@ -164,6 +165,52 @@ static int build_pattern(long N, const int *tet, const int *ptr, const int *lst,
     }
     free(tmp);
     *rowptr_out = rowptr; *nnz_out = rowptr[N];
+    return ORC_OK;
+}
+
+/* the same two builders for elements with nen nodes (list entries nen * e + k) */
+static int build_n2e_n(long N, long Ne, const int *conn, int nen, int **ptr_out, int **lst_out)
+{
+    int *ptr = (int *)calloc((size_t)N + 1, sizeof(int));
+    int *lst = (int *)malloc((size_t)Ne * nen * sizeof(int));
+    int *fill = (int *)malloc((size_t)N * sizeof(int));
+    if (!ptr || !lst || !fill) return ORC_E_ALLOC;
+    for (long q = 0; q < nen * Ne; q++) ptr[conn[q] + 1]++;
+    for (long i = 0; i < N; i++) ptr[i + 1] += ptr[i];
+    memcpy(fill, ptr, (size_t)N * sizeof(int));
+    for (long q = 0; q < nen * Ne; q++) lst[fill[conn[q]]++] = (int)q;
+    free(fill);
+    *ptr_out = ptr; *lst_out = lst;
+    return ORC_OK;
+}
+
+static int build_pattern_n(long N, const int *conn, int nen, const int *ptr, const int *lst, int **rowptr_out, int **col_out, long *nnz_out)
+{
+    int *rowptr = (int *)calloc((size_t)N + 1, sizeof(int));
+    if (!rowptr) return ORC_E_ALLOC;
+    int *col = NULL;
+    for (int pass = 0; pass < 2; pass++) {
+        for (long i = 0; i < N; i++) {
+            int cnt = ptr[i + 1] - ptr[i], m = 0;
+            int *tmp = (int *)malloc(((size_t)nen * cnt + 1) * sizeof(int));
+            tmp[m++] = (int)i;
+            for (int s = ptr[i]; s < ptr[i + 1]; s++) {
+                long e = lst[s] / nen;
+                for (int k = 0; k < nen; k++) tmp[m++] = conn[nen * e + k];
+            }
+            qsort(tmp, m, sizeof(int), cmp_int);
+            int u = 0;
+            for (int q = 0; q < m; q++) if (q == 0 || tmp[q] != tmp[q - 1]) tmp[u++] = tmp[q];
+            if (!pass) rowptr[i + 1] = u; else memcpy(col + rowptr[i], tmp, u * sizeof(int));
+            free(tmp);
+        }
+        if (!pass) {
+            for (long i = 0; i < N; i++) rowptr[i + 1] += rowptr[i];
+            col = (int *)malloc((size_t)rowptr[N] * sizeof(int));
+            if (!col) return ORC_E_ALLOC;
+        }
+    }
+    *rowptr_out = rowptr; *col_out = col; *nnz_out = rowptr[N];
     return ORC_OK;
 }
 
@@ -569,9 +616,176 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     return orc_create_wrapped(xyz_m, N, tets, Ne, magnetic, elastic_id, NULL, N, mat, dt, clamp_dof, pin_node, out);
 }
 
+/* round the fp64 sums once (R20) and apply the constraints as P A P + (I - P) (R11, R12) -- as in orc_create */
+static int finish_matrices(oracle *o, const double *K, const double *Km, const double *Mm, const double *Kme)
+{
+    long N = o->N, nnz = o->nnz;
+    o->K = (real *)malloc((size_t)nnz * sizeof(real)); o->Kms = (real *)malloc((size_t)nnz * sizeof(real));
+    o->Km = (real *)malloc((size_t)nnz * sizeof(real)); o->Mm = (real *)malloc((size_t)nnz * sizeof(real));
+    o->Kgs1 = (real *)malloc((size_t)nnz * sizeof(real)); o->Kgs2 = (real *)malloc((size_t)nnz * sizeof(real));
+    if (Kme) { o->Kmech = (real *)malloc((size_t)nnz * 9 * sizeof(real)); o->Kmech_free = (real *)malloc((size_t)nnz * 9 * sizeof(real)); }
+    if (!o->K || !o->Kms || !o->Km || !o->Mm || !o->Kgs1 || !o->Kgs2 || (Kme && (!o->Kmech || !o->Kmech_free))) return ORC_E_ALLOC;
+    for (long i = 0; i < N; i++)
+        for (long q = o->rowptr[i]; q < o->rowptr[i + 1]; q++) {
+            long j = o->col[q];
+            o->K[q] = (real)K[q]; o->Km[q] = (real)Km[q]; o->Mm[q] = (real)Mm[q];
+            double kms = K[q];
+            if (i == o->pin || j == o->pin) kms = (i == j) ? 1.0 : 0.0;
+            o->Kms[q] = (real)kms;
+            double dead = (i == j && !o->live[i]) ? 1.0 : 0.0;
+            o->Kgs1[q] = (real)(Mm[q] + o->eps1 * Km[q] + dead);
+            o->Kgs2[q] = (real)(Mm[q] + o->eps2 * Km[q] + dead);
+            if (Kme) for (int r = 0; r < 3; r++) for (int s = 0; s < 3; s++) {
+                double v = Kme[9 * q + 3 * r + s];
+                o->Kmech_free[9 * q + 3 * r + s] = (real)v;
+                if (o->clamp[3 * i + r] || o->clamp[3 * j + s]) v = (i == j && r == s) ? 1.0 : 0.0;
+                o->Kmech[9 * q + 3 * r + s] = (real)v;
+            }
+        }
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* Linear hexahedral (Q1) elements (R26) */
+/* ------------------------------------------------------------------------------------ */
+/* "Currently, only linear hexahedral and tetrahedral Lagrange elements are supported"; the paper's Fig. 2-3
+ * workloads are structured hexahedral meshes.  Trilinear shape functions on the reference cube
+ * [-1,1]^3, local node a = i + 2 j + 4 k <-> (xi, eta, zeta) = (2i-1, 2j-1, 2k-1):
+ *   phi_a = (1 + xi_a xi)(1 + eta_a eta)(1 + zeta_a zeta) / 8,
+ * integrated with the 2 x 2 x 2 Gauss rule (points +-1/sqrt 3, unit weights; Eq. 17's |J(e,p)| w_p):
+ *   K_ab = sum_p |J_p| grad phi_a . grad phi_b,  M_ab = sum_p |J_p| phi_a phi_b,  K^mech_ab = sum_p |J_p| B_a^T C B_b,
+ *   grad phi_a = J^-T grad_xi phi_a,  J = sum_a x_a (x) grad_xi phi_a.
+ * This build covers the MATRICES of Eq. 12 (all of K^ms, K^GS, M, K^mech with their constraints), the lumped masses
+ * int phi_a and the volume average of Eq. 17 -- the systems of the paper's CG benchmark (Fig. 2b-d); the element-wise
+ * right-hand sides of the GSPM step stay tetrahedral. */
+static void hex_gauss_point(const double *X /* 8 x 3 */, int p, double *detJ, double phi[8], double g[8][3])
+{
+    const double q = 0.57735026918962576451; /* 1/sqrt(3) */
+    double xi[3] = {(p & 1) ? q : -q, (p & 2) ? q : -q, (p & 4) ? q : -q};
+    double dN[8][3], J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    for (int a = 0; a < 8; a++) {
+        double s[3] = {(a & 1) ? 1.0 : -1.0, (a & 2) ? 1.0 : -1.0, (a & 4) ? 1.0 : -1.0};
+        double f[3] = {1 + s[0] * xi[0], 1 + s[1] * xi[1], 1 + s[2] * xi[2]};
+        phi[a] = f[0] * f[1] * f[2] / 8;
+        dN[a][0] = s[0] * f[1] * f[2] / 8; dN[a][1] = f[0] * s[1] * f[2] / 8; dN[a][2] = f[0] * f[1] * s[2] / 8;
+        for (int r = 0; r < 3; r++) for (int c = 0; c < 3; c++) J[r][c] += X[3 * a + r] * dN[a][c]; /* J_rc = d x_r / d xi_c */
+    }
+    double cof[3][3];
+    cof[0][0] = J[1][1] * J[2][2] - J[1][2] * J[2][1]; cof[0][1] = J[1][2] * J[2][0] - J[1][0] * J[2][2]; cof[0][2] = J[1][0] * J[2][1] - J[1][1] * J[2][0];
+    cof[1][0] = J[0][2] * J[2][1] - J[0][1] * J[2][2]; cof[1][1] = J[0][0] * J[2][2] - J[0][2] * J[2][0]; cof[1][2] = J[0][1] * J[2][0] - J[0][0] * J[2][1];
+    cof[2][0] = J[0][1] * J[1][2] - J[0][2] * J[1][1]; cof[2][1] = J[0][2] * J[1][0] - J[0][0] * J[1][2]; cof[2][2] = J[0][0] * J[1][1] - J[0][1] * J[1][0];
+    double det = J[0][0] * cof[0][0] + J[0][1] * cof[0][1] + J[0][2] * cof[0][2];
+    *detJ = det;
+    /* grad phi_a = J^-T grad_xi phi_a;  (J^-1)_cr = cof_rc / det  =>  (grad phi_a)_r = sum_c cof_rc dN_ac / det */
+    for (int a = 0; a < 8; a++)
+        for (int r = 0; r < 3; r++) g[a][r] = (cof[r][0] * dN[a][0] + cof[r][1] * dN[a][1] + cof[r][2] * dN[a][2]) / det;
+}
+
+int orc_create_hex(const double *xyz_m, long N, const int *hexes, long Ne, const uchar *magnetic, const int *elastic_id,
+                   const orc_material *mat, double dt, const uchar *clamp_dof, long pin_node, oracle **out)
+{
+    if (!xyz_m || !hexes || !mat || !out || N <= 0 || Ne <= 0 || pin_node < 0 || pin_node >= N) return ORC_E_BADARG;
+    for (long q = 0; q < 8 * Ne; q++) if (hexes[q] < 0 || hexes[q] >= N) return ORC_E_RANGE;
+    oracle *o = (oracle *)calloc(1, sizeof(oracle));
+    if (!o) return ORC_E_ALLOC;
+    o->N = N; o->Ne = Ne; o->nen = 8;
+    double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
+    o->Ms = mat->Ms; o->dt = dt;
+    o->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
+    o->Kstar = mat->K1 / mu0Ms2;
+    o->dtau = mat->gamma * mat->Ms * dt;
+    o->alpha = mat->alpha;
+    o->eps1 = o->Astar * o->dtau; o->eps2 = o->alpha * o->Astar * o->dtau;
+    o->lam100 = mat->lambda100; o->lam111 = mat->lambda111;
+    memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
+    for (int q = 0; q < 9; q++) o->R[q] = (q % 4 == 0);
+    o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
+    o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
+    for (int q = 0; q < 36 * o->n_elastic; q++) o->Cstar[q] = mat->C_voigt[q] / mu0Ms2;
+    o->x = (double *)malloc((size_t)N * 3 * sizeof(double));
+    o->hex = (int *)malloc((size_t)Ne * 8 * sizeof(int));
+    o->mag = (uchar *)malloc((size_t)Ne);
+    o->eid = (int *)calloc((size_t)Ne, sizeof(int));
+    o->V = (real *)malloc((size_t)Ne * sizeof(real));
+    o->mL = (real *)malloc((size_t)N * sizeof(real)); o->mLm = (real *)malloc((size_t)N * sizeof(real));
+    o->live = (uchar *)calloc((size_t)N, 1);
+    o->clamp = (uchar *)calloc((size_t)N * 3, 1);
+    for (long i = 0; i < 3 * N; i++) o->x[i] = xyz_m[i] / ld;
+    memcpy(o->hex, hexes, (size_t)Ne * 8 * sizeof(int));
+    for (long e = 0; e < Ne; e++) o->mag[e] = magnetic ? (magnetic[e] != 0) : 1;
+    if (elastic_id) memcpy(o->eid, elastic_id, (size_t)Ne * sizeof(int));
+    if (clamp_dof) for (long i = 0; i < 3 * N; i++) o->clamp[i] = clamp_dof[i] != 0;
+    o->pin = pin_node;
+    for (long e = 0; e < Ne; e++) if (o->n_elastic && (o->eid[e] < 0 || o->eid[e] >= o->n_elastic)) { orc_destroy(o); return ORC_E_RANGE; }
+
+    /* pattern: { j : i, j share a hexahedron } U { i }, ascending */
+    int rc = build_n2e_n(N, Ne, o->hex, 8, &o->n2e_ptr, &o->n2e); if (rc) { orc_destroy(o); return rc; }
+    rc = build_pattern_n(N, o->hex, 8, o->n2e_ptr, o->n2e, &o->rowptr, &o->col, &o->nnz); if (rc) { orc_destroy(o); return rc; }
+    long nnz = o->nnz;
+    double *K = (double *)calloc((size_t)nnz, sizeof(double)), *Km = (double *)calloc((size_t)nnz, sizeof(double)),
+           *Mm = (double *)calloc((size_t)nnz, sizeof(double)), *mL = (double *)calloc((size_t)N, sizeof(double)),
+           *mLm = (double *)calloc((size_t)N, sizeof(double));
+    double *Kme = o->n_elastic ? (double *)calloc((size_t)nnz * 9, sizeof(double)) : NULL;
+    if (!K || !Km || !Mm || !mL || !mLm || (o->n_elastic && !Kme)) { orc_destroy(o); return ORC_E_ALLOC; }
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++) {
+        if (o->x[3 * i + d] < lo[d]) lo[d] = o->x[3 * i + d];
+        if (o->x[3 * i + d] > hi[d]) hi[d] = o->x[3 * i + d];
+    }
+    double diag = sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
+    double Jmin = 1e-14 * diag * diag * diag;
+    o->Vtot = 0; o->Vmag = 0;
+    for (long e = 0; e < Ne; e++) {
+        const int *t = o->hex + 8 * e;
+        double X[24];
+        for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)t[a] + d];
+        const double *C = o->n_elastic ? o->Cstar + 36 * o->eid[e] : NULL;
+        double Ve = 0;
+        for (int p = 0; p < 8; p++) {
+            double det, phi[8], g[8][3];
+            hex_gauss_point(X, p, &det, phi, g);
+            if (!(det > Jmin)) { free(K); free(Km); free(Mm); free(mL); free(mLm); free(Kme); orc_destroy(o); return ORC_E_DEGENERATE; }
+            Ve += det;
+            for (int a = 0; a < 8; a++) {
+                mL[t[a]] += det * phi[a];
+                if (o->mag[e]) { mLm[t[a]] += det * phi[a]; o->live[t[a]] = 1; }
+                for (int b = 0; b < 8; b++) {
+                    long q = find_col(o, t[a], t[b]);
+                    double kab = det * (g[a][0] * g[b][0] + g[a][1] * g[b][1] + g[a][2] * g[b][2]);
+                    double mab = det * phi[a] * phi[b];
+                    K[q] += kab;
+                    if (o->mag[e]) { Km[q] += kab; Mm[q] += mab; }
+                    if (C) {
+                        double Ba[6][3], Bb[6][3], CB[6][3];
+                        strain_disp(g[a], Ba); strain_disp(g[b], Bb);
+                        for (int r = 0; r < 6; r++) for (int s = 0; s < 3; s++) {
+                            double acc = 0; for (int w = 0; w < 6; w++) acc += C[6 * r + w] * Bb[w][s];
+                            CB[r][s] = acc;
+                        }
+                        for (int r = 0; r < 3; r++) for (int s = 0; s < 3; s++) {
+                            double acc = 0; for (int w = 0; w < 6; w++) acc += Ba[w][r] * CB[w][s];
+                            Kme[9 * q + 3 * r + s] += det * acc;
+                        }
+                    }
+                }
+            }
+        }
+        o->V[e] = (real)Ve;
+        o->Vtot += Ve;
+        if (o->mag[e]) o->Vmag += Ve;
+    }
+    for (long i = 0; i < N; i++) { o->mL[i] = (real)mL[i]; o->mLm[i] = (real)mLm[i]; }
+    rc = finish_matrices(o, K, Km, Mm, Kme);
+    free(K); free(Km); free(Mm); free(mL); free(mLm); free(Kme);
+    if (rc) { orc_destroy(o); return rc; }
+    *out = o;
+    return ORC_OK;
+}
+
 void orc_destroy(oracle *o)
 {
     if (!o) return;
+    free(o->hex);
     free(o->x); free(o->tet); free(o->mag); free(o->eid); free(o->V); free(o->G); free(o->mL); free(o->mLm);
     free(o->live); free(o->n2e_ptr); free(o->n2e); free(o->rowptr); free(o->col); free(o->K); free(o->Kms);
     free(o->Km); free(o->Mm); free(o->Kgs1); free(o->Kgs2); free(o->Kmech); free(o->Kmech_free); free(o->clamp);
@@ -595,9 +809,9 @@ int orc_get(const oracle *o, int what, void *dst)
     case 0: memcpy(dst, o->rowptr, (size_t)(o->N + 1) * sizeof(int)); break;
     case 1: memcpy(dst, o->col, (size_t)o->nnz * sizeof(int)); break;
     case 2: memcpy(dst, o->n2e_ptr, (size_t)(o->N + 1) * sizeof(int)); break;
-    case 3: memcpy(dst, o->n2e, (size_t)o->Ne * 4 * sizeof(int)); break;
+    case 3: memcpy(dst, o->n2e, (size_t)o->Ne * (o->nen == 8 ? 8 : 4) * sizeof(int)); break;
     case 4: memcpy(dst, o->V, (size_t)o->Ne * sizeof(real)); break;
-    case 5: memcpy(dst, o->G, (size_t)o->Ne * 12 * sizeof(real)); break;
+    case 5: if (o->nen == 8) return ORC_E_BADARG; memcpy(dst, o->G, (size_t)o->Ne * 12 * sizeof(real)); break;
     case 6: memcpy(dst, o->mL, (size_t)o->N * sizeof(real)); break;
     case 7: memcpy(dst, o->mLm, (size_t)o->N * sizeof(real)); break;
     case 8: memcpy(dst, o->live, (size_t)o->N); break;
@@ -730,6 +944,25 @@ int orc_volume_average(const oracle *o, const void *g_, int ncomp, double *out)
     double den = 0; double num[16];
     if (ncomp < 1 || ncomp > 16) return ORC_E_BADARG;
     for (int c = 0; c < ncomp; c++) num[c] = 0;
+    if (o->nen == 8) { /* Eq. 17 with the 2 x 2 x 2 Gauss rule: sum_e sum_p g_e(r_p) |J(e,p)| w_p */
+        for (long e = 0; e < o->Ne; e++) {
+            const int *t = o->hex + 8 * e;
+            double X[24];
+            for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)t[a] + d];
+            for (int p = 0; p < 8; p++) {
+                double det, phi[8], gr[8][3];
+                hex_gauss_point(X, p, &det, phi, gr);
+                for (int c = 0; c < ncomp; c++) {
+                    double ge = 0;
+                    for (int a = 0; a < 8; a++) ge += phi[a] * (double)g[(long)t[a] * ncomp + c];
+                    num[c] += ge * det;
+                }
+                den += det;
+            }
+        }
+        for (int c = 0; c < ncomp; c++) out[c] = num[c] / den;
+        return ORC_OK;
+    }
     for (long e = 0; e < o->Ne; e++) {
         const int *t = o->tet + 4 * e;
         for (int c = 0; c < ncomp; c++) {
@@ -749,6 +982,7 @@ int orc_volume_average(const oracle *o, const void *g_, int ncomp, double *out)
 /* ------------------------------------------------------------------------------------ */
 int orc_rhs_ms(const oracle *o, const void *m_, const double *mbar, void *b_)
 {
+    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
     const real *m = (const real *)m_; real *b = (real *)b_;
     for (long i = 0; i < o->N; i++) b[i] = 0;
     for (long e = 0; e < o->Ne; e++) {
@@ -768,6 +1002,7 @@ int orc_rhs_ms(const oracle *o, const void *m_, const double *mbar, void *b_)
  * h_d,i = -sum_{e contains i} V_e grad U_e/(4 mL_i) [+ <grad U>] (DEMAG)  - N_d mbar (FARFIELD). */
 int orc_demag_field(const oracle *o, const void *U_, const double *mbar, unsigned terms, void *hd_, double *gradU_mean)
 {
+    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
     const real *U = (const real *)U_; real *hd = (real *)hd_;
     long N = o->N;
     for (long i = 0; i < 3 * N; i++) hd[i] = 0;
@@ -876,6 +1111,7 @@ static void C_times(const oracle *o, long e, const real eps[6], real sig[6])
  * b_(i,a) = sum_{e contains i, magnetic} V_e [C*_e : mean_e E0(m)]_ab d_b phi_i; clamped DOFs zeroed. */
 int orc_rhs_mech(const oracle *o, const void *m_, void *b_)
 {
+    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
     const real *m = (const real *)m_; real *b = (real *)b_;
     if (!o->n_elastic) return ORC_E_BADARG;
     for (long i = 0; i < 3 * o->N; i++) b[i] = 0;
@@ -914,6 +1150,7 @@ static void elem_strain(const oracle *o, long e, const real *u, real eps[6])
  * sigma_hat_i = sum_{e contains i, magnetic} V_e sigma_e/(4 mLm_i).  Output N x 6 Voigt. */
 int orc_stress_recover(const oracle *o, const void *u_, const void *w_, void *sig_)
 {
+    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
     const real *u = (const real *)u_, *w = (const real *)w_; real *sg = (real *)sig_;
     if (!o->n_elastic) return ORC_E_BADARG;
     for (long i = 0; i < 6 * o->N; i++) sg[i] = 0;
@@ -976,6 +1213,7 @@ double orc_energy(const oracle *o, const void *m_, const void *U_, const void *u
     const real *m = (const real *)m_, *U = (const real *)U_, *u = (const real *)u_;
     long N = o->N;
     double E = 0;
+    if (o->nen == 8) return NAN; /* tetrahedral only (R26) */
     real *y = (real *)malloc((size_t)3 * N * sizeof(real));
     for (int c = 0; c < 3; c++) { /* exchange 1/2 A* m_a^T K_m m_a */
         spmv(o, MAT_K_M, m, y, 3, c);
@@ -1020,6 +1258,7 @@ static int helmholtz(const oracle *o, int id, const real *f, real *g, int a, con
 
 int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_, void *u_, orc_step_info *info)
 {
+    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
     real *m = (real *)m_, *U = (real *)U_, *u = (real *)u_;
     long N = o->N; unsigned terms = p->terms;
     int worst = ORC_OK, rc;

@@ -148,10 +148,45 @@ def kuhn_box(grid, box, jitter=0.15, seed_mesh=1, seed_perm=2, permute=True) -> 
                 grid=tuple(grid), box=tuple(box), node_perm=P)
 
 
+@dataclass
+class HexMesh:
+    """Linear hexahedra; local node a = i + 2 j + 4 k of hexes[e] sits at corner (i, j, k) of the cell (R26)."""
+    xyz: np.ndarray          # (N, 3) metres
+    hexes: np.ndarray        # (Ne, 8) int32
+    magnetic: np.ndarray
+    elastic_id: np.ndarray
+    grid: Tuple[int, int, int] = (0, 0, 0)
+    box: Tuple[float, float, float] = (0.0, 0.0, 0.0)
+    node_perm: Optional[np.ndarray] = None
+
+    @property
+    def n_nodes(self) -> int:
+        return int(self.xyz.shape[0])
+
+    @property
+    def n_tets(self) -> int:          # number of elements (the name the binding and the oracle read)
+        return int(self.hexes.shape[0])
+
+
+def hex_box(grid, box, jitter=0.15, seed_mesh=1, seed_perm=2, permute=True) -> HexMesh:
+    """Structured nx x ny x nz node grid of linear hexahedra (the paper's Fig. 2-3 meshes): same node numbering,
+    jitter and label permutation as kuhn_box, one hexahedron per cell."""
+    t = kuhn_box(grid, box, jitter=jitter, seed_mesh=seed_mesh, seed_perm=seed_perm, permute=permute)
+    nx, ny, nz = grid
+    hx, hy, hz = np.meshgrid(np.arange(nx - 1), np.arange(ny - 1), np.arange(nz - 1), indexing="ij")
+    hx, hy, hz = hx.ravel(), hy.ravel(), hz.ravel()
+    cols = [((hz + k) * ny + (hy + j)) * nx + (hx + i) for k in (0, 1) for j in (0, 1) for i in (0, 1)]   # a = i + 2 j + 4 k
+    hexes = t.node_perm[np.stack(cols, axis=1)].astype(np.int32)
+    ne = hexes.shape[0]
+    return HexMesh(xyz=t.xyz, hexes=np.ascontiguousarray(hexes), magnetic=np.ones(ne, np.uint8), elastic_id=np.zeros(ne, np.int32),
+                   grid=tuple(grid), box=tuple(box), node_perm=t.node_perm)
+
+
 def flag_inclusion(mesh: Mesh, center, semi_axes, rotation: Optional[np.ndarray] = None) -> Mesh:
-    """Flag tets whose centroid lies inside the (rotated) ellipsoid as non-magnetic,
+    """Flag elements (tets or hexahedra) whose centroid lies inside the (rotated) ellipsoid as non-magnetic,
     elastic material 1."""
-    c = mesh.xyz[mesh.tets].mean(axis=1) - np.asarray(center)
+    conn = mesh.hexes if hasattr(mesh, "hexes") else mesh.tets
+    c = mesh.xyz[conn].mean(axis=1) - np.asarray(center)
     if rotation is not None:
         c = c @ rotation          # coordinates in the ellipsoid frame (columns = axes)
     inside = ((c / np.asarray(semi_axes)) ** 2).sum(axis=1) <= 1.0

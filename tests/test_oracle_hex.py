@@ -1,0 +1,158 @@
+"""Pins for the oracle's linear hexahedral (Q1) matrices (R26).  CPU only.
+Closed forms of the trilinear element on a uniform grid (the classical 27-point stiffness and the tensor-product mass),
+exactness properties of the 2 x 2 x 2 Gauss rule on distorted cells (volume, patch test, rigid-body modes, linear-field
+energies and averages), and dense solves."""
+import numpy as np
+import pytest
+
+from paper_2510_09812_b200 import inputs
+
+NM = 1e-9
+MU0 = 4e-7 * np.pi
+
+
+@pytest.fixture(scope="module")
+def orc(oracle_mod):
+    return oracle_mod
+
+
+def mat2():
+    C = inputs.isotropic_voigt(200e9, 0.3)
+    return inputs.Material(C_voigt=np.stack([C, 2 * C]))
+
+
+@pytest.fixture(scope="module")
+def jit(orc):
+    mesh = inputs.hex_box((7, 6, 5), (18 * NM, 15 * NM, 10 * NM), seed_mesh=3, seed_perm=4)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (5 * NM, 4 * NM, 3 * NM))
+    clamp = inputs.clamp_bottom(mesh)
+    return mesh, orc.Oracle(mesh, mat2(), 1e-12, clamp_dof=clamp, pin_node=2), clamp
+
+
+def test_hex_generator_local_node_order():
+    mesh = inputs.hex_box((3, 4, 5), (2 * NM, 3 * NM, 4 * NM), jitter=0.0)
+    x = mesh.xyz[mesh.hexes] / NM                     # (Ne, 8, 3)
+    assert np.allclose(x[:, 1] - x[:, 0], [1, 0, 0]) and np.allclose(x[:, 2] - x[:, 0], [0, 1, 0])
+    assert np.allclose(x[:, 4] - x[:, 0], [0, 0, 1]) and np.allclose(x[:, 7] - x[:, 0], [1, 1, 1])
+    assert mesh.n_tets == 2 * 3 * 4
+
+
+def test_uniform_grid_closed_forms(orc):
+    """Cubic cells of side h: K = 27-point stencil (8h/3 centre, 0 faces, -h/6 edges, -h/12 corners);
+    M = tensor product of the 1D consistent mass h/6 [1 4 1]."""
+    n, h = 6, 2.0
+    mesh = inputs.hex_box((n, n, n), ((n - 1) * h * NM,) * 3, jitter=0.0, permute=False)
+    o = orc.Oracle(mesh, inputs.Material(), 1e-12)
+    assert o.nnz == (3 * n - 2) ** 3                               # (sum over a line of 2,3,...,3,2)^3
+    K = o.csr(orc.MAT_K_FREE).toarray(); M = o.csr(orc.MAT_MASS).toarray()
+    nid = lambda a, b, c: (c * n + b) * n + a
+    i = nid(2, 3, 2)
+    kexp = {0: 8 * h / 3, 1: 0.0, 2: -h / 6, 3: -h / 12}
+    m1 = {0: 4 * h / 6, 1: h / 6}
+    for da in (-1, 0, 1):
+        for db in (-1, 0, 1):
+            for dc in (-1, 0, 1):
+                j = nid(2 + da, 3 + db, 2 + dc)
+                assert K[i, j] == pytest.approx(kexp[abs(da) + abs(db) + abs(dc)], abs=1e-13)
+                assert M[i, j] == pytest.approx(m1[abs(da)] * m1[abs(db)] * m1[abs(dc)], rel=1e-13)
+    assert np.count_nonzero(np.abs(K[i]) > 1e-12) == 1 + 12 + 8
+    assert np.allclose(o.mL().reshape(n, n, n)[1:-1, 1:-1, 1:-1], h ** 3, rtol=1e-13)
+
+
+def test_symmetry_rowsums_volume_patch(orc, jit):
+    mesh, o, clamp = jit
+    K = o.csr(orc.MAT_K_FREE); Km = o.csr(orc.MAT_K_M); M = o.csr(orc.MAT_MASS)
+    for A in (K, Km, M):
+        assert abs(A - A.T).max() <= 1e-14 * abs(A).max()
+    assert np.abs(K.sum(1)).max() <= 1e-13 * abs(K).sum(1).max()
+    vol = np.prod(np.array(mesh.box) / NM)
+    assert o.Vtot == pytest.approx(vol, rel=1e-13) and o.V().sum() == pytest.approx(vol, rel=1e-13)
+    assert o.mL().sum() == pytest.approx(vol, rel=1e-13)
+    assert np.allclose(np.asarray(M.sum(1)).ravel(), o.mLm(), rtol=1e-12, atol=1e-13)
+    assert M.sum() == pytest.approx(o.Vmag, rel=1e-13) and 0 < o.Vmag < vol
+    # patch test: a linear field gives zero at every node off the outer boundary (2 x 2 x 2 Gauss is exact for it)
+    x = mesh.xyz / NM
+    u = x @ np.array([0.3, -0.7, 0.2]) + 1.5
+    r = K @ u
+    L = np.array(mesh.box) / NM
+    interior = ((x > 1e-9) & (x < L - 1e-9)).all(1)
+    assert interior.sum() > 20 and np.abs(r[interior]).max() <= 1e-12 * np.abs(K).max() * np.abs(u).max()
+    assert u @ r == pytest.approx(vol * (0.09 + 0.49 + 0.04), rel=1e-12)          # int |grad u|^2
+    w = np.linalg.eigvalsh(K.toarray())
+    assert np.sum(np.abs(w) < 1e-10 * w.max()) == 1 and w.min() > -1e-10 * w.max()
+    # consistent mass: u^T M u = int_{Omega_m} u^2 is NOT exact on distorted cells (degree 4 per variable), but 1^T M u is
+    assert np.ones(o.N) @ (M @ u) == pytest.approx((o.mLm() * u).sum(), rel=1e-13)
+
+
+def test_mech_matrix_rigid_modes_and_linear_energy(orc, jit):
+    mesh, o, clamp = jit
+    A = o.csr(orc.MAT_K_MECH_FREE)
+    assert abs(A - A.T).max() <= 1e-13 * abs(A).max()
+    x = mesh.xyz / NM
+    for a in range(3):
+        t = np.zeros((o.N, 3)); t[:, a] = 1
+        assert np.abs(A @ t.ravel()).max() <= 1e-12 * abs(A).max()
+        rot = np.cross(np.eye(3)[a], x)
+        assert np.abs(A @ rot.ravel()).max() <= 1e-11 * abs(A).max() * np.abs(x).max()
+    w = np.linalg.eigvalsh(A.toarray())
+    assert np.sum(np.abs(w) < 1e-9 * w.max()) == 6
+    # homogeneous body: u = G x has energy vol * symG : C* : symG
+    mesh1 = inputs.hex_box((5, 5, 4), (10 * NM, 12 * NM, 9 * NM), seed_mesh=5, seed_perm=6)
+    m1 = inputs.Material()
+    o1 = orc.Oracle(mesh1, m1, 1e-12)
+    G = np.array([[1e-3, 2e-3, 0.0], [-1e-3, 5e-4, 3e-3], [2e-3, 0.0, -1e-3]])
+    u = (mesh1.xyz / NM) @ G.T
+    E = 0.5 * (G + G.T)
+    ev = np.array([E[0, 0], E[1, 1], E[2, 2], 2 * E[1, 2], 2 * E[0, 2], 2 * E[0, 1]])
+    Cs = m1.C_voigt[0] / (MU0 * m1.Ms ** 2)
+    A1 = o1.csr(orc.MAT_K_MECH_FREE)
+    assert u.ravel() @ (A1 @ u.ravel()) == pytest.approx(10 * 12 * 9 * ev @ Cs @ ev, rel=1e-12)
+    # constrained matrix: identity rows / columns at clamped DOFs
+    Ac = o.csr(orc.MAT_K_MECH).toarray()
+    c = np.flatnonzero(clamp)
+    assert np.array_equal(Ac[c][:, c], np.eye(len(c))) and np.abs(Ac[c]).sum() == len(c)
+
+
+def test_constraints_dead_nodes_and_helmholtz(orc, jit):
+    mesh, o, clamp = jit
+    live = o.live().astype(bool)
+    assert 0 < (~live).sum() < o.N
+    Kms = o.csr(orc.MAT_K_MS).toarray()
+    assert Kms[2, 2] == 1 and np.abs(Kms[2]).sum() == 1 and np.abs(Kms[:, 2]).sum() == 1
+    G1 = o.csr(orc.MAT_K_GS1).toarray()
+    d = np.flatnonzero(~live)
+    assert np.array_equal(G1[d][:, d], np.eye(len(d))) and np.abs(G1[d]).sum() == len(d)
+    M = o.csr(orc.MAT_MASS).toarray(); Km = o.csr(orc.MAT_K_M).toarray()
+    eps1 = o.Astar * o.dtau
+    assert np.allclose(G1[live][:, live], (M + eps1 * Km)[live][:, live], rtol=1e-13, atol=1e-15)
+    assert np.linalg.eigvalsh(G1).min() > 0
+
+
+def test_volume_average_and_cg(orc, jit):
+    mesh, o, clamp = jit
+    x = mesh.xyz / NM
+    g = np.stack([x @ [0.2, 0.1, -0.4] + 3.0, np.ones(o.N), x[:, 2]], axis=1)
+    L = np.array(mesh.box) / NM
+    assert np.allclose(o.volume_average(g), [L @ [0.2, 0.1, -0.4] / 2 + 3.0, 1.0, L[2] / 2], rtol=1e-13)
+    rng = np.random.default_rng(1)
+    for mat, n in ((orc.MAT_K_MS, o.N), (orc.MAT_K_GS1, o.N), (orc.MAT_K_MECH, 3 * o.N)):
+        b = rng.normal(size=n)
+        if mat == orc.MAT_K_MS:
+            b[2] = 0
+        if mat == orc.MAT_K_MECH:
+            b[clamp.astype(bool)] = 0
+        xs, it, res, rc = o.cg(mat, b, tol=1e-12)
+        assert rc == 0 and it > 3
+        assert np.abs(xs - np.linalg.solve(o.csr(mat).toarray(), b)).max() <= 1e-9 * np.abs(xs).max()
+
+
+def test_tet_only_entry_points_refuse_hexahedra(orc, jit):
+    mesh, o, clamp = jit
+    m = np.zeros((o.N, 3)); m[:, 0] = 1
+    with pytest.raises(AssertionError):
+        o.rhs_mech(m)
+    info, rc = o.gspm_step(m, np.zeros(o.N), np.zeros((o.N, 3)), 1e-12, [0, 0, 0], 0)
+    assert rc == -1
+    bad = inputs.replace(mesh, hexes=mesh.hexes[:, [1, 0, 2, 3, 4, 5, 6, 7]].copy())     # inverted cell
+    with pytest.raises(RuntimeError, match="rc=-2"):
+        orc.Oracle(bad, mat2(), 1e-12)
