@@ -150,7 +150,8 @@ def test_rotated_fields_are_energy_gradients(orc, R):
     fd = _fd_field(lambda mm: o.energy(mm, None, u, [0, 0, 0], TERM_MAGEL) - o.energy(mm, None, u, [0, 0, 0], 0),
                    m, nodes, o.mLm(), 1e-4)
     assert np.abs(h[nodes]).max() > 1e-4
-    assert np.allclose(h[nodes], fd, rtol=1e-6, atol=2e-9)
+    # (the two energies are OpenMP sums of ~1e3-sized terms in no fixed order: a few 1e-9 of noise after dividing by 2h)
+    assert np.allclose(h[nodes], fd, rtol=2e-6, atol=2e-8)
 
 
 @pytest.mark.parametrize("R", [inputs.R_111, rot(7)])
