@@ -29,7 +29,7 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
-EXPORTS = ("cm_mesh_create", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
+EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
            "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_field_rhs", "cm_volume_average",
            "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
@@ -87,6 +87,7 @@ def lib():
         vp, lg, it, db = C.c_void_p, C.c_long, C.c_int, C.c_double
         L.cm_mesh_create.argtypes = [vp, lg, vp, lg, vp, vp, it, vp, C.POINTER(vp)]
         L.cm_mesh_create_wrapped.argtypes = [vp, lg, vp, lg, vp, vp, vp, lg, it, vp, C.POINTER(vp)]
+        L.cm_mesh_create_hex.argtypes = [vp, lg, vp, lg, vp, vp, it, vp, C.POINTER(vp)]
         L.cm_periodic_wrap.argtypes = [vp, lg, C.c_uint, db, vp, C.POINTER(lg)]
         L.cm_mesh_destroy.argtypes = [vp]
         L.cm_mesh_get.argtypes = [vp, it, vp, lg]
@@ -162,7 +163,12 @@ class Mesh:
         xyz = _np(xyz, np.float64); tets = _np(tets, np.int32)
         mag = _np(magnetic, np.uint8); eid = _np(elastic_id, np.int32)
         self.h = C.c_void_p()
-        if dof_of_node is None:
+        self.nen = 8 if tets.shape[1] == 8 else 4            # (Ne, 8): linear hexahedra, local node a = i + 2 j + 4 k
+        if self.nen == 8:
+            assert dof_of_node is None
+            _check(L.cm_mesh_create_hex(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), reorder, _stream(),
+                                        C.byref(self.h)))
+        elif dof_of_node is None:
             _check(L.cm_mesh_create(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), reorder, _stream(),
                                     C.byref(self.h)))
         else:
@@ -175,11 +181,12 @@ class Mesh:
         self.n_nodes, self.n_tets, self.nnz = (int(c) for c in cnt)
 
     def get(self, what):
-        n = {CM_GET_ORDER: self.n_nodes, CM_GET_IPERM: self.n_nodes, CM_GET_TETS: 4 * self.n_tets, CM_GET_TET_ORDER: self.n_tets,
-             CM_GET_ROWPTR: self.n_nodes + 1, CM_GET_COLIDX: self.nnz, CM_GET_N2E_PTR: self.n_nodes + 1, CM_GET_N2E: 4 * self.n_tets}[what]
+        n = {CM_GET_ORDER: self.n_nodes, CM_GET_IPERM: self.n_nodes, CM_GET_TETS: self.nen * self.n_tets, CM_GET_TET_ORDER: self.n_tets,
+             CM_GET_ROWPTR: self.n_nodes + 1, CM_GET_COLIDX: self.nnz, CM_GET_N2E_PTR: self.n_nodes + 1,
+             CM_GET_N2E: self.nen * self.n_tets}[what]
         a = np.empty(n, np.int32)
         _check(lib().cm_mesh_get(self.h, what, _hp(a), n))
-        return a.reshape(-1, 4) if what == CM_GET_TETS else a
+        return a.reshape(-1, self.nen) if what == CM_GET_TETS else a
 
     def volume_average(self, g):
         """cm_volume_average of a torch CUDA tensor (N,) or (N, ncomp), float64 / float32."""

@@ -161,6 +161,100 @@ __global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const
     }
 }
 
+// ---- linear hexahedra (R26): one thread per row i accumulates, over the incident elements in ascending order and the
+// 2 x 2 x 2 Gauss points in order, row i of K, K_m, M_m, K^mech and the lumped masses int phi_i.
+__device__ __forceinline__ double hex_point(const double X[8][3], int p, double phi[8], double g[8][3])
+{
+    const double q = 0.57735026918962576451;
+    const double xi[3] = {(p & 1) ? q : -q, (p & 2) ? q : -q, (p & 4) ? q : -q};
+    double dN[8][3], J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+    for (int a = 0; a < 8; a++) {
+        const double s[3] = {(a & 1) ? 1.0 : -1.0, (a & 2) ? 1.0 : -1.0, (a & 4) ? 1.0 : -1.0};
+        const double f[3] = {1 + s[0] * xi[0], 1 + s[1] * xi[1], 1 + s[2] * xi[2]};
+        phi[a] = f[0] * f[1] * f[2] / 8;
+        dN[a][0] = s[0] * f[1] * f[2] / 8; dN[a][1] = f[0] * s[1] * f[2] / 8; dN[a][2] = f[0] * f[1] * s[2] / 8;
+#pragma unroll
+        for (int r = 0; r < 3; r++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) J[r][c] += X[a][r] * dN[a][c];
+    }
+    double cof[3][3];
+    cof[0][0] = J[1][1] * J[2][2] - J[1][2] * J[2][1]; cof[0][1] = J[1][2] * J[2][0] - J[1][0] * J[2][2]; cof[0][2] = J[1][0] * J[2][1] - J[1][1] * J[2][0];
+    cof[1][0] = J[0][2] * J[2][1] - J[0][1] * J[2][2]; cof[1][1] = J[0][0] * J[2][2] - J[0][2] * J[2][0]; cof[1][2] = J[0][1] * J[2][0] - J[0][0] * J[2][1];
+    cof[2][0] = J[0][1] * J[1][2] - J[0][2] * J[1][1]; cof[2][1] = J[0][2] * J[1][0] - J[0][0] * J[1][2]; cof[2][2] = J[0][0] * J[1][1] - J[0][1] * J[1][0];
+    const double det = J[0][0] * cof[0][0] + J[0][1] * cof[0][1] + J[0][2] * cof[0][2];
+#pragma unroll
+    for (int a = 0; a < 8; a++)
+#pragma unroll
+        for (int r = 0; r < 3; r++) g[a][r] = (cof[r][0] * dN[a][0] + cof[r][1] * dN[a][1] + cof[r][2] * dN[a][2]) / det;
+    return det;
+}
+
+template <typename T>
+__global__ void hex_rows_kernel(long N, const int *__restrict__ hexes, const double *__restrict__ xyz, double ld,
+                                const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const uchar *__restrict__ mag,
+                                const int *__restrict__ eid, const double *__restrict__ Cstar, const int *__restrict__ rowptr,
+                                const int *__restrict__ col, double *K, double *Km, double *Mm, double *Kme, T *mL, T *mLm, uchar *live)
+{
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int q0 = rowptr[i], q1 = rowptr[i + 1];
+    double ml = 0, mlm = 0;
+    bool lv = false;
+    for (int s = n2e_ptr[i]; s < n2e_ptr[i + 1]; s++) {
+        const int e = n2e[s] >> 3, k = n2e[s] & 7;
+        int t[8], pos[8];
+        double X[8][3];
+        for (int a = 0; a < 8; a++) {
+            t[a] = hexes[8 * (long)e + a];
+            for (int d = 0; d < 3; d++) X[a][d] = xyz[3 * (long)t[a] + d] / ld;
+            int lo = q0, hi = q1 - 1; // position of column t[a] in the sorted row
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (col[mid] < t[a]) lo = mid + 1; else hi = mid;
+            }
+            pos[a] = lo;
+        }
+        const bool m = mag[e];
+        const double *C = Cstar ? Cstar + 36 * eid[e] : nullptr;
+        for (int p = 0; p < 8; p++) {
+            double phi[8], g[8][3];
+            const double det = hex_point(X, p, phi, g);
+            ml += det * phi[k];
+            if (m) { mlm += det * phi[k]; lv = true; }
+            double CBt[3][6];
+            if (C) {
+                double Bk[6][3];
+                strain_disp(g[k], Bk);
+                for (int r = 0; r < 3; r++)
+                    for (int w = 0; w < 6; w++) {
+                        double acc = 0;
+                        for (int v = 0; v < 6; v++) acc += Bk[v][r] * C[6 * v + w];
+                        CBt[r][w] = acc;
+                    }
+            }
+            for (int b = 0; b < 8; b++) {
+                const double kab = det * (g[k][0] * g[b][0] + g[k][1] * g[b][1] + g[k][2] * g[b][2]);
+                const double mab = det * phi[k] * phi[b];
+                K[pos[b]] += kab;
+                if (m) { Km[pos[b]] += kab; Mm[pos[b]] += mab; }
+                if (C) {
+                    double Bb[6][3];
+                    strain_disp(g[b], Bb);
+                    for (int r = 0; r < 3; r++)
+                        for (int c = 0; c < 3; c++) {
+                            double acc = 0;
+                            for (int w = 0; w < 6; w++) acc += CBt[r][w] * Bb[w][c];
+                            Kme[9 * (long)pos[b] + 3 * r + c] += det * acc;
+                        }
+                }
+            }
+        }
+    }
+    mL[i] = (T)ml; mLm[i] = (T)mlm; live[i] = lv;
+}
+
 // one thread per row: apply constraints (P A P + (I - P)), form K^GS(eps), round to T and store in the sliced
 // layouts (cm_internal.h): scalar matrices at spS[i / CS] + j * CS + i % CS, the 9 entries of a K^mech block in
 // the 9 planes of its slice, plane k at 9 * spB[s] + k * L_s + (j * CB + i % CB).
@@ -328,31 +422,42 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         CM_CUDA(cudaStreamSynchronize(st));
     }
     // geometry
+    const bool hex = M->nen == 8;
     double *Vd = nullptr, *vsum = nullptr;
-    CM_CUDA(cudaMalloc((void **)&Vd, Ne * sizeof(double)));
-    CM_CUDA(cudaMalloc((void **)&vsum, 2 * sizeof(double)));
     const int B = 256;
-    geom_kernel<T><<<M->ck.nchunks, B, 0, st>>>(M->ck.d_eptr, M->d_gtets, M->d_gxyz, ld, S->EG, Vd);
-    lump_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, M->d_n2e_ptr, M->d_n2e, Vd, M->d_mag, S->mL, S->mLm, S->live);
-    volume_sum_kernel<<<1, 1024, 0, st>>>(Ne, Vd, M->d_mag, vsum);
-    CM_CUDA(cudaGetLastError());
-    double hv[2];
-    CM_CUDA(cudaMemcpyAsync(hv, vsum, sizeof(hv), cudaMemcpyDeviceToHost, st));
-    CM_CUDA(cudaStreamSynchronize(st));
-    S->Vtot = hv[0]; S->Vmag = hv[1];
-    {
-        std::vector<uchar> lv(N);
-        CM_CUDA(cudaMemcpy(lv.data(), S->live, N, cudaMemcpyDeviceToHost));
-        S->nlive = 0;
-        for (long i = 0; i < N; i++) S->nlive += lv[i];
+    if (!hex) {
+        CM_CUDA(cudaMalloc((void **)&Vd, Ne * sizeof(double)));
+        CM_CUDA(cudaMalloc((void **)&vsum, 2 * sizeof(double)));
+        geom_kernel<T><<<M->ck.nchunks, B, 0, st>>>(M->ck.d_eptr, M->d_gtets, M->d_gxyz, ld, S->EG, Vd);
+        lump_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, M->d_n2e_ptr, M->d_n2e, Vd, M->d_mag, S->mL, S->mLm, S->live);
+        volume_sum_kernel<<<1, 1024, 0, st>>>(Ne, Vd, M->d_mag, vsum);
+        CM_CUDA(cudaGetLastError());
+        double hv[2];
+        CM_CUDA(cudaMemcpyAsync(hv, vsum, sizeof(hv), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaStreamSynchronize(st));
+        S->Vtot = hv[0]; S->Vmag = hv[1];
+    } else {
+        S->Vtot = M->vtot_m3 / (ld * ld * ld); S->Vmag = M->vmag_m3 / (ld * ld * ld);
     }
     // matrices: fp64 scratch on the pattern
     double *K = nullptr, *Km = nullptr, *Mm = nullptr, *Kme = nullptr;
     CM_TRY(alloc(&K, nnz)); CM_TRY(alloc(&Km, nnz)); CM_TRY(alloc(&Mm, nnz));
     if (S->n_elastic) CM_TRY(alloc(&Kme, 9 * nnz));
     const int BA = 128;
-    assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_gtets, M->d_gxyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag,
-                                                                      M->d_eid, Cd, M->d_rowptr, M->d_col, K, Km, Mm, Kme);
+    if (hex)
+        hex_rows_kernel<T><<<(unsigned)((N + 63) / 64), 64, 0, st>>>(N, M->d_tets, M->d_xyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag, M->d_eid, Cd,
+                                                                    M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->mL, S->mLm, S->live);
+    else
+        assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_gtets, M->d_gxyz, ld, M->d_n2e_ptr, M->d_n2e,
+                                                                          M->d_mag, M->d_eid, Cd, M->d_rowptr, M->d_col, K, Km, Mm, Kme);
+    CM_CUDA(cudaGetLastError());
+    CM_CUDA(cudaStreamSynchronize(st));
+    {
+        std::vector<uchar> lv(N);
+        CM_CUDA(cudaMemcpy(lv.data(), S->live, N, cudaMemcpyDeviceToHost));
+        S->nlive = 0;
+        for (long i = 0; i < N; i++) S->nlive += lv[i];
+    }
     finalize_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, nnz, M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->live, S->clamp, S->pin,
                                                                  S->eps1, S->eps2, M->sell[0].d_sp, M->sell[1].d_sp, S->Kms, S->Kgs1, S->Kgs2,
                                                                  S->Mm, S->Kmech);

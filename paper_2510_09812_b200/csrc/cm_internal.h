@@ -72,6 +72,8 @@ struct Chunks {
 
 struct cm_mesh {
     long N = 0, Ne = 0, nnz = 0;
+    int nen = 4;               // nodes per element: 4 = linear tetrahedra, 8 = linear hexahedra (matrices and averages only, R26)
+    double vtot_m3 = 0, vmag_m3 = 0; // hexahedra: volumes summed on the host (metres^3)
     bool identity = true;
     // host copies, library order
     std::vector<int> order, iperm, tets, tet_order, rowptr, col, n2e_ptr, n2e, eid;
@@ -199,6 +201,8 @@ struct System : SystemBase {
 // ---- cm_mesh.cu ----
 int mesh_build_host(cm_mesh *M, const double *xyz, long Ng, const int *gtets, long Ne, const uchar *mag, const int *eid,
                     const int *dof, long N, cm_reorder reorder);
+int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes, long Ne, const uchar *mag, const int *eid,
+                        cm_reorder reorder);
 int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out);
 int build_chunks(long N, long Ne, const int *tets, Chunks *out);
 

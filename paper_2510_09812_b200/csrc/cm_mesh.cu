@@ -60,18 +60,18 @@ void morton_order(long N, const double *xyz, std::vector<int> &order)
     for (long i = 0; i < N; i++) order[i] = key[i].second;
 }
 
-void build_n2e(long N, long Ne, const int *tets, std::vector<int> &ptr, std::vector<int> &lst)
+void build_n2e(long N, long Ne, const int *tets, std::vector<int> &ptr, std::vector<int> &lst, int nen = 4)
 {
     ptr.assign(N + 1, 0);
-    lst.resize(4 * Ne);
-    for (long q = 0; q < 4 * Ne; q++) ptr[tets[q] + 1]++;
+    lst.resize((long)nen * Ne);
+    for (long q = 0; q < (long)nen * Ne; q++) ptr[tets[q] + 1]++;
     for (long i = 0; i < N; i++) ptr[i + 1] += ptr[i];
     std::vector<int> fill(ptr.begin(), ptr.end() - 1);
-    for (long q = 0; q < 4 * Ne; q++) lst[fill[tets[q]]++] = (int)q; // q = 4 e + k, ascending
+    for (long q = 0; q < (long)nen * Ne; q++) lst[fill[tets[q]]++] = (int)q; // q = nen e + k, ascending
 }
 
 void build_pattern(long N, const int *tets, const std::vector<int> &ptr, const std::vector<int> &lst, std::vector<int> &rowptr,
-                   std::vector<int> &col)
+                   std::vector<int> &col, int nen = 4)
 {
     rowptr.assign(N + 1, 0);
     std::vector<int> cnt(N);
@@ -83,8 +83,8 @@ void build_pattern(long N, const int *tets, const std::vector<int> &ptr, const s
             tmp.clear();
             tmp.push_back((int)i);
             for (int s = ptr[i]; s < ptr[i + 1]; s++) {
-                const int *t = tets + 4 * (lst[s] >> 2);
-                tmp.insert(tmp.end(), t, t + 4);
+                const int *t = tets + (long)nen * (lst[s] / nen);
+                tmp.insert(tmp.end(), t, t + nen);
             }
             std::sort(tmp.begin(), tmp.end());
             cnt[i] = (int)(std::unique(tmp.begin(), tmp.end()) - tmp.begin());
@@ -100,8 +100,8 @@ void build_pattern(long N, const int *tets, const std::vector<int> &ptr, const s
             tmp.clear();
             tmp.push_back((int)i);
             for (int s = ptr[i]; s < ptr[i + 1]; s++) {
-                const int *t = tets + 4 * (lst[s] >> 2);
-                tmp.insert(tmp.end(), t, t + 4);
+                const int *t = tets + (long)nen * (lst[s] / nen);
+                tmp.insert(tmp.end(), t, t + nen);
             }
             std::sort(tmp.begin(), tmp.end());
             auto e = std::unique(tmp.begin(), tmp.end());
@@ -279,6 +279,110 @@ int mesh_build_host(cm_mesh *M, const double *gx, long Ng, const int *gtets, lon
         if (M->eid[e] < 0 || M->eid[e] > 0x7ffe) { cm_set_error("cm_mesh_create: elastic_id %d outside [0, 32766]", M->eid[e]); return CM_E_INDEX_RANGE; }
         M->emat[e] = (unsigned short)(M->eid[e] << 1 | (M->mag[e] ? 1 : 0));
     }
+    return CM_OK;
+}
+
+// ---- linear hexahedra (R26): host-side Gauss quadrature used for validation, volumes and lumped volume fractions
+// local node a = i + 2 j + 4 k <-> (xi, eta, zeta) = (2i-1, 2j-1, 2k-1); 2 x 2 x 2 Gauss points, unit weights
+static double hex_detJ_phi(const double X[8][3], int p, double phi[8])
+{
+    const double g = 0.57735026918962576451;
+    const double xi[3] = {(p & 1) ? g : -g, (p & 2) ? g : -g, (p & 4) ? g : -g};
+    double J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    for (int a = 0; a < 8; a++) {
+        const double s[3] = {(a & 1) ? 1.0 : -1.0, (a & 2) ? 1.0 : -1.0, (a & 4) ? 1.0 : -1.0};
+        const double f[3] = {1 + s[0] * xi[0], 1 + s[1] * xi[1], 1 + s[2] * xi[2]};
+        phi[a] = f[0] * f[1] * f[2] / 8;
+        const double dN[3] = {s[0] * f[1] * f[2] / 8, f[0] * s[1] * f[2] / 8, f[0] * f[1] * s[2] / 8};
+        for (int r = 0; r < 3; r++)
+            for (int c = 0; c < 3; c++) J[r][c] += X[a][r] * dN[c];
+    }
+    return J[0][0] * (J[1][1] * J[2][2] - J[1][2] * J[2][1]) - J[0][1] * (J[1][0] * J[2][2] - J[1][2] * J[2][0]) +
+           J[0][2] * (J[1][0] * J[2][1] - J[1][1] * J[2][0]);
+}
+
+int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes, long Ne, const uchar *mag, const int *eid,
+                        cm_reorder reorder)
+{
+    M->N = N; M->Ne = Ne; M->Ng = N; M->nen = 8; M->wrapped = false;
+    for (long q = 0; q < 8 * Ne; q++)
+        if (hexes[q] < 0 || hexes[q] >= N) {
+            cm_set_error("cm_mesh_create_hex: element %ld references node %d outside [0, %ld)", q / 8, hexes[q], N);
+            return CM_E_INDEX_RANGE;
+        }
+    double lo[3], hi[3];
+    for (int d = 0; d < 3; d++) lo[d] = hi[d] = xyz[d];
+    for (long i = 0; i < N; i++)
+        for (int d = 0; d < 3; d++) { lo[d] = std::min(lo[d], xyz[3 * i + d]); hi[d] = std::max(hi[d], xyz[3 * i + d]); }
+    const double diag = std::sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
+    const double jmin = 1e-14 * diag * diag * diag;
+    std::vector<double> w_user(N, 0.0);
+    double vtot = 0, vmag = 0;
+    for (long e = 0; e < Ne; e++) {
+        double X[8][3], phi[8];
+        for (int a = 0; a < 8; a++)
+            for (int d = 0; d < 3; d++) X[a][d] = xyz[3 * (long)hexes[8 * e + a] + d];
+        double ve = 0;
+        for (int p = 0; p < 8; p++) {
+            const double det = hex_detJ_phi(X, p, phi);
+            if (!(det > jmin)) {
+                cm_set_error("cm_mesh_create_hex: element %ld is degenerate or inverted (det J = %.3e at Gauss point %d)", e, det, p);
+                return CM_E_DEGENERATE_TET;
+            }
+            ve += det;
+            for (int a = 0; a < 8; a++) w_user[hexes[8 * e + a]] += det * phi[a];
+        }
+        vtot += ve;
+        if (!mag || mag[e]) vmag += ve;
+    }
+    M->vtot_m3 = vtot; M->vmag_m3 = vmag;
+    std::vector<int> ptr_u, lst_u;
+    if (reorder == CM_REORDER_NONE) {
+        M->order.resize(N);
+        std::iota(M->order.begin(), M->order.end(), 0);
+    } else if (reorder == CM_REORDER_MORTON) {
+        morton_order(N, xyz, M->order);
+    } else if (reorder == CM_REORDER_RCM) {
+        std::vector<int> rp, cl;
+        build_n2e(N, Ne, hexes, ptr_u, lst_u, 8);
+        build_pattern(N, hexes, ptr_u, lst_u, rp, cl, 8);
+        rcm_order(N, rp, cl, M->order);
+    } else {
+        cm_set_error("cm_mesh_create_hex: unknown reorder %d", (int)reorder);
+        return CM_E_BADARG;
+    }
+    M->identity = true;
+    M->iperm.resize(N);
+    for (long i = 0; i < N; i++) { M->iperm[M->order[i]] = (int)i; if (M->order[i] != i) M->identity = false; }
+    // elements: relabel, keep the local node order, sort by (min new id, user index)
+    std::vector<std::pair<int, int>> key(Ne);
+    for (long e = 0; e < Ne; e++) {
+        int mn = M->iperm[hexes[8 * e]];
+        for (int k = 1; k < 8; k++) mn = std::min(mn, M->iperm[hexes[8 * e + k]]);
+        key[e] = {mn, (int)e};
+    }
+    std::sort(key.begin(), key.end());
+    M->tets.resize(8 * Ne); M->tet_order.resize(Ne); M->mag.resize(Ne); M->eid.resize(Ne); M->emat.resize(Ne);
+    for (long e = 0; e < Ne; e++) {
+        const int old = key[e].second;
+        M->tet_order[e] = old;
+        for (int k = 0; k < 8; k++) M->tets[8 * e + k] = M->iperm[hexes[8 * (long)old + k]];
+        M->mag[e] = mag ? (mag[old] != 0) : 1;
+        M->eid[e] = eid ? eid[old] : 0;
+        if (M->eid[e] < 0 || M->eid[e] > 0x7ffe) { cm_set_error("cm_mesh_create_hex: elastic_id %d outside [0, 32766]", M->eid[e]); return CM_E_INDEX_RANGE; }
+        M->emat[e] = (unsigned short)(M->eid[e] << 1 | (M->mag[e] ? 1 : 0));
+    }
+    M->xyz.resize(3 * N); M->wvol.resize(N);
+    for (long i = 0; i < N; i++) {
+        for (int d = 0; d < 3; d++) M->xyz[3 * i + d] = xyz[3 * (long)M->order[i] + d];
+        M->wvol[i] = w_user[M->order[i]] / vtot;
+    }
+    build_n2e(N, Ne, M->tets.data(), M->n2e_ptr, M->n2e, 8);
+    build_pattern(N, M->tets.data(), M->n2e_ptr, M->n2e, M->rowptr, M->col, 8);
+    M->nnz = M->rowptr[N];
+    if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
+    if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
+    M->ck.nchunks = 0; M->ck.nslots = 0; // no element passes on hexahedra
     return CM_OK;
 }
 
@@ -487,9 +591,26 @@ extern "C" int cm_mesh_create(const double *xyz, long n_nodes, const int *tets, 
     return cm_mesh_create_wrapped(xyz, n_nodes, tets, n_tets, magnetic, elastic_id, nullptr, n_nodes, reorder, stream, out);
 }
 
+static int mesh_create_any(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
+                           const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream, cm_mesh **out,
+                           int nen);
+
 extern "C" int cm_mesh_create_wrapped(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
                                       const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream,
                                       cm_mesh **out)
+{
+    return mesh_create_any(xyz, n_nodes, tets, n_tets, magnetic, elastic_id, dof_of_node, n_dof, reorder, stream, out, 4);
+}
+
+extern "C" int cm_mesh_create_hex(const double *xyz, long n_nodes, const int *hexes, long n_hexes, const unsigned char *magnetic,
+                                  const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out)
+{
+    return mesh_create_any(xyz, n_nodes, hexes, n_hexes, magnetic, elastic_id, nullptr, n_nodes, reorder, stream, out, 8);
+}
+
+static int mesh_create_any(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
+                           const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream, cm_mesh **out,
+                           int nen)
 {
     if (!xyz || !tets || !out || n_nodes <= 0 || n_tets <= 0 || n_nodes > 0x7fffffffL / 4 || n_tets > 0x7fffffffL / 16 || n_dof <= 0 ||
         n_dof > n_nodes || (!dof_of_node && n_dof != n_nodes)) {
@@ -506,7 +627,8 @@ extern "C" int cm_mesh_create_wrapped(const double *xyz, long n_nodes, const int
     if (!M) return CM_E_ALLOC;
     int rc;
     try {
-        rc = mesh_build_host(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, dof_of_node, n_dof, reorder);
+        rc = nen == 8 ? mesh_build_host_hex(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, reorder)
+                      : mesh_build_host(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, dof_of_node, n_dof, reorder);
     } catch (const std::bad_alloc &) {
         cm_set_error("cm_mesh_create: out of host memory");
         rc = CM_E_ALLOC;
