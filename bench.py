@@ -225,6 +225,15 @@ def run_ours(args):
                                "algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak}
     for name in ("spmv", "element", "pointwise"):
         per_class[name] = {"ms": prof[name]["ms"], "launches": prof[name]["launches"]}
+    # assembly (element passes S3, S5, S6, 2 x S8 per step, each followed by its node pass) and the 3 mass products b = M_m f:
+    # SURVEY 8(d) bytes -- per tet 16 B connectivity + 13 words, nodal input and output once
+    Ne = mesh.n_tets
+    elem_step = 5 * Ne * (16 + 13 * s) + N * s * (4 + 4 + 6 + 2 * 12)
+    spmv_step = 3 * ab["spmv_csr3"]
+    for name, byts in (("element", elem_step), ("spmv", spmv_step)):
+        if per_class[name]["ms"] > 0:
+            gbs = byts * args.steps / (per_class[name]["ms"] * 1e-3) / 1e9
+            per_class[name].update({"algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak})
     dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
     # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_c_cg_full.md: config 3, 21 passes per launch);
     # scaled to the average launch of this run, like `achieved`.  Only known for the captured workload.

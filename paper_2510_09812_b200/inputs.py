@@ -302,6 +302,12 @@ def make_config4_mesh(n_side: int, permute: bool = True) -> Mesh:
     return kuhn_box((n_side,) * 3, (L, L, L), seed_mesh=41, seed_perm=42, permute=permute)
 
 
+def make_config4_hex_mesh(n_side: int, permute: bool = True) -> HexMesh:
+    """The same cube as make_config4_mesh meshed with linear hexahedra (the paper's Fig. 2 workload)."""
+    L = (n_side - 1) * 2.5e-9
+    return hex_box((n_side,) * 3, (L,) * 3, seed_mesh=41, seed_perm=42, permute=permute)
+
+
 def clamp_face_x0(mesh: Mesh) -> np.ndarray:
     c = np.zeros((mesh.n_nodes, 3), dtype=np.uint8)
     c[mesh.xyz[:, 0] == 0.0] = 1

@@ -42,7 +42,7 @@ def elem_bytes(N, Ne, s):
             "elem_sigma": tet + N * 12 * s}
 
 
-def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False):
+def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=False):
     import torch
     from . import binding as cm
     peak = peak_gbs()
@@ -62,11 +62,11 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False):
         return float(np.median(ts))
 
     for side in sides:
-        mesh = inputs.make_config4_mesh(side)
+        mesh = inputs.make_config4_hex_mesh(side) if hex_mesh else inputs.make_config4_mesh(side)
         clamp = inputs.clamp_face_x0(mesh)
         mat = inputs.Material()
         for ro in reorders:
-            gm = cm.Mesh(mesh.xyz, mesh.tets, reorder=names[ro])
+            gm = cm.Mesh(mesh.xyz, mesh.hexes if hex_mesh else mesh.tets, reorder=names[ro])
             for dtype in dtypes:
                 gs = cm.System(gm, mat, 1e-12, dtype, clamp, 0)
                 td = torch.float64 if dtype == "f64" else torch.float32
@@ -117,11 +117,11 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False):
                     t, p = kernel_ms(ft, cls, 2)
                     cases.append((name + "_tol1e-8", t, its[-1] * mb[key], its[-1]))
                 eb = elem_bytes(N, gm.n_tets, s)
-                m3 = torch.as_tensor(inputs.init_m_noisy_x(mesh, 44), dtype=td, device="cuda").contiguous()
+                m3 = None if hex_mesh else torch.as_tensor(inputs.init_m_noisy_x(mesh, 44), dtype=td, device="cuda").contiguous()
                 for name, rid, kw in (("elem_rhs_ms", cm.CM_RHS_MS, {}), ("elem_hd", cm.CM_OUT_HD, {"U": b1}),
                                       ("elem_rhs_mech", cm.CM_RHS_MECH, {}), ("elem_sigma", cm.CM_OUT_SIGMA, {"u": b3})):
-                    if only and name not in only and "elem" not in only:
-                        continue
+                    if hex_mesh or (only and name not in only and "elem" not in only):
+                        continue          # (element passes are tetrahedral only)
                     t, p = kernel_ms(lambda: gs.field_rhs(rid, m3, **kw), "element", reps)
                     # kernel_ms divides by launches; a pass is 2-3 launches, so take the class total per call
                     cases.append((name, p["ms"] / reps, eb[name], None))
@@ -151,10 +151,11 @@ def main(argv=None):
     ap.add_argument("--only", default="")
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--json", default="")
+    ap.add_argument("--hex", action="store_true", help="linear hexahedral meshes (27 nnz/row; the paper's Fig. 2 workload) instead of tetrahedra")
     ap.add_argument("--skip-tol", action="store_true", help="skip the CG-to-1e-8 solves (fixed 3 iterations only)")
     a = ap.parse_args(argv)
     rows = run([int(s) for s in a.sides.split(",")], a.dtypes.split(","), a.reorders.split(","),
-               set(a.only.split(",")) if a.only else set(), a.reps, skip_tol=a.skip_tol)
+               set(a.only.split(",")) if a.only else set(), a.reps, skip_tol=a.skip_tol, hex_mesh=a.hex)
     if a.json:
         Path(a.json).write_text(json.dumps(rows, indent=1))
 
