@@ -106,6 +106,11 @@ typedef struct {
 } oracle;
 
 static const double MU0 = 4.0e-7 * 3.14159265358979323846;
+static int hex_rhs_ms(const oracle *o, const real *m, const double *mbar, real *b);
+static int hex_demag_field(const oracle *o, const real *U, const double *mbar, unsigned terms, real *hd, double *gradU_mean);
+static int hex_rhs_mech(const oracle *o, const real *m, real *b);
+static int hex_stress_recover(const oracle *o, const real *u, const real *w, real *sig);
+static double hex_elastic_energy(const oracle *o, const real *m, const real *u);
 
 /* ------------------------------------------------------------------------------------ */
 /* S0: reordering, relabelling, node->element lists, sparsity pattern (R21)              */
@@ -982,7 +987,7 @@ int orc_volume_average(const oracle *o, const void *g_, int ncomp, double *out)
 /* ------------------------------------------------------------------------------------ */
 int orc_rhs_ms(const oracle *o, const void *m_, const double *mbar, void *b_)
 {
-    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
+    if (o->nen == 8) return hex_rhs_ms(o, (const real *)m_, mbar, (real *)b_);
     const real *m = (const real *)m_; real *b = (real *)b_;
     for (long i = 0; i < o->N; i++) b[i] = 0;
     for (long e = 0; e < o->Ne; e++) {
@@ -1002,7 +1007,7 @@ int orc_rhs_ms(const oracle *o, const void *m_, const double *mbar, void *b_)
  * h_d,i = -sum_{e contains i} V_e grad U_e/(4 mL_i) [+ <grad U>] (DEMAG)  - N_d mbar (FARFIELD). */
 int orc_demag_field(const oracle *o, const void *U_, const double *mbar, unsigned terms, void *hd_, double *gradU_mean)
 {
-    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
+    if (o->nen == 8) return hex_demag_field(o, (const real *)U_, mbar, terms, (real *)hd_, gradU_mean);
     const real *U = (const real *)U_; real *hd = (real *)hd_;
     long N = o->N;
     for (long i = 0; i < 3 * N; i++) hd[i] = 0;
@@ -1107,11 +1112,164 @@ static void C_times(const oracle *o, long e, const real eps[6], real sig[6])
     }
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* Element-wise right-hand sides on linear hexahedra (R26): the tetrahedral definitions   */
+/* of O-3 with every element integral taken by the 2 x 2 x 2 Gauss rule:                  */
+/*   b^ms_i     = sum_e sum_p |J_p| grad phi_i(p) . (m_h(p) - mbar),   m_h = sum_a phi_a m_a */
+/*   h_d,i      = -[sum_e sum_p |J_p| phi_i(p) grad U_h(p)] / mL_i + <grad U> - N_d mbar    */
+/*   b^mech_ia  = sum_{e mag} sum_p |J_p| [C_e : E0_h(p)]_ab d_b phi_i(p), E0_h = sum_a phi_a E0(m_a) */
+/*   sigma^_i   = [sum_{e mag} sum_p |J_p| phi_i(p) C_e : (E_h(p) - E0_h(p))] / mLm_i        */
+/* (for a one-point rule on a tetrahedron these are the formulas above them in this file) */
+/* Geometry (|J|, phi, grad phi) is fp64 and rounded once to `real` (R20).                */
+/* ------------------------------------------------------------------------------------ */
+static void hex_coords(const oracle *o, long e, double X[24])
+{
+    const int *t = o->hex + 8 * e;
+    for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)t[a] + d];
+}
+
+static int hex_rhs_ms(const oracle *o, const real *m, const double *mbar, real *b)
+{
+    for (long i = 0; i < o->N; i++) b[i] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        const int *t = o->hex + 8 * e;
+        double X[24]; hex_coords(o, e, X);
+        for (int p = 0; p < 8; p++) {
+            double det, phi[8], g[8][3];
+            hex_gauss_point(X, p, &det, phi, g);
+            real mt[3] = {0, 0, 0};
+            for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) mt[d] += (real)phi[a] * m[3 * (long)t[a] + d];
+            for (int d = 0; d < 3; d++) mt[d] -= (real)mbar[d];
+            for (int a = 0; a < 8; a++)
+                b[t[a]] += (real)det * ((real)g[a][0] * mt[0] + (real)g[a][1] * mt[1] + (real)g[a][2] * mt[2]);
+        }
+    }
+    b[o->pin] = 0;
+    return ORC_OK;
+}
+
+static int hex_demag_field(const oracle *o, const real *U, const double *mbar, unsigned terms, real *hd, double *gradU_mean)
+{
+    long N = o->N;
+    for (long i = 0; i < 3 * N; i++) hd[i] = 0;
+    double gm[3] = {0, 0, 0};
+    if (terms & T_DEMAG) {
+        double acc[3] = {0, 0, 0};
+        for (long e = 0; e < o->Ne; e++) {
+            const int *t = o->hex + 8 * e;
+            double X[24]; hex_coords(o, e, X);
+            for (int p = 0; p < 8; p++) {
+                double det, phi[8], g[8][3];
+                hex_gauss_point(X, p, &det, phi, g);
+                real gU[3] = {0, 0, 0};
+                for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) gU[d] += U[t[a]] * (real)g[a][d];
+                for (int d = 0; d < 3; d++) acc[d] += det * (double)gU[d];
+                for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) hd[3 * (long)t[a] + d] += (real)det * (real)phi[a] * gU[d];
+            }
+        }
+        for (int d = 0; d < 3; d++) gm[d] = acc[d] / o->Vtot;
+        for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++) hd[3 * i + d] = -hd[3 * i + d] / o->mL[i] + (real)gm[d];
+    }
+    if (terms & T_FARFIELD)
+        for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++)
+            hd[3 * i + d] -= (real)(o->Nd[3 * d] * mbar[0] + o->Nd[3 * d + 1] * mbar[1] + o->Nd[3 * d + 2] * mbar[2]);
+    if (gradU_mean) for (int d = 0; d < 3; d++) gradU_mean[d] = gm[d];
+    return ORC_OK;
+}
+
+/* E0_h(p) = sum_a phi_a(p) E0(w_a) and, if u != NULL, eps = E_h(p)(u) - E0_h(p); else eps = E0_h(p) */
+static void hex_point_strain(const oracle *o, const int *t, const double phi[8], double g[8][3], const real *u, const real *w, real eps[6])
+{
+    real e0[6] = {0, 0, 0, 0, 0, 0};
+    for (int a = 0; a < 8; a++) {
+        real ek[6]; E0_voigt(o, w + 3 * (long)t[a], ek);
+        for (int q = 0; q < 6; q++) e0[q] += (real)phi[a] * ek[q];
+    }
+    if (!u) { for (int q = 0; q < 6; q++) eps[q] = e0[q]; return; }
+    real H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}; /* H[a][b] = d_b u_a */
+    for (int k = 0; k < 8; k++) for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) H[a][b] += u[3 * (long)t[k] + a] * (real)g[k][b];
+    eps[0] = H[0][0] - e0[0]; eps[1] = H[1][1] - e0[1]; eps[2] = H[2][2] - e0[2];
+    eps[3] = H[1][2] + H[2][1] - e0[3]; eps[4] = H[0][2] + H[2][0] - e0[4]; eps[5] = H[0][1] + H[1][0] - e0[5];
+}
+
+static int hex_rhs_mech(const oracle *o, const real *m, real *b)
+{
+    for (long i = 0; i < 3 * o->N; i++) b[i] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        if (!o->mag[e]) continue;
+        const int *t = o->hex + 8 * e;
+        double X[24]; hex_coords(o, e, X);
+        for (int p = 0; p < 8; p++) {
+            double det, phi[8], g[8][3];
+            hex_gauss_point(X, p, &det, phi, g);
+            real e0[6], s[6];
+            hex_point_strain(o, t, phi, g, NULL, m, e0);
+            C_times(o, e, e0, s);
+            for (int a = 0; a < 8; a++) {
+                real gx = (real)g[a][0], gy = (real)g[a][1], gz = (real)g[a][2], w = (real)det;
+                b[3 * (long)t[a] + 0] += w * (s[0] * gx + s[5] * gy + s[4] * gz);
+                b[3 * (long)t[a] + 1] += w * (s[5] * gx + s[1] * gy + s[3] * gz);
+                b[3 * (long)t[a] + 2] += w * (s[4] * gx + s[3] * gy + s[2] * gz);
+            }
+        }
+    }
+    for (long i = 0; i < 3 * o->N; i++) if (o->clamp[i]) b[i] = 0;
+    return ORC_OK;
+}
+
+static int hex_stress_recover(const oracle *o, const real *u, const real *w, real *sig)
+{
+    for (long i = 0; i < 6 * o->N; i++) sig[i] = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        if (!o->mag[e]) continue;
+        const int *t = o->hex + 8 * e;
+        double X[24]; hex_coords(o, e, X);
+        for (int p = 0; p < 8; p++) {
+            double det, phi[8], g[8][3];
+            hex_gauss_point(X, p, &det, phi, g);
+            real eps[6], s[6];
+            hex_point_strain(o, t, phi, g, u, w, eps);
+            C_times(o, e, eps, s);
+            for (int a = 0; a < 8; a++) for (int q = 0; q < 6; q++) sig[6 * (long)t[a] + q] += (real)det * (real)phi[a] * s[q];
+        }
+    }
+    for (long i = 0; i < o->N; i++)
+        for (int q = 0; q < 6; q++) sig[6 * i + q] = o->live[i] ? sig[6 * i + q] / o->mLm[i] : (real)0;
+    return ORC_OK;
+}
+
+static double hex_elastic_energy(const oracle *o, const real *m, const real *u)
+{
+    double E = 0;
+    for (long e = 0; e < o->Ne; e++) {
+        const int *t = o->hex + 8 * e;
+        double X[24]; hex_coords(o, e, X);
+        for (int p = 0; p < 8; p++) {
+            double det, phi[8], g[8][3];
+            hex_gauss_point(X, p, &det, phi, g);
+            real eps[6], s[6];
+            if (o->mag[e]) hex_point_strain(o, t, phi, g, u, m, eps);
+            else {
+                real zero[24] = {0};
+                (void)zero;
+                real H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+                for (int k = 0; k < 8; k++) for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) H[a][b] += u[3 * (long)t[k] + a] * (real)g[k][b];
+                eps[0] = H[0][0]; eps[1] = H[1][1]; eps[2] = H[2][2];
+                eps[3] = H[1][2] + H[2][1]; eps[4] = H[0][2] + H[2][0]; eps[5] = H[0][1] + H[1][0];
+            }
+            C_times(o, e, eps, s);
+            double w = 0; for (int q = 0; q < 6; q++) w += (double)eps[q] * (double)s[q];
+            E += 0.5 * det * w;
+        }
+    }
+    return E;
+}
+
 /* S6 mechanical RHS (Eq. 10, 13, 14):
  * b_(i,a) = sum_{e contains i, magnetic} V_e [C*_e : mean_e E0(m)]_ab d_b phi_i; clamped DOFs zeroed. */
 int orc_rhs_mech(const oracle *o, const void *m_, void *b_)
 {
-    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
+    if (o->nen == 8) return hex_rhs_mech(o, (const real *)m_, (real *)b_);
     const real *m = (const real *)m_; real *b = (real *)b_;
     if (!o->n_elastic) return ORC_E_BADARG;
     for (long i = 0; i < 3 * o->N; i++) b[i] = 0;
@@ -1150,7 +1308,7 @@ static void elem_strain(const oracle *o, long e, const real *u, real eps[6])
  * sigma_hat_i = sum_{e contains i, magnetic} V_e sigma_e/(4 mLm_i).  Output N x 6 Voigt. */
 int orc_stress_recover(const oracle *o, const void *u_, const void *w_, void *sig_)
 {
-    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
+    if (o->nen == 8) return hex_stress_recover(o, (const real *)u_, (const real *)w_, (real *)sig_);
     const real *u = (const real *)u_, *w = (const real *)w_; real *sg = (real *)sig_;
     if (!o->n_elastic) return ORC_E_BADARG;
     for (long i = 0; i < 6 * o->N; i++) sg[i] = 0;
@@ -1213,7 +1371,7 @@ double orc_energy(const oracle *o, const void *m_, const void *U_, const void *u
     const real *m = (const real *)m_, *U = (const real *)U_, *u = (const real *)u_;
     long N = o->N;
     double E = 0;
-    if (o->nen == 8) return NAN; /* tetrahedral only (R26) */
+
     real *y = (real *)malloc((size_t)3 * N * sizeof(real));
     for (int c = 0; c < 3; c++) { /* exchange 1/2 A* m_a^T K_m m_a */
         spmv(o, MAT_K_M, m, y, 3, c);
@@ -1231,7 +1389,8 @@ double orc_energy(const oracle *o, const void *m_, const void *U_, const void *u
     if (terms & T_DEMAG) { spmv(o, MAT_K_FREE, U, y, 1, 0); E += 0.5 * dot(N, U, y, 1, 0); }
     if (terms & T_FARFIELD)
         for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) E += 0.5 * o->Vtot * mbar[a] * o->Nd[3 * a + b] * mbar[b];
-    if ((terms & T_MAGEL) && o->n_elastic)
+    if ((terms & T_MAGEL) && o->n_elastic && o->nen == 8) E += hex_elastic_energy(o, m, u);
+    else if ((terms & T_MAGEL) && o->n_elastic)
         for (long e = 0; e < o->Ne; e++) {
             real eps[6], e0[6], s[6];
             elem_strain(o, e, u, eps);
@@ -1258,7 +1417,6 @@ static int helmholtz(const oracle *o, int id, const real *f, real *g, int a, con
 
 int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_, void *u_, orc_step_info *info)
 {
-    if (o->nen == 8) return ORC_E_BADARG; /* element-wise right-hand sides are tetrahedral only (R26) */
     real *m = (real *)m_, *U = (real *)U_, *u = (real *)u_;
     long N = o->N; unsigned terms = p->terms;
     int worst = ORC_OK, rc;

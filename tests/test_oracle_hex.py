@@ -146,13 +146,109 @@ def test_volume_average_and_cg(orc, jit):
         assert np.abs(xs - np.linalg.solve(o.csr(mat).toarray(), b)).max() <= 1e-9 * np.abs(xs).max()
 
 
-def test_tet_only_entry_points_refuse_hexahedra(orc, jit):
+def test_hex_rhs_identities(orc, jit):
+    """The tetrahedral pins of S3 / S5 / S6 / S8 carry over: uniform m gives b^ms = 0 and h_d = -N_d mbar; sum_i b_i = 0; the
+    recovered gradient of a linear potential is exact; u = E0 x is stress free on a homogeneous body."""
     mesh, o, clamp = jit
-    m = np.zeros((o.N, 3)); m[:, 0] = 1
-    with pytest.raises(AssertionError):
-        o.rhs_mech(m)
-    info, rc = o.gspm_step(m, np.zeros(o.N), np.zeros((o.N, 3)), 1e-12, [0, 0, 0], 0)
-    assert rc == -1
-    bad = inputs.replace(mesh, hexes=mesh.hexes[:, [1, 0, 2, 3, 4, 5, 6, 7]].copy())     # inverted cell
+    from paper_2510_09812_b200.inputs import TERM_DEMAG, TERM_FARFIELD, TERM_MAGEL
+    mu = np.tile([0.6, 0.0, 0.8], (o.N, 1))
+    mbar = o.volume_average(mu)
+    assert np.allclose(mbar, [0.6, 0.0, 0.8], rtol=1e-14)
+    assert np.abs(o.rhs_ms(mu)).max() < 1e-12
+    hd, gm = o.demag_field(np.zeros(o.N), mbar, TERM_DEMAG | TERM_FARFIELD)
+    assert np.allclose(hd, -mbar / 3, rtol=1e-13)
+    rng = np.random.default_rng(3)
+    m = rng.normal(size=(o.N, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True)
+    b = o.rhs_ms(m)
+    o3 = orc.Oracle(mesh, mat2(), 1e-12, clamp_dof=clamp, pin_node=3)          # same body, other pin: gives the entry zeroed above
+    b_full = b.copy(); b_full[2] = o3.rhs_ms(m)[2]
+    assert b[2] == 0 and abs(b_full.sum()) < 1e-12 * np.abs(b_full).sum()      # sum_i grad phi_i = 0 pointwise
+    x = mesh.xyz / NM
+    a = np.array([0.3, -0.2, 0.5])
+    hd, gm = o.demag_field(x @ a, np.zeros(3), TERM_DEMAG)
+    assert np.allclose(gm, a, rtol=1e-13) and np.abs(hd).max() < 1e-12       # -grad U + <grad U> = 0 for linear U
+    hd, gm = o.demag_field(x[:, 0] ** 2, np.zeros(3), TERM_DEMAG)
+    assert np.abs(hd[:, 1:]).max() < 0.3 and np.abs(hd[:, 0]).max() > 1   # quadratic U: x-gradient only
+    # stress-free state on a homogeneous, unclamped body
+    mesh1 = inputs.hex_box((5, 5, 4), (10 * NM, 12 * NM, 9 * NM), seed_mesh=5, seed_perm=6)
+    mat = inputs.Material()
+    o1 = orc.Oracle(mesh1, mat, 1e-12)
+    mdir = np.array([0.6, -0.48, 0.64])
+    m1 = np.tile(mdir, (o1.N, 1))
+    l1, l2 = mat.lambda100, mat.lambda111
+    E0 = 1.5 * l2 * np.outer(mdir, mdir); E0[np.arange(3), np.arange(3)] = 1.5 * l1 * (mdir ** 2 - 1 / 3)
+    u = (mesh1.xyz / NM) @ E0.T
+    bm = o1.rhs_mech(m1)
+    Ku = (o1.csr(orc.MAT_K_MECH_FREE) @ u.ravel()).reshape(-1, 3)
+    assert np.abs(bm).max() > 1e-3 and np.abs(Ku - bm).max() < 1e-12 * np.abs(bm).max()
+    sig = o1.stress_recover(u, m1)
+    Cs = mat.C_voigt[0] / (MU0 * mat.Ms ** 2)
+    e0v = np.array([E0[0, 0], E0[1, 1], E0[2, 2], 2 * E0[1, 2], 2 * E0[0, 2], 2 * E0[0, 1]])
+    assert np.abs(sig).max() < 1e-12 * np.abs(Cs @ e0v).max()
+    assert np.abs(o1.field(m1, None, sig, [0, 0, 0], TERM_MAGEL)).max() < 1e-13
+    assert np.allclose(o1.stress_recover(np.zeros_like(u), m1), np.tile(-(Cs @ e0v), (o1.N, 1)), rtol=1e-12, atol=1e-16)
+
+
+def _fd_field(energy, m, nodes, mass, h):
+    out = np.zeros((len(nodes), 3))
+    for a, i in enumerate(nodes):
+        for c in range(3):
+            mp = m.copy(); mp[i, c] += h
+            mm = m.copy(); mm[i, c] -= h
+            out[a, c] = -(energy(mp) - energy(mm)) / (2 * h) / mass[i]
+    return out
+
+
+def test_hex_fields_are_energy_gradients(orc, jit):
+    """h_me = -(1/mLm_i) dE_el/dm_i at fixed u, and h_d = -(1/mLm_i) d/dm_i [1/2 U^T K U + far field] with U re-solved
+    (central differences of the hexahedral discrete energy)."""
+    mesh, o, clamp = jit
+    from paper_2510_09812_b200.inputs import TERM_DEMAG, TERM_FARFIELD, TERM_MAGEL
+    rng = np.random.default_rng(4)
+    live = np.flatnonzero(o.live())
+    m = rng.normal(size=(o.N, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True); m[o.live() == 0] = 0
+    u = 1e-3 * rng.normal(size=(o.N, 3))
+    nodes = rng.choice(live, 4, replace=False)
+    sig = o.stress_recover(u, m)
+    h = o.field(m, None, sig, [0, 0, 0], TERM_MAGEL)
+    fd = _fd_field(lambda mm: o.energy(mm, None, u, [0, 0, 0], TERM_MAGEL) - o.energy(mm, None, u, [0, 0, 0], 0), m, nodes, o.mLm(), 1e-4)
+    assert np.abs(h[nodes]).max() > 1e-4 and np.allclose(h[nodes], fd, rtol=2e-6, atol=2e-8)
+    assert np.abs(sig[o.live() == 0]).max() == 0
+
+    def demag_energy(mm):
+        b = o.rhs_ms(mm)
+        U = o.cg(orc.MAT_K_MS, b, tol=1e-13)[0]
+        return o.energy(mm, U, None, [0, 0, 0], TERM_DEMAG | TERM_FARFIELD) - o.energy(mm, U, None, [0, 0, 0], 0)
+    U = o.cg(orc.MAT_K_MS, o.rhs_ms(m), tol=1e-13)[0]
+    hd, _ = o.demag_field(U, o.volume_average(m), TERM_DEMAG | TERM_FARFIELD)
+    interior_live = [i for i in live if o.mL()[i] == pytest.approx(o.mLm()[i], rel=1e-12)][:3]
+    fd = _fd_field(demag_energy, m, interior_live, o.mL(), 1e-4)
+    assert np.allclose(hd[interior_live], fd, rtol=1e-5, atol=1e-7)
+
+
+def test_hex_gspm_step_invariants(orc):
+    """|m| = 1 after every step, dead nodes stay zero, the discrete energy decays (config-0 physics on a hexahedral mesh),
+    and uniform m along an easy axis with the field along it is a fixed point."""
+    from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD, TERM_ZEEMAN
+    mesh = inputs.hex_box((8, 8, 8), (20 * NM,) * 3, seed_mesh=1, seed_perm=2)
+    o = orc.Oracle(mesh, inputs.Material(), 1e-12)
+    terms = TERM_ANIS | TERM_DEMAG | TERM_FARFIELD
+    m = np.tile([0.0, 0.0, 1.0], (o.N, 1)); U = np.zeros(o.N); u = np.zeros((o.N, 3))
+    info, rc = o.gspm_step(m, U, u, 1e-12, [0, 0, 5e4], TERM_ANIS | TERM_ZEEMAN | TERM_FARFIELD, cg_tol=1e-12)
+    assert rc == 0 and np.abs(m - [0, 0, 1]).max() < 1e-14
+    rng = np.random.default_rng(3)
+    m = rng.normal(size=(o.N, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True)
+    E = [o.energy(m, U, u, np.zeros(3), terms)]
+    for _ in range(8):
+        info, rc = o.gspm_step(m, U, u, 1e-12, [0, 0, 0], terms, cg_tol=1e-12)
+        assert rc == 0 and info.it_ms > 5
+        assert np.abs(np.linalg.norm(m, axis=1) - 1).max() <= 4 * np.finfo(float).eps
+        E.append(o.energy(m, U, u, np.zeros(3), terms))
+    assert all(b < a for a, b in zip(E, E[1:])), E
+
+
+def test_hex_degenerate_cell_rejected(orc, jit):
+    mesh, o, clamp = jit
+    bad = inputs.replace(mesh, hexes=mesh.hexes[:, [1, 0, 2, 3, 4, 5, 6, 7]].copy())     # inverted cells
     with pytest.raises(RuntimeError, match="rc=-2"):
         orc.Oracle(bad, mat2(), 1e-12)
