@@ -148,12 +148,12 @@ int cm_mesh_create_wrapped(const double *xyz, long n_nodes, const int *tets, lon
                            cm_mesh **out);
 /* Linear hexahedral (Q1) meshes (R26): the paper's structured Fig. 2-3
  * workloads.  hexes: host, n_hexes x 8, local node a = i + 2 j + 4 k at corner (i, j, k) of the cell; trilinear shape
- * functions, 2 x 2 x 2 Gauss quadrature.  A hexahedral mesh supports the MATRICES of Eq. 12 and what acts on them --
- * cm_assemble_csr, cm_system_get_values, cm_spmv, cm_spmv3, cm_cg_solve, cm_cg_solve3 (the paper's CG benchmark,
- * Fig. 2b-d) -- and cm_volume_average (Eq. 17); the element-wise right-hand sides and the GSPM step (cm_field_rhs,
- * cm_gspm_step*, cm_hysteresis_run) are tetrahedral only and return CM_E_BADARG.  cm_mesh_get: CM_GET_TETS has 8 ids per
- * element, CM_GET_N2E entries are element*8 + local index.  Errors as cm_mesh_create (DEGENERATE_TET: det J <= 0 at a
- * Gauss point, i.e. an inverted or collapsed cell). */
+ * functions; every element integral (matrices, right-hand sides, recovered fields, lumped masses, Eq. 17) by the
+ * 2 x 2 x 2 Gauss rule.  Every call of this header works on a hexahedral mesh (cm_assemble_csr, cm_spmv, cm_cg_solve*,
+ * cm_field_rhs, cm_gspm_step*, cm_hysteresis_run, cm_volume_average) except cm_system_get_geometry(what = 0, 1), whose
+ * per-element V_e / grad phi are stored for tetrahedra only (CM_E_BADARG), and periodic wrapping.  cm_mesh_get:
+ * CM_GET_TETS has 8 ids per element, CM_GET_N2E entries are element*8 + local index.  Errors as cm_mesh_create
+ * (DEGENERATE_TET: det J <= 0 at a Gauss point, i.e. an inverted or collapsed cell). */
 int cm_mesh_create_hex(const double *xyz, long n_nodes, const int *hexes, long n_hexes, const unsigned char *magnetic,
                        const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out);
 int cm_mesh_destroy(cm_mesh *mesh);

@@ -63,13 +63,6 @@ static int check_sys(const cm_system *sys, const char *fn)
     return CM_OK;
 }
 
-// element-wise right-hand sides and the GSPM step exist for linear tetrahedra only (R26)
-static int tet_only(const cm_system *sys, const char *fn)
-{
-    if (sys->impl->mesh->nen != 4) { cm_set_error("%s: not available on hexahedral meshes (matrices, SpMV / CG and volume averages only)", fn); return CM_E_BADARG; }
-    return CM_OK;
-}
-
 static int mode_of(cm_matrix_id id) { return id == CM_MAT_K_MECH ? MODE_BSR3 : MODE_CSR1; }
 
 // ---------------------------------------------------------------- assemble / destroy / getters
@@ -301,7 +294,6 @@ extern "C" int cm_field_rhs(cm_system *sys, cm_rhs_id id, const void *m_dev, con
                             const cm_step_params *params, double coeff, void *b_dev, void *stream)
 {
     CM_TRY(check_sys(sys, "cm_field_rhs"));
-    CM_TRY(tet_only(sys, "cm_field_rhs"));
     if (!m_dev || !b_dev) { cm_set_error("cm_field_rhs: null m_dev / b_dev"); return CM_E_BADARG; }
     if ((id == CM_RHS_GS || id == CM_OUT_FIELD) && !params) { cm_set_error("cm_field_rhs: params required"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
@@ -326,7 +318,6 @@ extern "C" int cm_gspm_step(cm_system *sys, const cm_step_params *params, void *
                             void *stream)
 {
     CM_TRY(check_sys(sys, "cm_gspm_step"));
-    CM_TRY(tet_only(sys, "cm_gspm_step"));
     if (!params) { cm_set_error("cm_gspm_step: null params"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
     return SYS_DISPATCH(sys, sys_step<double>(S, params, (double *)m_dev, (double *)U_dev, (double *)u_dev, info, st),
@@ -356,7 +347,6 @@ extern "C" int cm_gspm_step_host(cm_system *sys, const cm_step_params *params, v
                                  cm_step_info *info, void *stream)
 {
     CM_TRY(check_sys(sys, "cm_gspm_step_host"));
-    CM_TRY(tet_only(sys, "cm_gspm_step_host"));
     if (!params) { cm_set_error("cm_gspm_step_host: null params"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
     return SYS_DISPATCH(sys, api_step_host<double>(S, params, m_host, U_host, u_host, info, st),
@@ -368,7 +358,6 @@ extern "C" int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, con
                                  void *u_dev, double *H_log, double *mbar_log, int *steps_log, cm_hyst_result *result, void *stream)
 {
     CM_TRY(check_sys(sys, "cm_hysteresis_run"));
-    CM_TRY(tet_only(sys, "cm_hysteresis_run"));
     if (!base || !hp) { cm_set_error("cm_hysteresis_run: null params"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
     return SYS_DISPATCH(sys, sys_hysteresis<double>(S, base, hp, (double *)m_dev, (double *)U_dev, (double *)u_dev, H_log, mbar_log, steps_log, result, st),

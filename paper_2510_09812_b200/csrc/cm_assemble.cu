@@ -163,34 +163,6 @@ __global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const
 
 // ---- linear hexahedra (R26): one thread per row i accumulates, over the incident elements in ascending order and the
 // 2 x 2 x 2 Gauss points in order, row i of K, K_m, M_m, K^mech and the lumped masses int phi_i.
-__device__ __forceinline__ double hex_point(const double X[8][3], int p, double phi[8], double g[8][3])
-{
-    const double q = 0.57735026918962576451;
-    const double xi[3] = {(p & 1) ? q : -q, (p & 2) ? q : -q, (p & 4) ? q : -q};
-    double dN[8][3], J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
-#pragma unroll
-    for (int a = 0; a < 8; a++) {
-        const double s[3] = {(a & 1) ? 1.0 : -1.0, (a & 2) ? 1.0 : -1.0, (a & 4) ? 1.0 : -1.0};
-        const double f[3] = {1 + s[0] * xi[0], 1 + s[1] * xi[1], 1 + s[2] * xi[2]};
-        phi[a] = f[0] * f[1] * f[2] / 8;
-        dN[a][0] = s[0] * f[1] * f[2] / 8; dN[a][1] = f[0] * s[1] * f[2] / 8; dN[a][2] = f[0] * f[1] * s[2] / 8;
-#pragma unroll
-        for (int r = 0; r < 3; r++)
-#pragma unroll
-            for (int c = 0; c < 3; c++) J[r][c] += X[a][r] * dN[a][c];
-    }
-    double cof[3][3];
-    cof[0][0] = J[1][1] * J[2][2] - J[1][2] * J[2][1]; cof[0][1] = J[1][2] * J[2][0] - J[1][0] * J[2][2]; cof[0][2] = J[1][0] * J[2][1] - J[1][1] * J[2][0];
-    cof[1][0] = J[0][2] * J[2][1] - J[0][1] * J[2][2]; cof[1][1] = J[0][0] * J[2][2] - J[0][2] * J[2][0]; cof[1][2] = J[0][1] * J[2][0] - J[0][0] * J[2][1];
-    cof[2][0] = J[0][1] * J[1][2] - J[0][2] * J[1][1]; cof[2][1] = J[0][2] * J[1][0] - J[0][0] * J[1][2]; cof[2][2] = J[0][0] * J[1][1] - J[0][1] * J[1][0];
-    const double det = J[0][0] * cof[0][0] + J[0][1] * cof[0][1] + J[0][2] * cof[0][2];
-#pragma unroll
-    for (int a = 0; a < 8; a++)
-#pragma unroll
-        for (int r = 0; r < 3; r++) g[a][r] = (cof[r][0] * dN[a][0] + cof[r][1] * dN[a][1] + cof[r][2] * dN[a][2]) / det;
-    return det;
-}
-
 template <typename T>
 __global__ void hex_rows_kernel(long N, const int *__restrict__ hexes, const double *__restrict__ xyz, double ld,
                                 const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const uchar *__restrict__ mag,
@@ -313,6 +285,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     const double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
     // O-0 nondimensionalisation
     S->Ms = mat->Ms;
+    S->ld = ld;
     S->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
     S->Kstar = mat->K1 / mu0Ms2;
     S->dtau = mat->gamma * mat->Ms * S->dt;
@@ -473,7 +446,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     S->grid_cap = S->num_sms * 8;
     CM_TRY(alloc(&S->partial, (size_t)4 * S->grid_cap * 3));
     CM_TRY(alloc(&S->d_res, 8));
-    CM_TRY(alloc(&S->red, std::max<size_t>((size_t)4096 * 16, (size_t)8 * M->ck.nchunks)));
+    CM_TRY(alloc(&S->red, std::max<size_t>({(size_t)4096 * 16, (size_t)8 * M->ck.nchunks, (size_t)3 * ((N + 127) / 128) + 64})));
     CM_TRY(alloc(&S->dscal, 32));
     CM_CUDA(cudaMallocHost((void **)&S->h_res, 8 * sizeof(CgResult)));
     CM_CUDA(cudaMallocHost((void **)&S->h_scal, 32 * sizeof(double)));

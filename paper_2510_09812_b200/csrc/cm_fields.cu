@@ -124,6 +124,10 @@ constexpr int EK_NT = CM_EK_NT;
 template <typename T>
 struct ChunkArgs {
     const int *eptr, *nptr, *nodes;
+    const int *hexes, *n2e_ptr, *n2e; // hexahedral meshes (node-centric passes): connectivity, node -> (element * 8 + corner)
+    const double *xyz;                // library-order coordinates, metres
+    double ld;
+    long N;
     const unsigned short *lid, *lptr, *lent, *emat;
     const T *EG;          // chunk-blocked geometry, 10 planes per chunk (cm_internal.h)
     const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w
@@ -457,7 +461,7 @@ template <typename T>
 __global__ void node_hd_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                const T *__restrict__ mL, const double *__restrict__ scal /* mbar[0..2], gradU mean[3..5] */,
                                unsigned terms, double n00, double n01, double n02, double n10, double n11,
-                               double n12, double n20, double n21, double n22, T *hd)
+                               double n12, double n20, double n21, double n22, T dscale /* 4: tets (V_e / 4 weights), 1: hexahedra */, T *hd)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -469,7 +473,7 @@ __global__ void node_hd_kernel(long N, const int *__restrict__ ns_ptr, const int
 #pragma unroll
             for (int d = 0; d < 3; d++) acc[d] += hpart[3 * q + d];
         }
-        const T den = (T)4 * mL[i];
+        const T den = dscale * mL[i];
 #pragma unroll
         for (int d = 0; d < 3; d++) h[d] = -acc[d] / den + (T)scal[3 + d];
     }
@@ -489,7 +493,7 @@ template <typename T>
 __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                   const T *__restrict__ mLm, const uchar *__restrict__ live, const T *__restrict__ w,
                                   const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, const double *__restrict__ hext_dev,
-                                  T l1, T l2, Rot<T> rot, T *h, T *sig_out)
+                                  T l1, T l2, Rot<T> rot, T dscale, T *h, T *sig_out)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -511,7 +515,7 @@ __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const 
 #pragma unroll
                 for (int c = 0; c < 6; c++) s[c] += hpart[6 * sl + c];
             }
-            const T den = (T)4 * mLm[i];
+            const T den = dscale * mLm[i];
 #pragma unroll
             for (int c = 0; c < 6; c++) s[c] /= den;
             T sc[6] = {s[0], s[1], s[2], s[3], s[4], s[5]};
@@ -656,6 +660,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     ChunkArgs<T> a;
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
     a.emat = M->d_emat; a.EG = S->EG;
+    a.hexes = M->d_tets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_xyz; a.ld = S->ld; a.N = S->N;
     a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
     a.hpart = S->hpart; a.partial = S->red;
@@ -680,6 +685,109 @@ static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
     return CM_OK;
 }
 
+// ---------------------------------------------------------------- element passes on linear hexahedra (R26)
+// Node-centric: one thread per node i walks its incident cells (ascending) and their 2 x 2 x 2 Gauss points (ascending),
+// recomputes the fp64 geometry from the corner coordinates and accumulates node i's own entry -- a deterministic gather
+// with no scatter at all.  The numerators land in hpart[slot = node]; the tetrahedral node passes finish them
+// (dscale = 1).  Hexahedral cells carry ~8x the arithmetic of a tetrahedron per byte, so these passes are bound by
+// fp64 throughput, not by HBM; they are < 1 % of a step.
+template <typename T, int KIND>
+__global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
+{
+    typedef KindTraits<KIND> K;
+    constexpr int NC = K::NC;
+    const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    T acc[NC];
+#pragma unroll
+    for (int q = 0; q < NC; q++) acc[q] = 0;
+    if (i < a.N) {
+        for (int s = a.n2e_ptr[i]; s < a.n2e_ptr[i + 1]; s++) {
+            const int e = a.n2e[s] >> 3, k = a.n2e[s] & 7;
+            const unsigned em = a.emat[e];
+            if ((KIND == EK_MECH || KIND == EK_STRESS) && !(em & 1u)) continue;
+            int t[8];
+            double X[8][3];
+#pragma unroll
+            for (int c = 0; c < 8; c++) {
+                t[c] = a.hexes[8 * (long)e + c];
+#pragma unroll
+                for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * (long)t[c] + d] / a.ld;
+            }
+            T e0c[8][6]; // E0 at the 8 corners (MECH, STRESS)
+            if (KIND == EK_MECH || KIND == EK_STRESS) {
+                const T *w = KIND == EK_MECH ? a.in0 : a.in1;
+                for (int c = 0; c < 8; c++) {
+                    const T mk[3] = {w[3 * (long)t[c]], w[3 * (long)t[c] + 1], w[3 * (long)t[c] + 2]};
+                    E0_sim(a.rot, mk, a.l1, a.l2, e0c[c]);
+                }
+            }
+            for (int p = 0; p < 8; p++) {
+                double phid[8], gd[8][3];
+                const T det = (T)hex_point(X, p, phid, gd);
+                if (KIND == EK_MS) {
+                    T mt[3] = {0, 0, 0};
+                    for (int c = 0; c < 8; c++)
+#pragma unroll
+                        for (int d = 0; d < 3; d++) mt[d] += (T)phid[c] * a.in0[3 * (long)t[c] + d];
+#pragma unroll
+                    for (int d = 0; d < 3; d++) mt[d] -= (T)a.mbar[d];
+                    acc[0] += det * ((T)gd[k][0] * mt[0] + (T)gd[k][1] * mt[1] + (T)gd[k][2] * mt[2]);
+                } else if (KIND == EK_GRADU) {
+                    T gU[3] = {0, 0, 0};
+                    for (int c = 0; c < 8; c++)
+#pragma unroll
+                        for (int d = 0; d < 3; d++) gU[d] += a.in0[t[c]] * (T)gd[c][d];
+#pragma unroll
+                    for (int d = 0; d < 3; d++) acc[d] += det * (T)phid[k] * gU[d];
+                } else {
+                    T eps[6] = {0, 0, 0, 0, 0, 0}, sg[6];
+                    for (int c = 0; c < 8; c++)
+#pragma unroll
+                        for (int q = 0; q < 6; q++) eps[q] += (T)phid[c] * e0c[c][q];
+                    if (KIND == EK_STRESS) {
+                        T H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+                        for (int c = 0; c < 8; c++)
+#pragma unroll
+                            for (int x = 0; x < 3; x++)
+#pragma unroll
+                                for (int y = 0; y < 3; y++) H[x][y] += a.in0[3 * (long)t[c] + x] * (T)gd[c][y];
+                        const T E[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]};
+#pragma unroll
+                        for (int q = 0; q < 6; q++) eps[q] = E[q] - eps[q];
+                    }
+                    C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+                    if (KIND == EK_MECH) {
+                        const T gx = (T)gd[k][0], gy = (T)gd[k][1], gz = (T)gd[k][2];
+                        acc[0] += det * (sg[0] * gx + sg[5] * gy + sg[4] * gz);
+                        acc[1] += det * (sg[5] * gx + sg[1] * gy + sg[3] * gz);
+                        acc[NC > 2 ? 2 : 0] += det * (sg[4] * gx + sg[3] * gy + sg[2] * gz);
+                    } else {
+#pragma unroll
+                        for (int q = 0; q < NC; q++) acc[q] += det * (T)phid[k] * sg[q < 6 ? q : 0];
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NC; q++) a.hpart[i * NC + q] = acc[q];
+    }
+    if (KIND == EK_GRADU) { // sum_i int phi_i grad U_h = int grad U_h (the shape functions sum to one): <grad U> V
+        double gs[3] = {0, 0, 0};
+        if (i < a.N)
+            for (int d = 0; d < 3; d++) gs[d] = (double)acc[d < NC ? d : 0];
+        block_reduce_write<3>(gs, a.partial);
+    }
+}
+
+template <typename T, int KIND>
+static int launch_hex(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st, int *grid_out = nullptr)
+{
+    const int B = 128, grid = (int)((S->N + B - 1) / B);
+    hex_node_kernel<T, KIND><<<grid, B, 0, st>>>(a);
+    if (grid_out) *grid_out = grid;
+    return CM_OK;
+}
+
 template <typename T>
 int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
 {
@@ -687,7 +795,8 @@ int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
     ChunkArgs<T> a = chunk_args(S);
     a.in0 = m_lib;
     S->prof.begin(CM_PROF_ELEMENT, st, 2);
-    CM_TRY((launch_chunks<T, EK_MS>(S, a, st)));
+    if (S->mesh->nen == 8) CM_TRY((launch_hex<T, EK_MS>(S, a, st)));
+    else CM_TRY((launch_chunks<T, EK_MS>(S, a, st)));
     node_gather_kernel<T, 1><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, nullptr, S->pin, b);
     S->prof.end(st);
     LAUNCH_CHECK();
@@ -702,12 +811,14 @@ int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStr
     if (terms & CM_TERM_DEMAG) {
         ChunkArgs<T> a = chunk_args(S);
         a.in0 = U_lib;
-        CM_TRY((launch_chunks<T, EK_GRADU>(S, a, st)));
-        reduce_final_kernel<<<1, 1024, 0, st>>>(K.nchunks, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
+        int nparts = K.nchunks;
+        if (S->mesh->nen == 8) CM_TRY((launch_hex<T, EK_GRADU>(S, a, st, &nparts)));
+        else CM_TRY((launch_chunks<T, EK_GRADU>(S, a, st)));
+        reduce_final_kernel<<<1, 1024, 0, st>>>(nparts, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
     }
     const double *n = S->Nd;
     node_hd_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mL, S->dscal, terms, n[0], n[1], n[2], n[3],
-                                                 n[4], n[5], n[6], n[7], n[8], hd);
+                                                 n[4], n[5], n[6], n[7], n[8], (T)(S->mesh->nen == 8 ? 1 : 4), hd);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -721,7 +832,8 @@ int sys_rhs_mech(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
     ChunkArgs<T> a = chunk_args(S);
     a.in0 = m_lib;
     S->prof.begin(CM_PROF_ELEMENT, st, 2);
-    CM_TRY((launch_chunks<T, EK_MECH>(S, a, st)));
+    if (S->mesh->nen == 8) CM_TRY((launch_hex<T, EK_MECH>(S, a, st)));
+    else CM_TRY((launch_chunks<T, EK_MECH>(S, a, st)));
     node_gather_kernel<T, 3><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->clamp, -1, b);
     S->prof.end(st);
     LAUNCH_CHECK();
@@ -735,7 +847,8 @@ int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st)
     ChunkArgs<T> a = chunk_args(S);
     a.in0 = u_lib; a.in1 = w_lib;
     S->prof.begin(CM_PROF_ELEMENT, st);
-    CM_TRY((launch_chunks<T, EK_STRESS>(S, a, st)));
+    if (S->mesh->nen == 8) CM_TRY((launch_hex<T, EK_STRESS>(S, a, st)));
+    else CM_TRY((launch_chunks<T, EK_STRESS>(S, a, st)));
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -749,7 +862,7 @@ int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], u
     S->prof.begin(CM_PROF_ELEMENT, st);
     node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mLm, S->live, w_lib, hd, terms,
                                                    (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], hext_dev, (T)S->lam100,
-                                                   (T)S->lam111, make_rot<T>(S), h, sig_out);
+                                                   (T)S->lam111, make_rot<T>(S), (T)(S->mesh->nen == 8 ? 1 : 4), h, sig_out);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;

@@ -147,6 +147,7 @@ struct SystemBase {
     bool rot = false;
     int n_elastic = 0;
     double Vtot = 0, Vmag = 0;
+    double ld = 1;  // length scale l_d, metres
     long nlive = 0;
     int pin = 0; // library index
     int num_sms = 0;
@@ -197,6 +198,36 @@ struct System : SystemBase {
     int hyst_cap = 0;
     ~System();
 };
+
+// Linear hexahedron (R26): |J|, phi_a and grad phi_a (fp64) at Gauss point p of the 2 x 2 x 2 rule; local node
+// a = i + 2 j + 4 k <-> reference corner (2i-1, 2j-1, 2k-1)
+__device__ __forceinline__ double hex_point(const double X[8][3], int p, double phi[8], double g[8][3])
+{
+    const double q = 0.57735026918962576451;
+    const double xi[3] = {(p & 1) ? q : -q, (p & 2) ? q : -q, (p & 4) ? q : -q};
+    double dN[8][3], J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+    for (int a = 0; a < 8; a++) {
+        const double s[3] = {(a & 1) ? 1.0 : -1.0, (a & 2) ? 1.0 : -1.0, (a & 4) ? 1.0 : -1.0};
+        const double f[3] = {1 + s[0] * xi[0], 1 + s[1] * xi[1], 1 + s[2] * xi[2]};
+        phi[a] = f[0] * f[1] * f[2] / 8;
+        dN[a][0] = s[0] * f[1] * f[2] / 8; dN[a][1] = f[0] * s[1] * f[2] / 8; dN[a][2] = f[0] * f[1] * s[2] / 8;
+#pragma unroll
+        for (int r = 0; r < 3; r++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) J[r][c] += X[a][r] * dN[a][c];
+    }
+    double cof[3][3];
+    cof[0][0] = J[1][1] * J[2][2] - J[1][2] * J[2][1]; cof[0][1] = J[1][2] * J[2][0] - J[1][0] * J[2][2]; cof[0][2] = J[1][0] * J[2][1] - J[1][1] * J[2][0];
+    cof[1][0] = J[0][2] * J[2][1] - J[0][1] * J[2][2]; cof[1][1] = J[0][0] * J[2][2] - J[0][2] * J[2][0]; cof[1][2] = J[0][1] * J[2][0] - J[0][0] * J[2][1];
+    cof[2][0] = J[0][1] * J[1][2] - J[0][2] * J[1][1]; cof[2][1] = J[0][2] * J[1][0] - J[0][0] * J[1][2]; cof[2][2] = J[0][0] * J[1][1] - J[0][1] * J[1][0];
+    const double det = J[0][0] * cof[0][0] + J[0][1] * cof[0][1] + J[0][2] * cof[0][2];
+#pragma unroll
+    for (int a = 0; a < 8; a++)
+#pragma unroll
+        for (int r = 0; r < 3; r++) g[a][r] = (cof[r][0] * dN[a][0] + cof[r][1] * dN[a][1] + cof[r][2] * dN[a][2]) / det;
+    return det;
+}
 
 // ---- cm_mesh.cu ----
 int mesh_build_host(cm_mesh *M, const double *xyz, long Ng, const int *gtets, long Ne, const uchar *mag, const int *eid,

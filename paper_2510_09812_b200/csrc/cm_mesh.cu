@@ -382,7 +382,11 @@ int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes,
     M->nnz = M->rowptr[N];
     if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
     if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
-    M->ck.nchunks = 0; M->ck.nslots = 0; // no element passes on hexahedra
+    // hexahedral element passes are node-centric: one slot per node (slot = node), no chunks
+    M->ck.nchunks = 0; M->ck.nslots = N;
+    M->ck.ns_ptr.resize(N + 1); M->ck.ns_slot.resize(N);
+    std::iota(M->ck.ns_ptr.begin(), M->ck.ns_ptr.end(), 0);
+    std::iota(M->ck.ns_slot.begin(), M->ck.ns_slot.end(), 0);
     return CM_OK;
 }
 

@@ -133,7 +133,8 @@ def test_hex_matrices_spmv_cg_average(cm, oracle_mod, torch, dtype):
         xo, ito, reso, rco = o.cg(mo, b.astype(np.float64).ravel(), tol=tol_cg)
         assert rc == 0 and rco == 0 and res < tol_cg
         # (fp32 against the fp64 oracle at the fp32 rounding floor of a ~300-iteration recurrence: 3 %)
-        assert abs(it - ito) <= (1 if f64 else max(2, ito // 33)), (mg, it, ito)
+        # fp64: +-1; the ~460-iteration mechanical solve gets 1 % (two runs of the ORACLE differ by +-2 there: DESIGN.md section 8)
+        assert abs(it - ito) <= (max(1, ito // 100 if mg == cm.CM_MAT_K_MECH else 1) if f64 else max(2, ito // 33)), (mg, it, ito)
         x64 = o.cg(mo, b.astype(np.float64).ravel(), tol=1e-13)[0]
         assert rel(xg.cpu().numpy().ravel(), x64) < (1e-7 if f64 else 2e-3)
         xg.zero_()
@@ -142,19 +143,82 @@ def test_hex_matrices_spmv_cg_average(cm, oracle_mod, torch, dtype):
         assert it == 3 and rel(xg.cpu().numpy().ravel(), x3o) < (1e-11 if f64 else 1e-4)
 
 
-def test_hex_refusals_and_errors(cm, torch):
-    mesh = inputs.hex_box((5, 5, 5), (9 * NM,) * 3)
+def test_hex_rhs_fields_and_steps(cm, oracle_mod, torch):
+    """Element-wise right-hand sides, recovered fields and ten GSPM steps (all terms, x2-stiff non-magnetic inclusion, clamped
+    bottom) on hexahedra: <= 1e-12 / 1e-5 on every pass, max |dm| <= 1e-9 (fp64) / 1e-4 (fp32) after ten steps."""
+    from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD, TERM_MAGEL, TERM_ZEEMAN
+    ALL = TERM_ANIS | TERM_ZEEMAN | TERM_DEMAG | TERM_FARFIELD | TERM_MAGEL
+    mesh = inputs.hex_box((13, 12, 8), (40 * NM, 36 * NM, 22 * NM), seed_mesh=21, seed_perm=22)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (9 * NM, 8 * NM, 6 * NM))
+    clamp = inputs.clamp_bottom(mesh)
+    for dtype, tol, cgt, bar in (("f64", 1e-12, 1e-12, 1e-9), ("f32", 1e-5, 1e-6, 1e-4)):
+        gm = cm.Mesh(mesh.xyz, mesh.hexes, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+        gs = cm.System(gm, mat2(), 1e-12, dtype, clamp, 3)
+        o = oracle_mod.Oracle(mesh, mat2(), 1e-12, clamp_dof=clamp, pin_node=3)
+        td = torch.float64 if dtype == "f64" else torch.float32
+        dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=td, device="cuda")
+        N = o.N
+        rng = np.random.default_rng(8)
+        live = o.live().astype(bool)
+        assert 0 < (~live).sum() < N
+        m = rng.normal(size=(N, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True); m[~live] = 0
+        m = m.astype(gs.np_dtype); m64 = m.astype(np.float64)
+        U = rng.normal(size=N).astype(gs.np_dtype); u = (1e-3 * rng.normal(size=(N, 3))).astype(gs.np_dtype)
+        md, Ud, ud = dev(m), dev(U), dev(u)
+        Hext = np.array([3e4, -1e4, 2e4])
+        p = cm.make_params(1e-12, Hext, ALL)
+        assert rel(gs.field_rhs(cm.CM_RHS_MS, md).cpu().numpy(), o.rhs_ms(m64)) < tol
+        assert rel(gs.field_rhs(cm.CM_RHS_MECH, md).cpu().numpy(), o.rhs_mech(m64)) < tol
+        hd_o, _ = o.demag_field(U.astype(np.float64), o.volume_average(m64), TERM_DEMAG | TERM_FARFIELD)
+        assert rel(gs.field_rhs(cm.CM_OUT_HD, md, Ud, None, p).cpu().numpy(), hd_o) < tol
+        sig_o = o.stress_recover(u.astype(np.float64), m64)
+        assert rel(gs.field_rhs(cm.CM_OUT_SIGMA, md, None, ud, p).cpu().numpy(), sig_o) < tol
+        h_o = o.field(m64, hd_o, sig_o, Hext / 1.2e6, ALL)
+        assert rel(gs.field_rhs(cm.CM_OUT_FIELD, md, Ud, ud, p).cpu().numpy(), h_o) < tol
+        assert rel(gs.field_rhs(cm.CM_RHS_GS, md, Ud, ud, p, coeff=0.37).cpu().numpy(), o.rhs_gs(m64 + 0.37 * h_o)) < tol
+        # ten steps
+        m0 = np.array([1.0, 0, 0]) + 0.1 * rng.normal(size=(N, 3)); m0 /= np.linalg.norm(m0, axis=1, keepdims=True); m0[~live] = 0
+        mo = m0.copy(); Uo = np.zeros(N); uo = np.zeros((N, 3))
+        mg = torch.as_tensor(m0, dtype=td, device="cuda").contiguous()
+        Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+        for k in range(10):
+            io, rco = o.gspm_step(mo, Uo, uo, 1e-12, [2e4, 0, 0], ALL, cg_tol=cgt)
+            ig, rcg = gs.gspm_step(cm.make_params(1e-12, [2e4, 0, 0], ALL, 0, cgt), mg, Ug, ug)
+            assert rco == 0 and rcg == 0
+            if dtype == "f64" and k == 0:
+                assert abs(io.it_ms - ig.it_ms) <= 1 and abs(io.it_mech - ig.it_mech) <= max(1, io.it_mech // 100)
+                assert all(abs(io.it_gs[a] - ig.it_gs[a]) <= 1 for a in range(8)) and io.it_mech > 10
+        mgh = mg.cpu().numpy().astype(np.float64)
+        assert np.abs(mgh - mo).max() <= bar
+        assert np.abs(mgh[~live]).max() == 0
+        if dtype == "f64":
+            assert np.abs(ug.cpu().numpy() - uo).max() <= 1e-9 * max(1.0, np.abs(uo).max())
+            assert np.abs(np.linalg.norm(mgh[live], axis=1) - 1).max() <= 4 * np.finfo(float).eps
+
+
+def test_hex_hysteresis_loop_and_errors(cm, oracle_mod, torch):
+    """The device-resident hysteresis loop runs on hexahedra too (two fields of three steps each against the oracle's loop)."""
+    from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD, TERM_ZEEMAN
+    terms = TERM_ANIS | TERM_ZEEMAN | TERM_DEMAG | TERM_FARFIELD
+    mesh = inputs.hex_box((8, 8, 8), (20 * NM,) * 3, seed_mesh=1, seed_perm=2)
     gm = cm.Mesh(mesh.xyz, mesh.hexes)
     gs = cm.System(gm, inputs.Material(), 1e-12)
-    N = gm.n_nodes
-    m = torch.zeros((N, 3), dtype=torch.float64, device="cuda"); m[:, 0] = 1
-    U = torch.zeros(N, dtype=torch.float64, device="cuda")
-    for call in (lambda: gs.field_rhs(cm.CM_RHS_MS, m), lambda: gs.gspm_step(cm.make_params(1e-12, terms=1), m, U, m.clone()),
-                 lambda: gs.hysteresis_run(cm.make_params(1e-12, terms=1), m, None, None, [1e4, 0, 0], [-1, 0, 0], max_fields=1, max_steps=1),
-                 lambda: gs.geometry(0)):
-        with pytest.raises(cm.CmError) as e:
-            call()
-        assert e.value.code == cm.CM_E_BADARG
+    o = oracle_mod.Oracle(mesh, inputs.Material(), 1e-12)
+    N = o.N
+    rng = np.random.default_rng(5)
+    m0 = np.array([1.0, 0, 0]) + 0.1 * rng.normal(size=(N, 3)); m0 /= np.linalg.norm(m0, axis=1, keepdims=True)
+    m = m0.copy(); U = np.zeros(N); u = np.zeros((N, 3))
+    Hl, ml, sl, res, rc = o.hysteresis_run(m, U, u, 1e-12, [4e4, 0, 0], [-3e4, 0, 0], terms, conv_tol=0.0, max_fields=2, max_steps=3, cg_tol=1e-12)
+    mg = torch.as_tensor(m0, dtype=torch.float64, device="cuda").contiguous()
+    Ug = torch.zeros(N, dtype=torch.float64, device="cuda")
+    Hg, mlg, slg, resg, rcg = gs.hysteresis_run(cm.make_params(1e-12, (0, 0, 0), terms, 0, 1e-12), mg, Ug, None, [4e4, 0, 0], [-3e4, 0, 0],
+                                                conv_tol=0.0, max_fields=2, max_steps=3)
+    assert rc == 0 and rcg == 0 and resg.n_fields == 2 and list(slg) == [3, 3]
+    assert np.array_equal(Hg, Hl) and np.abs(mlg - ml).max() < 1e-11
+    assert np.abs(mg.cpu().numpy() - m).max() <= 1e-9
+    with pytest.raises(cm.CmError) as e:
+        gs.geometry(0)                                            # chunk-blocked element geometry exists for tetrahedra only
+    assert e.value.code == cm.CM_E_BADARG
     bad = mesh.hexes.copy(); bad[3] = bad[3][[1, 0, 2, 3, 4, 5, 6, 7]]
     with pytest.raises(cm.CmError) as e:
         cm.Mesh(mesh.xyz, bad)
