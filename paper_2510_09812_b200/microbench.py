@@ -42,6 +42,13 @@ def elem_bytes(N, Ne, s):
             "elem_sigma": tet + N * 12 * s}
 
 
+def hex_elem_bytes(N, Ne, s):
+    """Node-centric hexahedral passes: 32 B connectivity per cell, coordinates (fp64) and nodal input / output once."""
+    cell = Ne * 32 + N * 24
+    return {"elem_rhs_ms": cell + N * 4 * s, "elem_hd": cell + N * 4 * s, "elem_rhs_mech": cell + N * 6 * s,
+            "elem_sigma": cell + N * 12 * s}
+
+
 def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=False):
     import torch
     from . import binding as cm
@@ -116,12 +123,14 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=
                         x.zero_(); its.append(gs.cg_solve(matid, b, x, tol=tol, maxiter=200000)[0])
                     t, p = kernel_ms(ft, cls, 2)
                     cases.append((name + "_tol1e-8", t, its[-1] * mb[key], its[-1]))
-                eb = elem_bytes(N, gm.n_tets, s)
-                m3 = None if hex_mesh else torch.as_tensor(inputs.init_m_noisy_x(mesh, 44), dtype=td, device="cuda").contiguous()
+                eb = elem_bytes(N, gm.n_tets, s) if not hex_mesh else hex_elem_bytes(N, gm.n_tets, s)
+                rng44 = np.random.default_rng(44)
+                m0 = np.array([1.0, 0.0, 0.0]) + 0.1 * rng44.normal(size=(N, 3))
+                m3 = torch.as_tensor(m0 / np.linalg.norm(m0, axis=1, keepdims=True), dtype=td, device="cuda").contiguous()
                 for name, rid, kw in (("elem_rhs_ms", cm.CM_RHS_MS, {}), ("elem_hd", cm.CM_OUT_HD, {"U": b1}),
                                       ("elem_rhs_mech", cm.CM_RHS_MECH, {}), ("elem_sigma", cm.CM_OUT_SIGMA, {"u": b3})):
-                    if hex_mesh or (only and name not in only and "elem" not in only):
-                        continue          # (element passes are tetrahedral only)
+                    if only and name not in only and "elem" not in only:
+                        continue
                     t, p = kernel_ms(lambda: gs.field_rhs(rid, m3, **kw), "element", reps)
                     # kernel_ms divides by launches; a pass is 2-3 launches, so take the class total per call
                     cases.append((name, p["ms"] / reps, eb[name], None))
