@@ -149,10 +149,9 @@ class Oracle:
         h = C.c_void_p()
         self.is_hex = hasattr(mesh, "hexes")
         if self.is_hex:
-            assert dof is None
             hexes = np.ascontiguousarray(mesh.hexes, np.int32)
-            rc = self.L.orc_create_hex(_p(xyz), C.c_long(self.Ng), _p(hexes), C.c_long(self.Ne), _p(mag), _p(eid), C.byref(m),
-                                       C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
+            rc = self.L.orc_create_hex(_p(xyz), C.c_long(self.Ng), _p(hexes), C.c_long(self.Ne), _p(mag), _p(eid), _p(dof),
+                                       C.c_long(self.N), C.byref(m), C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))
         else:
             rc = self.L.orc_create_wrapped(_p(xyz), C.c_long(self.Ng), _p(tets), C.c_long(self.Ne), _p(mag), _p(eid), _p(dof),
                                            C.c_long(self.N), C.byref(m), C.c_double(dt), _p(clamp), C.c_long(pin_node), C.byref(h))

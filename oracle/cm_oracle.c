@@ -102,7 +102,8 @@ typedef struct {
     int n_elastic; double *Cstar; /* n_elastic x 36, C/(mu0 Ms^2) */
     double Vtot, Vmag;
     double R[9]; int rot; /* App. D rotation (identity: rot = 0) */
-    int nen; int *hex;    /* nen = 8: linear hexahedra (matrices and averages only); hex = Ne x 8 connectivity; 0 / 4: tetrahedra */
+    int nen; int *hex;    /* nen = 8: linear hexahedra; hex = Ne x 8 connectivity in DOF numbering; 0 / 4: tetrahedra */
+    int *ghex;            /* hexahedra: Ne x 8 geometric node ids (coordinates); differs from hex on a wrapped (periodic) mesh */
 } oracle;
 
 static const double MU0 = 4.0e-7 * 3.14159265358979323846;
@@ -686,11 +687,20 @@ static void hex_gauss_point(const double *X /* 8 x 3 */, int p, double *detJ, do
         for (int r = 0; r < 3; r++) g[a][r] = (cof[r][0] * dN[a][0] + cof[r][1] * dN[a][1] + cof[r][2] * dN[a][2]) / det;
 }
 
-int orc_create_hex(const double *xyz_m, long N, const int *hexes, long Ne, const uchar *magnetic, const int *elastic_id,
-                   const orc_material *mat, double dt, const uchar *clamp_dof, long pin_node, oracle **out)
+/* dof (NULL = identity): periodic node wrapping as for tetrahedra: geometry from the cell's own corners, every
+ * nodal quantity indexed by DOF. */
+int orc_create_hex(const double *xyz_m, long Ng, const int *hexes, long Ne, const uchar *magnetic, const int *elastic_id,
+                   const int *dof, long N, const orc_material *mat, double dt, const uchar *clamp_dof, long pin_node, oracle **out)
 {
-    if (!xyz_m || !hexes || !mat || !out || N <= 0 || Ne <= 0 || pin_node < 0 || pin_node >= N) return ORC_E_BADARG;
-    for (long q = 0; q < 8 * Ne; q++) if (hexes[q] < 0 || hexes[q] >= N) return ORC_E_RANGE;
+    if (!xyz_m || !hexes || !mat || !out || N <= 0 || Ng <= 0 || Ne <= 0 || pin_node < 0 || pin_node >= N) return ORC_E_BADARG;
+    if (!dof && N != Ng) return ORC_E_BADARG;
+    for (long q = 0; q < 8 * Ne; q++) if (hexes[q] < 0 || hexes[q] >= Ng) return ORC_E_RANGE;
+    if (dof) {
+        for (long i = 0; i < Ng; i++) if (dof[i] < 0 || dof[i] >= N) return ORC_E_RANGE;
+        for (long e = 0; e < Ne; e++)
+            for (int a = 0; a < 8; a++) for (int b = a + 1; b < 8; b++)
+                if (dof[hexes[8 * e + a]] == dof[hexes[8 * e + b]]) return ORC_E_BADARG; /* one cell wide in a periodic direction */
+    }
     oracle *o = (oracle *)calloc(1, sizeof(oracle));
     if (!o) return ORC_E_ALLOC;
     o->N = N; o->Ne = Ne; o->nen = 8;
@@ -707,16 +717,18 @@ int orc_create_hex(const double *xyz_m, long N, const int *hexes, long Ne, const
     o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
     o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
     for (int q = 0; q < 36 * o->n_elastic; q++) o->Cstar[q] = mat->C_voigt[q] / mu0Ms2;
-    o->x = (double *)malloc((size_t)N * 3 * sizeof(double));
+    o->x = (double *)malloc((size_t)Ng * 3 * sizeof(double));
     o->hex = (int *)malloc((size_t)Ne * 8 * sizeof(int));
+    o->ghex = (int *)malloc((size_t)Ne * 8 * sizeof(int));
     o->mag = (uchar *)malloc((size_t)Ne);
     o->eid = (int *)calloc((size_t)Ne, sizeof(int));
     o->V = (real *)malloc((size_t)Ne * sizeof(real));
     o->mL = (real *)malloc((size_t)N * sizeof(real)); o->mLm = (real *)malloc((size_t)N * sizeof(real));
     o->live = (uchar *)calloc((size_t)N, 1);
     o->clamp = (uchar *)calloc((size_t)N * 3, 1);
-    for (long i = 0; i < 3 * N; i++) o->x[i] = xyz_m[i] / ld;
-    memcpy(o->hex, hexes, (size_t)Ne * 8 * sizeof(int));
+    for (long i = 0; i < 3 * Ng; i++) o->x[i] = xyz_m[i] / ld;
+    memcpy(o->ghex, hexes, (size_t)Ne * 8 * sizeof(int));
+    for (long q = 0; q < 8 * Ne; q++) o->hex[q] = dof ? dof[hexes[q]] : hexes[q];
     for (long e = 0; e < Ne; e++) o->mag[e] = magnetic ? (magnetic[e] != 0) : 1;
     if (elastic_id) memcpy(o->eid, elastic_id, (size_t)Ne * sizeof(int));
     if (clamp_dof) for (long i = 0; i < 3 * N; i++) o->clamp[i] = clamp_dof[i] != 0;
@@ -733,7 +745,7 @@ int orc_create_hex(const double *xyz_m, long N, const int *hexes, long Ne, const
     double *Kme = o->n_elastic ? (double *)calloc((size_t)nnz * 9, sizeof(double)) : NULL;
     if (!K || !Km || !Mm || !mL || !mLm || (o->n_elastic && !Kme)) { orc_destroy(o); return ORC_E_ALLOC; }
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-    for (long i = 0; i < N; i++) for (int d = 0; d < 3; d++) {
+    for (long i = 0; i < Ng; i++) for (int d = 0; d < 3; d++) {
         if (o->x[3 * i + d] < lo[d]) lo[d] = o->x[3 * i + d];
         if (o->x[3 * i + d] > hi[d]) hi[d] = o->x[3 * i + d];
     }
@@ -741,9 +753,9 @@ int orc_create_hex(const double *xyz_m, long N, const int *hexes, long Ne, const
     double Jmin = 1e-14 * diag * diag * diag;
     o->Vtot = 0; o->Vmag = 0;
     for (long e = 0; e < Ne; e++) {
-        const int *t = o->hex + 8 * e;
+        const int *t = o->hex + 8 * e, *tg = o->ghex + 8 * e;
         double X[24];
-        for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)t[a] + d];
+        for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)tg[a] + d];
         const double *C = o->n_elastic ? o->Cstar + 36 * o->eid[e] : NULL;
         double Ve = 0;
         for (int p = 0; p < 8; p++) {
@@ -790,7 +802,7 @@ int orc_create_hex(const double *xyz_m, long N, const int *hexes, long Ne, const
 void orc_destroy(oracle *o)
 {
     if (!o) return;
-    free(o->hex);
+    free(o->hex); free(o->ghex);
     free(o->x); free(o->tet); free(o->mag); free(o->eid); free(o->V); free(o->G); free(o->mL); free(o->mLm);
     free(o->live); free(o->n2e_ptr); free(o->n2e); free(o->rowptr); free(o->col); free(o->K); free(o->Kms);
     free(o->Km); free(o->Mm); free(o->Kgs1); free(o->Kgs2); free(o->Kmech); free(o->Kmech_free); free(o->clamp);
@@ -951,9 +963,9 @@ int orc_volume_average(const oracle *o, const void *g_, int ncomp, double *out)
     for (int c = 0; c < ncomp; c++) num[c] = 0;
     if (o->nen == 8) { /* Eq. 17 with the 2 x 2 x 2 Gauss rule: sum_e sum_p g_e(r_p) |J(e,p)| w_p */
         for (long e = 0; e < o->Ne; e++) {
-            const int *t = o->hex + 8 * e;
+            const int *t = o->hex + 8 * e, *tg = o->ghex + 8 * e;
             double X[24];
-            for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)t[a] + d];
+            for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)tg[a] + d];
             for (int p = 0; p < 8; p++) {
                 double det, phi[8], gr[8][3];
                 hex_gauss_point(X, p, &det, phi, gr);
@@ -1124,7 +1136,7 @@ static void C_times(const oracle *o, long e, const real eps[6], real sig[6])
 /* ------------------------------------------------------------------------------------ */
 static void hex_coords(const oracle *o, long e, double X[24])
 {
-    const int *t = o->hex + 8 * e;
+    const int *t = o->ghex + 8 * e;
     for (int a = 0; a < 8; a++) for (int d = 0; d < 3; d++) X[3 * a + d] = o->x[3 * (long)t[a] + d];
 }
 

@@ -252,3 +252,74 @@ def test_hex_degenerate_cell_rejected(orc, jit):
     bad = inputs.replace(mesh, hexes=mesh.hexes[:, [1, 0, 2, 3, 4, 5, 6, 7]].copy())     # inverted cells
     with pytest.raises(RuntimeError, match="rc=-2"):
         orc.Oracle(bad, mat2(), 1e-12)
+
+
+def test_periodic_hexahedra(orc):
+    """Node wrapping on hexahedra -- the paper's own setting (structured hexahedral meshes, periodic): 27 entries
+    in every row; on the uniform grid the stiffness is circulant with the closed-form symbol of the trilinear element;
+    ker K = constants, ker K^mech = the three translations (Eq. 20: d = 3); the literal Eq. 14 right-hand side equals the
+    adjoint one (R9); uniform m along an easy axis is a fixed point and the energy decays."""
+    from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD
+    grid, box = (7, 6, 5), (24 * NM, 15 * NM, 10 * NM)
+    mesh = inputs.hex_box(grid, box, jitter=0.0, seed_mesh=5, seed_perm=6)
+    dof, nd = orc.periodic_wrap(mesh.xyz, 7)
+    assert nd == 6 * 5 * 4
+    o = orc.Oracle(mesh, inputs.Material(), 1e-12, dof_of_node=dof, n_dof=nd)
+    assert o.N == nd and np.all(np.diff(o.rowptr()) == 27)
+    h = np.array(box) / NM / (np.array(grid) - 1)
+    L = np.array(box) / NM
+    x = np.zeros((nd, 3)); x[dof] = np.where(mesh.xyz / NM >= L - 1e-9, 0.0, mesh.xyz / NM)
+    assert np.allclose(o.mL(), h.prod(), rtol=1e-13)
+    for d in range(3):
+        u = np.cos(2 * np.pi * x[:, d] / L[d])
+        th = 2 * np.pi * h[d] / L[d]
+        lam = h.prod() / h[d] ** 2 * (2 - 2 * np.cos(th))        # k1(theta) m1(0) m1(0): 1D stiffness symbol x full 1D masses
+        assert np.abs(o.spmv(orc.MAT_K_FREE, u) - lam * u).max() <= 1e-12 * lam
+        mu = h.prod() * (4 + 2 * np.cos(th)) / 6                 # 1D consistent-mass symbol h (4 + 2 cos theta) / 6
+        assert np.abs(o.spmv(orc.MAT_MASS, u) - mu * u).max() <= 1e-12 * mu
+    # jittered periodic cells with mechanics
+    C = inputs.isotropic_voigt(200e9, 0.3)
+    mesh = inputs.hex_box((6, 5, 5), (20 * NM, 16 * NM, 16 * NM), seed_mesh=5, seed_perm=6)
+    dof, nd = orc.periodic_wrap(mesh.xyz, 7)
+    clamp = np.zeros((nd, 3), np.uint8); clamp[4] = 1
+    o = orc.Oracle(mesh, inputs.Material(C_voigt=C[None]), 1e-12, clamp_dof=clamp.ravel(), pin_node=3, dof_of_node=dof, n_dof=nd)
+    assert o.Vtot == pytest.approx(20 * 16 * 16, rel=1e-13)
+    w = np.linalg.eigvalsh(o.csr(orc.MAT_K_FREE).toarray())
+    assert np.sum(np.abs(w) < 1e-10 * w.max()) == 1
+    w = np.linalg.eigvalsh(o.csr(orc.MAT_K_MECH_FREE).toarray())
+    assert np.sum(np.abs(w) < 1e-10 * w.max()) == 3
+    rng = np.random.default_rng(7)
+    m = rng.normal(size=(nd, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True)
+    # literal Eq. 14: -sum_e sum_p |J| phi_i div m_h, written out here with numpy from the trilinear shape functions
+    g = 1 / np.sqrt(3)
+    lit = np.zeros(nd)
+    sgn = np.array([[(a >> d & 1) * 2 - 1 for d in range(3)] for a in range(8)], float)
+    for e in range(mesh.n_tets):
+        X = mesh.xyz[mesh.hexes[e]] / NM
+        t = dof[mesh.hexes[e]]
+        for p in range(8):
+            xi = np.array([(p >> d & 1) * 2 - 1 for d in range(3)], float) * g
+            f = 1 + sgn * xi
+            phi = f.prod(1) / 8
+            dN = np.stack([sgn[:, 0] * f[:, 1] * f[:, 2], f[:, 0] * sgn[:, 1] * f[:, 2], f[:, 0] * f[:, 1] * sgn[:, 2]], 1) / 8
+            J = X.T @ dN
+            G = dN @ np.linalg.inv(J)
+            lit[t] += -np.linalg.det(J) * phi * np.einsum("ad,ad->", G, m[t])
+    b = o.rhs_ms(m)
+    keep = np.arange(nd) != 3
+    assert b[3] == 0 and np.abs(b[keep] - lit[keep]).max() <= 1e-11 * np.abs(lit).max()
+    terms = TERM_ANIS | TERM_DEMAG | TERM_FARFIELD
+    mz = np.tile([0.0, 0.0, 1.0], (nd, 1)); U = np.zeros(nd); u = np.zeros((nd, 3))
+    info, rc = o.gspm_step(mz, U, u, 1e-12, [0, 0, 0], terms, cg_tol=1e-12)
+    assert rc == 0 and np.abs(mz - [0, 0, 1]).max() < 1e-14
+    E = [o.energy(m, U, u, np.zeros(3), terms)]
+    for _ in range(6):
+        info, rc = o.gspm_step(m, U, u, 1e-12, [0, 0, 0], terms, cg_tol=1e-12)
+        assert rc == 0 and np.abs(np.linalg.norm(m, axis=1) - 1).max() <= 4 * np.finfo(float).eps
+        E.append(o.energy(m, U, u, np.zeros(3), terms))
+    assert all(b2 < a2 for a2, b2 in zip(E, E[1:])), E
+    # one cell across a periodic direction collapses the cell
+    thin = inputs.hex_box((2, 4, 4), (5 * NM, 12 * NM, 12 * NM))
+    dof, nd = orc.periodic_wrap(thin.xyz, 1)
+    with pytest.raises(RuntimeError, match="rc=-1"):
+        orc.Oracle(thin, inputs.Material(), 1e-12, dof_of_node=dof, n_dof=nd)
