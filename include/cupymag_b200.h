@@ -151,11 +151,15 @@ int cm_mesh_create_wrapped(const double *xyz, long n_nodes, const int *tets, lon
  * functions; every element integral (matrices, right-hand sides, recovered fields, lumped masses, Eq. 17) by the
  * 2 x 2 x 2 Gauss rule.  Every call of this header works on a hexahedral mesh (cm_assemble_csr, cm_spmv, cm_cg_solve*,
  * cm_field_rhs, cm_gspm_step*, cm_hysteresis_run, cm_volume_average) except cm_system_get_geometry(what = 0, 1), whose
- * per-element V_e / grad phi are stored for tetrahedra only (CM_E_BADARG), and periodic wrapping.  cm_mesh_get:
+ * per-element V_e / grad phi are stored for tetrahedra only (CM_E_BADARG).  cm_mesh_create_hex_wrapped: periodic node
+ * wrapping exactly as cm_mesh_create_wrapped (dof_of_node from cm_periodic_wrap) -- the paper's own setting.  cm_mesh_get:
  * CM_GET_TETS has 8 ids per element, CM_GET_N2E entries are element*8 + local index.  Errors as cm_mesh_create
  * (DEGENERATE_TET: det J <= 0 at a Gauss point, i.e. an inverted or collapsed cell). */
 int cm_mesh_create_hex(const double *xyz, long n_nodes, const int *hexes, long n_hexes, const unsigned char *magnetic,
                        const int *elastic_id, cm_reorder reorder, void *stream, cm_mesh **out);
+int cm_mesh_create_hex_wrapped(const double *xyz, long n_nodes, const int *hexes, long n_hexes, const unsigned char *magnetic,
+                               const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream,
+                               cm_mesh **out);
 int cm_mesh_destroy(cm_mesh *mesh);
 /* Copies structure arrays to host_out (capacity in elements); returns BADARG if capacity is too small. */
 int cm_mesh_get(const cm_mesh *mesh, int what, void *host_out, long capacity);

@@ -29,7 +29,7 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
-EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
+EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_hex_wrapped", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
            "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_field_rhs", "cm_volume_average",
            "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
@@ -88,6 +88,7 @@ def lib():
         L.cm_mesh_create.argtypes = [vp, lg, vp, lg, vp, vp, it, vp, C.POINTER(vp)]
         L.cm_mesh_create_wrapped.argtypes = [vp, lg, vp, lg, vp, vp, vp, lg, it, vp, C.POINTER(vp)]
         L.cm_mesh_create_hex.argtypes = [vp, lg, vp, lg, vp, vp, it, vp, C.POINTER(vp)]
+        L.cm_mesh_create_hex_wrapped.argtypes = [vp, lg, vp, lg, vp, vp, vp, lg, it, vp, C.POINTER(vp)]
         L.cm_periodic_wrap.argtypes = [vp, lg, C.c_uint, db, vp, C.POINTER(lg)]
         L.cm_mesh_destroy.argtypes = [vp]
         L.cm_mesh_get.argtypes = [vp, it, vp, lg]
@@ -164,8 +165,12 @@ class Mesh:
         mag = _np(magnetic, np.uint8); eid = _np(elastic_id, np.int32)
         self.h = C.c_void_p()
         self.nen = 8 if tets.shape[1] == 8 else 4            # (Ne, 8): linear hexahedra, local node a = i + 2 j + 4 k
-        if self.nen == 8:
-            assert dof_of_node is None
+        if self.nen == 8 and dof_of_node is not None:
+            dof = _np(dof_of_node, np.int32)
+            assert dof.shape[0] == xyz.shape[0]
+            _check(L.cm_mesh_create_hex_wrapped(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), _hp(dof), int(n_dof),
+                                                reorder, _stream(), C.byref(self.h)))
+        elif self.nen == 8:
             _check(L.cm_mesh_create_hex(_hp(xyz), xyz.shape[0], _hp(tets), tets.shape[0], _hp(mag), _hp(eid), reorder, _stream(),
                                         C.byref(self.h)))
         elif dof_of_node is None:

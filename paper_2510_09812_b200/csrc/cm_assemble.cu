@@ -164,7 +164,7 @@ __global__ void assemble_rows_kernel(long N, const int *__restrict__ tets, const
 // ---- linear hexahedra (R26): one thread per row i accumulates, over the incident elements in ascending order and the
 // 2 x 2 x 2 Gauss points in order, row i of K, K_m, M_m, K^mech and the lumped masses int phi_i.
 template <typename T>
-__global__ void hex_rows_kernel(long N, const int *__restrict__ hexes, const double *__restrict__ xyz, double ld,
+__global__ void hex_rows_kernel(long N, const int *__restrict__ hexes, const int *__restrict__ ghexes, const double *__restrict__ xyz, double ld,
                                 const int *__restrict__ n2e_ptr, const int *__restrict__ n2e, const uchar *__restrict__ mag,
                                 const int *__restrict__ eid, const double *__restrict__ Cstar, const int *__restrict__ rowptr,
                                 const int *__restrict__ col, double *K, double *Km, double *Mm, double *Kme, T *mL, T *mLm, uchar *live)
@@ -180,7 +180,8 @@ __global__ void hex_rows_kernel(long N, const int *__restrict__ hexes, const dou
         double X[8][3];
         for (int a = 0; a < 8; a++) {
             t[a] = hexes[8 * (long)e + a];
-            for (int d = 0; d < 3; d++) X[a][d] = xyz[3 * (long)t[a] + d] / ld;
+            const long ga = ghexes[8 * (long)e + a]; // coordinates come from the cell's own corner (wrapped meshes: != DOF)
+            for (int d = 0; d < 3; d++) X[a][d] = xyz[3 * ga + d] / ld;
             int lo = q0, hi = q1 - 1; // position of column t[a] in the sorted row
             while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
@@ -418,7 +419,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     if (S->n_elastic) CM_TRY(alloc(&Kme, 9 * nnz));
     const int BA = 128;
     if (hex)
-        hex_rows_kernel<T><<<(unsigned)((N + 63) / 64), 64, 0, st>>>(N, M->d_tets, M->d_xyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag, M->d_eid, Cd,
+        hex_rows_kernel<T><<<(unsigned)((N + 63) / 64), 64, 0, st>>>(N, M->d_tets, M->d_gtets, M->d_gxyz, ld, M->d_n2e_ptr, M->d_n2e, M->d_mag, M->d_eid, Cd,
                                                                     M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->mL, S->mLm, S->live);
     else
         assemble_rows_kernel<<<(unsigned)((N + BA - 1) / BA), BA, 0, st>>>(N, M->d_tets, M->d_gtets, M->d_gxyz, ld, M->d_n2e_ptr, M->d_n2e,

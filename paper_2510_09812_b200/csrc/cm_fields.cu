@@ -124,8 +124,8 @@ constexpr int EK_NT = CM_EK_NT;
 template <typename T>
 struct ChunkArgs {
     const int *eptr, *nptr, *nodes;
-    const int *hexes, *n2e_ptr, *n2e; // hexahedral meshes (node-centric passes): connectivity, node -> (element * 8 + corner)
-    const double *xyz;                // library-order coordinates, metres
+    const int *hexes, *ghexes, *n2e_ptr, *n2e; // hexahedral meshes (node-centric passes): DOF / geometric connectivity, node -> (element * 8 + corner)
+    const double *xyz;                // coordinates of the geometric nodes, metres
     double ld;
     long N;
     const unsigned short *lid, *lptr, *lent, *emat;
@@ -660,7 +660,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     ChunkArgs<T> a;
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
     a.emat = M->d_emat; a.EG = S->EG;
-    a.hexes = M->d_tets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_xyz; a.ld = S->ld; a.N = S->N;
+    a.hexes = M->d_tets; a.ghexes = M->d_gtets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_gxyz; a.ld = S->ld; a.N = S->N;
     a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
     a.hpart = S->hpart; a.partial = S->red;
@@ -710,8 +710,9 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
 #pragma unroll
             for (int c = 0; c < 8; c++) {
                 t[c] = a.hexes[8 * (long)e + c];
+                const long gc = a.ghexes[8 * (long)e + c];
 #pragma unroll
-                for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * (long)t[c] + d] / a.ld;
+                for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * gc + d] / a.ld;
             }
             T e0c[8][6]; // E0 at the 8 corners (MECH, STRESS)
             if (KIND == EK_MECH || KIND == EK_STRESS) {

@@ -232,8 +232,8 @@ __device__ __forceinline__ double hex_point(const double X[8][3], int p, double 
 // ---- cm_mesh.cu ----
 int mesh_build_host(cm_mesh *M, const double *xyz, long Ng, const int *gtets, long Ne, const uchar *mag, const int *eid,
                     const int *dof, long N, cm_reorder reorder);
-int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes, long Ne, const uchar *mag, const int *eid,
-                        cm_reorder reorder);
+int mesh_build_host_hex(cm_mesh *M, const double *xyz, long Ng, const int *ghexes, long Ne, const uchar *mag, const int *eid,
+                        const int *dof, long N, cm_reorder reorder);
 int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out);
 int build_chunks(long N, long Ne, const int *tets, Chunks *out);
 

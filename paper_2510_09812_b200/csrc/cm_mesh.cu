@@ -301,19 +301,44 @@ static double hex_detJ_phi(const double X[8][3], int p, double phi[8])
            J[0][2] * (J[1][0] * J[2][1] - J[1][1] * J[2][0]);
 }
 
-int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes, long Ne, const uchar *mag, const int *eid,
-                        cm_reorder reorder)
+int mesh_build_host_hex(cm_mesh *M, const double *gx, long Ng, const int *ghexes, long Ne, const uchar *mag, const int *eid,
+                        const int *dof, long N, cm_reorder reorder)
 {
-    M->N = N; M->Ne = Ne; M->Ng = N; M->nen = 8; M->wrapped = false;
+    M->N = N; M->Ne = Ne; M->Ng = Ng; M->nen = 8; M->wrapped = dof != nullptr;
     for (long q = 0; q < 8 * Ne; q++)
-        if (hexes[q] < 0 || hexes[q] >= N) {
-            cm_set_error("cm_mesh_create_hex: element %ld references node %d outside [0, %ld)", q / 8, hexes[q], N);
+        if (ghexes[q] < 0 || ghexes[q] >= Ng) {
+            cm_set_error("cm_mesh_create_hex: element %ld references node %d outside [0, %ld)", q / 8, ghexes[q], Ng);
             return CM_E_INDEX_RANGE;
         }
+    // DOF connectivity and DOF coordinates (wrapped mesh: as for tetrahedra)
+    std::vector<int> hex_v;
+    std::vector<double> xyz_v;
+    const int *hexes = ghexes;
+    const double *xyz = gx;
+    if (dof) {
+        for (long i = 0; i < Ng; i++)
+            if (dof[i] < 0 || dof[i] >= N) { cm_set_error("cm_mesh_create_hex_wrapped: dof_of_node[%ld] = %d outside [0, %ld)", i, dof[i], N); return CM_E_INDEX_RANGE; }
+        hex_v.resize(8 * Ne);
+        for (long q = 0; q < 8 * Ne; q++) hex_v[q] = dof[ghexes[q]];
+        for (long e = 0; e < Ne; e++)
+            for (int a = 0; a < 8; a++)
+                for (int b = a + 1; b < 8; b++)
+                    if (hex_v[8 * e + a] == hex_v[8 * e + b]) {
+                        cm_set_error("cm_mesh_create_hex_wrapped: element %ld has two corners on DOF %d (domain one cell wide in a periodic direction)", e, hex_v[8 * e + a]);
+                        return CM_E_BADARG;
+                    }
+        xyz_v.assign(3 * N, std::numeric_limits<double>::infinity());
+        for (long i = 0; i < Ng; i++)
+            for (int d = 0; d < 3; d++) xyz_v[3 * (long)dof[i] + d] = std::min(xyz_v[3 * (long)dof[i] + d], gx[3 * i + d]);
+        for (long i = 0; i < 3 * N; i++)
+            if (!std::isfinite(xyz_v[i])) { cm_set_error("cm_mesh_create_hex_wrapped: DOF %ld has no node", i / 3); return CM_E_BADARG; }
+        hexes = hex_v.data();
+        xyz = xyz_v.data();
+    }
     double lo[3], hi[3];
-    for (int d = 0; d < 3; d++) lo[d] = hi[d] = xyz[d];
-    for (long i = 0; i < N; i++)
-        for (int d = 0; d < 3; d++) { lo[d] = std::min(lo[d], xyz[3 * i + d]); hi[d] = std::max(hi[d], xyz[3 * i + d]); }
+    for (int d = 0; d < 3; d++) lo[d] = hi[d] = gx[d];
+    for (long i = 0; i < Ng; i++)
+        for (int d = 0; d < 3; d++) { lo[d] = std::min(lo[d], gx[3 * i + d]); hi[d] = std::max(hi[d], gx[3 * i + d]); }
     const double diag = std::sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) + (hi[2] - lo[2]) * (hi[2] - lo[2]));
     const double jmin = 1e-14 * diag * diag * diag;
     std::vector<double> w_user(N, 0.0);
@@ -321,7 +346,7 @@ int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes,
     for (long e = 0; e < Ne; e++) {
         double X[8][3], phi[8];
         for (int a = 0; a < 8; a++)
-            for (int d = 0; d < 3; d++) X[a][d] = xyz[3 * (long)hexes[8 * e + a] + d];
+            for (int d = 0; d < 3; d++) X[a][d] = gx[3 * (long)ghexes[8 * e + a] + d];
         double ve = 0;
         for (int p = 0; p < 8; p++) {
             const double det = hex_detJ_phi(X, p, phi);
@@ -371,6 +396,12 @@ int mesh_build_host_hex(cm_mesh *M, const double *xyz, long N, const int *hexes,
         M->eid[e] = eid ? eid[old] : 0;
         if (M->eid[e] < 0 || M->eid[e] > 0x7ffe) { cm_set_error("cm_mesh_create_hex: elastic_id %d outside [0, 32766]", M->eid[e]); return CM_E_INDEX_RANGE; }
         M->emat[e] = (unsigned short)(M->eid[e] << 1 | (M->mag[e] ? 1 : 0));
+    }
+    if (M->wrapped) {
+        M->gtets.resize(8 * Ne);
+        for (long e = 0; e < Ne; e++)
+            for (int k = 0; k < 8; k++) M->gtets[8 * e + k] = ghexes[8 * (long)M->tet_order[e] + k];
+        M->gxyz.assign(gx, gx + 3 * Ng);
     }
     M->xyz.resize(3 * N); M->wvol.resize(N);
     for (long i = 0; i < N; i++) {
@@ -612,6 +643,13 @@ extern "C" int cm_mesh_create_hex(const double *xyz, long n_nodes, const int *he
     return mesh_create_any(xyz, n_nodes, hexes, n_hexes, magnetic, elastic_id, nullptr, n_nodes, reorder, stream, out, 8);
 }
 
+extern "C" int cm_mesh_create_hex_wrapped(const double *xyz, long n_nodes, const int *hexes, long n_hexes, const unsigned char *magnetic,
+                                          const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream,
+                                          cm_mesh **out)
+{
+    return mesh_create_any(xyz, n_nodes, hexes, n_hexes, magnetic, elastic_id, dof_of_node, n_dof, reorder, stream, out, 8);
+}
+
 static int mesh_create_any(const double *xyz, long n_nodes, const int *tets, long n_tets, const unsigned char *magnetic,
                            const int *elastic_id, const int *dof_of_node, long n_dof, cm_reorder reorder, void *stream, cm_mesh **out,
                            int nen)
@@ -631,7 +669,7 @@ static int mesh_create_any(const double *xyz, long n_nodes, const int *tets, lon
     if (!M) return CM_E_ALLOC;
     int rc;
     try {
-        rc = nen == 8 ? mesh_build_host_hex(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, reorder)
+        rc = nen == 8 ? mesh_build_host_hex(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, dof_of_node, n_dof, reorder)
                       : mesh_build_host(M, xyz, n_nodes, tets, n_tets, magnetic, elastic_id, dof_of_node, n_dof, reorder);
     } catch (const std::bad_alloc &) {
         cm_set_error("cm_mesh_create: out of host memory");

@@ -227,3 +227,54 @@ def test_hex_hysteresis_loop_and_errors(cm, oracle_mod, torch):
     with pytest.raises(cm.CmError) as e:
         cm.Mesh(mesh.xyz, bad)
     assert e.value.code == cm.CM_E_INDEX_RANGE
+
+
+def test_periodic_hexahedra_parity(cm, oracle_mod, torch):
+    """Node-wrapped (fully periodic) hexahedral box with a x2-stiff non-magnetic inclusion, d = 3 displacement DOFs pinned --
+    the paper's own setting: structure, matrices, right-hand sides, ten GSPM steps (1e-9 fp64 / 1e-4 fp32)."""
+    from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD, TERM_MAGEL, TERM_ZEEMAN
+    ALL = TERM_ANIS | TERM_ZEEMAN | TERM_DEMAG | TERM_FARFIELD | TERM_MAGEL
+    mesh = inputs.hex_box((13, 12, 9), (40 * NM, 36 * NM, 26 * NM), seed_mesh=21, seed_perm=22)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (9 * NM, 8 * NM, 6 * NM))
+    dof, nd = cm.periodic_wrap(mesh.xyz, 7)
+    dof_o, nd_o = oracle_mod.periodic_wrap(mesh.xyz, 7)
+    assert nd == nd_o == 12 * 11 * 8 and np.array_equal(dof, dof_o)
+    clamp = np.zeros((nd, 3), np.uint8); clamp[7] = 1; clamp = clamp.ravel()
+    for dtype, tol, cgt, bar in (("f64", 1e-12, 1e-12, 1e-9), ("f32", 1e-5, 1e-6, 1e-4)):
+        gm = cm.Mesh(mesh.xyz, mesh.hexes, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON, dof_of_node=dof, n_dof=nd)
+        assert gm.n_nodes == nd and gm.nnz == 27 * nd
+        gs = cm.System(gm, mat2(), 1e-12, dtype, clamp, 3)
+        o = oracle_mod.Oracle(mesh, mat2(), 1e-12, clamp_dof=clamp, pin_node=3, dof_of_node=dof, n_dof=nd)
+        td = torch.float64 if dtype == "f64" else torch.float32
+        dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=td, device="cuda")
+        vtol = 1e-12 if dtype == "f64" else 2e-7
+        order = gm.get(cm.CM_GET_ORDER)
+        assert rel(gs.geometry(2), o.mL()[order]) < vtol
+        for mg, mo in ((cm.CM_MAT_K_MS, oracle_mod.MAT_K_MS), (cm.CM_MAT_K_GS1, oracle_mod.MAT_K_GS1), (cm.CM_MAT_K_MECH, oracle_mod.MAT_K_MECH)):
+            A = _to_user(gm, gs.values(mg), mg == cm.CM_MAT_K_MECH)
+            B = o.csr(mo)
+            assert abs(A - B).max() < vtol * abs(B).max(), mg
+        rng = np.random.default_rng(9)
+        live = o.live().astype(bool)
+        m = rng.normal(size=(nd, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True); m[~live] = 0
+        m = m.astype(gs.np_dtype); m64 = m.astype(np.float64)
+        u = (1e-3 * rng.normal(size=(nd, 3))).astype(gs.np_dtype)
+        p = cm.make_params(1e-12, [3e4, -1e4, 2e4], ALL)
+        assert rel(gs.field_rhs(cm.CM_RHS_MS, dev(m)).cpu().numpy(), o.rhs_ms(m64)) < tol
+        assert rel(gs.field_rhs(cm.CM_RHS_MECH, dev(m)).cpu().numpy(), o.rhs_mech(m64)) < tol
+        assert rel(gs.field_rhs(cm.CM_OUT_SIGMA, dev(m), None, dev(u), p).cpu().numpy(), o.stress_recover(u.astype(np.float64), m64)) < tol
+        assert np.abs(gm.volume_average(dev(m)) - o.volume_average(m64)).max() < (1e-13 if dtype == "f64" else 1e-6)
+        m0 = np.array([1.0, 0, 0]) + 0.1 * rng.normal(size=(nd, 3)); m0 /= np.linalg.norm(m0, axis=1, keepdims=True); m0[~live] = 0
+        mo_ = m0.copy(); Uo = np.zeros(nd); uo = np.zeros((nd, 3))
+        mg_ = torch.as_tensor(m0, dtype=td, device="cuda").contiguous()
+        Ug = torch.zeros(nd, dtype=td, device="cuda"); ug = torch.zeros((nd, 3), dtype=td, device="cuda")
+        for k in range(10):
+            io, rco = o.gspm_step(mo_, Uo, uo, 1e-12, [2e4, 0, 0], ALL, cg_tol=cgt)
+            ig, rcg = gs.gspm_step(cm.make_params(1e-12, [2e4, 0, 0], ALL, 0, cgt), mg_, Ug, ug)
+            assert rco == 0 and rcg == 0
+        assert np.abs(mg_.cpu().numpy().astype(np.float64) - mo_).max() <= bar
+    thin = inputs.hex_box((2, 4, 4), (5 * NM, 12 * NM, 12 * NM))
+    dof, nd = cm.periodic_wrap(thin.xyz, 1)
+    with pytest.raises(cm.CmError) as e:
+        cm.Mesh(thin.xyz, thin.hexes, dof_of_node=dof, n_dof=nd)
+    assert e.value.code == cm.CM_E_BADARG
