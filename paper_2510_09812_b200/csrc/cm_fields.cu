@@ -700,6 +700,7 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
     T acc[NC];
 #pragma unroll
     for (int q = 0; q < NC; q++) acc[q] = 0;
+    const double ild = 1.0 / a.ld;
     if (i < a.N) {
         for (int s = a.n2e_ptr[i]; s < a.n2e_ptr[i + 1]; s++) {
             const int e = a.n2e[s] >> 3, k = a.n2e[s] & 7;
@@ -712,7 +713,7 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
                 t[c] = a.hexes[8 * (long)e + c];
                 const long gc = a.ghexes[8 * (long)e + c];
 #pragma unroll
-                for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * gc + d] / a.ld;
+                for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * gc + d] * ild;
             }
             T e0c[8][6]; // E0 at the 8 corners (MECH, STRESS)
             if (KIND == EK_MECH || KIND == EK_STRESS) {
