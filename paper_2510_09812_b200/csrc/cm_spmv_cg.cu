@@ -14,9 +14,9 @@
 //
 // CG.  ONE cooperative launch per solve; a CTA owns a contiguous range of slices, hence of rows, for the whole
 // solve.  Per iteration k (three grid-wide barriers, the two dot products ride on two of them):
-//   C   p_k = r_k + beta p_{k-1} on the own rows (128-bit accesses);                       -> barrier
+//   C   x += alpha_{k-1} p_{k-1} (deferred: p_{k-1} is read here anyway), p_k = r_k + beta p_{k-1} on the own rows;  -> barrier
 //   A   Ap = A p_k, dot p.Ap;                                                              -> barrier, alpha
-//   B   x += alpha p, r -= alpha Ap, dot r.r;                                              -> barrier, beta
+//   B   r -= alpha Ap, dot r.r;                                                            -> barrier, beta
 // (CM_HALO selects a two-barrier variant that recomputes p on halo columns; measured slower, see below.)
 // Every CTA reduces the per-CTA partial sums in the same fixed order, so all CTAs take the same decisions and the
 // result is bit-reproducible run to run.  Dot products accumulate in fp64 in both precisions (R20).
@@ -340,65 +340,90 @@ __device__ __forceinline__ void vsq(double (&acc)[4], float4 v)
 // of 8 entries because slices hold 8 or 16 rows) plus a scalar tail.  e0 % 3 == 0 and blockDim.x * W % 3 == 0, so
 // the component served by lane j of a thread's vectors is the same in every trip: (tid * W + j) % 3.
 
-// C': pnew = r + beta pold
+// C': x += alpha_prev pold (the x update of the PREVIOUS iteration, deferred to here because pold is read anyway: one
+// vector stream less per iteration than updating x in phase B; the fma is the same, so x is bit-identical), then
+// pnew = r + beta pold
 template <typename T, int NR>
-__device__ __forceinline__ void phase_p(T *pnew, const T *pold, const T *r, long e0, long e1, const T (&beta)[NR])
-{
-    constexpr int W = VecOf<T>::W, UN = 4;
-    typedef typename VecOf<T>::V V;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    const long a1 = e0 + (e1 - e0) / W * W, nv = (a1 - e0) / W;
-    T be[W];
-#pragma unroll
-    for (int j = 0; j < W; j++) be[j] = pick<NR>(beta, NR == 3 ? (tid * W + j) % 3 : 0);
-    V *pn = reinterpret_cast<V *>(pnew + e0);
-    const V *po = reinterpret_cast<const V *>(pold + e0), *rv = reinterpret_cast<const V *>(r + e0);
-    long v = tid;
-    for (; v + (long)(UN - 1) * nt < nv; v += (long)nt * UN) {
-        V a[UN], b[UN];
-#pragma unroll
-        for (int q = 0; q < UN; q++) { a[q] = po[v + (long)q * nt]; b[q] = rv[v + (long)q * nt]; }
-#pragma unroll
-        for (int q = 0; q < UN; q++) pn[v + (long)q * nt] = vfma(be, a[q], b[q]);
-    }
-    for (; v < nv; v += nt) pn[v] = vfma(be, po[v], rv[v]);
-    for (long i = a1 + tid; i < e1; i += nt) pnew[i] = fma_t(pick<NR>(beta, NR == 3 ? (int)(i % 3) : 0), pold[i], r[i]);
-}
-
-// B: x += alpha p, r -= alpha Ap; s[c] += sum of r_new^2 per component
-template <typename T, int NR>
-__device__ __forceinline__ void phase_xr(T *x, T *r, const T *p, const T *Ap, long e0, long e1, const T (&alpha)[NR], double (&s)[3])
+__device__ __forceinline__ void phase_p(T *pnew, const T *pold, const T *r, T *x, long e0, long e1, const T (&beta)[NR],
+                                        const T (&aprev)[NR], bool upd_x)
 {
     constexpr int W = VecOf<T>::W, UN = 2;
     typedef typename VecOf<T>::V V;
     const int tid = threadIdx.x, nt = blockDim.x;
     const long a1 = e0 + (e1 - e0) / W * W, nv = (a1 - e0) / W;
-    T al[W], nal[W];
+    T be[W], al[W];
+#pragma unroll
+    for (int j = 0; j < W; j++) {
+        const int cj = NR == 3 ? (tid * W + j) % 3 : 0;
+        be[j] = pick<NR>(beta, cj); al[j] = pick<NR>(aprev, cj);
+    }
+    V *pn = reinterpret_cast<V *>(pnew + e0), *xv = reinterpret_cast<V *>(x + e0);
+    const V *po = reinterpret_cast<const V *>(pold + e0), *rv = reinterpret_cast<const V *>(r + e0);
+    long v = tid;
+    if (upd_x) {
+        for (; v + (long)(UN - 1) * nt < nv; v += (long)nt * UN) {
+            V a[UN], b[UN], c[UN];
+#pragma unroll
+            for (int q = 0; q < UN; q++) { a[q] = po[v + (long)q * nt]; b[q] = rv[v + (long)q * nt]; c[q] = xv[v + (long)q * nt]; }
+#pragma unroll
+            for (int q = 0; q < UN; q++) { xv[v + (long)q * nt] = vfma(al, a[q], c[q]); pn[v + (long)q * nt] = vfma(be, a[q], b[q]); }
+        }
+        for (; v < nv; v += nt) { const V a = po[v]; xv[v] = vfma(al, a, xv[v]); pn[v] = vfma(be, a, rv[v]); }
+        for (long i = a1 + tid; i < e1; i += nt) {
+            const int c = NR == 3 ? (int)(i % 3) : 0;
+            const T pv = pold[i];
+            x[i] = fma_t(pick<NR>(aprev, c), pv, x[i]);
+            pnew[i] = fma_t(pick<NR>(beta, c), pv, r[i]);
+        }
+    } else {
+        for (; v + (long)(UN - 1) * nt < nv; v += (long)nt * UN) {
+            V a[UN], b[UN];
+#pragma unroll
+            for (int q = 0; q < UN; q++) { a[q] = po[v + (long)q * nt]; b[q] = rv[v + (long)q * nt]; }
+#pragma unroll
+            for (int q = 0; q < UN; q++) pn[v + (long)q * nt] = vfma(be, a[q], b[q]);
+        }
+        for (; v < nv; v += nt) pn[v] = vfma(be, po[v], rv[v]);
+        for (long i = a1 + tid; i < e1; i += nt) pnew[i] = fma_t(pick<NR>(beta, NR == 3 ? (int)(i % 3) : 0), pold[i], r[i]);
+    }
+}
+
+// the x update still pending when the loop ends: x += alpha_last p_last
+template <typename T, int NR>
+__device__ __forceinline__ void phase_x_final(T *x, const T *p, long e0, long e1, const T (&alpha)[NR])
+{
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (long i = e0 + tid; i < e1; i += nt) x[i] = fma_t(pick<NR>(alpha, NR == 3 ? (int)(i % 3) : 0), p[i], x[i]);
+}
+
+// B: r -= alpha Ap; s[c] += sum of r_new^2 per component
+template <typename T, int NR>
+__device__ __forceinline__ void phase_xr(T *r, const T *Ap, long e0, long e1, const T (&alpha)[NR], double (&s)[3])
+{
+    constexpr int W = VecOf<T>::W, UN = 4;
+    typedef typename VecOf<T>::V V;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const long a1 = e0 + (e1 - e0) / W * W, nv = (a1 - e0) / W;
+    T nal[W];
     int cj[W];
     double acc[W];
 #pragma unroll
-    for (int j = 0; j < W; j++) { cj[j] = NR == 3 ? (tid * W + j) % 3 : 0; al[j] = pick<NR>(alpha, cj[j]); nal[j] = -al[j]; acc[j] = 0; }
-    V *xv = reinterpret_cast<V *>(x + e0), *rv = reinterpret_cast<V *>(r + e0);
-    const V *pv = reinterpret_cast<const V *>(p + e0), *av = reinterpret_cast<const V *>(Ap + e0);
+    for (int j = 0; j < W; j++) { cj[j] = NR == 3 ? (tid * W + j) % 3 : 0; nal[j] = -pick<NR>(alpha, cj[j]); acc[j] = 0; }
+    V *rv = reinterpret_cast<V *>(r + e0);
+    const V *av = reinterpret_cast<const V *>(Ap + e0);
     long v = tid;
     for (; v + (long)(UN - 1) * nt < nv; v += (long)nt * UN) {
-        V a[UN], b[UN], c[UN], d[UN];
+        V b[UN], d[UN];
+#pragma unroll
+        for (int q = 0; q < UN; q++) { b[q] = av[v + (long)q * nt]; d[q] = rv[v + (long)q * nt]; }
 #pragma unroll
         for (int q = 0; q < UN; q++) {
-            const long vv = v + (long)q * nt;
-            a[q] = pv[vv]; b[q] = av[vv]; c[q] = xv[vv]; d[q] = rv[vv];
-        }
-#pragma unroll
-        for (int q = 0; q < UN; q++) {
-            const long vv = v + (long)q * nt;
-            xv[vv] = vfma(al, a[q], c[q]);
             const V rn = vfma(nal, b[q], d[q]);
-            rv[vv] = rn;
+            rv[v + (long)q * nt] = rn;
             vsq(acc, rn);
         }
     }
     for (; v < nv; v += nt) {
-        xv[v] = vfma(al, pv[v], xv[v]);
         const V rn = vfma(nal, av[v], rv[v]);
         rv[v] = rn;
         vsq(acc, rn);
@@ -409,9 +434,7 @@ __device__ __forceinline__ void phase_xr(T *x, T *r, const T *p, const T *Ap, lo
         for (int q = 0; q < 3; q++) s[q] += (cj[j] == q) ? acc[j] : 0.0;
     for (long i = a1 + tid; i < e1; i += nt) {
         const int c = NR == 3 ? (int)(i % 3) : 0;
-        const T a = pick<NR>(alpha, c);
-        x[i] = fma_t(a, p[i], x[i]);
-        const T ri = fma_t(-a, Ap[i], r[i]);
+        const T ri = fma_t(-pick<NR>(alpha, c), Ap[i], r[i]);
         r[i] = ri;
         s[c] += (double)ri * (double)ri;
     }
@@ -536,6 +559,9 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
     for (int q = 0; q < NR; q++) beta[q] = 0;
     const T *pold = a.r;
     T *pnew = a.p, *pother = a.p2;
+    T aprev[NR]; // alpha of the previous iteration: its x update is applied in the next phase C' (or after the loop)
+#pragma unroll
+    for (int q = 0; q < NR; q++) aprev[q] = 0;
 
     for (int k = 0;; k++) {
         bool any = false;
@@ -551,7 +577,7 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         if (!any) break;
         // ---- C': p_k on the own rows
         TRACE(k, 0);
-        phase_p<T, NR>(pnew, pold, a.r, e0, e1, beta);
+        phase_p<T, NR>(pnew, pold, a.r, a.x, e0, e1, beta, aprev, k > 0);
         double s_pap[3] = {0, 0, 0};
         if (HALO) {
             __syncthreads();
@@ -583,9 +609,9 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
             if (!(pap[q] > 0.0)) { active[q] = false; status = CM_E_CG_BREAKDOWN; continue; }
             alpha[q] = (T)(rr[q] / pap[q]);
         }
-        // ---- B: x += alpha p, r -= alpha Ap, rr_new (alpha = 0 freezes a finished component)
+        // ---- B: r -= alpha Ap, rr_new (alpha = 0 freezes a finished component; x += alpha p is deferred to phase C')
         double snew[3] = {0, 0, 0};
-        phase_xr<T, NR>(a.x, a.r, pnew, a.Ap, e0, e1, alpha, snew);
+        phase_xr<T, NR>(a.r, a.Ap, e0, e1, alpha, snew);
         block_sum<3>(snew, red);
         if (tid == 0)
             for (int q = 0; q < 3; q++) part(1)[q] = snew[q];
@@ -597,11 +623,18 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         for (int q = 0; q < NR; q++) {
             beta[q] = active[q] ? (T)(rr_new[q] / rr[q]) : (T)0;
             if (active[q]) { rr[q] = rr_new[q]; iters[q]++; }
+            aprev[q] = alpha[q];
         }
         // rotate the p buffers: p_k becomes p_{k-1}
         T *t = (pold == a.r) ? pother : const_cast<T *>(pold);
         pold = pnew;
         pnew = t;
+    }
+    {
+        bool pending = false;
+#pragma unroll
+        for (int q = 0; q < NR; q++) pending |= aprev[q] != (T)0;
+        if (pending) phase_x_final<T, NR>(a.x, pold, e0, e1, aprev);
     }
     if (bid == 0 && tid == 0) {
         for (int q = 0; q < 3; q++) { a.out->iters[q] = 0; a.out->relres[q] = 0; }
