@@ -235,9 +235,9 @@ def run_ours(args):
             gbs = byts * args.steps / (per_class[name]["ms"] * 1e-3) / 1e9
             per_class[name].update({"algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak})
     dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
-    # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_c_cg_full.md: config 3, 21 passes per launch);
+    # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_f_cg_full.md: config 3, 21 passes per launch);
     # scaled to the average launch of this run, like `achieved`.  Only known for the captured workload.
-    ncu_bytes_per_pass = {("cg_mech", "f64"): 91.080732e9 / 21, ("cg_ms", "f64"): 14.065629e9 / 21, ("cg_gs", "f64"): 27.387826e9 / 21}
+    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.906508e9 / 21, ("cg_ms", "f64"): 14.160628e9 / 21, ("cg_gs", "f64"): 26.153006e9 / 21}
     traffic = None
     passes_per_launch = prof[dom]["cg_matrix_passes"] / max(1, prof[dom]["launches"])
     if (dom, dtype) in ncu_bytes_per_pass and not args.grid:
@@ -248,7 +248,7 @@ def run_ours(args):
             "share_of_step": prof[dom]["ms"] / ms_total,
             "algorithmic_bytes_per_matrix_pass": ab[{"cg_mech": "cg_iter_bsr3", "cg_ms": "cg_iter_csr1", "cg_gs": "cg_iter_csr3"}[dom]],
             "matrix_passes_per_launch": passes_per_launch,
-            "traffic_source": "ncu --set full dram__bytes_read+write per matrix pass (profiles/r01_c_cg_full.md) x passes per launch"}
+            "traffic_source": "ncu --set full dram__bytes_read+write per matrix pass (profiles/r01_f_cg_full.md) x passes per launch"}
 
     launches = sum(p["launches"] for p in prof.values())
     last = infos[-1]
