@@ -99,7 +99,7 @@ struct cm_mesh {
     unsigned short *d_emat = nullptr;
     // scratch for cm_volume_average
     double *d_red = nullptr;   // partials
-    void *d_tmp = nullptr;     // N x 16 x 8 bytes? (allocated lazily, see cm_volume_average)
+    void *d_tmp = nullptr;     // library-order copy of the averaged field (grown on demand by cm_volume_average)
     long tmp_bytes = 0;
     double *h_red = nullptr;   // pinned, 16 doubles
 };
