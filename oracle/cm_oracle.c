@@ -21,9 +21,16 @@
  * exact on linear fields; fields h_an, h_d, h_me = -(1/mass) dEnergy/dm by central finite
  * differences; closed-form energies of uniform states; CG against dense solves; the GSPM
  * step against the analytic macrospin solution (first order in dtau), fixed points,
- * |m| = 1 and energy decay.  Unpinned: the choice between gspm_variant 0 and 1 (R1) and
- * between the adjoint and literal magnetostatic RHS (R9) -- "parity unpinned" between
- * readings; each reading is pinned by the invariants above.
+ * |m| = 1 and energy decay.  Later rows have their own pin files: periodic node wrapping
+ * (tests/test_oracle_periodic.py: brute-force wrap, Fourier symbol of the periodic 7-point
+ * operator, Eq. 20, literal = adjoint Eq. 14 right-hand side), the hysteresis driver
+ * (tests/test_oracle_hysteresis.py: macrospin switching field), the rotated crystal frame
+ * (tests/test_oracle_rotation.py: numpy tensor rotations, <111> modulus) and linear
+ * hexahedra (tests/test_oracle_hex.py: 27-point stiffness and tensor-product mass in closed
+ * form, exactness of the 2 x 2 x 2 rule, energy gradients).
+ * Unpinned: the choice between gspm_variant 0 and 1 (R1) -- "parity unpinned" between the
+ * two readings; each is pinned by the invariants above.  The adjoint magnetostatic RHS
+ * (R9) is pinned against the paper's literal form on periodic domains, where they agree.
  */
 #include <math.h>
 #include <stdio.h>
