@@ -237,7 +237,8 @@ def run_ours(args):
     dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
     # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_f_cg_full.md: config 3, 21 passes per launch);
     # scaled to the average launch of this run, like `achieved`.  Only known for the captured workload.
-    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.906508e9 / 21, ("cg_ms", "f64"): 14.160628e9 / 21, ("cg_gs", "f64"): 26.153006e9 / 21}
+    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.906508e9 / 21, ("cg_ms", "f64"): 14.160628e9 / 21, ("cg_gs", "f64"): 26.153006e9 / 21,
+                          ("cg_mech", "f32"): 43.734836e9 / 21, ("cg_ms", "f32"): 7.856605e9 / 21, ("cg_gs", "f32"): 13.277198e9 / 21}
     traffic = None
     passes_per_launch = prof[dom]["cg_matrix_passes"] / max(1, prof[dom]["launches"])
     if (dom, dtype) in ncu_bytes_per_pass and not args.grid:
