@@ -127,7 +127,7 @@ class Oracle:
     """One mesh + material + dt, in the node order it is given (no reordering)."""
 
     def __init__(self, mesh, material, dt, clamp_dof=None, pin_node=0, dtype="f64", dof_of_node=None, n_dof=None):
-        """mesh: inputs.Mesh (tetrahedra) or inputs.HexMesh (linear hexahedra: matrices, lumped masses and volume averages only)."""
+        """mesh: inputs.Mesh (linear tetrahedra) or inputs.HexMesh (linear hexahedra, R26); dof_of_node / n_dof: periodic wrap (R23)."""
         self.dtype = dtype
         self.real = np.float64 if dtype == "f64" else np.float32
         self.L = _lib(dtype)

@@ -11,7 +11,8 @@
  *
  * Compiled twice: -DORC_F32 gives the single-precision twin (R20: matrices, geometry and
  * vectors stored in fp32; set-up quantities computed in fp64 then rounded; every
- * reduction accumulated in fp64).  OpenMP pragmas sit on independent row loops only.
+ * reduction accumulated in fp64).  OpenMP pragmas sit on independent row loops only; the
+ * dot products use fixed-order chunk partials, so results are bit-reproducible run to run.
  *
  * Pins (tests/test_oracle_pins.py): element volumes sum to the box volume; grad(phi)
  * duality; K symmetric, zero row sums, patch test, u^T K u = |a|^2 vol for linear u;
@@ -431,6 +432,47 @@ static long find_col(const oracle *o, long i, int j)
 void orc_destroy(oracle *o);
 void orc_voigt_rotation(const double *R, double *M);
 
+static int finish_matrices(oracle *o, const double *K, const double *Km, const double *Mm, const double *Kme);
+
+/* O-0 nondimensionalisation and Appendix D (R25): R (all zeros = identity) must be a
+ * proper rotation; C_sim = M C_crystal M^T (Eq. D.4, Alg. D.1 line 1).  Shared by tetrahedra and hexahedra. */
+static int setup_material(oracle *o, const orc_material *mat, double dt)
+{
+    double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
+    o->Ms = mat->Ms; o->dt = dt;
+    o->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
+    o->Kstar = mat->K1 / mu0Ms2;
+    o->dtau = mat->gamma * mat->Ms * dt;
+    o->alpha = mat->alpha;
+    o->eps1 = o->Astar * o->dtau;              /* Step 1, P:432 */
+    o->eps2 = o->alpha * o->Astar * o->dtau;   /* Step 3, P:442 */
+    o->lam100 = mat->lambda100; o->lam111 = mat->lambda111;
+    memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
+    o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
+    o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
+    double nrm = 0; for (int q = 0; q < 9; q++) nrm += mat->R[q] * mat->R[q];
+    for (int q = 0; q < 9; q++) o->R[q] = nrm == 0 ? (q % 4 == 0 ? 1.0 : 0.0) : mat->R[q];
+    double dev = 0;
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
+        double acc = 0; for (int k = 0; k < 3; k++) acc += o->R[3 * i + k] * o->R[3 * j + k];
+        dev = fmax(dev, fabs(acc - (i == j)));
+    }
+    const double *r = o->R;
+    double det = r[0] * (r[4] * r[8] - r[5] * r[7]) - r[1] * (r[3] * r[8] - r[5] * r[6]) + r[2] * (r[3] * r[7] - r[4] * r[6]);
+    if (dev > 1e-10 || det < 0) return ORC_E_BADARG;
+    o->rot = 0;
+    for (int q = 0; q < 9; q++) if (o->R[q] != (q % 4 == 0 ? 1.0 : 0.0)) o->rot = 1;
+    for (int k = 0; k < o->n_elastic; k++) {
+        const double *C = mat->C_voigt + 36 * k;
+        double M[36], MC[36];
+        if (!o->rot) { for (int q = 0; q < 36; q++) o->Cstar[36 * k + q] = C[q] / mu0Ms2; continue; }
+        orc_voigt_rotation(o->R, M);
+        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double acc = 0; for (int c = 0; c < 6; c++) acc += M[6 * a + c] * C[6 * c + b]; MC[6 * a + b] = acc; }
+        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double acc = 0; for (int c = 0; c < 6; c++) acc += MC[6 * a + c] * M[6 * b + c]; o->Cstar[36 * k + 6 * a + b] = acc / mu0Ms2; }
+    }
+    return ORC_OK;
+}
+
 /* Periodic boundary conditions: `dof` (NULL = identity) maps each of the Ng geometric nodes to one of N
  * unified degrees of freedom ("the two nodes in the pair are treated as one unified node").  Element geometry is
  * computed from the element's own corner coordinates; every nodal quantity (matrix rows, lumped masses, fields)
@@ -454,41 +496,8 @@ int orc_create_wrapped(const double *xyz_m, long Ng, const int *gtets, long Ne, 
     if (dof) for (long e = 0; e < Ne; e++) /* two corners on one DOF: the domain is a single cell wide in a periodic direction */
         for (int i = 0; i < 4; i++) for (int j = i + 1; j < 4; j++)
             if (tets[4 * e + i] == tets[4 * e + j]) { free(tets); free(o); return ORC_E_BADARG; }
-    /* O-0 nondimensionalisation */
-    double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
-    o->Ms = mat->Ms; o->dt = dt;
-    o->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
-    o->Kstar = mat->K1 / mu0Ms2;
-    o->dtau = mat->gamma * mat->Ms * dt;
-    o->alpha = mat->alpha;
-    o->eps1 = o->Astar * o->dtau;              /* Step 1, P:432 */
-    o->eps2 = o->alpha * o->Astar * o->dtau;   /* Step 3, P:442 */
-    o->lam100 = mat->lambda100; o->lam111 = mat->lambda111;
-    memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
-    o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
-    o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
-    {   /* App. D: R (all zeros = identity) must be a proper rotation; C_sim = M C_crystal M^T (Eq. D.4, Alg. D.1 line 1) */
-        double nrm = 0; for (int q = 0; q < 9; q++) nrm += mat->R[q] * mat->R[q];
-        for (int q = 0; q < 9; q++) o->R[q] = nrm == 0 ? (q % 4 == 0 ? 1.0 : 0.0) : mat->R[q];
-        double dev = 0;
-        for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
-            double acc = 0; for (int k = 0; k < 3; k++) acc += o->R[3 * i + k] * o->R[3 * j + k];
-            dev = fmax(dev, fabs(acc - (i == j)));
-        }
-        const double *r = o->R;
-        double det = r[0] * (r[4] * r[8] - r[5] * r[7]) - r[1] * (r[3] * r[8] - r[5] * r[6]) + r[2] * (r[3] * r[7] - r[4] * r[6]);
-        if (dev > 1e-10 || det < 0) { free(tets); free(o->Cstar); free(o); return ORC_E_BADARG; }
-        o->rot = 0;
-        for (int q = 0; q < 9; q++) if (o->R[q] != (q % 4 == 0 ? 1.0 : 0.0)) o->rot = 1;
-    }
-    for (int k = 0; k < o->n_elastic; k++) {
-        const double *C = mat->C_voigt + 36 * k;
-        double M[36], MC[36];
-        if (!o->rot) { for (int q = 0; q < 36; q++) o->Cstar[36 * k + q] = C[q] / mu0Ms2; continue; }
-        orc_voigt_rotation(o->R, M);
-        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double acc = 0; for (int c = 0; c < 6; c++) acc += M[6 * a + c] * C[6 * c + b]; MC[6 * a + b] = acc; }
-        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double acc = 0; for (int c = 0; c < 6; c++) acc += MC[6 * a + c] * M[6 * b + c]; o->Cstar[36 * k + 6 * a + b] = acc / mu0Ms2; }
-    }
+    double ld = mat->length_scale;
+    if (setup_material(o, mat, dt)) { free(tets); free(o->Cstar); free(o); return ORC_E_BADARG; }
 
     o->x = (double *)malloc((size_t)Ng * 3 * sizeof(double));
     o->tet = tets;
@@ -594,29 +603,8 @@ int orc_create_wrapped(const double *xyz_m, long Ng, const int *gtets, long Ne, 
             }
         }
     }
-    o->K = (real *)malloc((size_t)nnz * sizeof(real)); o->Kms = (real *)malloc((size_t)nnz * sizeof(real));
-    o->Km = (real *)malloc((size_t)nnz * sizeof(real)); o->Mm = (real *)malloc((size_t)nnz * sizeof(real));
-    o->Kgs1 = (real *)malloc((size_t)nnz * sizeof(real)); o->Kgs2 = (real *)malloc((size_t)nnz * sizeof(real));
-    if (Kme) { o->Kmech = (real *)malloc((size_t)nnz * 9 * sizeof(real)); o->Kmech_free = (real *)malloc((size_t)nnz * 9 * sizeof(real)); }
-    for (long i = 0; i < N; i++)
-        for (long q = o->rowptr[i]; q < o->rowptr[i + 1]; q++) {
-            long j = o->col[q];
-            o->K[q] = (real)K[q]; o->Km[q] = (real)Km[q]; o->Mm[q] = (real)Mm[q];
-            /* constraints as the symmetric projection P A P + (I-P)  (R11) */
-            double kms = K[q];
-            if (i == o->pin || j == o->pin) kms = (i == j) ? 1.0 : 0.0;
-            o->Kms[q] = (real)kms;
-            /* K^GS(eps) = M_m + eps K_m, identity rows on dead nodes (R12) */
-            double dead = (i == j && !o->live[i]) ? 1.0 : 0.0;
-            o->Kgs1[q] = (real)(Mm[q] + o->eps1 * Km[q] + dead);
-            o->Kgs2[q] = (real)(Mm[q] + o->eps2 * Km[q] + dead);
-            if (Kme) for (int r = 0; r < 3; r++) for (int s = 0; s < 3; s++) {
-                double v = Kme[9 * q + 3 * r + s];
-                o->Kmech_free[9 * q + 3 * r + s] = (real)v;
-                if (o->clamp[3 * i + r] || o->clamp[3 * j + s]) v = (i == j && r == s) ? 1.0 : 0.0;
-                o->Kmech[9 * q + 3 * r + s] = (real)v;
-            }
-        }
+    rc = finish_matrices(o, K, Km, Mm, Kme);
+    if (rc) { free(K); free(Km); free(Mm); free(Kme); orc_destroy(o); return rc; }
     free(K); free(Km); free(Mm); free(Kme);
     *out = o;
     return ORC_OK;
@@ -629,7 +617,8 @@ int orc_create(const double *xyz_m, long N, const int *tets, long Ne, const ucha
     return orc_create_wrapped(xyz_m, N, tets, Ne, magnetic, elastic_id, NULL, N, mat, dt, clamp_dof, pin_node, out);
 }
 
-/* round the fp64 sums once (R20) and apply the constraints as P A P + (I - P) (R11, R12) -- as in orc_create */
+/* round the fp64 sums once (R20); constraints as the symmetric projection P A P + (I - P) (R11);
+ * K^GS(eps) = M_m + eps K_m with identity rows on dead nodes (R12) */
 static int finish_matrices(oracle *o, const double *K, const double *Km, const double *Mm, const double *Kme)
 {
     long N = o->N, nnz = o->nnz;
@@ -668,9 +657,8 @@ static int finish_matrices(oracle *o, const double *K, const double *Km, const d
  * integrated with the 2 x 2 x 2 Gauss rule (points +-1/sqrt 3, unit weights; Eq. 17's |J(e,p)| w_p):
  *   K_ab = sum_p |J_p| grad phi_a . grad phi_b,  M_ab = sum_p |J_p| phi_a phi_b,  K^mech_ab = sum_p |J_p| B_a^T C B_b,
  *   grad phi_a = J^-T grad_xi phi_a,  J = sum_a x_a (x) grad_xi phi_a.
- * This build covers the MATRICES of Eq. 12 (all of K^ms, K^GS, M, K^mech with their constraints), the lumped masses
- * int phi_a and the volume average of Eq. 17 -- the systems of the paper's CG benchmark (Fig. 2b-d); the element-wise
- * right-hand sides of the GSPM step stay tetrahedral. */
+ * Covered: the matrices of Eq. 12 (K^ms, K^GS, M, K^mech with their constraints), the lumped masses int phi_a, the
+ * volume average of Eq. 17, and every element-wise right-hand side and recovered field of the GSPM step (hex_* below). */
 static void hex_gauss_point(const double *X /* 8 x 3 */, int p, double *detJ, double phi[8], double g[8][3])
 {
     const double q = 0.57735026918962576451; /* 1/sqrt(3) */
@@ -711,19 +699,8 @@ int orc_create_hex(const double *xyz_m, long Ng, const int *hexes, long Ne, cons
     oracle *o = (oracle *)calloc(1, sizeof(oracle));
     if (!o) return ORC_E_ALLOC;
     o->N = N; o->Ne = Ne; o->nen = 8;
-    double ld = mat->length_scale, mu0Ms2 = MU0 * mat->Ms * mat->Ms;
-    o->Ms = mat->Ms; o->dt = dt;
-    o->Astar = 2.0 * mat->Aex / (mu0Ms2 * ld * ld);
-    o->Kstar = mat->K1 / mu0Ms2;
-    o->dtau = mat->gamma * mat->Ms * dt;
-    o->alpha = mat->alpha;
-    o->eps1 = o->Astar * o->dtau; o->eps2 = o->alpha * o->Astar * o->dtau;
-    o->lam100 = mat->lambda100; o->lam111 = mat->lambda111;
-    memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
-    for (int q = 0; q < 9; q++) o->R[q] = (q % 4 == 0);
-    o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
-    o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
-    for (int q = 0; q < 36 * o->n_elastic; q++) o->Cstar[q] = mat->C_voigt[q] / mu0Ms2;
+    double ld = mat->length_scale;
+    if (setup_material(o, mat, dt)) { free(o->Cstar); free(o); return ORC_E_BADARG; }   /* App. D applies to hexahedra too */
     o->x = (double *)malloc((size_t)Ng * 3 * sizeof(double));
     o->hex = (int *)malloc((size_t)Ne * 8 * sizeof(int));
     o->ghex = (int *)malloc((size_t)Ne * 8 * sizeof(int));
@@ -899,11 +876,24 @@ int orc_spmv(const oracle *o, int id, const void *x, void *y)
     return ORC_OK;
 }
 
+/* Fixed-order dot product: partial sums over chunks of DOT_CHUNK consecutive entries (each summed in index order),
+ * then the partials added in index order.  The result does not depend on the number of threads or on scheduling,
+ * so two runs of the oracle are bit-identical. */
+#define DOT_CHUNK 4096
 static double dot(long n, const real *a, const real *b, int stride, int comp)
 {
+    long nch = (n + DOT_CHUNK - 1) / DOT_CHUNK;
+    double *part = (double *)malloc((size_t)(nch > 0 ? nch : 1) * sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (long c = 0; c < nch; c++) {
+        long i1 = (c + 1) * DOT_CHUNK < n ? (c + 1) * DOT_CHUNK : n;
+        double s = 0;
+        for (long i = c * DOT_CHUNK; i < i1; i++) s += (double)a[i * stride + comp] * (double)b[i * stride + comp];
+        part[c] = s;
+    }
     double s = 0;
-#pragma omp parallel for reduction(+ : s) schedule(static)
-    for (long i = 0; i < n; i++) s += (double)a[i * stride + comp] * (double)b[i * stride + comp];
+    for (long c = 0; c < nch; c++) s += part[c];
+    free(part);
     return s;
 }
 

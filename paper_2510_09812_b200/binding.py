@@ -7,15 +7,13 @@ no CUDA device is present, the calls fail loudly.
 from __future__ import annotations
 
 import ctypes as C
-import os
 from pathlib import Path
 from typing import Optional
 
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-# CUPYMAG_B200_LIB points at another build of the same library (e.g. one compiled with different tuning macros)
-LIB_PATH = Path(os.environ.get("CUPYMAG_B200_LIB", _HERE / "libcupymag_b200.so"))
+LIB_PATH = _HERE / "libcupymag_b200.so"
 
 CM_F64, CM_F32 = 0, 1
 CM_REORDER_NONE, CM_REORDER_MORTON, CM_REORDER_RCM = 0, 1, 2

@@ -29,7 +29,7 @@ def needs_build() -> bool:
 
 def build(force: bool = False, verbose: bool = False, defines: tuple = (), out: Path | None = None) -> Path:
     """Compiles csrc/*.cu and links the shared library.  `defines` (e.g. ("CM_U_CSR1=4",)) and `out` build a tuning
-    variant beside the default library; load it with CUPYMAG_B200_LIB=<out>."""
+    variant beside the default library (set `binding.LIB_PATH` before the first call to load it)."""
     if out is None and not defines and not force and not needs_build():
         return LIB
     lib = Path(out) if out is not None else LIB

@@ -17,7 +17,6 @@
 //   C   x += alpha_{k-1} p_{k-1} (deferred: p_{k-1} is read here anyway), p_k = r_k + beta p_{k-1} on the own rows;  -> barrier
 //   A   Ap = A p_k, dot p.Ap;                                                              -> barrier, alpha
 //   B   r -= alpha Ap, dot r.r;                                                            -> barrier, beta
-// (CM_HALO selects a two-barrier variant that recomputes p on halo columns; measured slower, see below.)
 // Every CTA reduces the per-CTA partial sums in the same fixed order, so all CTAs take the same decisions and the
 // result is bit-reproducible run to run.  Dot products accumulate in fp64 in both precisions (R20).
 #include <cooperative_groups.h>
@@ -48,19 +47,6 @@ template <int MODE> struct ModeTraits;
 #endif
 #ifndef CM_U_BSR3
 #define CM_U_BSR3 2
-#endif
-#ifndef CM_HALO
-// bit m set: the CG of mode m recomputes p = r + beta p_old on the columns outside the CTA's own rows instead of
-// waiting for their owners (two grid barriers per iteration instead of three).  Measured on B200 at 3M nodes, fp64,
-// algorithmic GB/s with / without: K^mech 5966 / 6185, K^ms 5020 / 6509, K^GS (3 rhs) 3868 / 4816 -- the extra
-// gather and the range test in the inner loop cost more than the ~3 us barrier, so it is off.
-#define CM_HALO 0
-#endif
-#ifndef CM_PIPELINE
-// bit m set: mode m issues the next batch's streaming loads before the current batch's gathers (two register
-// buffers).  Measured on B200 at 3M nodes: no gain for any mode (fp64 SpMV 91 % vs 95 % of the copy peak for CSR1,
-// register spills for BSR3), so it is off; the 24 resident warps per SM hide the gather latency by themselves.
-#define CM_PIPELINE 0
 #endif
 template <> struct ModeTraits<MODE_CSR1> { static constexpr int NC = 1, NR = 1, NV = 1, C = CM_C_SCALAR, U = CM_U_CSR1; };
 template <> struct ModeTraits<MODE_CSR3> { static constexpr int NC = 3, NR = 3, NV = 1, C = CM_C_SCALAR, U = CM_U_CSR3; };
@@ -134,57 +120,14 @@ __device__ __forceinline__ V pick(const V (&a)[NR], int c)
     return r;
 }
 
-#ifndef CM_GATHER2
-// 1: gather the three words of a node with one aligned two-word load plus one word instead of three loads.  Measured on
-// B200 at 3M nodes (ms with / without): 3-rhs SpMV fp64 0.172 / 0.155, 3-rhs CG (3 iterations) 1.27 / 1.07, block SpMV
-// 0.556 / 0.550 -- the selects and the misaligned halves cost more than the saved request, so it is off.
-#define CM_GATHER2 0
-#endif
-template <typename T> struct Pair;
-template <> struct Pair<double> { typedef double2 V; };
-template <> struct Pair<float> { typedef float2 V; };
-
-// Where the multiplied vector comes from.  Plain: x.  Fused (CG): p_k = x on the rows [own0, own1) the CTA has
-// already updated, fma(beta, pold, r) elsewhere.
-template <typename T, int MODE, bool FUSED>
-struct XSource {
-    const T *x;
-    const T *pold, *r;
-    T beta[ModeTraits<MODE>::NR];
-    int own0, own1;
-};
-
-template <typename T, int MODE, bool FUSED>
-__device__ __forceinline__ void fetch(const XSource<T, MODE, FUSED> &X, int col, T (&out)[ModeTraits<MODE>::NC])
+// x[col] for all NC components of a node
+template <typename T, int MODE>
+__device__ __forceinline__ void fetch(const T *__restrict__ x, int col, T (&out)[ModeTraits<MODE>::NC])
 {
-    constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR;
+    constexpr int NC = ModeTraits<MODE>::NC;
     const long o = (long)col * NC;
-    if (!FUSED) {
-        if (NC == 3 && CM_GATHER2) {
-            // three consecutive words at word offset 3 col: one aligned two-word load plus one word, branch-free.
-            // col even: {x0, x1} is aligned, x2 alone;  col odd: x0 alone, {x1, x2} is aligned.
-            typedef typename Pair<T>::V V2;
-            const int odd = col & 1;
-            const V2 v = *reinterpret_cast<const V2 *>(X.x + o + odd);
-            const T w = X.x[o + 2 - 2 * odd];
-            out[0] = odd ? w : v.x;
-            out[1] = odd ? v.x : v.y;
-            out[NC - 1] = odd ? v.y : w;
-        } else {
 #pragma unroll
-            for (int c = 0; c < NC; c++) out[c] = X.x[o + c];
-        }
-    } else {
-        // branch-free: one unconditional load (own: p_k, halo: r_k) and one predicated load (halo: p_{k-1})
-        const bool own = col >= X.own0 && col < X.own1;
-        const T *a = own ? X.x : X.r;
-#pragma unroll
-        for (int c = 0; c < NC; c++) {
-            const T av = a[o + c];
-            const T pv = own ? (T)0 : X.pold[o + c];
-            out[c] = own ? av : fma_t(X.beta[NR == 3 ? c : 0], pv, av);
-        }
-    }
+    for (int c = 0; c < NC; c++) out[c] = x[o + c];
 }
 
 // Batches in flight per warp.  The fp32 block matrix streams half the bytes per element, so it takes twice the batches
@@ -228,12 +171,11 @@ __device__ __forceinline__ void load_batch(const MatView<T> &A, const Cursor &c,
 }
 
 // y = A x on the slices [u0, u1) of this CTA (warp w takes u0 + w, u0 + w + nwarps, ...); optionally accumulates
-// dot[c] += y.x over the rows written (x must then be valid on those rows: the own range when FUSED).
-template <typename T, int MODE, bool FUSED, bool DOT>
-__device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T, MODE, FUSED> &X, T *y, int u0, int u1, double (&dot)[3])
+// dot[c] += y.x over the rows written.
+template <typename T, int MODE, bool DOT>
+__device__ __forceinline__ void spmv_units(const MatView<T> &A, const T *__restrict__ x, T *y, int u0, int u1, double (&dot)[3])
 {
     constexpr int NC = ModeTraits<MODE>::NC, C = ModeTraits<MODE>::C, U = batch_u<T, MODE>();
-    constexpr bool PIPE = (CM_PIPELINE >> MODE) & 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int rl = lane % C, jl = lane / C;
     const unsigned long long pol = policy_evict_first();
@@ -246,7 +188,7 @@ __device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T,
     // extent of the slice after the current one, fetched one slice ahead
     int n0 = 0, n1 = 0;
     if (cur.s + nw < u1) { n0 = __ldg(A.sp + cur.s + nw); n1 = __ldg(A.sp + cur.s + nw + 1); }
-    Batch<T, MODE> Bc, Bn;
+    Batch<T, MODE> Bc;
     load_batch<T, MODE>(A, cur, lane, pol, Bc);
     T acc[NC];
 #pragma unroll
@@ -261,14 +203,13 @@ __device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T,
             if (nxt.s + nw < u1) { n0 = __ldg(A.sp + nxt.s + nw); n1 = __ldg(A.sp + nxt.s + nw + 1); }
         }
         const bool more = nxt.s < u1;
-        if (PIPE && more) load_batch<T, MODE>(A, nxt, lane, pol, Bn);
         // ---- current batch: dependent gathers, multiply-accumulate in column order
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const int e = cur.it + 32 * u + lane;
             if (e < cur.L) {
                 T xv[NC];
-                fetch<T, MODE, FUSED>(X, Bc.col[u], xv);
+                fetch<T, MODE>(x, Bc.col[u], xv);
                 if (MODE == MODE_BSR3) {
                     acc[0] += Bc.v[u][0] * xv[0] + Bc.v[u][1] * xv[1] + Bc.v[u][2] * xv[2];
                     acc[1] += Bc.v[u][3] * xv[0] + Bc.v[u][4] * xv[1] + Bc.v[u][5] * xv[2];
@@ -292,13 +233,13 @@ __device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T,
                     if (jl < 3) {
                         const T a = jl == 0 ? acc[0] : (jl == 1 ? acc[1] : acc[2]);
                         y[3 * row + jl] = a;
-                        if (DOT) dot[0] += (double)a * (double)X.x[3 * row + jl];
+                        if (DOT) dot[0] += (double)a * (double)x[3 * row + jl];
                     }
                 } else if (jl == 0) {
 #pragma unroll
                     for (int c = 0; c < NC; c++) {
                         y[NC * row + c] = acc[c];
-                        if (DOT) dot[c] += (double)acc[c] * (double)X.x[NC * row + c];
+                        if (DOT) dot[c] += (double)acc[c] * (double)x[NC * row + c];
                     }
                 }
             }
@@ -307,8 +248,7 @@ __device__ __forceinline__ void spmv_units(const MatView<T> &A, const XSource<T,
         }
         if (!more) break;
         cur = nxt;
-        if (PIPE) Bc = Bn;
-        else load_batch<T, MODE>(A, cur, lane, pol, Bc);
+        load_batch<T, MODE>(A, cur, lane, pol, Bc);
     }
 }
 
@@ -317,10 +257,8 @@ __global__ void __launch_bounds__(CM_NT, 2) spmv_kernel(MatView<T> A, const T *x
 {
     int u0, u1;
     cta_units(A.nslices, blockIdx.x, gridDim.x, u0, u1);
-    XSource<T, MODE, false> X;
-    X.x = x;
     double dot[3] = {0, 0, 0};
-    spmv_units<T, MODE, false, false>(A, X, y, u0, u1, dot);
+    spmv_units<T, MODE, false>(A, x, y, u0, u1, dot);
 }
 
 // --------------------------------------------------------------------------------------------------
@@ -451,30 +389,6 @@ __device__ __forceinline__ void phase_xr(T *r, const T *Ap, long e0, long e1, co
 // --------------------------------------------------------------------------------------------------
 // persistent CG
 // --------------------------------------------------------------------------------------------------
-#ifdef CM_TRACE
-// tuning aid (not built by default): per-CTA phase time stamps of the first CM_TRACE_IT iterations
-constexpr int CM_TRACE_IT = 8;
-__device__ unsigned long long cm_trace_buf[2048 * CM_TRACE_IT * 4];
-__device__ __forceinline__ unsigned long long gtime()
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-__device__ __forceinline__ unsigned smid()
-{
-    unsigned s;
-    asm volatile("mov.u32 %0, %%smid;" : "=r"(s));
-    return s;
-}
-#define TRACE(k, slot) if (threadIdx.x == 0 && (k) < CM_TRACE_IT) cm_trace_buf[((long)blockIdx.x * CM_TRACE_IT + (k)) * 4 + (slot)] = (slot) == 3 ? (unsigned long long)smid() : gtime()
-extern "C" int cm_debug_trace(unsigned long long *host_out, long n)
-{
-    return cudaMemcpyFromSymbol(host_out, cm_trace_buf, n * sizeof(unsigned long long)) == cudaSuccess ? 0 : -1;
-}
-#else
-#define TRACE(k, slot)
-#endif
 template <typename T>
 struct CgArgs {
     MatView<T> A;
@@ -507,7 +421,6 @@ template <typename T, int MODE>
 __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
 {
     constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR, C = ModeTraits<MODE>::C;
-    constexpr bool HALO = (CM_HALO >> MODE) & 1;
     __shared__ double red[6 * 32];
     cg::grid_group grid = cg::this_grid();
     const int tid = threadIdx.x, nt = blockDim.x, nb = gridDim.x, bid = blockIdx.x;
@@ -522,11 +435,7 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
     double nodot[3] = {0, 0, 0};
 
     // ---- r = b - A x0, rr, bb
-    {
-        XSource<T, MODE, false> X0;
-        X0.x = a.x;
-        spmv_units<T, MODE, false, false>(a.A, X0, a.Ap, u0, u1, nodot);
-    }
+    spmv_units<T, MODE, false>(a.A, a.x, a.Ap, u0, u1, nodot);
     __syncthreads(); // Ap of the CTA's rows was written by other warps
     {
         double srr = 0, sbb = 0;
@@ -584,29 +493,14 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         }
         if (!any) break;
         // ---- C': p_k on the own rows
-        TRACE(k, 0);
         phase_p<T, NR>(pnew, pold, a.r, a.x, e0, e1, beta, aprev, k > 0);
         double s_pap[3] = {0, 0, 0};
-        if (HALO) {
-            __syncthreads();
-            // ---- A: Ap = A p_k (halo columns recomputed from r_k, p_{k-1}), pAp
-            XSource<T, MODE, true> X;
-            X.x = pnew; X.pold = pold; X.r = a.r; X.own0 = own0; X.own1 = own1;
-#pragma unroll
-            for (int q = 0; q < NR; q++) X.beta[q] = beta[q];
-            spmv_units<T, MODE, true, true>(a.A, X, a.Ap, u0, u1, s_pap);
-        } else {
-            grid.sync(); // textbook loop: p_k visible everywhere before the product
-            XSource<T, MODE, false> X;
-            X.x = pnew;
-            spmv_units<T, MODE, false, true>(a.A, X, a.Ap, u0, u1, s_pap);
-        }
+        grid.sync(); // textbook loop: p_k visible everywhere before the product
+        spmv_units<T, MODE, true>(a.A, pnew, a.Ap, u0, u1, s_pap);
         block_sum<3>(s_pap, red);
         if (tid == 0)
             for (int q = 0; q < 3; q++) part(0)[q] = s_pap[q];
-        TRACE(k, 1);
         grid.sync();
-        TRACE(k, 3);
         double pap[NR];
         grid_sum<NR>(a.partial, 0, pap, red);
         T alpha[NR];
@@ -623,7 +517,6 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         block_sum<3>(snew, red);
         if (tid == 0)
             for (int q = 0; q < 3; q++) part(1)[q] = snew[q];
-        TRACE(k, 2);
         grid.sync();
         double rr_new[NR];
         grid_sum<NR>(a.partial, 1, rr_new, red);

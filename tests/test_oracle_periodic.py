@@ -187,3 +187,38 @@ def test_periodic_gspm_fixed_point_energy_decay_unit_length(orc):
         assert np.abs(np.linalg.norm(m, axis=1) - 1).max() <= 4 * np.finfo(float).eps
         E.append(o.energy(m, U, u, hext, terms))
     assert all(b < a for a, b in zip(E, E[1:])), E
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_plane_wave_demag_chain_closed_form(orc, d):
+    """The SOLVED magnetostatic chain (right-hand side -> CG on the pinned K^ms -> gradient recovery, O-3 items 2-3)
+    against a closed form.  Fully periodic un-jittered Kuhn grid, m~ = a cos(k x_d) with k = 2 pi n / L_d.  Then m_h
+    depends on x_d only, the nodal basis functions of a lattice plane sum to the 1-D hat function, and every node's
+    support is point-symmetric, so all three steps collapse to 1-D central differences:
+        b_i = a_d (V_cell / h_d) sin(k h_d) sin(k x_i),   K U = (V_cell / h_d^2)(2 - 2 cos k h_d) U,
+        recovered dU/dx_d = (U_{+} - U_{-}) / (2 h_d)
+    =>  h_d = -e_d a_d cos^2(k h_d / 2) cos(k x_d)   (continuum: -k (k.a)/|k|^2 cos(k.x); mbar = 0)."""
+    grid, box = (9, 7, 6), (24 * NM, 15 * NM, 10 * NM)
+    mesh, dof, nd, o = _periodic(orc, grid, box, 7, jitter=0.0, pin_node=11)
+    L = np.array(box) / 1e-9
+    h = L / (np.array(grid) - 1)
+    x = np.zeros((nd, 3)); x[dof] = np.where(mesh.xyz / 1e-9 >= L - 1e-9, 0.0, mesh.xyz / 1e-9)
+    a = np.array([0.7, -0.4, 0.55])
+    n = 2 if d == 0 else 1
+    k = 2 * np.pi * n / L[d]
+    m = np.outer(np.cos(k * x[:, d]), a)
+    mbar = o.volume_average(m)
+    assert np.abs(mbar).max() < 1e-14
+    b = o.rhs_ms(m, mbar)
+    b_exact = a[d] * h.prod() / h[d] * np.sin(k * h[d]) * np.sin(k * x[:, d])
+    keep = np.arange(nd) != 11
+    assert b[11] == 0.0 and np.abs(b[keep] - b_exact[keep]).max() <= 1e-13 * np.abs(b_exact).max()
+    U, it, res, rc = o.cg(orc.MAT_K_MS, b, tol=1e-14)
+    assert rc == 0 and it > 0
+    A = a[d] * h[d] / 2 / np.tan(k * h[d] / 2)
+    U_exact = A * (np.sin(k * x[:, d]) - np.sin(k * x[11, d]))
+    assert np.abs(U - U_exact).max() <= 1e-11 * abs(A)
+    hd, gm = o.demag_field(U, mbar, TERM_DEMAG | TERM_FARFIELD)
+    assert np.abs(gm).max() <= 1e-13
+    hd_exact = np.zeros((nd, 3)); hd_exact[:, d] = -a[d] * np.cos(k * h[d] / 2) ** 2 * np.cos(k * x[:, d])
+    assert np.abs(hd - hd_exact).max() <= 1e-11 * abs(a[d])

@@ -684,3 +684,41 @@ def test_f32_twin_close_to_f64(orc, oi):
     assert rel(o32.rhs_ms(m), o64.rhs_ms(m)) < 1e-5
     assert rel(o32.rhs_mech(m), o64.rhs_mech(m)) < 1e-5
     assert np.allclose(o32.volume_average(m), o64.volume_average(m), atol=1e-7)
+
+
+_DET_SCRIPT = r"""
+import hashlib, sys
+import numpy as np
+sys.path.insert(0, {root!r})
+import oracle
+from paper_2510_09812_b200 import inputs
+nm = 1e-9
+mesh = inputs.kuhn_box((13, 11, 7), (40 * nm, 34 * nm, 20 * nm), seed_mesh=21, seed_perm=22)
+mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * nm,) * 3)
+C = inputs.isotropic_voigt(200e9, 0.3)
+mat = inputs.Material(C_voigt=np.stack([C, 2 * C]))
+o = oracle.Oracle(mesh, mat, 1e-12, clamp_dof=inputs.clamp_bottom(mesh))
+m = inputs.init_m_noisy_x(mesh, 23); U = np.zeros(o.N); u = np.zeros((o.N, 3))
+its = []
+for _ in range(2):
+    info, rc = o.gspm_step(m, U, u, 1e-12, [2e4, 0, 0], 31, cg_tol=1e-7)
+    its += [info.it_ms, info.it_mech] + list(info.it_gs)
+E = o.energy(m, U, u, [0, 0, 0], 31)
+print(hashlib.sha256(m.tobytes() + U.tobytes() + u.tobytes() + np.float64(E).tobytes()).hexdigest(), its)
+"""
+
+
+def test_oracle_is_bit_reproducible_across_runs_and_thread_counts():
+    """The oracle's only reductions across threads are the CG dot products; they use fixed-order chunk partials, so
+    two runs -- and runs with different OpenMP thread counts -- give bit-identical states, energies and CG counts."""
+    import os
+    import subprocess
+    import sys
+    root = str(Path(__file__).resolve().parent.parent)
+    outs = []
+    for nt in ("8", "8", "3", "1"):
+        env = dict(os.environ, OMP_NUM_THREADS=nt)
+        r = subprocess.run([sys.executable, "-c", _DET_SCRIPT.format(root=root)], capture_output=True, text=True, env=env, timeout=600)
+        assert r.returncode == 0, r.stderr
+        outs.append(r.stdout.strip())
+    assert len(set(outs)) == 1, outs
