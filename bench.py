@@ -169,7 +169,7 @@ def run_ours(args):
     u = torch.zeros((N, 3), dtype=td, device=dev)
 
     def params(k):
-        return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, 0, CG_TOL, 100000, args.fixed_iters)
+        return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, args.variant, CG_TOL, 100000, args.fixed_iters)
 
     def barrier():
         torch.cuda.synchronize()
@@ -260,7 +260,10 @@ def run_ours(args):
                        "n_tets": mesh.n_tets, "nnz": nnz, "dt_ps": cfg.dt * 1e12, "cg_tol": CG_TOL, "cg_fixed_iters": args.fixed_iters,
                        "terms": "exchange+anis+zeeman+demag+farfield+magel", "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2 (matrices 3.2 GB fp64 per solve)", "setup_s": t_setup,
-                       "cg_iters_last_step": {"ms": last.it_ms, "mech": last.it_mech, "gs": list(last.it_gs)}},
+                       "gspm_variant": args.variant,
+                       "cg_iters_last_step": {"ms": last.it_ms, "mech": last.it_mech, "gs": list(last.it_gs)},
+                       "cg_iters_per_step": [[i.it_ms, i.it_mech, int(sum(i.it_gs))] for i in infos],
+                       "mean_dm_per_step": [float(i.mean_dm) for i in infos]},
             "clocks": clocks.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "steps": e2e_steps},
@@ -281,6 +284,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--fixed-iters", type=int, default=-1, help="run every CG solve for exactly this many iterations")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1], help="Alg. B.1 Step 2: 0 as printed (P:438), 1 fully Gauss-Seidel (R1)")
     ap.add_argument("--grid", default="", help="override the node grid, e.g. 81x81x21 (not the headline workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -77,7 +77,7 @@ def _lib(dtype: str):
         L.orc_nnz.restype = C.c_long
         for name in ("orc_scalar", "orc_nnz", "orc_get", "orc_get_values", "orc_spmv", "orc_cg", "orc_volume_average",
                      "orc_rhs_ms", "orc_demag_field", "orc_rhs_mech", "orc_stress_recover", "orc_field", "orc_energy",
-                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run", "orc_voigt_rotation", "orc_create_hex"):
+                     "orc_gspm_step", "orc_rhs_gs", "orc_destroy", "orc_create_wrapped", "orc_periodic_wrap", "orc_hysteresis_run", "orc_voigt_rotation", "orc_create_hex", "orc_cg_pc", "orc_set_cg_history"):
             getattr(L, name).argtypes = None
         _libs[dtype] = L
     return _libs[dtype]
@@ -228,6 +228,25 @@ class Oracle:
         rc = self.L.orc_cg(self.h, C.c_int(mat), _p(b), _p(x), C.c_double(tol), C.c_int(maxiter), C.c_int(fixed),
                            C.byref(it), C.byref(res))
         return x, it.value, res.value, rc
+
+    def cg_pc(self, mat, b, x0=None, tol=1e-7, maxiter=100000, fixed=-1, precond=1):
+        """Jacobi-preconditioned CG (precond = 1; 0 = plain CG through the same routine)."""
+        b = self._r(b)
+        x = np.zeros_like(b) if x0 is None else self._r(x0).copy()
+        it = C.c_int(); res = C.c_double()
+        rc = self.L.orc_cg_pc(self.h, C.c_int(mat), _p(b), _p(x), C.c_double(tol), C.c_int(maxiter), C.c_int(fixed),
+                              C.c_int(precond), C.byref(it), C.byref(res))
+        return x, it.value, res.value, rc
+
+    def cg_history(self, mat, b, x0=None, tol=1e-7, maxiter=100000, precond=0, cap=1 << 16):
+        """(x, iters, history): history[k] = ||r_k|| / ||b|| before iteration k, k = 0 .. iters."""
+        hist = np.zeros(cap); n = C.c_int()
+        self.L.orc_set_cg_history(_p(hist), C.c_int(cap), C.byref(n))
+        try:
+            x, it, res, rc = self.cg_pc(mat, b, x0, tol, maxiter, -1, precond)
+        finally:
+            self.L.orc_set_cg_history(None, C.c_int(0), None)
+        return x, it, hist[:n.value].copy()
 
     def volume_average(self, g):
         g = self._r(g)

@@ -897,55 +897,94 @@ static double dot(long n, const real *a, const real *b, int stride, int comp)
     return s;
 }
 
-/* Textbook unpreconditioned CG (O-4).  Stop when ||r|| < tol ||b||
- * (recurrence residual), tested before each iteration; fixed >= 0 runs exactly `fixed`
- * iterations.  Dots in fp64; alpha, beta formed in fp64 and cast to the vector type. */
-static int cg(const oracle *o, int id, const real *b, real *x, int stride, int comp, double tol, int maxiter,
-              int fixed, int *iters, double *relres)
+/* Optional residual history of the solves that follow: hist[k] = ||r_k|| / ||b|| of the recurrence residual before
+ * iteration k (k = 0 .. iters), for at most cap entries; *n = entries written by the LAST solve.  NULL switches it off. */
+static double *g_hist = NULL; static int g_hist_cap = 0; static int *g_hist_n = NULL;
+void orc_set_cg_history(double *hist, int cap, int *n) { g_hist = hist; g_hist_cap = cap; g_hist_n = n; }
+
+/* z = D^-1 r with D = diag(A) (Jacobi; the paper's "future work" row: "no preconditioner by choice") */
+static void apply_jacobi(const oracle *o, int id, const real *r, real *z, int stride, int comp)
+{
+    int bs; const real *v = mat_values(o, id, &bs);
+    long N = o->N;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < N; i++) {
+        long q = o->rowptr[i];
+        while (o->col[q] != i) q++;                       /* the diagonal is always present (R21) */
+        if (bs == 1) z[i * stride + comp] = r[i * stride + comp] / v[q];
+        else for (int c = 0; c < 3; c++) z[3 * i + c] = r[3 * i + c] / v[9 * q + 4 * c];
+    }
+}
+
+/* Textbook conjugate gradients (O-4).  precond = 0: unpreconditioned, as the paper runs it;
+ * precond = 1: Jacobi-preconditioned (z = D^-1 r, beta = r.z ratios; SURVEY 8f unranked row).  Stop when
+ * ||r|| < tol ||b|| (recurrence residual, the true 2-norm in both variants), tested before each iteration; fixed >= 0
+ * runs exactly `fixed` iterations.  Dots in fp64; alpha, beta formed in fp64 and cast to the vector type. */
+static int cg_pc(const oracle *o, int id, const real *b, real *x, int stride, int comp, double tol, int maxiter,
+                 int fixed, int precond, int *iters, double *relres)
 {
     int bs; mat_values(o, id, &bs);
     long N = o->N, n = (bs == 3) ? 3 * N : N;   /* entries visited through (stride, comp) */
     if (bs == 3) { stride = 1; comp = 0; }
     long len = (bs == 3) ? 3 * N : N * stride;
     real *r = (real *)calloc((size_t)len, sizeof(real)), *p = (real *)calloc((size_t)len, sizeof(real)),
-         *Ap = (real *)calloc((size_t)len, sizeof(real));
+         *Ap = (real *)calloc((size_t)len, sizeof(real)), *z = precond ? (real *)calloc((size_t)len, sizeof(real)) : NULL;
     int status = ORC_OK, k = 0;
+    if (g_hist_n) *g_hist_n = 0;
     double bb = dot(n, b, b, stride, comp);
     if (bb == 0.0 && fixed < 0) {       /* ||b|| = 0 -> x = 0, 0 iterations */
         for (long i = 0; i < n; i++) x[i * stride + comp] = 0;
-        *iters = 0; *relres = 0; free(r); free(p); free(Ap); return ORC_OK;
+        *iters = 0; *relres = 0; free(r); free(p); free(Ap); free(z); return ORC_OK;
     }
     spmv(o, id, x, Ap, stride, comp);
-    for (long i = 0; i < n; i++) { r[i * stride + comp] = b[i * stride + comp] - Ap[i * stride + comp]; p[i * stride + comp] = r[i * stride + comp]; }
+    for (long i = 0; i < n; i++) r[i * stride + comp] = b[i * stride + comp] - Ap[i * stride + comp];
+    if (precond) apply_jacobi(o, id, r, z, stride, comp);
+    const real *zz = precond ? z : r;
+    for (long i = 0; i < n; i++) p[i * stride + comp] = zz[i * stride + comp];
     double rr = dot(n, r, r, stride, comp);
+    double rz = precond ? dot(n, r, z, stride, comp) : rr;
     for (;;) {
+        if (g_hist && k < g_hist_cap) { g_hist[k] = bb > 0 ? sqrt(rr / bb) : 0.0; if (g_hist_n) *g_hist_n = k + 1; }
         if (rr == 0.0) break;
         if (fixed >= 0) { if (k == fixed) break; }
         else { if (rr < tol * tol * bb) break; if (k >= maxiter) { status = ORC_W_MAXITER; break; } }
         spmv(o, id, p, Ap, stride, comp);
         double pAp = dot(n, p, Ap, stride, comp);
         if (!(pAp > 0.0)) { status = ORC_E_BREAKDOWN; break; }
-        real alpha = (real)(rr / pAp);
+        real alpha = (real)(rz / pAp);
 #pragma omp parallel for schedule(static)
         for (long i = 0; i < n; i++) {
             x[i * stride + comp] += alpha * p[i * stride + comp];
             r[i * stride + comp] -= alpha * Ap[i * stride + comp];
         }
-        double rr_new = dot(n, r, r, stride, comp);
-        real beta = (real)(rr_new / rr);
+        double rr_new = dot(n, r, r, stride, comp), rz_new = rr_new;
+        if (precond) { apply_jacobi(o, id, r, z, stride, comp); rz_new = dot(n, r, z, stride, comp); }
+        real beta = (real)(rz_new / rz);
 #pragma omp parallel for schedule(static)
-        for (long i = 0; i < n; i++) p[i * stride + comp] = r[i * stride + comp] + beta * p[i * stride + comp];
-        rr = rr_new; k++;
+        for (long i = 0; i < n; i++) p[i * stride + comp] = zz[i * stride + comp] + beta * p[i * stride + comp];
+        rr = rr_new; rz = rz_new; k++;
     }
     *iters = k; *relres = bb > 0 ? sqrt(rr / bb) : 0.0;
-    free(r); free(p); free(Ap);
+    free(r); free(p); free(Ap); free(z);
     return status;
+}
+
+static int cg(const oracle *o, int id, const real *b, real *x, int stride, int comp, double tol, int maxiter,
+              int fixed, int *iters, double *relres)
+{
+    return cg_pc(o, id, b, x, stride, comp, tol, maxiter, fixed, 0, iters, relres);
 }
 
 int orc_cg(const oracle *o, int id, const void *b, void *x, double tol, int maxiter, int fixed, int *iters, double *relres)
 {
     int bs; if (!mat_values(o, id, &bs)) return ORC_E_BADARG;
     return cg(o, id, (const real *)b, (real *)x, 1, 0, tol, maxiter, fixed, iters, relres);
+}
+
+int orc_cg_pc(const oracle *o, int id, const void *b, void *x, double tol, int maxiter, int fixed, int precond, int *iters, double *relres)
+{
+    int bs; if (!mat_values(o, id, &bs) || precond < 0 || precond > 1) return ORC_E_BADARG;
+    return cg_pc(o, id, (const real *)b, (real *)x, 1, 0, tol, maxiter, fixed, precond, iters, relres);
 }
 
 /* ------------------------------------------------------------------------------------ */

@@ -119,3 +119,48 @@ def test_bad_rotation_rejected(cm, torch):
         with pytest.raises(cm.CmError) as e:
             cm.System(gm, inputs.Material(R=R), 1e-12)
         assert e.value.code == cm.CM_E_BADARG
+
+
+@pytest.mark.parametrize("dtype,tol,bar", [("f64", 1e-12, 1e-9), ("f32", 1e-6, 1e-4)])
+def test_rotated_hexahedra(cm, oracle_mod, torch, dtype, tol, bar):
+    """Appendix D on linear hexahedra (R25 x R26): both sides honour cm_material.R on a hexahedral mesh -- K^mech with
+    C_sim, mechanical right-hand side, recovered stress, field, and five GSPM steps in the <111> frame."""
+    mesh = inputs.hex_box((12, 11, 7), (33 * NM, 30 * NM, 18 * NM), seed_mesh=81, seed_perm=82)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * NM, 7 * NM, 5 * NM))
+    mat = material(inputs.R_111)
+    clamp = inputs.clamp_bottom(mesh)
+    gm = cm.Mesh(mesh.xyz, mesh.hexes, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+    gs = cm.System(gm, mat, 1e-12, dtype, clamp, 5)
+    o = oracle_mod.Oracle(mesh, mat, 1e-12, clamp_dof=clamp, pin_node=5)
+    f64 = dtype == "f64"
+    ftol = 1e-12 if f64 else 1e-5
+    td = torch.float64 if f64 else torch.float32
+    dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=td, device="cuda")
+    A = _to_user(gm, gs.values(cm.CM_MAT_K_MECH))
+    B = o.csr(oracle_mod.MAT_K_MECH)
+    assert abs(A - B).max() < (1e-12 if f64 else 2e-7) * abs(B).max()
+    rng = np.random.default_rng(83)
+    N = o.N
+    live = o.live().astype(bool)
+    m = rng.normal(size=(N, 3)); m /= np.linalg.norm(m, axis=1, keepdims=True); m[~live] = 0
+    m = m.astype(gs.np_dtype); m64 = m.astype(np.float64)
+    u = (1e-3 * rng.normal(size=(N, 3))).astype(gs.np_dtype)
+    p = cm.make_params(1e-12, [3e4, -1e4, 2e4], TERM_ANIS | TERM_ZEEMAN | TERM_MAGEL)
+    assert rel(gs.field_rhs(cm.CM_RHS_MECH, dev(m)).cpu().numpy(), o.rhs_mech(m64)) < ftol
+    sig_o = o.stress_recover(u.astype(np.float64), m64)
+    assert rel(gs.field_rhs(cm.CM_OUT_SIGMA, dev(m), None, dev(u), p).cpu().numpy(), sig_o) < ftol
+    h_o = o.field(m64, None, sig_o, np.array([3e4, -1e4, 2e4]) / mat.Ms, TERM_ANIS | TERM_ZEEMAN | TERM_MAGEL)
+    assert rel(gs.field_rhs(cm.CM_OUT_FIELD, dev(m), None, dev(u), p).cpu().numpy(), h_o) < ftol
+    # the rotation matters on hexahedra too
+    gsI = cm.System(gm, material(None), 1e-12, dtype, clamp, 5)
+    assert rel(gsI.field_rhs(cm.CM_RHS_MECH, dev(m)).cpu().numpy(), o.rhs_mech(m64)) > 1e-3
+    mo = m64.copy(); U = np.zeros(N); uo = np.zeros((N, 3))
+    mg = dev(m64); Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+    H = [2e4, 0, 0]
+    for k in range(5):
+        io, rco = o.gspm_step(mo, U, uo, 1e-12, H, ALL, cg_tol=tol)
+        ig, rcg = gs.gspm_step(cm.make_params(1e-12, H, ALL, 0, tol), mg, Ug, ug)
+        assert rco == 0 and rcg == 0
+        if f64 and k == 0:
+            assert abs(io.it_ms - ig.it_ms) <= 1 and abs(io.it_mech - ig.it_mech) <= 1
+    assert np.abs(mg.cpu().numpy().astype(np.float64) - mo).max() <= bar
