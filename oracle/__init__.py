@@ -42,12 +42,12 @@ class _Material(C.Structure):
     _fields_ = [("Ms", C.c_double), ("Aex", C.c_double), ("K1", C.c_double), ("lambda100", C.c_double),
                 ("lambda111", C.c_double), ("alpha", C.c_double), ("gamma", C.c_double),
                 ("length_scale", C.c_double), ("Nd", C.c_double * 9), ("n_elastic", C.c_int),
-                ("C_voigt", C.POINTER(C.c_double)), ("R", C.c_double * 9)]
+                ("C_voigt", C.POINTER(C.c_double)), ("R", C.c_double * 9), ("sigma_ext", C.c_double * 6)]
 
 
 class _StepParams(C.Structure):
     _fields_ = [("dt", C.c_double), ("Hext", C.c_double * 3), ("terms", C.c_uint), ("gspm_variant", C.c_int),
-                ("cg_tol", C.c_double), ("cg_maxiter", C.c_int), ("cg_fixed_iters", C.c_int)]
+                ("cg_tol", C.c_double), ("cg_maxiter", C.c_int), ("cg_fixed_iters", C.c_int), ("cg_precond", C.c_int)]
 
 
 class StepInfo(C.Structure):
@@ -144,7 +144,8 @@ class Oracle:
                       material.gamma, material.length_scale, (C.c_double * 9)(*material.Nd),
                       0 if self._Cv is None else self._Cv.shape[0],
                       None if self._Cv is None else self._Cv.ctypes.data_as(C.POINTER(C.c_double)),
-                      (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())))
+                      (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())),
+                      (C.c_double * 6)(*(np.zeros(6) if getattr(material, "sigma_ext", None) is None else np.asarray(material.sigma_ext, float).ravel())))
         clamp = None if clamp_dof is None else np.ascontiguousarray(clamp_dof, np.uint8)
         h = C.c_void_p()
         self.is_hex = hasattr(mesh, "hexes")
@@ -299,11 +300,11 @@ class Oracle:
         hext = np.ascontiguousarray(hext_nd, np.float64)
         return self.L.orc_energy(self.h, _p(m), _p(U), _p(u), _p(hext), C.c_uint(terms))
 
-    def gspm_step(self, m, U, u, dt, Hext, terms, variant=0, cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1):
+    def gspm_step(self, m, U, u, dt, Hext, terms, variant=0, cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1, cg_precond=0):
         """In-place on m (N,3), U (N,), u (N,3) arrays of self.real dtype.  Returns (StepInfo, rc)."""
         for a in (m, U, u):
             assert a.dtype == self.real and a.flags.c_contiguous
-        p = _StepParams(dt, (C.c_double * 3)(*Hext), terms, variant, cg_tol, cg_maxiter, cg_fixed_iters)
+        p = _StepParams(dt, (C.c_double * 3)(*Hext), terms, variant, cg_tol, cg_maxiter, cg_fixed_iters, cg_precond)
         info = StepInfo()
         rc = self.L.orc_gspm_step(self.h, C.byref(p), _p(m), _p(U), _p(u), C.byref(info))
         return info, rc
@@ -313,7 +314,7 @@ class Oracle:
         """in place on m, U, u.  Returns (H_log, mbar_log, steps_log, HystResult, rc), logs cut to n_fields."""
         for a in (m, U, u):
             assert a.dtype == self.real and a.flags.c_contiguous
-        p = _StepParams(dt, (C.c_double * 3)(0, 0, 0), terms, variant, cg_tol, cg_maxiter, cg_fixed_iters)
+        p = _StepParams(dt, (C.c_double * 3)(0, 0, 0), terms, variant, cg_tol, cg_maxiter, cg_fixed_iters, 0)
         hp = _HystParams((C.c_double * 3)(*H0), (C.c_double * 3)(*dH), conv_tol, max_fields, max_steps)
         Hl = np.zeros((max_fields, 3)); ml = np.zeros((max_fields, 3)); sl = np.zeros(max_fields, np.int32)
         res = HystResult()

@@ -69,6 +69,8 @@ typedef struct {
     int n_elastic;
     const double *C_voigt; /* n_elastic x 36, Pa; in CRYSTAL axes */
     double R[9];           /* App. D: crystal -> simulation frame, v_sim = R v_crystal (Eq. D.2), row-major; all zeros = identity */
+    double sigma_ext[6];   /* uniform external stress of Eq. 1 (term -sigma_ext : E), Pa, simulation frame,
+                              tensor components (xx,yy,zz,yz,xz,xy); R17: the homogeneous-strain part of ref. [2] stays out */
 } orc_material;
 
 typedef struct {
@@ -79,6 +81,7 @@ typedef struct {
     double cg_tol;
     int cg_maxiter;
     int cg_fixed_iters;
+    int cg_precond;        /* 0: none (the paper); 1: Jacobi in every solve */
 } orc_step_params;
 
 typedef struct {
@@ -110,6 +113,7 @@ typedef struct {
     int n_elastic; double *Cstar; /* n_elastic x 36, C/(mu0 Ms^2) */
     double Vtot, Vmag;
     double R[9]; int rot; /* App. D rotation (identity: rot = 0) */
+    double sext[6];       /* sigma_ext / (mu0 Ms^2) */
     int nen; int *hex;    /* nen = 8: linear hexahedra; hex = Ne x 8 connectivity in DOF numbering; 0 / 4: tetrahedra */
     int *ghex;            /* hexahedra: Ne x 8 geometric node ids (coordinates); differs from hex on a wrapped (periodic) mesh */
 } oracle;
@@ -448,6 +452,7 @@ static int setup_material(oracle *o, const orc_material *mat, double dt)
     o->eps2 = o->alpha * o->Astar * o->dtau;   /* Step 3 */
     o->lam100 = mat->lambda100; o->lam111 = mat->lambda111;
     memcpy(o->Nd, mat->Nd, sizeof(o->Nd));
+    for (int q = 0; q < 6; q++) o->sext[q] = mat->sigma_ext[q] / mu0Ms2;
     o->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
     o->Cstar = (double *)calloc((size_t)(o->n_elastic > 0 ? o->n_elastic : 1) * 36, sizeof(double));
     double nrm = 0; for (int q = 0; q < 9; q++) nrm += mat->R[q] * mat->R[q];
@@ -1244,15 +1249,17 @@ static int hex_rhs_mech(const oracle *o, const real *m, real *b)
 {
     for (long i = 0; i < 3 * o->N; i++) b[i] = 0;
     for (long e = 0; e < o->Ne; e++) {
-        if (!o->mag[e]) continue;
         const int *t = o->hex + 8 * e;
         double X[24]; hex_coords(o, e, X);
         for (int p = 0; p < 8; p++) {
             double det, phi[8], g[8][3];
             hex_gauss_point(X, p, &det, phi, g);
-            real e0[6], s[6];
-            hex_point_strain(o, t, phi, g, NULL, m, e0);
-            C_times(o, e, e0, s);
+            real e0[6], s[6] = {0, 0, 0, 0, 0, 0};
+            if (o->mag[e]) {
+                hex_point_strain(o, t, phi, g, NULL, m, e0);
+                C_times(o, e, e0, s);
+            }
+            for (int q = 0; q < 6; q++) s[q] += (real)o->sext[q];   /* uniform external stress (R17), all cells */
             for (int a = 0; a < 8; a++) {
                 real gx = (real)g[a][0], gy = (real)g[a][1], gz = (real)g[a][2], w = (real)det;
                 b[3 * (long)t[a] + 0] += w * (s[0] * gx + s[5] * gy + s[4] * gz);
@@ -1308,13 +1315,19 @@ static double hex_elastic_energy(const oracle *o, const real *m, const real *u)
             C_times(o, e, eps, s);
             double w = 0; for (int q = 0; q < 6; q++) w += (double)eps[q] * (double)s[q];
             E += 0.5 * det * w;
+            real H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   /* - sigma_ext : E_h(p), total strain */
+            for (int k = 0; k < 8; k++) for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) H[a][b] += u[3 * (long)t[k] + a] * (real)g[k][b];
+            real et[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]};
+            for (int q = 0; q < 6; q++) E -= det * o->sext[q] * (double)et[q];
         }
     }
     return E;
 }
 
 /* S6 mechanical RHS (Eq. 10, 13, 14):
- * b_(i,a) = sum_{e contains i, magnetic} V_e [C*_e : mean_e E0(m)]_ab d_b phi_i; clamped DOFs zeroed. */
+ * b_(i,a) = sum_{e contains i, magnetic} V_e [C*_e : mean_e E0(m)]_ab d_b phi_i
+ *         + sum_{e contains i}           V_e sigma_ext,ab d_b phi_i          (the -sigma_ext : E term of Eq. 1; R17)
+ * clamped DOFs zeroed. */
 int orc_rhs_mech(const oracle *o, const void *m_, void *b_)
 {
     if (o->nen == 8) return hex_rhs_mech(o, (const real *)m_, (real *)b_);
@@ -1322,11 +1335,13 @@ int orc_rhs_mech(const oracle *o, const void *m_, void *b_)
     if (!o->n_elastic) return ORC_E_BADARG;
     for (long i = 0; i < 3 * o->N; i++) b[i] = 0;
     for (long e = 0; e < o->Ne; e++) {
-        if (!o->mag[e]) continue;
         const int *t = o->tet + 4 * e; const real *G = o->G + 12 * e;
-        real e0[6], s[6];
-        mean_E0(o, m, t, e0);
-        C_times(o, e, e0, s);   /* Voigt stress xx,yy,zz,yz,xz,xy */
+        real e0[6], s[6] = {0, 0, 0, 0, 0, 0};
+        if (o->mag[e]) {
+            mean_E0(o, m, t, e0);
+            C_times(o, e, e0, s);   /* Voigt stress xx,yy,zz,yz,xz,xy */
+        }
+        for (int q = 0; q < 6; q++) s[q] += (real)o->sext[q];
         for (int k = 0; k < 4; k++) {
             const real *g = G + 3 * k;
             b[3 * (long)t[k] + 0] += o->V[e] * (s[0] * g[0] + s[5] * g[1] + s[4] * g[2]);
@@ -1446,6 +1461,8 @@ double orc_energy(const oracle *o, const void *m_, const void *U_, const void *u
             C_times(o, e, eps, s);
             double w = 0; for (int q = 0; q < 6; q++) w += (double)eps[q] * (double)s[q];
             E += 0.5 * (double)o->V[e] * w;
+            real et[6]; elem_strain(o, e, u, et);           /* - sigma_ext : E (Eq. 1), total strain */
+            for (int q = 0; q < 6; q++) E -= (double)o->V[e] * o->sext[q] * (double)et[q];
         }
     free(y);
     return E;
@@ -1460,7 +1477,7 @@ static int helmholtz(const oracle *o, int id, const real *f, real *g, int a, con
 {
     spmv(o, MAT_MASS, f, b, 3, a);                                  /* b = M_m f (Eq. 14) */
     for (long i = 0; i < o->N; i++) g[3 * i + a] = f[3 * i + a];
-    return cg(o, id, b, g, 3, a, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, it, res);
+    return cg_pc(o, id, b, g, 3, a, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, p->cg_precond, it, res);
 }
 
 int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_, void *u_, orc_step_info *info)
@@ -1468,7 +1485,7 @@ int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_,
     real *m = (real *)m_, *U = (real *)U_, *u = (real *)u_;
     long N = o->N; unsigned terms = p->terms;
     int worst = ORC_OK, rc;
-    if (p->dt != o->dt) return ORC_E_BADARG; /* K^GS was assembled for the dt given at create */
+    if (p->dt != o->dt || p->cg_precond < 0 || p->cg_precond > 1) return ORC_E_BADARG; /* K^GS was assembled for the dt given at create */
     real *b = (real *)calloc((size_t)3 * N, sizeof(real)), *hd = (real *)calloc((size_t)3 * N, sizeof(real)),
          *sg = (real *)calloc((size_t)6 * N, sizeof(real)), *hn = (real *)calloc((size_t)3 * N, sizeof(real)),
          *f = (real *)calloc((size_t)3 * N, sizeof(real)), *gn = (real *)calloc((size_t)3 * N, sizeof(real)),
@@ -1484,7 +1501,7 @@ int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_,
     /* 2. magnetostatic solve, warm start (Eq. 5, 9) */
     if (terms & T_DEMAG) {
         orc_rhs_ms(o, m, mbar, b);
-        rc = cg(o, MAT_K_MS, b, U, 1, 0, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, &info->it_ms, &info->res_ms);
+        rc = cg_pc(o, MAT_K_MS, b, U, 1, 0, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, p->cg_precond, &info->it_ms, &info->res_ms);
         if (rc < worst) worst = rc;
     }
     /* 3. demagnetising field (Eq. 4) */
@@ -1492,7 +1509,7 @@ int orc_gspm_step(const oracle *o, const orc_step_params *p, void *m_, void *U_,
     /* 4. mechanical equilibrium (Eq. 6, 10), warm start */
     if (terms & T_MAGEL) {
         orc_rhs_mech(o, m, b);
-        rc = cg(o, MAT_K_MECH, b, u, 1, 0, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, &info->it_mech, &info->res_mech);
+        rc = cg_pc(o, MAT_K_MECH, b, u, 1, 0, p->cg_tol, p->cg_maxiter, p->cg_fixed_iters, p->cg_precond, &info->it_mech, &info->res_mech);
         if (rc < worst) worst = rc;
         orc_stress_recover(o, u, m, sg);
     }

@@ -235,7 +235,7 @@ template <typename T>
 __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr, const int *__restrict__ col, const double *K,
                                 const double *Km, const double *Mm, const double *Kme, const uchar *__restrict__ live,
                                 const uchar *__restrict__ clamp, int pin, double eps1, double eps2, const int *__restrict__ spS,
-                                const int *__restrict__ spB, T *Kms, T *Kgs1, T *Kgs2, T *MmT, T *Kmech)
+                                const int *__restrict__ spB, T *Kms, T *Kgs1, T *Kgs2, T *MmT, T *Kmech, T *Dms, T *Dgs1, T *Dgs2, T *Dmech)
 {
     constexpr int CS = CM_C_SCALAR, CB = CM_C_BLOCK;
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -253,6 +253,7 @@ __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr
         Kgs1[dS] = (T)(Mm[q] + eps1 * Km[q] + dead);
         Kgs2[dS] = (T)(Mm[q] + eps2 * Km[q] + dead);
         MmT[dS] = (T)Mm[q];
+        if (i == j) { Dms[i] = Kms[dS]; Dgs1[i] = Kgs1[dS]; Dgs2[i] = Kgs2[dS]; } // diagonals as stored (Jacobi)
         if (Kme) {
             T *dst = Kmech + 9 * bB + (long)(q - q0) * CB + i % CB;
             for (int r = 0; r < 3; r++)
@@ -260,6 +261,7 @@ __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr
                     double v = Kme[9 * (long)q + 3 * r + c];
                     if (clamp[3 * i + r] || clamp[3 * (long)j + c]) v = (i == j && r == c) ? 1.0 : 0.0;
                     dst[LB * (3 * r + c)] = (T)v;
+                    if (i == j && r == c) Dmech[3 * i + r] = (T)v;
                 }
         }
     }
@@ -268,10 +270,10 @@ __global__ void finalize_kernel(long N, long nnz, const int *__restrict__ rowptr
 template <typename T>
 System<T>::~System()
 {
-    T *ptrs[] = {EG, mL, mLm, Cstar, Ccub, Kms, Kgs1, Kgs2, Mm, Kmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
+    T *ptrs[] = {EG, mL, mLm, Cstar, Ccub, Kms, Kgs1, Kgs2, Mm, Kmech, Dms, Dgs1, Dgs2, Dmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
-    cudaFree(hyst_ctl); cudaFree(hyst_log); cudaFree(hyst_steps);
+    cudaFree(hyst_ctl); cudaFree(hyst_log); cudaFree(hyst_steps); cudaFree(d_hist);
     if (h_res) cudaFreeHost(h_res);
     if (h_scal) cudaFreeHost(h_scal);
 }
@@ -325,6 +327,8 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     const long ES = M->sell[0].E, EB = M->sell[1].E; // stored elements of the sliced layouts (padding is zero)
     CM_TRY(alloc(&S->Kms, ES)); CM_TRY(alloc(&S->Kgs1, ES)); CM_TRY(alloc(&S->Kgs2, ES)); CM_TRY(alloc(&S->Mm, ES));
     if (S->n_elastic) CM_TRY(alloc(&S->Kmech, 9 * EB));
+    CM_TRY(alloc(&S->Dms, N)); CM_TRY(alloc(&S->Dgs1, N)); CM_TRY(alloc(&S->Dgs2, N));
+    if (S->n_elastic) CM_TRY(alloc(&S->Dmech, 3 * N));
 
     // elastic constants C* = C / (mu0 Ms^2): fp64 for assembly, T for the element kernels
     double *Cd = nullptr;
@@ -434,18 +438,21 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     }
     finalize_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, nnz, M->d_rowptr, M->d_col, K, Km, Mm, Kme, S->live, S->clamp, S->pin,
                                                                  S->eps1, S->eps2, M->sell[0].d_sp, M->sell[1].d_sp, S->Kms, S->Kgs1, S->Kgs2,
-                                                                 S->Mm, S->Kmech);
+                                                                 S->Mm, S->Kmech, S->Dms, S->Dgs1, S->Dgs2, S->Dmech);
     CM_CUDA(cudaGetLastError());
     CM_CUDA(cudaStreamSynchronize(st));
     cudaFree(K); cudaFree(Km); cudaFree(Mm); cudaFree(Kme); cudaFree(Vd); cudaFree(vsum); cudaFree(Cd);
 
     // work vectors
-    T **vecs3[] = {&S->r, &S->p, &S->p2, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->f, &S->gn, &S->gs, &S->ms, &S->mss, &S->xin, &S->xout, &S->stg_m, &S->stg_u};
+    T **vecs3[] = {&S->r, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->gn, &S->gs, &S->ms, &S->mss, &S->xout, &S->stg_m, &S->stg_u};
     for (T **v : vecs3) CM_TRY(alloc(v, 3 * N));
+    T **vecs4[] = {&S->p, &S->p2, &S->f, &S->xin}; // padded [node][4] when they hold a 3-vector that a product gathers
+    for (T **v : vecs4) CM_TRY(alloc(v, 4 * N));
     CM_TRY(alloc(&S->U, N)); CM_TRY(alloc(&S->stg_U, N)); CM_TRY(alloc(&S->sig, 6 * N));
     CM_TRY(alloc(&S->hpart, (size_t)6 * M->ck.nslots));
     S->grid_cap = S->num_sms * 8;
-    CM_TRY(alloc(&S->partial, (size_t)4 * S->grid_cap * 3));
+    CM_TRY(alloc(&S->partial, (size_t)5 * S->grid_cap * 3));
+    CM_TRY(alloc(&S->d_hist, (size_t)CM_HIST_CAP));
     CM_TRY(alloc(&S->d_res, 8));
     CM_TRY(alloc(&S->red, std::max<size_t>({(size_t)4096 * 16, (size_t)8 * M->ck.nchunks, (size_t)3 * ((N + 127) / 128) + 64})));
     CM_TRY(alloc(&S->dscal, 32));

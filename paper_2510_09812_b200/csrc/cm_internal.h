@@ -114,6 +114,7 @@ struct SystemBase;
 template <typename T>
 inline Rot<T> make_rot(const SystemBase *S);
 
+constexpr int CM_HIST_CAP = 3 << 16;
 struct CgResult {
     int iters[3];
     double relres[3];
@@ -178,11 +179,15 @@ struct System : SystemBase {
     // matrices
     T *Kms = nullptr, *Kgs1 = nullptr, *Kgs2 = nullptr, *Mm = nullptr;
     T *Kmech = nullptr; // sliced, 9 planes per slice: [slice][3 r + c][L_slice]
+    // diagonals of the constrained matrices (Jacobi preconditioner): N entries each, Dmech 3N
+    T *Dms = nullptr, *Dgs1 = nullptr, *Dgs2 = nullptr, *Dmech = nullptr;
     // CG work
     T *r = nullptr, *p = nullptr, *p2 = nullptr, *Ap = nullptr, *bvec = nullptr;
     double *partial = nullptr;
     int grid_cap = 0;
     CgResult *d_res = nullptr, *h_res = nullptr; // 8 slots
+    double *d_hist = nullptr;  // residual history of the last solve (cm_cg_history), CM_HIST_CAP doubles
+    bool hist_on = false;
     // step state (library order)
     T *m = nullptr, *U = nullptr, *u = nullptr, *hd = nullptr, *hn = nullptr, *f = nullptr, *gn = nullptr, *gs = nullptr,
       *ms = nullptr, *mss = nullptr, *xin = nullptr, *xout = nullptr;
@@ -242,7 +247,9 @@ int build_chunks(long N, long Ne, const int *tets, Chunks *out);
 template <typename T> int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, long pin_user, cudaStream_t st);
 template <typename T> int sys_spmv(System<T> *S, cm_matrix_id id, int mode, const T *x, T *y, cudaStream_t st);
 template <typename T> int sys_cg(System<T> *S, cm_matrix_id id, int mode, const T *b, T *x, double tol, int maxiter, int fixed,
-                                 unsigned mask, int slot, int prof_cls, cudaStream_t st);
+                                 unsigned mask, int slot, int prof_cls, int precond, cudaStream_t st);
+template <typename T> int sys_helmholtz(System<T> *S, cm_matrix_id id, const T *f4, T *x, double tol, int maxiter, int fixed, unsigned mask,
+                                        int slot, int precond, cudaStream_t st);
 template <typename T> int sys_get_values(const System<T> *S, cm_matrix_id id, void *host_out, long capacity);
 template <typename T> int sys_permute_in(System<T> *S, const T *user, T *lib, int ncomp, cudaStream_t st);
 template <typename T> int sys_permute_out(System<T> *S, const T *lib, T *user, int ncomp, cudaStream_t st);

@@ -49,6 +49,7 @@ class Material:
     Nd: Tuple[float, ...] = (1 / 3, 0, 0, 0, 1 / 3, 0, 0, 0, 1 / 3)   # sphere
     C_voigt: np.ndarray = field(default_factory=lambda: isotropic_voigt(200e9, 0.3)[None])   # crystal axes
     R: Optional[np.ndarray] = None   # App. D: crystal -> simulation frame (3x3, v_sim = R v_crystal); None = identity
+    sigma_ext: Optional[np.ndarray] = None   # uniform external stress (6,) Pa, Voigt xx,yy,zz,yz,xz,xy (Eq. 1); None = 0
 
 
 def isotropic_voigt(E: float, nu: float) -> np.ndarray:
