@@ -87,53 +87,77 @@ def sample_config():
     return inputs.make_config(3, grid=SAMPLE_GRID, box=SAMPLE_BOX)
 
 
-def time_oracle(steps: int, warmup: int):
-    """The oracle as it stands, on the box's host cores, on the bounded sample.  Returns (steps/s scaled to the
-    3M-node mesh by node count, description, threads)."""
+def time_oracle(steps: int, warmup: int, variant: int = 0, full_mesh: bool = False, maxiter: int = 100000):
+    """The oracle as it stands, on the box's host cores, on a bounded sample of config 3.  Default sample: a sub-box at
+    the same spacing / physics / tolerance, `warmup` untimed steps first (warm starts of U and u as on the GPU side),
+    steps/s scaled to the 3M-node mesh by node count.  full_mesh: config 3 ITSELF with every solve capped at `maxiter`
+    iterations (the truncation is part of the sample's description).  Returns a dict."""
     import oracle
-    cfg = sample_config()
+    cfg = inputs.make_config(3) if full_mesh else sample_config()
+    t_setup = time.perf_counter()
     o = oracle.Oracle(cfg.mesh, cfg.material, cfg.dt, clamp_dof=cfg.clamp_dof)
+    t_setup = time.perf_counter() - t_setup
     m = cfg.m0.copy(); U = np.zeros(o.N); u = np.zeros((o.N, 3))
     its = []
-    t0 = None
+    t0 = time.perf_counter()
     for k in range(warmup + steps):
         if k == warmup:
             t0 = time.perf_counter()
-        info, rc = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, cg_tol=CG_TOL)
-        its.append((info.it_ms, info.it_mech, sum(info.it_gs)))
+        info, rc = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, variant=variant, cg_tol=CG_TOL, cg_maxiter=maxiter)
+        its.append((info.it_ms, info.it_mech, int(sum(info.it_gs))))
     dt = time.perf_counter() - t0
     n_full = FULL_GRID[0] * FULL_GRID[1] * FULL_GRID[2]
     scale = o.N / n_full
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    desc = (f"{steps} GSPM step(s) of config 3 on a {SAMPLE_GRID[0]}x{SAMPLE_GRID[1]}x{SAMPLE_GRID[2]}-node sub-box "
-            f"({o.N} nodes, same spacing/physics/tol {CG_TOL:g}); steps/s multiplied by {o.N}/{n_full} (node count); "
-            f"CG its (ms, mech, sum gs) last step {its[-1]}")
-    return steps / dt * scale, dt / steps, desc, cores
+    timed = its[warmup:]
+    n_it = sum(a + b + c for a, b, c in timed)
+    where = (f"config 3 itself ({o.N} nodes), every CG solve capped at {maxiter} iterations" if full_mesh else
+             f"a {SAMPLE_GRID[0]}x{SAMPLE_GRID[1]}x{SAMPLE_GRID[2]}-node sub-box of config 3 ({o.N} nodes, same spacing/physics); "
+             f"steps/s multiplied by {o.N}/{n_full} (node count)")
+    desc = (f"{steps} GSPM step(s) after {warmup} warm-up step(s), gspm_variant {variant}, tol {CG_TOL:g}, on {where}; "
+            f"CG its per timed step (ms, mech, sum gs) {timed}")
+    return {"value": steps / dt * scale, "sec_per_step": dt / steps, "desc": desc, "cores": cores, "cg_iters_per_step": timed,
+            "ms_per_cg_iteration_all_solves": 1e3 * dt / max(1, n_it), "nodes": o.N, "setup_s": t_setup}
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    value, sec_per_step, desc, cores = time_oracle(args.steps, args.warmup)
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+    r = time_oracle(args.steps, args.warmup, args.variant, args.full_mesh, args.oracle_maxiter)
+    cb = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["desc"],
+          "cg_iters_per_step": r["cg_iters_per_step"], "ms_per_cg_iteration_all_solves": r["ms_per_cg_iteration_all_solves"],
+          "setup_s": r["setup_s"]}
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": r["sec_per_step"] * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config3_paper_scale (bounded CPU sample)", "sample": desc},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
-            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+            "config": {"workload": "config3_paper_scale (bounded CPU sample)", "sample": r["desc"], "gspm_variant": args.variant},
+            "cpu_baseline": cb,
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
 
 def algorithmic_bytes(N, nnz, s):
-    """SURVEY 8(d) per-unit figures (x-vector gathers counted once), s = bytes per value."""
+    """Bytes per matrix pass, s = bytes per value.  `*_iter_*`: SURVEY 8(d)'s per-unit figures for one CG iteration
+    (SpMV with its x read and y write + 10 vector words per DOF; the figure `roofline.achieved` uses).  `*_streams_*`: what
+    the kernel actually streams per iteration -- p, Ap of the product are among the 10 words, so 8 more on top of the
+    SpMV (x, r, p_old read, x, p written in phase C'; Ap, r read, r written in phase B; p gathered, Ap written by the
+    product) -- reported beside it.  `*_r0_*`: the r0 = b - A x0 pass of a launch (product + b, Ap read, r written).
+    The three-right-hand-side solver keeps p padded to four words per node (one 32 B / 16 B gather per nonzero)."""
     spmv_csr = nnz * (s + 4) + N * (4 + s + s)
     spmv_bsr = nnz * (9 * s + 4) + N * (4 + 3 * s + 3 * s)
+    spmv_csr3 = nnz * (s + 4) + N * 4 + 2 * 3 * N * s
     return {
-        "cg_iter_csr1": spmv_csr + 10 * N * s,                  # SpMV + ~10 vector words (SURVEY: 277 B/row fp64)
+        "cg_iter_csr1": spmv_csr + 10 * N * s,                  # SURVEY: 277 B/row fp64
         "cg_iter_bsr3": spmv_bsr + 10 * 3 * N * s,              # SURVEY: 1415 B/node fp64
-        "cg_iter_csr3": nnz * (s + 4) + N * 4 + 2 * 3 * N * s + 10 * 3 * N * s,   # 3-RHS: matrix read once per iteration
-        "spmv_csr3": nnz * (s + 4) + N * 4 + 2 * 3 * N * s,
+        "cg_iter_csr3": spmv_csr3 + 10 * 3 * N * s,             # 3-RHS: matrix read once per iteration
+        "cg_streams_csr1": spmv_csr + 8 * N * s,
+        "cg_streams_bsr3": spmv_bsr + 8 * 3 * N * s,
+        "cg_streams_csr3": nnz * (s + 4) + N * 4 + N * s * (4 + 3) + N * s * (3 + 3 + 4 + 3 + 4 + 3 + 3 + 3),
+        "cg_r0_csr1": spmv_csr + 3 * N * s,
+        "cg_r0_bsr3": spmv_bsr + 3 * 3 * N * s,
+        "cg_r0_csr3": nnz * (2 * s + 4) + N * 4 + N * s * (4 + 4 + 3 + 3),   # Helmholtz start: K^GS and M_m streamed together, f4 gathered and read, r0 and x0 written
+        "spmv_csr3": spmv_csr3,
     }
 
 
@@ -152,8 +176,6 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
     dtype = args.dtype
-    td = torch.float64 if dtype == "f64" else torch.float32
-    s = 8 if dtype == "f64" else 4
 
     grid = tuple(int(g) for g in args.grid.split("x")) if args.grid else None
     cfg = inputs.make_config(3, grid=grid)
@@ -163,13 +185,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup
     N, nnz = mesh.n_nodes, mesh.nnz
-
-    m = torch.as_tensor(cfg.m0, dtype=td, device=dev).contiguous()
-    U = torch.zeros(N, dtype=td, device=dev)
-    u = torch.zeros((N, 3), dtype=td, device=dev)
-
-    def params(k):
-        return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, args.variant, CG_TOL, 100000, args.fixed_iters)
+    peak, peak_src = measured_peaks()
 
     def barrier():
         torch.cuda.synchronize()
@@ -177,36 +193,106 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    k = 0
-    for _ in range(args.warmup):
-        sysm.gspm_step(params(k), m, U, u); k += 1
-    sysm.profile_enable(True)
-    sysm.profile_reset()
-    infos = []
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    with ClockSampler(local) as clocks:
-        ev0.record()
-        for _ in range(args.steps):
-            info, rc = sysm.gspm_step(params(k), m, U, u); k += 1
-            infos.append(info)
-        ev1.record()
-        barrier()
-    ms_total = ev0.elapsed_time(ev1)
-    prof = sysm.profile()
-    sysm.profile_enable(False)
-    _, ms_total, value = replicas.aggregate(args.steps, ms_total, dist if world > 1 else None, dev)
+    def timed_run(system, dt_name, steps, warmup, variant, fixed, precond):
+        """W untimed + K timed cm_gspm_step calls from the config's initial state; CUDA events on the launching stream."""
+        td = torch.float64 if dt_name == "f64" else torch.float32
+        m = torch.as_tensor(cfg.m0, dtype=td, device=dev).contiguous()
+        U = torch.zeros(N, dtype=td, device=dev)
+        u = torch.zeros((N, 3), dtype=td, device=dev)
 
-    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+        def params(k):
+            return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, variant, CG_TOL, 100000, fixed, precond)
+
+        k = 0
+        for _ in range(warmup):
+            system.gspm_step(params(k), m, U, u); k += 1
+        system.profile_enable(True)
+        system.profile_reset()
+        infos = []
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        with ClockSampler(local) as clocks:
+            ev0.record()
+            for _ in range(steps):
+                info, rc = system.gspm_step(params(k), m, U, u); k += 1
+                infos.append(info)
+            ev1.record()
+            barrier()
+        ms = ev0.elapsed_time(ev1)
+        prof = system.profile()
+        system.profile_enable(False)
+        _, ms, value = replicas.aggregate(steps, ms, dist if world > 1 else None, dev)
+        return {"value": value, "ms_total": ms, "prof": prof, "infos": infos, "clocks": clocks.summary(), "state": (m, U, u),
+                "params": params, "k": k}
+
+    def kernel_table(prof, steps, s):
+        """Per kernel class: device time, launches, algorithmic GB/s (SURVEY 8d figures) and fraction of the measured peak."""
+        ab = algorithmic_bytes(N, nnz, s)
+        out = {}
+        for name, key in (("cg_mech", "bsr3"), ("cg_ms", "csr1"), ("cg_gs", "csr3")):
+            p = prof[name]
+            if p["ms"] > 0 and p["cg_matrix_passes"] > 0:
+                iters = p["cg_matrix_passes"] - p["launches"]        # every launch makes one r0 pass
+                byts = ab["cg_iter_" + key] * iters + ab["cg_r0_" + key] * p["launches"]
+                streamed = ab["cg_streams_" + key] * iters + ab["cg_r0_" + key] * p["launches"]
+                gbs = byts / (p["ms"] * 1e-3) / 1e9
+                out[name] = {"ms": p["ms"], "launches": p["launches"], "matrix_passes": p["cg_matrix_passes"], "iterations": iters,
+                             "algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_spec_8000": gbs / 8000.0,
+                             "streamed_GBps": streamed / (p["ms"] * 1e-3) / 1e9}
+        for name in ("spmv", "element", "pointwise"):
+            out[name] = {"ms": prof[name]["ms"], "launches": prof[name]["launches"]}
+        # assembly (element passes S3, S5, S6, 2 x S8 per step, each followed by its node pass): SURVEY 8(d) bytes -- per tet
+        # 16 B connectivity + 13 words, nodal input and output once
+        elem_step = 5 * mesh.n_tets * (16 + 13 * s) + N * s * (4 + 4 + 6 + 2 * 12)
+        if out["element"]["ms"] > 0:
+            gbs = elem_step * steps / (out["element"]["ms"] * 1e-3) / 1e9
+            out["element"].update({"algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_spec_8000": gbs / 8000.0})
+        return out, ab
+
+    s = 8 if dtype == "f64" else 4
+    main = timed_run(sysm, dtype, args.steps, args.warmup, args.variant, args.fixed_iters, args.precond)
+    ms_total, value, prof, infos = main["ms_total"], main["value"], main["prof"], main["infos"]
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region, all --steps
+    m, U, u = main["state"]
     mh = m.cpu().pin_memory(); Uh = U.cpu().pin_memory(); uh = u.cpu().pin_memory()
-    e2e_steps = max(1, min(args.steps, 3))
+    k = main["k"]
     barrier()
     t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        sysm.gspm_step_host(params(k), mh, Uh, uh); k += 1
+    for _ in range(args.steps):
+        sysm.gspm_step_host(main["params"](k), mh, Uh, uh); k += 1
     torch.cuda.synchronize()
-    _, _, e2e_value = replicas.aggregate(e2e_steps, (time.perf_counter() - t0) * 1e3, dist if world > 1 else None, dev)
+    _, _, e2e_value = replicas.aggregate(args.steps, (time.perf_counter() - t0) * 1e3, dist if world > 1 else None, dev)
     io_bytes = 7 * N * s
+    del m, U, u, mh, Uh, uh
+
+    # ---- variants SURVEY 8(d) asks for beside steps/s (each its own W + K steps from the initial state, same mesh):
+    # every solve cut at 3 iterations (the paper's regime for the Helmholtz solves, P:286), fp32 (north_star (4)),
+    # Jacobi-preconditioned CG (the paper's future work, P:355), and the other reading of Alg. B.1 Step 2 (R1)
+    variants = {}
+    if not args.no_variants:
+        vs = max(1, min(args.steps, args.variant_steps))
+
+        def brief(r, extra=None):
+            d = {"value": r["value"], "unit": UNIT, "ms_per_step": r["ms_total"] / len(r["infos"]), "steps": len(r["infos"]),
+                 "cg_iters_per_step": [[i.it_ms, i.it_mech, int(sum(i.it_gs))] for i in r["infos"]],
+                 "mean_dm_last_step": float(r["infos"][-1].mean_dm)}
+            d.update(extra or {})
+            return d
+
+        r = timed_run(sysm, dtype, vs, args.warmup, args.variant, 3, args.precond)
+        kt, _ = kernel_table(r["prof"], vs, s)
+        variants["fixed3"] = brief(r, {"kernels": {n: {q: v[q] for q in ("ms", "frac_of_measured_peak") if q in v} for n, v in kt.items()}})
+        r = timed_run(sysm, dtype, vs, args.warmup, args.variant, args.fixed_iters, 1 - args.precond)
+        variants["jacobi" if args.precond == 0 else "plain_cg"] = brief(r)
+        r = timed_run(sysm, dtype, vs, args.warmup, 1 - args.variant, args.fixed_iters, args.precond)
+        variants[f"gspm_variant{1 - args.variant}"] = brief(r)
+        other = "f32" if dtype == "f64" else "f64"
+        sys2 = cm.System(mesh, cfg.material, cfg.dt, other, cfg.clamp_dof, cfg.pin_node)
+        r = timed_run(sys2, other, vs, args.warmup, args.variant, args.fixed_iters, args.precond)
+        kt, _ = kernel_table(r["prof"], vs, 12 - s)
+        variants[other] = brief(r, {"kernels": {n: {q: v[q] for q in ("ms", "frac_of_measured_peak") if q in v} for n, v in kt.items()}})
+        sys2.close()
 
     if rank != 0:
         if world > 1:
@@ -214,31 +300,13 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant kernel (by accumulated device time)
-    ab = algorithmic_bytes(N, nnz, s)
-    peak, peak_src = measured_peaks()
-    per_class = {}
-    for name, key in (("cg_mech", "cg_iter_bsr3"), ("cg_ms", "cg_iter_csr1"), ("cg_gs", "cg_iter_csr3")):
-        p = prof[name]
-        if p["ms"] > 0 and p["cg_matrix_passes"] > 0:
-            gbs = ab[key] * p["cg_matrix_passes"] / (p["ms"] * 1e-3) / 1e9
-            per_class[name] = {"ms": p["ms"], "launches": p["launches"], "matrix_passes": p["cg_matrix_passes"],
-                               "algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_spec_8000": gbs / 8000.0}
-    for name in ("spmv", "element", "pointwise"):
-        per_class[name] = {"ms": prof[name]["ms"], "launches": prof[name]["launches"]}
-    # assembly (element passes S3, S5, S6, 2 x S8 per step, each followed by its node pass) and the 3 mass products b = M_m f:
-    # SURVEY 8(d) bytes -- per tet 16 B connectivity + 13 words, nodal input and output once
-    Ne = mesh.n_tets
-    elem_step = 5 * Ne * (16 + 13 * s) + N * s * (4 + 4 + 6 + 2 * 12)
-    spmv_step = 3 * ab["spmv_csr3"]
-    for name, byts in (("element", elem_step), ("spmv", spmv_step)):
-        if per_class[name]["ms"] > 0:
-            gbs = byts * args.steps / (per_class[name]["ms"] * 1e-3) / 1e9
-            per_class[name].update({"algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_spec_8000": gbs / 8000.0})
+    per_class, ab = kernel_table(prof, args.steps, s)
     dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
-    # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_f_cg_full.md: config 3, 21 passes per launch);
-    # scaled to the average launch of this run, like `achieved`.  Only known for the captured workload.
-    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.906508e9 / 21, ("cg_ms", "f64"): 14.160628e9 / 21, ("cg_gs", "f64"): 26.153006e9 / 21,
-                          ("cg_mech", "f32"): 43.734836e9 / 21, ("cg_ms", "f32"): 7.856605e9 / 21, ("cg_gs", "f32"): 13.277198e9 / 21}
+    key = {"cg_mech": "bsr3", "cg_ms": "csr1", "cg_gs": "csr3"}[dom]
+    # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_f_cg_full.md: config 3, 21 passes per launch),
+    # EXTRAPOLATED to the average launch of this run, like `achieved`.  Only known for the captured workload.
+    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.906508e9 / 21, ("cg_ms", "f64"): 14.160628e9 / 21,
+                          ("cg_mech", "f32"): 43.734836e9 / 21, ("cg_ms", "f32"): 7.856605e9 / 21}
     traffic = None
     passes_per_launch = prof[dom]["cg_matrix_passes"] / max(1, prof[dom]["launches"])
     if (dom, dtype) in ncu_bytes_per_pass and not args.grid:
@@ -247,9 +315,11 @@ def run_ours(args):
             "achieved": per_class.get(dom, {}).get("algorithmic_GBps"), "peak": peak, "unit": "GB/s",
             "frac": per_class.get(dom, {}).get("frac_of_measured_peak"), "traffic": traffic, "peak_source": peak_src,
             "share_of_step": prof[dom]["ms"] / ms_total,
-            "algorithmic_bytes_per_matrix_pass": ab[{"cg_mech": "cg_iter_bsr3", "cg_ms": "cg_iter_csr1", "cg_gs": "cg_iter_csr3"}[dom]],
-            "matrix_passes_per_launch": passes_per_launch,
-            "traffic_source": "ncu --set full dram__bytes_read+write per matrix pass (profiles/r01_f_cg_full.md) x passes per launch"}
+            "algorithmic_bytes_per_iteration": ab["cg_iter_" + key], "streamed_bytes_per_iteration": ab["cg_streams_" + key],
+            "bytes_r0_pass": ab["cg_r0_" + key], "matrix_passes_per_launch": passes_per_launch,
+            "achieved_streamed": per_class.get(dom, {}).get("streamed_GBps"),
+            "traffic_source": "extrapolated: ncu --set full dram__bytes_read+write per matrix pass of a 21-pass capture "
+                              "(profiles/r01_f_cg_full.md) x matrix passes per launch of this run"}
 
     launches = sum(p["launches"] for p in prof.values())
     last = infos[-1]
@@ -258,19 +328,22 @@ def run_ours(args):
             "dtype": dtype, "data": "synthetic",
             "config": {"workload": "config3_paper_scale", "grid": "x".join(map(str, cfg.mesh.grid)), "n_nodes": N,
                        "n_tets": mesh.n_tets, "nnz": nnz, "dt_ps": cfg.dt * 1e12, "cg_tol": CG_TOL, "cg_fixed_iters": args.fixed_iters,
+                       "cg_precond": args.precond,
                        "terms": "exchange+anis+zeeman+demag+farfield+magel", "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2 (matrices 3.2 GB fp64 per solve)", "setup_s": t_setup,
                        "gspm_variant": args.variant,
                        "cg_iters_last_step": {"ms": last.it_ms, "mech": last.it_mech, "gs": list(last.it_gs)},
                        "cg_iters_per_step": [[i.it_ms, i.it_mech, int(sum(i.it_gs))] for i in infos],
                        "mean_dm_per_step": [float(i.mean_dm) for i in infos]},
-            "clocks": clocks.summary(),
+            "clocks": main["clocks"],
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
-                    "steps": e2e_steps},
-            "gpu_launches": launches, "roofline": roof, "kernels": per_class}
+                    "steps": args.steps},
+            "gpu_launches": launches, "roofline": roof, "kernels": per_class, "variants": variants}
     if world == 1 and not args.no_cpu_baseline:
-        v, sps, desc, cores = time_oracle(1, 0)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        r = time_oracle(2, 1, args.variant)
+        line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["desc"],
+                                "cg_iters_per_step": r["cg_iters_per_step"],
+                                "ms_per_cg_iteration_all_solves": r["ms_per_cg_iteration_all_solves"]}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -285,6 +358,11 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--fixed-iters", type=int, default=-1, help="run every CG solve for exactly this many iterations")
     ap.add_argument("--variant", type=int, default=0, choices=[0, 1], help="Alg. B.1 Step 2: 0 as printed (P:438), 1 fully Gauss-Seidel (R1)")
+    ap.add_argument("--precond", type=int, default=0, choices=[0, 1], help="CG preconditioner: 0 none (the paper's), 1 Jacobi (P:355)")
+    ap.add_argument("--no-variants", action="store_true", help="skip the fixed3 / f32 / jacobi / other-variant re-runs")
+    ap.add_argument("--variant-steps", type=int, default=4, help="timed steps of each variant re-run")
+    ap.add_argument("--full-mesh", action="store_true", help="--impl reference: time the oracle on config 3 itself (capped solves)")
+    ap.add_argument("--oracle-maxiter", type=int, default=100000, help="--impl reference: cap of every CG solve")
     ap.add_argument("--grid", default="", help="override the node grid, e.g. 81x81x21 (not the headline workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -11,7 +11,11 @@
  *    device pointers owned by the CALLER (e.g. torch tensors' data_ptr()); `stream` is a
  *    cudaStream_t passed as void* (NULL = default stream).
  *  - The library owns cm_mesh / cm_system and every internal device buffer; nothing is
- *    allocated inside cm_spmv / cm_cg_solve / cm_field_rhs / cm_gspm_step.
+ *    allocated inside cm_spmv / cm_cg_solve* / cm_field_rhs / cm_gspm_step.  Two calls may allocate:
+ *    cm_hysteresis_run (a capture stream, the graph, logs grown to max_fields) and cm_volume_average
+ *    (a library-order staging copy kept in the mesh, grown on demand).
+ *  - Calls on one cm_system, and cm_volume_average calls on one cm_mesh, share scratch buffers: they
+ *    must not run concurrently (one stream at a time per handle).
  *  - All field vectors are in USER node order, interleaved [node][component], of the
  *    system's dtype (double for CM_F64, float for CM_F32).  The locality reordering is
  *    internal; cm_mesh_get exposes it for bit-exact structure parity.
@@ -41,6 +45,10 @@ typedef enum { CM_REORDER_NONE = 0, CM_REORDER_MORTON = 1, CM_REORDER_RCM = 2 } 
  * identity rows on non-magnetic ("dead") nodes.  MASS = M_m = F^GS of Eq. 13.
  * K_MECH: 3x3 blocks, clamped DOFs. */
 typedef enum { CM_MAT_K_MS = 0, CM_MAT_K_GS1 = 1, CM_MAT_K_GS2 = 2, CM_MAT_MASS = 3, CM_MAT_K_MECH = 4 } cm_matrix_id;
+
+/* Preconditioner of the CG solves.  The paper runs plain CG ("no preconditioner") and names preconditioning as
+ * future work; CM_PC_JACOBI is z = r / diag(A) with the diagonal of the constrained matrix as stored. */
+typedef enum { CM_PC_NONE = 0, CM_PC_JACOBI = 1 } cm_precond;
 
 /* Outputs of cm_field_rhs (Eq. 14; Eq. 15). */
 typedef enum {
@@ -94,6 +102,10 @@ typedef struct {
                             (Eq. D.2), row-major; all zeros = identity.  The library forms C_sim = M C M^T (Eq. D.3-D.4) and
                             evaluates E0(m), the anisotropy and the magnetoelastic field in crystal axes (Alg. D.1).
                             Not a proper rotation: CM_E_BADARG. */
+    double sigma_ext[6]; /* uniform external stress of Eq. 1 (energy term -sigma_ext : E), Pa, simulation frame, tensor
+                            components xx,yy,zz,yz,xz,xy.  DESIGN.md R17: with E = sym grad u it is one more mechanical
+                            right-hand-side term, sum_e V_e sigma_ext,ab d_b phi_i over ALL elements; the homogeneous-strain
+                            treatment of periodic domains (defined in the paper's ref. [2] only) is not built. */
 } cm_material;
 
 typedef struct {
@@ -104,6 +116,7 @@ typedef struct {
     double cg_tol;        /* stop when ||r||_2 < cg_tol ||b||_2 */
     int cg_maxiter;
     int cg_fixed_iters;   /* >= 0: run exactly this many iterations in every solve; < 0: off */
+    int cg_precond;       /* cm_precond of every solve of the step; CM_PC_NONE = the paper's unpreconditioned CG */
 } cm_step_params;
 
 /* it_gs / res_gs slots: 0-2 g^n components, 3-4 g*_1, g*_2, 5-7 m** components. */
@@ -191,6 +204,19 @@ int cm_cg_solve(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev,
  * iteration; iters_out / relres_out have 3 entries. */
 int cm_cg_solve3(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter,
                  int fixed_iters, int *iters_out, double *relres_out, void *stream);
+
+/* The same solves with a preconditioner (cm_precond).  The stopping rule is unchanged (||r||_2 < tol ||b||_2 on the
+ * unpreconditioned recurrence residual); CM_PC_NONE gives cm_cg_solve / cm_cg_solve3 bit for bit.  CM_MAT_MASS has no
+ * Jacobi preconditioner (it is singular on non-magnetic nodes): BADARG. */
+int cm_cg_solve_pc(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter,
+                   int fixed_iters, int precond, int *iters_out, double *relres_out, void *stream);
+int cm_cg_solve3_pc(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter,
+                    int fixed_iters, int precond, int *iters_out, double *relres_out, void *stream);
+/* Residual history of the solves that follow (on != 0): the kernel records ||r_k|| / ||b|| before iteration k,
+ * k = 0 .. iters, per right-hand side (up to 65536 iterations).  cm_cg_history copies the history of the LAST solve to
+ * host_out ([k][n_rhs] doubles, n_rhs = 1, or 3 for cm_cg_solve3*), at most `capacity` doubles; *n_out = entries written. */
+int cm_cg_history_enable(cm_system *sys, int on);
+int cm_cg_history(cm_system *sys, double *host_out, long capacity, long *n_out);
 
 /* Element-wise gather / compute / deterministic gather-scatter assembly (see cm_rhs_id).  m_dev: N x 3;
  * U_dev: N (may be NULL when DEMAG is off); u_dev: N x 3 (may be NULL when MAGEL is off); coeff: dtau or

@@ -24,11 +24,12 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
     0, -1, -2, -3, -4, -5, -6, -7
 (CM_GET_COUNTS, CM_GET_ORDER, CM_GET_IPERM, CM_GET_TETS, CM_GET_TET_ORDER, CM_GET_ROWPTR, CM_GET_COLIDX, CM_GET_N2E_PTR,
  CM_GET_N2E) = range(9)
+CM_PC_NONE, CM_PC_JACOBI = 0, 1
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
 EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_hex_wrapped", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
-           "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_field_rhs", "cm_volume_average",
+           "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_cg_solve_pc", "cm_cg_solve3_pc", "cm_cg_history_enable", "cm_cg_history", "cm_field_rhs", "cm_volume_average",
            "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
 
@@ -42,12 +43,13 @@ class CmError(RuntimeError):
 class cm_material(C.Structure):
     _fields_ = [("Ms", C.c_double), ("Aex", C.c_double), ("K1", C.c_double), ("lambda100", C.c_double),
                 ("lambda111", C.c_double), ("alpha", C.c_double), ("gamma", C.c_double), ("length_scale", C.c_double),
-                ("Nd", C.c_double * 9), ("n_elastic", C.c_int), ("C_voigt", C.POINTER(C.c_double)), ("R", C.c_double * 9)]
+                ("Nd", C.c_double * 9), ("n_elastic", C.c_int), ("C_voigt", C.POINTER(C.c_double)), ("R", C.c_double * 9),
+                ("sigma_ext", C.c_double * 6)]
 
 
 class cm_step_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("Hext", C.c_double * 3), ("terms", C.c_uint), ("gspm_variant", C.c_int),
-                ("cg_tol", C.c_double), ("cg_maxiter", C.c_int), ("cg_fixed_iters", C.c_int)]
+                ("cg_tol", C.c_double), ("cg_maxiter", C.c_int), ("cg_fixed_iters", C.c_int), ("cg_precond", C.c_int)]
 
 
 class cm_step_info(C.Structure):
@@ -98,6 +100,10 @@ def lib():
         L.cm_spmv3.argtypes = [vp, it, vp, vp, vp]
         L.cm_cg_solve.argtypes = [vp, it, vp, vp, db, it, it, C.POINTER(it), C.POINTER(db), vp]
         L.cm_cg_solve3.argtypes = [vp, it, vp, vp, db, it, it, C.POINTER(it), C.POINTER(db), vp]
+        L.cm_cg_solve_pc.argtypes = [vp, it, vp, vp, db, it, it, it, C.POINTER(it), C.POINTER(db), vp]
+        L.cm_cg_solve3_pc.argtypes = [vp, it, vp, vp, db, it, it, it, C.POINTER(it), C.POINTER(db), vp]
+        L.cm_cg_history_enable.argtypes = [vp, it]
+        L.cm_cg_history.argtypes = [vp, vp, lg, C.POINTER(lg)]
         L.cm_field_rhs.argtypes = [vp, it, vp, vp, vp, C.POINTER(cm_step_params), db, vp, vp]
         L.cm_volume_average.argtypes = [vp, it, vp, it, C.POINTER(db), vp]
         L.cm_gspm_step.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
@@ -139,9 +145,9 @@ def _dp(t):
     return None if t is None else C.c_void_p(t.data_ptr())
 
 
-def make_params(dt, Hext=(0, 0, 0), terms=0, variant=0, cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1):
+def make_params(dt, Hext=(0, 0, 0), terms=0, variant=0, cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1, cg_precond=CM_PC_NONE):
     return cm_step_params(dt, (C.c_double * 3)(*[float(h) for h in Hext]), int(terms), int(variant), cg_tol, int(cg_maxiter),
-                          int(cg_fixed_iters))
+                          int(cg_fixed_iters), int(cg_precond))
 
 
 def periodic_wrap(xyz, axes: int, rel_tol: float = 1e-9):
@@ -230,7 +236,9 @@ class System:
         m = cm_material(material.Ms, material.Aex, material.K1, material.lambda100, material.lambda111, material.alpha,
                         material.gamma, material.length_scale, (C.c_double * 9)(*material.Nd),
                         0 if Cv is None else Cv.shape[0], None if Cv is None else Cv.ctypes.data_as(C.POINTER(C.c_double)),
-                        (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())))
+                        (C.c_double * 9)(*(np.zeros(9) if getattr(material, "R", None) is None else np.asarray(material.R, float).ravel())),
+                        (C.c_double * 6)(*(np.zeros(6) if getattr(material, "sigma_ext", None) is None
+                                           else np.asarray(material.sigma_ext, float).ravel())))
         clamp = _np(clamp_dof, np.uint8)
         self.h = C.c_void_p()
         _check(L.cm_assemble_csr(mesh.h, C.byref(m), self.cm_dtype, dt, _hp(clamp), pin_node, _stream(), C.byref(self.h)))
@@ -266,18 +274,35 @@ class System:
         _check(lib().cm_spmv3(self.h, mat, _dp(x), _dp(y), _stream()))
         return y
 
-    def cg_solve(self, mat, b, x, tol=1e-7, maxiter=100000, fixed_iters=-1):
-        """In place on x.  Returns (iters, relres, status)."""
+    def cg_solve(self, mat, b, x, tol=1e-7, maxiter=100000, fixed_iters=-1, precond=None):
+        """In place on x.  Returns (iters, relres, status).  precond: None = cm_cg_solve, else cm_cg_solve_pc."""
         it = C.c_int(); res = C.c_double()
-        rc = _check(lib().cm_cg_solve(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, C.byref(it),
-                                      C.byref(res), _stream()), allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
-        return it.value, res.value, rc
+        if precond is None:
+            rc = lib().cm_cg_solve(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, C.byref(it),
+                                   C.byref(res), _stream())
+        else:
+            rc = lib().cm_cg_solve_pc(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, int(precond),
+                                      C.byref(it), C.byref(res), _stream())
+        return it.value, res.value, _check(rc, allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
 
-    def cg_solve3(self, mat, b, x, tol=1e-7, maxiter=100000, fixed_iters=-1):
+    def cg_solve3(self, mat, b, x, tol=1e-7, maxiter=100000, fixed_iters=-1, precond=None):
         it = (C.c_int * 3)(); res = (C.c_double * 3)()
-        rc = _check(lib().cm_cg_solve3(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, it, res,
-                                       _stream()), allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
-        return list(it), list(res), rc
+        if precond is None:
+            rc = lib().cm_cg_solve3(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, it, res, _stream())
+        else:
+            rc = lib().cm_cg_solve3_pc(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, int(precond), it,
+                                       res, _stream())
+        return list(it), list(res), _check(rc, allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
+
+    def cg_history_enable(self, on=True):
+        _check(lib().cm_cg_history_enable(self.h, int(on)))
+
+    def cg_history(self, n_rhs=1, cap=3 << 16):
+        """Residual history of the last cg_solve* call: array [k] (n_rhs = 1) or [k][3]."""
+        a = np.zeros(cap); n = C.c_long()
+        _check(lib().cm_cg_history(self.h, _hp(a), cap, C.byref(n)))
+        a = a[:n.value]
+        return a if n_rhs == 1 else a.reshape(-1, n_rhs)
 
     def field_rhs(self, rhs_id, m, U=None, u=None, params: Optional[cm_step_params] = None, coeff=0.0):
         import torch

@@ -172,7 +172,8 @@ template <typename T>
 static int api_spmv(System<T> *S, cm_matrix_id id, int mode, const void *x, void *y, cudaStream_t st)
 {
     const int nc = (mode == MODE_CSR1) ? 1 : 3;
-    CM_TRY(sys_permute_in<T>(S, (const T *)x, S->xin, nc, st));
+    // the three-right-hand-side product gathers from a padded copy, four words per node
+    CM_TRY(sys_permute_in<T>(S, (const T *)x, S->xin, mode == MODE_CSR3 ? -3 : nc, st));
     CM_TRY(sys_spmv<T>(S, id, mode, S->xin, S->xout, st));
     CM_TRY(sys_permute_out<T>(S, S->xout, (T *)y, nc, st));
     return CM_OK;
@@ -197,14 +198,15 @@ extern "C" int cm_spmv3(cm_system *sys, cm_matrix_id id, const void *x_dev, void
 
 // ---------------------------------------------------------------- CG
 template <typename T>
-static int api_cg(System<T> *S, cm_matrix_id id, int mode, const void *b, void *x, double tol, int maxiter, int fixed, int *iters,
-                  double *relres, cudaStream_t st)
+static int api_cg(System<T> *S, cm_matrix_id id, int mode, const void *b, void *x, double tol, int maxiter, int fixed, int precond,
+                  int *iters, double *relres, cudaStream_t st)
 {
     const int nc = (mode == MODE_CSR1) ? 1 : 3, nr = (mode == MODE_CSR3) ? 3 : 1;
     const int cls = id == CM_MAT_K_MS ? CM_PROF_CG_MS : (id == CM_MAT_K_MECH ? CM_PROF_CG_MECH : CM_PROF_CG_GS);
     CM_TRY(sys_permute_in<T>(S, (const T *)b, S->bvec, nc, st));
     CM_TRY(sys_permute_in<T>(S, (const T *)x, S->xin, nc, st));
-    CM_TRY(sys_cg<T>(S, id, mode, S->bvec, S->xin, tol, maxiter, fixed, nr == 3 ? 7u : 1u, 7, cls, st));
+    CM_TRY(sys_cg<T>(S, id, mode, S->bvec, S->xin, tol, maxiter, fixed, nr == 3 ? 7u : 1u, 7, cls, precond, st));
+    S->hist_nr = nr;
     CM_TRY(sys_permute_out<T>(S, S->xin, (T *)x, nc, st));
     CM_CUDA(cudaMemcpyAsync(S->h_res + 7, S->d_res + 7, sizeof(CgResult), cudaMemcpyDeviceToHost, st));
     CM_CUDA(cudaStreamSynchronize(st));
@@ -216,29 +218,60 @@ static int api_cg(System<T> *S, cm_matrix_id id, int mode, const void *b, void *
         S->prof.cg_iters[cls] += R.iters[c];
         mxit = std::max(mxit, R.iters[c]);
     }
-    S->prof.cg_passes[cls] += mxit;
+    S->prof.cg_passes[cls] += mxit + 1; // one matrix pass per iteration plus the r0 = b - A x0 pass
+    S->hist_len = (long)std::min<long>((long)(mxit + 1) * nr, CM_HIST_CAP / nr * nr);
     return R.status;
 }
 
-extern "C" int cm_cg_solve(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters,
-                           int *iters_out, double *relres_out, void *stream)
+extern "C" int cm_cg_solve_pc(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters,
+                              int precond, int *iters_out, double *relres_out, void *stream)
 {
     CM_TRY(check_sys(sys, "cm_cg_solve"));
     if (!b_dev || !x_dev || (int)id < 0 || (int)id > CM_MAT_K_MECH) { cm_set_error("cm_cg_solve: bad argument"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
     const int mode = mode_of(id);
-    return SYS_DISPATCH(sys, api_cg<double>(S, id, mode, b_dev, x_dev, tol, maxiter, fixed_iters, iters_out, relres_out, st),
-                        api_cg<float>(S, id, mode, b_dev, x_dev, tol, maxiter, fixed_iters, iters_out, relres_out, st));
+    return SYS_DISPATCH(sys, api_cg<double>(S, id, mode, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st),
+                        api_cg<float>(S, id, mode, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st));
+}
+
+extern "C" int cm_cg_solve3_pc(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters,
+                               int precond, int *iters_out, double *relres_out, void *stream)
+{
+    CM_TRY(check_sys(sys, "cm_cg_solve3"));
+    if (!b_dev || !x_dev || (int)id < 0 || (int)id >= CM_MAT_K_MECH) { cm_set_error("cm_cg_solve3: bad argument (scalar matrices only)"); return CM_E_BADARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return SYS_DISPATCH(sys, api_cg<double>(S, id, MODE_CSR3, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st),
+                        api_cg<float>(S, id, MODE_CSR3, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st));
+}
+
+extern "C" int cm_cg_solve(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters,
+                           int *iters_out, double *relres_out, void *stream)
+{
+    return cm_cg_solve_pc(sys, id, b_dev, x_dev, tol, maxiter, fixed_iters, CM_PC_NONE, iters_out, relres_out, stream);
 }
 
 extern "C" int cm_cg_solve3(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters,
                             int *iters_out, double *relres_out, void *stream)
 {
-    CM_TRY(check_sys(sys, "cm_cg_solve3"));
-    if (!b_dev || !x_dev || (int)id < 0 || (int)id >= CM_MAT_K_MECH) { cm_set_error("cm_cg_solve3: bad argument (scalar matrices only)"); return CM_E_BADARG; }
-    cudaStream_t st = (cudaStream_t)stream;
-    return SYS_DISPATCH(sys, api_cg<double>(S, id, MODE_CSR3, b_dev, x_dev, tol, maxiter, fixed_iters, iters_out, relres_out, st),
-                        api_cg<float>(S, id, MODE_CSR3, b_dev, x_dev, tol, maxiter, fixed_iters, iters_out, relres_out, st));
+    return cm_cg_solve3_pc(sys, id, b_dev, x_dev, tol, maxiter, fixed_iters, CM_PC_NONE, iters_out, relres_out, stream);
+}
+
+extern "C" int cm_cg_history_enable(cm_system *sys, int on)
+{
+    CM_TRY(check_sys(sys, "cm_cg_history_enable"));
+    sys->impl->hist_on = on != 0;
+    sys->impl->hist_len = 0;
+    return CM_OK;
+}
+
+extern "C" int cm_cg_history(cm_system *sys, double *host_out, long capacity, long *n_out)
+{
+    CM_TRY(check_sys(sys, "cm_cg_history"));
+    if (!host_out || !n_out || capacity < 0) { cm_set_error("cm_cg_history: bad argument"); return CM_E_BADARG; }
+    const long n = std::min(capacity, sys->impl->hist_len);
+    if (n > 0) CM_CUDA(cudaMemcpy(host_out, sys->impl->d_hist, n * sizeof(double), cudaMemcpyDeviceToHost));
+    *n_out = n;
+    return CM_OK;
 }
 
 // ---------------------------------------------------------------- field / RHS

@@ -312,6 +312,8 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         S->rot = !ident;
     }
     S->n_elastic = mat->n_elastic > 0 ? mat->n_elastic : 0;
+    S->has_sext = false;
+    for (int q = 0; q < 6; q++) { S->sext[q] = mat->sigma_ext[q] / mu0Ms2; S->has_sext = S->has_sext || mat->sigma_ext[q] != 0.0; }
     S->pin = M->iperm[pin_user];
     int dev = 0;
     CM_CUDA(cudaGetDevice(&dev));
@@ -331,7 +333,12 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     if (S->n_elastic) CM_TRY(alloc(&S->Dmech, 3 * N));
 
     // elastic constants C* = C / (mu0 Ms^2): fp64 for assembly, T for the element kernels
-    double *Cd = nullptr;
+    // set-up scratch (fp64 matrices on the CSR pattern, volumes, C*): freed on every exit path
+    struct Scratch {
+        double *Cd = nullptr, *Vd = nullptr, *vsum = nullptr, *K = nullptr, *Km = nullptr, *Mm = nullptr, *Kme = nullptr;
+        ~Scratch() { cudaFree(Cd); cudaFree(Vd); cudaFree(vsum); cudaFree(K); cudaFree(Km); cudaFree(Mm); cudaFree(Kme); }
+    } scr;
+    double *&Cd = scr.Cd;
     if (S->n_elastic) {
         std::vector<double> Cs(36 * S->n_elastic);
         std::vector<T> Ct(36 * S->n_elastic);
@@ -401,7 +408,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     }
     // geometry
     const bool hex = M->nen == 8;
-    double *Vd = nullptr, *vsum = nullptr;
+    double *&Vd = scr.Vd, *&vsum = scr.vsum;
     const int B = 256;
     if (!hex) {
         CM_CUDA(cudaMalloc((void **)&Vd, Ne * sizeof(double)));
@@ -418,7 +425,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         S->Vtot = M->vtot_m3 / (ld * ld * ld); S->Vmag = M->vmag_m3 / (ld * ld * ld);
     }
     // matrices: fp64 scratch on the pattern
-    double *K = nullptr, *Km = nullptr, *Mm = nullptr, *Kme = nullptr;
+    double *&K = scr.K, *&Km = scr.Km, *&Mm = scr.Mm, *&Kme = scr.Kme;
     CM_TRY(alloc(&K, nnz)); CM_TRY(alloc(&Km, nnz)); CM_TRY(alloc(&Mm, nnz));
     if (S->n_elastic) CM_TRY(alloc(&Kme, 9 * nnz));
     const int BA = 128;
@@ -441,7 +448,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
                                                                  S->Mm, S->Kmech, S->Dms, S->Dgs1, S->Dgs2, S->Dmech);
     CM_CUDA(cudaGetLastError());
     CM_CUDA(cudaStreamSynchronize(st));
-    cudaFree(K); cudaFree(Km); cudaFree(Mm); cudaFree(Kme); cudaFree(Vd); cudaFree(vsum); cudaFree(Cd);
+    for (double **q : {&K, &Km, &Mm, &Kme, &Vd, &vsum, &Cd}) { cudaFree(*q); *q = nullptr; } // before the work vectors are allocated
 
     // work vectors
     T **vecs3[] = {&S->r, &S->Ap, &S->bvec, &S->m, &S->u, &S->hd, &S->hn, &S->gn, &S->gs, &S->ms, &S->mss, &S->xout, &S->stg_m, &S->stg_u};

@@ -84,6 +84,16 @@ __global__ void permute_in_kernel(long N, int nc, const int *__restrict__ order,
     int c = (int)(k - i * nc);
     lib[k] = user[(long)order[i] * nc + c];
 }
+// user [node][3] -> library PADDED [node][4] (order == NULL: identity)
+template <typename T>
+__global__ void permute_in4_kernel(long N, const int *__restrict__ order, const T *__restrict__ user, T *lib4)
+{
+    long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (k >= 3 * N) return;
+    const long i = k / 3;
+    const int c = (int)(k - 3 * i);
+    lib4[4 * i + c] = user[(order ? (long)order[i] : i) * 3 + c];
+}
 template <typename T>
 __global__ void permute_out_kernel(long N, int nc, const int *__restrict__ order, const T *__restrict__ lib, T *user)
 {
@@ -134,6 +144,8 @@ struct ChunkArgs {
     const double *mbar;   // MS
     const T *Cstar;       // MECH, STRESS: 36 words per material, or the 12 of the cubic pattern
     T l1, l2;
+    T sext[6];            // MECH: sigma_ext / (mu0 Ms^2), added to the stress of EVERY element (R17)
+    int has_sext;
     Rot<T> rot;           // App. D: crystal -> simulation frame
     T *hpart;             // [slot][NC]
     double *partial;      // GRADU: per-chunk sums of V_e grad U_e (fp64)
@@ -377,15 +389,20 @@ __global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs
             }
         } else {
             const unsigned em = sem[el];
-            if (!(em & 1u)) {
+            if (!(em & 1u) && !(KIND == EK_MECH && a.has_sext)) {
 #pragma unroll
                 for (int q = 0; q < NOUT; q++) scr[q * ne8 + el] = 0;
             } else if (KIND == EK_MECH) {
-                // S = C*_e : mean_e E0(m);  c_(k,a) = V_e (S grad phi_k)_a
-                T e0v[6], sg[6];
-                mean_E0<T, 3, 0>(a.rot, sin, l, a.l1, a.l2, e0v);
-                if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), e0v, sg);
-                else C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
+                // S = C*_e : mean_e E0(m) (magnetic elements) + sigma_ext (all elements);  c_(k,a) = V_e (S grad phi_k)_a
+                T e0v[6], sg[6] = {0, 0, 0, 0, 0, 0};
+                if (em & 1u) {
+                    mean_E0<T, 3, 0>(a.rot, sin, l, a.l1, a.l2, e0v);
+                    if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), e0v, sg);
+                    else C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
+                }
+                if (a.has_sext)
+#pragma unroll
+                    for (int q = 0; q < 6; q++) sg[q] += a.sext[q];
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
                     scr[(3 * k + 0) * ne8 + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
@@ -536,16 +553,18 @@ __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const 
 }
 
 // ---------------------------------------------------------------- pointwise GSPM algebra (S9, S11, S12)
-// f = base + c h   (3N entries)
+// f = base + c h per node; f is PADDED, four words per node (what the three-right-hand-side products gather)
 template <typename T>
-__global__ void axpby_kernel(long n, const T *__restrict__ base, const T *__restrict__ h, T c, T *f)
+__global__ void axpby_kernel(long N, const T *__restrict__ base, const T *__restrict__ h, T c, T *f4)
 {
     long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (k < n) f[k] = base[k] + c * h[k];
+    if (k >= 3 * N) return;
+    const long i = k / 3;
+    f4[4 * i + (k - 3 * i)] = base[k] + c * h[k];
 }
 
 // Step 2, first part.  variant 0: m*_1, m*_2 from level-n values; f_a = m*_a + dtau h_a[m^n], a = 1, 2.
-// variant 1, stage 0: m*_1 and f_1 only; stage 1: m*_2 = m_2 + (g^n_3 m*_1 - g*_1 m_3) and f_2.
+// variant 1, stage 0: m*_1 and f_1 only; stage 1: m*_2 = m_2 + (g^n_3 m*_1 - g*_1 m_3) and f_2.  f is padded [node][4].
 template <typename T>
 __global__ void gs_step2_kernel(long N, int variant, int stage, const T *__restrict__ m, const T *__restrict__ gn,
                                 const T *__restrict__ gs, const T *__restrict__ hn, T dtau, T *ms, T *f)
@@ -556,16 +575,16 @@ __global__ void gs_step2_kernel(long N, int variant, int stage, const T *__restr
     if (variant == 0 || stage == 0) {
         const T s0 = m0 + (gn[3 * i + 1] * m2 - gn[3 * i + 2] * m1);
         ms[3 * i] = s0;
-        f[3 * i] = s0 + dtau * hn[3 * i];
+        f[4 * i] = s0 + dtau * hn[3 * i];
     }
     if (variant == 0) {
         const T s1 = m1 + (gn[3 * i + 2] * m0 - gn[3 * i] * m2);
         ms[3 * i + 1] = s1;
-        f[3 * i + 1] = s1 + dtau * hn[3 * i + 1];
+        f[4 * i + 1] = s1 + dtau * hn[3 * i + 1];
     } else if (stage == 1) {
         const T s1 = m1 + (gn[3 * i + 2] * ms[3 * i] - gs[3 * i] * m2);
         ms[3 * i + 1] = s1;
-        f[3 * i + 1] = s1 + dtau * hn[3 * i + 1];
+        f[4 * i + 1] = s1 + dtau * hn[3 * i + 1];
     }
 }
 
@@ -607,6 +626,13 @@ __global__ void project_kernel(long N, const uchar *__restrict__ live, const T *
 template <typename T>
 int sys_permute_in(System<T> *S, const T *user, T *lib, int nc, cudaStream_t st)
 {
+    if (nc == -3) { // three components into the padded layout
+        S->prof.begin(CM_PROF_POINTWISE, st);
+        permute_in4_kernel<T><<<nblk(3 * S->N), BS, 0, st>>>(S->N, S->mesh->identity ? nullptr : S->mesh->d_order, user, lib);
+        S->prof.end(st);
+        LAUNCH_CHECK();
+        return CM_OK;
+    }
     const long n = S->N * nc;
     if (S->mesh->identity) { CM_CUDA(cudaMemcpyAsync(lib, user, n * sizeof(T), cudaMemcpyDeviceToDevice, st)); return CM_OK; }
     S->prof.begin(CM_PROF_POINTWISE, st);
@@ -663,6 +689,8 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     a.hexes = M->d_tets; a.ghexes = M->d_gtets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_gxyz; a.ld = S->ld; a.N = S->N;
     a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
+    for (int q = 0; q < 6; q++) a.sext[q] = (T)S->sext[q];
+    a.has_sext = S->has_sext ? 1 : 0;
     a.hpart = S->hpart; a.partial = S->red;
     return a;
 }
@@ -705,7 +733,7 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
         for (int s = a.n2e_ptr[i]; s < a.n2e_ptr[i + 1]; s++) {
             const int e = a.n2e[s] >> 3, k = a.n2e[s] & 7;
             const unsigned em = a.emat[e];
-            if ((KIND == EK_MECH || KIND == EK_STRESS) && !(em & 1u)) continue;
+            if ((KIND == EK_MECH || KIND == EK_STRESS) && !(em & 1u) && !(KIND == EK_MECH && a.has_sext)) continue;
             int t[8];
             double X[8][3];
 #pragma unroll
@@ -716,7 +744,7 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
                 for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * gc + d] * ild;
             }
             T e0c[8][6]; // E0 at the 8 corners (MECH, STRESS)
-            if (KIND == EK_MECH || KIND == EK_STRESS) {
+            if ((KIND == EK_MECH || KIND == EK_STRESS) && (em & 1u)) {
                 const T *w = KIND == EK_MECH ? a.in0 : a.in1;
                 for (int c = 0; c < 8; c++) {
                     const T mk[3] = {w[3 * (long)t[c]], w[3 * (long)t[c] + 1], w[3 * (long)t[c] + 2]};
@@ -743,9 +771,10 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
                     for (int d = 0; d < 3; d++) acc[d] += det * (T)phid[k] * gU[d];
                 } else {
                     T eps[6] = {0, 0, 0, 0, 0, 0}, sg[6];
-                    for (int c = 0; c < 8; c++)
+                    if (em & 1u)
+                        for (int c = 0; c < 8; c++)
 #pragma unroll
-                        for (int q = 0; q < 6; q++) eps[q] += (T)phid[c] * e0c[c][q];
+                            for (int q = 0; q < 6; q++) eps[q] += (T)phid[c] * e0c[c][q];
                     if (KIND == EK_STRESS) {
                         T H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
                         for (int c = 0; c < 8; c++)
@@ -757,8 +786,14 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
 #pragma unroll
                         for (int q = 0; q < 6; q++) eps[q] = E[q] - eps[q];
                     }
-                    C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+                    if (em & 1u) C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+                    else
+#pragma unroll
+                        for (int q = 0; q < 6; q++) sg[q] = 0;
                     if (KIND == EK_MECH) {
+                        if (a.has_sext)
+#pragma unroll
+                            for (int q = 0; q < 6; q++) sg[q] += a.sext[q];
                         const T gx = (T)gd[k][0], gy = (T)gd[k][1], gz = (T)gd[k][2];
                         acc[0] += det * (sg[0] * gx + sg[5] * gy + sg[4] * gz);
                         acc[1] += det * (sg[5] * gx + sg[1] * gy + sg[3] * gz);
@@ -874,7 +909,7 @@ template <typename T>
 int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t st)
 {
     S->prof.begin(CM_PROF_POINTWISE, st);
-    axpby_kernel<T><<<nblk(3 * S->N), BS, 0, st>>>(3 * S->N, base, h, c, f);
+    axpby_kernel<T><<<nblk(3 * S->N), BS, 0, st>>>(S->N, base, h, c, f);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -889,6 +924,7 @@ static int step_check(System<T> *S, const cm_step_params *p, const T *m_user, co
     const unsigned terms = p->terms;
     if (p->dt != S->dt) { cm_set_error("%s: params->dt differs from the dt given to cm_assemble_csr", fn); return CM_E_BADARG; }
     if ((terms & CM_TERM_MAGEL) && !S->n_elastic) { cm_set_error("%s: MAGEL needs elastic constants", fn); return CM_E_BADARG; }
+    if (p->cg_precond != CM_PC_NONE && p->cg_precond != CM_PC_JACOBI) { cm_set_error("%s: unknown cg_precond %d", fn, p->cg_precond); return CM_E_BADARG; }
     if (((terms & CM_TERM_DEMAG) && !U_user) || ((terms & CM_TERM_MAGEL) && !u_user) || !m_user) {
         cm_set_error("%s: null field pointer", fn);
         return CM_E_BADARG;
@@ -907,50 +943,42 @@ static int step_core(System<T> *S, const cm_step_params *p, const double *hext_d
     const double hext[3] = {p->Hext[0] / S->Ms, p->Hext[1] / S->Ms, p->Hext[2] / S->Ms};
     const T dtau = (T)S->dtau, adtau = (T)(S->alpha * S->dtau);
     const double tol = p->cg_tol;
-    const int mx = p->cg_maxiter, fx = p->cg_fixed_iters;
+    const int mx = p->cg_maxiter, fx = p->cg_fixed_iters, pc = p->cg_precond;
     CM_CUDA(cudaMemsetAsync(S->d_res, 0, 8 * sizeof(CgResult), st));
     // 1. mbar (Eq. 17)
     CM_TRY(sys_mbar(S, S->m, st));
     // 2. magnetostatic solve, warm start (Eq. 5, 9)
     if (terms & CM_TERM_DEMAG) {
         CM_TRY(sys_rhs_ms(S, S->m, S->bvec, st));
-        CM_TRY(sys_cg(S, CM_MAT_K_MS, MODE_CSR1, S->bvec, S->U, tol, mx, fx, 1u, 0, CM_PROF_CG_MS, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_MS, MODE_CSR1, S->bvec, S->U, tol, mx, fx, 1u, 0, CM_PROF_CG_MS, pc, st));
     }
     // 3. demagnetising field (Eq. 4)
     if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) CM_TRY(sys_demag_field(S, S->U, terms, S->hd, st));
     // 4. mechanical equilibrium (Eq. 6, 10), warm start; stress at m^n
     if (terms & CM_TERM_MAGEL) {
         CM_TRY(sys_rhs_mech(S, S->m, S->bvec, st));
-        CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, st));
+        CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, pc, st));
         CM_TRY(sys_stress(S, S->u, S->m, st));
     }
-    // 5. h[m^n];  6. Step 1: g^n
+    // 5. h[m^n];  6. Step 1: g^n.  A Helmholtz solve is ONE launch: b = M_m f, x0 = f, r0 = b - A f in its first pass
     CM_TRY(sys_field(S, S->m, S->hd, hext, terms, S->hn, (T *)nullptr, st, hext_dev));
     CM_TRY(sys_axpby3(S, S->m, S->hn, dtau, S->f, st));
-    CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
-    CM_CUDA(cudaMemcpyAsync(S->gn, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gn, tol, mx, fx, p->gspm_variant == 1 ? 6u : 7u, 2, CM_PROF_CG_GS, st));
+    CM_TRY(sys_helmholtz(S, CM_MAT_K_GS1, S->f, S->gn, tol, mx, fx, p->gspm_variant == 1 ? 6u : 7u, 2, pc, st));
     // 7. Step 2 interleaved with the g* solves
     S->prof.begin(CM_PROF_POINTWISE, st);
     gs_step2_kernel<T><<<nblk(N), BS, 0, st>>>(N, p->gspm_variant, 0, S->m, S->gn, S->gs, S->hn, dtau, S->ms, S->f);
     S->prof.end(st);
     LAUNCH_CHECK();
     if (p->gspm_variant == 0) {
-        CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
-        CM_CUDA(cudaMemcpyAsync(S->gs, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
-        CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gs, tol, mx, fx, 3u, 3, CM_PROF_CG_GS, st));
+        CM_TRY(sys_helmholtz(S, CM_MAT_K_GS1, S->f, S->gs, tol, mx, fx, 3u, 3, pc, st));
     } else {
-        CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
-        CM_CUDA(cudaMemcpyAsync(S->gs, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
-        CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gs, tol, mx, fx, 1u, 3, CM_PROF_CG_GS, st));
+        CM_TRY(sys_helmholtz(S, CM_MAT_K_GS1, S->f, S->gs, tol, mx, fx, 1u, 3, pc, st));
         S->prof.begin(CM_PROF_POINTWISE, st);
         gs_step2_kernel<T><<<nblk(N), BS, 0, st>>>(N, 1, 1, S->m, S->gn, S->gs, S->hn, dtau, S->ms, S->f);
         S->prof.end(st);
         LAUNCH_CHECK();
-        CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
-        // x0 = f for component 2 only (component 1 already holds g*_1)
-        CM_CUDA(cudaMemcpy2DAsync(S->gs + 1, 3 * sizeof(T), S->f + 1, 3 * sizeof(T), sizeof(T), N, cudaMemcpyDeviceToDevice, st));
-        CM_TRY(sys_cg(S, CM_MAT_K_GS1, MODE_CSR3, S->bvec, S->gs, tol, mx, fx, 2u, 4, CM_PROF_CG_GS, st));
+        // x0 = f for component 2 only (component 1 already holds g*_1): the solve writes the masked components
+        CM_TRY(sys_helmholtz(S, CM_MAT_K_GS1, S->f, S->gs, tol, mx, fx, 2u, 4, pc, st));
     }
     S->prof.begin(CM_PROF_POINTWISE, st);
     gs_step2c_kernel<T><<<nblk(N), BS, 0, st>>>(N, S->m, S->gs, S->ms);
@@ -960,9 +988,7 @@ static int step_core(System<T> *S, const cm_step_params *p, const double *hext_d
     if (terms & CM_TERM_MAGEL) CM_TRY(sys_stress(S, S->u, S->ms, st));
     CM_TRY(sys_field(S, S->ms, S->hd, hext, terms, S->hn, (T *)nullptr, st, hext_dev));
     CM_TRY(sys_axpby3(S, S->ms, S->hn, adtau, S->f, st));
-    CM_TRY(sys_spmv(S, CM_MAT_MASS, MODE_CSR3, S->f, S->bvec, st));
-    CM_CUDA(cudaMemcpyAsync(S->mss, S->f, 3 * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    CM_TRY(sys_cg(S, CM_MAT_K_GS2, MODE_CSR3, S->bvec, S->mss, tol, mx, fx, 7u, 5, CM_PROF_CG_GS, st));
+    CM_TRY(sys_helmholtz(S, CM_MAT_K_GS2, S->f, S->mss, tol, mx, fx, 7u, 5, pc, st));
     // 9. Step 4 projection; 10. diagnostics
     {
         const int nb = (int)std::min<long>(RED_BLOCKS, nblk(N));
@@ -1010,12 +1036,16 @@ int sys_step(System<T> *S, const cm_step_params *p, T *m_user, T *U_user, T *u_u
         info->energy = std::numeric_limits<double>::quiet_NaN();
         for (int s = 0; s < 6; s++) worst = std::min(worst, R[s].status);
         // profiler bookkeeping of CG work
-        S->prof.cg_iters[CM_PROF_CG_MS] += R[0].iters[0]; S->prof.cg_passes[CM_PROF_CG_MS] += R[0].iters[0];
-        S->prof.cg_iters[CM_PROF_CG_MECH] += R[1].iters[0]; S->prof.cg_passes[CM_PROF_CG_MECH] += R[1].iters[0];
+        // (a launch makes one matrix pass per iteration plus the r0 = b - A x0 pass)
+        S->prof.cg_iters[CM_PROF_CG_MS] += R[0].iters[0];
+        if (terms & CM_TERM_DEMAG) S->prof.cg_passes[CM_PROF_CG_MS] += R[0].iters[0] + 1;
+        S->prof.cg_iters[CM_PROF_CG_MECH] += R[1].iters[0];
+        if (terms & CM_TERM_MAGEL) S->prof.cg_passes[CM_PROF_CG_MECH] += R[1].iters[0] + 1;
         for (int s = 2; s < 6; s++) {
+            if (s == 4 && p->gspm_variant == 0) continue; // slot 4 is used by variant 1 only
             int mxit = 0;
             for (int a = 0; a < 3; a++) { S->prof.cg_iters[CM_PROF_CG_GS] += R[s].iters[a]; mxit = std::max(mxit, R[s].iters[a]); }
-            S->prof.cg_passes[CM_PROF_CG_GS] += mxit;
+            S->prof.cg_passes[CM_PROF_CG_GS] += mxit + 1;
         }
     }
     return worst;

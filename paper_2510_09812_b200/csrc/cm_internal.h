@@ -146,6 +146,8 @@ struct SystemBase {
     double Nd[9] = {0};
     double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}; // App. D: crystal -> simulation frame
     bool rot = false;
+    double sext[6] = {0}; // sigma_ext / (mu0 Ms^2), tensor components xx,yy,zz,yz,xz,xy (Eq. 1; R17)
+    bool has_sext = false;
     int n_elastic = 0;
     double Vtot = 0, Vmag = 0;
     double ld = 1;  // length scale l_d, metres
@@ -153,6 +155,10 @@ struct SystemBase {
     int pin = 0; // library index
     int num_sms = 0;
     Profiler prof;
+    double *d_hist = nullptr;  // residual history of the last solve (cm_cg_history), CM_HIST_CAP doubles
+    bool hist_on = false;
+    long hist_len = 0;
+    int hist_nr = 1;
     virtual ~SystemBase() {}
 };
 
@@ -186,8 +192,6 @@ struct System : SystemBase {
     double *partial = nullptr;
     int grid_cap = 0;
     CgResult *d_res = nullptr, *h_res = nullptr; // 8 slots
-    double *d_hist = nullptr;  // residual history of the last solve (cm_cg_history), CM_HIST_CAP doubles
-    bool hist_on = false;
     // step state (library order)
     T *m = nullptr, *U = nullptr, *u = nullptr, *hd = nullptr, *hn = nullptr, *f = nullptr, *gn = nullptr, *gs = nullptr,
       *ms = nullptr, *mss = nullptr, *xin = nullptr, *xout = nullptr;
@@ -251,7 +255,7 @@ template <typename T> int sys_cg(System<T> *S, cm_matrix_id id, int mode, const 
 template <typename T> int sys_helmholtz(System<T> *S, cm_matrix_id id, const T *f4, T *x, double tol, int maxiter, int fixed, unsigned mask,
                                         int slot, int precond, cudaStream_t st);
 template <typename T> int sys_get_values(const System<T> *S, cm_matrix_id id, void *host_out, long capacity);
-template <typename T> int sys_permute_in(System<T> *S, const T *user, T *lib, int ncomp, cudaStream_t st);
+template <typename T> int sys_permute_in(System<T> *S, const T *user, T *lib, int ncomp, cudaStream_t st); // ncomp = -3: [node][3] -> padded [node][4]
 template <typename T> int sys_permute_out(System<T> *S, const T *lib, T *user, int ncomp, cudaStream_t st);
 template <typename T> int sys_mbar(System<T> *S, const T *m_lib, cudaStream_t st);                         // -> dscal[0..2]
 template <typename T> int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st);                 // uses dscal[0..2]

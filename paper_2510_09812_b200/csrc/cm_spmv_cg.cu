@@ -536,7 +536,7 @@ __global__ void __launch_bounds__(CM_NT, 2) cg_kernel(CgArgs<T> a)
         double v[9];
 #pragma unroll
         for (int k = 0; k < 9; k++) v[k] = 0;
-        if (HELM) {
+        if constexpr (HELM) {
             HelmStore<T, PRE> st{a.r, a.x, a.f4, a.diag, a.mask};
             spmv_units<T, MODE, 4, 2>(a.A, a.Mval, a.f4, st, u0, u1, v);
         } else {

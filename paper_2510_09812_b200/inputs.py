@@ -168,6 +168,12 @@ class HexMesh:
     def n_tets(self) -> int:          # number of elements (the name the binding and the oracle read)
         return int(self.hexes.shape[0])
 
+    def live_nodes(self) -> np.ndarray:
+        """Nodes touched by at least one magnetic cell (mesh bookkeeping only)."""
+        live = np.zeros(self.n_nodes, dtype=bool)
+        live[self.hexes[self.magnetic != 0].ravel()] = True
+        return live
+
 
 def hex_box(grid, box, jitter=0.15, seed_mesh=1, seed_perm=2, permute=True) -> HexMesh:
     """Structured nx x ny x nz node grid of linear hexahedra (the paper's Fig. 2-3 meshes): same node numbering,

@@ -1,0 +1,242 @@
+"""GPU parity of the rows built in round 2 on top of the tetrahedral / hexahedral path:
+  * Jacobi-preconditioned CG (the paper's future work): cm_cg_solve_pc / cm_cg_solve3_pc / cg_precond of the step
+    against the oracle's PCG -- iteration counts +-1, iterates of a fixed number of iterations element by element, residual
+    histories, CM_PC_NONE bit-identical to cm_cg_solve;
+  * the fused Helmholtz start of the step (b = M_m f, x0 = f, r0 = b - A f inside the CG launch) is exercised by every
+    multi-step test of the suite; here the step runs with both preconditioners;
+  * uniform external stress sigma_ext (Eq. 1; R17): mechanical right-hand side and whole steps on
+    tetrahedra and hexahedra."""
+import numpy as np
+import pytest
+
+from paper_2510_09812_b200 import inputs
+from paper_2510_09812_b200.inputs import TERM_ANIS, TERM_DEMAG, TERM_FARFIELD, TERM_MAGEL, TERM_ZEEMAN
+
+pytestmark = pytest.mark.gpu
+NM = 1e-9
+ALL = TERM_ANIS | TERM_ZEEMAN | TERM_DEMAG | TERM_FARFIELD | TERM_MAGEL
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def cm():
+    from paper_2510_09812_b200 import binding
+    binding.lib()
+    return binding
+
+
+def rel(a, b):
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
+
+
+def mat2(**kw):
+    C = inputs.isotropic_voigt(200e9, 0.3)
+    return inputs.Material(C_voigt=np.stack([C, 2 * C]), **kw)
+
+
+def inclusion_mesh():
+    mesh = inputs.kuhn_box((23, 19, 17), (66 * NM, 54 * NM, 48 * NM), seed_mesh=51, seed_perm=52)
+    return inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (14 * NM, 12 * NM, 10 * NM))
+
+
+@pytest.fixture(scope="module", params=["f64", "f32"])
+def case(request, cm, oracle_mod, torch):
+    mesh = inclusion_mesh()
+    clamp = inputs.clamp_bottom(mesh)
+    dtype = request.param
+    gm = cm.Mesh(mesh.xyz, mesh.tets, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+    gs = cm.System(gm, mat2(), 2e-12, dtype, clamp, 5)
+    o = oracle_mod.Oracle(mesh, mat2(), 2e-12, clamp_dof=clamp, pin_node=5, dtype=dtype)   # fp32 build against the fp32 twin for counts
+    o64 = o if dtype == "f64" else oracle_mod.Oracle(mesh, mat2(), 2e-12, clamp_dof=clamp, pin_node=5, dtype="f64")
+    td = torch.float64 if dtype == "f64" else torch.float32
+    return dict(mesh=mesh, clamp=clamp, gm=gm, gs=gs, o=o, o64=o64, dtype=dtype, td=td, torch=torch)
+
+
+def test_jacobi_pcg_against_oracle(case, cm, oracle_mod):
+    gs, o, o64, torch, td = case["gs"], case["o"], case["o64"], case["torch"], case["td"]
+    f64 = case["dtype"] == "f64"
+    N = o.N
+    rng = np.random.default_rng(110)
+    tol_cg = 1e-10 if f64 else 1e-5
+    for mat_g, mat_o, n in ((cm.CM_MAT_K_MS, oracle_mod.MAT_K_MS, N), (cm.CM_MAT_K_GS1, oracle_mod.MAT_K_GS1, N),
+                            (cm.CM_MAT_K_MECH, oracle_mod.MAT_K_MECH, 3 * N)):
+        b = rng.normal(size=n).astype(gs.np_dtype)
+        if mat_g == cm.CM_MAT_K_MS:
+            b[5] = 0
+        if mat_g == cm.CM_MAT_K_MECH:
+            b[case["clamp"].astype(bool)] = 0
+        shape = (N, 3) if mat_g == cm.CM_MAT_K_MECH else (N,)
+        bd = torch.as_tensor(b.reshape(shape), dtype=td, device="cuda")
+        # converged solve: counts +-1 against the oracle's PCG in the same precision, solution against a tight fp64 solve
+        x = torch.zeros(shape, dtype=td, device="cuda")
+        gs.cg_history_enable(True)
+        it, res, rc = gs.cg_solve(mat_g, bd, x, tol=tol_cg, precond=cm.CM_PC_JACOBI)
+        hist = gs.cg_history()
+        gs.cg_history_enable(False)
+        xo, ito, reso, rco = o.cg_pc(mat_o, b, tol=tol_cg, precond=1)
+        assert rc == 0 and rco == 0
+        assert abs(it - ito) <= (1 if f64 else max(2, ito // 50)), (mat_g, it, ito)
+        assert res < tol_cg
+        x64, _, _, _ = o64.cg_pc(mat_o, b.astype(np.float64), tol=1e-13, precond=1)
+        assert rel(x.cpu().numpy().ravel(), x64) < (1e-7 if f64 else 2e-3), mat_g
+        # residual history: the same curve as the oracle's, iteration by iteration (the curve, not only its end)
+        _, _, ho = o64.cg_history(mat_o, b.astype(np.float64), tol=tol_cg, precond=1)
+        k = min(len(hist), len(ho)) - 2
+        assert len(hist) == it + 1 and k > 5
+        assert np.allclose(hist[:k], ho[:k], rtol=1e-6 if f64 else 5e-2), mat_g
+        # the preconditioner must pay on the mechanical matrix (x2-stiffness inclusion): not more iterations than plain CG
+        if mat_g == cm.CM_MAT_K_MECH:
+            xp = torch.zeros(shape, dtype=td, device="cuda")
+            itp, _, _ = gs.cg_solve(mat_g, bd, xp, tol=tol_cg)
+            assert it <= itp, (it, itp)
+        # three iterations: identical algorithm step by step
+        x = torch.zeros(shape, dtype=td, device="cuda")
+        it3, res3, _ = gs.cg_solve(mat_g, bd, x, fixed_iters=3, precond=cm.CM_PC_JACOBI)
+        xo3, ito3, reso3, _ = o64.cg_pc(mat_o, b.astype(np.float64), fixed=3, precond=1)
+        assert it3 == 3 and ito3 == 3
+        assert rel(x.cpu().numpy().ravel(), xo3) < (1e-11 if f64 else 1e-4)
+        assert res3 == pytest.approx(reso3, rel=1e-9 if f64 else 1e-3)
+        # CM_PC_NONE through the _pc entry point == cm_cg_solve, bit for bit
+        xa = torch.zeros(shape, dtype=td, device="cuda"); xb = torch.zeros(shape, dtype=td, device="cuda")
+        ita, _, _ = gs.cg_solve(mat_g, bd, xa, tol=tol_cg)
+        itb, _, _ = gs.cg_solve(mat_g, bd, xb, tol=tol_cg, precond=cm.CM_PC_NONE)
+        assert ita == itb and torch.equal(xa, xb)
+    # the mass matrix has no Jacobi preconditioner (singular on dead nodes); unknown codes are refused
+    x = torch.zeros(N, dtype=td, device="cuda")
+    with pytest.raises(cm.CmError) as e:
+        gs.cg_solve(cm.CM_MAT_MASS, x, x.clone(), precond=cm.CM_PC_JACOBI)
+    assert e.value.code == cm.CM_E_BADARG
+    with pytest.raises(cm.CmError):
+        gs.cg_solve(cm.CM_MAT_K_MS, x, x.clone(), precond=7)
+
+
+def test_jacobi_pcg_three_rhs(case, cm, oracle_mod):
+    gs, o, o64, torch, td = case["gs"], case["o"], case["o64"], case["torch"], case["td"]
+    f64 = case["dtype"] == "f64"
+    N = o.N
+    rng = np.random.default_rng(111)
+    b = rng.normal(size=(N, 3)).astype(gs.np_dtype)
+    b[:, 1] *= 1e-3
+    b[:, 2] = 0
+    x0 = rng.normal(size=(N, 3)).astype(gs.np_dtype)
+    x = torch.as_tensor(x0, dtype=td, device="cuda")
+    tol_cg = 1e-11 if f64 else 1e-5
+    its, ress, rc = gs.cg_solve3(cm.CM_MAT_K_GS2, torch.as_tensor(b, dtype=td, device="cuda"), x, tol=tol_cg, precond=cm.CM_PC_JACOBI)
+    xh = x.cpu().numpy()
+    for c in range(3):
+        xo, ito, _, _ = o64.cg_pc(oracle_mod.MAT_K_GS2, b[:, c].astype(np.float64), x0=x0[:, c].astype(np.float64), tol=tol_cg, precond=1)
+        assert abs(its[c] - ito) <= 1, (c, its, ito)
+        if c < 2:
+            assert rel(xh[:, c], xo) < (1e-9 if f64 else 1e-3)
+    assert its[2] == 0 and np.abs(xh[:, 2]).max() == 0
+
+
+def _steps(cm, orc, torch, mesh, mat, dt, terms, nsteps, dtype, H, clamp, variant, precond, cg_tol, hexa=False):
+    conn = mesh.hexes if hexa else mesh.tets
+    gm = cm.Mesh(mesh.xyz, conn, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+    gs = cm.System(gm, mat, dt, dtype, clamp)
+    o = orc.Oracle(mesh, mat, dt, clamp_dof=clamp, dtype="f64")
+    td = torch.float64 if dtype == "f64" else torch.float32
+    N = mesh.n_nodes
+    m0 = inputs.init_m_noisy_x(mesh, 23)
+    m, U, u = m0.copy(), np.zeros(N), np.zeros((N, 3))
+    mg = torch.as_tensor(m0, dtype=td, device="cuda").contiguous()
+    Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+    infos = []
+    for k in range(nsteps):
+        io, rco = o.gspm_step(m, U, u, dt, H, terms, variant=variant, cg_tol=cg_tol, cg_precond=precond)
+        ig, rcg = gs.gspm_step(cm.make_params(dt, H, terms, variant, cg_tol, 100000, -1, precond), mg, Ug, ug)
+        assert rco == 0 and rcg == 0
+        infos.append((io, ig))
+    return m, U, u, mg.cpu().numpy(), Ug.cpu().numpy(), ug.cpu().numpy(), infos
+
+
+def _check_iters(infos, slack=1):
+    for k, (io, ig) in enumerate(infos):
+        assert abs(io.it_ms - ig.it_ms) <= slack, (k, io.it_ms, ig.it_ms)
+        assert abs(io.it_mech - ig.it_mech) <= slack, (k, io.it_mech, ig.it_mech)
+        for a in range(8):
+            assert abs(io.it_gs[a] - ig.it_gs[a]) <= slack, (k, a, list(io.it_gs), list(ig.it_gs))
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_gspm_steps_with_jacobi(cm, oracle_mod, torch, variant):
+    """Ten magnetoelastic steps with every solve Jacobi-preconditioned: the same states as the oracle's, counts +-1."""
+    mesh = inputs.kuhn_box((13, 13, 7), (40 * NM, 40 * NM, 20 * NM), seed_mesh=21, seed_perm=22)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * NM,) * 3)
+    clamp = inputs.clamp_bottom(mesh)
+    m, U, u, mg, Ug, ug, infos = _steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 10, "f64", [2e4, 0, 0], clamp, variant, 1, 1e-12)
+    assert np.abs(mg - m).max() <= 1e-9
+    assert np.abs(ug - u).max() <= 1e-9 * max(1.0, np.abs(u).max())
+    _check_iters(infos)
+    # and the preconditioned and plain steps reach the same state (both solve the same systems to 1e-12)
+    m0, U0, u0, mg0, _, _, infos0 = _steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 10, "f64", [2e4, 0, 0], clamp, variant, 0, 1e-12)
+    assert np.abs(mg - mg0).max() <= 1e-8
+    assert infos[0][1].it_mech < infos0[0][1].it_mech
+
+
+def test_gspm_steps_with_jacobi_f32(cm, oracle_mod, torch):
+    cfg = inputs.make_config(0)
+    m, U, u, mg, Ug, ug, infos = _steps(cm, oracle_mod, torch, cfg.mesh, cfg.material, cfg.dt, cfg.terms, 10, "f32", cfg.Hext[0], None, 0, 1, 1e-6)
+    # config 0 starts from its own m0
+    assert np.abs(np.linalg.norm(mg, axis=1) - 1).max() <= 4 * np.finfo(np.float32).eps
+    assert np.abs(mg - m).max() <= 1e-4
+    _check_iters(infos, slack=3)
+
+
+# ---------------------------------------------------------------------------------------------- sigma_ext
+SIG = np.array([3e8, -1e8, 2e8, 5e7, -4e7, 6e7])   # Pa, xx yy zz yz xz xy
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("hexa", [False, True])
+def test_sigma_ext_rhs(cm, oracle_mod, torch, dtype, hexa):
+    """b^mech with a uniform external stress: one more term over ALL elements (non-magnetic inclusion too)."""
+    if hexa:
+        mesh = inputs.hex_box((12, 11, 9), (33 * NM, 30 * NM, 24 * NM), seed_mesh=71, seed_perm=72)
+    else:
+        mesh = inputs.kuhn_box((12, 11, 9), (33 * NM, 30 * NM, 24 * NM), seed_mesh=71, seed_perm=72)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * NM, 7 * NM, 6 * NM))
+    assert 0 < mesh.magnetic.sum() < mesh.n_tets
+    clamp = inputs.clamp_bottom(mesh)
+    tol = 1e-12 if dtype == "f64" else 1e-5
+    td = torch.float64 if dtype == "f64" else torch.float32
+    conn = mesh.hexes if hexa else mesh.tets
+    gm = cm.Mesh(mesh.xyz, conn, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+    m = inputs.init_m_random(mesh, 64)
+    md = torch.as_tensor(m, dtype=td, device="cuda")
+    ref = {}
+    for name, sig in (("with", SIG), ("without", None)):
+        mat = mat2(sigma_ext=sig)
+        gs = cm.System(gm, mat, 2e-12, dtype, clamp)
+        o = oracle_mod.Oracle(mesh, mat, 2e-12, clamp_dof=clamp)
+        b = gs.field_rhs(cm.CM_RHS_MECH, md).cpu().numpy()
+        bo = o.rhs_mech(md.cpu().numpy().astype(np.float64))
+        assert rel(b, bo) < tol, name
+        ref[name] = bo
+    assert np.abs(ref["with"] - ref["without"]).max() > 1e-3 * np.abs(ref["without"]).max()   # the term is not negligible here
+
+
+@pytest.mark.parametrize("hexa", [False, True])
+def test_sigma_ext_steps(cm, oracle_mod, torch, hexa):
+    """Five steps under external stress: the stress-induced field rotates m; parity 1e-9, counts +-1."""
+    if hexa:
+        mesh = inputs.hex_box((10, 10, 6), (30 * NM, 30 * NM, 16 * NM), seed_mesh=21, seed_perm=22)
+    else:
+        mesh = inputs.kuhn_box((10, 10, 6), (30 * NM, 30 * NM, 16 * NM), seed_mesh=21, seed_perm=22)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (6 * NM,) * 3)
+    clamp = inputs.clamp_bottom(mesh)
+    m, U, u, mg, Ug, ug, infos = _steps(cm, oracle_mod, torch, mesh, mat2(sigma_ext=SIG), 1e-12, ALL, 5, "f64", [2e4, 0, 0], clamp, 0, 0,
+                                        1e-12, hexa=hexa)
+    assert np.abs(mg - m).max() <= 1e-9
+    assert np.abs(ug - u).max() <= 1e-9 * max(1.0, np.abs(u).max())
+    _check_iters(infos)
+    assert np.abs(u).max() > 0
