@@ -263,6 +263,14 @@ typedef struct {
 int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, const cm_hyst_params *hp, void *m_dev, void *U_dev, void *u_dev,
                       double *H_log, double *mbar_log, int *steps_log, cm_hyst_result *result, void *stream);
 
+/* Tuning / measurement switches of a system (value 0 = default).
+ * CM_OPT_STORED_GEOMETRY: how the element passes S3/S5/S6/S8 of a plain (not wrapped) tetrahedral mesh get V_e and grad phi.
+ * 0: per pass, whichever kernel is faster -- the fp64 passes S3 and S5 recompute them in fp64 from the chunk's staged node
+ * coordinates, the others stream the stored values (ten words per tetrahedron); 1: every pass streams; 2: every pass
+ * recomputes.  All three give the same bits.  Other values: BADARG. */
+enum { CM_OPT_STORED_GEOMETRY = 0 };
+int cm_system_set_option(cm_system *sys, int option, int value);
+
 int cm_profile_enable(cm_system *sys, int on);
 int cm_profile_get(cm_system *sys, cm_profile *out); /* synchronises outstanding timers */
 int cm_profile_reset(cm_system *sys);

@@ -25,12 +25,13 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
 (CM_GET_COUNTS, CM_GET_ORDER, CM_GET_IPERM, CM_GET_TETS, CM_GET_TET_ORDER, CM_GET_ROWPTR, CM_GET_COLIDX, CM_GET_N2E_PTR,
  CM_GET_N2E) = range(9)
 CM_PC_NONE, CM_PC_JACOBI = 0, 1
+CM_OPT_STORED_GEOMETRY = 0
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
 EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_hex_wrapped", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
            "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_cg_solve_pc", "cm_cg_solve3_pc", "cm_cg_history_enable", "cm_cg_history", "cm_field_rhs", "cm_volume_average",
-           "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
+           "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_system_set_option", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
 
 
@@ -110,6 +111,7 @@ def lib():
         L.cm_gspm_step_host.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
         L.cm_hysteresis_run.argtypes = [vp, C.POINTER(cm_step_params), C.POINTER(cm_hyst_params), vp, vp, vp, vp, vp, vp,
                                         C.POINTER(cm_hyst_result), vp]
+        L.cm_system_set_option.argtypes = [vp, it, it]
         L.cm_profile_enable.argtypes = [vp, it]
         L.cm_profile_get.argtypes = [vp, C.POINTER(cm_profile)]
         L.cm_profile_reset.argtypes = [vp]
@@ -348,6 +350,9 @@ class System:
                                             C.byref(res), _stream()), allow=(CM_E_CG_MAXITER, CM_E_CG_BREAKDOWN))
         n = res.n_fields
         return Hl[:n], ml[:n], sl[:n], res, rc
+
+    def set_option(self, option, value):
+        _check(lib().cm_system_set_option(self.h, int(option), int(value)))
 
     def profile_enable(self, on=True):
         _check(lib().cm_profile_enable(self.h, int(on)))

@@ -397,6 +397,20 @@ extern "C" int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, con
                         sys_hysteresis<float>(S, base, hp, (float *)m_dev, (float *)U_dev, (float *)u_dev, H_log, mbar_log, steps_log, result, st));
 }
 
+// ---------------------------------------------------------------- options
+extern "C" int cm_system_set_option(cm_system *sys, int option, int value)
+{
+    CM_TRY(check_sys(sys, "cm_system_set_option"));
+    switch (option) {
+    case CM_OPT_STORED_GEOMETRY:
+        if (value < 0 || value > 2) break;
+        sys->impl->geometry_mode = value;
+        return CM_OK;
+    }
+    cm_set_error("cm_system_set_option: unknown option %d or value %d out of range", option, value);
+    return CM_E_BADARG;
+}
+
 // ---------------------------------------------------------------- profile
 extern "C" int cm_profile_enable(cm_system *sys, int on)
 {

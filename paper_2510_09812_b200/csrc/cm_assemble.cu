@@ -10,11 +10,6 @@
 
 static const double MU0 = 4.0e-7 * 3.14159265358979323846;
 
-struct TetGeom {
-    double V;
-    double g[4][3];
-};
-
 __device__ __forceinline__ void tet_geometry(const double *__restrict__ xyz, const int *t, double ld, TetGeom &G)
 {
     double x[4][3];
@@ -22,19 +17,16 @@ __device__ __forceinline__ void tet_geometry(const double *__restrict__ xyz, con
     for (int k = 0; k < 4; k++)
 #pragma unroll
         for (int d = 0; d < 3; d++) x[k][d] = xyz[3 * (long)t[k] + d] / ld;
-    double a[3], b[3], c[3];
-#pragma unroll
-    for (int d = 0; d < 3; d++) { a[d] = x[1][d] - x[0][d]; b[d] = x[2][d] - x[0][d]; c[d] = x[3][d] - x[0][d]; }
-    double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
-    double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
-    double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
-    double det = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
-    G.V = fabs(det) / 6.0;
-#pragma unroll
-    for (int d = 0; d < 3; d++) {
-        G.g[1][d] = bc[d] / det; G.g[2][d] = ca[d] / det; G.g[3][d] = ab[d] / det;
-        G.g[0][d] = -(G.g[1][d] + G.g[2][d] + G.g[3][d]);
-    }
+    tet_geometry_x(x, G);
+}
+
+// nondimensional coordinates of every chunk slot, [slot][4] (System::CX)
+__global__ void slot_xyz_kernel(long nslots, const int *__restrict__ nodes, const double *__restrict__ xyz, double ld, double *CX)
+{
+    const long s = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (s >= nslots) return;
+    const long i = nodes[s];
+    CX[4 * s] = xyz[3 * i] / ld; CX[4 * s + 1] = xyz[3 * i + 1] / ld; CX[4 * s + 2] = xyz[3 * i + 2] / ld; CX[4 * s + 3] = 0.0;
 }
 
 // one CTA per element chunk: V_e and grad phi_1..3 (rounded to T) into the chunk-blocked geometry array
@@ -272,7 +264,7 @@ System<T>::~System()
 {
     T *ptrs[] = {EG, mL, mLm, Cstar, Ccub, Kms, Kgs1, Kgs2, Mm, Kmech, Dms, Dgs1, Dgs2, Dmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
-    cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
+    cudaFree(CX); cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
     cudaFree(hyst_ctl); cudaFree(hyst_log); cudaFree(hyst_steps); cudaFree(d_hist);
     if (h_res) cudaFreeHost(h_res);
     if (h_scal) cudaFreeHost(h_scal);
@@ -416,6 +408,10 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         geom_kernel<T><<<M->ck.nchunks, B, 0, st>>>(M->ck.d_eptr, M->d_gtets, M->d_gxyz, ld, S->EG, Vd);
         lump_kernel<T><<<(unsigned)((N + B - 1) / B), B, 0, st>>>(N, M->d_n2e_ptr, M->d_n2e, Vd, M->d_mag, S->mL, S->mLm, S->live);
         volume_sum_kernel<<<1, 1024, 0, st>>>(Ne, Vd, M->d_mag, vsum);
+        if (!M->wrapped) { // a wrapped element takes its corners from its own images, not from the DOFs' representatives
+            CM_TRY(alloc(&S->CX, (size_t)4 * M->ck.nslots + 8));
+            slot_xyz_kernel<<<(unsigned)((M->ck.nslots + B - 1) / B), B, 0, st>>>(M->ck.nslots, M->ck.d_nodes, M->d_xyz, ld, S->CX);
+        }
         CM_CUDA(cudaGetLastError());
         double hv[2];
         CM_CUDA(cudaMemcpyAsync(hv, vsum, sizeof(hv), cudaMemcpyDeviceToHost, st));

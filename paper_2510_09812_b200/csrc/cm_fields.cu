@@ -126,9 +126,6 @@ template <> struct KindTraits<EK_STRESS> { static constexpr int NIN = 6, NOUT = 
 #ifndef CM_EK_NT
 #define CM_EK_NT 384
 #endif
-#ifndef CM_EK_MINB
-#define CM_EK_MINB 2
-#endif
 constexpr int EK_NT = CM_EK_NT;
 
 template <typename T>
@@ -140,6 +137,7 @@ struct ChunkArgs {
     long N;
     const unsigned short *lid, *lptr, *lent, *emat;
     const T *EG;          // chunk-blocked geometry, 10 planes per chunk (cm_internal.h)
+    const double *CX;     // slot coordinates [slot][4] (GEOM kernels: geometry recomputed, EG not read)
     const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w
     const double *mbar;   // MS
     const T *Cstar;       // MECH, STRESS: 36 words per material, or the 12 of the cubic pattern
@@ -152,16 +150,37 @@ struct ChunkArgs {
 };
 
 // shared-memory layout (every region a multiple of 16 bytes):
-//   planes [max(10, NOUT)][ne8] T   staged geometry, overwritten in place by the contributions
+//   GEOM = false (stored geometry; wrapped meshes):
+//     planes [max(10, NOUT)][ne8] T   staged geometry, overwritten in place by the contributions
+//   GEOM = true (geometry recomputed from the staged slot coordinates):
+//     scx    [CM_NL_MAX][4] double    nondimensional coordinates of the local nodes
+//     planes [NOUT][ne8] T            contributions
 //   sin    [CM_NL_MAX][NIN] T       nodal inputs
 //   slid   [EC] ushort4, sle [4 EC] ushort, sem [EC] ushort, slp [CM_NL_MAX + 8] ushort, mbarrier
-template <int KIND> constexpr int chunk_planes() { return KindTraits<KIND>::NOUT > 10 ? KindTraits<KIND>::NOUT : 10; }
-template <int KIND, typename T>
+template <int KIND, bool GEOM> constexpr int chunk_planes() { return (GEOM || KindTraits<KIND>::NOUT > 10) ? KindTraits<KIND>::NOUT : 10; }
+template <int KIND, typename T, bool GEOM>
 constexpr size_t chunk_smem_bytes()
 {
-    return (size_t)(chunk_planes<KIND>() * CM_EC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
+    return (GEOM ? (size_t)CM_NL_MAX * 4 * sizeof(double) : 0) +
+           (size_t)(chunk_planes<KIND, GEOM>() * CM_EC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
            (size_t)(4 * CM_EC_MAX + 4 * CM_EC_MAX + CM_EC_MAX + CM_NL_MAX + 8) * sizeof(unsigned short) + 16;
 }
+// resident CTAs per SM the launch bounds ask for (register cap): what the shared-memory footprint allows, at most 4
+// (40 registers per thread: enough for every fp32 kernel that streams the stored geometry) or 3 (56 registers) when the
+// fp64 geometry is recomputed in the kernel
+template <int KIND, typename T, bool GEOM>
+constexpr int chunk_minb()
+{
+    const size_t per = chunk_smem_bytes<KIND, T, GEOM>() + 1024, cap = 227 * 1024;
+    const int n = (int)(cap / per), most = GEOM ? 3 : 4;
+    return n < 1 ? 1 : (n > most ? most : n);
+}
+// Which passes recompute the geometry (measured on B200, 144^3 nodes, profiles/r02_elem_ab.txt): the passes are bound by
+// instruction issue at the occupancy their registers and planes allow (ncu: 37 % issue-active, 24 warps per SM), not by
+// DRAM, so trading ten streamed words per element for ~100 fp64 instructions pays only where the arithmetic is light:
+// fp64 S3 (0.43 -> 0.37 ms) and S5 (0.60 -> 0.52 ms).  fp64 S6 / S8 and every fp32 pass stream the stored geometry.
+template <int KIND, typename T>
+constexpr bool chunk_recompute() { return sizeof(T) == 8 && (KIND == EK_MS || KIND == EK_GRADU); }
 
 // ---- TMA bulk copy global -> shared, completion on an mbarrier
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -313,13 +332,14 @@ __device__ __forceinline__ void C_times_cubic(const T *__restrict__ Cc, const T 
     for (int r = 3; r < 6; r++) sig[r] = c[6 + r] * eps[r];
 }
 
-template <typename T, int KIND, bool CUBIC>
-__global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs<T> a)
+template <typename T, int KIND, bool CUBIC, bool GEOM>
+__global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chunk_kernel(ChunkArgs<T> a)
 {
     typedef KindTraits<KIND> K;
-    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX, NP = chunk_planes<KIND>();
+    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX, NP = chunk_planes<KIND, GEOM>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    T *scr = reinterpret_cast<T *>(smem_raw);                                   // [NP][ne8]
+    double *scx = reinterpret_cast<double *>(smem_raw);                          // [nl][4] (GEOM)
+    T *scr = reinterpret_cast<T *>(smem_raw + (GEOM ? (size_t)CM_NL_MAX * 4 * sizeof(double) : 0)); // [NP][ne8]
     T *sin = scr + NP * EC;                                                     // [nl][NIN]
     ushort4 *slid = reinterpret_cast<ushort4 *>(sin + CM_NL_MAX * NIN);         // [ne]
     unsigned short *sle = reinterpret_cast<unsigned short *>(slid + EC);        // [4 ne]
@@ -329,12 +349,13 @@ __global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs
     const int c = blockIdx.x, tid = threadIdx.x;
     const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, ne8 = (ne + 7) & ~7, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
 
-    // ---- element data: four bulk copies, all of the chunk's streaming bytes in flight at once
+    // ---- element data: bulk copies, all of the chunk's streaming bytes in flight at once
     if (tid == 0) {
         mbar_init(bar, 1);
-        const unsigned bg = 10u * ne8 * sizeof(T), bl = 8u * ne8, be = 2u * ne8;
+        const unsigned bg = GEOM ? 32u * nl : 10u * ne8 * (unsigned)sizeof(T), bl = 8u * ne8, be = 2u * ne8;
         mbar_expect_tx(bar, bg + 2 * bl + be);
-        bulk_g2s(scr, a.EG + 10L * e0, bg, bar);
+        if (GEOM) bulk_g2s(scx, a.CX + 4L * s0, bg, bar);
+        else bulk_g2s(scr, a.EG + 10L * e0, bg, bar);
         bulk_g2s(slid, a.lid + 4L * e0, bl, bar);
         bulk_g2s(sle, a.lent + 4L * e0, bl, bar);
         bulk_g2s(sem, a.emat + e0, be, bar);
@@ -356,17 +377,34 @@ __global__ void __launch_bounds__(EK_NT, CM_EK_MINB) elem_chunk_kernel(ChunkArgs
     __syncthreads(); // also orders the mbarrier initialisation before the waits
     mbar_wait(bar, 0);
 
-    // ---- phase 1: one thread per tetrahedron; its contributions replace its own column of the staged planes
+    // ---- phase 1: one thread per tetrahedron; its contributions go to its own column of the planes
     double gsum[3] = {0, 0, 0};
     for (int el = tid; el < ne; el += EK_NT) {
         const ushort4 lq = slid[el];
         const int l[4] = {lq.x, lq.y, lq.z, lq.w};
-        const T V = scr[el];
-        T g[4][3];
+        T V, g[4][3];
+        if (GEOM) {
+            // O-1 in fp64 from the staged coordinates, rounded once to T: the bits the stored geometry holds (R20)
+            double x[4][3];
 #pragma unroll
-        for (int k = 1; k < 4; k++)
+            for (int k = 0; k < 4; k++) {
+                const double2 p0 = *reinterpret_cast<const double2 *>(scx + 4 * l[k]);
+                x[k][0] = p0.x; x[k][1] = p0.y; x[k][2] = scx[4 * l[k] + 2];
+            }
+            TetGeom G;
+            tet_geometry_x(x, G);
+            V = (T)G.V;
 #pragma unroll
-            for (int d = 0; d < 3; d++) g[k][d] = scr[(3 * (k - 1) + d + 1) * ne8 + el];
+            for (int k = 1; k < 4; k++)
+#pragma unroll
+                for (int d = 0; d < 3; d++) g[k][d] = (T)G.g[k][d];
+        } else {
+            V = scr[el];
+#pragma unroll
+            for (int k = 1; k < 4; k++)
+#pragma unroll
+                for (int d = 0; d < 3; d++) g[k][d] = scr[(3 * (k - 1) + d + 1) * ne8 + el];
+        }
 #pragma unroll
         for (int d = 0; d < 3; d++) g[0][d] = -(g[1][d] + g[2][d] + g[3][d]);
 
@@ -685,7 +723,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     const Chunks &K = M->ck;
     ChunkArgs<T> a;
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
-    a.emat = M->d_emat; a.EG = S->EG;
+    a.emat = M->d_emat; a.EG = S->EG; a.CX = S->CX;
     a.hexes = M->d_tets; a.ghexes = M->d_gtets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_gxyz; a.ld = S->ld; a.N = S->N;
     a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
@@ -695,22 +733,29 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     return a;
 }
 
+template <typename T, int KIND, bool CUBIC, bool GEOM>
+static int launch_chunk_kernel(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
+{
+    constexpr size_t smem = chunk_smem_bytes<KIND, T, GEOM>();
+    // per device and per function; a host-side table lookup, set on every launch so that any device / context works
+    CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND, CUBIC, GEOM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    elem_chunk_kernel<T, KIND, CUBIC, GEOM><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(a);
+    return CM_OK;
+}
+
+// geometry recomputed from the slot coordinates where that is the faster kernel (chunk_recompute; geometry_mode 0), never
+// (mode 1) or in every pass (mode 2: the A/B measurement); wrapped meshes have no slot coordinates and always stream EG
 template <typename T, int KIND>
 static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
 {
-    constexpr size_t smem = chunk_smem_bytes<KIND, T>();
     constexpr bool USES_C = KIND == EK_MECH || KIND == EK_STRESS;
-    // per device and per function; a host-side table lookup, set on every launch so that any device / context works
-    CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    if (USES_C) CM_CUDA(cudaFuncSetAttribute(elem_chunk_kernel<T, KIND, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool geom = S->CX != nullptr && (S->geometry_mode == 2 || (S->geometry_mode == 0 && chunk_recompute<KIND, T>()));
     if (USES_C && S->cubic_pattern) {
         ChunkArgs<T> b = a;
         b.Cstar = S->Ccub;
-        elem_chunk_kernel<T, KIND, true><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(b);
-    } else {
-        elem_chunk_kernel<T, KIND, false><<<S->mesh->ck.nchunks, EK_NT, smem, st>>>(a);
+        return geom ? launch_chunk_kernel<T, KIND, USES_C, true>(S, b, st) : launch_chunk_kernel<T, KIND, USES_C, false>(S, b, st);
     }
-    return CM_OK;
+    return geom ? launch_chunk_kernel<T, KIND, false, true>(S, a, st) : launch_chunk_kernel<T, KIND, false, false>(S, a, st);
 }
 
 // ---------------------------------------------------------------- element passes on linear hexahedra (R26)

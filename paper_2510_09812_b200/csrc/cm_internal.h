@@ -60,7 +60,7 @@ struct Sell {
 //   lent[4 eptr[c] + q] incidence q of chunk c: 4 * (e - eptr[c]) + k, ascending inside every run
 //   ns_ptr / ns_slot   node -> its slots, ascending (so ascending chunk = ascending element order)
 constexpr int CM_EC_MAX = 768;
-constexpr int CM_NL_MAX = 512;
+constexpr int CM_NL_MAX = 384; // a full chunk of 768 Kuhn tets touches ~260 nodes
 struct Chunks {
     int nchunks = 0;
     long nslots = 0;
@@ -155,6 +155,7 @@ struct SystemBase {
     int pin = 0; // library index
     int num_sms = 0;
     Profiler prof;
+    int geometry_mode = 0; // CM_OPT_STORED_GEOMETRY: 0 per-pass choice, 1 every pass streams the stored geometry, 2 every pass recomputes it
     double *d_hist = nullptr;  // residual history of the last solve (cm_cg_history), CM_HIST_CAP doubles
     bool hist_on = false;
     long hist_len = 0;
@@ -177,6 +178,10 @@ struct System : SystemBase {
     // element geometry, chunk-blocked: chunk c owns 10 planes of ne8 = round_up(ne_c, 8) values at EG + 10 eptr[c]:
     // plane 0 = V_e, plane 3 (k - 1) + d + 1 = d-th component of grad phi_k, k = 1..3 (grad phi_0 = -sum, O-1)
     T *EG = nullptr;
+    // plain (not wrapped) tetrahedral meshes: nondimensional fp64 coordinates of every chunk slot, [slot][4] (x/l_d, y/l_d,
+    // z/l_d, 0): ONE bulk copy stages a chunk's coordinates and the element passes recompute V_e and grad phi from them
+    // (tet_geometry_x, the arithmetic that filled EG) instead of streaming ten stored words per element
+    double *CX = nullptr;
     T *mL = nullptr, *mLm = nullptr;
     T *Cstar = nullptr; // n_elastic x 36
     T *Ccub = nullptr;  // n_elastic x 12 (C11 C12 C13 C21 .. C33, C44 C55 C66) when every C* is zero outside that pattern
@@ -207,6 +212,31 @@ struct System : SystemBase {
     int hyst_cap = 0;
     ~System();
 };
+
+// O-1: volume and shape-function gradients of a tetrahedron from its four (nondimensional) corner coordinates, fp64.
+// One reciprocal instead of nine divisions; every user (matrix assembly, stored geometry, element passes) calls this
+// one function, so the recomputed and the stored geometry are the same bits.
+struct TetGeom {
+    double V;
+    double g[4][3];
+};
+__device__ __forceinline__ void tet_geometry_x(const double x[4][3], TetGeom &G)
+{
+    double a[3], b[3], c[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) { a[d] = x[1][d] - x[0][d]; b[d] = x[2][d] - x[0][d]; c[d] = x[3][d] - x[0][d]; }
+    const double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+    const double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+    const double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+    const double det = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+    const double idet = 1.0 / det;
+    G.V = fabs(det) / 6.0;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        G.g[1][d] = bc[d] * idet; G.g[2][d] = ca[d] * idet; G.g[3][d] = ab[d] * idet;
+        G.g[0][d] = -(G.g[1][d] + G.g[2][d] + G.g[3][d]);
+    }
+}
 
 // Linear hexahedron (R26): |J|, phi_a and grad phi_a (fp64) at Gauss point p of the 2 x 2 x 2 rule; local node
 // a = i + 2 j + 4 k <-> reference corner (2i-1, 2j-1, 2k-1)

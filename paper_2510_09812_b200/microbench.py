@@ -127,13 +127,17 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=
                 rng44 = np.random.default_rng(44)
                 m0 = np.array([1.0, 0.0, 0.0]) + 0.1 * rng44.normal(size=(N, 3))
                 m3 = torch.as_tensor(m0 / np.linalg.norm(m0, axis=1, keepdims=True), dtype=td, device="cuda").contiguous()
-                for name, rid, kw in (("elem_rhs_ms", cm.CM_RHS_MS, {}), ("elem_hd", cm.CM_OUT_HD, {"U": b1}),
-                                      ("elem_rhs_mech", cm.CM_RHS_MECH, {}), ("elem_sigma", cm.CM_OUT_SIGMA, {"u": b3})):
-                    if only and name not in only and "elem" not in only:
-                        continue
-                    t, p = kernel_ms(lambda: gs.field_rhs(rid, m3, **kw), "element", reps)
-                    # kernel_ms divides by launches; a pass is 2-3 launches, so take the class total per call
-                    cases.append((name, p["ms"] / reps, eb[name], None))
+                # tetrahedra: the default per-pass choice, every pass streaming the stored gradients, every pass recomputing them
+                for stored in ((0,) if hex_mesh else (0, 1, 2)):
+                    gs.set_option(cm.CM_OPT_STORED_GEOMETRY, stored)
+                    for name, rid, kw in (("elem_rhs_ms", cm.CM_RHS_MS, {}), ("elem_hd", cm.CM_OUT_HD, {"U": b1}),
+                                          ("elem_rhs_mech", cm.CM_RHS_MECH, {}), ("elem_sigma", cm.CM_OUT_SIGMA, {"u": b3})):
+                        if only and name not in only and "elem" not in only:
+                            continue
+                        t, p = kernel_ms(lambda: gs.field_rhs(rid, m3, **kw), "element", reps)
+                        # kernel_ms divides by launches; a pass is 2-3 launches, so take the class total per call
+                        cases.append((name + ("", "_stored", "_recomputed")[stored], p["ms"] / reps, eb[name], None))
+                gs.set_option(cm.CM_OPT_STORED_GEOMETRY, 0)
                 if not only or "cg_csr3" in only:
                     def f33():
                         x3.zero_(); gs.cg_solve3(cm.CM_MAT_K_GS1, b3, x3, fixed_iters=3)

@@ -91,7 +91,8 @@ def test_jacobi_pcg_against_oracle(case, cm, oracle_mod):
         _, _, ho = o64.cg_history(mat_o, b.astype(np.float64), tol=tol_cg, precond=1)
         k = min(len(hist), len(ho)) - 2
         assert len(hist) == it + 1 and k > 5
-        assert np.allclose(hist[:k], ho[:k], rtol=1e-6 if f64 else 5e-2), mat_g
+        assert np.allclose(hist[:12], ho[:12], rtol=1e-9 if f64 else 1e-3), mat_g       # the first iterations pin the algorithm
+        assert np.allclose(hist[:k], ho[:k], rtol=1e-2 if f64 else 2e-1), mat_g         # later ones drift apart by rounding (~300 its)
         # the preconditioner must pay on the mechanical matrix (x2-stiffness inclusion): not more iterations than plain CG
         if mat_g == cm.CM_MAT_K_MECH:
             xp = torch.zeros(shape, dtype=td, device="cuda")
@@ -159,10 +160,13 @@ def _steps(cm, orc, torch, mesh, mat, dt, terms, nsteps, dtype, H, clamp, varian
     return m, U, u, mg.cpu().numpy(), Ug.cpu().numpy(), ug.cpu().numpy(), infos
 
 
-def _check_iters(infos, slack=1):
+def _check_iters(infos, slack=1, mech_slack=None):
+    """+-1 on every solve; mech_slack = 3 only for mechanical solves driven to tol 1e-12 (~250-300 iterations, rounding floor;
+    tests/test_gpu_parity.py::_check_iters and DESIGN.md section 8 give the two residual histories)."""
+    mech_slack = slack if mech_slack is None else mech_slack
     for k, (io, ig) in enumerate(infos):
         assert abs(io.it_ms - ig.it_ms) <= slack, (k, io.it_ms, ig.it_ms)
-        assert abs(io.it_mech - ig.it_mech) <= slack, (k, io.it_mech, ig.it_mech)
+        assert abs(io.it_mech - ig.it_mech) <= mech_slack, (k, io.it_mech, ig.it_mech)
         for a in range(8):
             assert abs(io.it_gs[a] - ig.it_gs[a]) <= slack, (k, a, list(io.it_gs), list(ig.it_gs))
 
@@ -176,7 +180,7 @@ def test_gspm_steps_with_jacobi(cm, oracle_mod, torch, variant):
     m, U, u, mg, Ug, ug, infos = _steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 10, "f64", [2e4, 0, 0], clamp, variant, 1, 1e-12)
     assert np.abs(mg - m).max() <= 1e-9
     assert np.abs(ug - u).max() <= 1e-9 * max(1.0, np.abs(u).max())
-    _check_iters(infos)
+    _check_iters(infos, mech_slack=3)
     # and the preconditioned and plain steps reach the same state (both solve the same systems to 1e-12)
     m0, U0, u0, mg0, _, _, infos0 = _steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 10, "f64", [2e4, 0, 0], clamp, variant, 0, 1e-12)
     assert np.abs(mg - mg0).max() <= 1e-8
@@ -238,5 +242,9 @@ def test_sigma_ext_steps(cm, oracle_mod, torch, hexa):
                                         1e-12, hexa=hexa)
     assert np.abs(mg - m).max() <= 1e-9
     assert np.abs(ug - u).max() <= 1e-9 * max(1.0, np.abs(u).max())
-    _check_iters(infos)
+    _check_iters(infos, mech_slack=3)
     assert np.abs(u).max() > 0
+    # counts at the paper's tolerance and at 1e-10, where the two residual curves have not drifted apart yet: strict +-1
+    for tol in (1e-7, 1e-10):
+        infos_t = _steps(cm, oracle_mod, torch, mesh, mat2(sigma_ext=SIG), 1e-12, ALL, 2, "f64", [2e4, 0, 0], clamp, 0, 0, tol, hexa=hexa)[-1]
+        _check_iters(infos_t[:1])
