@@ -193,7 +193,7 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    def timed_run(system, dt_name, steps, warmup, variant, fixed, precond):
+    def timed_run(system, dt_name, steps, warmup, variant, fixed, precond, matfree=0):
         """W untimed + K timed cm_gspm_step calls from the config's initial state; CUDA events on the launching stream."""
         td = torch.float64 if dt_name == "f64" else torch.float32
         m = torch.as_tensor(cfg.m0, dtype=td, device=dev).contiguous()
@@ -201,7 +201,7 @@ def run_ours(args):
         u = torch.zeros((N, 3), dtype=td, device=dev)
 
         def params(k):
-            return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, variant, CG_TOL, 100000, fixed, precond)
+            return cm.make_params(cfg.dt, cfg.Hext[k % cfg.steps], cfg.terms, variant, CG_TOL, 100000, fixed, precond, matfree)
 
         k = 0
         for _ in range(warmup):
@@ -268,7 +268,8 @@ def run_ours(args):
 
     # ---- variants SURVEY 8(d) asks for beside steps/s (each its own W + K steps from the initial state, same mesh):
     # every solve cut at 3 iterations (the paper's regime for the Helmholtz solves), fp32 (north_star (4)),
-    # Jacobi-preconditioned CG (the paper's future work), and the other reading of Alg. B.1 Step 2 (R1)
+    # Jacobi-preconditioned CG and the matrix-free mechanical operator (the paper's future work), and the other
+    # reading of Alg. B.1 Step 2 (R1)
     variants = {}
     if not args.no_variants:
         vs = max(1, min(args.steps, args.variant_steps))
@@ -285,6 +286,10 @@ def run_ours(args):
         variants["fixed3"] = brief(r, {"kernels": {n: {q: v[q] for q in ("ms", "frac_of_measured_peak") if q in v} for n, v in kt.items()}})
         r = timed_run(sysm, dtype, vs, args.warmup, args.variant, args.fixed_iters, 1 - args.precond)
         variants["jacobi" if args.precond == 0 else "plain_cg"] = brief(r)
+        r = timed_run(sysm, dtype, vs, args.warmup, args.variant, args.fixed_iters, args.precond, matfree=1)
+        pm = r["prof"]["cg_mech"]
+        variants["mech_matfree"] = brief(r, {"cg_mech_ms_per_matrix_pass": pm["ms"] / max(1, pm["cg_matrix_passes"]),
+                                            "stored_matrix_ms_per_matrix_pass": prof["cg_mech"]["ms"] / max(1, prof["cg_mech"]["cg_matrix_passes"])})
         r = timed_run(sysm, dtype, vs, args.warmup, 1 - args.variant, args.fixed_iters, args.precond)
         variants[f"gspm_variant{1 - args.variant}"] = brief(r)
         other = "f32" if dtype == "f64" else "f64"

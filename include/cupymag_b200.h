@@ -117,6 +117,7 @@ typedef struct {
     int cg_maxiter;
     int cg_fixed_iters;   /* >= 0: run exactly this many iterations in every solve; < 0: off */
     int cg_precond;       /* cm_precond of every solve of the step; CM_PC_NONE = the paper's unpreconditioned CG */
+    int mech_matfree;     /* != 0: the mechanical solve applies K^mech matrix-free (cm_cg_solve_matfree); tetrahedra only */
 } cm_step_params;
 
 /* it_gs / res_gs slots: 0-2 g^n components, 3-4 g*_1, g*_2, 5-7 m** components. */
@@ -217,6 +218,16 @@ int cm_cg_solve3_pc(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_
  * host_out ([k][n_rhs] doubles, n_rhs = 1, or 3 for cm_cg_solve3*), at most `capacity` doubles; *n_out = entries written. */
 int cm_cg_history_enable(cm_system *sys, int on);
 int cm_cg_history(cm_system *sys, double *host_out, long capacity, long *n_out);
+
+/* Matrix-free K^mech (the paper's future work: it "assembles and stores sparse matrices explicitly").
+ * cm_spmv_matfree: y = (P K^mech P + (I - P)) x, the same operator as cm_spmv(CM_MAT_K_MECH), applied as an element pass
+ * (strain of x, stress C*_e : E, nodal forces V_e sigma grad phi_k per chunk slot) and a node pass; nothing of the stored
+ * matrix is read.  cm_cg_solve_matfree: CG (optionally Jacobi, with the stored diagonal) on that operator, same stopping
+ * rule and outputs as cm_cg_solve_pc; four launches per iteration, the stream is synchronised once per 16 iterations.
+ * Linear tetrahedra only (hexahedral meshes: BADARG).  x, y, b: N x 3, user order. */
+int cm_spmv_matfree(cm_system *sys, const void *x_dev, void *y_dev, void *stream);
+int cm_cg_solve_matfree(cm_system *sys, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters,
+                        int precond, int *iters_out, double *relres_out, void *stream);
 
 /* Element-wise gather / compute / deterministic gather-scatter assembly (see cm_rhs_id).  m_dev: N x 3;
  * U_dev: N (may be NULL when DEMAG is off); u_dev: N x 3 (may be NULL when MAGEL is off); coeff: dtau or

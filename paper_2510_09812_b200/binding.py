@@ -30,7 +30,7 @@ CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
 EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_hex_wrapped", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
-           "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_cg_solve_pc", "cm_cg_solve3_pc", "cm_cg_history_enable", "cm_cg_history", "cm_field_rhs", "cm_volume_average",
+           "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_cg_solve_pc", "cm_cg_solve3_pc", "cm_cg_history_enable", "cm_cg_history", "cm_spmv_matfree", "cm_cg_solve_matfree", "cm_field_rhs", "cm_volume_average",
            "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_system_set_option", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
 
@@ -50,7 +50,8 @@ class cm_material(C.Structure):
 
 class cm_step_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("Hext", C.c_double * 3), ("terms", C.c_uint), ("gspm_variant", C.c_int),
-                ("cg_tol", C.c_double), ("cg_maxiter", C.c_int), ("cg_fixed_iters", C.c_int), ("cg_precond", C.c_int)]
+                ("cg_tol", C.c_double), ("cg_maxiter", C.c_int), ("cg_fixed_iters", C.c_int), ("cg_precond", C.c_int),
+                ("mech_matfree", C.c_int)]
 
 
 class cm_step_info(C.Structure):
@@ -105,6 +106,8 @@ def lib():
         L.cm_cg_solve3_pc.argtypes = [vp, it, vp, vp, db, it, it, it, C.POINTER(it), C.POINTER(db), vp]
         L.cm_cg_history_enable.argtypes = [vp, it]
         L.cm_cg_history.argtypes = [vp, vp, lg, C.POINTER(lg)]
+        L.cm_spmv_matfree.argtypes = [vp, vp, vp, vp]
+        L.cm_cg_solve_matfree.argtypes = [vp, vp, vp, db, it, it, it, C.POINTER(it), C.POINTER(db), vp]
         L.cm_field_rhs.argtypes = [vp, it, vp, vp, vp, C.POINTER(cm_step_params), db, vp, vp]
         L.cm_volume_average.argtypes = [vp, it, vp, it, C.POINTER(db), vp]
         L.cm_gspm_step.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
@@ -147,9 +150,10 @@ def _dp(t):
     return None if t is None else C.c_void_p(t.data_ptr())
 
 
-def make_params(dt, Hext=(0, 0, 0), terms=0, variant=0, cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1, cg_precond=CM_PC_NONE):
+def make_params(dt, Hext=(0, 0, 0), terms=0, variant=0, cg_tol=1e-7, cg_maxiter=100000, cg_fixed_iters=-1, cg_precond=CM_PC_NONE,
+                mech_matfree=0):
     return cm_step_params(dt, (C.c_double * 3)(*[float(h) for h in Hext]), int(terms), int(variant), cg_tol, int(cg_maxiter),
-                          int(cg_fixed_iters), int(cg_precond))
+                          int(cg_fixed_iters), int(cg_precond), int(mech_matfree))
 
 
 def periodic_wrap(xyz, axes: int, rel_tol: float = 1e-9):
@@ -295,6 +299,18 @@ class System:
             rc = lib().cm_cg_solve3_pc(self.h, mat, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, int(precond), it,
                                        res, _stream())
         return list(it), list(res), _check(rc, allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
+
+    def spmv_matfree(self, x):
+        import torch
+        y = torch.empty_like(self._chk(x))
+        _check(lib().cm_spmv_matfree(self.h, _dp(x), _dp(y), _stream()))
+        return y
+
+    def cg_solve_matfree(self, b, x, tol=1e-7, maxiter=100000, fixed_iters=-1, precond=CM_PC_NONE):
+        it = C.c_int(); res = C.c_double()
+        rc = lib().cm_cg_solve_matfree(self.h, _dp(self._chk(b)), _dp(self._chk(x)), tol, maxiter, fixed_iters, int(precond),
+                                       C.byref(it), C.byref(res), _stream())
+        return it.value, res.value, _check(rc, allow=(CM_E_CG_BREAKDOWN, CM_E_CG_MAXITER))
 
     def cg_history_enable(self, on=True):
         _check(lib().cm_cg_history_enable(self.h, int(on)))

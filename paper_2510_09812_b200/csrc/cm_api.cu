@@ -256,6 +256,50 @@ extern "C" int cm_cg_solve3(cm_system *sys, cm_matrix_id id, const void *b_dev, 
     return cm_cg_solve3_pc(sys, id, b_dev, x_dev, tol, maxiter, fixed_iters, CM_PC_NONE, iters_out, relres_out, stream);
 }
 
+template <typename T>
+static int api_spmv_matfree(System<T> *S, const void *x, void *y, cudaStream_t st)
+{
+    CM_TRY(sys_permute_in<T>(S, (const T *)x, S->xin, 3, st));
+    CM_TRY(sys_spmv_matfree<T>(S, S->xin, S->xout, st));
+    return sys_permute_out<T>(S, S->xout, (T *)y, 3, st);
+}
+
+extern "C" int cm_spmv_matfree(cm_system *sys, const void *x_dev, void *y_dev, void *stream)
+{
+    CM_TRY(check_sys(sys, "cm_spmv_matfree"));
+    if (!x_dev || !y_dev) { cm_set_error("cm_spmv_matfree: null argument"); return CM_E_BADARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return SYS_DISPATCH(sys, api_spmv_matfree<double>(S, x_dev, y_dev, st), api_spmv_matfree<float>(S, x_dev, y_dev, st));
+}
+
+template <typename T>
+static int api_cg_matfree(System<T> *S, const void *b, void *x, double tol, int maxiter, int fixed, int precond, int *iters, double *relres,
+                          cudaStream_t st)
+{
+    CM_TRY(sys_permute_in<T>(S, (const T *)b, S->bvec, 3, st));
+    CM_TRY(sys_permute_in<T>(S, (const T *)x, S->xin, 3, st));
+    CM_TRY(sys_cg_matfree<T>(S, S->bvec, S->xin, tol, maxiter, fixed, precond, 7, st));
+    CM_TRY(sys_permute_out<T>(S, S->xin, (T *)x, 3, st));
+    CM_CUDA(cudaMemcpyAsync(S->h_res + 7, S->d_res + 7, sizeof(CgResult), cudaMemcpyDeviceToHost, st));
+    CM_CUDA(cudaStreamSynchronize(st));
+    const CgResult &R = S->h_res[7];
+    if (iters) *iters = R.iters[0];
+    if (relres) *relres = R.relres[0];
+    S->prof.cg_iters[CM_PROF_CG_MECH] += R.iters[0];
+    S->prof.cg_passes[CM_PROF_CG_MECH] += R.iters[0] + 1;
+    return R.status;
+}
+
+extern "C" int cm_cg_solve_matfree(cm_system *sys, const void *b_dev, void *x_dev, double tol, int maxiter, int fixed_iters, int precond,
+                                   int *iters_out, double *relres_out, void *stream)
+{
+    CM_TRY(check_sys(sys, "cm_cg_solve_matfree"));
+    if (!b_dev || !x_dev) { cm_set_error("cm_cg_solve_matfree: null argument"); return CM_E_BADARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return SYS_DISPATCH(sys, api_cg_matfree<double>(S, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st),
+                        api_cg_matfree<float>(S, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st));
+}
+
 extern "C" int cm_cg_history_enable(cm_system *sys, int on)
 {
     CM_TRY(check_sys(sys, "cm_cg_history_enable"));

@@ -265,7 +265,8 @@ System<T>::~System()
     T *ptrs[] = {EG, mL, mLm, Cstar, Ccub, Kms, Kgs1, Kgs2, Mm, Kmech, Dms, Dgs1, Dgs2, Dmech, r, p, p2, Ap, bvec, m, U, u, hd, hn, f, gn, gs, ms, mss, xin, xout, hpart, sig, stg_m, stg_U, stg_u};
     for (T *q : ptrs) cudaFree(q);
     cudaFree(CX); cudaFree(live); cudaFree(clamp); cudaFree(partial); cudaFree(d_res); cudaFree(red); cudaFree(dscal);
-    cudaFree(hyst_ctl); cudaFree(hyst_log); cudaFree(hyst_steps); cudaFree(d_hist);
+    cudaFree(hyst_ctl); cudaFree(hyst_log); cudaFree(hyst_steps); cudaFree(d_hist); cudaFree(mf_state);
+    if (h_mf) cudaFreeHost(h_mf);
     if (h_res) cudaFreeHost(h_res);
     if (h_scal) cudaFreeHost(h_scal);
 }
@@ -459,6 +460,9 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     CM_TRY(alloc(&S->d_res, 8));
     CM_TRY(alloc(&S->red, std::max<size_t>({(size_t)4096 * 16, (size_t)8 * M->ck.nchunks, (size_t)3 * ((N + 127) / 128) + 64})));
     CM_TRY(alloc(&S->dscal, 32));
+    CM_CUDA(cudaMalloc(&S->mf_state, 256));
+    CM_CUDA(cudaMemsetAsync(S->mf_state, 0, 256, st));
+    CM_CUDA(cudaMallocHost(&S->h_mf, 256));
     CM_CUDA(cudaMallocHost((void **)&S->h_res, 8 * sizeof(CgResult)));
     CM_CUDA(cudaMallocHost((void **)&S->h_scal, 32 * sizeof(double)));
     CM_CUDA(cudaStreamSynchronize(st));

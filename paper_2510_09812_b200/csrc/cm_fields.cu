@@ -114,7 +114,7 @@ __global__ void permute_out_kernel(long N, int nc, const int *__restrict__ order
 // node: sums the node's incidences inside the chunk in ascending element order and writes ONE partial per slot.  A
 // node pass then adds a node's slots in ascending chunk order -- a deterministic gather end to end, no float
 // atomics, and no per-element scratch in HBM.
-enum ElemKind { EK_MS = 0, EK_GRADU = 1, EK_MECH = 2, EK_STRESS = 3 };
+enum ElemKind { EK_MS = 0, EK_GRADU = 1, EK_MECH = 2, EK_STRESS = 3, EK_KMECH = 4 };
 // NIN staged words per node, NOUT shared-memory words per element, NC words per slot, PERK: contribution depends on
 // the local node index k (NOUT = 4 NC) or is the same for the 4 nodes (NOUT = NC).
 template <int KIND> struct KindTraits;
@@ -122,6 +122,8 @@ template <> struct KindTraits<EK_MS> { static constexpr int NIN = 3, NOUT = 4, N
 template <> struct KindTraits<EK_GRADU> { static constexpr int NIN = 1, NOUT = 3, NC = 3; static constexpr bool PERK = false; };
 template <> struct KindTraits<EK_MECH> { static constexpr int NIN = 3, NOUT = 12, NC = 3; static constexpr bool PERK = true; };
 template <> struct KindTraits<EK_STRESS> { static constexpr int NIN = 6, NOUT = 6, NC = 6; static constexpr bool PERK = false; };
+// matrix-free K^mech x (Eq. 12): in x (projected: clamped DOFs read as 0), out sum_e V_e B_k^T C_e B x per slot
+template <> struct KindTraits<EK_KMECH> { static constexpr int NIN = 3, NOUT = 12, NC = 3; static constexpr bool PERK = true; };
 
 #ifndef CM_EK_NT
 #define CM_EK_NT 384
@@ -139,6 +141,8 @@ struct ChunkArgs {
     const T *EG;          // chunk-blocked geometry, 10 planes per chunk (cm_internal.h)
     const double *CX;     // slot coordinates [slot][4] (GEOM kernels: geometry recomputed, EG not read)
     const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w
+    const uchar *clamp;   // KMECH: clamped DOFs of the input read as zero (the projection P of P A P + (I - P))
+    const int *skip;      // KMECH inside CG: the solve has finished, the launch is a no-op
     const double *mbar;   // MS
     const T *Cstar;       // MECH, STRESS: 36 words per material, or the 12 of the cubic pattern
     T l1, l2;
@@ -347,6 +351,7 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
     unsigned short *slp = sem + EC;                                             // [nl + 1]
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(slp + CM_NL_MAX + 8);
     const int c = blockIdx.x, tid = threadIdx.x;
+    if (KIND == EK_KMECH && a.skip && *a.skip) return;
     const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, ne8 = (ne + 7) & ~7, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
 
     // ---- element data: bulk copies, all of the chunk's streaming bytes in flight at once
@@ -365,6 +370,9 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
         const long g = a.nodes[s0 + l];
         if (KIND == EK_GRADU) {
             sin[l] = a.in0[g];
+        } else if (KIND == EK_KMECH) {
+#pragma unroll
+            for (int d = 0; d < 3; d++) sin[3 * l + d] = a.clamp[3 * g + d] ? (T)0 : a.in0[3 * g + d];
         } else {
 #pragma unroll
             for (int d = 0; d < 3; d++) sin[NIN * l + d] = a.in0[3 * g + d];
@@ -424,6 +432,29 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
                 const T gU = u0 * g[0][d] + u1 * g[1][d] + u2 * g[2][d] + u3 * g[3][d];
                 scr[d * ne8 + el] = V * gU;
                 gsum[d] += (double)V * (double)gU;
+            }
+        } else if (KIND == EK_KMECH) {
+            // sigma = C*_e : E_e(x), H[a][b] = d_b x_a;  c_(k,a) = V_e (sigma grad phi_k)_a   (every element is elastic)
+            T H[3][3];
+#pragma unroll
+            for (int x = 0; x < 3; x++)
+#pragma unroll
+                for (int y = 0; y < 3; y++) {
+                    T acc = 0;
+#pragma unroll
+                    for (int k = 0; k < 4; k++) acc += sin[3 * l[k] + x] * g[k][y];
+                    H[x][y] = acc;
+                }
+            const T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]};
+            T sg[6];
+            const unsigned em = sem[el];
+            if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), eps, sg);
+            else C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                scr[(3 * k + 0) * ne8 + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
+                scr[(3 * k + 1) * ne8 + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
+                scr[(3 * k + 2) * ne8 + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
             }
         } else {
             const unsigned em = sem[el];
@@ -725,7 +756,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
     a.emat = M->d_emat; a.EG = S->EG; a.CX = S->CX;
     a.hexes = M->d_tets; a.ghexes = M->d_gtets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_gxyz; a.ld = S->ld; a.N = S->N;
-    a.in0 = nullptr; a.in1 = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
+    a.in0 = nullptr; a.in1 = nullptr; a.clamp = S->clamp; a.skip = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
     for (int q = 0; q < 6; q++) a.sext[q] = (T)S->sext[q];
     a.has_sext = S->has_sext ? 1 : 0;
@@ -748,7 +779,7 @@ static int launch_chunk_kernel(System<T> *S, const ChunkArgs<T> &a, cudaStream_t
 template <typename T, int KIND>
 static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
 {
-    constexpr bool USES_C = KIND == EK_MECH || KIND == EK_STRESS;
+    constexpr bool USES_C = KIND == EK_MECH || KIND == EK_STRESS || KIND == EK_KMECH;
     const bool geom = S->CX != nullptr && (S->geometry_mode == 2 || (S->geometry_mode == 0 && chunk_recompute<KIND, T>()));
     if (USES_C && S->cubic_pattern) {
         ChunkArgs<T> b = a;
@@ -969,6 +1000,7 @@ static int step_check(System<T> *S, const cm_step_params *p, const T *m_user, co
     const unsigned terms = p->terms;
     if (p->dt != S->dt) { cm_set_error("%s: params->dt differs from the dt given to cm_assemble_csr", fn); return CM_E_BADARG; }
     if ((terms & CM_TERM_MAGEL) && !S->n_elastic) { cm_set_error("%s: MAGEL needs elastic constants", fn); return CM_E_BADARG; }
+    if (p->mech_matfree && (terms & CM_TERM_MAGEL) && S->mesh->nen != 4) { cm_set_error("%s: mech_matfree is built for tetrahedra", fn); return CM_E_BADARG; }
     if (p->cg_precond != CM_PC_NONE && p->cg_precond != CM_PC_JACOBI) { cm_set_error("%s: unknown cg_precond %d", fn, p->cg_precond); return CM_E_BADARG; }
     if (((terms & CM_TERM_DEMAG) && !U_user) || ((terms & CM_TERM_MAGEL) && !u_user) || !m_user) {
         cm_set_error("%s: null field pointer", fn);
@@ -1002,7 +1034,8 @@ static int step_core(System<T> *S, const cm_step_params *p, const double *hext_d
     // 4. mechanical equilibrium (Eq. 6, 10), warm start; stress at m^n
     if (terms & CM_TERM_MAGEL) {
         CM_TRY(sys_rhs_mech(S, S->m, S->bvec, st));
-        CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, pc, st));
+        if (p->mech_matfree) CM_TRY(sys_cg_matfree(S, S->bvec, S->u, tol, mx, fx, pc, 1, st));
+        else CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, pc, st));
         CM_TRY(sys_stress(S, S->u, S->m, st));
     }
     // 5. h[m^n];  6. Step 1: g^n.  A Helmholtz solve is ONE launch: b = M_m f, x0 = f, r0 = b - A f in its first pass
@@ -1142,6 +1175,7 @@ int sys_hysteresis(System<T> *S, const cm_step_params *base, const cm_hyst_param
 {
     const unsigned terms = base->terms;
     CM_TRY(step_check(S, base, m_user, U_user, u_user, "cm_hysteresis_run"));
+    if (base->mech_matfree) { cm_set_error("cm_hysteresis_run: the matrix-free mechanical solve synchronises the stream and cannot be captured"); return CM_E_BADARG; }
     const double n0 = std::sqrt(hp->H0[0] * hp->H0[0] + hp->H0[1] * hp->H0[1] + hp->H0[2] * hp->H0[2]);
     if (!(n0 > 0) || hp->max_fields < 1 || hp->max_steps < 1 || !H_log || !mbar_log || !steps_log || !res) {
         cm_set_error("cm_hysteresis_run: H0 must be non-zero, max_fields and max_steps positive, outputs non-null");
@@ -1240,6 +1274,282 @@ int sys_hysteresis(System<T> *S, const cm_step_params *base, const cm_hyst_param
     return rc;
 }
 
+// ------------------------------------------------------------------------------------------------
+// matrix-free K^mech (the paper's future work: "assembles and stores sparse matrices explicitly")
+// ------------------------------------------------------------------------------------------------
+// y = (P K P + (I - P)) x applied as an element pass (EK_KMECH: strain of x, stress, nodal forces per chunk slot) and a node
+// pass (slots summed in ascending chunk order; a clamped DOF returns x).  The CG around it is a sequence of four launches per
+// iteration on one stream; the scalars live in a double-buffered device state that every block re-reduces from per-block
+// partials in a fixed order (bit-reproducible), and a finished solve turns the remaining launches of a batch into no-ops.
+namespace {
+
+constexpr int MF_GRID = 1024, MF_BS = 256, MF_BATCH = 16;
+
+struct MfState {
+    double rr, bb, rz;
+    int iters, done, status, zero_rhs;
+};
+
+// sum over the MF_GRID per-block partials of component c (fixed order, the same bits in every block)
+template <int NV>
+__device__ __forceinline__ void mf_reduce(const double *partial, double (&out)[NV])
+{
+    __shared__ double sh[NV * 32];
+    double v[NV];
+#pragma unroll
+    for (int c = 0; c < NV; c++) v[c] = 0;
+    for (int j = threadIdx.x; j < MF_GRID; j += blockDim.x)
+#pragma unroll
+        for (int c = 0; c < NV; c++) v[c] += __ldcg(partial + (long)j * NV + c);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int c = 0; c < NV; c++)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    __syncthreads();
+    if (lane == 0)
+#pragma unroll
+        for (int c = 0; c < NV; c++) sh[c * 32 + warp] = v[c];
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < NV; c++) {
+        double t = 0;
+        for (int w = 0; w < nwarp; w++) t += sh[c * 32 + w];
+        out[c] = t;
+    }
+    __syncthreads();
+}
+
+template <int NV>
+__device__ __forceinline__ void mf_block_partial(double (&v)[NV], double *partial)
+{
+    __shared__ double sh[NV * 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int c = 0; c < NV; c++)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    __syncthreads();
+    if (lane == 0)
+#pragma unroll
+        for (int c = 0; c < NV; c++) sh[c * 32 + warp] = v[c];
+    __syncthreads();
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int c = 0; c < NV; c++) {
+            double t = 0;
+            for (int w = 0; w < nwarp; w++) t += sh[c * 32 + w];
+            partial[(long)blockIdx.x * NV + c] = t;
+        }
+}
+
+// node pass of the operator.  MODE 0: y = A x.  MODE 1 (start of a solve): r = b - A x, p = z = r or r / D, partials
+// (rr, bb, rz).  MODE 2 (iteration): y = A x with partial x . y.
+template <typename T, int MODE, bool PRE>
+__global__ void __launch_bounds__(MF_BS) mf_apply_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot,
+                                                          const T *__restrict__ hpart, const uchar *__restrict__ clamp, const T *__restrict__ x,
+                                                          T *y, const T *__restrict__ b, const T *__restrict__ D, T *r, double *partial,
+                                                          const MfState *st)
+{
+    if (MODE == 2 && st->done) return;
+    double acc3[3] = {0, 0, 0};
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < N; i += (long)gridDim.x * blockDim.x) {
+        T a[3] = {0, 0, 0};
+        for (int s = ns_ptr[i]; s < ns_ptr[i + 1]; s++) {
+            const long q = __ldg(ns_slot + s);
+#pragma unroll
+            for (int d = 0; d < 3; d++) a[d] += hpart[3 * q + d];
+        }
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            const long k = 3 * i + d;
+            const T xv = x[k];
+            if (clamp[k]) a[d] = xv;
+            if (MODE == 0) y[k] = a[d];
+            if (MODE == 2) { y[k] = a[d]; acc3[0] += (double)xv * (double)a[d]; }
+            if (MODE == 1) {
+                const T bi = b[k], ri = bi - a[d], zi = PRE ? ri / D[k] : ri;
+                r[k] = ri; y[k] = zi;
+                acc3[0] += (double)ri * (double)ri; acc3[1] += (double)bi * (double)bi; acc3[2] += (double)ri * (double)zi;
+            }
+        }
+    }
+    if (MODE == 1) mf_block_partial<3>(acc3, partial);
+    if (MODE == 2) { double v[1] = {acc3[0]}; mf_block_partial<1>(v, partial); }
+}
+
+// state before iteration 0: the stopping test of the textbook loop (O-4), zero right-hand side
+__global__ void mf_init_state_kernel(const double *partial, double tol, int maxiter, int fixed, MfState *st)
+{
+    double v[3];
+    mf_reduce<3>(partial, v);
+    if (threadIdx.x) return;
+    MfState s;
+    s.rr = v[0]; s.bb = v[1]; s.rz = v[2]; s.iters = 0; s.done = 0; s.status = CM_OK; s.zero_rhs = 0;
+    if (s.bb == 0.0 && fixed < 0) { s.zero_rhs = 1; s.rr = 0; s.done = 1; }
+    else if (s.rr == 0.0) s.done = 1;
+    else if (fixed >= 0) { if (fixed == 0) s.done = 1; }
+    else if (s.rr < tol * tol * s.bb) s.done = 1;
+    else if (maxiter <= 0) { s.done = 1; s.status = CM_E_CG_MAXITER; }
+    st[0] = s;
+}
+
+template <typename T>
+__global__ void mf_zero_x_kernel(long n, T *x, const MfState *st)
+{
+    if (!st->zero_rhs) return;
+    for (long k = blockIdx.x * (long)blockDim.x + threadIdx.x; k < n; k += (long)gridDim.x * blockDim.x) x[k] = 0;
+}
+
+// alpha = rz / pAp; x += alpha p; r -= alpha Ap; partials (rr, rz) of the new residual
+template <typename T, bool PRE>
+__global__ void __launch_bounds__(MF_BS) mf_update_kernel(long n, const T *__restrict__ p, const T *__restrict__ Ap, const T *__restrict__ D, T *x,
+                                                           T *r, const double *pap_partial, double *partial, const MfState *st)
+{
+    if (st->done) return;
+    double pap[1];
+    mf_reduce<1>(pap_partial, pap);
+    double acc[2] = {0, 0};
+    if (pap[0] > 0.0) {
+        const T alpha = (T)(st->rz / pap[0]);
+        for (long k = blockIdx.x * (long)blockDim.x + threadIdx.x; k < n; k += (long)gridDim.x * blockDim.x) {
+            x[k] = fma(alpha, p[k], x[k]);
+            const T ri = fma(-alpha, Ap[k], r[k]);
+            r[k] = ri;
+            acc[0] += (double)ri * (double)ri;
+            acc[1] += (double)ri * (double)(PRE ? ri / D[k] : ri);
+        }
+    }
+    mf_block_partial<2>(acc, partial);
+}
+
+// beta = rz_new / rz; p = z + beta p; next state with the stopping test before the next iteration
+template <typename T, bool PRE>
+__global__ void __launch_bounds__(MF_BS) mf_p_kernel(long n, const T *__restrict__ r, const T *__restrict__ D, T *p, const double *pap_partial,
+                                                      const double *partial, double tol, int maxiter, int fixed, const MfState *st, MfState *nxt)
+{
+    if (st->done) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) *nxt = *st;
+        return;
+    }
+    double pap[1], v[2];
+    mf_reduce<1>(pap_partial, pap);
+    mf_reduce<2>(partial, v);
+    const bool breakdown = !(pap[0] > 0.0);
+    MfState s = *st;
+    if (breakdown) { s.done = 1; s.status = CM_E_CG_BREAKDOWN; }
+    else {
+        const T beta = (T)(v[1] / s.rz);
+        s.rr = v[0]; s.rz = v[1]; s.iters += 1;
+        if (s.rr == 0.0) s.done = 1;
+        else if (fixed >= 0) { if (s.iters == fixed) s.done = 1; }
+        else if (s.rr < tol * tol * s.bb) s.done = 1;
+        else if (s.iters >= maxiter) { s.done = 1; s.status = CM_E_CG_MAXITER; }
+        if (!s.done)
+            for (long k = blockIdx.x * (long)blockDim.x + threadIdx.x; k < n; k += (long)gridDim.x * blockDim.x)
+                p[k] = fma(beta, p[k], PRE ? r[k] / D[k] : r[k]);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) *nxt = s;
+}
+
+__global__ void mf_result_kernel(const MfState *st, CgResult *out)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    for (int q = 0; q < 3; q++) { out->iters[q] = 0; out->relres[q] = 0; }
+    out->iters[0] = st->iters;
+    out->relres[0] = st->bb > 0 ? sqrt(st->rr / st->bb) : 0.0;
+    out->status = st->status;
+}
+
+} // namespace
+
+template <typename T>
+static int mf_check(System<T> *S, const char *fn)
+{
+    if (!S->n_elastic) { cm_set_error("%s: the material has no elastic constants", fn); return CM_E_BADARG; }
+    if (S->mesh->nen != 4) { cm_set_error("%s: the matrix-free operator is built for tetrahedra", fn); return CM_E_BADARG; }
+    return CM_OK;
+}
+
+// element pass of the operator on library-order x -> S->hpart
+template <typename T>
+static int mf_elements(System<T> *S, const T *x, const int *skip, int prof_cls, cudaStream_t st)
+{
+    ChunkArgs<T> a = chunk_args(S);
+    a.in0 = x; a.skip = skip;
+    S->prof.begin(prof_cls, st);
+    CM_TRY((launch_chunks<T, EK_KMECH>(S, a, st)));
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+template <typename T>
+int sys_spmv_matfree(System<T> *S, const T *x, T *y, cudaStream_t st)
+{
+    CM_TRY(mf_check(S, "cm_spmv_matfree"));
+    const Chunks &K = S->mesh->ck;
+    CM_TRY(mf_elements(S, x, nullptr, CM_PROF_SPMV, st));
+    S->prof.begin(CM_PROF_SPMV, st);
+    mf_apply_kernel<T, 0, false><<<MF_GRID, MF_BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->clamp, x, y, nullptr, nullptr, nullptr, nullptr, nullptr);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
+// CG on the matrix-free operator; b, x in library order; result in S->d_res[slot].  Synchronises the stream once per
+// MF_BATCH iterations (the host has to know when to stop enqueueing).
+template <typename T>
+int sys_cg_matfree(System<T> *S, const T *b, T *x, double tol, int maxiter, int fixed, int precond, int slot, cudaStream_t st)
+{
+    CM_TRY(mf_check(S, "cm_cg_solve_matfree"));
+    if (precond != CM_PC_NONE && precond != CM_PC_JACOBI) { cm_set_error("unknown preconditioner %d", precond); return CM_E_BADARG; }
+    const bool pre = precond == CM_PC_JACOBI;
+    const Chunks &K = S->mesh->ck;
+    const long N = S->N, n = 3 * N;
+    MfState *ms = (MfState *)S->mf_state;
+    double *part_pap = S->red, *part2 = S->red + MF_GRID, *part3 = S->red + 3 * MF_GRID;
+    const T *D = S->Dmech;
+    // ---- r0 = b - A x0, p0 = z0
+    CM_TRY(mf_elements(S, x, nullptr, CM_PROF_CG_MECH, st));
+    S->prof.begin(CM_PROF_CG_MECH, st, 3);
+    if (pre) mf_apply_kernel<T, 1, true><<<MF_GRID, MF_BS, 0, st>>>(N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->clamp, x, S->p, b, D, S->r, part3, nullptr);
+    else mf_apply_kernel<T, 1, false><<<MF_GRID, MF_BS, 0, st>>>(N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->clamp, x, S->p, b, D, S->r, part3, nullptr);
+    mf_init_state_kernel<<<1, MF_BS, 0, st>>>(part3, tol, maxiter, fixed, ms);
+    mf_zero_x_kernel<T><<<MF_GRID, MF_BS, 0, st>>>(n, x, ms);
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    MfState *hs = (MfState *)S->h_mf;
+    const int cap = fixed >= 0 ? fixed : maxiter;
+    int k = 0; // iterations enqueued so far: iteration j reads ms[j & 1] and writes ms[(j + 1) & 1]
+    while (k < cap) {
+        const int kend = std::min(cap, k + MF_BATCH);
+        for (; k < kend; k++) {
+            const MfState *cur = ms + (k & 1);
+            MfState *nxt = ms + ((k + 1) & 1);
+            CM_TRY(mf_elements(S, S->p, &cur->done, CM_PROF_CG_MECH, st));
+            S->prof.begin(CM_PROF_CG_MECH, st, 3);
+            mf_apply_kernel<T, 2, false><<<MF_GRID, MF_BS, 0, st>>>(N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->clamp, S->p, S->Ap, nullptr, nullptr, nullptr, part_pap, cur);
+            if (pre) {
+                mf_update_kernel<T, true><<<MF_GRID, MF_BS, 0, st>>>(n, S->p, S->Ap, D, x, S->r, part_pap, part2, cur);
+                mf_p_kernel<T, true><<<MF_GRID, MF_BS, 0, st>>>(n, S->r, D, S->p, part_pap, part2, tol, maxiter, fixed, cur, nxt);
+            } else {
+                mf_update_kernel<T, false><<<MF_GRID, MF_BS, 0, st>>>(n, S->p, S->Ap, D, x, S->r, part_pap, part2, cur);
+                mf_p_kernel<T, false><<<MF_GRID, MF_BS, 0, st>>>(n, S->r, D, S->p, part_pap, part2, tol, maxiter, fixed, cur, nxt);
+            }
+            S->prof.end(st);
+            LAUNCH_CHECK();
+        }
+        CM_CUDA(cudaMemcpyAsync(hs, ms + (k & 1), sizeof(MfState), cudaMemcpyDeviceToHost, st));
+        CM_CUDA(cudaStreamSynchronize(st));
+        if (hs->done) break;
+    }
+    const int kfin = k & 1;
+    mf_result_kernel<<<1, 32, 0, st>>>(ms + kfin, S->d_res + slot);
+    LAUNCH_CHECK();
+    return CM_OK;
+}
+
 #define INST(T)                                                                                                       \
     template int sys_permute_in<T>(System<T> *, const T *, T *, int, cudaStream_t);                                   \
     template int sys_permute_out<T>(System<T> *, const T *, T *, int, cudaStream_t);                                  \
@@ -1250,6 +1560,8 @@ int sys_hysteresis(System<T> *S, const cm_step_params *base, const cm_hyst_param
     template int sys_stress<T>(System<T> *, const T *, const T *, cudaStream_t);                                      \
     template int sys_field<T>(System<T> *, const T *, const T *, const double *, unsigned, T *, T *, cudaStream_t, const double *); \
     template int sys_axpby3<T>(System<T> *, const T *, const T *, T, T *, cudaStream_t);                              \
+    template int sys_spmv_matfree<T>(System<T> *, const T *, T *, cudaStream_t);                                      \
+    template int sys_cg_matfree<T>(System<T> *, const T *, T *, double, int, int, int, int, cudaStream_t);            \
     template int sys_step<T>(System<T> *, const cm_step_params *, T *, T *, T *, cm_step_info *, cudaStream_t);        \
     template int sys_hysteresis<T>(System<T> *, const cm_step_params *, const cm_hyst_params *, T *, T *, T *, double *, double *, int *, \
                                    cm_hyst_result *, cudaStream_t);

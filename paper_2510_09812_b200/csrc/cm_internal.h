@@ -206,6 +206,7 @@ struct System : SystemBase {
     double *red = nullptr; // reduction partials
     double *dscal = nullptr, *h_scal = nullptr; // device / pinned scalars: mbar[3], gradU mean[3], dm sum, ...
     // hysteresis driver (cm_hysteresis_run): device-resident controller state and logs, grown on demand
+    void *mf_state = nullptr, *h_mf = nullptr; // matrix-free CG: two device states, pinned host copy
     void *hyst_ctl = nullptr;
     double *hyst_log = nullptr; // [cap][3] H, [cap][3] mbar
     int *hyst_steps = nullptr;  // [cap]
@@ -298,4 +299,7 @@ template <typename T> int sys_step(System<T> *S, const cm_step_params *p, T *m_u
                                    cudaStream_t st);
 template <typename T> int sys_hysteresis(System<T> *S, const cm_step_params *base, const cm_hyst_params *hp, T *m_user, T *U_user,
                                          T *u_user, double *H_log, double *mbar_log, int *steps_log, cm_hyst_result *res, cudaStream_t st);
+template <typename T> int sys_spmv_matfree(System<T> *S, const T *x_lib, T *y_lib, cudaStream_t st);
+template <typename T> int sys_cg_matfree(System<T> *S, const T *b_lib, T *x_lib, double tol, int maxiter, int fixed, int precond, int slot,
+                                         cudaStream_t st);
 template <typename T> int sys_axpby3(System<T> *S, const T *base, const T *h, T c, T *f, cudaStream_t st);

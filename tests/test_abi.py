@@ -30,7 +30,7 @@ def test_header_symbols_exported(binding):
 def test_struct_layouts_match_header(binding):
     # sizes implied by the header's field lists (x86-64 SysV)
     assert C.sizeof(binding.cm_material) == 8 * 8 + 9 * 8 + 8 + 8 + 9 * 8 + 6 * 8
-    assert C.sizeof(binding.cm_step_params) == 8 + 24 + 4 + 4 + 8 + 4 + 4 + 4 + 4   # cg_precond + tail padding
+    assert C.sizeof(binding.cm_step_params) == 8 + 24 + 4 + 4 + 8 + 4 + 4 + 4 + 4   # ... cg_precond, mech_matfree
     assert C.sizeof(binding.cm_step_info) == 4 * 10 + 8 * 10 + 24 + 8 + 8
     assert C.sizeof(binding.cm_profile) == 4 * 6 * 8
 
