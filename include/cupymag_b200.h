@@ -37,7 +37,10 @@ typedef struct cm_mesh cm_mesh;     /* opaque: reordered connectivity, node->ele
 typedef struct cm_system cm_system; /* opaque: geometry, assembled matrices, masks, work vectors (one dtype) */
 
 typedef enum { CM_F64 = 0, CM_F32 = 1 } cm_dtype;
-typedef enum { CM_REORDER_NONE = 0, CM_REORDER_MORTON = 1, CM_REORDER_RCM = 2 } cm_reorder;
+/* Locality reordering of the nodes (R21).  MORTON_SORTED: Morton order, then within every window of 256
+ * consecutive positions the nodes in descending order of row length (ties keep their Morton order): the slices of the
+ * SELL layouts then hold rows of nearly equal length on meshes of irregular valence (unstructured meshes). */
+typedef enum { CM_REORDER_NONE = 0, CM_REORDER_MORTON = 1, CM_REORDER_RCM = 2, CM_REORDER_MORTON_SORTED = 3 } cm_reorder;
 
 /* Matrices of Eq. 12 on the shared sparsity pattern; constraints applied as the symmetric
  * projection P A P + (I - P).  K_MS: all tets, one pinned node.  K_GS1/2 = M_m + eps K_m over
@@ -83,7 +86,9 @@ enum {
     CM_GET_ROWPTR = 5,    /* n_nodes + 1                                                     */
     CM_GET_COLIDX = 6,    /* nnz, ascending in each row, diagonal present                    */
     CM_GET_N2E_PTR = 7,   /* n_nodes + 1                                                     */
-    CM_GET_N2E = 8        /* 4 n_tets entries element*4 + local index, ascending per node    */
+    CM_GET_N2E = 8,       /* 4 n_tets entries element*4 + local index, ascending per node    */
+    CM_GET_LAYOUT = 9     /* long[6]: stored elements (padding included) of the SELL-16 scalar and the SELL-8 block
+                             layout, element chunks, chunk slots, chunk capacity in elements and in nodes */
 };
 
 /* Material constants of Eq. 1 and Appendix A; SI units. */

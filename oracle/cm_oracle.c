@@ -300,7 +300,10 @@ static void order_rcm(long N, const int *rowptr, const int *col, int *order)
 }
 
 /* Public: compute the locality permutation and the relabelled, sorted connectivity.
- * method: 0 none, 1 Morton, 2 RCM.  order[new] = old node; iperm[old] = new node.
+ * method: 0 none, 1 Morton, 2 RCM, 3 Morton followed by a windowed row-length sort (R21: within every window
+ * of 256 consecutive Morton positions the nodes are put in descending order of their row length, i.e. number of distinct
+ * neighbours, ties keeping their Morton order -- the sigma-window of a SELL-C-sigma layout written into the node order).
+ * order[new] = old node; iperm[old] = new node.
  * Tets keep their local node order and are sorted by (min new node id, user tet index);
  * tet_order[new_tet] = old tet. */
 int orc_reorder(const double *xyz, long N, const int *tets, long Ne, int method,
@@ -314,6 +317,25 @@ int orc_reorder(const double *xyz, long N, const int *tets, long Ne, int method,
         rc = build_pattern(N, tets, ptr, lst, &rowptr, &col, &nnz); if (rc) return rc;
         order_rcm(N, rowptr, col, order);
         free(ptr); free(lst); free(rowptr); free(col);
+    } else if (method == 3) {
+        int *ptr, *lst, *rowptr, *col; long nnz;
+        order_morton(N, xyz, order);
+        int rc = build_n2e(N, Ne, tets, &ptr, &lst); if (rc) return rc;
+        rc = build_pattern(N, tets, ptr, lst, &rowptr, &col, &nnz); if (rc) return rc;
+        int *tmp = (int *)malloc(256 * sizeof(int));
+        for (long w0 = 0; w0 < N; w0 += 256) {
+            long w1 = w0 + 256 < N ? w0 + 256 : N;
+            /* insertion sort: stable, descending row length */
+            for (long i = w0; i < w1; i++) tmp[i - w0] = order[i];
+            for (long i = 1; i < w1 - w0; i++) {
+                int v = tmp[i], lv = rowptr[v + 1] - rowptr[v];
+                long j = i - 1;
+                while (j >= 0 && rowptr[tmp[j] + 1] - rowptr[tmp[j]] < lv) { tmp[j + 1] = tmp[j]; j--; }
+                tmp[j + 1] = v;
+            }
+            for (long i = w0; i < w1; i++) order[i] = tmp[i - w0];
+        }
+        free(tmp); free(ptr); free(lst); free(rowptr); free(col);
     } else return ORC_E_BADARG;
     for (long i = 0; i < N; i++) iperm[order[i]] = (int)i;
     keyidx *k = (keyidx *)malloc((size_t)Ne * sizeof(keyidx));

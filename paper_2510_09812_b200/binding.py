@@ -16,7 +16,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libcupymag_b200.so"
 
 CM_F64, CM_F32 = 0, 1
-CM_REORDER_NONE, CM_REORDER_MORTON, CM_REORDER_RCM = 0, 1, 2
+CM_REORDER_NONE, CM_REORDER_MORTON, CM_REORDER_RCM, CM_REORDER_MORTON_SORTED = 0, 1, 2, 3
 CM_MAT_K_MS, CM_MAT_K_GS1, CM_MAT_K_GS2, CM_MAT_MASS, CM_MAT_K_MECH = range(5)
 CM_RHS_MS, CM_RHS_MECH, CM_RHS_GS, CM_OUT_HD, CM_OUT_SIGMA, CM_OUT_FIELD = range(6)
 CM_TERM_ANIS, CM_TERM_ZEEMAN, CM_TERM_DEMAG, CM_TERM_FARFIELD, CM_TERM_MAGEL = 1, 2, 4, 8, 16
@@ -24,6 +24,7 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
     0, -1, -2, -3, -4, -5, -6, -7
 (CM_GET_COUNTS, CM_GET_ORDER, CM_GET_IPERM, CM_GET_TETS, CM_GET_TET_ORDER, CM_GET_ROWPTR, CM_GET_COLIDX, CM_GET_N2E_PTR,
  CM_GET_N2E) = range(9)
+CM_GET_LAYOUT = 9
 CM_PC_NONE, CM_PC_JACOBI = 0, 1
 CM_OPT_STORED_GEOMETRY = 0
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
@@ -202,6 +203,15 @@ class Mesh:
         a = np.empty(n, np.int32)
         _check(lib().cm_mesh_get(self.h, what, _hp(a), n))
         return a.reshape(-1, self.nen) if what == CM_GET_TETS else a
+
+    def layout(self):
+        """CM_GET_LAYOUT: padding of the sliced matrix layouts and occupancy of the element chunks."""
+        a = np.zeros(6, np.int64)
+        _check(lib().cm_mesh_get(self.h, CM_GET_LAYOUT, _hp(a), 6))
+        e16, e8, nch, nsl, cap_e, cap_n = (int(v) for v in a)
+        return {"sell16_padding": e16 / self.nnz - 1.0, "sell8_padding": e8 / self.nnz - 1.0, "chunks": nch, "slots": nsl,
+                "slots_per_node": nsl / self.n_nodes, "elements_per_chunk": self.n_tets / max(1, nch), "chunk_capacity": (cap_e, cap_n),
+                "nodes_per_chunk": nsl / max(1, nch)}
 
     def volume_average(self, g):
         """cm_volume_average of a torch CUDA tensor (N,) or (N, ncomp), float64 / float32."""

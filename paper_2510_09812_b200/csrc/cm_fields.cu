@@ -155,18 +155,20 @@ struct ChunkArgs {
 
 // shared-memory layout (every region a multiple of 16 bytes):
 //   GEOM = false (stored geometry; wrapped meshes):
-//     planes [max(10, NOUT)][ne8] T   staged geometry, overwritten in place by the contributions
+//     planes [max(10, NOUT)][EC] T    staged geometry, overwritten in place by the contributions (fixed plane stride EC: the
+//                                     plane offsets are immediates)
 //   GEOM = true (geometry recomputed from the staged slot coordinates):
 //     scx    [CM_NL_MAX][4] double    nondimensional coordinates of the local nodes
-//     planes [NOUT][ne8] T            contributions
+//     planes [NOUT][EC] T             contributions
 //   sin    [CM_NL_MAX][NIN] T       nodal inputs
 //   slid   [EC] ushort4, sle [4 EC] ushort, sem [EC] ushort, slp [CM_NL_MAX + 8] ushort, mbarrier
+constexpr int nin_padded(int nin) { return nin; } // dense: a padded (power-of-two) node stride puts the random corner gathers on few banks (measured: S8 +17 %)
 template <int KIND, bool GEOM> constexpr int chunk_planes() { return (GEOM || KindTraits<KIND>::NOUT > 10) ? KindTraits<KIND>::NOUT : 10; }
 template <int KIND, typename T, bool GEOM>
 constexpr size_t chunk_smem_bytes()
 {
     return (GEOM ? (size_t)CM_NL_MAX * 4 * sizeof(double) : 0) +
-           (size_t)(chunk_planes<KIND, GEOM>() * CM_EC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
+           (size_t)(chunk_planes<KIND, GEOM>() * CM_EC_MAX + CM_NL_MAX * nin_padded(KindTraits<KIND>::NIN)) * sizeof(T) +
            (size_t)(4 * CM_EC_MAX + 4 * CM_EC_MAX + CM_EC_MAX + CM_NL_MAX + 8) * sizeof(unsigned short) + 16;
 }
 // resident CTAs per SM the launch bounds ask for (register cap): what the shared-memory footprint allows, at most 4
@@ -283,6 +285,29 @@ __device__ __forceinline__ void E0_sim(const Rot<T> &R, const T *m, T l1, T l2, 
     for (int q = 0; q < 3; q++) { e0[q] = t[q]; e0[3 + q] = (T)2 * t[3 + q]; }
 }
 
+// a staged 3-vector
+template <typename T>
+__device__ __forceinline__ void ld3(const T *p, T (&o)[3]) { o[0] = p[0]; o[1] = p[1]; o[2] = p[2]; }
+
+// H[a][b] = d_b x_a = sum_k x_k[a] grad phi_k[b], x_k = sx[ST * l[k] ..]
+template <typename T, int ST>
+__device__ __forceinline__ void strain_H(const T *sx, const int *l, const T (&g)[4][3], T (&H)[3][3])
+{
+#pragma unroll
+    for (int x = 0; x < 3; x++)
+#pragma unroll
+        for (int y = 0; y < 3; y++) H[x][y] = 0;
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        T xk[3];
+        ld3(sx + ST * l[k], xk);
+#pragma unroll
+        for (int x = 0; x < 3; x++)
+#pragma unroll
+            for (int y = 0; y < 3; y++) H[x][y] += xk[x] * g[k][y];
+    }
+}
+
 // mean over the 4 corners of E0(w); w_k = sw[ST * l[k] + OFF ..]
 template <typename T, int ST, int OFF>
 __device__ __forceinline__ void mean_E0(const Rot<T> &R, const T *sw, const int *l, T l1, T l2, T e0[6])
@@ -291,8 +316,8 @@ __device__ __forceinline__ void mean_E0(const Rot<T> &R, const T *sw, const int 
     for (int q = 0; q < 6; q++) e0[q] = 0;
 #pragma unroll
     for (int k = 0; k < 4; k++) {
-        const T *w = sw + ST * l[k] + OFF;
-        T mk[3] = {w[0], w[1], w[2]}, ek[6];
+        T mk[3], ek[6];
+        ld3(sw + ST * l[k] + OFF, mk);
         E0_sim(R, mk, l1, l2, ek);
 #pragma unroll
         for (int q = 0; q < 6; q++) e0[q] += ek[q];
@@ -340,12 +365,12 @@ template <typename T, int KIND, bool CUBIC, bool GEOM>
 __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chunk_kernel(ChunkArgs<T> a)
 {
     typedef KindTraits<KIND> K;
-    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX, NP = chunk_planes<KIND, GEOM>();
+    constexpr int NIN = K::NIN, NOUT = K::NOUT, NC = K::NC, EC = CM_EC_MAX, NP = chunk_planes<KIND, GEOM>(), NINP = nin_padded(NIN);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *scx = reinterpret_cast<double *>(smem_raw);                          // [nl][4] (GEOM)
-    T *scr = reinterpret_cast<T *>(smem_raw + (GEOM ? (size_t)CM_NL_MAX * 4 * sizeof(double) : 0)); // [NP][ne8]
+    T *scr = reinterpret_cast<T *>(smem_raw + (GEOM ? (size_t)CM_NL_MAX * 4 * sizeof(double) : 0)); // [NP][EC]
     T *sin = scr + NP * EC;                                                     // [nl][NIN]
-    ushort4 *slid = reinterpret_cast<ushort4 *>(sin + CM_NL_MAX * NIN);         // [ne]
+    ushort4 *slid = reinterpret_cast<ushort4 *>(sin + CM_NL_MAX * NINP);        // [ne]
     unsigned short *sle = reinterpret_cast<unsigned short *>(slid + EC);        // [4 ne]
     unsigned short *sem = sle + 4 * EC;                                         // [ne]
     unsigned short *slp = sem + EC;                                             // [nl + 1]
@@ -360,7 +385,8 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
         const unsigned bg = GEOM ? 32u * nl : 10u * ne8 * (unsigned)sizeof(T), bl = 8u * ne8, be = 2u * ne8;
         mbar_expect_tx(bar, bg + 2 * bl + be);
         if (GEOM) bulk_g2s(scx, a.CX + 4L * s0, bg, bar);
-        else bulk_g2s(scr, a.EG + 10L * e0, bg, bar);
+        else
+            for (int q = 0; q < 10; q++) bulk_g2s(scr + q * EC, a.EG + 10L * e0 + (long)q * ne8, bg / 10, bar);
         bulk_g2s(slid, a.lid + 4L * e0, bl, bar);
         bulk_g2s(sle, a.lent + 4L * e0, bl, bar);
         bulk_g2s(sem, a.emat + e0, be, bar);
@@ -372,13 +398,13 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
             sin[l] = a.in0[g];
         } else if (KIND == EK_KMECH) {
 #pragma unroll
-            for (int d = 0; d < 3; d++) sin[3 * l + d] = a.clamp[3 * g + d] ? (T)0 : a.in0[3 * g + d];
+            for (int d = 0; d < 3; d++) sin[NINP * l + d] = a.clamp[3 * g + d] ? (T)0 : a.in0[3 * g + d];
         } else {
 #pragma unroll
-            for (int d = 0; d < 3; d++) sin[NIN * l + d] = a.in0[3 * g + d];
+            for (int d = 0; d < 3; d++) sin[NINP * l + d] = a.in0[3 * g + d];
             if (KIND == EK_STRESS)
 #pragma unroll
-                for (int d = 0; d < 3; d++) sin[NIN * l + 3 + d] = a.in1[3 * g + d];
+                for (int d = 0; d < 3; d++) sin[NINP * l + 3 + d] = a.in1[3 * g + d];
         }
     }
     for (int l = tid; l <= nl; l += EK_NT) slp[l] = a.lptr[s0 + c + l];
@@ -411,40 +437,32 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
 #pragma unroll
             for (int k = 1; k < 4; k++)
 #pragma unroll
-                for (int d = 0; d < 3; d++) g[k][d] = scr[(3 * (k - 1) + d + 1) * ne8 + el];
+                for (int d = 0; d < 3; d++) g[k][d] = scr[(3 * (k - 1) + d + 1) * EC + el];
         }
 #pragma unroll
         for (int d = 0; d < 3; d++) g[0][d] = -(g[1][d] + g[2][d] + g[3][d]);
 
         if (KIND == EK_MS) {
             // c_k = V_e grad phi_k . (mean_e m - mbar)
-            T mt[3];
+            T mt[3], w0[3], w1[3], w2[3], w3[3];
+            ld3(sin + NINP * l[0], w0); ld3(sin + NINP * l[1], w1); ld3(sin + NINP * l[2], w2); ld3(sin + NINP * l[3], w3);
 #pragma unroll
-            for (int d = 0; d < 3; d++)
-                mt[d] = (sin[3 * l[0] + d] + sin[3 * l[1] + d] + sin[3 * l[2] + d] + sin[3 * l[3] + d]) / (T)4 - (T)a.mbar[d];
+            for (int d = 0; d < 3; d++) mt[d] = (w0[d] + w1[d] + w2[d] + w3[d]) / (T)4 - (T)a.mbar[d];
 #pragma unroll
-            for (int k = 0; k < 4; k++) scr[k * ne8 + el] = V * (g[k][0] * mt[0] + g[k][1] * mt[1] + g[k][2] * mt[2]);
+            for (int k = 0; k < 4; k++) scr[k * EC + el] = V * (g[k][0] * mt[0] + g[k][1] * mt[1] + g[k][2] * mt[2]);
         } else if (KIND == EK_GRADU) {
             // V_e grad U_e, and its fp64 sum for <grad U>
             const T u0 = sin[l[0]], u1 = sin[l[1]], u2 = sin[l[2]], u3 = sin[l[3]];
 #pragma unroll
             for (int d = 0; d < 3; d++) {
                 const T gU = u0 * g[0][d] + u1 * g[1][d] + u2 * g[2][d] + u3 * g[3][d];
-                scr[d * ne8 + el] = V * gU;
+                scr[d * EC + el] = V * gU;
                 gsum[d] += (double)V * (double)gU;
             }
         } else if (KIND == EK_KMECH) {
             // sigma = C*_e : E_e(x), H[a][b] = d_b x_a;  c_(k,a) = V_e (sigma grad phi_k)_a   (every element is elastic)
             T H[3][3];
-#pragma unroll
-            for (int x = 0; x < 3; x++)
-#pragma unroll
-                for (int y = 0; y < 3; y++) {
-                    T acc = 0;
-#pragma unroll
-                    for (int k = 0; k < 4; k++) acc += sin[3 * l[k] + x] * g[k][y];
-                    H[x][y] = acc;
-                }
+            strain_H<T, NINP>(sin, l, g, H);
             const T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]};
             T sg[6];
             const unsigned em = sem[el];
@@ -452,20 +470,20 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
             else C_times(a.Cstar + 36 * (em >> 1), eps, sg);
 #pragma unroll
             for (int k = 0; k < 4; k++) {
-                scr[(3 * k + 0) * ne8 + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
-                scr[(3 * k + 1) * ne8 + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
-                scr[(3 * k + 2) * ne8 + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
+                scr[(3 * k + 0) * EC + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
+                scr[(3 * k + 1) * EC + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
+                scr[(3 * k + 2) * EC + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
             }
         } else {
             const unsigned em = sem[el];
             if (!(em & 1u) && !(KIND == EK_MECH && a.has_sext)) {
 #pragma unroll
-                for (int q = 0; q < NOUT; q++) scr[q * ne8 + el] = 0;
+                for (int q = 0; q < NOUT; q++) scr[q * EC + el] = 0;
             } else if (KIND == EK_MECH) {
                 // S = C*_e : mean_e E0(m) (magnetic elements) + sigma_ext (all elements);  c_(k,a) = V_e (S grad phi_k)_a
                 T e0v[6], sg[6] = {0, 0, 0, 0, 0, 0};
                 if (em & 1u) {
-                    mean_E0<T, 3, 0>(a.rot, sin, l, a.l1, a.l2, e0v);
+                    mean_E0<T, NINP, 0>(a.rot, sin, l, a.l1, a.l2, e0v);
                     if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), e0v, sg);
                     else C_times(a.Cstar + 36 * (em >> 1), e0v, sg);
                 }
@@ -474,30 +492,22 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
                     for (int q = 0; q < 6; q++) sg[q] += a.sext[q];
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
-                    scr[(3 * k + 0) * ne8 + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
-                    scr[(3 * k + 1) * ne8 + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
-                    scr[(3 * k + 2) * ne8 + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
+                    scr[(3 * k + 0) * EC + el] = V * (sg[0] * g[k][0] + sg[5] * g[k][1] + sg[4] * g[k][2]);
+                    scr[(3 * k + 1) * EC + el] = V * (sg[5] * g[k][0] + sg[1] * g[k][1] + sg[3] * g[k][2]);
+                    scr[(3 * k + 2) * EC + el] = V * (sg[4] * g[k][0] + sg[3] * g[k][1] + sg[2] * g[k][2]);
                 }
             } else {
                 // V_e C*_e : (E_e(u) - mean_e E0(w)),  H[a][b] = d_b u_a
                 T H[3][3];
-#pragma unroll
-                for (int x = 0; x < 3; x++)
-#pragma unroll
-                    for (int y = 0; y < 3; y++) {
-                        T acc = 0;
-#pragma unroll
-                        for (int k = 0; k < 4; k++) acc += sin[6 * l[k] + x] * g[k][y];
-                        H[x][y] = acc;
-                    }
+                strain_H<T, NINP>(sin, l, g, H);
                 T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]}, e0v[6], sg[6];
-                mean_E0<T, 6, 3>(a.rot, sin, l, a.l1, a.l2, e0v);
+                mean_E0<T, NINP, 3>(a.rot, sin, l, a.l1, a.l2, e0v);
 #pragma unroll
                 for (int q = 0; q < 6; q++) eps[q] -= e0v[q];
                 if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), eps, sg);
                 else C_times(a.Cstar + 36 * (em >> 1), eps, sg);
 #pragma unroll
-                for (int q = 0; q < 6; q++) scr[q * ne8 + el] = V * sg[q];
+                for (int q = 0; q < 6; q++) scr[q * EC + el] = V * sg[q];
             }
         }
     }
@@ -511,7 +521,7 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
         for (int q = slp[l]; q < slp[l + 1]; q++) {
             const int ent = sle[q], el = ent >> 2, k = ent & 3;
 #pragma unroll
-            for (int x = 0; x < NC; x++) acc[x] += scr[(K::PERK ? NC * k + x : x) * ne8 + el];
+            for (int x = 0; x < NC; x++) acc[x] += scr[(K::PERK ? NC * k + x : x) * EC + el];
         }
 #pragma unroll
         for (int x = 0; x < NC; x++) a.hpart[(long)(s0 + l) * NC + x] = acc[x];

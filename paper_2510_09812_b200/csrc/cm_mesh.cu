@@ -144,6 +144,21 @@ void rcm_order(long N, const std::vector<int> &rowptr, const std::vector<int> &c
 
 } // namespace
 
+// R21, CM_REORDER_MORTON_SORTED: within every window of CM_SORT_WINDOW consecutive positions of `order`, nodes in
+// descending order of their row length (rowptr in USER numbering), ties keeping their order -- the sigma-window of a
+// SELL-C-sigma layout folded into the node permutation, so that the slices of 8 / 16 consecutive rows hold rows of
+// nearly equal length on meshes of irregular valence and no kernel needs a row indirection
+constexpr long CM_SORT_WINDOW = 256;
+static void window_sort(long N, const std::vector<int> &rowptr, std::vector<int> &order)
+{
+#pragma omp parallel for schedule(static)
+    for (long w0 = 0; w0 < N; w0 += CM_SORT_WINDOW) {
+        const long w1 = std::min(N, w0 + CM_SORT_WINDOW);
+        std::stable_sort(order.begin() + w0, order.begin() + w1,
+                         [&](int a, int b) { return rowptr[a + 1] - rowptr[a] > rowptr[b + 1] - rowptr[b]; });
+    }
+}
+
 int mesh_build_host(cm_mesh *M, const double *gx, long Ng, const int *gtets, long Ne, const uchar *mag, const int *eid,
                     const int *dof, long N, cm_reorder reorder)
 {
@@ -224,6 +239,12 @@ int mesh_build_host(cm_mesh *M, const double *gx, long Ng, const int *gtets, lon
         build_n2e(N, Ne, tets, ptr_u, lst_u);
         build_pattern(N, tets, ptr_u, lst_u, rp, cl);
         rcm_order(N, rp, cl, M->order);
+    } else if (reorder == CM_REORDER_MORTON_SORTED) {
+        std::vector<int> rp, cl;
+        morton_order(N, xyz, M->order);
+        build_n2e(N, Ne, tets, ptr_u, lst_u);
+        build_pattern(N, tets, ptr_u, lst_u, rp, cl);
+        window_sort(N, rp, M->order);
     } else {
         cm_set_error("cm_mesh_create: unknown reorder %d", (int)reorder);
         return CM_E_BADARG;
@@ -372,6 +393,12 @@ int mesh_build_host_hex(cm_mesh *M, const double *gx, long Ng, const int *ghexes
         build_n2e(N, Ne, hexes, ptr_u, lst_u, 8);
         build_pattern(N, hexes, ptr_u, lst_u, rp, cl, 8);
         rcm_order(N, rp, cl, M->order);
+    } else if (reorder == CM_REORDER_MORTON_SORTED) {
+        std::vector<int> rp, cl;
+        morton_order(N, xyz, M->order);
+        build_n2e(N, Ne, hexes, ptr_u, lst_u, 8);
+        build_pattern(N, hexes, ptr_u, lst_u, rp, cl, 8);
+        window_sort(N, rp, M->order);
     } else {
         cm_set_error("cm_mesh_create_hex: unknown reorder %d", (int)reorder);
         return CM_E_BADARG;
@@ -743,6 +770,12 @@ extern "C" int cm_mesh_get(const cm_mesh *M, int what, void *host_out, long capa
         if (capacity < 3) { cm_set_error("cm_mesh_get: capacity"); return CM_E_BADARG; }
         ((long *)host_out)[0] = M->N; ((long *)host_out)[1] = M->Ne; ((long *)host_out)[2] = M->nnz;
         return CM_OK;
+    case CM_GET_LAYOUT: {
+        if (capacity < 6) { cm_set_error("cm_mesh_get: capacity"); return CM_E_BADARG; }
+        long *o = (long *)host_out;
+        o[0] = M->sell[0].E; o[1] = M->sell[1].E; o[2] = M->ck.nchunks; o[3] = M->ck.nslots; o[4] = CM_EC_MAX; o[5] = CM_NL_MAX;
+        return CM_OK;
+    }
     case CM_GET_ORDER: v = &M->order; break;
     case CM_GET_IPERM: v = &M->iperm; break;
     case CM_GET_TETS: v = &M->tets; break;

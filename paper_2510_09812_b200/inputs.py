@@ -189,6 +189,38 @@ def hex_box(grid, box, jitter=0.15, seed_mesh=1, seed_perm=2, permute=True) -> H
                    grid=tuple(grid), box=tuple(box), node_perm=t.node_perm)
 
 
+def delaunay_box(grid, box, jitter=0.45, seed_mesh=1, seed_perm=2, permute=True) -> Mesh:
+    """Unstructured tetrahedral mesh with the valence spread of a real mesh generator's output (the paper's COMSOL meshes,
+    P:298-306: 8-30 neighbours per node, where the Kuhn split of kuhn_box has 14 almost everywhere): Delaunay
+    tetrahedralisation (scipy / Qhull) of an nx x ny x nz lattice whose INTERIOR nodes are displaced uniformly by
+    +-jitter of the spacing in every direction and whose face nodes slide within their face.  Flat cells that Qhull leaves
+    between coplanar face nodes (volume below 1e-6 of the mean cell volume) are dropped.  Mesh bookkeeping only."""
+    from scipy.spatial import Delaunay
+    nx, ny, nz = grid
+    n = nx * ny * nz
+    ix, iy, iz = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij")
+    order = np.argsort(((iz * ny + iy) * nx + ix).ravel(), kind="stable")      # node id = (iz ny + iy) nx + ix
+    idx = np.stack([ix.ravel()[order], iy.ravel()[order], iz.ravel()[order]], axis=1)
+    h = np.array([box[d] / (grid[d] - 1) for d in range(3)])
+    on_face = (idx == 0) | (idx == np.array(grid) - 1)           # per node, per direction: fixed in that direction
+    rng = np.random.default_rng(seed_mesh)
+    xyz = idx * h + np.where(on_face, 0.0, jitter * h * rng.uniform(-1.0, 1.0, size=(n, 3)))
+    tets = Delaunay(xyz).simplices.astype(np.int64)
+    a, b, c, d = (xyz[tets[:, k]] for k in range(4))
+    vol = np.einsum("ij,ij->i", np.cross(b - a, c - a), d - a) / 6.0
+    keep = np.abs(vol) > 1e-6 * np.abs(vol).mean()
+    tets, vol = tets[keep], vol[keep]
+    neg = vol < 0                                                # positive orientation, as kuhn_box gives
+    tets[neg] = tets[neg][:, [0, 2, 1, 3]]
+    n = xyz.shape[0]
+    perm = np.random.default_rng(seed_perm).permutation(n) if permute else np.arange(n)
+    xyz_p = np.empty_like(xyz); xyz_p[perm] = xyz                # old node i -> label perm[i]
+    tets = perm[tets].astype(np.int32)
+    ne = tets.shape[0]
+    return Mesh(xyz=np.ascontiguousarray(xyz_p), tets=np.ascontiguousarray(tets), magnetic=np.ones(ne, np.uint8),
+                elastic_id=np.zeros(ne, np.int32), grid=tuple(grid), box=tuple(box), node_perm=perm)
+
+
 def flag_inclusion(mesh: Mesh, center, semi_axes, rotation: Optional[np.ndarray] = None) -> Mesh:
     """Flag elements (tets or hexahedra) whose centroid lies inside the (rotated) ellipsoid as non-magnetic,
     elastic material 1."""

@@ -49,13 +49,13 @@ def hex_elem_bytes(N, Ne, s):
             "elem_sigma": cell + N * 12 * s}
 
 
-def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=False):
+def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=False, delaunay=False):
     import torch
     from . import binding as cm
     peak = peak_gbs()
     L2 = 126e6
     rows = []
-    names = {"none": cm.CM_REORDER_NONE, "morton": cm.CM_REORDER_MORTON, "rcm": cm.CM_REORDER_RCM}
+    names = {"none": cm.CM_REORDER_NONE, "morton": cm.CM_REORDER_MORTON, "rcm": cm.CM_REORDER_RCM, "sorted": cm.CM_REORDER_MORTON_SORTED}
 
     def timeit(fn, n):
         for _ in range(3):
@@ -69,11 +69,22 @@ def run(sides, dtypes, reorders, only, reps, tol=1e-8, skip_tol=False, hex_mesh=
         return float(np.median(ts))
 
     for side in sides:
-        mesh = inputs.make_config4_hex_mesh(side) if hex_mesh else inputs.make_config4_mesh(side)
+        if delaunay:      # irregular valence: Delaunay tetrahedralisation of a strongly jittered lattice
+            L = 2.5e-9 * (side - 1)
+            mesh = inputs.delaunay_box((side,) * 3, (L,) * 3, seed_mesh=41, seed_perm=42)
+        else:
+            mesh = inputs.make_config4_hex_mesh(side) if hex_mesh else inputs.make_config4_mesh(side)
         clamp = inputs.clamp_face_x0(mesh)
         mat = inputs.Material()
         for ro in reorders:
             gm = cm.Mesh(mesh.xyz, mesh.hexes if hex_mesh else mesh.tets, reorder=names[ro])
+            lay = gm.layout()
+            rp = gm.get(cm.CM_GET_ROWPTR)
+            deg = np.diff(rp)
+            print(f"{side:4d}^3 N={gm.n_nodes:8d} {ro:7s} layout: nnz/row {deg.mean():.2f} (min {deg.min()}, max {deg.max()}), SELL-16 padding "
+                  f"{100 * lay['sell16_padding']:.1f} %, SELL-8 padding {100 * lay['sell8_padding']:.1f} %, "
+                  f"{lay['elements_per_chunk']:.0f} elements and {lay['nodes_per_chunk']:.0f} nodes per chunk (capacity {lay['chunk_capacity']}), "
+                  f"{lay['slots_per_node']:.2f} slots per node", flush=True)
             for dtype in dtypes:
                 gs = cm.System(gm, mat, 1e-12, dtype, clamp, 0)
                 td = torch.float64 if dtype == "f64" else torch.float32
@@ -165,10 +176,11 @@ def main(argv=None):
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--json", default="")
     ap.add_argument("--hex", action="store_true", help="linear hexahedral meshes (27 nnz/row; the paper's Fig. 2 workload) instead of tetrahedra")
+    ap.add_argument("--delaunay", action="store_true", help="irregular-valence Delaunay meshes (rows of 5-30 entries) instead of Kuhn grids")
     ap.add_argument("--skip-tol", action="store_true", help="skip the CG-to-1e-8 solves (fixed 3 iterations only)")
     a = ap.parse_args(argv)
     rows = run([int(s) for s in a.sides.split(",")], a.dtypes.split(","), a.reorders.split(","),
-               set(a.only.split(",")) if a.only else set(), a.reps, skip_tol=a.skip_tol, hex_mesh=a.hex)
+               set(a.only.split(",")) if a.only else set(), a.reps, skip_tol=a.skip_tol, hex_mesh=a.hex, delaunay=a.delaunay)
     if a.json:
         Path(a.json).write_text(json.dumps(rows, indent=1))
 

@@ -3,6 +3,8 @@ Morton order -- the launch configuration `bench.py` times.  The oracle is fast e
 output of a single pass at this size (SpMV, right-hand sides, fields, a few CG iterations, one step with fixed
 iteration counts), so outputs are compared element by element, not sampled; what it cannot afford is the ~2000
 iterations per solve of a converged step, which the mid-size tests cover.  Tolerances: DESIGN.md section 8."""
+import os
+
 import numpy as np
 import pytest
 
@@ -200,3 +202,86 @@ def test_full_size_fp32_build_against_fp64_oracle(full, oracle_mod):
     it, res, rc = gs.cg_solve(cm.CM_MAT_K_MECH, dev(b3), xg, fixed_iters=3)
     xo, ito, reso, _ = o.cg(oracle_mod.MAT_K_MECH, b3.astype(np.float64).ravel(), fixed=3)
     assert it == 3 and rel(xg.cpu().numpy().ravel(), xo) < 1e-4 and res == pytest.approx(reso, rel=1e-3)
+
+
+def test_config3_one_converged_step(full, oracle_mod):
+    """ONE whole GSPM step of config 3 with every solve iterated to the paper's tolerance 1e-7 on both sides -- the
+    ~1800-iteration persistent launches `bench.py` times (about 2.5 minutes of oracle time on the GPU box's host cores).
+    Counts: magnetostatic and Helmholtz solves +-1, mechanical solve 1.5 % (tests/test_gpu_parity.py::_check_iters); the
+    device's U and u satisfy the ORACLE's operator to the reported residual; m agrees to the accuracy two tol-1e-7 solves
+    of the same systems can (each side's U, u carry an O(tol x condition) error of their own)."""
+    cfg, cm, gm, gs, o, torch = full
+    N = o.N
+    m = cfg.m0.copy(); U = np.zeros(N); u = np.zeros((N, 3))
+    mg = _dev(torch, m); Ug = torch.zeros(N, dtype=torch.float64, device="cuda")
+    ug = torch.zeros((N, 3), dtype=torch.float64, device="cuda")
+    ig, rcg = gs.gspm_step(cm.make_params(cfg.dt, cfg.Hext[0], cfg.terms, 0, 1e-7), mg, Ug, ug)
+    io, rco = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[0], cfg.terms, cg_tol=1e-7)
+    assert rco == 0 and rcg == 0
+    print(f"\nconfig 3, one converged step: CG its oracle ms/mech/gs {io.it_ms}/{io.it_mech}/{list(io.it_gs)}  "
+          f"device {ig.it_ms}/{ig.it_mech}/{list(ig.it_gs)}")
+    assert abs(io.it_ms - ig.it_ms) <= 1, (io.it_ms, ig.it_ms)
+    assert abs(io.it_mech - ig.it_mech) <= int(np.ceil(0.015 * io.it_mech)), (io.it_mech, ig.it_mech)
+    for a in range(8):
+        assert abs(io.it_gs[a] - ig.it_gs[a]) <= 1, (a, list(io.it_gs), list(ig.it_gs))
+    assert ig.it_ms > 1000 and ig.it_mech > 1000
+    # true residuals of the device's solutions under the oracle's operators and right-hand sides
+    b_ms = o.rhs_ms(cfg.m0)
+    r = b_ms - o.spmv(oracle_mod.MAT_K_MS, Ug.cpu().numpy())
+    assert np.linalg.norm(r) / np.linalg.norm(b_ms) < 1.05e-7
+    b_me = o.rhs_mech(cfg.m0)
+    r = b_me.ravel() - o.spmv(oracle_mod.MAT_K_MECH, ug.cpu().numpy().ravel())
+    assert np.linalg.norm(r) / np.linalg.norm(b_me) < 1.05e-7
+    assert ig.res_ms < 1e-7 and ig.res_mech < 1e-7
+    dm = np.abs(mg.cpu().numpy() - m).max()
+    print(f"config 3, one converged step at tol 1e-7: max |dm| = {dm:.2e}, max |dU| / max |U| = {rel(Ug.cpu().numpy(), U):.2e}, "
+          f"max |du| / max |u| = {rel(ug.cpu().numpy(), u):.2e}")
+    assert dm <= 1e-4
+    assert np.allclose(ig.mbar[:], io.mbar[:], atol=1e-12) and ig.mean_dm == pytest.approx(io.mean_dm, rel=1e-4)
+
+
+SLOW = pytest.mark.skipif(os.environ.get("CM_SLOW_TESTS", "0") != "1",
+                          reason="about 7 minutes of oracle time: set CM_SLOW_TESTS=1 (log of the last run: profiles/r02_fullsize_converged.txt)")
+
+
+@SLOW
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2_full_size_10_steps(oracle_mod, dtype):
+    """BASELINE config 2 at its own size (129x129x31 = 515,871 nodes, all physics, spherical inclusion with x2 stiffness,
+    clamped bottom face, dt = 10 ps): ten steps, every solve iterated to convergence on both sides.
+    fp64: tol 1e-12, max |dm| <= 1e-9, counts +-1 (mechanical 1.5 %).
+    fp32 against the fp64 oracle, tol 1e-6: <= 1e-4 after the FIRST step (the rounding level of an fp32 step).  Over ten steps
+    the difference grows by a factor ~2 per step -- config 2 runs at dtau = 2.65, where m changes by O(1) per step (R5) and
+    any perturbation, an fp32 rounding included, is amplified; north_star's 1e-4 after ten steps holds on the stable
+    configurations (0 and 1, tests/test_gpu_parity.py, test_config1_full_size_10_steps) and is reported, not met, here."""
+    import torch
+    from paper_2510_09812_b200 import binding as cm
+    cfg = inputs.make_config(2)
+    assert cfg.mesh.n_nodes == 515871
+    f64 = dtype == "f64"
+    tol = 1e-12 if f64 else 1e-6
+    td = torch.float64 if f64 else torch.float32
+    gm = cm.Mesh(cfg.mesh.xyz, cfg.mesh.tets, cfg.mesh.magnetic, cfg.mesh.elastic_id, cm.CM_REORDER_MORTON)
+    gs = cm.System(gm, cfg.material, cfg.dt, dtype, cfg.clamp_dof, cfg.pin_node)
+    o = oracle_mod.Oracle(cfg.mesh, cfg.material, cfg.dt, clamp_dof=cfg.clamp_dof, pin_node=cfg.pin_node)
+    N = o.N
+    m = cfg.m0.copy(); U = np.zeros(N); u = np.zeros((N, 3))
+    mg = torch.as_tensor(cfg.m0, dtype=td, device="cuda").contiguous()
+    Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+    errs = []
+    for k in range(10):
+        io, rco = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k], cfg.terms, cg_tol=tol)
+        ig, rcg = gs.gspm_step(cm.make_params(cfg.dt, cfg.Hext[k], cfg.terms, 0, tol), mg, Ug, ug)
+        assert rco == 0 and rcg == 0
+        errs.append(float(np.abs(mg.cpu().numpy().astype(np.float64) - m).max()))
+        if f64:
+            assert abs(io.it_ms - ig.it_ms) <= 1, (k, io.it_ms, ig.it_ms)
+            assert abs(io.it_mech - ig.it_mech) <= int(np.ceil(0.015 * io.it_mech)), (k, io.it_mech, ig.it_mech)
+            for a in range(8):
+                assert abs(io.it_gs[a] - ig.it_gs[a]) <= 1, (k, a, list(io.it_gs), list(ig.it_gs))
+    print(f"\nconfig 2 full size, {dtype}: max |dm| after steps 1..10 = {['%.1e' % e for e in errs]}; last-step CG its ms/mech "
+          f"{ig.it_ms}/{ig.it_mech}, <|dm|> per step {io.mean_dm:.2f}")
+    if f64:
+        assert errs[-1] <= 1e-9, errs
+    else:
+        assert errs[0] <= 1e-4 and errs[-1] <= 5e-2, errs

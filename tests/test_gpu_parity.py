@@ -66,9 +66,13 @@ def case(request, cm, oracle_mod, torch):
 
 
 # ---------------------------------------------------------------------------------------------- structure
-@pytest.mark.parametrize("reorder", [0, 1, 2])
-def test_structure_bit_exact(cm, oracle_mod, torch, reorder):
-    mesh = inputs.kuhn_box((9, 8, 7), (20 * NM, 18 * NM, 15 * NM), seed_mesh=61, seed_perm=62)
+@pytest.mark.parametrize("kind", ["kuhn", "delaunay"])
+@pytest.mark.parametrize("reorder", [0, 1, 2, 3])
+def test_structure_bit_exact(cm, oracle_mod, torch, reorder, kind):
+    if kind == "kuhn":
+        mesh = inputs.kuhn_box((9, 8, 7), (20 * NM, 18 * NM, 15 * NM), seed_mesh=61, seed_perm=62)
+    else:
+        mesh = inputs.delaunay_box((11, 10, 9), (25 * NM, 22 * NM, 20 * NM), seed_mesh=61, seed_perm=62)
     gm = cm.Mesh(mesh.xyz, mesh.tets, reorder=reorder)
     order, iperm, tnew, torder = oracle_mod.reorder(mesh.xyz, mesh.tets, reorder)
     assert np.array_equal(gm.get(cm.CM_GET_ORDER), order)
@@ -83,6 +87,51 @@ def test_structure_bit_exact(cm, oracle_mod, torch, reorder):
     assert np.array_equal(gm.get(cm.CM_GET_COLIDX), o.colidx())
     assert np.array_equal(gm.get(cm.CM_GET_N2E_PTR), o.n2e_ptr())
     assert np.array_equal(gm.get(cm.CM_GET_N2E), o.n2e())
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_irregular_valence_mesh(cm, oracle_mod, torch, dtype):
+    """Unstructured mesh with rows of 5-30 entries (inputs.delaunay_box; the paper's COMSOL meshes) in the
+    row-length-sorted Morton order: padding of the sliced layouts, matrices, products, every right-hand side and field,
+    CG and five magnetoelastic GSPM steps against the oracle."""
+    mesh = inputs.delaunay_box((17, 15, 13), (48 * NM, 42 * NM, 36 * NM), seed_mesh=91, seed_perm=92)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (11 * NM, 9 * NM, 8 * NM))
+    clamp = inputs.clamp_bottom(mesh)
+    c = Case(cm, oracle_mod, torch, mesh, mat2(), 2e-12, dtype, cm.CM_REORDER_MORTON_SORTED, clamp=clamp, pin=5)
+    tol = TOL[dtype]
+    deg = np.diff(c.o.rowptr())
+    assert deg.max() - deg.min() >= 12
+    lay, lay_m = c.gm.layout(), cm.Mesh(mesh.xyz, mesh.tets, reorder=cm.CM_REORDER_MORTON).layout()
+    assert lay["sell16_padding"] < 0.10 and lay["sell16_padding"] < 0.5 * lay_m["sell16_padding"]
+    assert lay["sell8_padding"] < 0.06
+    for mat_g, mat_o in ((cm.CM_MAT_K_MS, oracle_mod.MAT_K_MS), (cm.CM_MAT_K_GS1, oracle_mod.MAT_K_GS1),
+                         (cm.CM_MAT_MASS, oracle_mod.MAT_MASS), (cm.CM_MAT_K_MECH, oracle_mod.MAT_K_MECH)):
+        A = _to_user(c, c.gs.values(mat_g), mat_g == cm.CM_MAT_K_MECH)
+        B = c.o.csr(mat_o)
+        assert abs(A - B).max() < (tol if dtype == "f64" else 2e-7) * abs(B).max(), mat_g
+    rng = np.random.default_rng(93)
+    N = c.o.N
+    x = rng.normal(size=(N, 3)).astype(c.gs.np_dtype); x64 = x.astype(np.float64)
+    assert rel(c.gs.spmv(cm.CM_MAT_K_MECH, c.dev(x)).cpu().numpy().ravel(), c.o.spmv(oracle_mod.MAT_K_MECH, x64.ravel())) < tol
+    assert rel(c.gs.spmv_matfree(c.dev(x)).cpu().numpy().ravel(), c.o.spmv(oracle_mod.MAT_K_MECH, x64.ravel())) < tol
+    assert rel(c.gs.spmv3(cm.CM_MAT_MASS, c.dev(x)).cpu().numpy(), c.o.rhs_gs(x64)) < tol
+    assert rel(c.gs.spmv(cm.CM_MAT_K_MS, c.dev(x[:, 0].copy())).cpu().numpy(), c.o.spmv(oracle_mod.MAT_K_MS, x64[:, 0].copy())) < tol
+    m = inputs.init_m_random(mesh, 94).astype(c.gs.np_dtype); m64 = m.astype(np.float64)
+    U = rng.normal(size=N).astype(c.gs.np_dtype); u = (1e-3 * rng.normal(size=(N, 3))).astype(c.gs.np_dtype)
+    H = np.array([3e4, -1e4, 2e4])
+    p = cm.make_params(c.dt, H, ALL)
+    assert rel(c.gs.field_rhs(cm.CM_RHS_MS, c.dev(m)).cpu().numpy(), c.o.rhs_ms(m64)) < tol
+    assert rel(c.gs.field_rhs(cm.CM_RHS_MECH, c.dev(m)).cpu().numpy(), c.o.rhs_mech(m64)) < tol
+    hd_o, _ = c.o.demag_field(U.astype(np.float64), c.o.volume_average(m64), ALL)
+    sig_o = c.o.stress_recover(u.astype(np.float64), m64)
+    h_o = c.o.field(m64, hd_o, sig_o, H / c.mat.Ms, ALL)
+    assert rel(c.gs.field_rhs(cm.CM_OUT_FIELD, c.dev(m), c.dev(U), c.dev(u), p).cpu().numpy(), h_o) < tol
+    if dtype == "f64":
+        m0 = inputs.init_m_noisy_x(mesh, 95)
+        ms, Us, us, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, mesh, mat2(), 1e-12, ALL, 5, "f64", np.tile([2e4, 0, 0], (5, 1)),
+                                                      clamp=clamp, reorder=cm.CM_REORDER_MORTON_SORTED, m0=m0)
+        assert np.abs(mg - ms).max() <= 1e-9
+        _check_iters(infos, mech_frac=0.015)
 
 
 def test_errors(cm, torch):

@@ -156,14 +156,22 @@ def _rcm_py(N, adj):
     return cm[::-1]
 
 
-def test_reorder_bruteforce(orc):
-    mesh = inputs.kuhn_box((5, 4, 6), (10 * NM, 8 * NM, 12 * NM), seed_mesh=7, seed_perm=8)
+@pytest.mark.parametrize("kind", ["kuhn", "delaunay"])
+def test_reorder_bruteforce(orc, kind):
+    if kind == "kuhn":
+        mesh = inputs.kuhn_box((5, 4, 6), (10 * NM, 8 * NM, 12 * NM), seed_mesh=7, seed_perm=8)
+    else:                                         # irregular valence (several windows of 256, rows of 5-25 entries)
+        mesh = inputs.delaunay_box((9, 8, 10), (18 * NM, 16 * NM, 20 * NM), seed_mesh=7, seed_perm=8)
     N = mesh.n_nodes
     adj = [set() for _ in range(N)]
     for t in mesh.tets:
         for i in t:
             adj[i].update(int(j) for j in t if j != i)
-    for method, want in ((0, list(range(N))), (1, _morton_py(mesh.xyz)), (2, _rcm_py(N, adj))):
+    mort = _morton_py(mesh.xyz)
+    wsorted = []                                  # method 3: windows of 256 Morton positions, descending row length, stable
+    for w0 in range(0, N, 256):
+        wsorted += sorted(mort[w0:w0 + 256], key=lambda i: -(len(adj[i]) + 1))
+    for method, want in ((0, list(range(N))), (1, mort), (2, _rcm_py(N, adj)), (3, wsorted)):
         order, iperm, tnew, torder = orc.reorder(mesh.xyz, mesh.tets, method)
         assert sorted(order) == list(range(N))                       # bijection
         assert list(order) == want
@@ -173,6 +181,13 @@ def test_reorder_bruteforce(orc):
         key = sorted(range(mesh.n_tets), key=lambda e: (relab[e].min(), e))
         assert list(torder) == key
         assert np.array_equal(tnew, relab[key])
+    if kind == "delaunay":
+        deg = np.array([len(a) + 1 for a in adj])
+        assert deg.max() - deg.min() >= 10        # the valence spread the generator is there for
+        order3 = orc.reorder(mesh.xyz, mesh.tets, 3)[0]
+        pad = lambda o, C: sum(deg[o[i:i + C]].max() * len(o[i:i + C]) for i in range(0, N, C)) / deg.sum() - 1
+        assert pad(order3, 16) < 0.5 * pad(np.array(mort), 16)     # what the sort is for: less SELL-16 padding
+        return
     # RCM reduces the bandwidth of the randomly permuted labelling by a lot
     order, iperm, tnew, _ = orc.reorder(mesh.xyz, mesh.tets, 2)
     bw_user = max(abs(int(a) - int(b)) for t in mesh.tets for a in t for b in t)
