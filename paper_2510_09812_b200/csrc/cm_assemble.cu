@@ -420,6 +420,10 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         S->Vtot = hv[0]; S->Vmag = hv[1];
     } else {
         S->Vtot = M->vtot_m3 / (ld * ld * ld); S->Vmag = M->vmag_m3 / (ld * ld * ld);
+        if (!M->wrapped) {
+            CM_TRY(alloc(&S->CX, (size_t)4 * M->ck.nslots + 8));
+            slot_xyz_kernel<<<(unsigned)((M->ck.nslots + B - 1) / B), B, 0, st>>>(M->ck.nslots, M->ck.d_nodes, M->d_xyz, ld, S->CX);
+        }
     }
     // matrices: fp64 scratch on the pattern
     double *&K = scr.K, *&Km = scr.Km, *&Mm = scr.Mm, *&Kme = scr.Kme;

@@ -902,9 +902,209 @@ __global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
     }
 }
 
+// ---- element-centric passes on plain (not wrapped) hexahedral meshes: one CTA per chunk of at most CM_HC_MAX cells, EIGHT
+// lanes per cell, one per Gauss point.  A lane recomputes the fp64 geometry at its point from the chunk's staged slot
+// coordinates, evaluates the integrand there and its contribution to the cell's eight corners; a three-step exchange
+// inside the 8-lane group (halving the corners kept at every step) leaves lane p with the cell's total for corner p,
+// which goes to the contribution planes.  Phase 2 and the node passes are those of the tetrahedral kernels.  Each cell is
+// integrated once (the node-centric kernel above integrates it eight times, once per corner).
+constexpr int HK_NT = 256;
+
+__device__ __forceinline__ double shfl_x(unsigned mask, double v, int o) { return __shfl_xor_sync(mask, v, o); }
+__device__ __forceinline__ float shfl_x(unsigned mask, float v, int o) { return __shfl_xor_sync(mask, v, o); }
+
+// lane p holds the contribution ph[a] * w[x] (RANK1) or c[a][x] of its Gauss point to corner a; out[x] = sum over the 8
+// lanes of the contributions to corner p (fixed order)
+template <typename T, int NC, bool RANK1>
+__device__ __forceinline__ void cell_exchange(unsigned mask, int p, const T (&ph)[8], const T (&w)[NC], const T (&c)[8][NC], T (&out)[NC])
+{
+    const bool h4 = p & 4, h2 = p & 2, h1 = p & 1;
+    T k1[4][NC];
+#pragma unroll
+    for (int j = 0; j < 4; j++)
+#pragma unroll
+        for (int x = 0; x < NC; x++) {
+            const T lo = RANK1 ? ph[j] * w[x] : c[j][x], hi = RANK1 ? ph[4 + j] * w[x] : c[4 + j][x];
+            k1[j][x] = (h4 ? hi : lo) + shfl_x(mask, h4 ? lo : hi, 4);
+        }
+    T k2[2][NC];
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+#pragma unroll
+        for (int x = 0; x < NC; x++) k2[i][x] = (h2 ? k1[2 + i][x] : k1[i][x]) + shfl_x(mask, h2 ? k1[i][x] : k1[2 + i][x], 2);
+#pragma unroll
+    for (int x = 0; x < NC; x++) out[x] = (h1 ? k2[1][x] : k2[0][x]) + shfl_x(mask, h1 ? k2[0][x] : k2[1][x], 1);
+}
+
+template <int KIND, typename T>
+constexpr size_t hex_smem_bytes()
+{
+    return (size_t)CM_NL_MAX * 4 * sizeof(double) + (size_t)(8 * KindTraits<KIND>::NC * CM_HC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
+           (size_t)(8 * CM_HC_MAX + 8 * CM_HC_MAX + CM_HC_MAX + CM_NL_MAX + 8) * sizeof(unsigned short) + 16;
+}
+
+template <typename T, int KIND>
+__global__ void __launch_bounds__(HK_NT, 2) hex_chunk_kernel(ChunkArgs<T> a)
+{
+    typedef KindTraits<KIND> K;
+    constexpr int NIN = K::NIN, NC = K::NC, HC = CM_HC_MAX;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *scx = reinterpret_cast<double *>(smem_raw);                          // [nl][4]
+    T *scr = reinterpret_cast<T *>(scx + (size_t)CM_NL_MAX * 4);                 // [8 NC][HC]
+    T *sin = scr + 8 * NC * HC;                                                 // [nl][NIN]
+    unsigned short *slid = reinterpret_cast<unsigned short *>(sin + CM_NL_MAX * NIN); // [ne][8]
+    unsigned short *sle = slid + 8 * HC;                                        // [8 ne]
+    unsigned short *sem = sle + 8 * HC;                                         // [ne]
+    unsigned short *slp = sem + HC;                                             // [nl + 1]
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(slp + CM_NL_MAX + 8);
+    const int c = blockIdx.x, tid = threadIdx.x;
+    const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, ne8 = (ne + 7) & ~7, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        const unsigned bg = 32u * nl, bl = 16u * ne8, be = 2u * ne8;
+        mbar_expect_tx(bar, bg + 2 * bl + be);
+        bulk_g2s(scx, a.CX + 4L * s0, bg, bar);
+        bulk_g2s(slid, a.lid + 8L * e0, bl, bar);
+        bulk_g2s(sle, a.lent + 8L * e0, bl, bar);
+        bulk_g2s(sem, a.emat + e0, be, bar);
+    }
+    for (int l = tid; l < nl; l += HK_NT) {
+        const long g = a.nodes[s0 + l];
+        if (KIND == EK_GRADU) {
+            sin[l] = a.in0[g];
+        } else {
+#pragma unroll
+            for (int d = 0; d < 3; d++) sin[NIN * l + d] = a.in0[3 * g + d];
+            if (KIND == EK_STRESS)
+#pragma unroll
+                for (int d = 0; d < 3; d++) sin[NIN * l + 3 + d] = a.in1[3 * g + d];
+        }
+    }
+    for (int l = tid; l <= nl; l += HK_NT) slp[l] = a.lptr[s0 + c + l];
+    __syncthreads();
+    mbar_wait(bar, 0);
+
+    // ---- phase 1: lane (cell, Gauss point)
+    double gsum[3] = {0, 0, 0};
+    for (int base = 0; base < 8 * ne; base += HK_NT) {
+        const int pair = base + tid, el = pair >> 3, p = pair & 7;
+        const bool active = pair < 8 * ne;
+        const unsigned mask = __ballot_sync(0xffffffffu, active);
+        if (!active) continue;
+        int l[8];
+        {
+            const uint4 q = *reinterpret_cast<const uint4 *>(slid + 8 * el);
+            l[0] = q.x & 0xffff; l[1] = q.x >> 16; l[2] = q.y & 0xffff; l[3] = q.y >> 16;
+            l[4] = q.z & 0xffff; l[5] = q.z >> 16; l[6] = q.w & 0xffff; l[7] = q.w >> 16;
+        }
+        double X[8][3], phid[8], gd[8][3];
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            const double2 q = *reinterpret_cast<const double2 *>(scx + 4 * l[k]);
+            X[k][0] = q.x; X[k][1] = q.y; X[k][2] = scx[4 * l[k] + 2];
+        }
+        const T det = (T)hex_point(X, p, phid, gd);
+        const unsigned em = sem[el];
+        T ph[8], w[NC], cc[8][NC], out[NC];
+#pragma unroll
+        for (int k = 0; k < 8; k++) ph[k] = (T)phid[k];
+        constexpr bool RANK1 = KIND == EK_GRADU || KIND == EK_STRESS;
+        if (KIND == EK_MS) {
+            T mt[3] = {0, 0, 0};
+#pragma unroll
+            for (int k = 0; k < 8; k++)
+#pragma unroll
+                for (int d = 0; d < 3; d++) mt[d] += ph[k] * sin[3 * l[k] + d];
+#pragma unroll
+            for (int d = 0; d < 3; d++) mt[d] -= (T)a.mbar[d];
+#pragma unroll
+            for (int k = 0; k < 8; k++) cc[k][0] = det * ((T)gd[k][0] * mt[0] + (T)gd[k][1] * mt[1] + (T)gd[k][2] * mt[2]);
+        } else if (KIND == EK_GRADU) {
+            T gU[3] = {0, 0, 0};
+#pragma unroll
+            for (int k = 0; k < 8; k++)
+#pragma unroll
+                for (int d = 0; d < 3; d++) gU[d] += sin[l[k]] * (T)gd[k][d];
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                w[d < NC ? d : 0] = det * gU[d];
+                gsum[d] += (double)(det * gU[d]);   // sum_a phi_a = 1: the cell's share of int grad U_h
+            }
+        } else {
+            T eps[6] = {0, 0, 0, 0, 0, 0}, sg[6] = {0, 0, 0, 0, 0, 0};
+            if (em & 1u) {
+#pragma unroll
+                for (int k = 0; k < 8; k++) {
+                    const T *wk = sin + NIN * l[k] + (KIND == EK_STRESS ? 3 : 0);
+                    const T mk[3] = {wk[0], wk[1], wk[2]};
+                    T ek[6];
+                    E0_sim(a.rot, mk, a.l1, a.l2, ek);
+#pragma unroll
+                    for (int q = 0; q < 6; q++) eps[q] += ph[k] * ek[q];
+                }
+                if (KIND == EK_STRESS) {
+                    T H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+                    for (int k = 0; k < 8; k++)
+#pragma unroll
+                        for (int x = 0; x < 3; x++)
+#pragma unroll
+                            for (int y = 0; y < 3; y++) H[x][y] += sin[NIN * l[k] + x] * (T)gd[k][y];
+                    const T E[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]};
+#pragma unroll
+                    for (int q = 0; q < 6; q++) eps[q] = E[q] - eps[q];
+                }
+                C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+            }
+            if (KIND == EK_MECH) {
+                if (a.has_sext)
+#pragma unroll
+                    for (int q = 0; q < 6; q++) sg[q] += a.sext[q];
+#pragma unroll
+                for (int k = 0; k < 8; k++) {
+                    const T gx = (T)gd[k][0], gy = (T)gd[k][1], gz = (T)gd[k][2];
+                    cc[k][0] = det * (sg[0] * gx + sg[5] * gy + sg[4] * gz);
+                    cc[k][1 < NC ? 1 : 0] = det * (sg[5] * gx + sg[1] * gy + sg[3] * gz);
+                    cc[k][2 < NC ? 2 : 0] = det * (sg[4] * gx + sg[3] * gy + sg[2] * gz);
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < NC; q++) w[q] = det * sg[q < 6 ? q : 0];
+            }
+        }
+        cell_exchange<T, NC, RANK1>(mask, p, ph, w, cc, out);
+#pragma unroll
+        for (int x = 0; x < NC; x++) scr[(NC * p + x) * HC + el] = out[x];
+    }
+    __syncthreads();
+
+    // ---- phase 2: one thread per local node, incidences in ascending cell order
+    for (int l = tid; l < nl; l += HK_NT) {
+        T acc[NC];
+#pragma unroll
+        for (int q = 0; q < NC; q++) acc[q] = 0;
+        for (int q = slp[l]; q < slp[l + 1]; q++) {
+            const int ent = sle[q], el = ent >> 3, k = ent & 7;
+#pragma unroll
+            for (int x = 0; x < NC; x++) acc[x] += scr[(NC * k + x) * HC + el];
+        }
+#pragma unroll
+        for (int x = 0; x < NC; x++) a.hpart[(long)(s0 + l) * NC + x] = acc[x];
+    }
+    if (KIND == EK_GRADU) block_reduce_write<3>(gsum, a.partial);
+}
+
+// plain hexahedral meshes: the element-centric chunk kernel; wrapped ones (no chunks): the node-centric kernel
 template <typename T, int KIND>
 static int launch_hex(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st, int *grid_out = nullptr)
 {
+    if (S->mesh->ck.nchunks > 0 && S->CX) {
+        constexpr size_t smem = hex_smem_bytes<KIND, T>();
+        CM_CUDA(cudaFuncSetAttribute(hex_chunk_kernel<T, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        hex_chunk_kernel<T, KIND><<<S->mesh->ck.nchunks, HK_NT, smem, st>>>(a);
+        if (grid_out) *grid_out = S->mesh->ck.nchunks;
+        return CM_OK;
+    }
     const int B = 128, grid = (int)((S->N + B - 1) / B);
     hex_node_kernel<T, KIND><<<grid, B, 0, st>>>(a);
     if (grid_out) *grid_out = grid;

@@ -61,6 +61,7 @@ struct Sell {
 //   ns_ptr / ns_slot   node -> its slots, ascending (so ascending chunk = ascending element order)
 constexpr int CM_EC_MAX = 768;
 constexpr int CM_NL_MAX = 384; // a full chunk of 768 Kuhn tets touches ~260 nodes
+constexpr int CM_HC_MAX = 128; // hexahedral cells per chunk (plain meshes; 8 threads per cell, one per Gauss point)
 struct Chunks {
     int nchunks = 0;
     long nslots = 0;
@@ -276,7 +277,7 @@ int mesh_build_host(cm_mesh *M, const double *xyz, long Ng, const int *gtets, lo
 int mesh_build_host_hex(cm_mesh *M, const double *xyz, long Ng, const int *ghexes, long Ne, const uchar *mag, const int *eid,
                         const int *dof, long N, cm_reorder reorder);
 int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &col, int C, Sell *out);
-int build_chunks(long N, long Ne, const int *tets, Chunks *out);
+int build_chunks(long N, long Ne, const int *conn, int nen, int ecmax, Chunks *out);
 
 // ---- kernels (templated launchers; defined in the .cu files, instantiated for float and double) ----
 template <typename T> int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, long pin_user, cudaStream_t st);

@@ -294,7 +294,7 @@ int mesh_build_host(cm_mesh *M, const double *gx, long Ng, const int *gtets, lon
     M->nnz = M->rowptr[N];
     if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
     if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
-    CM_TRY(build_chunks(N, Ne, M->tets.data(), &M->ck));
+    CM_TRY(build_chunks(N, Ne, M->tets.data(), 4, CM_EC_MAX, &M->ck));
     M->emat.resize(Ne);
     for (long e = 0; e < Ne; e++) {
         if (M->eid[e] < 0 || M->eid[e] > 0x7ffe) { cm_set_error("cm_mesh_create: elastic_id %d outside [0, 32766]", M->eid[e]); return CM_E_INDEX_RANGE; }
@@ -440,11 +440,16 @@ int mesh_build_host_hex(cm_mesh *M, const double *gx, long Ng, const int *ghexes
     M->nnz = M->rowptr[N];
     if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
     if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
-    // hexahedral element passes are node-centric: one slot per node (slot = node), no chunks
-    M->ck.nchunks = 0; M->ck.nslots = N;
-    M->ck.ns_ptr.resize(N + 1); M->ck.ns_slot.resize(N);
-    std::iota(M->ck.ns_ptr.begin(), M->ck.ns_ptr.end(), 0);
-    std::iota(M->ck.ns_slot.begin(), M->ck.ns_slot.end(), 0);
+    if (!M->wrapped) {
+        // element-centric passes: chunks of at most CM_HC_MAX cells, as for tetrahedra
+        CM_TRY(build_chunks(N, Ne, M->tets.data(), 8, CM_HC_MAX, &M->ck));
+    } else {
+        // wrapped (periodic) cells take their corners from their own images: node-centric passes, one slot per node
+        M->ck.nchunks = 0; M->ck.nslots = N;
+        M->ck.ns_ptr.resize(N + 1); M->ck.ns_slot.resize(N);
+        std::iota(M->ck.ns_ptr.begin(), M->ck.ns_ptr.end(), 0);
+        std::iota(M->ck.ns_slot.begin(), M->ck.ns_slot.end(), 0);
+    }
     return CM_OK;
 }
 
@@ -483,7 +488,7 @@ int build_sell(long N, const std::vector<int> &rowptr, const std::vector<int> &c
 // Element chunks (cm_internal.h): greedy cut of the element sequence, local numbering, per-chunk incidence lists and
 // the node -> slot transpose.  Elements are sorted by their smallest node id, so with a locality ordering a chunk
 // touches a compact node set (about 230 nodes per 768 elements on the paper's meshes).
-int build_chunks(long N, long Ne, const int *tets, Chunks *out)
+int build_chunks(long N, long Ne, const int *conn, int nen, int ecmax, Chunks *out)
 {
     Chunks &K = *out;
     K.eptr.assign(1, 0);
@@ -498,17 +503,17 @@ int build_chunks(long N, long Ne, const int *tets, Chunks *out)
     for (long g0 = 0; g0 < Ne; g0 += 8) {
         const long g1 = std::min(Ne, g0 + 8);
         grp.clear();
-        for (long q = 4 * g0; q < 4 * g1; q++)
-            if (stamp[tets[q]] != cur) grp.push_back(tets[q]);
+        for (long q = nen * g0; q < nen * g1; q++)
+            if (stamp[conn[q]] != cur) grp.push_back(conn[q]);
         std::sort(grp.begin(), grp.end());
         const int fresh = (int)(std::unique(grp.begin(), grp.end()) - grp.begin());
-        if (ne > 0 && (ne + 8 > CM_EC_MAX || nl + fresh > CM_NL_MAX)) {
+        if (ne > 0 && (ne + 8 > ecmax || nl + fresh > CM_NL_MAX)) {
             K.eptr.push_back((int)g0);
             K.nptr.push_back((int)K.nodes.size());
             cur++; ne = 0; nl = 0;
         }
-        for (long q = 4 * g0; q < 4 * g1; q++) {
-            const int v = tets[q];
+        for (long q = nen * g0; q < nen * g1; q++) {
+            const int v = conn[q];
             if (stamp[v] != cur) { stamp[v] = cur; K.nodes.push_back(v); nl++; }
         }
         ne += (int)(g1 - g0);
@@ -519,8 +524,8 @@ int build_chunks(long N, long Ne, const int *tets, Chunks *out)
     K.nslots = (long)K.nodes.size();
     if (K.nslots > 0x7fffffffL / 8) { cm_set_error("cm_mesh_create: too many chunk slots for 32-bit offsets"); return CM_E_BADARG; }
     // pass 2 (parallel over chunks): sort the local nodes, local ids, incidence runs
-    K.lid.resize(4 * Ne);
-    K.lent.resize(4 * Ne);
+    K.lid.resize((size_t)nen * Ne);
+    K.lent.resize((size_t)nen * Ne);
     K.lptr.assign(K.nslots + K.nchunks, 0);
 #pragma omp parallel
     {
@@ -531,16 +536,16 @@ int build_chunks(long N, long Ne, const int *tets, Chunks *out)
             int *nd = K.nodes.data() + s0;
             std::sort(nd, nd + n);
             cnt.assign(n + 1, 0);
-            for (long q = 4L * e0; q < 4L * (e0 + m); q++) {
-                const int l = (int)(std::lower_bound(nd, nd + n, tets[q]) - nd);
+            for (long q = (long)nen * e0; q < (long)nen * (e0 + m); q++) {
+                const int l = (int)(std::lower_bound(nd, nd + n, conn[q]) - nd);
                 K.lid[q] = (unsigned short)l;
                 cnt[l + 1]++;
             }
             for (int l = 0; l < n; l++) cnt[l + 1] += cnt[l];
             unsigned short *lp = K.lptr.data() + s0 + c;
             for (int l = 0; l <= n; l++) lp[l] = (unsigned short)cnt[l];
-            unsigned short *le = K.lent.data() + 4L * e0;
-            for (int q = 0; q < 4 * m; q++) le[cnt[K.lid[4L * e0 + q]]++] = (unsigned short)q; // q = 4 (e - e0) + k ascending
+            unsigned short *le = K.lent.data() + (long)nen * e0;
+            for (int q = 0; q < nen * m; q++) le[cnt[K.lid[(long)nen * e0 + q]]++] = (unsigned short)q; // q = nen (e - e0) + k ascending
         }
     }
     // pass 3: node -> slots, ascending
