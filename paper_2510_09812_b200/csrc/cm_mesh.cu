@@ -558,10 +558,11 @@ int build_chunks(long N, long Ne, const int *conn, int nen, int ecmax, Chunks *o
     return CM_OK;
 }
 
+// (256 bytes of slack: the bulk copies of a ragged last chunk read its arrays up to the next multiple of 8 elements)
 template <typename U>
 static int upload(U **dst, const std::vector<U> &src, cudaStream_t st)
 {
-    CM_CUDA(cudaMalloc((void **)dst, std::max<size_t>(src.size(), 1) * sizeof(U) + 64));
+    CM_CUDA(cudaMalloc((void **)dst, std::max<size_t>(src.size(), 1) * sizeof(U) + 256));
     CM_CUDA(cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(U), cudaMemcpyHostToDevice, st));
     return CM_OK;
 }
