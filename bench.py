@@ -308,9 +308,9 @@ def run_ours(args):
     per_class, ab = kernel_table(prof, args.steps, s)
     dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
     key = {"cg_mech": "bsr3", "cg_ms": "csr1", "cg_gs": "csr3"}[dom]
-    # DRAM bytes per matrix pass measured by `ncu --set full` (profiles/r01_f_cg_full.md: config 3, 21 passes per launch),
-    # EXTRAPOLATED to the average launch of this run, like `achieved`.  Only known for the captured workload.
-    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.906508e9 / 21, ("cg_ms", "f64"): 14.160628e9 / 21,
+    # DRAM bytes per matrix pass measured by `ncu --set full` (fp64: profiles/r02_cg_full.md, fp32: profiles/r01_f_cg_full.md; config 3,
+    # 21 passes per launch), EXTRAPOLATED to the average launch of this run, like `achieved`.  Only known for the captured workload.
+    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.973014e9 / 21, ("cg_ms", "f64"): 14.287394e9 / 21,
                           ("cg_mech", "f32"): 43.734836e9 / 21, ("cg_ms", "f32"): 7.856605e9 / 21}
     traffic = None
     passes_per_launch = prof[dom]["cg_matrix_passes"] / max(1, prof[dom]["launches"])
@@ -324,7 +324,7 @@ def run_ours(args):
             "bytes_r0_pass": ab["cg_r0_" + key], "matrix_passes_per_launch": passes_per_launch,
             "achieved_streamed": per_class.get(dom, {}).get("streamed_GBps"),
             "traffic_source": "extrapolated: ncu --set full dram__bytes_read+write per matrix pass of a 21-pass capture "
-                              "(profiles/r01_f_cg_full.md) x matrix passes per launch of this run"}
+                              "(profiles/r02_cg_full.md; fp32: profiles/r01_f_cg_full.md) x matrix passes per launch of this run"}
 
     launches = sum(p["launches"] for p in prof.values())
     last = infos[-1]
