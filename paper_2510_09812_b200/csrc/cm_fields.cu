@@ -158,11 +158,13 @@ struct ChunkArgs {
 //     planes [max(10, NOUT)][EC] T    staged geometry, overwritten in place by the contributions (fixed plane stride EC: the
 //                                     plane offsets are immediates)
 //   GEOM = true (geometry recomputed from the staged slot coordinates):
-//     scx    [CM_NL_MAX][4] double    nondimensional coordinates of the local nodes
+//     scx    [CM_NL_MAX][3] double    nondimensional coordinates of the local nodes (region sized for 4 words per node)
 //     planes [NOUT][EC] T             contributions
 //   sin    [CM_NL_MAX][NIN] T       nodal inputs
 //   slid   [EC] ushort4, sle [4 EC] ushort, sem [EC] ushort, slp [CM_NL_MAX + 8] ushort, mbarrier
-constexpr int nin_padded(int nin) { return nin; } // dense: a padded (power-of-two) node stride puts the random corner gathers on few banks (measured: S8 +17 %)
+// node stride of the staged inputs: dense.  Measured at 144^3: records padded to a power-of-two stride for 128-bit loads put the
+// random corner gathers on 2-4 bank groups (S8 +17 %); an odd stride of 7 words for the 6-word records of S8: no change (fp64), +3 % (fp32)
+constexpr int nin_padded(int nin) { return nin; }
 template <int KIND, bool GEOM> constexpr int chunk_planes() { return (GEOM || KindTraits<KIND>::NOUT > 10) ? KindTraits<KIND>::NOUT : 10; }
 template <int KIND, typename T, bool GEOM>
 constexpr size_t chunk_smem_bytes()
@@ -382,17 +384,21 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
     // ---- element data: bulk copies, all of the chunk's streaming bytes in flight at once
     if (tid == 0) {
         mbar_init(bar, 1);
-        const unsigned bg = GEOM ? 32u * nl : 10u * ne8 * (unsigned)sizeof(T), bl = 8u * ne8, be = 2u * ne8;
+        const unsigned bg = GEOM ? 0u : 10u * ne8 * (unsigned)sizeof(T), bl = 8u * ne8, be = 2u * ne8;
         mbar_expect_tx(bar, bg + 2 * bl + be);
-        if (GEOM) bulk_g2s(scx, a.CX + 4L * s0, bg, bar);
-        else
+        if (!GEOM)
             for (int q = 0; q < 10; q++) bulk_g2s(scr + q * EC, a.EG + 10L * e0 + (long)q * ne8, bg / 10, bar);
         bulk_g2s(slid, a.lid + 4L * e0, bl, bar);
         bulk_g2s(sle, a.lent + 4L * e0, bl, bar);
         bulk_g2s(sem, a.emat + e0, be, bar);
     }
-    // ---- phase 0: nodal inputs, incidence runs
+    // ---- phase 0: nodal inputs, incidence runs; slot coordinates at a dense 3-word stride (coalesced read of the 32-byte
+    // slot records; the dense stride spreads the corner gathers of phase 1 over all bank pairs, the records' own stride over 4)
     for (int l = tid; l < nl; l += EK_NT) {
+        if (GEOM) {
+            const double2 c0 = *reinterpret_cast<const double2 *>(a.CX + 4L * (s0 + l));
+            scx[3 * l] = c0.x; scx[3 * l + 1] = c0.y; scx[3 * l + 2] = a.CX[4L * (s0 + l) + 2];
+        }
         const long g = a.nodes[s0 + l];
         if (KIND == EK_GRADU) {
             sin[l] = a.in0[g];
@@ -422,8 +428,7 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
             double x[4][3];
 #pragma unroll
             for (int k = 0; k < 4; k++) {
-                const double2 p0 = *reinterpret_cast<const double2 *>(scx + 4 * l[k]);
-                x[k][0] = p0.x; x[k][1] = p0.y; x[k][2] = scx[4 * l[k] + 2];
+                x[k][0] = scx[3 * l[k]]; x[k][1] = scx[3 * l[k] + 1]; x[k][2] = scx[3 * l[k] + 2];
             }
             TetGeom G;
             tet_geometry_x(x, G);
