@@ -28,7 +28,11 @@
  * (tests/test_oracle_hysteresis.py: macrospin switching field), the rotated crystal frame
  * (tests/test_oracle_rotation.py: numpy tensor rotations, <111> modulus) and linear
  * hexahedra (tests/test_oracle_hex.py: 27-point stiffness and tensor-product mass in closed
- * form, exactness of the 2 x 2 x 2 rule, energy gradients).
+ * form, exactness of the 2 x 2 x 2 rule, energy gradients), Jacobi-preconditioned CG
+ * (tests/test_oracle_pcg.py: plain CG on the symmetrically scaled system iterate by iterate,
+ * dense solves, precond 0 bitwise the plain solver), the external stress
+ * (tests/test_oracle_sigma_ext.py: homogeneous Hooke state, energy stationarity, traction
+ * moment) and the row-length-sorted Morton order (tests/test_oracle_pins.py, brute force).
  * Unpinned: the choice between gspm_variant 0 and 1 (R1) -- "parity unpinned" between the
  * two readings; each is pinned by the invariants above.  The adjoint magnetostatic RHS
  * (R9) is pinned against the paper's literal form on periodic domains, where they agree.
