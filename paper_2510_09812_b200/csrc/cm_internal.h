@@ -179,8 +179,8 @@ struct System : SystemBase {
     // element geometry, chunk-blocked: chunk c owns 10 planes of ne8 = round_up(ne_c, 8) values at EG + 10 eptr[c]:
     // plane 0 = V_e, plane 3 (k - 1) + d + 1 = d-th component of grad phi_k, k = 1..3 (grad phi_0 = -sum, O-1)
     T *EG = nullptr;
-    // plain (not wrapped) tetrahedral meshes: nondimensional fp64 coordinates of every chunk slot, [slot][4] (x/l_d, y/l_d,
-    // z/l_d, 0): ONE bulk copy stages a chunk's coordinates and the element passes recompute V_e and grad phi from them
+    // plain (not wrapped) meshes: nondimensional fp64 coordinates of every chunk slot, [slot][4] (x/l_d, y/l_d,
+    // z/l_d, 0), contiguous per chunk: staged by one bulk copy (hexahedra) or one coalesced read (tetrahedra); the element passes recompute V_e and grad phi from them
     // (tet_geometry_x, the arithmetic that filled EG) instead of streaming ten stored words per element
     double *CX = nullptr;
     T *mL = nullptr, *mLm = nullptr;
