@@ -372,3 +372,26 @@ def test_mechanical_residual_curves_part_by_rounding(cm, oracle_mod, torch, caps
         with capsys.disabled():
             print(f"  first crossing of {tol:g}: oracle {io}, device {ig}")
         assert abs(io - ig) <= max(1, int(np.ceil(0.015 * io)))
+
+
+def test_round2_entry_points_refuse_bad_arguments(cm, torch):
+    mesh = inputs.hex_box((5, 5, 4), (12 * NM, 12 * NM, 9 * NM), seed_mesh=1, seed_perm=2)
+    gm = cm.Mesh(mesh.xyz, mesh.hexes)
+    gs = cm.System(gm, mat2(), 1e-12, "f64", inputs.clamp_bottom(mesh))
+    x = torch.zeros((mesh.n_nodes, 3), dtype=torch.float64, device="cuda")
+    for call in (lambda: gs.spmv_matfree(x), lambda: gs.cg_solve_matfree(x, x.clone()),          # tetrahedra only
+                 lambda: gs.set_option(cm.CM_OPT_STORED_GEOMETRY, 3), lambda: gs.set_option(99, 0),
+                 lambda: gs.gspm_step(cm.make_params(1e-12, terms=ALL, cg_precond=5), x, x[:, 0].contiguous(), x),
+                 lambda: gs.gspm_step(cm.make_params(1e-12, terms=ALL, mech_matfree=1), x, x[:, 0].contiguous(), x)):
+        with pytest.raises(cm.CmError) as e:
+            call()
+        assert e.value.code == cm.CM_E_BADARG
+    assert len(gs.cg_history()) == 0                      # nothing recorded unless enabled
+    tets = inputs.kuhn_box((4, 4, 4), (9 * NM,) * 3)
+    gt = cm.Mesh(tets.xyz, tets.tets)
+    g0 = cm.System(gt, inputs.Material(C_voigt=None), 1e-12)   # no elastic constants: no mechanical operator of either kind
+    y = torch.zeros((tets.n_nodes, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(cm.CmError):
+        g0.spmv_matfree(y)
+    with pytest.raises(cm.CmError):
+        g0.cg_solve(cm.CM_MAT_K_MECH, y, y.clone(), precond=cm.CM_PC_JACOBI)
