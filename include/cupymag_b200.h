@@ -14,8 +14,8 @@
  *    allocated inside cm_spmv / cm_cg_solve* / cm_field_rhs / cm_gspm_step.  Two calls may allocate:
  *    cm_hysteresis_run (a capture stream, the graph, logs grown to max_fields) and cm_volume_average
  *    (a library-order staging copy kept in the mesh, grown on demand).
- *  - Calls on one cm_system, and cm_volume_average calls on one cm_mesh, share scratch buffers: they
- *    must not run concurrently (one stream at a time per handle).
+ *  - Calls on one cm_system share its scratch buffers: they must not run concurrently (one stream at a
+ *    time per system).  cm_volume_average calls on one cm_mesh are serialised inside the library.
  *  - All field vectors are in USER node order, interleaved [node][component], of the
  *    system's dtype (double for CM_F64, float for CM_F32).  The locality reordering is
  *    internal; cm_mesh_get exposes it for bit-exact structure parity.

@@ -1787,6 +1787,7 @@ INST(float)
 template <typename T>
 int mesh_volume_average(cm_mesh *M, const T *g_user, int nc, double *out_host, cudaStream_t st)
 {
+    std::lock_guard<std::mutex> hold(M->avg_lock); // the mesh's scratch is shared by every system built on it
     const long n = M->N * nc;
     const T *g_lib = g_user;
     if (!M->identity) {

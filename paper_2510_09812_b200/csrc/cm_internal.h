@@ -4,6 +4,7 @@
 
 #include <cstdarg>
 #include <cstdio>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -98,7 +99,8 @@ struct cm_mesh {
     Chunks ck;
     std::vector<unsigned short> emat; // per element: elastic id << 1 | magnetic flag
     unsigned short *d_emat = nullptr;
-    // scratch for cm_volume_average
+    // scratch for cm_volume_average; calls on one mesh are serialised by avg_lock (they synchronise their stream before returning)
+    std::mutex avg_lock;
     double *d_red = nullptr;   // partials
     void *d_tmp = nullptr;     // library-order copy of the averaged field (grown on demand by cm_volume_average)
     long tmp_bytes = 0;
