@@ -183,10 +183,11 @@ constexpr int chunk_minb()
     const int n = (int)(cap / per), most = GEOM ? 3 : 4;
     return n < 1 ? 1 : (n > most ? most : n);
 }
-// Which passes recompute the geometry (measured on B200, 144^3 nodes, profiles/r02_elem_ab.txt): the passes are bound by
-// instruction issue at the occupancy their registers and planes allow (ncu: 37 % issue-active, 24 warps per SM), not by
-// DRAM, so trading ten streamed words per element for ~100 fp64 instructions pays only where the arithmetic is light:
-// fp64 S3 (0.43 -> 0.37 ms) and S5 (0.60 -> 0.52 ms).  fp64 S6 / S8 and every fp32 pass stream the stored geometry.
+// Which passes recompute the geometry (measured on B200, 144^3 nodes, profiles/r02_microbench_elem.txt): the passes are bound
+// by the LSU data pipe that serves shared memory (ncu: 80-88 % of its peak, profiles/r02_elem_ncu.md), not by DRAM, so
+// trading ten streamed words per element for twelve more shared-memory gathers and ~100 fp64 instructions pays only where
+// the rest of the pass is light: fp64 S3 (0.43 -> 0.36 ms) and S5 (0.61 -> 0.50 ms).  fp64 S6 / S8 and every fp32 pass
+// stream the stored geometry.
 template <int KIND, typename T>
 constexpr bool chunk_recompute() { return sizeof(T) == 8 && (KIND == EK_MS || KIND == EK_GRADU); }
 
