@@ -283,8 +283,10 @@ int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, const cm_hyst_
  * CM_OPT_STORED_GEOMETRY: how the element passes S3/S5/S6/S8 of a plain (not wrapped) tetrahedral mesh get V_e and grad phi.
  * 0: per pass, whichever kernel is faster -- the fp64 passes S3 and S5 recompute them in fp64 from the chunk's staged node
  * coordinates, the others stream the stored values (ten words per tetrahedron); 1: every pass streams; 2: every pass
- * recomputes.  All three give the same bits.  Other values: BADARG. */
-enum { CM_OPT_STORED_GEOMETRY = 0 };
+ * recomputes.  All three give the same bits.  Other values: BADARG.
+ * CM_OPT_NO_FUSED_S5S8: 1 = cm_gspm_step runs gradient recovery (S5) and the first stress recovery (S8) as separate element
+ * passes; by default, with DEMAG and MAGEL on a tetrahedral mesh, one pass computes both (same bits). */
+enum { CM_OPT_STORED_GEOMETRY = 0, CM_OPT_NO_FUSED_S5S8 = 1 };
 int cm_system_set_option(cm_system *sys, int option, int value);
 
 int cm_profile_enable(cm_system *sys, int on);

@@ -26,7 +26,7 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
  CM_GET_N2E) = range(9)
 CM_GET_LAYOUT = 9
 CM_PC_NONE, CM_PC_JACOBI = 0, 1
-CM_OPT_STORED_GEOMETRY = 0
+CM_OPT_STORED_GEOMETRY, CM_OPT_NO_FUSED_S5S8 = 0, 1
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 

@@ -450,6 +450,10 @@ extern "C" int cm_system_set_option(cm_system *sys, int option, int value)
         if (value < 0 || value > 2) break;
         sys->impl->geometry_mode = value;
         return CM_OK;
+    case CM_OPT_NO_FUSED_S5S8:
+        if (value < 0 || value > 1) break;
+        sys->impl->no_fuse = value != 0;
+        return CM_OK;
     }
     cm_set_error("cm_system_set_option: unknown option %d or value %d out of range", option, value);
     return CM_E_BADARG;

@@ -457,7 +457,7 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
     T **vecs4[] = {&S->p, &S->p2, &S->f, &S->xin}; // padded [node][4] when they hold a 3-vector that a product gathers
     for (T **v : vecs4) CM_TRY(alloc(v, 4 * N));
     CM_TRY(alloc(&S->U, N)); CM_TRY(alloc(&S->stg_U, N)); CM_TRY(alloc(&S->sig, 6 * N));
-    CM_TRY(alloc(&S->hpart, (size_t)6 * M->ck.nslots));
+    CM_TRY(alloc(&S->hpart, (size_t)9 * M->ck.nslots));
     S->grid_cap = S->num_sms * 8;
     CM_TRY(alloc(&S->partial, (size_t)5 * S->grid_cap * 3));
     CM_TRY(alloc(&S->d_hist, (size_t)CM_HIST_CAP));

@@ -114,7 +114,7 @@ __global__ void permute_out_kernel(long N, int nc, const int *__restrict__ order
 // node: sums the node's incidences inside the chunk in ascending element order and writes ONE partial per slot.  A
 // node pass then adds a node's slots in ascending chunk order -- a deterministic gather end to end, no float
 // atomics, and no per-element scratch in HBM.
-enum ElemKind { EK_MS = 0, EK_GRADU = 1, EK_MECH = 2, EK_STRESS = 3, EK_KMECH = 4 };
+enum ElemKind { EK_MS = 0, EK_GRADU = 1, EK_MECH = 2, EK_STRESS = 3, EK_KMECH = 4, EK_GRADU_STRESS = 5 };
 // NIN staged words per node, NOUT shared-memory words per element, NC words per slot, PERK: contribution depends on
 // the local node index k (NOUT = 4 NC) or is the same for the 4 nodes (NOUT = NC).
 template <int KIND> struct KindTraits;
@@ -122,6 +122,9 @@ template <> struct KindTraits<EK_MS> { static constexpr int NIN = 3, NOUT = 4, N
 template <> struct KindTraits<EK_GRADU> { static constexpr int NIN = 1, NOUT = 3, NC = 3; static constexpr bool PERK = false; };
 template <> struct KindTraits<EK_MECH> { static constexpr int NIN = 3, NOUT = 12, NC = 3; static constexpr bool PERK = true; };
 template <> struct KindTraits<EK_STRESS> { static constexpr int NIN = 6, NOUT = 6, NC = 6; static constexpr bool PERK = false; };
+// S5 and S8 of the same state in ONE pass (both follow the two solves of a step and read the same geometry, ids and
+// incidences): in U, u, w; out V_e grad U_e (3) and V_e C*_e : (E_e(u) - mean_e E0(w)) (6) per slot
+template <> struct KindTraits<EK_GRADU_STRESS> { static constexpr int NIN = 7, NOUT = 9, NC = 9; static constexpr bool PERK = false; };
 // matrix-free K^mech x (Eq. 12): in x (projected: clamped DOFs read as 0), out sum_e V_e B_k^T C_e B x per slot
 template <> struct KindTraits<EK_KMECH> { static constexpr int NIN = 3, NOUT = 12, NC = 3; static constexpr bool PERK = true; };
 
@@ -140,7 +143,8 @@ struct ChunkArgs {
     const unsigned short *lid, *lptr, *lent, *emat;
     const T *EG;          // chunk-blocked geometry, 10 planes per chunk (cm_internal.h)
     const double *CX;     // slot coordinates [slot][4] (GEOM kernels: geometry recomputed, EG not read)
-    const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w
+    const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w;  GRADU_STRESS: u, w and U in in2
+    const T *in2;
     const uchar *clamp;   // KMECH: clamped DOFs of the input read as zero (the projection P of P A P + (I - P))
     const int *skip;      // KMECH inside CG: the solve has finished, the launch is a no-op
     const double *mbar;   // MS
@@ -406,6 +410,10 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
         } else if (KIND == EK_KMECH) {
 #pragma unroll
             for (int d = 0; d < 3; d++) sin[NINP * l + d] = a.clamp[3 * g + d] ? (T)0 : a.in0[3 * g + d];
+        } else if (KIND == EK_GRADU_STRESS) {
+            sin[NINP * l] = a.in2[g];
+#pragma unroll
+            for (int d = 0; d < 3; d++) { sin[NINP * l + 1 + d] = a.in0[3 * g + d]; sin[NINP * l + 4 + d] = a.in1[3 * g + d]; }
         } else {
 #pragma unroll
             for (int d = 0; d < 3; d++) sin[NINP * l + d] = a.in0[3 * g + d];
@@ -464,6 +472,30 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
                 const T gU = u0 * g[0][d] + u1 * g[1][d] + u2 * g[2][d] + u3 * g[3][d];
                 scr[d * EC + el] = V * gU;
                 gsum[d] += (double)V * (double)gU;
+            }
+        } else if (KIND == EK_GRADU_STRESS) {
+            const T u0 = sin[NINP * l[0]], u1 = sin[NINP * l[1]], u2 = sin[NINP * l[2]], u3 = sin[NINP * l[3]];
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                const T gU = u0 * g[0][d] + u1 * g[1][d] + u2 * g[2][d] + u3 * g[3][d];
+                scr[d * EC + el] = V * gU;
+                gsum[d] += (double)V * (double)gU;
+            }
+            const unsigned em = sem[el];
+            if (!(em & 1u)) {
+#pragma unroll
+                for (int q = 0; q < 6; q++) scr[(3 + q) * EC + el] = 0;
+            } else {
+                T H[3][3];
+                strain_H<T, NINP>(sin + 1, l, g, H);
+                T eps[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]}, e0v[6], sg[6];
+                mean_E0<T, NINP, 4>(a.rot, sin, l, a.l1, a.l2, e0v);
+#pragma unroll
+                for (int q = 0; q < 6; q++) eps[q] -= e0v[q];
+                if (CUBIC) C_times_cubic(a.Cstar + 12 * (em >> 1), eps, sg);
+                else C_times(a.Cstar + 36 * (em >> 1), eps, sg);
+#pragma unroll
+                for (int q = 0; q < 6; q++) scr[(3 + q) * EC + el] = V * sg[q];
             }
         } else if (KIND == EK_KMECH) {
             // sigma = C*_e : E_e(x), H[a][b] = d_b x_a;  c_(k,a) = V_e (sigma grad phi_k)_a   (every element is elastic)
@@ -532,7 +564,7 @@ __global__ void __launch_bounds__(EK_NT, (chunk_minb<KIND, T, GEOM>())) elem_chu
 #pragma unroll
         for (int x = 0; x < NC; x++) a.hpart[(long)(s0 + l) * NC + x] = acc[x];
     }
-    if (KIND == EK_GRADU) block_reduce_write<3>(gsum, a.partial);
+    if (KIND == EK_GRADU || KIND == EK_GRADU_STRESS) block_reduce_write<3>(gsum, a.partial);
 }
 
 // node pass: b_i = sum of the node's slot partials (ascending chunk order); zero where the mask says so
@@ -563,7 +595,8 @@ template <typename T>
 __global__ void node_hd_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                const T *__restrict__ mL, const double *__restrict__ scal /* mbar[0..2], gradU mean[3..5] */,
                                unsigned terms, double n00, double n01, double n02, double n10, double n11,
-                               double n12, double n20, double n21, double n22, T dscale /* 4: tets (V_e / 4 weights), 1: hexahedra */, T *hd)
+                               double n12, double n20, double n21, double n22, T dscale /* 4: tets (V_e / 4 weights), 1: hexahedra */,
+                               int hs /* words per slot in hpart */, T *hd)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -573,7 +606,7 @@ __global__ void node_hd_kernel(long N, const int *__restrict__ ns_ptr, const int
         for (int s = ns_ptr[i]; s < ns_ptr[i + 1]; s++) {
             const long q = __ldg(ns_slot + s);
 #pragma unroll
-            for (int d = 0; d < 3; d++) acc[d] += hpart[3 * q + d];
+            for (int d = 0; d < 3; d++) acc[d] += hpart[hs * q + d];
         }
         const T den = dscale * mL[i];
 #pragma unroll
@@ -595,7 +628,7 @@ template <typename T>
 __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const int *__restrict__ ns_slot, const T *__restrict__ hpart,
                                   const T *__restrict__ mLm, const uchar *__restrict__ live, const T *__restrict__ w,
                                   const T *__restrict__ hd, unsigned terms, T Kstar2, T hx, T hy, T hz, const double *__restrict__ hext_dev,
-                                  T l1, T l2, Rot<T> rot, T dscale, T *h, T *sig_out)
+                                  T l1, T l2, Rot<T> rot, T dscale, int hs /* words per slot in hpart */, T *h, T *sig_out)
 {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -615,7 +648,7 @@ __global__ void node_field_kernel(long N, const int *__restrict__ ns_ptr, const 
             for (int q = ns_ptr[i]; q < ns_ptr[i + 1]; q++) {
                 const long sl = __ldg(ns_slot + q);
 #pragma unroll
-                for (int c = 0; c < 6; c++) s[c] += hpart[6 * sl + c];
+                for (int c = 0; c < 6; c++) s[c] += hpart[hs * sl + c];
             }
             const T den = dscale * mLm[i];
 #pragma unroll
@@ -772,7 +805,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
     a.emat = M->d_emat; a.EG = S->EG; a.CX = S->CX;
     a.hexes = M->d_tets; a.ghexes = M->d_gtets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_gxyz; a.ld = S->ld; a.N = S->N;
-    a.in0 = nullptr; a.in1 = nullptr; a.clamp = S->clamp; a.skip = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
+    a.in0 = nullptr; a.in1 = nullptr; a.in2 = nullptr; a.clamp = S->clamp; a.skip = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
     for (int q = 0; q < 6; q++) a.sext[q] = (T)S->sext[q];
     a.has_sext = S->has_sext ? 1 : 0;
@@ -795,7 +828,7 @@ static int launch_chunk_kernel(System<T> *S, const ChunkArgs<T> &a, cudaStream_t
 template <typename T, int KIND>
 static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
 {
-    constexpr bool USES_C = KIND == EK_MECH || KIND == EK_STRESS || KIND == EK_KMECH;
+    constexpr bool USES_C = KIND == EK_MECH || KIND == EK_STRESS || KIND == EK_KMECH || KIND == EK_GRADU_STRESS;
     const bool geom = S->CX != nullptr && (S->geometry_mode == 2 || (S->geometry_mode == 0 && chunk_recompute<KIND, T>()));
     if (USES_C && S->cubic_pattern) {
         ChunkArgs<T> b = a;
@@ -1132,24 +1165,49 @@ int sys_rhs_ms(System<T> *S, const T *m_lib, T *b, cudaStream_t st)
     return CM_OK;
 }
 
+// node pass of S5 (and the mean of grad U) from slot partials of `hs` words per slot; nparts per-block sums of V grad U in S->red
+template <typename T>
+static int demag_node_pass(System<T> *S, unsigned terms, int nparts, int hs, T *hd, cudaStream_t st)
+{
+    const Chunks &K = S->mesh->ck;
+    if (terms & CM_TERM_DEMAG) reduce_final_kernel<<<1, 1024, 0, st>>>(nparts, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
+    const double *n = S->Nd;
+    node_hd_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mL, S->dscal, terms, n[0], n[1], n[2], n[3],
+                                                 n[4], n[5], n[6], n[7], n[8], (T)(S->mesh->nen == 8 ? 1 : 4), hs, hd);
+    return CM_OK;
+}
+
 template <typename T>
 int sys_demag_field(System<T> *S, const T *U_lib, unsigned terms, T *hd, cudaStream_t st)
 {
     const Chunks &K = S->mesh->ck;
     S->prof.begin(CM_PROF_ELEMENT, st, (terms & CM_TERM_DEMAG) ? 3 : 1);
+    int nparts = K.nchunks;
     if (terms & CM_TERM_DEMAG) {
         ChunkArgs<T> a = chunk_args(S);
         a.in0 = U_lib;
-        int nparts = K.nchunks;
         if (S->mesh->nen == 8) CM_TRY((launch_hex<T, EK_GRADU>(S, a, st, &nparts)));
         else CM_TRY((launch_chunks<T, EK_GRADU>(S, a, st)));
-        reduce_final_kernel<<<1, 1024, 0, st>>>(nparts, 3, S->red, 1.0 / S->Vtot, S->dscal + 3);
     }
-    const double *n = S->Nd;
-    node_hd_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mL, S->dscal, terms, n[0], n[1], n[2], n[3],
-                                                 n[4], n[5], n[6], n[7], n[8], (T)(S->mesh->nen == 8 ? 1 : 4), hd);
+    CM_TRY(demag_node_pass(S, terms, nparts, 3, hd, st));
     S->prof.end(st);
     LAUNCH_CHECK();
+    return CM_OK;
+}
+
+// S5 and S8 of the state (U, u, w) in one element pass (tetrahedra): h_d into hd, the stress partials stay in S->hpart
+// (9 words per slot, the stress in words 3..8) for the sys_field call that follows
+template <typename T>
+int sys_demag_stress(System<T> *S, const T *U_lib, const T *u_lib, const T *w_lib, unsigned terms, T *hd, cudaStream_t st)
+{
+    ChunkArgs<T> a = chunk_args(S);
+    a.in0 = u_lib; a.in1 = w_lib; a.in2 = U_lib;
+    S->prof.begin(CM_PROF_ELEMENT, st, 3);
+    CM_TRY((launch_chunks<T, EK_GRADU_STRESS>(S, a, st)));
+    CM_TRY(demag_node_pass(S, terms, S->mesh->ck.nchunks, 9, hd, st));
+    S->prof.end(st);
+    LAUNCH_CHECK();
+    S->sig_hs = 9; S->sig_ho = 3;
     return CM_OK;
 }
 
@@ -1180,6 +1238,7 @@ int sys_stress(System<T> *S, const T *u_lib, const T *w_lib, cudaStream_t st)
     else CM_TRY((launch_chunks<T, EK_STRESS>(S, a, st)));
     S->prof.end(st);
     LAUNCH_CHECK();
+    S->sig_hs = 6; S->sig_ho = 0;
     return CM_OK;
 }
 
@@ -1189,9 +1248,9 @@ int sys_field(System<T> *S, const T *w_lib, const T *hd, const double hext[3], u
 {
     const Chunks &K = S->mesh->ck;
     S->prof.begin(CM_PROF_ELEMENT, st);
-    node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart, S->mLm, S->live, w_lib, hd, terms,
+    node_field_kernel<T><<<nblk(S->N), BS, 0, st>>>(S->N, K.d_ns_ptr, K.d_ns_slot, S->hpart + S->sig_ho, S->mLm, S->live, w_lib, hd, terms,
                                                    (T)(2.0 * S->Kstar), (T)hext[0], (T)hext[1], (T)hext[2], hext_dev, (T)S->lam100,
-                                                   (T)S->lam111, make_rot<T>(S), (T)(S->mesh->nen == 8 ? 1 : 4), h, sig_out);
+                                                   (T)S->lam111, make_rot<T>(S), (T)(S->mesh->nen == 8 ? 1 : 4), S->sig_hs, h, sig_out);
     S->prof.end(st);
     LAUNCH_CHECK();
     return CM_OK;
@@ -1245,14 +1304,16 @@ static int step_core(System<T> *S, const cm_step_params *p, const double *hext_d
         CM_TRY(sys_rhs_ms(S, S->m, S->bvec, st));
         CM_TRY(sys_cg(S, CM_MAT_K_MS, MODE_CSR1, S->bvec, S->U, tol, mx, fx, 1u, 0, CM_PROF_CG_MS, pc, st));
     }
-    // 3. demagnetising field (Eq. 4)
-    if (terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) CM_TRY(sys_demag_field(S, S->U, terms, S->hd, st));
+    // 3. demagnetising field (Eq. 4); with mechanics on a tetrahedral mesh S5 waits for S8 and shares its element pass
+    const bool fuse = (terms & CM_TERM_DEMAG) && (terms & CM_TERM_MAGEL) && S->mesh->nen == 4 && !S->no_fuse;
+    if ((terms & (CM_TERM_DEMAG | CM_TERM_FARFIELD)) && !fuse) CM_TRY(sys_demag_field(S, S->U, terms, S->hd, st));
     // 4. mechanical equilibrium (Eq. 6, 10), warm start; stress at m^n
     if (terms & CM_TERM_MAGEL) {
         CM_TRY(sys_rhs_mech(S, S->m, S->bvec, st));
         if (p->mech_matfree) CM_TRY(sys_cg_matfree(S, S->bvec, S->u, tol, mx, fx, pc, 1, st));
         else CM_TRY(sys_cg(S, CM_MAT_K_MECH, MODE_BSR3, S->bvec, S->u, tol, mx, fx, 1u, 1, CM_PROF_CG_MECH, pc, st));
-        CM_TRY(sys_stress(S, S->u, S->m, st));
+        if (fuse) CM_TRY(sys_demag_stress(S, S->U, S->u, S->m, terms, S->hd, st));
+        else CM_TRY(sys_stress(S, S->u, S->m, st));
     }
     // 5. h[m^n];  6. Step 1: g^n.  A Helmholtz solve is ONE launch: b = M_m f, x0 = f, r0 = b - A f in its first pass
     CM_TRY(sys_field(S, S->m, S->hd, hext, terms, S->hn, (T *)nullptr, st, hext_dev));

@@ -158,6 +158,8 @@ struct SystemBase {
     int pin = 0; // library index
     int num_sms = 0;
     Profiler prof;
+    bool no_fuse = false;  // CM_OPT_NO_FUSED_S5S8: the step runs S5 and S8 as separate element passes (A/B measurement)
+    int sig_hs = 6, sig_ho = 0; // where the stress partials of the last stress pass sit in hpart: words per slot, first word
     int geometry_mode = 0; // CM_OPT_STORED_GEOMETRY: 0 per-pass choice, 1 every pass streams the stored geometry, 2 every pass recomputes it
     double *d_hist = nullptr;  // residual history of the last solve (cm_cg_history), CM_HIST_CAP doubles
     bool hist_on = false;
