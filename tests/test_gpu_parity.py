@@ -534,3 +534,25 @@ def test_profile_counters(case, cm):
     assert prof["spmv"]["launches"] == 1 and prof["spmv"]["ms"] > 0
     assert prof["cg_gs"]["launches"] == 1 and prof["cg_gs"]["cg_iters"] == it and prof["cg_gs"]["ms"] > 0
     gs.profile_enable(False)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_fused_and_separate_recovery_passes_give_the_same_bits(cm, torch, dtype):
+    """Inside a step with DEMAG and MAGEL, gradient recovery (S5) and the first stress recovery (S8) share one element pass
+    (default) or run separately (CM_OPT_NO_FUSED_S5S8): the same sums in the same order, so the same bits after three steps."""
+    mesh = inputs.kuhn_box((13, 12, 9), (40 * NM, 36 * NM, 26 * NM), seed_mesh=21, seed_perm=22)
+    mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * NM,) * 3)
+    gm = cm.Mesh(mesh.xyz, mesh.tets, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+    gs = cm.System(gm, mat2(), 1e-12, dtype, inputs.clamp_bottom(mesh))
+    td = torch.float64 if dtype == "f64" else torch.float32
+    out = []
+    for nofuse in (0, 1):
+        gs.set_option(cm.CM_OPT_NO_FUSED_S5S8, nofuse)
+        m = torch.as_tensor(inputs.init_m_noisy_x(mesh, 23), dtype=td, device="cuda").contiguous()
+        U = torch.zeros(mesh.n_nodes, dtype=td, device="cuda"); u = torch.zeros((mesh.n_nodes, 3), dtype=td, device="cuda")
+        for k in range(3):
+            info, rc = gs.gspm_step(cm.make_params(1e-12, [2e4, 1e4, 0], ALL, 0, 1e-8), m, U, u)
+            assert rc == 0
+        out.append((m, U, u))
+    for a, b in zip(*out):
+        assert torch.equal(a, b)
