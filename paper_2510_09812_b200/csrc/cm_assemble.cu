@@ -20,7 +20,16 @@ __device__ __forceinline__ void tet_geometry(const double *__restrict__ xyz, con
     tet_geometry_x(x, G);
 }
 
-// nondimensional coordinates of every chunk slot, [slot][4] (System::CX)
+// nondimensional corner coordinates of every hexahedral cell, [cell][8][3] (System::CX on hexahedral meshes)
+__global__ void cell_xyz_kernel(long ncorners, const int *__restrict__ gconn, const double *__restrict__ gxyz, double ld, double *CX)
+{
+    const long q = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (q >= ncorners) return;
+    const long i = gconn[q];
+    CX[3 * q] = gxyz[3 * i] / ld; CX[3 * q + 1] = gxyz[3 * i + 1] / ld; CX[3 * q + 2] = gxyz[3 * i + 2] / ld;
+}
+
+// nondimensional coordinates of every chunk slot, [slot][4] (System::CX on tetrahedral meshes)
 __global__ void slot_xyz_kernel(long nslots, const int *__restrict__ nodes, const double *__restrict__ xyz, double ld, double *CX)
 {
     const long s = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -420,10 +429,9 @@ int sys_assemble(System<T> *S, const cm_material *mat, const uchar *clamp_user, 
         S->Vtot = hv[0]; S->Vmag = hv[1];
     } else {
         S->Vtot = M->vtot_m3 / (ld * ld * ld); S->Vmag = M->vmag_m3 / (ld * ld * ld);
-        if (!M->wrapped) {
-            CM_TRY(alloc(&S->CX, (size_t)4 * M->ck.nslots + 8));
-            slot_xyz_kernel<<<(unsigned)((M->ck.nslots + B - 1) / B), B, 0, st>>>(M->ck.nslots, M->ck.d_nodes, M->d_xyz, ld, S->CX);
-        }
+        // corner coordinates per CELL (a wrapped cell takes them from its own images): [cell][8][3]
+        CM_TRY(alloc(&S->CX, (size_t)24 * Ne + 32));
+        cell_xyz_kernel<<<(unsigned)((8 * Ne + B - 1) / B), B, 0, st>>>(8 * Ne, M->d_gtets, M->d_gxyz, ld, S->CX);
     }
     // matrices: fp64 scratch on the pattern
     double *&K = scr.K, *&Km = scr.Km, *&Mm = scr.Mm, *&Kme = scr.Kme;

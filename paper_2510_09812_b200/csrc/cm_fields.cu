@@ -136,13 +136,10 @@ constexpr int EK_NT = CM_EK_NT;
 template <typename T>
 struct ChunkArgs {
     const int *eptr, *nptr, *nodes;
-    const int *hexes, *ghexes, *n2e_ptr, *n2e; // hexahedral meshes (node-centric passes): DOF / geometric connectivity, node -> (element * 8 + corner)
-    const double *xyz;                // coordinates of the geometric nodes, metres
-    double ld;
     long N;
     const unsigned short *lid, *lptr, *lent, *emat;
     const T *EG;          // chunk-blocked geometry, 10 planes per chunk (cm_internal.h)
-    const double *CX;     // slot coordinates [slot][4] (GEOM kernels: geometry recomputed, EG not read)
+    const double *CX;     // tetrahedra: slot coordinates [slot][4] (GEOM kernels: geometry recomputed, EG not read); hexahedra: [cell][8][3]
     const T *in0, *in1;   // MS, MECH: m;  GRADU: U;  STRESS: u, w;  GRADU_STRESS: u, w and U in in2
     const T *in2;
     const uchar *clamp;   // KMECH: clamped DOFs of the input read as zero (the projection P of P A P + (I - P))
@@ -804,7 +801,7 @@ static ChunkArgs<T> chunk_args(System<T> *S)
     ChunkArgs<T> a;
     a.eptr = K.d_eptr; a.nptr = K.d_nptr; a.nodes = K.d_nodes; a.lid = K.d_lid; a.lptr = K.d_lptr; a.lent = K.d_lent;
     a.emat = M->d_emat; a.EG = S->EG; a.CX = S->CX;
-    a.hexes = M->d_tets; a.ghexes = M->d_gtets; a.n2e_ptr = M->d_n2e_ptr; a.n2e = M->d_n2e; a.xyz = M->d_gxyz; a.ld = S->ld; a.N = S->N;
+    a.N = S->N;
     a.in0 = nullptr; a.in1 = nullptr; a.in2 = nullptr; a.clamp = S->clamp; a.skip = nullptr; a.mbar = S->dscal; a.Cstar = S->Cstar; a.l1 = (T)S->lam100; a.l2 = (T)S->lam111;
     a.rot = make_rot<T>(S);
     for (int q = 0; q < 6; q++) a.sext[q] = (T)S->sext[q];
@@ -839,114 +836,14 @@ static int launch_chunks(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st)
 }
 
 // ---------------------------------------------------------------- element passes on linear hexahedra (R26)
-// Node-centric: one thread per node i walks its incident cells (ascending) and their 2 x 2 x 2 Gauss points (ascending),
-// recomputes the fp64 geometry from the corner coordinates and accumulates node i's own entry -- a deterministic gather
-// with no scatter at all.  The numerators land in hpart[slot = node]; the tetrahedral node passes finish them
-// (dscale = 1).  Hexahedral cells carry ~8x the arithmetic of a tetrahedron per byte, so these passes are bound by
-// fp64 throughput, not by HBM; they are < 1 % of a step.
-template <typename T, int KIND>
-__global__ void __launch_bounds__(128) hex_node_kernel(ChunkArgs<T> a)
-{
-    typedef KindTraits<KIND> K;
-    constexpr int NC = K::NC;
-    const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    T acc[NC];
-#pragma unroll
-    for (int q = 0; q < NC; q++) acc[q] = 0;
-    const double ild = 1.0 / a.ld;
-    if (i < a.N) {
-        for (int s = a.n2e_ptr[i]; s < a.n2e_ptr[i + 1]; s++) {
-            const int e = a.n2e[s] >> 3, k = a.n2e[s] & 7;
-            const unsigned em = a.emat[e];
-            if ((KIND == EK_MECH || KIND == EK_STRESS) && !(em & 1u) && !(KIND == EK_MECH && a.has_sext)) continue;
-            int t[8];
-            double X[8][3];
-#pragma unroll
-            for (int c = 0; c < 8; c++) {
-                t[c] = a.hexes[8 * (long)e + c];
-                const long gc = a.ghexes[8 * (long)e + c];
-#pragma unroll
-                for (int d = 0; d < 3; d++) X[c][d] = a.xyz[3 * gc + d] * ild;
-            }
-            T e0c[8][6]; // E0 at the 8 corners (MECH, STRESS)
-            if ((KIND == EK_MECH || KIND == EK_STRESS) && (em & 1u)) {
-                const T *w = KIND == EK_MECH ? a.in0 : a.in1;
-                for (int c = 0; c < 8; c++) {
-                    const T mk[3] = {w[3 * (long)t[c]], w[3 * (long)t[c] + 1], w[3 * (long)t[c] + 2]};
-                    E0_sim(a.rot, mk, a.l1, a.l2, e0c[c]);
-                }
-            }
-            for (int p = 0; p < 8; p++) {
-                double phid[8], gd[8][3];
-                const T det = (T)hex_point(X, p, phid, gd);
-                if (KIND == EK_MS) {
-                    T mt[3] = {0, 0, 0};
-                    for (int c = 0; c < 8; c++)
-#pragma unroll
-                        for (int d = 0; d < 3; d++) mt[d] += (T)phid[c] * a.in0[3 * (long)t[c] + d];
-#pragma unroll
-                    for (int d = 0; d < 3; d++) mt[d] -= (T)a.mbar[d];
-                    acc[0] += det * ((T)gd[k][0] * mt[0] + (T)gd[k][1] * mt[1] + (T)gd[k][2] * mt[2]);
-                } else if (KIND == EK_GRADU) {
-                    T gU[3] = {0, 0, 0};
-                    for (int c = 0; c < 8; c++)
-#pragma unroll
-                        for (int d = 0; d < 3; d++) gU[d] += a.in0[t[c]] * (T)gd[c][d];
-#pragma unroll
-                    for (int d = 0; d < 3; d++) acc[d] += det * (T)phid[k] * gU[d];
-                } else {
-                    T eps[6] = {0, 0, 0, 0, 0, 0}, sg[6];
-                    if (em & 1u)
-                        for (int c = 0; c < 8; c++)
-#pragma unroll
-                            for (int q = 0; q < 6; q++) eps[q] += (T)phid[c] * e0c[c][q];
-                    if (KIND == EK_STRESS) {
-                        T H[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
-                        for (int c = 0; c < 8; c++)
-#pragma unroll
-                            for (int x = 0; x < 3; x++)
-#pragma unroll
-                                for (int y = 0; y < 3; y++) H[x][y] += a.in0[3 * (long)t[c] + x] * (T)gd[c][y];
-                        const T E[6] = {H[0][0], H[1][1], H[2][2], H[1][2] + H[2][1], H[0][2] + H[2][0], H[0][1] + H[1][0]};
-#pragma unroll
-                        for (int q = 0; q < 6; q++) eps[q] = E[q] - eps[q];
-                    }
-                    if (em & 1u) C_times(a.Cstar + 36 * (em >> 1), eps, sg);
-                    else
-#pragma unroll
-                        for (int q = 0; q < 6; q++) sg[q] = 0;
-                    if (KIND == EK_MECH) {
-                        if (a.has_sext)
-#pragma unroll
-                            for (int q = 0; q < 6; q++) sg[q] += a.sext[q];
-                        const T gx = (T)gd[k][0], gy = (T)gd[k][1], gz = (T)gd[k][2];
-                        acc[0] += det * (sg[0] * gx + sg[5] * gy + sg[4] * gz);
-                        acc[1] += det * (sg[5] * gx + sg[1] * gy + sg[3] * gz);
-                        acc[NC > 2 ? 2 : 0] += det * (sg[4] * gx + sg[3] * gy + sg[2] * gz);
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < NC; q++) acc[q] += det * (T)phid[k] * sg[q < 6 ? q : 0];
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < NC; q++) a.hpart[i * NC + q] = acc[q];
-    }
-    if (KIND == EK_GRADU) { // sum_i int phi_i grad U_h = int grad U_h (the shape functions sum to one): <grad U> V
-        double gs[3] = {0, 0, 0};
-        if (i < a.N)
-            for (int d = 0; d < 3; d++) gs[d] = (double)acc[d < NC ? d : 0];
-        block_reduce_write<3>(gs, a.partial);
-    }
-}
-
-// ---- element-centric passes on plain (not wrapped) hexahedral meshes: one CTA per chunk of at most CM_HC_MAX cells, EIGHT
-// lanes per cell, one per Gauss point.  A lane recomputes the fp64 geometry at its point from the chunk's staged slot
-// coordinates, evaluates the integrand there and its contribution to the cell's eight corners; a three-step exchange
+// Element-centric: one CTA per chunk of at most CM_HC_MAX cells, EIGHT lanes per cell, one per Gauss point.  A lane recomputes
+// the fp64 geometry at its point from the cell's own corner coordinates (staged per cell, 24 words: a wrapped -- periodic --
+// cell takes its corners from its own images, so coordinates cannot be shared per node, R23), evaluates the
+// integrand there and its contribution to the cell's eight corners; a three-step exchange
 // inside the 8-lane group (halving the corners kept at every step) leaves lane p with the cell's total for corner p,
 // which goes to the contribution planes.  Phase 2 and the node passes are those of the tetrahedral kernels.  Each cell is
-// integrated once (the node-centric kernel above integrates it eight times, once per corner).
+// integrated once (round 1's node-centric kernel integrated it eight times, once per corner: 1.3-3.0 ms per pass at 10^6
+// nodes against 0.23-0.61 ms).
 constexpr int HK_NT = 256;
 
 __device__ __forceinline__ double shfl_x(unsigned mask, double v, int o) { return __shfl_xor_sync(mask, v, o); }
@@ -978,7 +875,7 @@ __device__ __forceinline__ void cell_exchange(unsigned mask, int p, const T (&ph
 template <int KIND, typename T>
 constexpr size_t hex_smem_bytes()
 {
-    return (size_t)CM_NL_MAX * 4 * sizeof(double) + (size_t)(8 * KindTraits<KIND>::NC * CM_HC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
+    return (size_t)CM_HC_MAX * 24 * sizeof(double) + (size_t)(8 * KindTraits<KIND>::NC * CM_HC_MAX + CM_NL_MAX * KindTraits<KIND>::NIN) * sizeof(T) +
            (size_t)(8 * CM_HC_MAX + 8 * CM_HC_MAX + CM_HC_MAX + CM_NL_MAX + 8) * sizeof(unsigned short) + 16;
 }
 
@@ -988,8 +885,8 @@ __global__ void __launch_bounds__(HK_NT, 2) hex_chunk_kernel(ChunkArgs<T> a)
     typedef KindTraits<KIND> K;
     constexpr int NIN = K::NIN, NC = K::NC, HC = CM_HC_MAX;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *scx = reinterpret_cast<double *>(smem_raw);                          // [nl][4]
-    T *scr = reinterpret_cast<T *>(scx + (size_t)CM_NL_MAX * 4);                 // [8 NC][HC]
+    double *scx = reinterpret_cast<double *>(smem_raw);                          // [ne][8][3] corner coordinates of the cells
+    T *scr = reinterpret_cast<T *>(scx + (size_t)CM_HC_MAX * 24);                // [8 NC][HC]
     T *sin = scr + 8 * NC * HC;                                                 // [nl][NIN]
     unsigned short *slid = reinterpret_cast<unsigned short *>(sin + CM_NL_MAX * NIN); // [ne][8]
     unsigned short *sle = slid + 8 * HC;                                        // [8 ne]
@@ -1000,9 +897,9 @@ __global__ void __launch_bounds__(HK_NT, 2) hex_chunk_kernel(ChunkArgs<T> a)
     const int e0 = a.eptr[c], ne = a.eptr[c + 1] - e0, ne8 = (ne + 7) & ~7, s0 = a.nptr[c], nl = a.nptr[c + 1] - s0;
     if (tid == 0) {
         mbar_init(bar, 1);
-        const unsigned bg = 32u * nl, bl = 16u * ne8, be = 2u * ne8;
+        const unsigned bg = 192u * ne, bl = 16u * ne8, be = 2u * ne8;
         mbar_expect_tx(bar, bg + 2 * bl + be);
-        bulk_g2s(scx, a.CX + 4L * s0, bg, bar);
+        bulk_g2s(scx, a.CX + 24L * e0, bg, bar);
         bulk_g2s(slid, a.lid + 8L * e0, bl, bar);
         bulk_g2s(sle, a.lent + 8L * e0, bl, bar);
         bulk_g2s(sem, a.emat + e0, be, bar);
@@ -1038,9 +935,12 @@ __global__ void __launch_bounds__(HK_NT, 2) hex_chunk_kernel(ChunkArgs<T> a)
         }
         double X[8][3], phid[8], gd[8][3];
 #pragma unroll
-        for (int k = 0; k < 8; k++) {
-            const double2 q = *reinterpret_cast<const double2 *>(scx + 4 * l[k]);
-            X[k][0] = q.x; X[k][1] = q.y; X[k][2] = scx[4 * l[k] + 2];
+        for (int k = 0; k < 4; k++) { // the cell's 24 words as twelve 128-bit loads, the same addresses in its eight lanes
+            const double2 q0 = *reinterpret_cast<const double2 *>(scx + 24 * el + 6 * k);
+            const double2 q1 = *reinterpret_cast<const double2 *>(scx + 24 * el + 6 * k + 2);
+            const double2 q2 = *reinterpret_cast<const double2 *>(scx + 24 * el + 6 * k + 4);
+            X[2 * k][0] = q0.x; X[2 * k][1] = q0.y; X[2 * k][2] = q1.x;
+            X[2 * k + 1][0] = q1.y; X[2 * k + 1][1] = q2.x; X[2 * k + 1][2] = q2.y;
         }
         const T det = (T)hex_point(X, p, phid, gd);
         const unsigned em = sem[el];
@@ -1133,20 +1033,13 @@ __global__ void __launch_bounds__(HK_NT, 2) hex_chunk_kernel(ChunkArgs<T> a)
     if (KIND == EK_GRADU) block_reduce_write<3>(gsum, a.partial);
 }
 
-// plain hexahedral meshes: the element-centric chunk kernel; wrapped ones (no chunks): the node-centric kernel
 template <typename T, int KIND>
 static int launch_hex(System<T> *S, const ChunkArgs<T> &a, cudaStream_t st, int *grid_out = nullptr)
 {
-    if (S->mesh->ck.nchunks > 0 && S->CX) {
-        constexpr size_t smem = hex_smem_bytes<KIND, T>();
-        CM_CUDA(cudaFuncSetAttribute(hex_chunk_kernel<T, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        hex_chunk_kernel<T, KIND><<<S->mesh->ck.nchunks, HK_NT, smem, st>>>(a);
-        if (grid_out) *grid_out = S->mesh->ck.nchunks;
-        return CM_OK;
-    }
-    const int B = 128, grid = (int)((S->N + B - 1) / B);
-    hex_node_kernel<T, KIND><<<grid, B, 0, st>>>(a);
-    if (grid_out) *grid_out = grid;
+    constexpr size_t smem = hex_smem_bytes<KIND, T>();
+    CM_CUDA(cudaFuncSetAttribute(hex_chunk_kernel<T, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    hex_chunk_kernel<T, KIND><<<S->mesh->ck.nchunks, HK_NT, smem, st>>>(a);
+    if (grid_out) *grid_out = S->mesh->ck.nchunks;
     return CM_OK;
 }
 

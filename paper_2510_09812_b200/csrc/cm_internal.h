@@ -62,7 +62,7 @@ struct Sell {
 //   ns_ptr / ns_slot   node -> its slots, ascending (so ascending chunk = ascending element order)
 constexpr int CM_EC_MAX = 768;
 constexpr int CM_NL_MAX = 384; // a full chunk of 768 Kuhn tets touches ~260 nodes
-constexpr int CM_HC_MAX = 128; // hexahedral cells per chunk (plain meshes; 8 threads per cell, one per Gauss point)
+constexpr int CM_HC_MAX = 128; // hexahedral cells per chunk (8 threads per cell, one per Gauss point)
 struct Chunks {
     int nchunks = 0;
     long nslots = 0;
@@ -183,9 +183,10 @@ struct System : SystemBase {
     // element geometry, chunk-blocked: chunk c owns 10 planes of ne8 = round_up(ne_c, 8) values at EG + 10 eptr[c]:
     // plane 0 = V_e, plane 3 (k - 1) + d + 1 = d-th component of grad phi_k, k = 1..3 (grad phi_0 = -sum, O-1)
     T *EG = nullptr;
-    // plain (not wrapped) meshes: nondimensional fp64 coordinates of every chunk slot, [slot][4] (x/l_d, y/l_d,
-    // z/l_d, 0), contiguous per chunk: staged by one bulk copy (hexahedra) or one coalesced read (tetrahedra); the element passes recompute V_e and grad phi from them
-    // (tet_geometry_x, the arithmetic that filled EG) instead of streaming ten stored words per element
+    // nondimensional fp64 coordinates for the passes that recompute the geometry with the set-up's own arithmetic
+    // (tet_geometry_x / hex_point).  Plain tetrahedral meshes: of every chunk slot, [slot][4] (x/l_d, y/l_d, z/l_d, 0),
+    // contiguous per chunk, staged by one coalesced read.  Hexahedral meshes (plain and wrapped): the cell's own eight
+    // corners, [cell][8][3], staged by one bulk copy.  Wrapped tetrahedral meshes: none (they stream the stored geometry EG).
     double *CX = nullptr;
     T *mL = nullptr, *mLm = nullptr;
     T *Cstar = nullptr; // n_elastic x 36

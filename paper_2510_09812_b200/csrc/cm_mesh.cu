@@ -440,16 +440,9 @@ int mesh_build_host_hex(cm_mesh *M, const double *gx, long Ng, const int *ghexes
     M->nnz = M->rowptr[N];
     if (build_sell(N, M->rowptr, M->col, CM_C_SCALAR, &M->sell[0]) != CM_OK) return CM_E_BADARG;
     if (build_sell(N, M->rowptr, M->col, CM_C_BLOCK, &M->sell[1]) != CM_OK) return CM_E_BADARG;
-    if (!M->wrapped) {
-        // element-centric passes: chunks of at most CM_HC_MAX cells, as for tetrahedra
-        CM_TRY(build_chunks(N, Ne, M->tets.data(), 8, CM_HC_MAX, &M->ck));
-    } else {
-        // wrapped (periodic) cells take their corners from their own images: node-centric passes, one slot per node
-        M->ck.nchunks = 0; M->ck.nslots = N;
-        M->ck.ns_ptr.resize(N + 1); M->ck.ns_slot.resize(N);
-        std::iota(M->ck.ns_ptr.begin(), M->ck.ns_ptr.end(), 0);
-        std::iota(M->ck.ns_slot.begin(), M->ck.ns_slot.end(), 0);
-    }
+    // element-centric passes: chunks of at most CM_HC_MAX cells, as for tetrahedra (DOF connectivity; the cells' own corner
+    // coordinates are staged per cell, so wrapped meshes need nothing else)
+    CM_TRY(build_chunks(N, Ne, M->tets.data(), 8, CM_HC_MAX, &M->ck));
     return CM_OK;
 }
 
