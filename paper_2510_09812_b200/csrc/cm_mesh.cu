@@ -772,7 +772,7 @@ extern "C" int cm_mesh_get(const cm_mesh *M, int what, void *host_out, long capa
     case CM_GET_LAYOUT: {
         if (capacity < 6) { cm_set_error("cm_mesh_get: capacity"); return CM_E_BADARG; }
         long *o = (long *)host_out;
-        o[0] = M->sell[0].E; o[1] = M->sell[1].E; o[2] = M->ck.nchunks; o[3] = M->ck.nslots; o[4] = CM_EC_MAX; o[5] = CM_NL_MAX;
+        o[0] = M->sell[0].E; o[1] = M->sell[1].E; o[2] = M->ck.nchunks; o[3] = M->ck.nslots; o[4] = M->nen == 8 ? CM_HC_MAX : CM_EC_MAX; o[5] = CM_NL_MAX;
         return CM_OK;
     }
     case CM_GET_ORDER: v = &M->order; break;

@@ -43,7 +43,8 @@ def elem_bytes(N, Ne, s):
 
 
 def hex_elem_bytes(N, Ne, s):
-    """Node-centric hexahedral passes: 32 B connectivity per cell, coordinates (fp64) and nodal input / output once."""
+    """Hexahedral passes: 32 B connectivity per cell, coordinates (fp64) and nodal input / output once (not their bound: they are
+    fp64-ALU-bound)."""
     cell = Ne * 32 + N * 24
     return {"elem_rhs_ms": cell + N * 4 * s, "elem_hd": cell + N * 4 * s, "elem_rhs_mech": cell + N * 6 * s,
             "elem_sigma": cell + N * 12 * s}
