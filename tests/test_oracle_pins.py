@@ -737,3 +737,28 @@ def test_oracle_is_bit_reproducible_across_runs_and_thread_counts():
         assert r.returncode == 0, r.stderr
         outs.append(r.stdout.strip())
     assert len(set(outs)) == 1, outs
+
+
+def test_delaunay_generator_gives_a_valid_unstructured_mesh(orc):
+    """inputs.delaunay_box stands in for the paper's unstructured COMSOL meshes: the cells tile the box (planar
+    faces), are positively oriented, the valence is spread like a mesh generator's, and the oracle's invariants that hold
+    on ANY conforming P1 mesh hold on it: zero row sums and symmetry of K, patch test at interior nodes, rigid-body null
+    space of K^mech."""
+    box = (24 * NM, 21 * NM, 18 * NM)
+    mesh = inputs.delaunay_box((9, 8, 7), box, seed_mesh=1, seed_perm=2)
+    a, b, c, d = (mesh.xyz[mesh.tets[:, k]] for k in range(4))
+    vol = np.einsum("ij,ij->i", np.cross(b - a, c - a), d - a) / 6.0
+    assert (vol > 0).all() and abs(vol.sum() - np.prod(box)) <= 1e-12 * np.prod(box)
+    o = orc.Oracle(mesh, mat2(), 1e-12)
+    deg = np.diff(o.rowptr())
+    assert deg.max() - deg.min() >= 10 and 11 < deg.mean() < 18      # (a boundary-dominated 504-node mesh; 16.2 at 10^6 nodes)
+    K = o.csr(orc.MAT_K_FREE)
+    assert abs(K - K.T).max() == 0 and np.abs(K.sum(axis=1)).max() <= 1e-12 * abs(K).max()
+    lin = mesh.xyz @ np.array([0.3, -1.1, 0.7]) / NM + 2.0
+    y = K @ lin
+    interior = np.all((mesh.xyz > 1e-12) & (mesh.xyz < np.array(box) - 1e-12), axis=1)
+    assert interior.sum() > 100 and np.abs(y[interior]).max() <= 1e-11 * np.abs(y).max()
+    Km = o.csr(orc.MAT_K_MECH_FREE)
+    x = mesh.xyz / NM
+    for rb in (np.tile([1.0, 0, 0], (mesh.n_nodes, 1)), np.stack([-x[:, 1], x[:, 0], 0 * x[:, 0]], axis=1)):
+        assert np.abs(Km @ rb.ravel()).max() <= 1e-9 * abs(Km).max() * np.abs(rb).max()
