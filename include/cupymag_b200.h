@@ -141,7 +141,8 @@ typedef struct {
     double ms[CM_PROF_NCLASS];        /* accumulated device time per class, milliseconds */
     long launches[CM_PROF_NCLASS];    /* kernel launches per class */
     long cg_iters[CM_PROF_NCLASS];    /* CG iterations summed over right-hand sides (CG classes only) */
-    long cg_matrix_passes[CM_PROF_NCLASS]; /* SpMV passes over the matrix inside CG (a 3-RHS solve reads it once per iteration) */
+    long cg_matrix_passes[CM_PROF_NCLASS]; /* passes over the matrix inside CG: one per iteration (a 3-RHS solve reads it once per
+                                              iteration) plus the r0 = b - A x0 pass of every launch */
 } cm_profile;
 
 /* S0: validate, reorder (R21), relabel, node->element lists, CSR pattern.
