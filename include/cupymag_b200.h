@@ -245,6 +245,31 @@ int cm_field_rhs(cm_system *sys, cm_rhs_id id, const void *m_dev, const void *U_
 int cm_volume_average(const cm_mesh *mesh, cm_dtype dtype, const void *g_dev, int ncomp, double *out_host,
                       void *stream);
 
+/* The same volume average for callers that must not allocate device memory: a host program that gave the whole
+ * device to its own memory pool at start-up (cudaMalloc then fails), or a time loop that monitors <m> while other
+ * streams work (cudaMalloc / cudaFree may synchronise the whole device).  cm_volume_average grows a staging copy
+ * inside the mesh with cudaFree + cudaMalloc; this call allocates and frees nothing, calls no allocating library
+ * routine and does not synchronise: it is asynchronous on `stream`.
+ *   g_dev    device, N x ncomp, user order, of `dtype`            (input, caller's)
+ *   out_dev  DEVICE pointer to ncomp doubles, written on `stream`  (output, caller's; read it after the stream
+ *            has reached this point)
+ * Its scratch memory (one partial sum per tile of 8192 nodes) is a fixed device array inside the library, 96 KiB
+ * that every GPU which loads the library holds until the process exits.  Consequences:
+ *   - limits: mesh nodes <= CM_NOALLOC_MAX_NODES and ncomp in {1, 3, 6}; beyond them CM_E_BADARG with a message and
+ *     nothing is launched (cm_volume_average has no node limit);
+ *   - every call on a GPU shares that one array, whatever mesh or stream it is given: calls that can overlap on the
+ *     GPU race and give garbage.  Keep them on one stream or order them with events.  The array keeps the previous
+ *     call's partial sums; no part of it has to start at zero (each call writes every row it reads), so back-to-back
+ *     calls of different sizes need nothing cleared;
+ *   - the first call on each GPU looks up the array's device address (cudaGetSymbolAddress, that GPU current) and
+ *     caches it; make that first call once per GPU at set-up, before any stream capture begins.  Call with the
+ *     mesh's GPU current.
+ * Result: the same sum as cm_volume_average in another (fixed, run-to-run reproducible) order; they agree to
+ * rounding (<= 1e-13 fp64 / 1e-7 fp32 on O(1) fields, tests/test_zz_no_alloc.py). */
+#define CM_NOALLOC_MAX_NODES 16777216L
+int cm_volume_average_noalloc(const cm_mesh *mesh, cm_dtype dtype, const void *g_dev, int ncomp, double *out_dev,
+                              void *stream);
+
 /* One Gauss-Seidel projection step (Alg. B.1; SURVEY O-3).  m_dev (N x 3), U_dev (N), u_dev
  * (N x 3) are updated in place (U, u are the warm starts of the magnetostatic / mechanical CG).
  * info may be NULL (then the call does not synchronise).  Returns the worst CG status. */

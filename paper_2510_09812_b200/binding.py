@@ -26,12 +26,13 @@ CM_OK, CM_E_BADARG, CM_E_DEGENERATE_TET, CM_E_INDEX_RANGE, CM_E_ALLOC, CM_E_CUDA
  CM_GET_N2E) = range(9)
 CM_GET_LAYOUT = 9
 CM_PC_NONE, CM_PC_JACOBI = 0, 1
+CM_NOALLOC_MAX_NODES = 16777216
 CM_OPT_STORED_GEOMETRY, CM_OPT_NO_FUSED_S5S8 = 0, 1
 CM_PROF_CG_MS, CM_PROF_CG_MECH, CM_PROF_CG_GS, CM_PROF_SPMV, CM_PROF_ELEMENT, CM_PROF_POINTWISE, CM_PROF_NCLASS = range(7)
 PROF_NAMES = ("cg_ms", "cg_mech", "cg_gs", "spmv", "element", "pointwise")
 
 EXPORTS = ("cm_mesh_create", "cm_mesh_create_hex", "cm_mesh_create_hex_wrapped", "cm_mesh_create_wrapped", "cm_periodic_wrap", "cm_mesh_destroy", "cm_mesh_get", "cm_assemble_csr", "cm_system_destroy", "cm_system_get_values",
-           "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_cg_solve_pc", "cm_cg_solve3_pc", "cm_cg_history_enable", "cm_cg_history", "cm_spmv_matfree", "cm_cg_solve_matfree", "cm_field_rhs", "cm_volume_average",
+           "cm_system_get_geometry", "cm_spmv", "cm_spmv3", "cm_cg_solve", "cm_cg_solve3", "cm_cg_solve_pc", "cm_cg_solve3_pc", "cm_cg_history_enable", "cm_cg_history", "cm_spmv_matfree", "cm_cg_solve_matfree", "cm_field_rhs", "cm_volume_average", "cm_volume_average_noalloc",
            "cm_gspm_step", "cm_gspm_step_host", "cm_hysteresis_run", "cm_system_set_option", "cm_profile_enable", "cm_profile_get", "cm_profile_reset", "cm_last_error",
            "cm_version")
 
@@ -111,6 +112,7 @@ def lib():
         L.cm_cg_solve_matfree.argtypes = [vp, vp, vp, db, it, it, it, C.POINTER(it), C.POINTER(db), vp]
         L.cm_field_rhs.argtypes = [vp, it, vp, vp, vp, C.POINTER(cm_step_params), db, vp, vp]
         L.cm_volume_average.argtypes = [vp, it, vp, it, C.POINTER(db), vp]
+        L.cm_volume_average_noalloc.argtypes = [vp, it, vp, it, vp, vp]
         L.cm_gspm_step.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
         L.cm_gspm_step_host.argtypes = [vp, C.POINTER(cm_step_params), vp, vp, vp, C.POINTER(cm_step_info), vp]
         L.cm_hysteresis_run.argtypes = [vp, C.POINTER(cm_step_params), C.POINTER(cm_hyst_params), vp, vp, vp, vp, vp, vp,
@@ -222,6 +224,21 @@ class Mesh:
         dt = CM_F64 if g.dtype == torch.float64 else CM_F32
         _check(lib().cm_volume_average(self.h, dt, _dp(g), nc, out, _stream()))
         return np.array(out[:])
+
+    def volume_average_noalloc(self, g, out):
+        """cm_volume_average_noalloc: the same average for callers that must not allocate device memory (their own pool
+        owns the device, or a cudaMalloc would stall their other streams).  `g`: CUDA tensor (N,) or (N, ncomp);
+        `out`: the CALLER's float64 CUDA tensor of ncomp elements, written asynchronously on the current stream
+        (read it after that stream has been waited for).  Nothing is allocated here or in the library; the scratch is
+        a fixed array inside the library shared by every call on this GPU, so calls that may overlap on the GPU race.
+        At most binding.CM_NOALLOC_MAX_NODES nodes, ncomp 1, 3 or 6 (else CmError)."""
+        import torch
+        assert g.is_cuda and g.is_contiguous() and out.is_cuda and out.is_contiguous() and out.dtype == torch.float64
+        nc = 1 if g.dim() == 1 else g.shape[1]
+        assert out.numel() == nc
+        dt = CM_F64 if g.dtype == torch.float64 else CM_F32
+        _check(lib().cm_volume_average_noalloc(self.h, dt, _dp(g), nc, _dp(out), _stream()))
+        return out
 
     def close(self):
         if self.h:

@@ -10,7 +10,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libcupymag_b200.so"
-SOURCES = ["cm_mesh.cu", "cm_assemble.cu", "cm_spmv_cg.cu", "cm_fields.cu", "cm_api.cu"]
+SOURCES = ["cm_mesh.cu", "cm_assemble.cu", "cm_spmv_cg.cu", "cm_fields.cu", "cm_api.cu", "cm_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC,-fopenmp",
               "--expt-relaxed-constexpr"]
 
