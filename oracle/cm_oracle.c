@@ -33,8 +33,10 @@
  * dense solves, precond 0 bitwise the plain solver), the external stress
  * (tests/test_oracle_sigma_ext.py: homogeneous Hooke state, energy stationarity, traction
  * moment) and the row-length-sorted Morton order (tests/test_oracle_pins.py, brute force).
- * Unpinned: the choice between gspm_variant 0 and 1 (R1) -- "parity unpinned" between the
- * two readings; each is pinned by the invariants above.  The adjoint magnetostatic RHS
+ * The two readings of Alg. B.1 Step 2 (gspm_variant 0 and 1, R1) are pinned by the 2 x 2
+ * maps they reduce to for an undamped macrospin (alpha = 0, h || z: forward Euler with
+ * determinant 1 + a^2 as printed, symplectic Euler with determinant 1 for Gauss-Seidel) and
+ * by the conservation of m . h that Eq. 7 demands there.  The adjoint magnetostatic RHS
  * (R9) is pinned against the paper's literal form on periodic domains, where they agree.
  */
 #include <math.h>

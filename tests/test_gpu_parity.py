@@ -438,6 +438,30 @@ def test_gspm_magnetoelastic_inclusion_f64(cm, oracle_mod, torch, variant):
     _check_iters(infos10, mech_frac=0.015)
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+def test_gspm_undamped_precession_both_variants(cm, oracle_mod, torch, variant):
+    """The case that decides DESIGN R1 (tests/test_oracle_pins.py::test_gspm_step2_maps_and_the_conservation_law_of_eq7):
+    alpha = 0, Zeeman only, h || z, a = h dtau = 0.2, uniform start.  100 steps through cm_gspm_step against the oracle
+    (<= 1e-9, north_star), and the device trajectory itself shows the law: variant 1 (Gauss-Seidel) keeps m_z within
+    O(a) of 0.64, variant 0 (2nd row of P:438 as printed) spirals to tan^2(theta_100) = (1 + a^2)^100 tan^2(theta_0)."""
+    mesh = inputs.kuhn_box((6, 5, 4), (15 * NM, 12 * NM, 9 * NM), seed_mesh=61, seed_perm=62)
+    mat = inputs.Material(alpha=0.0)
+    dt, a, n = 1e-12, 0.2, 100
+    h = a / oracle_mod.Oracle(mesh, mat, dt).dtau
+    m0 = np.tile(np.array([0.6, 0.48, 0.64]), (mesh.n_nodes, 1))
+    ms, Us, us, mg, Ug, ug, infos, o = _run_steps(cm, oracle_mod, torch, mesh, mat, dt, TERM_ZEEMAN, n, "f64",
+                                                  np.tile([0, 0, h * mat.Ms], (n, 1)), variant=variant, m0=m0)
+    assert np.abs(mg - ms).max() <= 1e-9
+    _check_iters(infos)
+    assert np.abs(mg - mg[0]).max() < 1e-12                                   # stays uniform
+    t2 = (mg[0, 0] ** 2 + mg[0, 1] ** 2) / mg[0, 2] ** 2
+    if variant == 0:
+        assert abs(t2 / ((0.36 + 0.2304) / 0.4096 * (1 + a * a) ** n) - 1) < 1e-9
+        assert mg[0, 2] < 0.13
+    else:
+        assert abs(mg[0, 2] - 0.64) < 0.06
+
+
 def test_gspm_host_buffers_and_config1_terms(cm, oracle_mod, torch):
     """Reduced instance of config 1 (anisotropy + Zeeman, -50 mT) through the HOST-buffer entry point."""
     cfg = inputs.make_config(1, grid=(21, 21, 7))

@@ -628,6 +628,64 @@ def test_gspm_macrospin_first_order(orc, variant):
     assert 1.6 < errs[0] / errs[1] < 2.4 and 1.6 < errs[1] / errs[2] < 2.4
 
 
+def _precession_run(orc, variant, nsteps, a=0.2, m0=(0.6, 0.48, 0.64)):
+    """Undamped macrospin in h || z, Zeeman term only: every Helmholtz solve acts on a uniform field (K 1 = 0, so
+    g = f exactly) and Alg. B.1 collapses to a 2 x 2 linear map of (m1, m2) with m3* = m3, then the projection."""
+    mesh = _mesh_small()
+    mat = inputs.Material(alpha=0.0)
+    dt = 1e-12
+    o = orc.Oracle(mesh, mat, dt)
+    h = a / o.dtau                                   # a = h dtau
+    m = np.tile(np.array(m0, float), (o.N, 1)); U = np.zeros(o.N); u = np.zeros((o.N, 3))
+    traj = [m[0].copy()]
+    for _ in range(nsteps):
+        info, rc = o.gspm_step(m, U, u, dt, np.array([0, 0, h * mat.Ms]), TERM_ZEEMAN, variant=variant, cg_tol=1e-14)
+        assert rc == 0
+        traj.append(m[0].copy())
+    assert np.abs(m - m[0]).max() < 1e-12
+    return np.array(traj)
+
+
+def test_gspm_step2_maps_and_the_conservation_law_of_eq7(orc):
+    """Pins the arithmetic of BOTH readings of Alg. B.1 Step 2 (DESIGN R1) and decides between them.
+
+    Eq. 7 with alpha = 0 is pure precession: m . h is conserved, so in h || z the component m_z never changes.
+    For a uniform m the Helmholtz solves are identities (g^n = m^n + dtau h, g* = m* + dtau h) and Step 2 is, with
+    a = h dtau,      m1* = m1 - a m2,
+      variant 0 (2nd row as printed, level-n values):  m2* = m2 + a m1        -> map [[1, -a], [a, 1]],      det 1 + a^2
+      variant 1 (Gauss-Seidel):                 m2* = m2 + a m1*       -> map [[1, -a], [a, 1 - a^2]], det 1
+    and m3* = m3 + (m1* m2* - m2* m1*) = m3 in both; Step 3 is the identity at alpha = 0; Step 4 normalises.
+    Consequences that hold exactly and that the oracle must reproduce:
+      variant 0: tan^2(theta) = (m1^2 + m2^2) / m3^2 grows by exactly (1 + a^2) per step (forward Euler spirals out):
+                 m_z = 0.64 -> 0.12 after 100 steps at a = 0.2 -- the printed row breaks m . h conservation at O(1);
+      variant 1: Q / m3^2 with Q = m1^2 - a m1 m2 + m2^2 is invariant (symplectic Euler), so m_z oscillates within
+                 O(a) of its start for ever.
+    A variant-1 branch miscoded with g1^n for g1* (an extra -a m2 m3 in m2*) or with m1^n for m1* (variant 0's row)
+    fails the one-step map at O(a) resp. O(a^2), because m2 != 0 in the start vector."""
+    a, m0 = 0.2, np.array([0.6, 0.48, 0.64])
+    maps = {0: np.array([[1, -a], [a, 1]]), 1: np.array([[1, -a], [a, 1 - a * a]])}
+    for variant, A in maps.items():
+        traj = _precession_run(orc, variant, 400 if variant == 0 else 3000, a, m0)
+        # the reduced map, iterated in numpy: every step to rounding
+        m = m0.copy()
+        for k in range(1, len(traj)):
+            v = np.array([*(A @ m[:2]), m[2]])
+            m = v / np.linalg.norm(v)
+            assert np.abs(traj[k] - m).max() < 2e-13, (variant, k)
+        assert abs(np.linalg.det(A) - (1 + a * a if variant == 0 else 1)) < 1e-15
+        t2 = (traj[:, 0] ** 2 + traj[:, 1] ** 2) / traj[:, 2] ** 2
+        if variant == 0:
+            n = np.arange(len(traj))
+            assert np.allclose(t2, t2[0] * (1 + a * a) ** n, rtol=1e-10, atol=0)
+            assert np.all(np.diff(traj[:, 2]) < 0)                        # m_z decays monotonically ...
+            assert traj[100, 2] < 0.13 and traj[400, 2] < 4e-4            # ... from 0.64: conservation broken at O(1)
+        else:
+            Q = (traj[:, 0] ** 2 - a * traj[:, 0] * traj[:, 1] + traj[:, 1] ** 2) / traj[:, 2] ** 2
+            assert np.abs(Q / Q[0] - 1).max() < 1e-11                     # invariant of the symplectic map
+            assert np.abs(traj[:, 2] - m0[2]).max() < 0.06                # bounded O(a) oscillation over 3000 steps
+            assert traj[:, 2].min() < m0[2] - 0.01 or traj[:, 2].max() > m0[2] + 0.01   # (it does oscillate)
+
+
 def test_gspm_energy_decay_config0(orc, cfg0):
     """Energy non-increasing under damping on config 0 (stable regime), |m| = 1 within 4 ulp."""
     o = orc.Oracle(cfg0.mesh, cfg0.material, cfg0.dt)
