@@ -221,7 +221,10 @@ int cm_cg_solve3_pc(cm_system *sys, cm_matrix_id id, const void *b_dev, void *x_
                     int fixed_iters, int precond, int *iters_out, double *relres_out, void *stream);
 /* Residual history of the solves that follow (on != 0): the kernel records ||r_k|| / ||b|| before iteration k,
  * k = 0 .. iters, per right-hand side (up to 65536 iterations).  cm_cg_history copies the history of the LAST solve to
- * host_out ([k][n_rhs] doubles, n_rhs = 1, or 3 for cm_cg_solve3*), at most `capacity` doubles; *n_out = entries written. */
+ * host_out ([k][n_rhs] doubles, n_rhs = 1, or 3 for cm_cg_solve3*), at most `capacity` doubles; *n_out = entries written.
+ * Only cm_cg_solve, cm_cg_solve3 and their _pc forms record.  *n_out = 0 when the last solve ran with the history off, and
+ * after cm_cg_solve_matfree, cm_gspm_step, cm_gspm_step_host or cm_hysteresis_run (their solves are not recorded as a
+ * history; a step with the history on reuses the buffer). */
 int cm_cg_history_enable(cm_system *sys, int on);
 int cm_cg_history(cm_system *sys, double *host_out, long capacity, long *n_out);
 

@@ -219,7 +219,7 @@ static int api_cg(System<T> *S, cm_matrix_id id, int mode, const void *b, void *
         mxit = std::max(mxit, R.iters[c]);
     }
     S->prof.cg_passes[cls] += mxit + 1; // one matrix pass per iteration plus the r0 = b - A x0 pass
-    S->hist_len = (long)std::min<long>((long)(mxit + 1) * nr, CM_HIST_CAP / nr * nr);
+    S->hist_len = S->hist_on ? (long)std::min<long>((long)(mxit + 1) * nr, CM_HIST_CAP / nr * nr) : 0; // nothing was recorded otherwise
     return R.status;
 }
 
@@ -296,6 +296,7 @@ extern "C" int cm_cg_solve_matfree(cm_system *sys, const void *b_dev, void *x_de
     CM_TRY(check_sys(sys, "cm_cg_solve_matfree"));
     if (!b_dev || !x_dev) { cm_set_error("cm_cg_solve_matfree: null argument"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
+    sys->impl->hist_len = 0; // cm_cg_history covers cm_cg_solve* only: after this call it reads empty, not an earlier solve's curve
     return SYS_DISPATCH(sys, api_cg_matfree<double>(S, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st),
                         api_cg_matfree<float>(S, b_dev, x_dev, tol, maxiter, fixed_iters, precond, iters_out, relres_out, st));
 }
@@ -397,6 +398,7 @@ extern "C" int cm_gspm_step(cm_system *sys, const cm_step_params *params, void *
     CM_TRY(check_sys(sys, "cm_gspm_step"));
     if (!params) { cm_set_error("cm_gspm_step: null params"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
+    sys->impl->hist_len = 0; // cm_cg_history covers cm_cg_solve* only: after this call it reads empty, not an earlier solve's curve
     return SYS_DISPATCH(sys, sys_step<double>(S, params, (double *)m_dev, (double *)U_dev, (double *)u_dev, info, st),
                         sys_step<float>(S, params, (float *)m_dev, (float *)U_dev, (float *)u_dev, info, st));
 }
@@ -426,6 +428,7 @@ extern "C" int cm_gspm_step_host(cm_system *sys, const cm_step_params *params, v
     CM_TRY(check_sys(sys, "cm_gspm_step_host"));
     if (!params) { cm_set_error("cm_gspm_step_host: null params"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
+    sys->impl->hist_len = 0; // cm_cg_history covers cm_cg_solve* only: after this call it reads empty, not an earlier solve's curve
     return SYS_DISPATCH(sys, api_step_host<double>(S, params, m_host, U_host, u_host, info, st),
                         api_step_host<float>(S, params, m_host, U_host, u_host, info, st));
 }
@@ -437,6 +440,7 @@ extern "C" int cm_hysteresis_run(cm_system *sys, const cm_step_params *base, con
     CM_TRY(check_sys(sys, "cm_hysteresis_run"));
     if (!base || !hp) { cm_set_error("cm_hysteresis_run: null params"); return CM_E_BADARG; }
     cudaStream_t st = (cudaStream_t)stream;
+    sys->impl->hist_len = 0; // cm_cg_history covers cm_cg_solve* only: after this call it reads empty, not an earlier solve's curve
     return SYS_DISPATCH(sys, sys_hysteresis<double>(S, base, hp, (double *)m_dev, (double *)U_dev, (double *)u_dev, H_log, mbar_log, steps_log, result, st),
                         sys_hysteresis<float>(S, base, hp, (float *)m_dev, (float *)U_dev, (float *)u_dev, H_log, mbar_log, steps_log, result, st));
 }

@@ -340,12 +340,32 @@ def test_gspm_steps_matfree(cm, oracle_mod, torch):
         gs.hysteresis_run(cm.make_params(1e-12, terms=ALL, mech_matfree=1), mg, Ug, ug, [2e4, 0, 0], [-1e3, 0, 0], max_fields=2, max_steps=2)
 
 
+def _cg_history_extended(A, b, tol):
+    """Textbook CG (x0 = 0) on a scipy CSR matrix with every product, dot and update in numpy long double (64-bit
+    mantissa on x86): the reference the two fp64 runs are measured against.  Returns ||r_k|| / ||b||, k = 0 .. iters."""
+    ft = np.longdouble
+    data, idx, ptr = A.data.astype(ft), A.indices, A.indptr[:-1]
+    b = b.astype(ft); x = np.zeros_like(b); r = b.copy(); pv = r.copy()
+    bb = b @ b; rr = r @ r
+    h = [float(np.sqrt(rr / bb))]
+    while h[-1] >= tol and len(h) < 5000:
+        Ap = np.add.reduceat(data * pv[idx], ptr)
+        al = rr / (pv @ Ap); x += al * pv; r -= al * Ap
+        rn = r @ r; pv = r + (rn / rr) * pv; rr = rn
+        h.append(float(np.sqrt(rr / bb)))
+    return np.array(h)
+
+
 def test_mechanical_residual_curves_part_by_rounding(cm, oracle_mod, torch, capsys):
     """Why the in-step mechanical CG count is compared with 1.5 % instead of +-1.  Step-0 mechanical solve
-    of the inclusion mesh (b = b^mech(m0), x0 = 0): the device's and the oracle's recurrence residuals agree to rounding for
-    the first ~60 iterations, then part abruptly (loss of orthogonality amplifies the different rounding of fused / unfused
-    products) and from there on are two finite-precision CG runs of the same system: same average rate, non-monotone
-    residual norm, first crossings of 1e-7 / 1e-10 / 1e-12 a few iterations apart.  Run with -s to print the table."""
+    of the inclusion mesh (b = b^mech(m0), x0 = 0), three runs of the same recurrence: the device (fp64, fused products,
+    sliced summation order), the oracle (fp64, no contraction, row order) and an extended-precision CG (numpy long double).
+    All three agree to rounding for the first ~60 iterations; then loss of orthogonality amplifies the rounding
+    differences by about x4 per iteration and BOTH fp64 runs leave the extended-precision curve at the same iteration
+    and by the same order (a few per cent to tens of per cent of a residual that falls twelve decades): the device is as
+    far from the reference as the oracle is, which is what "two finite-precision CG runs of one system" means, and not
+    what a defect in either would look like (that shows from iteration 0).  How far the device is from the oracle after
+    the parting is printed, not asserted: a more accurate dot product would be welcome."""
     mesh = inputs.kuhn_box((13, 13, 7), (40 * NM, 40 * NM, 20 * NM), seed_mesh=21, seed_perm=22)
     mesh = inputs.flag_inclusion(mesh, np.array(mesh.box) / 2, (8 * NM,) * 3)
     clamp = inputs.clamp_bottom(mesh)
@@ -354,24 +374,70 @@ def test_mechanical_residual_curves_part_by_rounding(cm, oracle_mod, torch, caps
     gs = cm.System(gm, mat2(), 1e-12, "f64", clamp)
     b = o.rhs_mech(inputs.init_m_noisy_x(mesh, 23))
     _, ito, ho = o.cg_history(oracle_mod.MAT_K_MECH, b.ravel(), tol=1e-12)
+    hx = _cg_history_extended(o.csr(oracle_mod.MAT_K_MECH), b.ravel(), 1e-12)
     gs.cg_history_enable(True)
     x = torch.zeros((mesh.n_nodes, 3), dtype=torch.float64, device="cuda")
     itg, _, _ = gs.cg_solve(cm.CM_MAT_K_MECH, torch.as_tensor(b, device="cuda"), x, tol=1e-12)
     hg = gs.cg_history()
     gs.cg_history_enable(False)
-    n = min(len(ho), len(hg))
+    assert len(hg) == itg + 1 and len(ho) == ito + 1
+    n = min(len(ho), len(hg), len(hx))
     dev = np.abs(ho[:n] - hg[:n]) / ho[:n]
-    assert dev[:40].max() < 1e-12                      # the same algorithm, iteration by iteration, while rounding is small
-    assert dev.max() > 1e-3                            # ... and two different finite-precision runs later on
+    dev_o = np.abs(ho[:n] - hx[:n]) / hx[:n]
+    dev_g = np.abs(hg[:n] - hx[:n]) / hx[:n]
+    # the same algorithm, iteration by iteration, while rounding is small: all three curves
+    assert dev[:40].max() < 1e-12 and dev_o[:40].max() < 1e-12 and dev_g[:40].max() < 1e-12
+    # both fp64 runs leave the extended-precision curve at the same place ...
+    on_o, on_g = int(np.argmax(dev_o > 1e-6)), int(np.argmax(dev_g > 1e-6))
+    assert 40 < on_o < n and 40 < on_g < n and abs(on_o - on_g) <= 10, (on_o, on_g)
+    # ... and stay in the same envelope around it (measured here: oracle up to 0.41)
+    assert dev_g.max() <= max(3 * dev_o.max(), 0.5) and dev_o.max() <= max(3 * dev_g.max(), 0.5), (dev_o.max(), dev_g.max())
     with capsys.disabled():
-        print(f"\nmechanical CG, step 0 of the inclusion mesh, tol 1e-12: oracle {ito} iterations, device {itg}")
+        print(f"\nmechanical CG, step 0 of the inclusion mesh, tol 1e-12: oracle {ito} iterations, device {itg}, long double {len(hx) - 1}")
+        print(f"  parting from the long-double run (rel.dev > 1e-6): oracle at k={on_o}, device at k={on_g}; "
+              f"max rel.dev oracle {dev_o.max():.2e}, device {dev_g.max():.2e}; device vs oracle {dev.max():.2e}")
         for j in range(0, n, 20):
-            print(f"  k={j:3d}  oracle {ho[j]:.6e}  device {hg[j]:.6e}  rel.dev {dev[j]:.1e}")
+            print(f"  k={j:3d}  oracle {ho[j]:.6e}  device {hg[j]:.6e}  long double {hx[j]:.6e}  dev-orc {dev[j]:.1e}  orc-ld {dev_o[j]:.1e}  dev-ld {dev_g[j]:.1e}")
     for tol in (1e-7, 1e-10, 1e-12):
-        io, ig = int(np.argmax(ho < tol)), int(np.argmax(hg < tol))
+        io, ig, ix = int(np.argmax(ho < tol)), int(np.argmax(hg < tol)), int(np.argmax(hx < tol))
         with capsys.disabled():
-            print(f"  first crossing of {tol:g}: oracle {io}, device {ig}")
+            print(f"  first crossing of {tol:g}: oracle {io}, device {ig}, long double {ix}")
         assert abs(io - ig) <= max(1, int(np.ceil(0.015 * io)))
+        assert abs(ix - ig) <= max(1, int(np.ceil(0.015 * ix))) and abs(ix - io) <= max(1, int(np.ceil(0.015 * ix)))
+
+
+def test_cg_history_covers_recorded_solves_only(cm, torch):
+    """cm_cg_history returns the curve of the last RECORDED solve and nothing else: empty after a solve with the history
+    off, after cm_cg_history_enable(0), and after the calls that do not record (a GSPM step, a matrix-free solve) -- never
+    an earlier solve's curve or unwritten memory (cm_api.cu)."""
+    mesh = inputs.kuhn_box((7, 6, 5), (18 * NM, 15 * NM, 12 * NM), seed_mesh=5, seed_perm=6)
+    clamp = inputs.clamp_bottom(mesh)
+    gs = cm.System(cm.Mesh(mesh.xyz, mesh.tets), mat2(), 1e-12, "f64", clamp)
+    N = mesh.n_nodes
+    b = torch.as_tensor(np.random.default_rng(8).normal(size=N), device="cuda"); b[0] = 0
+    x = torch.zeros(N, dtype=torch.float64, device="cuda")
+    it, _, _ = gs.cg_solve(cm.CM_MAT_K_MS, b, x, tol=1e-10)
+    assert it > 3 and len(gs.cg_history()) == 0                      # history never enabled
+    gs.cg_history_enable(True)
+    x.zero_(); it, res, _ = gs.cg_solve(cm.CM_MAT_K_MS, b, x, tol=1e-10)
+    h = gs.cg_history()
+    assert len(h) == it + 1 and h[0] == 1.0 and h[-1] < 1e-10 <= h[-2]
+    b3 = torch.as_tensor(np.random.default_rng(9).normal(size=(N, 3)), device="cuda"); x3 = torch.zeros_like(b3)
+    it3, _, _ = gs.cg_solve3(cm.CM_MAT_K_GS1, b3, x3, tol=1e-10)
+    assert gs.cg_history(3).shape == (max(it3) + 1, 3)
+    m = torch.as_tensor(inputs.init_m_random(mesh, 3), device="cuda")
+    gs.gspm_step(cm.make_params(1e-12, terms=TERM_ANIS | TERM_ZEEMAN), m, torch.zeros(N, dtype=torch.float64, device="cuda"), torch.zeros_like(m))
+    assert len(gs.cg_history()) == 0                                 # a step does not leave a history behind
+    x.zero_(); gs.cg_solve(cm.CM_MAT_K_MS, b, x, tol=1e-10)
+    assert len(gs.cg_history()) == it + 1
+    bm = b3.clone(); bm[torch.as_tensor(clamp.reshape(N, 3).astype(bool), device="cuda")] = 0
+    gs.cg_solve_matfree(bm, torch.zeros_like(bm), tol=1e-8)
+    assert len(gs.cg_history()) == 0                                 # nor does a matrix-free solve
+    x.zero_(); gs.cg_solve(cm.CM_MAT_K_MS, b, x, tol=1e-10)
+    gs.cg_history_enable(False)
+    assert len(gs.cg_history()) == 0
+    x.zero_(); gs.cg_solve(cm.CM_MAT_K_MS, b, x, tol=1e-10)
+    assert len(gs.cg_history()) == 0
 
 
 def test_round2_entry_points_refuse_bad_arguments(cm, torch):
