@@ -236,17 +236,28 @@ def test_config3_one_converged_step(full, oracle_mod):
     dm = np.abs(mg.cpu().numpy() - m).max()
     print(f"config 3, one converged step at tol 1e-7: max |dm| = {dm:.2e}, max |dU| / max |U| = {rel(Ug.cpu().numpy(), U):.2e}, "
           f"max |du| / max |u| = {rel(ug.cpu().numpy(), u):.2e}")
-    assert dm <= 1e-4
-    assert np.allclose(ig.mbar[:], io.mbar[:], atol=1e-12) and ig.mean_dm == pytest.approx(io.mean_dm, rel=1e-4)
+    assert dm <= 1e-7                                  # measured 6.1e-9 (profiles/r02_fullsize_converged.txt); two tol-1e-7 solves
+    assert np.allclose(ig.mbar[:], io.mbar[:], atol=1e-12) and ig.mean_dm == pytest.approx(io.mean_dm, rel=1e-7)
 
 
 SLOW = pytest.mark.skipif(os.environ.get("CM_SLOW_TESTS", "0") != "1",
                           reason="about 7 minutes of oracle time: set CM_SLOW_TESTS=1 (log of the last run: profiles/r02_fullsize_converged.txt)")
 
 
+def test_config2_full_size_3_steps_f64(oracle_mod):
+    """BASELINE config 2 at its own 515,871 nodes in the DEFAULT suite: three converged steps, fp64, tol 1e-12, max |dm| <= 1e-9,
+    counts +-1 (mechanical 1.5 %).  The ten-step fp64 / fp32 runs of the same configuration stay behind CM_SLOW_TESTS=1."""
+    _config2_full_size(oracle_mod, "f64", 3)
+
+
 @SLOW
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config2_full_size_10_steps(oracle_mod, dtype):
+    """Ten steps of the same (see _config2_full_size)."""
+    _config2_full_size(oracle_mod, dtype, 10)
+
+
+def _config2_full_size(oracle_mod, dtype, nsteps):
     """BASELINE config 2 at its own size (129x129x31 = 515,871 nodes, all physics, spherical inclusion with x2 stiffness,
     clamped bottom face, dt = 10 ps): ten steps, every solve iterated to convergence on both sides.
     fp64: tol 1e-12, max |dm| <= 1e-9, counts +-1 (mechanical 1.5 %).
@@ -269,7 +280,7 @@ def test_config2_full_size_10_steps(oracle_mod, dtype):
     mg = torch.as_tensor(cfg.m0, dtype=td, device="cuda").contiguous()
     Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
     errs = []
-    for k in range(10):
+    for k in range(nsteps):
         io, rco = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k], cfg.terms, cg_tol=tol)
         ig, rcg = gs.gspm_step(cm.make_params(cfg.dt, cfg.Hext[k], cfg.terms, 0, tol), mg, Ug, ug)
         assert rco == 0 and rcg == 0
@@ -279,9 +290,11 @@ def test_config2_full_size_10_steps(oracle_mod, dtype):
             assert abs(io.it_mech - ig.it_mech) <= int(np.ceil(0.015 * io.it_mech)), (k, io.it_mech, ig.it_mech)
             for a in range(8):
                 assert abs(io.it_gs[a] - ig.it_gs[a]) <= 1, (k, a, list(io.it_gs), list(ig.it_gs))
-    print(f"\nconfig 2 full size, {dtype}: max |dm| after steps 1..10 = {['%.1e' % e for e in errs]}; last-step CG its ms/mech "
+    print(f"\nconfig 2 full size, {dtype}: max |dm| after steps 1..{nsteps} = {['%.1e' % e for e in errs]}; last-step CG its ms/mech "
           f"{ig.it_ms}/{ig.it_mech}, <|dm|> per step {io.mean_dm:.2f}")
     if f64:
         assert errs[-1] <= 1e-9, errs
     else:
+        # ten steps: reported, not met (1e-4 is north_star's) -- first-step accuracy times the amplification of the dynamics,
+        # pinned at reduced size in tests/test_gpu_parity.py::test_config2_fp32_error_is_first_step_accuracy_times_...
         assert errs[0] <= 1e-4 and errs[-1] <= 5e-2, errs

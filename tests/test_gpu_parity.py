@@ -482,6 +482,65 @@ def test_gspm_f32_10_steps(cm, oracle_mod, torch):
     _check_iters(infos, slack=3)
 
 
+def test_config2_fp32_error_is_first_step_accuracy_times_the_amplification_of_the_dynamics(cm, oracle_mod, torch):
+    """Config 2 (reduced: 41 x 41 x 11 nodes, same recipe and 3.125 nm spacing) is where fp32 misses north_star's 1e-4
+    after ten steps.  The explanation -- the dynamics at dtau = 2.65 amplify any perturbation, an fp32 rounding included --
+    is pinned here instead of being told (ADVICE round 2; CPU half: tests/test_oracle_pins.py::
+    test_config2_dynamics_amplify_any_perturbation):
+      (1) the fp64 DEVICE started from m0 rounded once to fp32 (a 3e-8 perturbation), against the fp64 oracle from m0:
+          the distance grows by more than x10 over ten steps although both sides compute in fp64 and agree to 1e-9 from
+          equal starts (test_gspm_magnetoelastic_inclusion_f64) -- amplification by the dynamics alone;
+      (2) the fp32 device against the fp64 oracle: <= 1e-4 after the FIRST step (north_star's level for one fp32 step),
+          and never above 1e-4 times a small multiple of the amplification measured in (1) (every step adds its own fp32
+          rounding, so the curve is a sum of amplified contributions, not one);
+      (3) the fp32 device is no further from the fp64 oracle than a small multiple of what the oracle's own fp32 twin
+          (the same source compiled in float, on the CPU) is: a kernel or precision defect growing at the same rate
+          would show as a device curve above the twin's."""
+    nm = 1e-9
+    g = (41, 41, 11)
+    cfg = inputs.make_config(2, grid=g, box=tuple((n - 1) * 3.125 * nm for n in g))
+    mesh, N = cfg.mesh, cfg.mesh.n_nodes
+    gm = cm.Mesh(mesh.xyz, mesh.tets, mesh.magnetic, mesh.elastic_id, cm.CM_REORDER_MORTON)
+
+    def oracle_run(dtype, tol):
+        o = oracle_mod.Oracle(mesh, cfg.material, cfg.dt, clamp_dof=cfg.clamp_dof, pin_node=cfg.pin_node, dtype=dtype)
+        m = cfg.m0.astype(o.real).copy(); U = np.zeros(N, o.real); u = np.zeros((N, 3), o.real)
+        out = []
+        for k in range(10):
+            _, rc = o.gspm_step(m, U, u, cfg.dt, cfg.Hext[k], cfg.terms, cg_tol=tol)
+            assert rc == 0
+            out.append(m.astype(np.float64).copy())
+        return out
+
+    def device_run(m0, dtype, tol):
+        gs = cm.System(gm, cfg.material, cfg.dt, dtype, cfg.clamp_dof, cfg.pin_node)
+        td = torch.float64 if dtype == "f64" else torch.float32
+        mg = torch.as_tensor(m0, dtype=td, device="cuda").contiguous()
+        Ug = torch.zeros(N, dtype=td, device="cuda"); ug = torch.zeros((N, 3), dtype=td, device="cuda")
+        out = []
+        for k in range(10):
+            _, rc = gs.gspm_step(cm.make_params(cfg.dt, cfg.Hext[k], cfg.terms, 0, tol), mg, Ug, ug)
+            assert rc == 0
+            out.append(mg.cpu().numpy().astype(np.float64))
+        return out
+
+    ref = oracle_run("f64", 1e-12)
+    twin = oracle_run("f32", 1e-6)
+    err = lambda run: np.array([np.abs(a - b).max() for a, b in zip(run, ref)])
+    e_same = err(device_run(cfg.m0, "f64", 1e-12))
+    e_pert = err(device_run(cfg.m0.astype(np.float32).astype(np.float64), "f64", 1e-12))
+    e_32 = err(device_run(cfg.m0, "f32", 1e-6))
+    e_twin = err(twin)
+    amp_p, amp_32 = e_pert.max() / e_pert[0], e_32.max() / e_32[0]
+    print(f"\nconfig 2 reduced {g}, max |dm| from the fp64 oracle after steps 1..10:\n  fp64 device, same start      {['%.1e' % e for e in e_same]}"
+          f"\n  fp64 device, m0 rounded once {['%.1e' % e for e in e_pert]} (x{amp_p:.0f})\n  fp32 device                  {['%.1e' % e for e in e_32]} (x{amp_32:.0f})"
+          f"\n  fp32 oracle twin             {['%.1e' % e for e in e_twin]}")
+    assert e_same.max() <= 1e-9                                          # equal starts: fp64 parity, north_star
+    assert e_pert[0] < 1e-7 and amp_p > 10                               # (1)
+    assert e_32[0] <= 1e-4 and e_32.max() <= 1e-4 * 3 * amp_p            # (2): inside 1e-4 after one step, then no more than that x amplification
+    assert e_32.max() <= 5 * e_twin.max() and e_32[0] <= 5 * e_twin[0]   # (3)
+
+
 def test_gspm_fixed_iterations(cm, oracle_mod, torch):
     """cg_fixed_iters = 3 (the throughput variant of SURVEY 8d): identical arithmetic, no stopping test."""
     cfg = inputs.make_config(0)
