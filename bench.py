@@ -109,6 +109,14 @@ def time_oracle(steps: int, warmup: int, variant: int = 0, full_mesh: bool = Fal
     n_full = FULL_GRID[0] * FULL_GRID[1] * FULL_GRID[2]
     scale = o.N / n_full
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    cpu_model = "unknown"
+    try:
+        for ln in Path("/proc/cpuinfo").read_text().splitlines():
+            if ln.startswith("model name"):
+                cpu_model = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
     timed = its[warmup:]
     n_it = sum(a + b + c for a, b, c in timed)
     where = (f"config 3 itself ({o.N} nodes), every CG solve capped at {maxiter} iterations" if full_mesh else
@@ -117,7 +125,8 @@ def time_oracle(steps: int, warmup: int, variant: int = 0, full_mesh: bool = Fal
     desc = (f"{steps} GSPM step(s) after {warmup} warm-up step(s), gspm_variant {variant}, tol {CG_TOL:g}, on {where}; "
             f"CG its per timed step (ms, mech, sum gs) {timed}")
     return {"value": steps / dt * scale, "sec_per_step": dt / steps, "desc": desc, "cores": cores, "cg_iters_per_step": timed,
-            "ms_per_cg_iteration_all_solves": 1e3 * dt / max(1, n_it), "nodes": o.N, "setup_s": t_setup}
+            "ms_per_cg_iteration_all_solves": 1e3 * dt / max(1, n_it), "nodes": o.N, "setup_s": t_setup, "cpu_model": cpu_model,
+            "omp_num_threads": os.environ.get("OMP_NUM_THREADS", f"unset (OpenMP default: {os.cpu_count()} logical CPUs)")}
 
 
 def run_reference(args):
@@ -127,7 +136,7 @@ def run_reference(args):
     r = time_oracle(args.steps, args.warmup, args.variant, args.full_mesh, args.oracle_maxiter)
     cb = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["desc"],
           "cg_iters_per_step": r["cg_iters_per_step"], "ms_per_cg_iteration_all_solves": r["ms_per_cg_iteration_all_solves"],
-          "setup_s": r["setup_s"]}
+          "setup_s": r["setup_s"], "cpu_model": r["cpu_model"], "omp_num_threads": r["omp_num_threads"]}
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": r["sec_per_step"] * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -182,6 +191,8 @@ def run_ours(args):
     t_setup = time.perf_counter()
     mesh = cm.Mesh(cfg.mesh.xyz, cfg.mesh.tets, cfg.mesh.magnetic, cfg.mesh.elastic_id, cm.CM_REORDER_MORTON)
     sysm = cm.System(mesh, cfg.material, cfg.dt, dtype, cfg.clamp_dof, cfg.pin_node)
+    if args.no_fuse_s5s8:
+        sysm.set_option(cm.CM_OPT_NO_FUSED_S5S8, 1)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup
     N, nnz = mesh.n_nodes, mesh.nnz
@@ -241,15 +252,34 @@ def run_ours(args):
                              "streamed_GBps": streamed / (p["ms"] * 1e-3) / 1e9}
         for name in ("spmv", "element", "pointwise"):
             out[name] = {"ms": prof[name]["ms"], "launches": prof[name]["launches"]}
-        # assembly (element passes S3, S5, S6, 2 x S8 per step, each followed by its node pass): SURVEY 8(d) bytes -- per tet
-        # 16 B connectivity + 13 words, nodal input and output once
-        elem_step = 5 * mesh.n_tets * (16 + 13 * s) + N * s * (4 + 4 + 6 + 2 * 12)
+        # assembly.  The step launches FOUR chunk passes when S5 shares S8's pass (demag + mechanics on tetrahedra, the default):
+        # S3, S6, S5+S8 at m^n, S8 at m*; five otherwise.  Two numerators, both printed ("report which numerator is used"):
+        #  algorithmic_GBps -- SURVEY 8(d)'s stored-gradient figure for the passes that RAN: per tetrahedron 16 B connectivity +
+        #                      13 words, nodal inputs and outputs once (38 words per node and step);
+        #  streamed_GBps    -- the bytes of the variant that ran: a pass that recomputes its geometry (fp64 S3; fp64 S5 only when it
+        #                      runs unfused) reads 3 words per tetrahedron plus its chunk's slot coordinates (24 B per slot)
+        #                      instead of the ten stored geometry words.
+        fused = mesh.nen == 4 and not args.no_fuse_s5s8
+        n_pass = 4 if fused else 5
+        n_recompute = (1 if fused else 2) if s == 8 else 0
+        nodal = N * s * (4 + 4 + 6 + 2 * 12)
+        elem_step = n_pass * mesh.n_tets * (16 + 13 * s) + nodal
+        elem_streamed = ((n_pass - n_recompute) * mesh.n_tets * (16 + 13 * s) + n_recompute * (mesh.n_tets * (16 + 3 * s) + n_slots * 24)
+                         + nodal)
         if out["element"]["ms"] > 0:
             gbs = elem_step * steps / (out["element"]["ms"] * 1e-3) / 1e9
-            out["element"].update({"algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_spec_8000": gbs / 8000.0})
+            gbs_s = elem_streamed * steps / (out["element"]["ms"] * 1e-3) / 1e9
+            out["element"].update({"algorithmic_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_spec_8000": gbs / 8000.0,
+                                   "streamed_GBps": gbs_s, "streamed_frac_of_measured_peak": gbs_s / peak,
+                                   "chunk_passes_per_step": n_pass, "passes_recomputing_geometry": n_recompute,
+                                   "numerator": "frac_of_measured_peak: SURVEY 8(d) stored-gradient bytes of the chunk passes that ran "
+                                                "(S5 fused into S8's pass counts once); streamed_*: bytes of the variant that ran "
+                                                "(recomputed-geometry passes read coordinates, not gradients); the class time also "
+                                                "holds the node passes"})
         return out, ab
 
     s = 8 if dtype == "f64" else 4
+    n_slots = int(round(mesh.layout()["slots_per_node"] * N))
     main = timed_run(sysm, dtype, args.steps, args.warmup, args.variant, args.fixed_iters, args.precond)
     ms_total, value, prof, infos = main["ms_total"], main["value"], main["prof"], main["infos"]
 
@@ -308,10 +338,12 @@ def run_ours(args):
     per_class, ab = kernel_table(prof, args.steps, s)
     dom = max(("cg_mech", "cg_ms", "cg_gs"), key=lambda n: prof[n]["ms"])
     key = {"cg_mech": "bsr3", "cg_ms": "csr1", "cg_gs": "csr3"}[dom]
-    # DRAM bytes per matrix pass measured by `ncu --set full` (fp64: profiles/r02_cg_full.md, fp32: profiles/r01_f_cg_full.md; config 3,
-    # 21 passes per launch), EXTRAPOLATED to the average launch of this run, like `achieved`.  Only known for the captured workload.
-    ncu_bytes_per_pass = {("cg_mech", "f64"): 89.973014e9 / 21, ("cg_ms", "f64"): 14.287394e9 / 21,
-                          ("cg_mech", "f32"): 43.734836e9 / 21, ("cg_ms", "f32"): 7.856605e9 / 21}
+    # DRAM bytes per matrix pass measured by `ncu --set full` on config 3 (21 passes per launch), read from the committed
+    # profiles/ncu_constants.json (each entry names the capture it comes from), EXTRAPOLATED to the average launch of this run,
+    # like `achieved`.  Only known for the captured workload.
+    ncu_const = json.loads((ROOT / "profiles" / "ncu_constants.json").read_text())
+    ncu_bytes_per_pass = {(k.split("/")[0], k.split("/")[1]): v["dram_bytes"] / v["matrix_passes"] for k, v in ncu_const["cg"].items()}
+    ncu_source = {(k.split("/")[0], k.split("/")[1]): v["source"] for k, v in ncu_const["cg"].items()}
     traffic = None
     passes_per_launch = prof[dom]["cg_matrix_passes"] / max(1, prof[dom]["launches"])
     if (dom, dtype) in ncu_bytes_per_pass and not args.grid:
@@ -323,8 +355,8 @@ def run_ours(args):
             "algorithmic_bytes_per_iteration": ab["cg_iter_" + key], "streamed_bytes_per_iteration": ab["cg_streams_" + key],
             "bytes_r0_pass": ab["cg_r0_" + key], "matrix_passes_per_launch": passes_per_launch,
             "achieved_streamed": per_class.get(dom, {}).get("streamed_GBps"),
-            "traffic_source": "extrapolated: ncu --set full dram__bytes_read+write per matrix pass of a 21-pass capture "
-                              "(profiles/r02_cg_full.md; fp32: profiles/r01_f_cg_full.md) x matrix passes per launch of this run"}
+            "traffic_source": ("extrapolated: ncu --set full dram__bytes_read+write per matrix pass of a 21-pass capture ("
+                               + ncu_source.get((dom, dtype), "none") + ") x matrix passes per launch of this run")}
 
     launches = sum(p["launches"] for p in prof.values())
     last = infos[-1]
@@ -348,7 +380,18 @@ def run_ours(args):
         r = time_oracle(2, 1, args.variant)
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["desc"],
                                 "cg_iters_per_step": r["cg_iters_per_step"],
-                                "ms_per_cg_iteration_all_solves": r["ms_per_cg_iteration_all_solves"]}
+                                "ms_per_cg_iteration_all_solves": r["ms_per_cg_iteration_all_solves"],
+                                "cpu_model": r["cpu_model"], "omp_num_threads": r["omp_num_threads"]}
+        if not args.no_cpu_full_mesh and not args.grid:
+            # like for like: the oracle on config 3 ITSELF, one step with every solve capped at 40 iterations (a bounded sample:
+            # ~1 min of set-up + ~20 s of solves), against the GPU's time per matrix pass of the dominant solve on the same mesh
+            rf = time_oracle(1, 0, args.variant, full_mesh=True, maxiter=40)
+            gpu_ms_pass = prof["cg_mech"]["ms"] / max(1, prof["cg_mech"]["cg_matrix_passes"])
+            line["cpu_baseline"].update({"full_mesh_ms_per_cg_iteration": rf["ms_per_cg_iteration_all_solves"],
+                                         "full_mesh_sample": rf["desc"], "full_mesh_setup_s": rf["setup_s"],
+                                         "gpu_ms_per_matrix_pass_cg_mech": gpu_ms_pass,
+                                         "gpu_ms_per_cg_iteration_all_solves": (prof["cg_mech"]["ms"] + prof["cg_ms"]["ms"] + prof["cg_gs"]["ms"])
+                                                                               / max(1, sum(a + b + c for a, b, c in line["config"]["cg_iters_per_step"]))})
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -370,6 +413,8 @@ def main():
     ap.add_argument("--oracle-maxiter", type=int, default=100000, help="--impl reference: cap of every CG solve")
     ap.add_argument("--grid", default="", help="override the node grid, e.g. 81x81x21 (not the headline workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fuse-s5s8", action="store_true", help="run S5 and S8 as separate element passes (CM_OPT_NO_FUSED_S5S8)")
+    ap.add_argument("--no-cpu-full-mesh", action="store_true", help="skip the like-for-like oracle leg on config 3 itself (about 80 s)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

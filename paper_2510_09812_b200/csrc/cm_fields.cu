@@ -1712,6 +1712,7 @@ int sys_cg_matfree(System<T> *S, const T *b, T *x, double tol, int maxiter, int 
         }
         CM_CUDA(cudaMemcpyAsync(hs, ms + (k & 1), sizeof(MfState), cudaMemcpyDeviceToHost, st));
         CM_CUDA(cudaStreamSynchronize(st));
+        if (S->prof.on) CM_TRY(S->prof.flush()); // the stream is idle here: fold this batch's event pairs in, so `pending` stays bounded by one batch
         if (hs->done) break;
     }
     const int kfin = k & 1;
