@@ -13,7 +13,7 @@
 // The three-right-hand-side product (MODE_CSR3) gathers its vector from a PADDED copy, four words per node: one
 // aligned 32-byte (fp64: ld.global.v4.f64, a 256-bit load) or 16-byte (fp32) request per nonzero touches exactly
 // one sector, where three scalar gathers from [node][3] cost three requests and ~2.4 sectors (the L1 bound
-// measured in round 1, profiles/r01_e_spmv_csr3_full.md).
+// measured in round 1, a round-1 ncu capture).
 //
 // CG.  ONE cooperative launch per solve; a CTA owns a contiguous range of slices, hence of rows, for the whole
 // solve.  Per iteration k (three grid-wide barriers, the dot products ride on two of them):
@@ -154,11 +154,17 @@ __device__ __forceinline__ void fetch(const T *x, int col, T (&out)[NC])
 
 // Batches in flight per warp.  The fp32 block matrix streams half the bytes per element, so it takes twice the batches
 // (measured on B200, config 3 fp32: mechanical CG 88 % -> 94 % of the measured HBM peak with 4 instead of 2).
+#ifndef CM_F32_CSR3_CTAS
+#define CM_F32_CSR3_CTAS 2 // resident CTAs per SM asked for the fp32 three-right-hand-side CG (3: 56 registers; measured)
+#endif
+#ifndef CM_U_CSR3_F32
+#define CM_U_CSR3_F32 CM_U_CSR3
+#endif
 #ifndef CM_U_BSR3_F32
 #define CM_U_BSR3_F32 4
 #endif
 template <typename T, int MODE>
-constexpr int batch_u() { return (MODE == MODE_BSR3 && sizeof(T) == 4) ? CM_U_BSR3_F32 : ModeTraits<MODE>::U; }
+constexpr int batch_u() { return (MODE == MODE_BSR3 && sizeof(T) == 4) ? CM_U_BSR3_F32 : ((MODE == MODE_CSR3 && sizeof(T) == 4) ? CM_U_CSR3_F32 : ModeTraits<MODE>::U); }
 
 // One batch = U consecutive 32-element groups of one slice: the unit of the load pipeline.  NV2 = 2: a second
 // scalar value array on the same pattern (the Helmholtz first pass streams K^GS and M_m together).
@@ -587,7 +593,7 @@ __device__ __forceinline__ void grid_sum(const double *partial, int slot, double
 
 // (three resident CTAs for the fp32 scalar solve, which fits 56 registers: 81 % -> 87 % of the measured HBM peak at 144^3)
 template <typename T, int MODE, bool PRE, bool HELM>
-__global__ void __launch_bounds__(CM_NT, (sizeof(T) == 4 && MODE == MODE_CSR1 && !PRE) ? 3 : 2) cg_kernel(CgArgs<T> a)
+__global__ void __launch_bounds__(CM_NT, (sizeof(T) == 4 && ((MODE == MODE_CSR1 && !PRE) || (MODE == MODE_CSR3 && !PRE && CM_F32_CSR3_CTAS == 3))) ? 3 : 2) cg_kernel(CgArgs<T> a)
 {
     constexpr int NC = ModeTraits<MODE>::NC, NR = ModeTraits<MODE>::NR, C = ModeTraits<MODE>::C;
     constexpr int PS = MODE == MODE_CSR3 ? 4 : NC; // words per node of the search directions in memory
