@@ -238,6 +238,21 @@ def test_config3_one_converged_step(full, oracle_mod):
           f"max |du| / max |u| = {rel(ug.cpu().numpy(), u):.2e}")
     assert dm <= 1e-7                                  # measured 6.1e-9 (profiles/r02_fullsize_converged.txt); two tol-1e-7 solves
     assert np.allclose(ig.mbar[:], io.mbar[:], atol=1e-12) and ig.mean_dm == pytest.approx(io.mean_dm, rel=1e-7)
+    # the fp32 build on the same step (BASELINE config 3 lists fp64 AND fp32), same tolerance as `bench.py --dtype f32` runs it with,
+    # against the fp64 oracle's step: north_star's 1e-4 (measured 6.95e-5), counts within 0.5 % of the fp64 oracle's (measured 1625 / 1969
+    # against 1623 / 1964, the eight Helmholtz counts identical)
+    gs32 = cm.System(gm, cfg.material, cfg.dt, "f32", cfg.clamp_dof, cfg.pin_node)
+    m32 = torch.as_tensor(cfg.m0, dtype=torch.float32, device="cuda").contiguous()
+    U32 = torch.zeros(N, dtype=torch.float32, device="cuda"); u32 = torch.zeros((N, 3), dtype=torch.float32, device="cuda")
+    i32, rc32 = gs32.gspm_step(cm.make_params(cfg.dt, cfg.Hext[0], cfg.terms, 0, 1e-7), m32, U32, u32)
+    dm32 = np.abs(m32.cpu().numpy().astype(np.float64) - m).max()
+    print(f"config 3, one converged step, fp32 device against the fp64 oracle: max |dm| = {dm32:.2e}, CG its ms/mech/gs "
+          f"{i32.it_ms}/{i32.it_mech}/{list(i32.it_gs)} (rc {rc32}), <|dm|> {i32.mean_dm:.6f} against {io.mean_dm:.6f}")
+    gs32.close()
+    assert rc32 == 0
+    assert abs(i32.it_ms - io.it_ms) <= 0.005 * io.it_ms and abs(i32.it_mech - io.it_mech) <= 0.005 * io.it_mech
+    assert all(abs(i32.it_gs[a] - io.it_gs[a]) <= 1 for a in range(8))
+    assert dm32 <= 1e-4
 
 
 SLOW = pytest.mark.skipif(os.environ.get("CM_SLOW_TESTS", "0") != "1",
