@@ -13,7 +13,8 @@
  *  - The library owns cm_mesh / cm_system and every internal device buffer; nothing is
  *    allocated inside cm_spmv / cm_cg_solve* / cm_field_rhs / cm_gspm_step.  Two calls may allocate:
  *    cm_hysteresis_run (a capture stream, the graph, logs grown to max_fields) and cm_volume_average
- *    (a library-order staging copy kept in the mesh, grown on demand).
+ *    (a library-order staging copy kept in the mesh, grown on demand).  cm_volume_average_noalloc is the variant of the latter that
+ *    allocates nothing (fixed scratch inside the library, see its declaration).
  *  - Calls on one cm_system share its scratch buffers: they must not run concurrently (one stream at a
  *    time per system).  cm_volume_average calls on one cm_mesh are serialised inside the library.
  *  - All field vectors are in USER node order, interleaved [node][component], of the
